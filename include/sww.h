@@ -1,0 +1,114 @@
+/*
+ * sww.h -- C ABI of the B200-native Dirichlet-to-Neumann (DtN) hot path of
+ * Wilkening & Yu, "Overdetermined shooting methods for computing standing water waves with spectral accuracy"
+ * (arXiv 1210.5672).  Citations are PAPER.md:<line> (+ section / equation); readings R1.. are listed in DESIGN.md section 3.
+ *
+ * Scope: the spectrally accurate boundary-integral DtN operator of Appendix A / section 2.1-2.2 on a uniform grid
+ * alpha_j = 2 pi j / N over a flat bottom, its linearization (Appendix B), and the explicit Runge-Kutta stepper of the
+ * free-surface Euler equations (2.1) with the batched variational equation (3.32).
+ *
+ * Conventions (all entry points)
+ *   - Every pointer named DEVICE is a CUDA device pointer valid on the current device; nothing is copied from the host
+ *     except by the *_host convenience calls at the bottom, which are explicitly marked HOST.
+ *   - A batch of nrhs columns of N reals is column-major N x nrhs: column c starts at element offset c*N.
+ *   - prec = SWW_F64: one double per element.
+ *     prec = SWW_DD : double-double ("quadruple"), PLANAR layout: an array of L logical elements is 2L doubles,
+ *                     hi[0..L) followed by lo[0..L), value = hi + lo with |lo| <= ulp(hi)/2.  (L = N*nrhs for a batch.)
+ *   - h, g, dt are plain doubles.  h = INFINITY selects infinite depth (image kernels dropped).
+ *   - eta is the elevation about the mean level; the bottom is y = 0 and the surface is y = h + eta_j (R2).
+ *   - Work is enqueued on the CUDA stream given at creation; calls return without synchronising unless stated.
+ *     Data-dependent failures (SWW_EBOTTOM, SWW_ESINGULAR) are recorded in a device flag and returned by the next
+ *     synchronising call (sww_dtn_status, sww_state_read).
+ *   - The caller owns every in/out buffer; handles own everything else.  Functions never throw or exit; they return a status.
+ *   - N must be a power of two, 16 <= N <= 8192.
+ */
+#ifndef SWW_H
+#define SWW_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sww_dtn_s*   sww_dtn_t;   /* one surface: K, G, LU(I/2+K), node tables, base state, workspace (device)  */
+typedef struct sww_state_s* sww_state_t; /* time-stepper state: eta, phi, optional variational columns, RK stage storage */
+
+enum { SWW_F64 = 0, SWW_DD = 1 };
+enum {
+    SWW_OK = 0,
+    SWW_EINVAL = -1,    /* bad argument (N not a power of two in range, nrhs < 0, null pointer, unknown prec)           */
+    SWW_ENOMEM = -2,    /* device or host allocation failed                                                           */
+    SWW_ECUDA = -3,     /* a CUDA runtime call failed; sww_last_cuda_error() has the text                             */
+    SWW_EBOTTOM = -4,   /* some h + eta_j <= 0: the surface touches the bottom                                         */
+    SWW_ESINGULAR = -5, /* a pivot of the unpivoted LU fell below the guard (|U_ii| < 1e-3): I/2+K is not benign here  */
+    SWW_ENOBASE = -6    /* sww_dtn_linearized_apply before sww_dtn_set_base                                            */
+};
+
+/* ---- DtN operator of one surface -------------------------------------------------------------------------------
+ * sww_dtn_setup: steps S0-S2 of DESIGN.md.
+ *   S0  eta', eta'' = D eta, D(D eta) by spectral differentiation carried in double-double (R8);
+ *   S1  K_ij, G_ij for all i, j from (2.13) with the image kernels SUBTRACTED (R1: (A.2),(A.3),(A.8),
+ *       PAPER.md:637-663), diagonal entries from the limits of PAPER.md:150, 653, 673;
+ *   S2  LU factorisation of A = I/2 + K (the matrix of (2.7); "LU-factorization"), unpivoted
+ *       (DESIGN.md section 5 justifies: sigma(A) in [0.46, 1.01]) with a |U_ii| guard -> SWW_ESINGULAR.
+ * eta: DEVICE, N reals (layout by prec), read during the call's enqueued work; may be reused after the stream reaches it.
+ * stream: a cudaStream_t cast to void* (NULL = legacy default stream).  *out receives the handle. */
+int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_dtn_t* out);
+
+/* Re-run S0-S2 for a new surface of the same N, h, prec in an existing handle (no allocation; what every RK stage does). */
+int sww_dtn_refactor(sww_dtn_t d, const void* eta);
+
+/* out_c = G(eta) phi_c, c < nrhs: solve (I/2 + K) mu_c = phi_c (2.7); gamma_c = D mu_c; out_c = H gamma_c / 2 + G gamma_c (2.8)
+ * (1/|xi'| = 1 on the uniform grid, R3).  phi, out: DEVICE, N x nrhs; may alias.  Pure: no hidden state. */
+int sww_dtn_apply(sww_dtn_t d, const void* phi, int nrhs, void* out);
+
+/* Store the state the linearization is taken about: phi0' = D phi0, W0 = G phi0, and the surface velocities of (2.9)
+ * (PAPER.md:116): u = (phi0' - eta' W0)/(1+eta'^2), v = (eta' phi0' + W0)/(1+eta'^2).  phi0: DEVICE, N reals. */
+int sww_dtn_set_base(sww_dtn_t d, const void* phi0);
+
+/* out_c = d/de G(eta + e deta_c)[phi0 + e dphi_c] at e = 0 = G[dphi_c - v deta_c] - D(u deta_c)   ((B.1d),(B.2)).
+ * deta, dphi, out: DEVICE, N x nrhs.  Needs sww_dtn_set_base first (else SWW_ENOBASE). */
+int sww_dtn_linearized_apply(sww_dtn_t d, const void* deta, const void* dphi, int nrhs, void* out);
+
+/* Read-only views for tests and diagnostics.  which: 0 = K, 1 = G (column-major N x N: entry (i,j) at i + j*N, i = target
+ * alpha_i, j = source alpha_j; DD: planar hi then lo), 2 = eta' , 3 = eta'', 4 = phi0', 5 = W0, 6 = u, 7 = v (N reals each).
+ * dst: DEVICE buffer of the right size; the copy is enqueued on the handle's stream. */
+int sww_dtn_get(sww_dtn_t d, int which, void* dst);
+
+int sww_dtn_status(sww_dtn_t d);   /* synchronises the stream; returns the sticky status */
+int sww_dtn_destroy(sww_dtn_t d);
+
+/* ---- time stepper (2.1) + variational equation (3.32), PAPER.md:70-72, 294-305, 689-714 ------------------------
+ * sww_state_create copies the initial state (DEVICE pointers; deta/dphi may be NULL when ncols = 0).
+ * flags bit 0: switch the 36th-order filter (2.14) off (R5).
+ * sww_rk_advance: nsteps steps of size dt of the 11-stage order-8 explicit Runge-Kutta scheme (R6), one setup S0-S2 and
+ * one batched linearized solve per stage, state filtered after each step; advances (q, Qdot) together, in place.
+ * sww_state_read: DEVICE destinations (any may be NULL); synchronises; *t (HOST) receives the elapsed time; returns the
+ * sticky status. */
+int sww_state_create(int N, double h, double g, int prec, int ncols, const void* eta, const void* phi,
+                     const void* deta, const void* dphi, unsigned flags, void* stream, sww_state_t* out);
+int sww_rk_advance(sww_state_t s, double dt, int nsteps);
+int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, double* t);
+/* E = (1/2) int (phi G phi + g eta^2) dx = (pi/N) sum_j [phi_j (G phi)_j + g eta_j^2] of the current state;
+ * energy_hl: HOST, 2 doubles (hi, lo; lo = 0 for SWW_F64); synchronises. */
+int sww_state_energy(sww_state_t s, double* energy_hl);
+int sww_state_destroy(sww_state_t s);
+
+/* ---- diagnostics ---------------------------------------------------------------------------------------------- */
+const char* sww_strerror(int status);
+const char* sww_last_cuda_error(void);
+/* Number of kernels this library has launched since it was loaded (bench.py reports the count per step). */
+unsigned long long sww_launch_count(void);
+/* Microbenchmarks used to measure the roofline denominators on the box: returns achieved FLOP/s of a
+ * register-resident DFMA loop (which = 0) or DMMA.8x8x4 loop (which = 1) over the whole chip, timed with CUDA events. */
+int sww_probe_fp64_peak(int which, double* flops_per_s);
+
+/* ---- HOST-buffer convenience path (what bench.py's "e2e" leg times) -------------------------------------------
+ * Same computation as setup + set_base + linearized_apply, but every array is a HOST pointer (pinned or pageable);
+ * the call copies inputs to the device, runs the device path, copies the result back and synchronises. */
+int sww_dtn_linearized_host(const void* eta, const void* phi0, const void* deta, const void* dphi, void* out,
+                            int N, double h, int prec, int nrhs);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SWW_H */

@@ -1,0 +1,247 @@
+"""ctypes binding of include/sww.h.  Argument marshalling only (see the package docstring)."""
+from __future__ import annotations
+
+import ctypes
+import math
+from pathlib import Path
+
+import torch
+
+F64, DD = 0, 1
+_HERE = Path(__file__).resolve().parent
+_LIB = None
+
+# every symbol include/sww.h declares (tests check the library exports each of them)
+EXPORTS = [
+    "sww_dtn_setup", "sww_dtn_refactor", "sww_dtn_apply", "sww_dtn_set_base", "sww_dtn_linearized_apply", "sww_dtn_get",
+    "sww_dtn_status", "sww_dtn_destroy", "sww_state_create", "sww_rk_advance", "sww_state_read", "sww_state_energy",
+    "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
+    "sww_dtn_linearized_host",
+]
+
+
+class SwwError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        msg = lib().sww_strerror(status).decode()
+        if status == -3:
+            msg += ": " + lib().sww_last_cuda_error().decode()
+        super().__init__(f"{what}: {msg} (status {status})")
+
+
+def lib_path() -> Path:
+    return _HERE / "libsww.so"
+
+
+def lib() -> ctypes.CDLL:
+    """Load libsww.so (built in-tree by paper_1210_5672_b200.build).  Fails loudly when it is missing."""
+    global _LIB
+    if _LIB is None:
+        p = lib_path()
+        if not p.exists():
+            raise ImportError(f"{p} is missing: run `python -m paper_1210_5672_b200.build` (there is no fallback path)")
+        L = ctypes.CDLL(str(p))
+        vp, ci, cd = ctypes.c_void_p, ctypes.c_int, ctypes.c_double
+        L.sww_dtn_setup.argtypes = [vp, ci, cd, ci, vp, ctypes.POINTER(vp)]
+        L.sww_dtn_refactor.argtypes = [vp, vp]
+        L.sww_dtn_apply.argtypes = [vp, vp, ci, vp]
+        L.sww_dtn_set_base.argtypes = [vp, vp]
+        L.sww_dtn_linearized_apply.argtypes = [vp, vp, vp, ci, vp]
+        L.sww_dtn_get.argtypes = [vp, ci, vp]
+        L.sww_dtn_status.argtypes = [vp]
+        L.sww_dtn_destroy.argtypes = [vp]
+        L.sww_state_create.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, ctypes.c_uint, vp, ctypes.POINTER(vp)]
+        L.sww_rk_advance.argtypes = [vp, cd, ci]
+        L.sww_state_read.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(cd)]
+        L.sww_state_energy.argtypes = [vp, ctypes.POINTER(cd)]
+        L.sww_state_destroy.argtypes = [vp]
+        L.sww_strerror.argtypes = [ci]
+        L.sww_strerror.restype = ctypes.c_char_p
+        L.sww_last_cuda_error.restype = ctypes.c_char_p
+        L.sww_launch_count.restype = ctypes.c_ulonglong
+        L.sww_probe_fp64_peak.argtypes = [ci, ctypes.POINTER(cd)]
+        L.sww_dtn_linearized_host.argtypes = [vp, vp, vp, vp, vp, ci, cd, ci, ci]
+        _LIB = L
+    return _LIB
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise SwwError(rc, what)
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_1210_5672_b200 needs a CUDA device: there is no CPU path")
+
+
+def _dev(t: torch.Tensor, n: int, what: str) -> int:
+    if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n):
+        raise ValueError(f"{what}: expected a contiguous CUDA float64 tensor of {n} elements, got {tuple(t.shape)} {t.dtype} {t.device}")
+    return t.data_ptr()
+
+
+def dd_pack(hi, lo, device="cuda") -> torch.Tensor:
+    """(hi, lo) arrays of equal shape -> planar dd tensor of shape (2, *shape) on the device"""
+    hi = torch.as_tensor(hi, dtype=torch.float64)
+    lo = torch.zeros_like(hi) if lo is None else torch.as_tensor(lo, dtype=torch.float64)
+    return torch.stack([hi, lo]).contiguous().to(device)
+
+
+def dd_unpack(t: torch.Tensor):
+    c = t.detach().cpu().numpy()
+    return c[0], c[1]
+
+
+def launch_count() -> int:
+    return int(lib().sww_launch_count())
+
+
+def probe_fp64_peak(which: int) -> float:
+    """which: 0 = DFMA loop, 1 = DMMA.8x8x4 loop.  Returns FLOP/s."""
+    _require_cuda()
+    out = ctypes.c_double(0.0)
+    _check(lib().sww_probe_fp64_peak(which, ctypes.byref(out)), "sww_probe_fp64_peak")
+    return out.value
+
+
+class DtN:
+    """One surface: sww_dtn_setup / apply / set_base / linearized_apply.  Tensors are CUDA float64; batches are (nrhs, N)
+    C-contiguous (= column-major N x nrhs); dd quantities are planar (2, ...) tensors (hi plane, lo plane)."""
+
+    def __init__(self, eta: torch.Tensor, h: float, prec: int = F64, stream: torch.cuda.Stream | None = None):
+        _require_cuda()
+        self.prec = prec
+        self.mul = 2 if prec == DD else 1
+        self.N = eta.numel() // self.mul
+        self.h = float(h)
+        self._stream = stream if stream is not None else torch.cuda.current_stream()
+        h_ = ctypes.c_void_p()
+        _check(lib().sww_dtn_setup(_dev(eta, self.N * self.mul, "eta"), self.N, self.h, prec, self._stream.cuda_stream, ctypes.byref(h_)),
+               "sww_dtn_setup")
+        self._h = h_
+
+    def _shape(self, nrhs):
+        return (2, nrhs, self.N) if self.prec == DD else (nrhs, self.N)
+
+    def refactor(self, eta: torch.Tensor):
+        _check(lib().sww_dtn_refactor(self._h, _dev(eta, self.N * self.mul, "eta")), "sww_dtn_refactor")
+
+    def apply(self, phi: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        nrhs = phi.numel() // (self.N * self.mul)
+        if out is None:
+            out = torch.empty_like(phi)
+        _check(lib().sww_dtn_apply(self._h, _dev(phi, nrhs * self.N * self.mul, "phi"), nrhs, _dev(out, phi.numel(), "out")), "sww_dtn_apply")
+        return out
+
+    def set_base(self, phi0: torch.Tensor):
+        _check(lib().sww_dtn_set_base(self._h, _dev(phi0, self.N * self.mul, "phi0")), "sww_dtn_set_base")
+
+    def linearized_apply(self, deta: torch.Tensor, dphi: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
+        nrhs = dphi.numel() // (self.N * self.mul)
+        if out is None:
+            out = torch.empty_like(dphi)
+        n = nrhs * self.N * self.mul
+        _check(lib().sww_dtn_linearized_apply(self._h, _dev(deta, n, "deta"), _dev(dphi, n, "dphi"), nrhs, _dev(out, n, "out")),
+               "sww_dtn_linearized_apply")
+        return out
+
+    _WHICH = {"K": 0, "G": 1, "d1": 2, "d2": 3, "dphi0": 4, "W0": 5, "u": 6, "v": 7, "LU": 8}
+
+    def get(self, name: str) -> torch.Tensor:
+        """K, G, LU: (N, N) tensors indexed [j, i] (column-major storage: entry (i, j) of the matrix is t[j, i])."""
+        which = self._WHICH[name]
+        N = self.N
+        if name in ("K", "G"):
+            shape = (2, N, N) if self.prec == DD else (N, N)
+        elif name == "LU":
+            shape = (N, N)
+        else:
+            shape = (2, N) if self.prec == DD else (N,)
+        t = torch.empty(shape, dtype=torch.float64, device="cuda")
+        _check(lib().sww_dtn_get(self._h, which, t.data_ptr()), "sww_dtn_get")
+        return t
+
+    def status(self) -> int:
+        return int(lib().sww_dtn_status(self._h))
+
+    def check(self):
+        _check(self.status(), "sww_dtn_status")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().sww_dtn_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class State:
+    """Time-stepper state: sww_state_create / sww_rk_advance / sww_state_read / sww_state_energy."""
+
+    def __init__(self, eta, phi, h: float, g: float = 1.0, prec: int = F64, deta=None, dphi=None, filter: bool = True,
+                 stream: torch.cuda.Stream | None = None):
+        _require_cuda()
+        self.prec = prec
+        self.mul = 2 if prec == DD else 1
+        self.N = eta.numel() // self.mul
+        self.ncols = 0 if deta is None else deta.numel() // (self.N * self.mul)
+        self._stream = stream if stream is not None else torch.cuda.current_stream()
+        h_ = ctypes.c_void_p()
+        n1, nc = self.N * self.mul, self.N * self.mul * self.ncols
+        _check(lib().sww_state_create(self.N, float(h), float(g), prec, self.ncols, _dev(eta, n1, "eta"), _dev(phi, n1, "phi"),
+                                      None if deta is None else _dev(deta, nc, "deta"), None if dphi is None else _dev(dphi, nc, "dphi"),
+                                      0 if filter else 1, self._stream.cuda_stream, ctypes.byref(h_)), "sww_state_create")
+        self._h = h_
+
+    def advance(self, dt: float, nsteps: int):
+        _check(lib().sww_rk_advance(self._h, float(dt), int(nsteps)), "sww_rk_advance")
+
+    def read(self):
+        N, nc = self.N, self.ncols
+        sh1 = (2, N) if self.prec == DD else (N,)
+        shc = (2, nc, N) if self.prec == DD else (nc, N)
+        eta = torch.empty(sh1, dtype=torch.float64, device="cuda")
+        phi = torch.empty_like(eta)
+        deta = torch.empty(shc, dtype=torch.float64, device="cuda") if nc else None
+        dphi = torch.empty_like(deta) if nc else None
+        t = ctypes.c_double(0.0)
+        _check(lib().sww_state_read(self._h, eta.data_ptr(), phi.data_ptr(), deta.data_ptr() if nc else None,
+                                    dphi.data_ptr() if nc else None, ctypes.byref(t)), "sww_state_read")
+        return {"eta": eta, "phi": phi, "deta": deta, "dphi": dphi, "t": t.value}
+
+    def energy(self):
+        e = (ctypes.c_double * 2)()
+        _check(lib().sww_state_energy(self._h, e), "sww_state_energy")
+        return e[0], e[1]
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().sww_state_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def dtn_linearized_host(eta, phi0, deta, dphi, h: float, prec: int = F64):
+    """HOST-buffer path (sww_dtn_linearized_host): CPU float64 tensors in, CPU tensor out; copies are inside the call."""
+    _require_cuda()
+    mul = 2 if prec == DD else 1
+    N = eta.numel() // mul
+    nrhs = dphi.numel() // (N * mul)
+    for t in (eta, phi0, deta, dphi):
+        assert (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous()
+    out = torch.empty_like(dphi)
+    if dphi.is_pinned():
+        out = out.pin_memory()
+    _check(lib().sww_dtn_linearized_host(eta.data_ptr(), phi0.data_ptr(), deta.data_ptr(), dphi.data_ptr(), out.data_ptr(), N, float(h), prec, nrhs),
+           "sww_dtn_linearized_host")
+    return out

@@ -1,0 +1,246 @@
+// api.cu -- the C ABI of include/sww.h: handle management, right-hand-side formation (S3), the DtN apply (S4-S6), the base
+// state (2.9) and the linearized DtN (B.1d),(B.2).  Product code; shares nothing with oracle/.
+#include "common.cuh"
+#include "dd.cuh"
+#include <new>
+#include <cstring>
+
+using namespace sww;
+
+namespace sww {
+
+static bool valid_N(int N) { return N >= 16 && N <= 8192 && (N & (N - 1)) == 0; }
+static int pad64(int n) { return (n + 63) / 64 * 64; }
+
+int ensure_workspace(sww_dtn_s* d, int nrhs) {
+    int need = pad64(nrhs < 1 ? 1 : nrhs);
+    Workspace& w = d->ws;
+    if (need <= w.cap_cols) return SWW_OK;
+    SWW_CUDA(cudaStreamSynchronize(d->stream));
+    cudaFree(w.B); cudaFree(w.Gam); cudaFree(w.W); cudaFree(w.T); cudaFree(w.R);
+    w = Workspace();
+    size_t per = (size_t)d->N * need * sizeof(double) * (d->prec == SWW_DD ? 2 : 1);
+    if (cudaMalloc(&w.B, per) != cudaSuccess || cudaMalloc(&w.Gam, per) != cudaSuccess || cudaMalloc(&w.W, per) != cudaSuccess ||
+        cudaMalloc(&w.T, per) != cudaSuccess)
+        return SWW_ENOMEM;
+    if (d->prec == SWW_DD && cudaMalloc(&w.R, (size_t)d->N * need * sizeof(double)) != cudaSuccess) return SWW_ENOMEM;
+    SWW_CUDA(cudaMemsetAsync(w.B, 0, per, d->stream));
+    SWW_CUDA(cudaMemsetAsync(w.Gam, 0, per, d->stream));
+    SWW_CUDA(cudaMemsetAsync(w.W, 0, per, d->stream));
+    SWW_CUDA(cudaMemsetAsync(w.T, 0, per, d->stream));
+    w.cap_cols = need;
+    return SWW_OK;
+}
+
+// ---- S3: right-hand sides --------------------------------------------------------------------------------------------
+// plain apply: B = phi
+// linearized : B_c = dphi_c - v deta_c  (B.1d);  T_c = u deta_c  (for the shape term of (B.2))
+__global__ void k_rhs_lin_f64(int N, size_t total, const double* __restrict__ deta, const double* __restrict__ dphi,
+                              const double* __restrict__ u, const double* __restrict__ v, double* __restrict__ B, double* __restrict__ T) {
+    size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= total) return;
+    int j = (int)(e & (size_t)(N - 1));
+    double de = deta[e];
+    B[e] = fma(-v[j], de, dphi[e]);
+    T[e] = u[j] * de;
+}
+
+// (2.9):  u = (phi' - eta' W0)/(1 + eta'^2),  v = (eta' phi' + W0)/(1 + eta'^2)
+__global__ void k_base_uv_f64(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* __restrict__ W0,
+                              double* __restrict__ u, double* __restrict__ v) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    double e1 = d1[j], den = fma(e1, e1, 1.0);
+    u[j] = (dphi[j] - e1 * W0[j]) / den;
+    v[j] = fma(e1, dphi[j], W0[j]) / den;
+}
+
+static int apply_f64(sww_dtn_s* d, const double* rhs_dev /* N x nrhs, or NULL when ws.B is already filled */, const double* Tcols,
+                     int nrhs, double* out) {
+    const int N = d->N;
+    Workspace& w = d->ws;
+    if (rhs_dev) SWW_CUDA(cudaMemcpyAsync(w.B, rhs_dev, sizeof(double) * (size_t)N * nrhs, cudaMemcpyDeviceToDevice, d->stream));
+    SWW_TRY(run_solve(d, w.B, nrhs));                                           // S4: mu = A^{-1} b
+    SWW_TRY(spectral_gamma_w(d, w.B, Tcols, w.Gam, out, nrhs, nrhs));           // S5: gamma = D mu ; out = |D| mu / 2 - D t
+    SWW_TRY(gemm_f64(d->stream, N, nrhs, N, 1.0, d->G, N, w.Gam, N, 1.0, out, N, nrhs));  // S6: out += G gamma   (2.8)
+    return SWW_OK;
+}
+
+int dd_apply(sww_dtn_s* d, const double* rhs_dev, bool rhs_in_ws, const double* Tcols, int nrhs, double* out);
+int dd_set_base(sww_dtn_s* d, const double* phi0);
+int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out);
+
+static int do_setup(sww_dtn_s* d, const void* eta) {
+    const int N = d->N;
+    d->has_base = false;
+    if (d->prec == SWW_F64) {
+        SWW_CUDA(cudaMemcpyAsync(d->eta, eta, sizeof(double) * N, cudaMemcpyDeviceToDevice, d->stream));
+        SWW_CUDA(cudaMemsetAsync(d->eta + N, 0, sizeof(double) * N, d->stream));
+        SWW_TRY(run_setup_f64(d));
+    } else {
+        SWW_CUDA(cudaMemcpyAsync(d->eta, eta, sizeof(double) * 2 * N, cudaMemcpyDeviceToDevice, d->stream));
+        SWW_TRY(run_setup_dd(d));
+    }
+    return run_lu(d);
+}
+
+}  // namespace sww
+
+extern "C" {
+
+int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_dtn_t* out) {
+    if (!eta || !out || !valid_N(N) || (prec != SWW_F64 && prec != SWW_DD) || !(h > 0.0)) return SWW_EINVAL;
+    sww_dtn_s* d = new (std::nothrow) sww_dtn_s();
+    if (!d) return SWW_ENOMEM;
+    memset(d, 0, sizeof(*d));
+    new (&d->ws) Workspace();
+    d->N = N;
+    d->prec = prec;
+    d->h = h;
+    d->finite = !std::isinf(h);
+    d->stream = (cudaStream_t)stream;
+    int rc = get_tables(N, d->stream, &d->tab);
+    if (rc) { delete d; return rc; }
+    const size_t n2 = (size_t)N * N, mat = n2 * (prec == SWW_DD ? 2 : 1);
+    const int nb = N < NB ? N : NB;
+    bool ok = true;
+    auto alloc = [&](double** p, size_t n) { if (ok && cudaMalloc(p, n * sizeof(double)) != cudaSuccess) ok = false; };
+    alloc(&d->eta, 2 * N); alloc(&d->d1, 2 * N); alloc(&d->d2, 2 * N);
+    alloc(&d->E, 2 * N); alloc(&d->Dm, 2 * N); alloc(&d->Sh, 2 * N); alloc(&d->Ch, 2 * N);
+    alloc(&d->K, mat); alloc(&d->G, mat); alloc(&d->LU, n2); alloc(&d->invD, 2 * (size_t)N * nb);
+    alloc(&d->bphi, 2 * N); alloc(&d->bW0, 2 * N); alloc(&d->bu, 2 * N); alloc(&d->bv, 2 * N);
+    if (ok && cudaMalloc(&d->status, sizeof(int)) != cudaSuccess) ok = false;
+    if (!ok) { sww_dtn_destroy(d); return SWW_ENOMEM; }
+    if (cudaMemsetAsync(d->status, 0, sizeof(int), d->stream) != cudaSuccess) { sww_dtn_destroy(d); return SWW_ECUDA; }
+    rc = ensure_workspace(d, 64);
+    if (!rc) rc = do_setup(d, eta);
+    if (rc) { sww_dtn_destroy(d); return rc; }
+    *out = d;
+    return SWW_OK;
+}
+
+int sww_dtn_refactor(sww_dtn_t d, const void* eta) {
+    if (!d || !eta) return SWW_EINVAL;
+    return do_setup(d, eta);
+}
+
+int sww_dtn_apply(sww_dtn_t d, const void* phi, int nrhs, void* out) {
+    if (!d || !phi || !out || nrhs < 0) return SWW_EINVAL;
+    if (nrhs == 0) return SWW_OK;
+    SWW_TRY(ensure_workspace(d, nrhs));
+    if (d->prec == SWW_F64) return apply_f64(d, (const double*)phi, nullptr, nrhs, (double*)out);
+    return dd_apply(d, (const double*)phi, false, nullptr, nrhs, (double*)out);
+}
+
+int sww_dtn_set_base(sww_dtn_t d, const void* phi0) {
+    if (!d || !phi0) return SWW_EINVAL;
+    SWW_TRY(ensure_workspace(d, 1));
+    const int N = d->N;
+    if (d->prec == SWW_F64) {
+        SWW_TRY(spectral_deriv(d, (const double*)phi0, d->bphi, 1));
+        SWW_TRY(apply_f64(d, (const double*)phi0, nullptr, 1, d->bW0));
+        k_base_uv_f64<<<(N + 127) / 128, 128, 0, d->stream>>>(N, d->d1, d->bphi, d->bW0, d->bu, d->bv);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+    } else {
+        SWW_TRY(dd_set_base(d, (const double*)phi0));
+    }
+    d->has_base = true;
+    return SWW_OK;
+}
+
+int sww_dtn_linearized_apply(sww_dtn_t d, const void* deta, const void* dphi, int nrhs, void* out) {
+    if (!d || !deta || !dphi || !out || nrhs < 0) return SWW_EINVAL;
+    if (!d->has_base) return SWW_ENOBASE;
+    if (nrhs == 0) return SWW_OK;
+    SWW_TRY(ensure_workspace(d, nrhs));
+    if (d->prec == SWW_DD) return dd_linearized(d, (const double*)deta, (const double*)dphi, nrhs, (double*)out);
+    const int N = d->N;
+    size_t total = (size_t)N * nrhs;
+    k_rhs_lin_f64<<<(unsigned)((total + 255) / 256), 256, 0, d->stream>>>(N, total, (const double*)deta, (const double*)dphi, d->bu, d->bv,
+                                                                         d->ws.B, d->ws.T);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return apply_f64(d, nullptr, d->ws.T, nrhs, (double*)out);
+}
+
+int sww_dtn_get(sww_dtn_t d, int which, void* dst) {
+    if (!d || !dst) return SWW_EINVAL;
+    const int N = d->N;
+    const size_t mul = d->prec == SWW_DD ? 2 : 1;
+    const double* src = nullptr;
+    size_t n = 0;
+    switch (which) {
+        case 0: src = d->K; n = (size_t)N * N * mul; break;
+        case 1: src = d->G; n = (size_t)N * N * mul; break;
+        case 2: src = d->d1; n = N * mul; break;
+        case 3: src = d->d2; n = N * mul; break;
+        case 4: src = d->bphi; n = N * mul; break;
+        case 5: src = d->bW0; n = N * mul; break;
+        case 6: src = d->bu; n = N * mul; break;
+        case 7: src = d->bv; n = N * mul; break;
+        case 8: src = d->LU; n = (size_t)N * N; break;
+        default: return SWW_EINVAL;
+    }
+    SWW_CUDA(cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDeviceToDevice, d->stream));
+    return SWW_OK;
+}
+
+int sww_dtn_status(sww_dtn_t d) {
+    if (!d) return SWW_EINVAL;
+    int st = 0;
+    SWW_CUDA(cudaMemcpyAsync(&st, d->status, sizeof(int), cudaMemcpyDeviceToHost, d->stream));
+    SWW_CUDA(cudaStreamSynchronize(d->stream));
+    return st;
+}
+
+int sww_dtn_destroy(sww_dtn_t d) {
+    if (!d) return SWW_EINVAL;
+    cudaStreamSynchronize(d->stream);
+    double* ptrs[] = {d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, d->K, d->G, d->LU, d->invD, d->bphi, d->bW0, d->bu, d->bv,
+                      d->ws.B, d->ws.Gam, d->ws.W, d->ws.T, d->ws.R};
+    for (double* p : ptrs) cudaFree(p);
+    cudaFree(d->status);
+    delete d;
+    return SWW_OK;
+}
+
+const char* sww_strerror(int status) {
+    switch (status) {
+        case SWW_OK: return "ok";
+        case SWW_EINVAL: return "invalid argument";
+        case SWW_ENOMEM: return "out of memory";
+        case SWW_ECUDA: return "CUDA runtime error";
+        case SWW_EBOTTOM: return "surface touches the bottom (h + eta <= 0)";
+        case SWW_ESINGULAR: return "pivot below guard in the unpivoted LU of I/2 + K";
+        case SWW_ENOBASE: return "linearized apply before set_base";
+        default: return "unknown status";
+    }
+}
+const char* sww_last_cuda_error(void) { return g_cuda_err; }
+unsigned long long sww_launch_count(void) { return g_launches; }
+
+int sww_dtn_linearized_host(const void* eta, const void* phi0, const void* deta, const void* dphi, void* out, int N, double h,
+                            int prec, int nrhs) {
+    if (!eta || !phi0 || !deta || !dphi || !out || nrhs < 1 || !valid_N(N)) return SWW_EINVAL;
+    const size_t mul = prec == SWW_DD ? 2 : 1, vec = sizeof(double) * N * mul, bat = vec * nrhs;
+    double *de = nullptr, *dp = nullptr, *dde = nullptr, *ddp = nullptr, *dout = nullptr;
+    cudaStream_t st = nullptr;
+    int rc = SWW_OK;
+    sww_dtn_t h_ = nullptr;
+    if (cudaMalloc(&de, vec) || cudaMalloc(&dp, vec) || cudaMalloc(&dde, bat) || cudaMalloc(&ddp, bat) || cudaMalloc(&dout, bat))
+        rc = SWW_ENOMEM;
+    if (!rc && (cudaMemcpyAsync(de, eta, vec, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(dp, phi0, vec, cudaMemcpyHostToDevice, st) ||
+                cudaMemcpyAsync(dde, deta, bat, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(ddp, dphi, bat, cudaMemcpyHostToDevice, st)))
+        rc = SWW_ECUDA;
+    if (!rc) rc = sww_dtn_setup(de, N, h, prec, st, &h_);
+    if (!rc) rc = sww_dtn_set_base(h_, dp);
+    if (!rc) rc = sww_dtn_linearized_apply(h_, dde, ddp, nrhs, dout);
+    if (!rc && cudaMemcpyAsync(out, dout, bat, cudaMemcpyDeviceToHost, st)) rc = SWW_ECUDA;
+    if (!rc) rc = sww_dtn_status(h_);
+    if (h_) sww_dtn_destroy(h_);
+    cudaFree(de); cudaFree(dp); cudaFree(dde); cudaFree(ddp); cudaFree(dout);
+    return rc;
+}
+
+}  // extern "C"

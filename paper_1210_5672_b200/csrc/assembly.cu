@@ -1,0 +1,289 @@
+// assembly.cu -- steps S0 (node preparation) and S1 (kernel-matrix assembly) of the DtN setup.
+//   S0: eta' = D eta, eta'' = D(D eta) by the Fourier differentiation circulant carried in double-double (R4, R8),
+//       per-node tables exp(-(h+eta_j)) (image term) and, for the dd path, sinh/cosh(eta_j).
+//   S1: K_ij, G_ij of (2.13) with the image kernels subtracted (R1; (A.2),(A.3),(A.8));
+//       diagonal from the limits of PAPER.md:150, 653, 673.  Also writes A = I/2 + K (2.7) into the LU buffer.
+// Layout: K, G, LU column-major (entry (i,j) at i + j*N): a warp writes 32 consecutive i for one j (coalesced 256 B).
+// Product code; shares nothing with oracle/.
+#include "common.cuh"
+#include "dd.cuh"
+
+namespace sww {
+
+// ------------------------------------------------------------------------------------------------ S0: D in double-double
+// out_i = sum_{m=1}^{N/2-1} dc[m] (f_{i-m} - f_{i+m}),  dc[m] = (1/2)(-1)^m cot(pi m/N)  (dc[N-m] = -dc[m]; Nyquist symbol 0).
+// One warp per output node; N dd multiply-adds per node.  in/out: dd planar 2N.
+__global__ void __launch_bounds__(256) k_deriv_dd(int N, const double* __restrict__ dc, const double* __restrict__ f, double* __restrict__ out) {
+    int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= N) return;
+    int i = warp, mask = N - 1;
+    dd acc{0.0, 0.0};
+    for (int m = 1 + lane; m < N / 2; m += 32) {
+        dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
+        dd c = dd_load(dc, N, m);
+        acc = dd_fma(c, dd_sub(a, b), acc);
+    }
+    acc = dd_warp_sum(acc);
+    if (lane == 0) dd_store(out, N, i, acc);
+}
+
+// per-node tables.  f64 path: E = exp(-(h+eta)), Dm = 1 - E (via expm1), in fp64.  dd path: the same in dd plus sinh/cosh(eta).
+__global__ void k_node_tables(int N, double h, int finite, int prec, const double* __restrict__ eta, double* __restrict__ E,
+                              double* __restrict__ Dm, double* __restrict__ Sh, double* __restrict__ Ch, int* status) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    dd e = dd_load(eta, N, j);
+    if (finite) {
+        dd Y = dd_add_d(e, h);
+        if (!(Y.hi > 0.0)) atomicCAS(status, SWW_OK, SWW_EBOTTOM);
+        if (prec == SWW_F64) {
+            E[j] = exp(-Y.hi);
+            Dm[j] = -expm1(-Y.hi);
+            E[N + j] = 0.0;
+            Dm[N + j] = 0.0;
+        } else {
+            dd nY = dd_neg(Y);
+            dd_store(E, N, j, dd_exp(nY));
+            dd_store(Dm, N, j, dd_neg(dd_expm1(nY)));
+        }
+    }
+    if (prec == SWW_DD) {
+        dd sh, ch;
+        dd_sinhcosh(e, &sh, &ch);
+        dd_store(Sh, N, j, sh);
+        dd_store(Ch, N, j, ch);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ S1: fp64 assembly
+// sinh(y), cosh(y) evaluated DIRECTLY from y = eta_i - eta_j (never from per-node tables: next to the diagonal the addition
+// formulas lose N/(2 pi |i-j|) digits -- DESIGN.md section 5).  |y| <= 1: odd/even Taylor polynomials in y^2; else from exp.
+__device__ __forceinline__ void sinhcosh_f64(double y, double* sh, double* ch) {
+    double a = fabs(y);
+    if (a <= 1.0) {
+        double t = y * y;
+        // sinh(y)/y = sum t^n/(2n+1)!, n = 0..10 ; cosh(y) = sum t^n/(2n)!, n = 0..10
+        double ps = 1.9572941063391263e-20;  // 1/21!
+        ps = fma(ps, t, 8.2206352466243295e-18);  // 1/19!
+        ps = fma(ps, t, 2.8114572543455206e-15);  // 1/17!
+        ps = fma(ps, t, 7.6471637318198164e-13);  // 1/15!
+        ps = fma(ps, t, 1.6059043836821613e-10);  // 1/13!
+        ps = fma(ps, t, 2.5052108385441720e-08);  // 1/11!
+        ps = fma(ps, t, 2.7557319223985893e-06);  // 1/9!
+        ps = fma(ps, t, 1.9841269841269841e-04);  // 1/7!
+        ps = fma(ps, t, 8.3333333333333332e-03);  // 1/5!
+        ps = fma(ps, t, 1.6666666666666666e-01);  // 1/3!
+        *sh = fma(y * t, ps, y);
+        double pc = 4.1103176233121648e-19;  // 1/20!
+        pc = fma(pc, t, 1.5619206968586225e-16);  // 1/18!
+        pc = fma(pc, t, 4.7794773323873853e-14);  // 1/16!
+        pc = fma(pc, t, 1.1470745597729725e-11);  // 1/14!
+        pc = fma(pc, t, 2.0876756987868100e-09);  // 1/12!
+        pc = fma(pc, t, 2.7557319223985888e-07);  // 1/10!
+        pc = fma(pc, t, 2.4801587301587302e-05);  // 1/8!
+        pc = fma(pc, t, 1.3888888888888889e-03);  // 1/6!
+        pc = fma(pc, t, 4.1666666666666664e-02);  // 1/4!
+        pc = fma(pc, t, 0.5);
+        *ch = fma(t, pc, 1.0);
+    } else {
+        double e = exp(a), ei = 1.0 / e;
+        *ch = 0.5 * (e + ei);
+        *sh = copysign(0.5 * (e - ei), y);
+    }
+}
+
+constexpr int ASM_TI = 128;  // rows (targets i) per block = threads per block
+constexpr int ASM_TJ = 32;   // columns (sources j) per block
+
+template <bool FINITE>
+__global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __restrict__ eta, const double* __restrict__ d1,
+                                                         const double* __restrict__ d2, const double* __restrict__ E,
+                                                         const double* __restrict__ Dm, const double* __restrict__ cs,
+                                                         const double* __restrict__ sn, const double* __restrict__ c0,
+                                                         const double* __restrict__ s2, double* __restrict__ K,
+                                                         double* __restrict__ G, double* __restrict__ LU) {
+    __shared__ double s_eta[ASM_TJ], s_d1[ASM_TJ], s_E[ASM_TJ], s_Dm[ASM_TJ];
+    __shared__ double s_cs[ASM_TI + ASM_TJ], s_sn[ASM_TI + ASM_TJ], s_c0[ASM_TI + ASM_TJ], s_s2[ASM_TI + ASM_TJ];
+    const int tid = threadIdx.x, mask = N - 1;
+    const int i0 = blockIdx.x * ASM_TI, j0 = blockIdx.y * ASM_TJ;
+    if (tid < ASM_TJ) {
+        int j = (j0 + tid) & mask;
+        s_eta[tid] = eta[j];
+        s_d1[tid] = d1[j];
+        if (FINITE) {
+            s_E[tid] = E[j];
+            s_Dm[tid] = Dm[j];
+        }
+    }
+    // table slice: index s <-> m = (i0 - j0 - (TJ-1) + s) mod N, s = tid - jj + TJ - 1
+    for (int s = tid; s < ASM_TI + ASM_TJ - 1; s += ASM_TI) {
+        int m = (i0 - j0 - (ASM_TJ - 1) + s) & mask;
+        s_cs[s] = cs[m];
+        s_sn[s] = sn[m];
+        s_c0[s] = c0[m];
+        s_s2[s] = s2[m];
+    }
+    __syncthreads();
+    const int i = i0 + tid;
+    if (i >= N) return;
+    const double eta_i = eta[i], d1_i = d1[i], d2_i = d2[i];
+    const double E_i = FINITE ? E[i] : 0.0, Dm_i = FINITE ? Dm[i] : 0.0;
+    const double rN = 1.0 / (double)N;
+    const int jmax = min(ASM_TJ, N - j0);
+    for (int jj = 0; jj < jmax; jj++) {
+        const int j = j0 + jj, s = tid - jj + ASM_TJ - 1;
+        const double sx = s_sn[s], cx = s_cs[s], d1_j = s_d1[jj];
+        double k1, g1;
+        if (i != j) {
+            double y = eta_i - s_eta[jj];  // Im(zeta_i - zeta_j) from the raw inputs
+            double sh, ch;
+            sinhcosh_f64(y, &sh, &ch);
+            // (1/2) cot((x+iy)/2) = (1/2) p (sin x - i sinh y), two-branch p of PAPER.md:154
+            double p = (cx >= 0.0) ? (cx + ch) / fma(sx, sx, sh * sh) : 1.0 / (ch - cx);
+            double hp = 0.5 * p;
+            k1 = hp * fma(d1_j, sx, -sh);           // Im{ zeta'_j (1/2)cot }
+            g1 = fma(hp, fma(d1_i, sh, sx), -s_c0[s]);  // Re{ zeta'_i (1/2)cot } - (1/2)cot(x/2)
+        } else {
+            double den = 2.0 * fma(d1_i, d1_i, 1.0);
+            k1 = -d2_i / den;        // -Im{ zeta''/(2 zeta') }
+            g1 = d1_i * d2_i / den;  //  Re{ zeta''/(2 zeta') }
+        }
+        double k2 = 0.0, g2 = 0.0;
+        if (FINITE) {
+            // image point: (1/2)cot((x + i y2)/2), y2 = Y_i + Y_j > 0, written with Eij = exp(-y2) = E_i E_j:
+            //   c_r = Eij sin x / den, c_i = -(1 - Eij^2) / (2 den), den = (1 - Eij)^2 + 4 Eij sin^2(x/2)   (all terms positive)
+            double Eij = E_i * s_E[jj];
+            double omE = fma(E_i, s_Dm[jj], Dm_i);  // 1 - E_i E_j = Dm_i + E_i Dm_j
+            double den = fma(omE, omE, 4.0 * Eij * s_s2[s]);
+            double inv = 1.0 / den;
+            double cr = Eij * sx * inv;
+            double ci = -0.5 * omE * (1.0 + Eij) * inv;
+            k2 = fma(-d1_j, cr, ci);  // Im{ conj(zeta'_j) (1/2)cot }
+            g2 = fma(-d1_i, ci, cr);  // Re{ zeta'_i (1/2)cot }
+        }
+        double kv = (k1 - k2) * rN, gv = (g1 - g2) * rN;
+        size_t o = (size_t)i + (size_t)j * N;
+        K[o] = kv;
+        G[o] = gv;
+        LU[o] = (i == j) ? 0.5 + kv : kv;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ S1: double-double assembly
+// Same formulas in dd.  sinh/cosh(eta_i - eta_j): direct series within the circular band |i-j| <= DD_BAND of the diagonal,
+// addition formulas on the per-node sinh/cosh tables outside (dd has the margin: DESIGN.md section 5).
+constexpr int DD_BAND = 16;
+constexpr int ASMDD_TI = 128;
+constexpr int ASMDD_TJ = 16;
+
+template <bool FINITE>
+__global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* __restrict__ eta, const double* __restrict__ d1,
+                                                          const double* __restrict__ d2, const double* __restrict__ E,
+                                                          const double* __restrict__ Dm, const double* __restrict__ Sh,
+                                                          const double* __restrict__ Ch, const double* __restrict__ cs,
+                                                          const double* __restrict__ sn, const double* __restrict__ c0,
+                                                          const double* __restrict__ s2, double* __restrict__ K,
+                                                          double* __restrict__ G, double* __restrict__ LU) {
+    const int tid = threadIdx.x, mask = N - 1;
+    const int i0 = blockIdx.x * ASMDD_TI, j0 = blockIdx.y * ASMDD_TJ;
+    const int i = i0 + tid;
+    if (i >= N) return;
+    const size_t NN = (size_t)N * N;
+    const dd eta_i = dd_load(eta, N, i), d1_i = dd_load(d1, N, i), d2_i = dd_load(d2, N, i);
+    dd E_i{0, 0}, Dm_i{0, 0};
+    if (FINITE) {
+        E_i = dd_load(E, N, i);
+        Dm_i = dd_load(Dm, N, i);
+    }
+    const dd Sh_i = dd_load(Sh, N, i), Ch_i = dd_load(Ch, N, i);
+    const double rN = 1.0 / (double)N;  // exact power of two
+    const int jmax = min(ASMDD_TJ, N - j0);
+    for (int jj = 0; jj < jmax; jj++) {
+        const int j = j0 + jj, m = (i - j) & mask;
+        const dd sx = dd_load(sn, N, m), cx = dd_load(cs, N, m), d1_j = dd_load(d1, N, j);
+        dd k1, g1;
+        if (i != j) {
+            dd sh, ch;
+            int dist = min(m, N - m);
+            if (dist <= DD_BAND) {
+                dd_sinhcosh(dd_sub(eta_i, dd_load(eta, N, j)), &sh, &ch);
+            } else {
+                dd Sh_j = dd_load(Sh, N, j), Ch_j = dd_load(Ch, N, j);
+                sh = dd_sub(dd_mul(Sh_i, Ch_j), dd_mul(Ch_i, Sh_j));
+                ch = dd_sub(dd_mul(Ch_i, Ch_j), dd_mul(Sh_i, Sh_j));
+            }
+            dd p;
+            if (cx.hi >= 0.0)
+                p = dd_div(dd_add(cx, ch), dd_add(dd_sqr(sx), dd_sqr(sh)));
+            else
+                p = dd_div(dd{1.0, 0.0}, dd_sub(ch, cx));
+            dd hp = dd_half(p);
+            k1 = dd_mul(hp, dd_sub(dd_mul(d1_j, sx), sh));
+            g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(d1_i, sh), sx)), dd_load(c0, N, m));
+        } else {
+            dd den = dd_mul_d(dd_add_d(dd_sqr(d1_i), 1.0), 2.0);
+            k1 = dd_neg(dd_div(d2_i, den));
+            g1 = dd_div(dd_mul(d1_i, d2_i), den);
+        }
+        dd k2{0, 0}, g2{0, 0};
+        if (FINITE) {
+            dd E_j = dd_load(E, N, j), Dm_j = dd_load(Dm, N, j);
+            dd Eij = dd_mul(E_i, E_j);
+            dd omE = dd_add(dd_mul(E_i, Dm_j), Dm_i);
+            dd den = dd_add(dd_sqr(omE), dd_mul_d(dd_mul(Eij, dd_load(s2, N, m)), 4.0));
+            dd cr = dd_div(dd_mul(Eij, sx), den);
+            dd ci = dd_neg(dd_half(dd_div(dd_mul(omE, dd_add_d(Eij, 1.0)), den)));
+            k2 = dd_sub(ci, dd_mul(d1_j, cr));
+            g2 = dd_sub(cr, dd_mul(d1_i, ci));
+        }
+        dd kv = dd_mul_d(dd_sub(k1, k2), rN), gv = dd_mul_d(dd_sub(g1, g2), rN);
+        size_t o = (size_t)i + (size_t)j * N;
+        dd_store(K, NN, o, kv);
+        dd_store(G, NN, o, gv);
+        LU[o] = (i == j) ? dd_add_d(kv, 0.5).hi : kv.hi;
+    }
+}
+
+static int run_node_prep(sww_dtn_s* d) {
+    const int N = d->N;
+    cudaStream_t st = d->stream;
+    int blocks = (N * 32 + 255) / 256;
+    k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->eta, d->d1);
+    SWW_LAUNCHED();
+    k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->d1, d->d2);
+    SWW_LAUNCHED();
+    k_node_tables<<<(N + 127) / 128, 128, 0, st>>>(N, d->h, d->finite ? 1 : 0, d->prec, d->eta, d->E, d->Dm, d->Sh, d->Ch, d->status);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int run_setup_f64(sww_dtn_s* d) {
+    SWW_TRY(run_node_prep(d));
+    const int N = d->N;
+    const Tables* t = d->tab;
+    dim3 grid((N + ASM_TI - 1) / ASM_TI, (N + ASM_TJ - 1) / ASM_TJ);
+    if (d->finite)
+        k_assemble_f64<true><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
+    else
+        k_assemble_f64<false><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int run_setup_dd(sww_dtn_s* d) {
+    SWW_TRY(run_node_prep(d));
+    const int N = d->N;
+    const Tables* t = d->tab;
+    dim3 grid((N + ASMDD_TI - 1) / ASMDD_TI, (N + ASMDD_TJ - 1) / ASMDD_TJ);
+    if (d->finite)
+        k_assemble_dd<true><<<grid, ASMDD_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
+    else
+        k_assemble_dd<false><<<grid, ASMDD_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+}  // namespace sww

@@ -1,0 +1,97 @@
+// common.cuh -- shared declarations of the sww CUDA library (product code; shares nothing with oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <cmath>
+#include "../../include/sww.h"
+
+namespace sww {
+
+// ---------------------------------------------------------------- launch accounting / error capture
+extern unsigned long long g_launches;
+extern char g_cuda_err[256];
+int note_cuda(cudaError_t e, const char* where);
+#define SWW_CUDA(call)                                                        \
+    do {                                                                      \
+        cudaError_t e_ = (call);                                              \
+        if (e_ != cudaSuccess) return ::sww::note_cuda(e_, #call);            \
+    } while (0)
+#define SWW_TRY(call)                                                         \
+    do {                                                                      \
+        int rc_ = (call);                                                     \
+        if (rc_ != SWW_OK) return rc_;                                        \
+    } while (0)
+#define SWW_LAUNCHED() (++::sww::g_launches)
+
+// ---------------------------------------------------------------- per-N constant tables (device, cached per N per device)
+// "computed once and for all".  All double-double, planar (hi[N], lo[N]).
+struct Tables {
+    int N;
+    double* cs;    // cos(2 pi m / N), m = 0..N-1        (hi at [m], lo at [N+m])
+    double* sn;    // sin(2 pi m / N)
+    double* c0;    // (1/2) cot(pi m / N), m >= 1; c0[0] = 0
+    double* s2;    // sin^2(pi m / N)
+    double* dc;    // differentiation circulant: (1/2) (-1)^m cot(pi m / N), m >= 1; dc[0] = 0, dc[N/2] = 0
+    double2* tw;   // fp64 FFT twiddles exp(-2 pi i m / N) = (cs, -sn) rounded, m = 0..N-1
+};
+int get_tables(int N, cudaStream_t st, const Tables** out);
+
+// ---------------------------------------------------------------- the DtN handle
+struct Workspace {
+    int cap_cols = 0;          // padded column capacity
+    double* B = nullptr;       // right-hand sides / mu           (f64: N*cap ; dd: 2*N*cap planar)
+    double* Gam = nullptr;     // gamma = D mu
+    double* W = nullptr;       // result accumulator
+    double* T = nullptr;       // scratch columns (u*deta etc.)
+    double* R = nullptr;       // dd: fp64 residual / correction
+};
+
+}  // namespace sww
+
+struct sww_dtn_s {
+    int N, prec;
+    double h;
+    bool finite;
+    cudaStream_t stream;
+    const sww::Tables* tab;
+    // node vectors, each dd planar 2N (lo = 0-filled / unused in the f64 path)
+    double *eta, *d1, *d2;
+    // f64 node tables: E = exp(-(h+eta)), Dm = 1 - E;   dd node tables: sinh(eta), cosh(eta), E, Dm (planar 2N each)
+    double *E, *Dm, *Sh, *Ch;
+    double *K, *G;        // column-major N x N (dd: planar 2*N*N)
+    double *LU;           // fp64 LU factors of I/2 + K (unit lower L below the diagonal, U on and above), column-major
+    double *invD;         // inverses of the diagonal blocks of L and U: 2 * (N/NB) blocks of NB x NB
+    // base state (dd planar 2N each): phi0', W0, u, v
+    double *bphi, *bW0, *bu, *bv;
+    bool has_base;
+    int* status;          // device sticky status
+    sww::Workspace ws;
+};
+
+namespace sww {
+
+// block size of the LU / triangular-solve blocking (diag blocks are inverted explicitly)
+constexpr int NB = 64;
+
+int ensure_workspace(sww_dtn_s* d, int nrhs);
+
+// node prep + assembly (assembly.cu)
+int run_setup_f64(sww_dtn_s* d);
+int run_setup_dd(sww_dtn_s* d);
+// LU (lu.cu)
+int run_lu(sww_dtn_s* d);
+// multi-RHS triangular solves with the factors in d->LU; B is N x ncols_pad (ld = N), in place
+int run_solve(sww_dtn_s* d, double* B, int ncols_pad);
+// GEMM (gemm.cu): C[M x Nc] = alpha * A[M x K] * B[K x Nc] + beta * C, all column-major fp64; C may alias A or B only in the
+// panel patterns documented in gemm.cu.  n_valid: columns >= n_valid are not stored.
+int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* A, int lda, const double* B, int ldb,
+             double beta, double* C, int ldc, int n_valid);
+// spectral (fft.cu)
+enum SpecMode { SPEC_APPLY = 0, SPEC_LIN = 1 };
+// For each column c < ncols: Gam_c = D M_c ;  W_c = |D| M_c / 2  - (T ? D T_c : 0)
+int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols);
+// out_c = D in_c
+int spectral_deriv(sww_dtn_s* d, const double* in, double* out, int ncols);
+
+}  // namespace sww

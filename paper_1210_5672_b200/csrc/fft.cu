@@ -1,0 +1,187 @@
+// fft.cu -- S5/S7: hand-written shared-memory FFTs and the Fourier multipliers of the method (no cuFFT):
+//   D = d/dalpha (symbol i k), H = Hilbert transform (-i sgn k), |D| = H D (|k|), all with symbol 0 at the
+//   Nyquist mode k = N/2 (R4); "the FFT is used to compute mu', H gamma ...".
+// One CTA transforms one PAIR of real columns packed as z = a + i b: every multiplier here has m(-k) = conj m(k), so it maps
+// real columns to real columns and acts on a and b independently -- no untangling pass is needed.
+// Forward transform: radix-2 decimation in frequency (natural order in, bit-reversed out); the symbol is applied in bit-reversed
+// order; inverse transform: radix-2 decimation in time (bit-reversed in, natural out).  No permutation pass.
+// Twiddles exp(-2 pi i m/N) come from the dd-accurate table rounded to fp64 (tables.cu).
+// Product code; shares nothing with oracle/.
+#include "common.cuh"
+
+namespace sww {
+
+__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
+    return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ double2 cmulc(double2 a, double2 b) {  // a * conj(b)
+    return make_double2(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -a.x * b.y));
+}
+
+// in-place forward DIF FFT of z[0..N) in shared memory; output in bit-reversed order
+__device__ void fft_dif(double2* z, int N, const double2* __restrict__ tw) {
+    for (int half = N >> 1; half >= 1; half >>= 1) {
+        int tstride = N / (2 * half);
+        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
+            int blk = t / half, o = t - blk * half;
+            int i = blk * 2 * half + o;
+            double2 a = z[i], b = z[i + half];
+            double2 w = tw[o * tstride];
+            z[i] = make_double2(a.x + b.x, a.y + b.y);
+            z[i + half] = cmul(make_double2(a.x - b.x, a.y - b.y), w);
+        }
+        __syncthreads();
+    }
+}
+// in-place inverse DIT FFT (input bit-reversed, output natural), unscaled
+__device__ void ifft_dit(double2* z, int N, const double2* __restrict__ tw) {
+    for (int half = 1; half < N; half <<= 1) {
+        int tstride = N / (2 * half);
+        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
+            int blk = t / half, o = t - blk * half;
+            int i = blk * 2 * half + o;
+            double2 a = z[i];
+            double2 b = cmulc(z[i + half], tw[o * tstride]);
+            z[i] = make_double2(a.x + b.x, a.y + b.y);
+            z[i + half] = make_double2(a.x - b.x, a.y - b.y);
+        }
+        __syncthreads();
+    }
+}
+// signed wavenumber of bit-reversed position p (Nyquist -> 0: every multiplier here vanishes there, R4)
+__device__ __forceinline__ int wavenumber(int p, int N, int logN) {
+    int k = (int)(__brev((unsigned)p) >> (32 - logN));
+    if (2 * k == N) return 0;
+    return (2 * k < N) ? k : k - N;
+}
+
+constexpr int FFT_MAX_PER_THREAD = 8;  // ceil(N / blockDim.x) <= 8
+
+// Gam_c = D M_c ;  W_c = |D| M_c / 2 - (T ? D T_c : 0)     for the column pair (2*blockIdx.x, 2*blockIdx.x + 1)
+__global__ void __launch_bounds__(1024) k_spectral_gamma_w(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ M,
+                                   const double* __restrict__ T, double* __restrict__ Gam, double* __restrict__ W, int ncols,
+                                   int w_cols) {
+    extern __shared__ __align__(16) double2 z[];
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const int per = (N + blockDim.x - 1) / blockDim.x;
+    double2 zt[FFT_MAX_PER_THREAD];
+    if (T) {
+        for (int j = threadIdx.x; j < N; j += blockDim.x)
+            z[j] = make_double2(T[(size_t)c0 * N + j], has1 ? T[(size_t)c1 * N + j] : 0.0);
+        __syncthreads();
+        fft_dif(z, N, tw);
+#pragma unroll
+        for (int r = 0; r < FFT_MAX_PER_THREAD; r++)
+            if (r < per && threadIdx.x + r * blockDim.x < N) zt[r] = z[threadIdx.x + r * blockDim.x];
+        __syncthreads();
+    }
+    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(M[(size_t)c0 * N + j], has1 ? M[(size_t)c1 * N + j] : 0.0);
+    __syncthreads();
+    fft_dif(z, N, tw);
+    double2 zm[FFT_MAX_PER_THREAD];
+    const double rN = 1.0 / (double)N;
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++)
+        if (r < per && threadIdx.x + r * blockDim.x < N) {
+            int p = threadIdx.x + r * blockDim.x;
+            zm[r] = z[p];
+            double k = (double)wavenumber(p, N, logN) * rN;  // fold the 1/N of the inverse transform into the symbol
+            z[p] = make_double2(-k * zm[r].y, k * zm[r].x);  // i k zhat
+        }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        double2 v = z[j];
+        Gam[(size_t)c0 * N + j] = v.x;
+        Gam[(size_t)c1 * N + j] = has1 ? v.y : 0.0;  // Gam is a padded buffer: the odd partner column is zeroed
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++)
+        if (r < per && threadIdx.x + r * blockDim.x < N) {
+            int p = threadIdx.x + r * blockDim.x;
+            double k = (double)wavenumber(p, N, logN) * rN;
+            double ha = 0.5 * fabs(k);
+            double2 v = make_double2(ha * zm[r].x, ha * zm[r].y);
+            if (T) {
+                v.x += k * zt[r].y;  // - i k that
+                v.y -= k * zt[r].x;
+            }
+            z[p] = v;
+        }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        double2 v = z[j];
+        if (c0 < w_cols) W[(size_t)c0 * N + j] = v.x;
+        if (c1 < w_cols) W[(size_t)c1 * N + j] = v.y;
+    }
+}
+
+// out_c = D in_c
+__global__ void __launch_bounds__(1024) k_spectral_deriv(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ in,
+                                 double* __restrict__ out, int ncols) {
+    extern __shared__ __align__(16) double2 z[];
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(in[(size_t)c0 * N + j], has1 ? in[(size_t)c1 * N + j] : 0.0);
+    __syncthreads();
+    fft_dif(z, N, tw);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        double2 v = z[p];
+        double k = (double)wavenumber(p, N, logN) * rN;
+        z[p] = make_double2(-k * v.y, k * v.x);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        double2 v = z[j];
+        out[(size_t)c0 * N + j] = v.x;
+        if (has1) out[(size_t)c1 * N + j] = v.y;
+    }
+}
+
+static int ilog2(int n) {
+    int l = 0;
+    while ((1 << l) < n) l++;
+    return l;
+}
+static int fft_threads(int N) {
+    int t = N / 2;
+    if (t > 1024) t = 1024;
+    if (t < 32) t = 32;
+    return t;
+}
+
+int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols) {
+    const int N = d->N;
+    size_t smem = sizeof(double2) * (size_t)N;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SWW_CUDA(cudaFuncSetAttribute(k_spectral_gamma_w, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        SWW_CUDA(cudaFuncSetAttribute(k_spectral_deriv, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        attr_set = true;
+    }
+    k_spectral_gamma_w<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, ilog2(N), d->tab->tw, M, T, Gam, W, ncols, w_cols);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int spectral_deriv(sww_dtn_s* d, const double* in, double* out, int ncols) {
+    const int N = d->N;
+    size_t smem = sizeof(double2) * (size_t)N;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SWW_CUDA(cudaFuncSetAttribute(k_spectral_deriv, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        attr_set = true;
+    }
+    k_spectral_deriv<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, ilog2(N), d->tab->tw, in, out, ncols);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+}  // namespace sww

@@ -1,0 +1,71 @@
+// tables.cu -- per-N constant tables: cos/sin(2 pi m/N), (1/2)cot(pi m/N), sin^2(pi m/N), differentiation circulant,
+// FFT twiddles.  "(1/2)cot((alpha_i - alpha_j)/2) ... computed once and for all", PAPER.md:150 (section 2.2).
+// Computed on the device in double-double, cached per (device, N) for the life of the process.
+#include "common.cuh"
+#include "dd.cuh"
+#include <mutex>
+#include <map>
+
+namespace sww {
+
+unsigned long long g_launches = 0;
+char g_cuda_err[256] = "";
+int note_cuda(cudaError_t e, const char* where) {
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return SWW_ECUDA;
+}
+
+__global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, double* dc, double2* tw) {
+    int m = blockIdx.x * blockDim.x + threadIdx.x;
+    if (m >= N) return;
+    dd s, c;
+    dd_sincos_2pi_frac(m, N, &s, &c);
+    dd_store(cs, N, m, c);
+    dd_store(sn, N, m, s);
+    tw[m] = make_double2(c.hi, -s.hi);
+    // half angle pi m / N = 2 pi m / (2N)
+    dd sh, ch;
+    dd_sincos_2pi_frac(m, 2LL * N, &sh, &ch);
+    dd cot = (m == 0) ? dd{0.0, 0.0} : dd_half(dd_div(ch, sh));
+    if (2 * m == N) cot = dd{0.0, 0.0};  // cot(pi/2) = 0 exactly
+    dd_store(c0, N, m, cot);
+    dd_store(s2, N, m, dd_sqr(sh));
+    dd d = (m & 1) ? dd_neg(cot) : cot;  // (1/2)(-1)^m cot(pi m/N): Fourier differentiation matrix for even N (Nyquist -> 0, R4)
+    dd_store(dc, N, m, d);
+}
+
+static std::mutex g_tab_mu;
+static std::map<std::pair<int, int>, Tables*> g_tabs;
+
+int get_tables(int N, cudaStream_t st, const Tables** out) {
+    int dev = 0;
+    SWW_CUDA(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lk(g_tab_mu);
+    auto key = std::make_pair(dev, N);
+    auto it = g_tabs.find(key);
+    if (it != g_tabs.end()) {
+        *out = it->second;
+        return SWW_OK;
+    }
+    Tables* t = new Tables();
+    t->N = N;
+    double* base = nullptr;
+    // 5 dd tables of 2N doubles + N double2
+    SWW_CUDA(cudaMalloc(&base, sizeof(double) * (size_t)N * 12));
+    t->cs = base;
+    t->sn = base + 2 * (size_t)N;
+    t->c0 = base + 4 * (size_t)N;
+    t->s2 = base + 6 * (size_t)N;
+    t->dc = base + 8 * (size_t)N;
+    t->tw = reinterpret_cast<double2*>(base + 10 * (size_t)N);
+    // the default stream orders this before any later stream work after the synchronize below
+    k_tables<<<(N + 127) / 128, 128, 0, st>>>(N, t->cs, t->sn, t->c0, t->s2, t->dc, t->tw);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    SWW_CUDA(cudaStreamSynchronize(st));
+    g_tabs[key] = t;
+    *out = t;
+    return SWW_OK;
+}
+
+}  // namespace sww
