@@ -17,13 +17,14 @@ int ensure_workspace(sww_dtn_s* d, int nrhs) {
     Workspace& w = d->ws;
     if (need <= w.cap_cols) return SWW_OK;
     SWW_CUDA(cudaStreamSynchronize(d->stream));
-    cudaFree(w.B); cudaFree(w.Gam); cudaFree(w.W); cudaFree(w.T); cudaFree(w.R);
+    cudaFree(w.B); cudaFree(w.Gam); cudaFree(w.W); cudaFree(w.T); cudaFree(w.R); cudaFree(w.S);
     w = Workspace();
     size_t per = (size_t)d->N * need * sizeof(double) * (d->prec == SWW_DD ? 2 : 1);
     if (cudaMalloc(&w.B, per) != cudaSuccess || cudaMalloc(&w.Gam, per) != cudaSuccess || cudaMalloc(&w.W, per) != cudaSuccess ||
         cudaMalloc(&w.T, per) != cudaSuccess)
         return SWW_ENOMEM;
     if (d->prec == SWW_DD && cudaMalloc(&w.R, (size_t)d->N * need * sizeof(double)) != cudaSuccess) return SWW_ENOMEM;
+    if (cudaMalloc(&w.S, (size_t)d->N * need * sizeof(double)) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaMemsetAsync(w.B, 0, per, d->stream));
     SWW_CUDA(cudaMemsetAsync(w.Gam, 0, per, d->stream));
     SWW_CUDA(cudaMemsetAsync(w.W, 0, per, d->stream));
@@ -45,29 +46,18 @@ __global__ void k_rhs_lin_f64(int N, size_t total, const double* __restrict__ de
     T[e] = u[j] * de;
 }
 
-// (2.9):  u = (phi' - eta' W0)/(1 + eta'^2),  v = (eta' phi' + W0)/(1 + eta'^2)
-__global__ void k_base_uv_f64(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* __restrict__ W0,
-                              double* __restrict__ u, double* __restrict__ v) {
-    int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= N) return;
-    double e1 = d1[j], den = fma(e1, e1, 1.0);
-    u[j] = (dphi[j] - e1 * W0[j]) / den;
-    v[j] = fma(e1, dphi[j], W0[j]) / den;
-}
-
 static int apply_f64(sww_dtn_s* d, const double* rhs_dev /* N x nrhs, or NULL when ws.B is already filled */, const double* Tcols,
                      int nrhs, double* out) {
     const int N = d->N;
     Workspace& w = d->ws;
     if (rhs_dev) SWW_CUDA(cudaMemcpyAsync(w.B, rhs_dev, sizeof(double) * (size_t)N * nrhs, cudaMemcpyDeviceToDevice, d->stream));
-    SWW_TRY(run_solve(d, w.B, nrhs));                                           // S4: mu = A^{-1} b
+    SWW_TRY(run_solve(d, w.B, w.S, nrhs));                                       // S4: mu = A^{-1} b
     SWW_TRY(spectral_gamma_w(d, w.B, Tcols, w.Gam, out, nrhs, nrhs));           // S5: gamma = D mu ; out = |D| mu / 2 - D t
     SWW_TRY(gemm_f64(d->stream, N, nrhs, N, 1.0, d->G, N, w.Gam, N, 1.0, out, N, nrhs));  // S6: out += G gamma   (2.8)
     return SWW_OK;
 }
 
 int dd_apply(sww_dtn_s* d, const double* rhs_dev, bool rhs_in_ws, const double* Tcols, int nrhs, double* out);
-int dd_set_base(sww_dtn_s* d, const double* phi0);
 int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out);
 
 static int do_setup(sww_dtn_s* d, const void* eta) {
@@ -108,7 +98,9 @@ int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_
     alloc(&d->eta, 2 * N); alloc(&d->d1, 2 * N); alloc(&d->d2, 2 * N);
     alloc(&d->E, 2 * N); alloc(&d->Dm, 2 * N); alloc(&d->Sh, 2 * N); alloc(&d->Ch, 2 * N);
     alloc(&d->K, mat); alloc(&d->G, mat); alloc(&d->LU, n2); alloc(&d->invD, 2 * (size_t)N * nb);
-    alloc(&d->bphi, 2 * N); alloc(&d->bW0, 2 * N); alloc(&d->bu, 2 * N); alloc(&d->bv, 2 * N);
+    alloc(&d->bphi, 2 * N); alloc(&d->bW0, 2 * N); alloc(&d->bu, 2 * N); alloc(&d->bv, 2 * N); alloc(&d->tmp, 14 * (size_t)N);
+    d->bp_chunks = N / 32 < 1 ? 1 : (N / 32 > 64 ? 64 : N / 32);
+    alloc(&d->bp_part, (size_t)d->bp_chunks * 4 * N);
     if (ok && cudaMalloc(&d->status, sizeof(int)) != cudaSuccess) ok = false;
     if (!ok) { sww_dtn_destroy(d); return SWW_ENOMEM; }
     if (cudaMemsetAsync(d->status, 0, sizeof(int), d->stream) != cudaSuccess) { sww_dtn_destroy(d); return SWW_ECUDA; }
@@ -135,16 +127,7 @@ int sww_dtn_apply(sww_dtn_t d, const void* phi, int nrhs, void* out) {
 int sww_dtn_set_base(sww_dtn_t d, const void* phi0) {
     if (!d || !phi0) return SWW_EINVAL;
     SWW_TRY(ensure_workspace(d, 1));
-    const int N = d->N;
-    if (d->prec == SWW_F64) {
-        SWW_TRY(spectral_deriv(d, (const double*)phi0, d->bphi, 1));
-        SWW_TRY(apply_f64(d, (const double*)phi0, nullptr, 1, d->bW0));
-        k_base_uv_f64<<<(N + 127) / 128, 128, 0, d->stream>>>(N, d->d1, d->bphi, d->bW0, d->bu, d->bv);
-        SWW_LAUNCHED();
-        SWW_CUDA(cudaGetLastError());
-    } else {
-        SWW_TRY(dd_set_base(d, (const double*)phi0));
-    }
+    SWW_TRY(accurate_base(d, (const double*)phi0));
     d->has_base = true;
     return SWW_OK;
 }
@@ -197,8 +180,8 @@ int sww_dtn_status(sww_dtn_t d) {
 int sww_dtn_destroy(sww_dtn_t d) {
     if (!d) return SWW_EINVAL;
     cudaStreamSynchronize(d->stream);
-    double* ptrs[] = {d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, d->K, d->G, d->LU, d->invD, d->bphi, d->bW0, d->bu, d->bv,
-                      d->ws.B, d->ws.Gam, d->ws.W, d->ws.T, d->ws.R};
+    double* ptrs[] = {d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, d->K, d->G, d->LU, d->invD, d->bphi, d->bW0, d->bu, d->bv, d->tmp, d->bp_part,
+                      d->ws.B, d->ws.Gam, d->ws.W, d->ws.T, d->ws.R, d->ws.S};
     for (double* p : ptrs) cudaFree(p);
     cudaFree(d->status);
     delete d;

@@ -2,7 +2,7 @@
 //   S0: eta' = D eta, eta'' = D(D eta) by the Fourier differentiation circulant carried in double-double (R4, R8),
 //       per-node tables exp(-(h+eta_j)) (image term) and, for the dd path, sinh/cosh(eta_j).
 //   S1: K_ij, G_ij of (2.13) with the image kernels subtracted (R1; (A.2),(A.3),(A.8));
-//       diagonal from the limits of PAPER.md:150, 653, 673.  Also writes A = I/2 + K (2.7) into the LU buffer.
+//       diagonal from the limits of PAPER.md:150, 653, 673.  Also writes A - I/2 = K (2.7) into the LU buffer (lu.cu keeps the 1/2 of the pivots implicit).
 // Layout: K, G, LU column-major (entry (i,j) at i + j*N): a warp writes 32 consecutive i for one j (coalesced 256 B).
 // Product code; shares nothing with oracle/.
 #include "common.cuh"
@@ -27,8 +27,9 @@ __global__ void __launch_bounds__(256) k_deriv_dd(int N, const double* __restric
     if (lane == 0) dd_store(out, N, i, acc);
 }
 
-// per-node tables.  f64 path: E = exp(-(h+eta)), Dm = 1 - E (via expm1), in fp64.  dd path: the same in dd plus sinh/cosh(eta).
-__global__ void k_node_tables(int N, double h, int finite, int prec, const double* __restrict__ eta, double* __restrict__ E,
+// per-node tables in dd (planar): E = exp(-(h+eta)), Dm = 1 - E (via expm1) for the image term, sinh/cosh(eta) for the dd kernels.
+// The fp64 assembly reads the hi planes of E, Dm; the dd assembly and the dd base-state pass read everything.
+__global__ void k_node_tables(int N, double h, int finite, const double* __restrict__ eta, double* __restrict__ E,
                               double* __restrict__ Dm, double* __restrict__ Sh, double* __restrict__ Ch, int* status) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
@@ -36,23 +37,14 @@ __global__ void k_node_tables(int N, double h, int finite, int prec, const doubl
     if (finite) {
         dd Y = dd_add_d(e, h);
         if (!(Y.hi > 0.0)) atomicCAS(status, SWW_OK, SWW_EBOTTOM);
-        if (prec == SWW_F64) {
-            E[j] = exp(-Y.hi);
-            Dm[j] = -expm1(-Y.hi);
-            E[N + j] = 0.0;
-            Dm[N + j] = 0.0;
-        } else {
-            dd nY = dd_neg(Y);
-            dd_store(E, N, j, dd_exp(nY));
-            dd_store(Dm, N, j, dd_neg(dd_expm1(nY)));
-        }
+        dd nY = dd_neg(Y);
+        dd_store(E, N, j, dd_exp(nY));
+        dd_store(Dm, N, j, dd_neg(dd_expm1(nY)));
     }
-    if (prec == SWW_DD) {
-        dd sh, ch;
-        dd_sinhcosh(e, &sh, &ch);
-        dd_store(Sh, N, j, sh);
-        dd_store(Ch, N, j, ch);
-    }
+    dd sh, ch;
+    dd_sinhcosh(e, &sh, &ch);
+    dd_store(Sh, N, j, sh);
+    dd_store(Ch, N, j, ch);
 }
 
 // ------------------------------------------------------------------------------------------------ S1: fp64 assembly
@@ -165,7 +157,7 @@ __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __
         size_t o = (size_t)i + (size_t)j * N;
         K[o] = kv;
         G[o] = gv;
-        LU[o] = (i == j) ? 0.5 + kv : kv;
+        LU[o] = kv;  // the LU buffer holds A - I/2 (lu.cu keeps the pivot's 1/2 implicit)
     }
 }
 
@@ -175,6 +167,65 @@ __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __
 constexpr int DD_BAND = 16;
 constexpr int ASMDD_TI = 128;
 constexpr int ASMDD_TJ = 16;
+
+struct NodeDD {  // per-node quantities of one collocation point
+    dd eta, d1, d2, E, Dm, Sh, Ch;
+};
+struct TabDD {  // functions of m = (i - j) mod N
+    dd sn, cs, c0, s2;
+};
+
+// K_ij, G_ij of (2.13) in dd (already scaled by 1/N); dist = circular distance |i-j|
+template <bool FINITE>
+__device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, const TabDD& t, int dist, double rN, dd* kv, dd* gv) {
+    dd k1, g1;
+    if (dist != 0) {
+        dd sh, ch;
+        if (dist <= DD_BAND) {
+            dd_sinhcosh(dd_sub(ni.eta, nj.eta), &sh, &ch);
+        } else {
+            sh = dd_sub(dd_mul(ni.Sh, nj.Ch), dd_mul(ni.Ch, nj.Sh));
+            ch = dd_sub(dd_mul(ni.Ch, nj.Ch), dd_mul(ni.Sh, nj.Sh));
+        }
+        dd p;
+        if (t.cs.hi >= 0.0)
+            p = dd_div(dd_add(t.cs, ch), dd_add(dd_sqr(t.sn), dd_sqr(sh)));
+        else
+            p = dd_div(dd{1.0, 0.0}, dd_sub(ch, t.cs));
+        dd hp = dd_half(p);
+        k1 = dd_mul(hp, dd_sub(dd_mul(nj.d1, t.sn), sh));
+        g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(ni.d1, sh), t.sn)), t.c0);
+    } else {
+        dd den = dd_mul_d(dd_add_d(dd_sqr(ni.d1), 1.0), 2.0);
+        k1 = dd_neg(dd_div(ni.d2, den));
+        g1 = dd_div(dd_mul(ni.d1, ni.d2), den);
+    }
+    dd k2{0, 0}, g2{0, 0};
+    if (FINITE) {
+        dd Eij = dd_mul(ni.E, nj.E);
+        dd omE = dd_add(dd_mul(ni.E, nj.Dm), ni.Dm);
+        dd den = dd_add(dd_sqr(omE), dd_mul_d(dd_mul(Eij, t.s2), 4.0));
+        dd cr = dd_div(dd_mul(Eij, t.sn), den);
+        dd ci = dd_neg(dd_half(dd_div(dd_mul(omE, dd_add_d(Eij, 1.0)), den)));
+        k2 = dd_sub(ci, dd_mul(nj.d1, cr));
+        g2 = dd_sub(cr, dd_mul(ni.d1, ci));
+    }
+    *kv = dd_mul_d(dd_sub(k1, k2), rN);
+    *gv = dd_mul_d(dd_sub(g1, g2), rN);
+}
+
+__device__ __forceinline__ NodeDD load_node(int N, int j, const double* eta, const double* d1, const double* d2, const double* E,
+                                            const double* Dm, const double* Sh, const double* Ch, bool finite) {
+    NodeDD n;
+    n.eta = dd_load(eta, N, j);
+    n.d1 = dd_load(d1, N, j);
+    n.d2 = dd_load(d2, N, j);
+    n.Sh = dd_load(Sh, N, j);
+    n.Ch = dd_load(Ch, N, j);
+    n.E = finite ? dd_load(E, N, j) : dd{0, 0};
+    n.Dm = finite ? dd_load(Dm, N, j) : dd{0, 0};
+    return n;
+}
 
 template <bool FINITE>
 __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* __restrict__ eta, const double* __restrict__ d1,
@@ -189,59 +240,89 @@ __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* _
     const int i = i0 + tid;
     if (i >= N) return;
     const size_t NN = (size_t)N * N;
-    const dd eta_i = dd_load(eta, N, i), d1_i = dd_load(d1, N, i), d2_i = dd_load(d2, N, i);
-    dd E_i{0, 0}, Dm_i{0, 0};
-    if (FINITE) {
-        E_i = dd_load(E, N, i);
-        Dm_i = dd_load(Dm, N, i);
-    }
-    const dd Sh_i = dd_load(Sh, N, i), Ch_i = dd_load(Ch, N, i);
+    const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
     const double rN = 1.0 / (double)N;  // exact power of two
     const int jmax = min(ASMDD_TJ, N - j0);
     for (int jj = 0; jj < jmax; jj++) {
         const int j = j0 + jj, m = (i - j) & mask;
-        const dd sx = dd_load(sn, N, m), cx = dd_load(cs, N, m), d1_j = dd_load(d1, N, j);
-        dd k1, g1;
-        if (i != j) {
-            dd sh, ch;
-            int dist = min(m, N - m);
-            if (dist <= DD_BAND) {
-                dd_sinhcosh(dd_sub(eta_i, dd_load(eta, N, j)), &sh, &ch);
-            } else {
-                dd Sh_j = dd_load(Sh, N, j), Ch_j = dd_load(Ch, N, j);
-                sh = dd_sub(dd_mul(Sh_i, Ch_j), dd_mul(Ch_i, Sh_j));
-                ch = dd_sub(dd_mul(Ch_i, Ch_j), dd_mul(Sh_i, Sh_j));
-            }
-            dd p;
-            if (cx.hi >= 0.0)
-                p = dd_div(dd_add(cx, ch), dd_add(dd_sqr(sx), dd_sqr(sh)));
-            else
-                p = dd_div(dd{1.0, 0.0}, dd_sub(ch, cx));
-            dd hp = dd_half(p);
-            k1 = dd_mul(hp, dd_sub(dd_mul(d1_j, sx), sh));
-            g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(d1_i, sh), sx)), dd_load(c0, N, m));
-        } else {
-            dd den = dd_mul_d(dd_add_d(dd_sqr(d1_i), 1.0), 2.0);
-            k1 = dd_neg(dd_div(d2_i, den));
-            g1 = dd_div(dd_mul(d1_i, d2_i), den);
-        }
-        dd k2{0, 0}, g2{0, 0};
-        if (FINITE) {
-            dd E_j = dd_load(E, N, j), Dm_j = dd_load(Dm, N, j);
-            dd Eij = dd_mul(E_i, E_j);
-            dd omE = dd_add(dd_mul(E_i, Dm_j), Dm_i);
-            dd den = dd_add(dd_sqr(omE), dd_mul_d(dd_mul(Eij, dd_load(s2, N, m)), 4.0));
-            dd cr = dd_div(dd_mul(Eij, sx), den);
-            dd ci = dd_neg(dd_half(dd_div(dd_mul(omE, dd_add_d(Eij, 1.0)), den)));
-            k2 = dd_sub(ci, dd_mul(d1_j, cr));
-            g2 = dd_sub(cr, dd_mul(d1_i, ci));
-        }
-        dd kv = dd_mul_d(dd_sub(k1, k2), rN), gv = dd_mul_d(dd_sub(g1, g2), rN);
+        const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
+        TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
+        dd kv, gv;
+        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, &kv, &gv);
         size_t o = (size_t)i + (size_t)j * N;
         dd_store(K, NN, o, kv);
         dd_store(G, NN, o, gv);
-        LU[o] = (i == j) ? dd_add_d(kv, 0.5).hi : kv.hi;
+        LU[o] = kv.hi;  // the LU buffer holds A - I/2 rounded to fp64
     }
+}
+
+// ------------------------------------------------------------------------------------------------ fused dd pass of the base state
+// For the fp64 handle: the residual of (2.7) and the product with G of (2.8) for ONE vector pair (mu, gam), with the kernel
+// entries evaluated in dd on the fly (nothing stored):  pK_i = sum_j K_ij mu_j ,  pG_i = sum_j G_ij gam_j  over the j-chunk of
+// this CTA; partial sums go to part[chunk][4][N] (pK.hi, pK.lo, pG.hi, pG.lo) and are summed by k_base_reduce.
+// Why dd: the base-state velocities u, v are multiplied into every linearized right-hand side and differentiated twice more,
+// so their rounding noise is amplified by ~N^2/3.
+constexpr int BP_TI = 128;
+template <bool FINITE>
+__global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const double* __restrict__ eta, const double* __restrict__ d1,
+                                                        const double* __restrict__ d2, const double* __restrict__ E,
+                                                        const double* __restrict__ Dm, const double* __restrict__ Sh,
+                                                        const double* __restrict__ Ch, const double* __restrict__ cs,
+                                                        const double* __restrict__ sn, const double* __restrict__ c0,
+                                                        const double* __restrict__ s2, const double* __restrict__ mu,
+                                                        const double* __restrict__ gam, double* __restrict__ part) {
+    const int tid = threadIdx.x, mask = N - 1;
+    const int i = blockIdx.x * BP_TI + tid, j0 = blockIdx.y * jchunk;
+    if (i >= N) return;
+    const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
+    const double rN = 1.0 / (double)N;
+    dd aK{0, 0}, aG{0, 0};
+    for (int jj = 0; jj < jchunk; jj++) {
+        const int j = j0 + jj, m = (i - j) & mask;  // j is uniform over the CTA: node loads broadcast
+        const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
+        TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
+        dd kv, gv;
+        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, &kv, &gv);
+        aK = dd_fma(kv, dd_load(mu, N, j), aK);
+        aG = dd_fma(gv, dd_load(gam, N, j), aG);
+    }
+    double* p = part + (size_t)blockIdx.y * 4 * N;
+    p[i] = aK.hi;
+    p[N + i] = aK.lo;
+    p[2 * N + i] = aG.hi;
+    p[3 * N + i] = aG.lo;
+}
+// res = b - mu/2 - sum pK  (2.7) ;  w = sum pG ;  res_f64 = RN(res)
+__global__ void k_base_reduce(int N, int nchunk, const double* __restrict__ part, const double* __restrict__ b, const double* __restrict__ mu,
+                              double* __restrict__ res, double* __restrict__ res_f64, double* __restrict__ w) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    dd sK{0, 0}, sG{0, 0};
+    for (int c = 0; c < nchunk; c++) {
+        const double* p = part + (size_t)c * 4 * N;
+        sK = dd_add(sK, dd{p[i], p[N + i]});
+        sG = dd_add(sG, dd{p[2 * N + i], p[3 * N + i]});
+    }
+    dd r = dd_sub(dd_sub(dd_load(b, N, i), dd_half(dd_load(mu, N, i))), sK);
+    dd_store(res, N, i, r);
+    res_f64[i] = r.hi;
+    dd_store(w, N, i, sG);
+}
+
+int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* gam, double* res, double* res_f64, double* w) {
+    const int N = d->N;
+    const Tables* t = d->tab;
+    const int nchunk = d->bp_chunks, jchunk = N / nchunk;
+    dim3 grid((N + BP_TI - 1) / BP_TI, nchunk);
+    if (d->finite)
+        k_base_pass_dd<true><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
+    else
+        k_base_pass_dd<false><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
+    SWW_LAUNCHED();
+    k_base_reduce<<<(N + 127) / 128, 128, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
 }
 
 static int run_node_prep(sww_dtn_s* d) {
@@ -252,7 +333,7 @@ static int run_node_prep(sww_dtn_s* d) {
     SWW_LAUNCHED();
     k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->d1, d->d2);
     SWW_LAUNCHED();
-    k_node_tables<<<(N + 127) / 128, 128, 0, st>>>(N, d->h, d->finite ? 1 : 0, d->prec, d->eta, d->E, d->Dm, d->Sh, d->Ch, d->status);
+    k_node_tables<<<(N + 31) / 32, 32, 0, st>>>(N, d->h, d->finite ? 1 : 0, d->eta, d->E, d->Dm, d->Sh, d->Ch, d->status);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

@@ -45,6 +45,7 @@ struct Workspace {
     double* W = nullptr;       // result accumulator
     double* T = nullptr;       // scratch columns (u*deta etc.)
     double* R = nullptr;       // dd: fp64 residual / correction
+    double* S = nullptr;       // low words of the compensated triangular solves (N*cap)
 };
 
 }  // namespace sww
@@ -64,6 +65,9 @@ struct sww_dtn_s {
     double *invD;         // inverses of the diagonal blocks of L and U: 2 * (N/NB) blocks of NB x NB
     // base state (dd planar 2N each): phi0', W0, u, v
     double *bphi, *bW0, *bu, *bv;
+    double *bp_part;      // partial sums of the dd base-state pass: bp_chunks x 4 x N doubles
+    int bp_chunks;
+    double *tmp;          // 14 N doubles: dd scratch vectors of the accurate base state (ddpath.cu)
     bool has_base;
     int* status;          // device sticky status
     sww::Workspace ws;
@@ -81,12 +85,22 @@ int run_setup_f64(sww_dtn_s* d);
 int run_setup_dd(sww_dtn_s* d);
 // LU (lu.cu)
 int run_lu(sww_dtn_s* d);
-// multi-RHS triangular solves with the factors in d->LU; B is N x ncols_pad (ld = N), in place
-int run_solve(sww_dtn_s* d, double* B, int ncols_pad);
+// multi-RHS triangular solves with the factors in d->LU; B is N x ncols (ld = N), in place; Blo (same shape) receives the
+// low word of the compensated solution (B already holds RN(B + Blo)); Blo's incoming content is ignored
+int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols);
 // GEMM (gemm.cu): C[M x Nc] = alpha * A[M x K] * B[K x Nc] + beta * C, all column-major fp64; C may alias A or B only in the
 // panel patterns documented in gemm.cu.  n_valid: columns >= n_valid are not stored.
+struct Epi {
+    double* Clo = nullptr;  // compensated target: C + Clo (same layout and ldc as C)
+    int lo_mode = 1;        // 1: read and write Clo ; 2: write only (incoming Clo taken as zero)
+    int fold = 0;           // 1: renormalise, C = RN(C + Clo), Clo = remainder
+};
 int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* A, int lda, const double* B, int ldb,
-             double beta, double* C, int ldc, int n_valid);
+             double beta, double* C, int ldc, int n_valid, Epi epi = Epi());
+// accurate base state (ddpath.cu): phi0', W0, u, v of (2.9) with mu0 refined to dd; phi0 is dd planar iff prec == SWW_DD
+int accurate_base(sww_dtn_s* d, const double* phi0);
+// fused dd pass (assembly.cu): res = b - mu/2 - K mu, w = G gam with the kernel entries evaluated in dd on the fly; all dd planar 2N
+int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* gam, double* res, double* res_f64, double* w);
 // spectral (fft.cu)
 enum SpecMode { SPEC_APPLY = 0, SPEC_LIN = 1 };
 // For each column c < ncols: Gam_c = D M_c ;  W_c = |D| M_c / 2  - (T ? D T_c : 0)

@@ -1,7 +1,465 @@
-// ddpath.cu -- double-double DtN apply (placeholder until the dd kernels land; returns SWW_EINVAL)
+// ddpath.cu -- double-double ("quadruple precision") kernels of the DtN path, all error-free-transformation FMA
+// code on the CUDA cores, and the two flows that use them:
+//   (1) the ACCURATE BASE STATE (both precisions): W0 = G phi0, u, v of (2.9) with mu0 carried as a dd pair out
+//       of iterative refinement, differentiated by the dd circulant, so that the noise of a first-order operator applied to a
+//       rounded fp64 density (~N eps) does not get amplified a second time by the linearized solve;
+//   (2) the dd DtN apply / linearized apply: "iterative refinement around the double-precision LU ... residuals by a blocked quad
+//       matrix-matrix multiply": mu = sum of fp64 corrections, each from the fp64 LU applied to a dd residual.
+// Product code; shares nothing with oracle/.
 #include "common.cuh"
+#include "dd.cuh"
+
 namespace sww {
-int dd_apply(sww_dtn_s*, const double*, bool, const double*, int, double*) { return SWW_EINVAL; }
-int dd_set_base(sww_dtn_s*, const double*) { return SWW_EINVAL; }
-int dd_linearized(sww_dtn_s*, const double*, const double*, int, double*) { return SWW_EINVAL; }
+
+// ------------------------------------------------------------------------------------------------ dd circulants: D and H
+// mode 0: out = D f,  coefficient (1/2)(-1)^m cot(pi m/N)                       (Fourier differentiation, Nyquist symbol 0, R4)
+// mode 1: out = H f,  coefficient (1/N) cot(pi m/N) (1 - (-1)^m) = 4 c0[m]/N for odd m, 0 for even m   (symbol -i sgn k)
+// Both kernels are odd in m, so out_i = sum_{m=1}^{N/2-1} coef[m] (f_{i-m} - f_{i+m}).  One warp per output node.
+__global__ void __launch_bounds__(256) k_circ_dd(int N, int mode, const double* __restrict__ dc, const double* __restrict__ c0,
+                                                 const double* __restrict__ f, double* __restrict__ out) {
+    int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    if (warp >= N) return;
+    int i = warp, mask = N - 1;
+    dd acc{0.0, 0.0};
+    const double hs = 4.0 / (double)N;  // exact (power of two)
+    for (int m = 1 + lane; m < N / 2; m += 32) {
+        dd c;
+        if (mode == 0) {
+            c = dd_load(dc, N, m);
+        } else {
+            if (!(m & 1)) continue;
+            c = dd_load(c0, N, m);
+            c.hi *= hs;
+            c.lo *= hs;
+        }
+        dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
+        acc = dd_fma(c, dd_sub(a, b), acc);
+    }
+    acc = dd_warp_sum(acc);
+    if (lane == 0) dd_store(out, N, i, acc);
 }
+
+int circ_dd(sww_dtn_s* d, int mode, const double* in, double* out) {
+    const int N = d->N;
+    k_circ_dd<<<(N * 32 + 255) / 256, 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in, out);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ dd mat-vec (one column)
+// y = zs * z + beta * x + alpha * (A x), accumulated in dd.  A column-major N x N, fp64 (Alo == nullptr) or dd (Alo = lo plane).
+// x, z, y dd planar (2N).  y_f64 (optional) receives y rounded to fp64.  zs, beta, alpha must be powers of two or 0 (exact).
+// Block = 8 warps x 32 rows: warp q sums the columns j = q (mod 8) for 32 consecutive rows (coalesced 256 B per load).
+__global__ void __launch_bounds__(256) k_matvec_dd(int N, const double* __restrict__ A, const double* __restrict__ Alo,
+                                                   const double* __restrict__ x, double zs, const double* __restrict__ z, double beta,
+                                                   double alpha, double* __restrict__ y, double* __restrict__ y_f64) {
+    __shared__ double red_hi[8][32], red_lo[8][32];
+    const int lane = threadIdx.x & 31, q = threadIdx.x >> 5;
+    const int i = blockIdx.x * 32 + lane;
+    dd acc{0.0, 0.0};
+    if (i < N) {
+        for (int j = q; j < N; j += 8) {
+            dd xj = dd_load(x, N, j);
+            size_t o = (size_t)j * N + i;
+            dd a{A[o], Alo ? Alo[o] : 0.0};
+            acc = dd_fma(a, xj, acc);
+        }
+    }
+    red_hi[q][lane] = acc.hi;
+    red_lo[q][lane] = acc.lo;
+    __syncthreads();
+    if (q == 0 && i < N) {
+        for (int w = 1; w < 8; w++) acc = dd_add(acc, dd{red_hi[w][lane], red_lo[w][lane]});
+        dd r{alpha * acc.hi, alpha * acc.lo};
+        if (beta != 0.0) {
+            dd xi = dd_load(x, N, i);
+            r = dd_add(r, dd{beta * xi.hi, beta * xi.lo});
+        }
+        if (zs != 0.0) {
+            dd zi = dd_load(z, N, i);
+            r = dd_add(r, dd{zs * zi.hi, zs * zi.lo});
+        }
+        dd_store(y, N, i, r);
+        if (y_f64) y_f64[i] = r.hi;
+    }
+}
+
+static int matvec_dd(sww_dtn_s* d, const double* A, const double* Alo, const double* x, double zs, const double* z, double beta,
+                     double alpha, double* y, double* y_f64) {
+    const int N = d->N;
+    k_matvec_dd<<<(N + 31) / 32, 256, 0, d->stream>>>(N, A, Alo, x, zs, z, beta, alpha, y, y_f64);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ dd GEMM (many columns)
+// Y = zs * Z + beta * X + alpha * (A X): A dd (or fp64) N x N, X, Z, Y dd planar N x ncols (plane size L = N * ld_cols).
+// CTA tile 64 rows x 32 columns, 256 threads, thread tile 4 x 2 (rows ty + 16 r, columns tx + 16 c), k-slab 16.
+constexpr int DG_BM = 64, DG_BN = 32, DG_BK = 16;
+__global__ void __launch_bounds__(256) k_gemm_dd(int N, int ncols, size_t L, const double* __restrict__ A, const double* __restrict__ Alo,
+                                                 const double* __restrict__ X, double zs, const double* __restrict__ Z, double beta,
+                                                 double alpha, double* __restrict__ Y, double* __restrict__ Y_f64) {
+    __shared__ double As_hi[DG_BK][DG_BM], As_lo[DG_BK][DG_BM];
+    __shared__ double Xs_hi[DG_BN][DG_BK + 1], Xs_lo[DG_BN][DG_BK + 1];
+    const int tid = threadIdx.x, ty = tid & 15, tx = tid >> 4;
+    const int i0 = blockIdx.x * DG_BM, c0 = blockIdx.y * DG_BN;
+    dd acc[4][2];
+#pragma unroll
+    for (int r = 0; r < 4; r++)
+#pragma unroll
+        for (int c = 0; c < 2; c++) acc[r][c] = dd{0.0, 0.0};
+    for (int k0 = 0; k0 < N; k0 += DG_BK) {
+        for (int e = tid; e < DG_BK * DG_BM; e += 256) {
+            int kk = e / DG_BM, ii = e % DG_BM;
+            size_t o = (size_t)(k0 + kk) * N + i0 + ii;
+            As_hi[kk][ii] = A[o];
+            As_lo[kk][ii] = Alo ? Alo[o] : 0.0;
+        }
+        for (int e = tid; e < DG_BN * DG_BK; e += 256) {
+            int cc = e / DG_BK, kk = e % DG_BK;
+            int c = c0 + cc;
+            size_t o = (size_t)c * N + k0 + kk;
+            bool ok = c < ncols;
+            Xs_hi[cc][kk] = ok ? X[o] : 0.0;
+            Xs_lo[cc][kk] = ok ? X[L + o] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll 4
+        for (int kk = 0; kk < DG_BK; kk++) {
+            dd a[4], x[2];
+#pragma unroll
+            for (int r = 0; r < 4; r++) a[r] = dd{As_hi[kk][ty + 16 * r], As_lo[kk][ty + 16 * r]};
+#pragma unroll
+            for (int c = 0; c < 2; c++) x[c] = dd{Xs_hi[tx + 16 * c][kk], Xs_lo[tx + 16 * c][kk]};
+#pragma unroll
+            for (int r = 0; r < 4; r++)
+#pragma unroll
+                for (int c = 0; c < 2; c++) acc[r][c] = dd_fma(a[r], x[c], acc[r][c]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int c = 0; c < 2; c++) {
+        int col = c0 + tx + 16 * c;
+        if (col >= ncols) continue;
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+            int i = i0 + ty + 16 * r;
+            size_t o = (size_t)col * N + i;
+            dd v{alpha * acc[r][c].hi, alpha * acc[r][c].lo};
+            if (beta != 0.0) v = dd_add(v, dd{beta * X[o], beta * X[L + o]});
+            if (zs != 0.0) v = dd_add(v, dd{zs * Z[o], zs * Z[L + o]});
+            Y[o] = v.hi;
+            Y[L + o] = v.lo;
+            if (Y_f64) Y_f64[o] = v.hi;
+        }
+    }
+}
+
+static int gemm_dd(sww_dtn_s* d, int ncols, size_t L, const double* A, const double* Alo, const double* X, double zs, const double* Z,
+                   double beta, double alpha, double* Y, double* Y_f64) {
+    const int N = d->N;
+    if (N < DG_BM) {  // tiny N: column by column through the mat-vec kernel (planes are L apart, so repack is not needed when ncols == 1)
+        return SWW_EINVAL;
+    }
+    dim3 grid(N / DG_BM, (ncols + DG_BN - 1) / DG_BN);
+    k_gemm_dd<<<grid, 256, 0, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ pointwise dd helpers
+// mu += delta + delta_lo (the compensated fp64 solve's two words), planar with plane size L; first sweep: mu = delta + delta_lo
+__global__ void k_dd_axpy_f64(size_t n, size_t L, int first, const double* __restrict__ delta, const double* __restrict__ delta_lo,
+                              double* __restrict__ mu) {
+    size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    if (first) {
+        mu[e] = delta[e];
+        mu[L + e] = delta_lo[e];
+    } else {
+        dd m = dd_add(dd{mu[e], mu[L + e]}, dd{delta[e], delta_lo[e]});
+        mu[e] = m.hi;
+        mu[L + e] = m.lo;
+    }
+}
+// planar copy with a different plane stride: dst (plane Ld) <- src (plane Ls), n elements per plane; src_lo may be absent
+__global__ void k_dd_copy(size_t n, size_t Ls, size_t Ld, int has_lo, const double* __restrict__ src, double* __restrict__ dst,
+                          double* __restrict__ dst_f64) {
+    size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= n) return;
+    double hi = src[e], lo = has_lo ? src[Ls + e] : 0.0;
+    dst[e] = hi;
+    dst[Ld + e] = lo;
+    if (dst_f64) dst_f64[e] = hi;
+}
+// (2.9), in dd
+__global__ void k_base_uv_dd(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* __restrict__ W0,
+                             double* __restrict__ u, double* __restrict__ v) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    dd e1 = dd_load(d1, N, j), p = dd_load(dphi, N, j), w = dd_load(W0, N, j);
+    dd den = dd_add_d(dd_sqr(e1), 1.0);
+    dd_store(u, N, j, dd_div(dd_sub(p, dd_mul(e1, w)), den));
+    dd_store(v, N, j, dd_div(dd_add(dd_mul(e1, p), w), den));
+}
+// linearized right-hand sides in dd: B_c = dphi_c - v deta_c (B.1d) ; T_c = u deta_c ; also the fp64 rounding of B for the LU
+__global__ void k_rhs_lin_dd(int N, size_t total, size_t Lin, size_t Lws, const double* __restrict__ deta, const double* __restrict__ dphi,
+                             const double* __restrict__ u, const double* __restrict__ v, double* __restrict__ B, double* __restrict__ T,
+                             double* __restrict__ R) {
+    size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= total) return;
+    int j = (int)(e & (size_t)(N - 1));
+    dd de{deta[e], deta[Lin + e]}, dp{dphi[e], dphi[Lin + e]};
+    dd uj = dd_load(u, N, j), vj = dd_load(v, N, j);
+    dd b = dd_sub(dp, dd_mul(vj, de));
+    dd t = dd_mul(uj, de);
+    B[e] = b.hi;
+    B[Lws + e] = b.lo;
+    T[e] = t.hi;
+    T[Lws + e] = t.lo;
+    R[e] = b.hi;
+}
+
+// ------------------------------------------------------------------------------------------------ dd FFT (column pairs)
+struct cdd {
+    dd re, im;
+};
+__device__ __forceinline__ cdd cdd_add(cdd a, cdd b) { return cdd{dd_add(a.re, b.re), dd_add(a.im, b.im)}; }
+__device__ __forceinline__ cdd cdd_sub(cdd a, cdd b) { return cdd{dd_sub(a.re, b.re), dd_sub(a.im, b.im)}; }
+// a * (wr + i wi)
+__device__ __forceinline__ cdd cdd_mul(cdd a, dd wr, dd wi) {
+    return cdd{dd_sub(dd_mul(a.re, wr), dd_mul(a.im, wi)), dd_add(dd_mul(a.re, wi), dd_mul(a.im, wr))};
+}
+__device__ void fft_dif_dd(cdd* z, int N, const double* __restrict__ cs, const double* __restrict__ sn) {
+    for (int half = N >> 1; half >= 1; half >>= 1) {
+        int tstride = N / (2 * half);
+        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
+            int blk = t / half, o = t - blk * half, i = blk * 2 * half + o, m = o * tstride;
+            cdd a = z[i], b = z[i + half];
+            dd wr = dd_load(cs, N, m), wi = dd_neg(dd_load(sn, N, m));  // exp(-2 pi i m/N)
+            z[i] = cdd_add(a, b);
+            z[i + half] = cdd_mul(cdd_sub(a, b), wr, wi);
+        }
+        __syncthreads();
+    }
+}
+__device__ void ifft_dit_dd(cdd* z, int N, const double* __restrict__ cs, const double* __restrict__ sn) {
+    for (int half = 1; half < N; half <<= 1) {
+        int tstride = N / (2 * half);
+        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
+            int blk = t / half, o = t - blk * half, i = blk * 2 * half + o, m = o * tstride;
+            cdd a = z[i];
+            cdd b = cdd_mul(z[i + half], dd_load(cs, N, m), dd_load(sn, N, m));  // conj twiddle exp(+2 pi i m/N)
+            z[i] = cdd_add(a, b);
+            z[i + half] = cdd_sub(a, b);
+        }
+        __syncthreads();
+    }
+}
+__device__ __forceinline__ int wavenumber_dd(int p, int N, int logN) {
+    int k = (int)(__brev((unsigned)p) >> (32 - logN));
+    if (2 * k == N) return 0;
+    return (2 * k < N) ? k : k - N;
+}
+// Gam_c = D M_c ;  W_c = |D| M_c / 2 - (T ? D T_c : 0), dd planar in/out (plane sizes Lws for M, T, Gam; Lw for W)
+__global__ void __launch_bounds__(512) k_spectral_gamma_w_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
+                                                             size_t Lws, size_t Lw, const double* __restrict__ M, const double* __restrict__ T,
+                                                             double* __restrict__ Gam, double* __restrict__ W, int ncols, int w_cols) {
+    extern __shared__ __align__(16) unsigned char dd_fft_sm[];
+    cdd* z = reinterpret_cast<cdd*>(dd_fft_sm);
+    cdd* zt = z + N;  // second buffer: transform of T (only touched when T != nullptr)
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const double rN = 1.0 / (double)N;
+    if (T) {
+        for (int j = threadIdx.x; j < N; j += blockDim.x) {
+            size_t o0 = (size_t)c0 * N + j, o1 = (size_t)c1 * N + j;
+            zt[j] = cdd{dd{T[o0], T[Lws + o0]}, has1 ? dd{T[o1], T[Lws + o1]} : dd{0, 0}};
+        }
+        __syncthreads();
+        fft_dif_dd(zt, N, cs, sn);
+    }
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        size_t o0 = (size_t)c0 * N + j, o1 = (size_t)c1 * N + j;
+        z[j] = cdd{dd{M[o0], M[Lws + o0]}, has1 ? dd{M[o1], M[Lws + o1]} : dd{0, 0}};
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    // zt <- |k|/2 zhat - i k that (kept for the second inverse transform);  z <- i k zhat
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        double k = (double)wavenumber_dd(p, N, logN) * rN;  // exact: integer times a power of two
+        cdd v = z[p];
+        cdd w{dd_mul_d(v.re, 0.5 * fabs(k)), dd_mul_d(v.im, 0.5 * fabs(k))};
+        if (T) {
+            cdd t = zt[p];
+            w.re = dd_add(w.re, dd_mul_d(t.im, k));
+            w.im = dd_sub(w.im, dd_mul_d(t.re, k));
+        }
+        zt[p] = w;
+        z[p] = cdd{dd_mul_d(v.im, -k), dd_mul_d(v.re, k)};
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        cdd v = z[j];
+        size_t o0 = (size_t)c0 * N + j, o1 = (size_t)c1 * N + j;
+        Gam[o0] = v.re.hi;
+        Gam[Lws + o0] = v.re.lo;
+        Gam[o1] = has1 ? v.im.hi : 0.0;
+        Gam[Lws + o1] = has1 ? v.im.lo : 0.0;
+    }
+    ifft_dit_dd(zt, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        cdd v = zt[j];
+        size_t o0 = (size_t)c0 * N + j, o1 = (size_t)c1 * N + j;
+        if (c0 < w_cols) {
+            W[o0] = v.re.hi;
+            W[Lw + o0] = v.re.lo;
+        }
+        if (c1 < w_cols) {
+            W[o1] = v.im.hi;
+            W[Lw + o1] = v.im.lo;
+        }
+    }
+}
+
+static int ilog2(int n) {
+    int l = 0;
+    while ((1 << l) < n) l++;
+    return l;
+}
+
+// out = a + b, dd planar with plane size N
+__global__ void k_dd_add(int N, const double* a, const double* b, double* out) {  // out may alias a or b
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    dd_store(out, N, j, dd_add(dd_load(a, N, j), dd_load(b, N, j)));
+}
+
+// ------------------------------------------------------------------------------------------------ flow (1): accurate base state
+// phi0: dd planar (2N) when d->prec == SWW_DD, N doubles otherwise.  Uses d->tmp (14N doubles) and column 0 of ws.T|R and ws.S.
+//   dd handle : mu0 by refinement sweeps around the fp64 LU with residuals from the stored dd K; W0 from the stored dd G.
+//   f64 handle: the stored K, G are fp64-rounded, which is not enough here (their rounding alone leaves ~2e-15 of white noise in
+//               v at N = 2048, and every linearized column multiplies v into its right-hand side and differentiates: 3e-12 in
+//               the output).  One fused pass evaluates the kernels in dd on the fly (assembly.cu, base_pass_dd):
+//               mu~ = LU \ phi0 ; gam~ = D mu~ ; [res, w~] = [phi0 - mu~/2 - K mu~, G gam~] (dd) ; delta = LU \ res ;
+//               mu0 = mu~ + delta ; W0 = H D mu0 / 2 + w~ + G_f64 (D delta)   (2.7), (2.8).
+int accurate_base(sww_dtn_s* d, const double* phi0) {
+    const int N = d->N;
+    cudaStream_t st = d->stream;
+    const bool isdd = d->prec == SWW_DD;
+    const size_t NN = (size_t)N * N;
+    double* b = d->tmp;             // phi0 as dd planar
+    double* mu = d->tmp + 2 * N;    // mu0 dd
+    double* gam = d->tmp + 4 * N;   // gamma = D mu0
+    double* hg = d->tmp + 6 * N;    // H gamma
+    double* res = d->tmp + 8 * N;   // residual dd / delta dd
+    double* wt = d->tmp + 10 * N;   // w~ = G gam~
+    double* dgam = d->tmp + 12 * N; // D delta
+    // fp64 scratch column for the LU solves (+ its low word in ws.S)
+    double* rcol = isdd ? d->ws.R : d->ws.T;
+    double* rlo = d->ws.S;
+    unsigned blocks = (unsigned)((N + 255) / 256);
+    k_dd_copy<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, (size_t)N, isdd ? 1 : 0, phi0, b, rcol);
+    SWW_LAUNCHED();
+    if (isdd) {
+        const int nsweep = 3;
+        for (int s = 0; s < nsweep; s++) {
+            SWW_TRY(run_solve(d, rcol, rlo, 1));  // delta = (LU)^{-1} round(r)
+            k_dd_axpy_f64<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, s == 0, rcol, rlo, mu);
+            SWW_LAUNCHED();
+            if (s + 1 < nsweep)  // r = b - mu/2 - K mu   (2.7)
+                SWW_TRY(matvec_dd(d, d->K, d->K + NN, mu, 1.0, b, -0.5, -1.0, res, rcol));
+        }
+        SWW_TRY(circ_dd(d, 0, mu, gam));                                                   // gamma = D mu
+        SWW_TRY(circ_dd(d, 1, gam, hg));                                                   // H gamma
+        SWW_TRY(matvec_dd(d, d->G, d->G + NN, gam, 0.5, hg, 0.0, 1.0, d->bW0, nullptr));   // W0 = H gamma / 2 + G gamma   (2.8)
+    } else {
+        SWW_TRY(run_solve(d, rcol, rlo, 1));
+        k_dd_axpy_f64<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, 1, rcol, rlo, mu);     // mu~
+        SWW_LAUNCHED();
+        SWW_TRY(circ_dd(d, 0, mu, gam));                                                   // gam~ = D mu~
+        SWW_TRY(base_pass_dd(d, b, mu, gam, res, rcol, wt));
+        SWW_TRY(run_solve(d, rcol, rlo, 1));                                               // delta
+        k_dd_axpy_f64<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, 1, rcol, rlo, res);    // res <- delta as dd
+        SWW_LAUNCHED();
+        SWW_TRY(circ_dd(d, 0, res, dgam));                                                 // D delta
+        k_dd_add<<<blocks, 256, 0, st>>>(N, mu, res, mu);                                  // mu0 = mu~ + delta
+        SWW_LAUNCHED();
+        k_dd_add<<<blocks, 256, 0, st>>>(N, gam, dgam, gam);                               // gamma = D mu0
+        SWW_LAUNCHED();
+        SWW_TRY(circ_dd(d, 1, gam, hg));                                                   // H gamma
+        SWW_TRY(matvec_dd(d, d->G, nullptr, dgam, 0.5, hg, 0.0, 1.0, res, nullptr));       // H gamma / 2 + G_f64 (D delta)
+        k_dd_add<<<blocks, 256, 0, st>>>(N, res, wt, d->bW0);                              // W0   (2.8)
+        SWW_LAUNCHED();
+    }
+    SWW_TRY(circ_dd(d, 0, b, d->bphi));                                                    // phi0'
+    k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, d->bW0, d->bu, d->bv);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ flow (2): dd apply
+// rhs: dd planar N x nrhs with plane size Lin (ignored when rhs_in_ws: ws.B (dd) and ws.R (fp64 rounding) are already filled).
+// Tcols: dd planar in ws layout or nullptr.  out: dd planar N x nrhs, plane size Lout = N * nrhs.
+int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcols, int nrhs, double* out) {
+    const int N = d->N;
+    if (N > 2048) return SWW_EINVAL;  // the dd FFT keeps two N-point complex dd arrays in shared memory (2 x 32 B x N <= 128 KB)
+    cudaStream_t st = d->stream;
+    Workspace& w = d->ws;
+    const size_t NN = (size_t)N * N, Lws = (size_t)N * w.cap_cols, Lio = (size_t)N * nrhs, n = Lio;
+    unsigned blocks = (unsigned)((n + 255) / 256);
+    if (!rhs_in_ws) {
+        k_dd_copy<<<blocks, 256, 0, st>>>(n, Lio, Lws, 1, rhs, w.B, w.R);
+        SWW_LAUNCHED();
+    }
+    double* mu = w.W;  // dd planar, ws layout
+    const int nsweep = 3;
+    for (int s = 0; s < nsweep; s++) {
+        SWW_TRY(run_solve(d, w.R, w.S, nrhs));
+        k_dd_axpy_f64<<<blocks, 256, 0, st>>>(n, Lws, s == 0, w.R, w.S, mu);
+        SWW_LAUNCHED();
+        if (s + 1 < nsweep) {  // R = B - mu/2 - K mu in dd, rounded to fp64 for the next LU solve
+            if (N >= DG_BM)
+                SWW_TRY(gemm_dd(d, nrhs, Lws, d->K, d->K + NN, mu, 1.0, w.B, -0.5, -1.0, w.Gam, w.R));
+            else
+                return SWW_EINVAL;
+        }
+    }
+    static bool attr_set = false;
+    if (!attr_set) {
+        SWW_CUDA(cudaFuncSetAttribute(k_spectral_gamma_w_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, 2048 * 32 * 2));
+        attr_set = true;
+    }
+    size_t smem = (size_t)N * sizeof(cdd) * 2;
+    int threads = N / 2 > 512 ? 512 : (N / 2 < 32 ? 32 : N / 2);
+    // Gam = D mu (ws layout) ; out = |D| mu / 2 - D T  (user layout)
+    k_spectral_gamma_w_dd<<<(nrhs + 1) / 2, threads, smem, st>>>(N, ilog2(N), d->tab->cs, d->tab->sn, Lws, Lio, mu, Tcols, w.Gam, out, nrhs, nrhs);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    // out += G Gam : Y = 1*Z + 0*X + 1*(A X) with Z = out (plane Lio) -- the kernel takes one plane size, so go through w.B:
+    k_dd_copy<<<blocks, 256, 0, st>>>(n, Lio, Lws, 1, out, w.B, nullptr);
+    SWW_LAUNCHED();
+    SWW_TRY(gemm_dd(d, nrhs, Lws, d->G, d->G + NN, w.Gam, 1.0, w.B, 0.0, 1.0, w.T == Tcols ? w.W : w.T, nullptr));
+    k_dd_copy<<<blocks, 256, 0, st>>>(n, Lws, Lio, 1, w.T == Tcols ? w.W : w.T, out, nullptr);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out) {
+    const int N = d->N;
+    Workspace& w = d->ws;
+    const size_t Lws = (size_t)N * w.cap_cols, Lio = (size_t)N * nrhs;
+    k_rhs_lin_dd<<<(unsigned)((Lio + 255) / 256), 256, 0, d->stream>>>(N, Lio, Lio, Lws, deta, dphi, d->bu, d->bv, w.B, w.T, w.R);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return dd_apply(d, nullptr, true, w.T, nrhs, out);
+}
+
+}  // namespace sww

@@ -12,11 +12,15 @@ namespace sww {
 
 constexpr double PIVOT_GUARD = 1e-3;
 
+// Storage convention of the LU buffer: the DIAGONAL holds kappa_ii = A_ii - 1/2 (the assembly writes K, not I/2 + K): every
+// trailing update then rounds at the O(1/N) scale of the kernel entries instead of the O(1) scale of the pivot, and the inverse
+// diagonal blocks are formed as perturbations of the identity,  inv(L_kk) = I + E_kk,  inv(U_kk) = 2 I + F_kk,  with
+// L_kk E = -(L_kk - I)  and  U_kk F = -2 (U_kk - I/2)  solved on small quantities only.
+//
 // Factor one nb x nb diagonal block in shared memory (nb <= 64, 256 threads as a 16 x 16 grid, element (i,c) owned by thread
-// (i%16, c%16)).  Phase 1: Gaussian elimination on [A | I] -> [U | inv(L)], multipliers scaled at the end.
-// Phase 2: back substitution on [U | I] -> inv(U).
-__global__ void __launch_bounds__(256) k_lu_diag(double* __restrict__ A, int lda, int nb, double* __restrict__ invL,
-                                                 double* __restrict__ invU, int* status) {
+// (i%16, c%16)).  Phase 1: Gaussian elimination on [A | I] -> [U | inv(L)].  Phase 2: back substitution U F = -2 (U - I/2).
+__global__ void __launch_bounds__(256) k_lu_diag(double* __restrict__ A, int lda, int nb, double* __restrict__ Eout,
+                                                 double* __restrict__ Fout, int* status) {
     extern __shared__ double lu_sm[];
     double(*a)[65] = reinterpret_cast<double(*)[65]>(lu_sm);
     double(*x)[65] = reinterpret_cast<double(*)[65]>(lu_sm + 64 * 65);
@@ -27,11 +31,10 @@ __global__ void __launch_bounds__(256) k_lu_diag(double* __restrict__ A, int lda
         int i = e % nb, c = e / nb;
         a[i][c] = A[(size_t)c * lda + i];
         x[i][c] = (i == c) ? 1.0 : 0.0;
-        y[i][c] = (i == c) ? 1.0 : 0.0;
     }
     for (int j = 0; j < nb; j++) {
         __syncthreads();
-        const double piv = a[j][j];
+        const double piv = 0.5 + a[j][j];
         if (tid == 0) {
             if (!(fabs(piv) >= PIVOT_GUARD)) atomicCAS(status, SWW_OK, SWW_ESINGULAR);
         }
@@ -56,7 +59,12 @@ __global__ void __launch_bounds__(256) k_lu_diag(double* __restrict__ A, int lda
         }
     }
     __syncthreads();
-    // phase 2: U Y = I.  Row k of Y is final (up to the scaling by 1/u_kk) when step k starts.
+    for (int e = tid; e < nb * nb; e += 256) {
+        int i = e % nb, c = e / nb;
+        y[i][c] = (i <= c) ? -2.0 * a[i][c] : 0.0;
+    }
+    __syncthreads();
+    // phase 2: row k of y is final (up to the scaling by 1/u_kk) when step k starts
     for (int k = nb - 1; k > 0; k--) {
         const double rk = rinv[k];
 #pragma unroll
@@ -78,8 +86,8 @@ __global__ void __launch_bounds__(256) k_lu_diag(double* __restrict__ A, int lda
         double v = a[i][c];
         if (i > c) v *= rinv[c];  // L multipliers
         A[(size_t)c * lda + i] = v;
-        invL[(size_t)c * nb + i] = (i >= c) ? x[i][c] : 0.0;
-        invU[(size_t)c * nb + i] = (i <= c) ? y[i][c] * rinv[i] : 0.0;
+        Eout[(size_t)c * nb + i] = (i > c) ? x[i][c] : 0.0;
+        Fout[(size_t)c * nb + i] = (i <= c) ? y[i][c] * rinv[i] : 0.0;
     }
 }
 
@@ -87,8 +95,8 @@ int run_lu(sww_dtn_s* d) {
     const int N = d->N, nb = (N < NB) ? N : NB, nblk = N / nb;
     cudaStream_t st = d->stream;
     double* A = d->LU;
-    double* invLs = d->invD;
-    double* invUs = d->invD + (size_t)nblk * nb * nb;
+    double* Es = d->invD;
+    double* Fs = d->invD + (size_t)nblk * nb * nb;
     constexpr int LU_SMEM = (3 * 64 * 65 + 64) * (int)sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
@@ -98,51 +106,91 @@ int run_lu(sww_dtn_s* d) {
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * nb, rem = N - k0 - nb;
         double* Akk = A + (size_t)k0 * N + k0;
-        double* iL = invLs + (size_t)kb * nb * nb;
-        double* iU = invUs + (size_t)kb * nb * nb;
-        k_lu_diag<<<1, 256, LU_SMEM, st>>>(Akk, N, nb, iL, iU, d->status);
+        double* E = Es + (size_t)kb * nb * nb;
+        double* F = Fs + (size_t)kb * nb * nb;
+        k_lu_diag<<<1, 256, LU_SMEM, st>>>(Akk, N, nb, E, F, d->status);
         SWW_LAUNCHED();
         SWW_CUDA(cudaGetLastError());
         if (rem <= 0) break;
         double* A21 = Akk + nb;               // rows k0+nb.., cols k0..k0+nb
         double* A12 = Akk + (size_t)nb * N;   // rows k0..k0+nb, cols k0+nb..
         double* A22 = A12 + nb;
-        // L21 = A21 inv(U11)   (in place: each CTA owns a 64-row panel with all of its K = nb columns)
-        SWW_TRY(gemm_f64(st, rem, nb, nb, 1.0, A21, N, iU, nb, 0.0, A21, N, nb));
-        // U12 = inv(L11) A12
-        SWW_TRY(gemm_f64(st, nb, rem, nb, 1.0, iL, nb, A12, N, 0.0, A12, N, rem));
+        // L21 = A21 inv(U11) = 2 A21 + A21 F   (in place: each CTA owns a 64-row panel with all of its K = nb columns)
+        SWW_TRY(gemm_f64(st, rem, nb, nb, 1.0, A21, N, F, nb, 2.0, A21, N, nb));
+        // U12 = inv(L11) A12 = A12 + E A12
+        SWW_TRY(gemm_f64(st, nb, rem, nb, 1.0, E, nb, A12, N, 1.0, A12, N, rem));
         // A22 -= L21 U12
         SWW_TRY(gemm_f64(st, rem, rem, nb, -1.0, A21, N, A12, N, 1.0, A22, N, rem));
     }
     return SWW_OK;
 }
 
+// N <= 64 (a single diagonal block): one CTA per column, x = (2 I + F)(I + E) b with the same compensation as below
+__global__ void __launch_bounds__(64) k_solve_small(int N, const double* __restrict__ E, const double* __restrict__ F,
+                                                    double* __restrict__ B, double* __restrict__ Blo) {
+    __shared__ double v[64];
+    const int i = threadIdx.x;
+    double* b = B + (size_t)blockIdx.x * N;
+    double bi = 0.0;
+    if (i < N) v[i] = bi = b[i];
+    __syncthreads();
+    double acc = 0.0;
+    if (i < N)
+        for (int c = 0; c < i; c++) acc = fma(E[(size_t)c * N + i], v[c], acc);
+    double yh = bi + acc;
+    double bb = yh - bi;
+    double yl = (bi - (yh - bb)) + (acc - bb);
+    __syncthreads();
+    if (i < N) v[i] = yh;
+    __syncthreads();
+    if (i < N) {
+        acc = 0.0;
+        for (int c = i; c < N; c++) acc = fma(F[(size_t)c * N + i], v[c], acc);
+        double c2 = 2.0 * yh;
+        double s = __dadd_rn(c2, acc);
+        bb = __dsub_rn(s, c2);
+        double err = __dadd_rn(__dsub_rn(c2, __dsub_rn(s, bb)), __dsub_rn(acc, bb));
+        double lo = fma(2.0, yl, err);
+        double t = __dadd_rn(s, lo);
+        b[i] = t;
+        Blo[(size_t)blockIdx.x * N + i] = __dsub_rn(lo, __dsub_rn(t, s));
+    }
+}
+
 // Solve (LU) X = B for ncols columns, in place.  Forward then backward, right-looking by 64-row blocks:
-//   X_kb = inv(L_kk) B_kb ;  B_below -= L_below,kb X_kb          (and the mirror image with U)
-int run_solve(sww_dtn_s* d, double* B, int ncols) {
+//   Y_kb = B_kb + E_kb B_kb ;  B_below -= L_below,kb Y_kb     then     X_kb = 2 Y_kb + F_kb Y_kb ;  Y_above -= U_above,kb X_kb.
+// The O(1) vectors are carried as hi + lo (B + Blo) through every accumulation (gemm.cu, compensated epilogue).
+int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
     const int N = d->N, nb = (N < NB) ? N : NB, nblk = N / nb;
     cudaStream_t st = d->stream;
     const double* A = d->LU;
-    const double* invLs = d->invD;
-    const double* invUs = d->invD + (size_t)nblk * nb * nb;
+    const double* Es = d->invD;
+    const double* Fs = d->invD + (size_t)nblk * nb * nb;
     if (nblk == 1) {
-        // N < 64 or N == 64: two small products through the scratch buffer (no aliasing in the naive kernel)
-        double* tmp = d->ws.W;
-        SWW_TRY(gemm_f64(st, N, ncols, N, 1.0, invLs, N, B, N, 0.0, tmp, N, ncols));
-        SWW_TRY(gemm_f64(st, N, ncols, N, 1.0, invUs, N, tmp, N, 0.0, B, N, ncols));
+        k_solve_small<<<ncols, 64, 0, st>>>(N, Es, Fs, B, Blo);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
         return SWW_OK;
     }
     for (int kb = 0; kb < nblk; kb++) {
         const int k0 = kb * nb, rem = N - k0 - nb;
         double* Bk = B + k0;
-        SWW_TRY(gemm_f64(st, nb, ncols, nb, 1.0, invLs + (size_t)kb * nb * nb, nb, Bk, N, 0.0, Bk, N, ncols));
-        if (rem > 0) SWW_TRY(gemm_f64(st, rem, ncols, nb, -1.0, A + (size_t)k0 * N + k0 + nb, N, Bk, N, 1.0, Bk + nb, N, ncols));
+        Epi e1{Blo + k0, kb == 0 ? 2 : 1, 1};
+        SWW_TRY(gemm_f64(st, nb, ncols, nb, 1.0, Es + (size_t)kb * nb * nb, nb, Bk, N, 1.0, Bk, N, ncols, e1));
+        if (rem > 0) {
+            Epi e2{Blo + k0 + nb, kb == 0 ? 2 : 1, 0};
+            SWW_TRY(gemm_f64(st, rem, ncols, nb, -1.0, A + (size_t)k0 * N + k0 + nb, N, Bk, N, 1.0, Bk + nb, N, ncols, e2));
+        }
     }
     for (int kb = nblk - 1; kb >= 0; kb--) {
         const int k0 = kb * nb;
         double* Bk = B + k0;
-        SWW_TRY(gemm_f64(st, nb, ncols, nb, 1.0, invUs + (size_t)kb * nb * nb, nb, Bk, N, 0.0, Bk, N, ncols));
-        if (k0 > 0) SWW_TRY(gemm_f64(st, k0, ncols, nb, -1.0, A + (size_t)k0 * N, N, Bk, N, 1.0, B, N, ncols));
+        Epi e1{Blo + k0, 1, 1};
+        SWW_TRY(gemm_f64(st, nb, ncols, nb, 1.0, Fs + (size_t)kb * nb * nb, nb, Bk, N, 2.0, Bk, N, ncols, e1));
+        if (k0 > 0) {
+            Epi e2{Blo, 1, 0};
+            SWW_TRY(gemm_f64(st, k0, ncols, nb, -1.0, A + (size_t)k0 * N, N, Bk, N, 1.0, B, N, ncols, e2));
+        }
     }
     return SWW_OK;
 }
