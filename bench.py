@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- BASELINE.json's metric: DtN right-hand-side columns per second at N = 2048 (fp64 and double-double) and the
+achieved fraction of the FP64 (DMMA) roofline, on synthetic surfaces of the paper's shape.
+
+One "step" = one pass of the whole hot path over one batch: setup of a new surface (node prep S0, K/G assembly S1, LU S2),
+base state (2.9), and the batched linearized DtN of all nrhs columns (S3-S7) -- what one Runge-Kutta stage of the trust-region
+Jacobian costs.  Setup is INSIDE the step: every stage has a new surface.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+N > 1 (torchrun, one rank per GPU): the columns are independent given the surface, so each rank runs the
+step on its own 512 columns -- no data-path collective, "scaling": "weak".  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import sww_inputs as si  # noqa: E402
+
+METRIC = "DtN RHS-columns/sec at N=2048 (fp64)"
+UNIT = "columns/s"
+N_METRIC, NRHS_METRIC, NRHS_DD = 2048, 512, 128
+NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # blackwell_cuda_programming.md: B200 FP64 tensor 45 TFLOP/s, bf16 dense 2250 TFLOP/s
+
+
+def rank_case(rank: int, nrhs: int) -> si.Case:
+    """metric-point surface; rank r perturbs its own set of Fourier coefficients (columns are independent given the surface)"""
+    c = si.metric_point(nrhs)
+    if rank:
+        N, j = c.N, np.arange(c.N, dtype=np.int64)
+        for i in range(nrhs // 2):
+            k = 1 + (rank * (nrhs // 2) + i) % (N // 2 - 1)
+            col = 2.0 * np.cos(2.0 * np.pi * ((k * j) % N) / N)
+            c.deta[2 * i] = col
+            c.dphi[2 * i + 1] = col
+    return c
+
+
+class ClockSampler(threading.Thread):
+    """samples SM clock and throttle reasons of one GPU while the timed region runs (NVML; nvidia-smi fallback)"""
+
+    def __init__(self, index: int, period: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt = threading.Event()
+        self._nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nvml = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nvml = None
+
+    def _sample(self):
+        p = self._nvml
+        if p is not None:
+            self.samples.append(p.nvmlDeviceGetClockInfo(self._h, p.NVML_CLOCK_SM))
+            r = p.nvmlDeviceGetCurrentClocksEventReasons(self._h)
+            names = {"sw_power_cap": p.nvmlClocksEventReasonSwPowerCap, "hw_slowdown": p.nvmlClocksEventReasonHwSlowdown,
+                     "hw_thermal_slowdown": p.nvmlClocksEventReasonHwThermalSlowdown,
+                     "sw_thermal_slowdown": p.nvmlClocksEventReasonSwThermalSlowdown,
+                     "applications_clocks_setting": p.nvmlClocksEventReasonApplicationsClocksSetting}
+            for n, bit in names.items():
+                if r & bit:
+                    self.reasons.add(n)
+        else:
+            import subprocess
+            q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+            o = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                               capture_output=True, text=True).stdout.strip().split(",")
+            if len(o) >= 6:
+                self.samples.append(int(o[0]))
+                self.max_mhz = int(o[1])
+                for n, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), o[2:6]):
+                    if v.strip() == "Active":
+                        self.reasons.add(n)
+
+    def run(self):
+        while not self._stop_evt.is_set():
+            try:
+                self._sample()
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=2.0)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def measured_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        d = json.loads(p.read_text())
+        return {"hbm_gbs": d["hbm_gbs"], "bf16_tflops": d["bf16_tflops"], "source": "measured (MEASURED_PEAKS.json)"}
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def cpu_oracle_columns_per_s(nrhs_target: int, small: int = 4, large: int = 16):
+    """the long-double oracle as it stands, timed on this host: setup + `small` and setup + `large` columns of the metric-point
+    workload; columns/s extrapolated to nrhs_target columns sharing one setup."""
+    import oracle
+    orc = oracle.Oracle("ld")
+    c = si.metric_point(nrhs_target)
+    ts = []
+    for n in (small, large):
+        t0 = time.perf_counter()
+        orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:n], c.dphi[:n])
+        ts.append(time.perf_counter() - t0)
+    t_col = max((ts[1] - ts[0]) / (large - small), 1e-9)
+    t_setup = max(ts[0] - small * t_col, 0.0)
+    value = nrhs_target / (t_setup + nrhs_target * t_col)
+    return {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+            "sample": f"long-double oracle, N={c.N}: setup+base+{small} columns ({ts[0]:.2f} s) and setup+base+{large} columns ({ts[1]:.2f} s) "
+                      f"of the {nrhs_target}; columns/s extrapolated as {nrhs_target}/(t_setup + {nrhs_target} t_col), "
+                      f"t_setup={t_setup:.2f} s, t_col={t_col:.4f} s"}
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle (the only 'reference implementation' this paper-only tier has), rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    import oracle
+    orc = oracle.Oracle("ld")
+    c = si.metric_point(NRHS_METRIC)
+    n_s = 4
+    t0 = time.perf_counter()
+    orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:16], c.dphi[:16])
+    t16 = time.perf_counter() - t0
+    step = lambda: orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:n_s], c.dphi[:n_s])
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    t_step = (time.perf_counter() - t0) / max(args.steps, 1)
+    t_col = max((t16 - t_step) / (16 - n_s), 1e-9)
+    t_setup = max(t_step - n_s * t_col, 0.0)
+    value = NRHS_METRIC / (t_setup + NRHS_METRIC * t_col)
+    sample = (f"each step = long-double oracle setup+base+{n_s} of the {NRHS_METRIC} columns at N={c.N} ({t_step:.2f} s); one untimed "
+              f"16-column call gives t_col={t_col:.4f} s; value = {NRHS_METRIC}/(t_setup + {NRHS_METRIC} t_col)")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * (t_setup + NRHS_METRIC * t_col), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f80 (x87 long double)", "data": "synthetic",
+            "config": {"workload": f"metric point: N={c.N}, h=1, config-3 surface family, nrhs={NRHS_METRIC} linearized-DtN columns, setup inside the step"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-dd", action="store_true", help="skip the double-double leg")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_1210_5672_b200 as sww
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU path (use --impl reference for the oracle arm)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    N, nrhs = N_METRIC, NRHS_METRIC
+    case = rank_case(rank, nrhs)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    eta, phi0, deta, dphi = dev(case.eta), dev(case.phi0), dev(case.deta), dev(case.dphi)
+    out = torch.empty_like(dphi)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")  # > 126 MB L2
+    d = sww.DtN(eta, case.h)
+
+    def step():
+        d.refactor(eta)
+        d.set_base(phi0)
+        d.linearized_apply(deta, dphi, out)
+
+    for _ in range(args.warmup):
+        step()
+    d.check()
+    K = args.steps
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(K)]
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    l0 = sww.launch_count()
+    t_wall = time.perf_counter()
+    for e0, e1 in ev:
+        flush.zero_()  # L2 flush between timed iterations (outside the event pair)
+        e0.record()
+        step()
+        e1.record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    launches = sww.launch_count() - l0
+    clocks = sampler.stop()
+    d.check()
+    total_ms = sum(e0.elapsed_time(e1) for e0, e1 in ev)
+    tt = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    total_ms = float(tt.item())
+    ms_per_step = total_ms / K
+    value = world * nrhs / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel: the DMMA GEMM (LU trailing updates, triangular solves, G product)
+    sww.timing_enable(True)
+    kp = min(K, 10)
+    for _ in range(kp):
+        flush.zero_()
+        step()
+    torch.cuda.synchronize()
+    tm = sww.timing_read()
+    sww.timing_enable(False)
+    kernels = {k: {"ms_per_step": v[0] / kp, "launches_per_step": v[1] / kp} for k, v in tm.items() if v[1]}
+    gemm_ms, gemm_launches = tm["gemm_dmma"][0] / kp, tm["gemm_dmma"][1] / kp
+    flops_step = (2.0 / 3.0) * N ** 3 + 4.0 * N * N * (nrhs + 2)  # LU + (solve + G product) for nrhs columns and the 2 base-state solves
+    peaks = measured_peaks()
+    peak_tf = peaks["bf16_tflops"] * NOMINAL_FP64_OVER_BF16
+    achieved_tf = flops_step / (gemm_ms * 1e-3) / 1e12
+    probe = {"dfma_tflops": sww.probe_fp64_peak(0) / 1e12, "dmma_tflops": sww.probe_fp64_peak(1) / 1e12}
+    roofline = {"bound": "tensor", "kernel": "k_gemm_f64 (DMMA.8x8x4), all launches of one step", "achieved": achieved_tf, "peak": peak_tf,
+                "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+                "peak_source": f"bf16 {peaks['bf16_tflops']} TFLOP/s {peaks['source']} x nominal FP64/bf16 ratio 45/2250",
+                "flops_per_step": flops_step, "kernel_ms_per_step": gemm_ms, "kernel_launches_per_step": gemm_launches,
+                "probe_peaks_this_box": probe, "frac_of_probe_dmma": achieved_tf / probe["dmma_tflops"] if probe["dmma_tflops"] else None,
+                "whole_step_tflops": flops_step / (ms_per_step * 1e-3) / 1e12}
+
+    # ---- e2e: the HOST-buffer entry point, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        h_eta, h_phi0, h_deta, h_dphi = pin(case.eta), pin(case.phi0), pin(case.deta), pin(case.dphi)
+        ke = max(3, min(K, 20))
+        for _ in range(2):
+            sww.dtn_linearized_host(h_eta, h_phi0, h_deta, h_dphi, case.h)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(ke):
+            res = sww.dtn_linearized_host(h_eta, h_phi0, h_deta, h_dphi, case.h)
+        barrier()
+        te = torch.tensor([(time.perf_counter() - t0) / ke], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * nrhs / float(te.item()), "unit": UNIT, "h2d_bytes_per_step": 8 * N * (2 + 2 * nrhs),
+               "d2h_bytes_per_step": 8 * N * nrhs, "ms_per_step": 1e3 * float(te.item()), "steps": ke,
+               "checksum": float(res.abs().sum())}
+
+    # ---- double-double leg of the metric (N = 2048, 128 columns)
+    ddres = None
+    if not args.no_dd:
+        cdd = si.metric_point_dd(NRHS_DD, N)
+        pk = lambda hi, lo: torch.from_numpy(np.stack([hi, lo])).cuda().contiguous()
+        eta_d, phi_d = pk(cdd.eta, cdd.eta_lo), pk(cdd.phi0, cdd.phi0_lo)
+        de_d, dp_d = pk(cdd.deta, cdd.deta_lo), pk(cdd.dphi, cdd.dphi_lo)
+        out_d = torch.empty_like(dp_d)
+        dd_ = sww.DtN(eta_d, cdd.h, sww.DD)
+
+        def step_dd():
+            dd_.refactor(eta_d)
+            dd_.set_base(phi_d)
+            dd_.linearized_apply(de_d, dp_d, out_d)
+
+        for _ in range(3):
+            step_dd()
+        dd_.check()
+        kd = max(3, min(K, 10))
+        evd = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(kd)]
+        barrier()
+        for e0, e1 in evd:
+            flush.zero_()
+            e0.record()
+            step_dd()
+            e1.record()
+        barrier()
+        ms_dd = sum(e0.elapsed_time(e1) for e0, e1 in evd) / kd
+        sww.timing_enable(True)
+        step_dd()
+        torch.cuda.synchronize()
+        tmd = sww.timing_read()
+        sww.timing_enable(False)
+        # dd multiply-adds of one step: 2 residual sweeps + 1 G product over NRHS_DD columns, and the same for the base column
+        ddfma = 3.0 * N * N * (NRHS_DD + 1)
+        t_ddg = tmd["dd_gemm"][0] * 1e-3
+        ddres = {"value": world * NRHS_DD / (ms_dd * 1e-3), "unit": UNIT, "ms_per_step": ms_dd, "N": N, "nrhs": NRHS_DD,
+                 "dd_fma_per_s_in_dd_gemm": ddfma / t_ddg if t_ddg > 0 else None,
+                 "kernels_ms": {k: v[0] for k, v in tmd.items() if v[1]}}
+        if t_ddg > 0 and probe["dfma_tflops"]:
+            # one dd multiply-add (dd_fma, dd.cuh) is 15 dependent fp64 instructions; the bound is the fp64 pipe issue rate = DFMA probe FLOP/s / 2
+            ddres["frac_of_dfma_issue_peak"] = (ddfma / t_ddg) * 15 / (probe["dfma_tflops"] * 1e12 / 2)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_oracle_columns_per_s(nrhs)
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+                "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic",
+                "config": {"workload": f"metric point: N={N}, h=1, config-3 surface family, nrhs={nrhs} linearized-DtN columns per GPU, "
+                                       "setup (assembly+LU) + base state + batched columns inside every step",
+                           "N": N, "nrhs_per_gpu": nrhs, "parallelism": f"columns sharded over {world} GPU(s), no data-path collective",
+                           "l2": "256 MB buffer written between timed iterations (L2 flush), outside the event pairs"},
+                "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "gpu_launches_per_step": launches / K,
+                "roofline": roofline, "kernels": kernels, "dd": ddres, "cpu_baseline": cpu,
+                "wall_s_timed_region_incl_flush": t_wall}
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

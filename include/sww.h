@@ -98,6 +98,14 @@ const char* sww_strerror(int status);
 const char* sww_last_cuda_error(void);
 /* Number of kernels this library has launched since it was loaded (bench.py reports the count per step). */
 unsigned long long sww_launch_count(void);
+/* Per-kernel-class device timing for bench.py's roofline block.  sww_timing_enable(1): from now on every kernel launch of
+ * this library is bracketed by a CUDA event pair on its stream (diagnostic mode: costs two event records per launch; not
+ * thread-safe).  sww_timing_read synchronises those events, adds up elapsed milliseconds and launch counts per class since
+ * the previous read and clears the list.  ms, launches: HOST arrays of nclass >= 6 entries; classes: 0 = K/G assembly (S1),
+ * 1 = LU diagonal-block factorisation, 2 = FP64 DMMA GEMM (LU trailing updates, triangular solves, G product: S2, S4, S6),
+ * 3 = FFT / spectral (S5, S7), 4 = double-double matrix products (EFT kernels), 5 = everything else (streaming). */
+int sww_timing_enable(int on);
+int sww_timing_read(double* ms, unsigned long long* launches, int nclass);
 /* Microbenchmarks used to measure the roofline denominators on the box: returns achieved FLOP/s of a
  * register-resident DFMA loop (which = 0) or DMMA.8x8x4 loop (which = 1) over the whole chip, timed with CUDA events. */
 int sww_probe_fp64_peak(int which, double* flops_per_s);

@@ -16,7 +16,7 @@ EXPORTS = [
     "sww_dtn_setup", "sww_dtn_refactor", "sww_dtn_apply", "sww_dtn_set_base", "sww_dtn_linearized_apply", "sww_dtn_get",
     "sww_dtn_status", "sww_dtn_destroy", "sww_state_create", "sww_rk_advance", "sww_state_read", "sww_state_energy",
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
-    "sww_dtn_linearized_host",
+    "sww_dtn_linearized_host", "sww_timing_enable", "sww_timing_read",
 ]
 
 
@@ -61,6 +61,8 @@ def lib() -> ctypes.CDLL:
         L.sww_launch_count.restype = ctypes.c_ulonglong
         L.sww_probe_fp64_peak.argtypes = [ci, ctypes.POINTER(cd)]
         L.sww_dtn_linearized_host.argtypes = [vp, vp, vp, vp, vp, ci, cd, ci, ci]
+        L.sww_timing_enable.argtypes = [ci]
+        L.sww_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_ulonglong), ci]
         _LIB = L
     return _LIB
 
@@ -95,6 +97,22 @@ def dd_unpack(t: torch.Tensor):
 
 def launch_count() -> int:
     return int(lib().sww_launch_count())
+
+
+KERNEL_CLASSES = ("assembly", "lu_diag", "gemm_dmma", "fft", "dd_gemm", "other")
+
+
+def timing_enable(on: bool):
+    _check(lib().sww_timing_enable(1 if on else 0), "sww_timing_enable")
+
+
+def timing_read() -> dict:
+    """-> {class: (milliseconds, launches)} since the previous read"""
+    n = len(KERNEL_CLASSES)
+    ms = (ctypes.c_double * n)()
+    cnt = (ctypes.c_ulonglong * n)()
+    _check(lib().sww_timing_read(ms, cnt, n), "sww_timing_read")
+    return {k: (ms[i], int(cnt[i])) for i, k in enumerate(KERNEL_CLASSES)}
 
 
 def probe_fp64_peak(which: int) -> float:

@@ -140,6 +140,7 @@ int sww_dtn_linearized_apply(sww_dtn_t d, const void* deta, const void* dphi, in
     if (d->prec == SWW_DD) return dd_linearized(d, (const double*)deta, (const double*)dphi, nrhs, (double*)out);
     const int N = d->N;
     size_t total = (size_t)N * nrhs;
+    SWW_BEGIN(KC_OTHER, d->stream);
     k_rhs_lin_f64<<<(unsigned)((total + 255) / 256), 256, 0, d->stream>>>(N, total, (const double*)deta, (const double*)dphi, d->bu, d->bv,
                                                                          d->ws.B, d->ws.T);
     SWW_LAUNCHED();

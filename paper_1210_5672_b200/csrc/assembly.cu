@@ -314,11 +314,13 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
     const Tables* t = d->tab;
     const int nchunk = d->bp_chunks, jchunk = N / nchunk;
     dim3 grid((N + BP_TI - 1) / BP_TI, nchunk);
+    SWW_BEGIN(KC_DDGEMM, d->stream);
     if (d->finite)
         k_base_pass_dd<true><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
     else
         k_base_pass_dd<false><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
     SWW_LAUNCHED();
+    SWW_BEGIN(KC_OTHER, d->stream);
     k_base_reduce<<<(N + 127) / 128, 128, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -329,10 +331,13 @@ static int run_node_prep(sww_dtn_s* d) {
     const int N = d->N;
     cudaStream_t st = d->stream;
     int blocks = (N * 32 + 255) / 256;
+    SWW_BEGIN(KC_OTHER, st);
     k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->eta, d->d1);
     SWW_LAUNCHED();
+    SWW_BEGIN(KC_OTHER, st);
     k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->d1, d->d2);
     SWW_LAUNCHED();
+    SWW_BEGIN(KC_OTHER, st);
     k_node_tables<<<(N + 31) / 32, 32, 0, st>>>(N, d->h, d->finite ? 1 : 0, d->eta, d->E, d->Dm, d->Sh, d->Ch, d->status);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -344,6 +349,7 @@ int run_setup_f64(sww_dtn_s* d) {
     const int N = d->N;
     const Tables* t = d->tab;
     dim3 grid((N + ASM_TI - 1) / ASM_TI, (N + ASM_TJ - 1) / ASM_TJ);
+    SWW_BEGIN(KC_ASM, d->stream);
     if (d->finite)
         k_assemble_f64<true><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
     else
@@ -358,6 +364,7 @@ int run_setup_dd(sww_dtn_s* d) {
     const int N = d->N;
     const Tables* t = d->tab;
     dim3 grid((N + ASMDD_TI - 1) / ASMDD_TI, (N + ASMDD_TJ - 1) / ASMDD_TJ);
+    SWW_BEGIN(KC_ASM, d->stream);
     if (d->finite)
         k_assemble_dd<true><<<grid, ASMDD_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
     else

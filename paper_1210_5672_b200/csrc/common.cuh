@@ -22,7 +22,21 @@ int note_cuda(cudaError_t e, const char* where);
         int rc_ = (call);                                                     \
         if (rc_ != SWW_OK) return rc_;                                        \
     } while (0)
-#define SWW_LAUNCHED() (++::sww::g_launches)
+// Per-kernel-class device timing (sww_timing_enable / sww_timing_read): when enabled, SWW_BEGIN / SWW_LAUNCHED bracket every
+// launch with a CUDA event pair on the launching stream; off by default (no events, no overhead beyond a branch).
+enum KClass { KC_ASM = 0, KC_LUDIAG = 1, KC_GEMM = 2, KC_FFT = 3, KC_DDGEMM = 4, KC_OTHER = 5, KC_COUNT = 6 };
+extern bool g_timing;
+void timing_begin(int cls, cudaStream_t st);
+void timing_end();
+#define SWW_BEGIN(cls, st)                                   \
+    do {                                                     \
+        if (::sww::g_timing) ::sww::timing_begin(cls, st);   \
+    } while (0)
+#define SWW_LAUNCHED()                                       \
+    do {                                                     \
+        ++::sww::g_launches;                                 \
+        if (::sww::g_timing) ::sww::timing_end();            \
+    } while (0)
 
 // ---------------------------------------------------------------- per-N constant tables (device, cached per N per device)
 // "computed once and for all".  All double-double, planar (hi[N], lo[N]).

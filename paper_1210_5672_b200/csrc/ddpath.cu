@@ -41,6 +41,7 @@ __global__ void __launch_bounds__(256) k_circ_dd(int N, int mode, const double* 
 
 int circ_dd(sww_dtn_s* d, int mode, const double* in, double* out) {
     const int N = d->N;
+    SWW_BEGIN(KC_OTHER, d->stream);
     k_circ_dd<<<(N * 32 + 255) / 256, 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in, out);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -88,6 +89,7 @@ __global__ void __launch_bounds__(256) k_matvec_dd(int N, const double* __restri
 static int matvec_dd(sww_dtn_s* d, const double* A, const double* Alo, const double* x, double zs, const double* z, double beta,
                      double alpha, double* y, double* y_f64) {
     const int N = d->N;
+    SWW_BEGIN(KC_DDGEMM, d->stream);
     k_matvec_dd<<<(N + 31) / 32, 256, 0, d->stream>>>(N, A, Alo, x, zs, z, beta, alpha, y, y_f64);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -165,6 +167,7 @@ static int gemm_dd(sww_dtn_s* d, int ncols, size_t L, const double* A, const dou
         return SWW_EINVAL;
     }
     dim3 grid(N / DG_BM, (ncols + DG_BN - 1) / DG_BN);
+    SWW_BEGIN(KC_DDGEMM, d->stream);
     k_gemm_dd<<<grid, 256, 0, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -364,12 +367,14 @@ int accurate_base(sww_dtn_s* d, const double* phi0) {
     double* rcol = isdd ? d->ws.R : d->ws.T;
     double* rlo = d->ws.S;
     unsigned blocks = (unsigned)((N + 255) / 256);
+    SWW_BEGIN(KC_OTHER, st);
     k_dd_copy<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, (size_t)N, isdd ? 1 : 0, phi0, b, rcol);
     SWW_LAUNCHED();
     if (isdd) {
         const int nsweep = 3;
         for (int s = 0; s < nsweep; s++) {
             SWW_TRY(run_solve(d, rcol, rlo, 1));  // delta = (LU)^{-1} round(r)
+            SWW_BEGIN(KC_OTHER, st);
             k_dd_axpy_f64<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, s == 0, rcol, rlo, mu);
             SWW_LAUNCHED();
             if (s + 1 < nsweep)  // r = b - mu/2 - K mu   (2.7)
@@ -380,24 +385,30 @@ int accurate_base(sww_dtn_s* d, const double* phi0) {
         SWW_TRY(matvec_dd(d, d->G, d->G + NN, gam, 0.5, hg, 0.0, 1.0, d->bW0, nullptr));   // W0 = H gamma / 2 + G gamma   (2.8)
     } else {
         SWW_TRY(run_solve(d, rcol, rlo, 1));
+        SWW_BEGIN(KC_OTHER, st);
         k_dd_axpy_f64<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, 1, rcol, rlo, mu);     // mu~
         SWW_LAUNCHED();
         SWW_TRY(circ_dd(d, 0, mu, gam));                                                   // gam~ = D mu~
         SWW_TRY(base_pass_dd(d, b, mu, gam, res, rcol, wt));
         SWW_TRY(run_solve(d, rcol, rlo, 1));                                               // delta
+        SWW_BEGIN(KC_OTHER, st);
         k_dd_axpy_f64<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, 1, rcol, rlo, res);    // res <- delta as dd
         SWW_LAUNCHED();
         SWW_TRY(circ_dd(d, 0, res, dgam));                                                 // D delta
+        SWW_BEGIN(KC_OTHER, st);
         k_dd_add<<<blocks, 256, 0, st>>>(N, mu, res, mu);                                  // mu0 = mu~ + delta
         SWW_LAUNCHED();
+        SWW_BEGIN(KC_OTHER, st);
         k_dd_add<<<blocks, 256, 0, st>>>(N, gam, dgam, gam);                               // gamma = D mu0
         SWW_LAUNCHED();
         SWW_TRY(circ_dd(d, 1, gam, hg));                                                   // H gamma
         SWW_TRY(matvec_dd(d, d->G, nullptr, dgam, 0.5, hg, 0.0, 1.0, res, nullptr));       // H gamma / 2 + G_f64 (D delta)
+        SWW_BEGIN(KC_OTHER, st);
         k_dd_add<<<blocks, 256, 0, st>>>(N, res, wt, d->bW0);                              // W0   (2.8)
         SWW_LAUNCHED();
     }
     SWW_TRY(circ_dd(d, 0, b, d->bphi));                                                    // phi0'
+    SWW_BEGIN(KC_OTHER, st);
     k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, d->bW0, d->bu, d->bv);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -415,6 +426,7 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
     const size_t NN = (size_t)N * N, Lws = (size_t)N * w.cap_cols, Lio = (size_t)N * nrhs, n = Lio;
     unsigned blocks = (unsigned)((n + 255) / 256);
     if (!rhs_in_ws) {
+        SWW_BEGIN(KC_OTHER, st);
         k_dd_copy<<<blocks, 256, 0, st>>>(n, Lio, Lws, 1, rhs, w.B, w.R);
         SWW_LAUNCHED();
     }
@@ -422,6 +434,7 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
     const int nsweep = 3;
     for (int s = 0; s < nsweep; s++) {
         SWW_TRY(run_solve(d, w.R, w.S, nrhs));
+        SWW_BEGIN(KC_OTHER, st);
         k_dd_axpy_f64<<<blocks, 256, 0, st>>>(n, Lws, s == 0, w.R, w.S, mu);
         SWW_LAUNCHED();
         if (s + 1 < nsweep) {  // R = B - mu/2 - K mu in dd, rounded to fp64 for the next LU solve
@@ -439,13 +452,16 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
     size_t smem = (size_t)N * sizeof(cdd) * 2;
     int threads = N / 2 > 512 ? 512 : (N / 2 < 32 ? 32 : N / 2);
     // Gam = D mu (ws layout) ; out = |D| mu / 2 - D T  (user layout)
+    SWW_BEGIN(KC_FFT, st);
     k_spectral_gamma_w_dd<<<(nrhs + 1) / 2, threads, smem, st>>>(N, ilog2(N), d->tab->cs, d->tab->sn, Lws, Lio, mu, Tcols, w.Gam, out, nrhs, nrhs);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     // out += G Gam : Y = 1*Z + 0*X + 1*(A X) with Z = out (plane Lio) -- the kernel takes one plane size, so go through w.B:
+    SWW_BEGIN(KC_OTHER, st);
     k_dd_copy<<<blocks, 256, 0, st>>>(n, Lio, Lws, 1, out, w.B, nullptr);
     SWW_LAUNCHED();
     SWW_TRY(gemm_dd(d, nrhs, Lws, d->G, d->G + NN, w.Gam, 1.0, w.B, 0.0, 1.0, w.T == Tcols ? w.W : w.T, nullptr));
+    SWW_BEGIN(KC_OTHER, st);
     k_dd_copy<<<blocks, 256, 0, st>>>(n, Lws, Lio, 1, w.T == Tcols ? w.W : w.T, out, nullptr);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -456,6 +472,7 @@ int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs
     const int N = d->N;
     Workspace& w = d->ws;
     const size_t Lws = (size_t)N * w.cap_cols, Lio = (size_t)N * nrhs;
+    SWW_BEGIN(KC_OTHER, d->stream);
     k_rhs_lin_dd<<<(unsigned)((Lio + 255) / 256), 256, 0, d->stream>>>(N, Lio, Lio, Lws, deta, dphi, d->bu, d->bv, w.B, w.T, w.R);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());

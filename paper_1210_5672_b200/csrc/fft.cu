@@ -164,6 +164,7 @@ int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam
         SWW_CUDA(cudaFuncSetAttribute(k_spectral_deriv, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
         attr_set = true;
     }
+    SWW_BEGIN(KC_FFT, d->stream);
     k_spectral_gamma_w<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, ilog2(N), d->tab->tw, M, T, Gam, W, ncols, w_cols);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -178,6 +179,7 @@ int spectral_deriv(sww_dtn_s* d, const double* in, double* out, int ncols) {
         SWW_CUDA(cudaFuncSetAttribute(k_spectral_deriv, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
         attr_set = true;
     }
+    SWW_BEGIN(KC_FFT, d->stream);
     k_spectral_deriv<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, ilog2(N), d->tab->tw, in, out, ncols);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());

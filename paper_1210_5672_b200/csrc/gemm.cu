@@ -176,6 +176,7 @@ static int launch_gemm(cudaStream_t st, int M, int Nc, int K, double alpha, cons
         attr_set = true;
     }
     dim3 grid(M / BM, (Nc + BN - 1) / BN);
+    SWW_BEGIN(KC_GEMM, st);
     kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid, epi);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -189,6 +190,7 @@ int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* 
     if (M % 64 != 0 || K % 16 != 0) {
         if (epi.Clo) return SWW_EINVAL;  // the compensated epilogue exists in the tiled kernel only
         dim3 grid((M + 63) / 64, n_valid);
+        SWW_BEGIN(KC_GEMM, st);
         k_gemm_naive<<<grid, 64, 0, st>>>(M, n_valid, K, alpha, A, lda, B, ldb, beta, C, ldc);
         SWW_LAUNCHED();
         SWW_CUDA(cudaGetLastError());

@@ -108,6 +108,7 @@ int run_lu(sww_dtn_s* d) {
         double* Akk = A + (size_t)k0 * N + k0;
         double* E = Es + (size_t)kb * nb * nb;
         double* F = Fs + (size_t)kb * nb * nb;
+        SWW_BEGIN(KC_LUDIAG, st);
         k_lu_diag<<<1, 256, LU_SMEM, st>>>(Akk, N, nb, E, F, d->status);
         SWW_LAUNCHED();
         SWW_CUDA(cudaGetLastError());
@@ -167,6 +168,7 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
     const double* Es = d->invD;
     const double* Fs = d->invD + (size_t)nblk * nb * nb;
     if (nblk == 1) {
+        SWW_BEGIN(KC_GEMM, st);
         k_solve_small<<<ncols, 64, 0, st>>>(N, Es, Fs, B, Blo);
         SWW_LAUNCHED();
         SWW_CUDA(cudaGetLastError());

@@ -5,6 +5,7 @@
 #include "dd.cuh"
 #include <mutex>
 #include <map>
+#include <vector>
 
 namespace sww {
 
@@ -13,6 +14,37 @@ char g_cuda_err[256] = "";
 int note_cuda(cudaError_t e, const char* where) {
     snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", where, cudaGetErrorString(e));
     return SWW_ECUDA;
+}
+
+// ---- per-kernel-class timing (diagnostics; see common.cuh)
+bool g_timing = false;
+namespace {
+struct TimedLaunch { cudaEvent_t e0, e1; int cls; };
+std::vector<TimedLaunch> g_timed;       // event pairs recorded since the last sww_timing_read
+std::vector<cudaEvent_t> g_event_pool;  // recycled events
+cudaStream_t g_cur_stream = nullptr;
+TimedLaunch g_cur;
+bool g_cur_open = false;
+cudaEvent_t take_event() {
+    if (!g_event_pool.empty()) { cudaEvent_t e = g_event_pool.back(); g_event_pool.pop_back(); return e; }
+    cudaEvent_t e = nullptr;
+    cudaEventCreate(&e);
+    return e;
+}
+}  // namespace
+void timing_begin(int cls, cudaStream_t st) {
+    g_cur.e0 = take_event();
+    g_cur.e1 = take_event();
+    g_cur.cls = cls;
+    g_cur_stream = st;
+    g_cur_open = true;
+    cudaEventRecord(g_cur.e0, st);
+}
+void timing_end() {
+    if (!g_cur_open) return;
+    cudaEventRecord(g_cur.e1, g_cur_stream);
+    g_timed.push_back(g_cur);
+    g_cur_open = false;
 }
 
 __global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, double* dc, double2* tw) {
@@ -59,6 +91,7 @@ int get_tables(int N, cudaStream_t st, const Tables** out) {
     t->dc = base + 8 * (size_t)N;
     t->tw = reinterpret_cast<double2*>(base + 10 * (size_t)N);
     // the default stream orders this before any later stream work after the synchronize below
+    SWW_BEGIN(KC_OTHER, st);
     k_tables<<<(N + 127) / 128, 128, 0, st>>>(N, t->cs, t->sn, t->c0, t->s2, t->dc, t->tw);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -69,3 +102,26 @@ int get_tables(int N, cudaStream_t st, const Tables** out) {
 }
 
 }  // namespace sww
+
+extern "C" {
+int sww_timing_enable(int on) {
+    sww::g_timing = on != 0;
+    return SWW_OK;
+}
+int sww_timing_read(double* ms, unsigned long long* launches, int nclass) {
+    using namespace sww;
+    if (!ms || !launches || nclass < KC_COUNT) return SWW_EINVAL;
+    for (int c = 0; c < nclass; c++) { ms[c] = 0.0; launches[c] = 0; }
+    int rc = SWW_OK;
+    for (auto& t : g_timed) {
+        float f = 0.f;
+        if (cudaEventSynchronize(t.e1) != cudaSuccess || cudaEventElapsedTime(&f, t.e0, t.e1) != cudaSuccess) rc = SWW_ECUDA;
+        ms[t.cls] += f;
+        launches[t.cls]++;
+        g_event_pool.push_back(t.e0);
+        g_event_pool.push_back(t.e1);
+    }
+    g_timed.clear();
+    return rc;
+}
+}

@@ -1,0 +1,85 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads, and exports every symbol include/sww.h declares;
+argument validation that returns before any CUDA call; the Python binding refuses to compute without a device."""
+from __future__ import annotations
+
+import ctypes
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+import torch
+
+ROOT = Path(__file__).resolve().parents[1]
+
+
+@pytest.fixture(scope="module")
+def sww():
+    from paper_1210_5672_b200 import build
+    build.build()
+    import paper_1210_5672_b200 as pkg
+    return pkg
+
+
+def declared_symbols():
+    text = (ROOT / "include" / "sww.h").read_text()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(sww_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_declares_the_north_star_calls():
+    names = declared_symbols()
+    for required in ("sww_dtn_setup", "sww_dtn_apply", "sww_dtn_linearized_apply", "sww_rk_advance"):
+        assert required in names
+
+
+def test_library_exports_every_declared_symbol(sww):
+    L = sww.lib()
+    names = declared_symbols()
+    assert names, "no declarations parsed from include/sww.h"
+    for n in names:
+        assert hasattr(L, n), f"libsww.so does not export {n}"
+    assert sorted(sww.EXPORTS) == names, "binding.EXPORTS and include/sww.h disagree"
+
+
+def test_strerror_and_codes(sww):
+    L = sww.lib()
+    assert L.sww_strerror(0) == b"ok"
+    texts = {L.sww_strerror(c) for c in range(-6, 1)}
+    assert len(texts) == 7 and b"unknown status" not in texts
+    assert L.sww_strerror(-99) == b"unknown status"
+
+
+def test_argument_validation_needs_no_device(sww):
+    L = sww.lib()
+    h = ctypes.c_void_p()
+    buf = np.zeros(64)
+    p = buf.ctypes.data
+    assert L.sww_dtn_setup(None, 64, 1.0, 0, None, ctypes.byref(h)) == -1          # null eta
+    assert L.sww_dtn_setup(p, 48, 1.0, 0, None, ctypes.byref(h)) == -1             # N not a power of two
+    assert L.sww_dtn_setup(p, 8, 1.0, 0, None, ctypes.byref(h)) == -1              # N too small
+    assert L.sww_dtn_setup(p, 16384, 1.0, 0, None, ctypes.byref(h)) == -1          # N too large
+    assert L.sww_dtn_setup(p, 64, 1.0, 7, None, ctypes.byref(h)) == -1             # unknown precision
+    assert L.sww_dtn_setup(p, 64, -1.0, 0, None, ctypes.byref(h)) == -1            # negative depth
+    assert L.sww_dtn_apply(None, p, 1, p) == -1
+    assert L.sww_dtn_linearized_apply(None, p, p, 1, p) == -1
+    assert L.sww_rk_advance(None, 0.1, 1) == -1
+    assert L.sww_dtn_linearized_host(p, p, p, p, p, 48, 1.0, 0, 1) == -1
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU behaviour")
+def test_no_cpu_fallback(sww):
+    eta = torch.zeros(64, dtype=torch.float64)
+    with pytest.raises(RuntimeError, match="no CPU path"):
+        sww.DtN(eta, 1.0)
+    with pytest.raises(RuntimeError, match="no CPU path"):
+        sww.State(eta, eta, 1.0)
+
+
+def test_product_never_imports_the_oracle():
+    for p in (ROOT / "paper_1210_5672_b200").rglob("*"):
+        if p.suffix in (".py", ".cu", ".cuh", ".h"):
+            assert "oracle" not in re.sub(r"(#|//).*", "", p.read_text()).replace("shares nothing with oracle/", ""), p
+    for p in (ROOT / "oracle").rglob("*"):
+        if p.suffix in (".py", ".c", ".h"):
+            assert "paper_1210_5672_b200" not in re.sub(r"(#|//|\*).*", "", p.read_text()), p

@@ -1,0 +1,265 @@
+"""GPU parity tests: the CUDA path (through the C ABI of include/sww.h) against the CPU oracle on the same seeded inputs.
+fp64 results are judged against the long-double oracle (bar 1e-11), double-double results against the __float128 oracle
+(bar 1e-25); the rule is in tests/parity_util.py.  Run on the B200 box with `pytest -m gpu`."""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import sww_inputs as si
+from parity_util import (BAR, check_columns, diff, from_dev, gpu_linearized, ld, lin_scales, oracle_linearized,
+                         sample_columns, to_dev)
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def sww():
+    import paper_1210_5672_b200 as pkg
+    assert pkg.lib_path().exists(), "libsww.so missing: the GPU tests never fall back"
+    assert torch.cuda.is_available()
+    return pkg
+
+
+# ------------------------------------------------------------------------------------------------ config 1
+def test_cfg1_flat_surface_symbol(sww):
+    """eta = 0, phi = cos 3a -> 3 tanh 3 cos 3a  ((4.34); BASELINE.json config 1)"""
+    c = si.config1_flat()
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    out = d.apply(to_dev(c.dphi, None, "f64")).cpu().numpy()[0]
+    d.check()
+    exact = 3.0 * math.tanh(3.0) * c.phi0
+    assert np.abs(out - exact).max() <= 1e-11 * np.abs(exact).max()
+
+
+@pytest.mark.parametrize("h", [1.0, 0.05, float("inf")])
+def test_flat_symbol_all_modes(sww, h):
+    """G e^{ikx} = k tanh(kh) e^{ikx} for every resolved k at once (a multi-column apply with a ragged column count)"""
+    N = 128
+    ks = np.arange(1, N // 2)
+    j = np.arange(N)
+    phi = np.cos(2 * np.pi * ((ks[:, None] * j[None, :]) % N) / N)
+    d = sww.DtN(torch.zeros(N, dtype=torch.float64, device="cuda"), h)
+    out = d.apply(torch.from_numpy(phi).cuda()).cpu().numpy()
+    d.check()
+    sym = ks * (np.tanh(ks * h) if math.isfinite(h) else 1.0)
+    err = np.abs(out - sym[:, None] * phi).max(axis=1) / sym
+    assert err.max() <= 1e-11, err.max()
+
+
+def test_cfg1_single_rhs(sww, orc_ld):
+    c = si.config1()
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    out = from_dev(d.apply(to_dev(c.dphi, None, "f64")), "f64")
+    d.check()
+    orc = orc_ld.dtn_apply(c.eta, c.h, c.dphi)
+    r = check_columns(out, orc, "f64", c.N, np.abs(c.dphi).max(axis=1), "cfg1")
+    assert r["E_col_max"] <= 1e-12  # N = 64 has three digits of margin
+
+
+# ------------------------------------------------------------------------------------------------ assembly, entry by entry
+@pytest.mark.parametrize("N,h", [(64, 1.0), (256, 1.0), (256, 0.05), (128, float("inf"))])
+def test_kernel_matrices_entrywise(sww, orc_ld, N, h):
+    """K, G of (2.13) and eta', eta'' against the oracle: N |dK_ij|, N |dG_ij| at the 1e-13 level"""
+    a, _ = si._family_surface(si.SEED_BASE + 3, N, 0.2 if h > 0.1 else 0.01, kmax=min(64, N // 4))
+    eta = si.synth(N, a)[0]
+    d = sww.DtN(torch.from_numpy(eta).cuda(), h)
+    d.check()
+    o = orc_ld.assemble(eta, h)
+    for name in ("d1", "d2"):
+        g = d.get(name).cpu().numpy()
+        ref = ld(o[name])
+        assert np.abs(g - ref).max() <= 4e-16 * max(1.0, float(np.abs(ref).max())), name
+    scale = {n: float(np.abs(ld(o[n])).max()) for n in ("K", "G")}
+    for name in ("K", "G"):
+        g = d.get(name).cpu().numpy().T  # column-major storage -> [i, j]
+        err = float(np.abs(g - ld(o[name])).max())
+        assert err <= 3e-14 * max(scale[name], 1.0 / N), (name, err, scale[name])
+
+
+def test_kernel_matrices_entrywise_dd(sww, orc_q):
+    N = 128
+    c = si.config4(N, 2)
+    d = sww.DtN(to_dev(c.eta, c.eta_lo, "dd"), c.h, sww.DD)
+    d.check()
+    o = orc_q.assemble((c.eta, c.eta_lo), c.h)
+    for name in ("K", "G"):
+        t = d.get(name).cpu().numpy()
+        g = (t[0].T, t[1].T)
+        err = float(np.abs(diff(g, o[name])).max())
+        assert err <= 1e-29 * N, (name, err)
+
+
+# ------------------------------------------------------------------------------------------------ config 3 (fp64 batch)
+def test_cfg3_linearized_batch(sww, orc_ld):
+    c = si.config3()
+    out, d = gpu_linearized(c)
+    orc, base = oracle_linearized(orc_ld, c)
+    r = check_columns(out, orc, "f64", c.N, lin_scales(c, base), "cfg3")
+    assert r["cols_with_floor_above_bar"] == 0
+    for name in ("dphi0", "W0", "u", "v"):
+        g = d.get(name).cpu().numpy()
+        ref = ld(base[name])
+        assert np.abs(g - ref).max() <= 1e-13 * np.abs(ref).max(), name
+    print("cfg3", r)
+
+
+@pytest.mark.parametrize("nrhs", [1, 2, 3, 63, 65, 130])
+def test_ragged_column_counts(sww, orc_ld, nrhs):
+    """column counts that are not multiples of any tile: every column must match, and nothing is written past nrhs"""
+    c = si.config3(256, 256)
+    sel = np.arange(nrhs) * (256 // nrhs)
+    c.deta, c.dphi = np.ascontiguousarray(c.deta[sel]), np.ascontiguousarray(c.dphi[sel])
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    d.set_base(to_dev(c.phi0, None, "f64"))
+    buf = torch.full((nrhs + 2, c.N), 777.0, dtype=torch.float64, device="cuda")
+    d.linearized_apply(to_dev(c.deta, None, "f64"), to_dev(c.dphi, None, "f64"), out=buf[:nrhs])
+    d.check()
+    assert bool((buf[nrhs:] == 777.0).all()), "wrote past the last column"
+    orc, base = oracle_linearized(orc_ld, c)
+    check_columns(from_dev(buf[:nrhs], "f64"), orc, "f64", c.N, lin_scales(c, base), f"ragged{nrhs}")
+
+
+def test_apply_is_pure_and_repeatable(sww):
+    c = si.config3(256, 64)
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    phi = to_dev(c.dphi, None, "f64")
+    a = d.apply(phi).clone()
+    d.set_base(to_dev(c.phi0, None, "f64"))
+    d.linearized_apply(to_dev(c.deta, None, "f64"), phi)
+    b = d.apply(phi)
+    assert torch.equal(a, b)
+    inplace = phi.clone()
+    d.apply(inplace, out=inplace)
+    assert torch.equal(a, inplace)
+
+
+def test_refactor_matches_fresh_setup(sww):
+    c3, c4 = si.config3(256, 16), si.config4(256, 2)
+    d = sww.DtN(to_dev(c4.eta, None, "f64"), 1.0)
+    d.refactor(to_dev(c3.eta, None, "f64"))
+    fresh = sww.DtN(to_dev(c3.eta, None, "f64"), 1.0)
+    phi = to_dev(c3.dphi, None, "f64")
+    assert torch.equal(d.apply(phi), fresh.apply(phi))
+
+
+# ------------------------------------------------------------------------------------------------ config 4 (double-double)
+def test_cfg4_double_double_batch(sww, orc_q):
+    c = si.config4()
+    out, d = gpu_linearized(c)
+    orc, base = oracle_linearized(orc_q, c)
+    r = check_columns(out, orc, "dd", c.N, lin_scales(c, base), "cfg4")
+    assert r["cols_with_floor_above_bar"] == 0
+    for name in ("dphi0", "W0", "u", "v"):
+        t = d.get(name).cpu().numpy()
+        err = np.abs(diff((t[0], t[1]), base[name])).max()
+        assert err <= 1e-27 * float(np.abs(ld(base[name])).max()), name
+    print("cfg4", r)
+
+
+def test_dd_plain_apply_and_fp64_consistency(sww, orc_q):
+    """dd apply against the __float128 oracle, and the fp64 handle on the rounded inputs agrees with it to fp64 accuracy"""
+    c = si.config4(256, 6)
+    d = sww.DtN(to_dev(c.eta, c.eta_lo, "dd"), c.h, sww.DD)
+    out = from_dev(d.apply(to_dev(c.dphi, c.dphi_lo, "dd")), "dd")
+    d.check()
+    orc = orc_q.dtn_apply((c.eta, c.eta_lo), c.h, (c.dphi, c.dphi_lo))
+    check_columns(out, orc, "dd", c.N, np.abs(c.dphi).max(axis=1), "dd apply")
+    d64 = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    out64 = d64.apply(to_dev(c.dphi, None, "f64")).cpu().numpy()
+    assert np.abs(out64 - out[0]).max() <= 1e-11 * np.abs(out[0]).max()
+
+
+# ------------------------------------------------------------------------------------------------ full sizes, sampled columns
+def test_metric_point_sampled_columns(sww, orc_ld):
+    """BASELINE.json metric point, N = 2048, nrhs = 512, in the launch configuration bench.py times; the oracle checks a
+    seeded subset of 32 columns (k = 1, 2, 3, N/8, N/4 always included)"""
+    c = si.metric_point(512)
+    cols = sample_columns(c, 32)
+    out, d = gpu_linearized(c, cols)
+    orc, base = oracle_linearized(orc_ld, c, cols)
+    r = check_columns(out, orc, "f64", c.N, lin_scales(c, base, cols), "metric")
+    assert r["cols_with_floor_above_bar"] == 0
+    print("metric point", r)
+
+
+def test_metric_point_dd_sampled_columns(sww, orc_q):
+    c = si.metric_point_dd(128, 1024)
+    cols = sample_columns(c, 8)
+    out, d = gpu_linearized(c, cols)
+    orc, base = oracle_linearized(orc_q, c, cols)
+    r = check_columns(out, orc, "dd", c.N, lin_scales(c, base, cols), "metric dd")
+    print("metric dd (N=1024)", r)
+
+
+def test_cfg5_shallow_sampled_columns(sww, orc_ld):
+    """config 5: N = 4096, h = 0.05, phi0 = 0 (u = v = 0: the deta part of every column has no effect); the fp64 floor binds
+    on the lowest wavenumbers only"""
+    c = si.config5()
+    cols = sample_columns(c, 16)
+    out, d = gpu_linearized(c, cols)
+    orc, base = oracle_linearized(orc_ld, c, cols)
+    r = check_columns(out, orc, "f64", c.N, lin_scales(c, base, cols), "cfg5")
+    assert r["cols_with_floor_above_bar"] <= 6
+    print("cfg5", r)
+
+
+def test_properties_at_full_size(sww):
+    """properties that hold at any size, on all 512 columns of the metric point: mean(G phi) = 0 (T4) and
+    self-adjointness int chi G phi = int phi G chi ((B.5))"""
+    c = si.metric_point(512)
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    phi = to_dev(c.dphi + c.deta, None, "f64")
+    w = d.apply(phi)
+    d.check()
+    assert float(w.mean(dim=1).abs().max()) <= 1e-12 * float(w.abs().max())
+    a = phi @ w.T
+    assert float((a - a.T).abs().max()) <= 1e-11 * float(a.abs().max())
+
+
+# ------------------------------------------------------------------------------------------------ degenerate cases and errors
+def test_zero_columns_and_zero_rhs(sww):
+    c = si.config3(256, 4)
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    d.set_base(to_dev(c.phi0, None, "f64"))
+    empty = torch.empty((0, c.N), dtype=torch.float64, device="cuda")
+    assert d.apply(empty).shape == (0, c.N)
+    z = torch.zeros((3, c.N), dtype=torch.float64, device="cuda")
+    assert float(d.linearized_apply(z, z).abs().max()) == 0.0
+    d.check()
+
+
+def test_minimum_size(sww, orc_ld):
+    N = 16
+    a = np.zeros(4); a[1] = 0.05
+    eta = si.synth(N, a)[0]
+    phi = si.synth(N, np.array([0, 0.3, 0.1]), np.array([0, 0.0, 0.2]))
+    d = sww.DtN(torch.from_numpy(eta).cuda(), 1.0)
+    out = from_dev(d.apply(torch.from_numpy(phi).cuda()), "f64")
+    d.check()
+    check_columns(out, orc_ld.dtn_apply(eta, 1.0, phi), "f64", N, np.abs(phi).max(axis=1), "N16")
+
+
+def test_error_codes(sww):
+    N = 64
+    eta = torch.zeros(N, dtype=torch.float64, device="cuda")
+    d = sww.DtN(eta, 1.0)
+    z = torch.zeros((1, N), dtype=torch.float64, device="cuda")
+    with pytest.raises(sww.SwwError) as e:
+        d.linearized_apply(z, z)
+    assert e.value.status == -6  # SWW_ENOBASE
+    bad = sww.DtN(eta - 2.0, 1.0)  # h + eta < 0
+    assert bad.status() == -4       # SWW_EBOTTOM
+    with pytest.raises(sww.SwwError) as e:
+        sww.DtN(torch.zeros(48, dtype=torch.float64, device="cuda"), 1.0)
+    assert e.value.status == -1
+
+
+def test_host_buffer_entry_point(sww):
+    c = si.config3(256, 32)
+    dev, _ = gpu_linearized(c)
+    host = sww.dtn_linearized_host(*(torch.from_numpy(np.ascontiguousarray(a)) for a in (c.eta, c.phi0, c.deta, c.dphi)), c.h)
+    assert np.array_equal(host.numpy(), dev[0])
