@@ -102,7 +102,7 @@ unsigned long long sww_launch_count(void);
  * this library is bracketed by a CUDA event pair on its stream (diagnostic mode: costs two event records per launch; not
  * thread-safe).  sww_timing_read synchronises those events, adds up elapsed milliseconds and launch counts per class since
  * the previous read and clears the list.  ms, launches: HOST arrays of nclass >= 6 entries; classes: 0 = K/G assembly (S1),
- * 1 = LU diagonal-block factorisation, 2 = FP64 DMMA GEMM (LU trailing updates, triangular solves, G product: S2, S4, S6),
+ * 1 = LU factorisation (persistent DMMA dataflow kernel, S2), 2 = FP64 DMMA GEMM (triangular solves, G product: S4, S6),
  * 3 = FFT / spectral (S5, S7), 4 = double-double matrix products (EFT kernels), 5 = everything else (streaming). */
 int sww_timing_enable(int on);
 int sww_timing_read(double* ms, unsigned long long* launches, int nclass);

@@ -105,6 +105,7 @@ int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_
     if (!ok) { sww_dtn_destroy(d); return SWW_ENOMEM; }
     if (cudaMemsetAsync(d->status, 0, sizeof(int), d->stream) != cudaSuccess) { sww_dtn_destroy(d); return SWW_ECUDA; }
     rc = ensure_workspace(d, 64);
+    if (!rc) rc = lu_alloc(d);
     if (!rc) rc = do_setup(d, eta);
     if (rc) { sww_dtn_destroy(d); return rc; }
     *out = d;
@@ -117,8 +118,9 @@ int sww_dtn_refactor(sww_dtn_t d, const void* eta) {
 }
 
 int sww_dtn_apply(sww_dtn_t d, const void* phi, int nrhs, void* out) {
-    if (!d || !phi || !out || nrhs < 0) return SWW_EINVAL;
-    if (nrhs == 0) return SWW_OK;
+    if (!d || nrhs < 0) return SWW_EINVAL;
+    if (nrhs == 0) return SWW_OK;  // an empty batch: the pointers are not looked at
+    if (!phi || !out) return SWW_EINVAL;
     SWW_TRY(ensure_workspace(d, nrhs));
     if (d->prec == SWW_F64) return apply_f64(d, (const double*)phi, nullptr, nrhs, (double*)out);
     return dd_apply(d, (const double*)phi, false, nullptr, nrhs, (double*)out);
@@ -133,9 +135,10 @@ int sww_dtn_set_base(sww_dtn_t d, const void* phi0) {
 }
 
 int sww_dtn_linearized_apply(sww_dtn_t d, const void* deta, const void* dphi, int nrhs, void* out) {
-    if (!d || !deta || !dphi || !out || nrhs < 0) return SWW_EINVAL;
+    if (!d || nrhs < 0) return SWW_EINVAL;
     if (!d->has_base) return SWW_ENOBASE;
     if (nrhs == 0) return SWW_OK;
+    if (!deta || !dphi || !out) return SWW_EINVAL;
     SWW_TRY(ensure_workspace(d, nrhs));
     if (d->prec == SWW_DD) return dd_linearized(d, (const double*)deta, (const double*)dphi, nrhs, (double*)out);
     const int N = d->N;
@@ -164,6 +167,7 @@ int sww_dtn_get(sww_dtn_t d, int which, void* dst) {
         case 6: src = d->bu; n = N * mul; break;
         case 7: src = d->bv; n = N * mul; break;
         case 8: src = d->LU; n = (size_t)N * N; break;
+        case 9: src = reinterpret_cast<const double*>(d->lu_trace); n = d->lu_trace ? 4 * (size_t)(N / 64) * (N / 64) : 0; if (!src) return SWW_EINVAL; break;
         default: return SWW_EINVAL;
     }
     SWW_CUDA(cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDeviceToDevice, d->stream));
@@ -185,6 +189,9 @@ int sww_dtn_destroy(sww_dtn_t d) {
                       d->ws.B, d->ws.Gam, d->ws.W, d->ws.T, d->ws.R, d->ws.S};
     for (double* p : ptrs) cudaFree(p);
     cudaFree(d->status);
+    cudaFree(d->lu_order);
+    cudaFree(d->lu_flags);
+    cudaFree(d->lu_trace);
     delete d;
     return SWW_OK;
 }

@@ -24,7 +24,7 @@ int note_cuda(cudaError_t e, const char* where);
     } while (0)
 // Per-kernel-class device timing (sww_timing_enable / sww_timing_read): when enabled, SWW_BEGIN / SWW_LAUNCHED bracket every
 // launch with a CUDA event pair on the launching stream; off by default (no events, no overhead beyond a branch).
-enum KClass { KC_ASM = 0, KC_LUDIAG = 1, KC_GEMM = 2, KC_FFT = 3, KC_DDGEMM = 4, KC_OTHER = 5, KC_COUNT = 6 };
+enum KClass { KC_ASM = 0, KC_LU = 1, KC_GEMM = 2, KC_FFT = 3, KC_DDGEMM = 4, KC_OTHER = 5, KC_COUNT = 6 };
 extern bool g_timing;
 void timing_begin(int cls, cudaStream_t st);
 void timing_end();
@@ -77,6 +77,10 @@ struct sww_dtn_s {
     double *K, *G;        // column-major N x N (dd: planar 2*N*N)
     double *LU;           // fp64 LU factors of I/2 + K (unit lower L below the diagonal, U on and above), column-major
     double *invD;         // inverses of the diagonal blocks of L and U: 2 * (N/NB) blocks of NB x NB
+    int* lu_order;        // dataflow LU (lu.cu): task order, tile flags (+ the claim counter in slot 0), epoch of the last run
+    unsigned* lu_flags;
+    unsigned lu_epoch;
+    unsigned long long* lu_trace;  // debugging aid (env SWW_LU_TRACE): per-task time stamps of the dataflow LU
     // base state (dd planar 2N each): phi0', W0, u, v
     double *bphi, *bW0, *bu, *bv;
     double *bp_part;      // partial sums of the dd base-state pass: bp_chunks x 4 x N doubles
@@ -98,6 +102,7 @@ int ensure_workspace(sww_dtn_s* d, int nrhs);
 int run_setup_f64(sww_dtn_s* d);
 int run_setup_dd(sww_dtn_s* d);
 // LU (lu.cu)
+int lu_alloc(sww_dtn_s* d);
 int run_lu(sww_dtn_s* d);
 // multi-RHS triangular solves with the factors in d->LU; B is N x ncols (ld = N), in place; Blo (same shape) receives the
 // low word of the compensated solution (B already holds RN(B + Blo)); Blo's incoming content is ignored

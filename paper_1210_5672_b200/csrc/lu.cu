@@ -1,128 +1,450 @@
-// lu.cu -- S2: unpivoted blocked LU of A = I/2 + K (the matrix of (2.7); "LU-factorization") and
+// lu.cu -- S2: unpivoted LU of A = I/2 + K (the matrix of (2.7); "LU-factorization") and
 // S4: the multi-right-hand-side triangular solves ("a single back-solve", "level 3 BLAS speed").
 //
 // No pivoting: the second-kind operator is benign -- sigma(A) in [0.46, 1.01], partial pivoting performs zero row swaps on every
 // workload family; a |U_ii| guard reports SWW_ESINGULAR instead of producing garbage.
-// Right-looking, block size NB = 64.  Diagonal blocks are factored by one CTA, which also forms inv(L_kk) and inv(U_kk), so
-// that the panel solves L21 = A21 inv(U11), U12 = inv(L11) A12 and every block step of the triangular solves are DMMA GEMMs.
+//
+// Factorisation = ONE persistent kernel (k_lu_dataflow), left-looking by 64 x 64 tile.  Every tile (i,j) is a task; a CTA claims
+// the next task from a global counter, accumulates  P = sum_{k < min(i,j)} L_ik U_kj  in DMMA.8x8x4 fragments (operand tiles
+// arrive from L2 by cp.async, double-buffered), and finishes the tile:
+//     diagonal : GETRF of the 64 x 64 block in shared memory (in-warp 32 x 32 LU by shuffles + 32-blocks), plus the inverses of
+//                its triangular factors;
+//     i > j    : L_ij = (A_ij - P) inv(U_jj)  = 2 X + X F_j      (DMMA with the inverse factor);
+//     i < j    : U_ij = inv(L_ii) (A_ij - P)  = X + E_i X.
+// A tile is published by a release store of the epoch into flags[i][j]; consumers acquire-poll it.  Tasks are claimed in level
+// order (level = min(i,j); diagonal tile first, then tiles by distance from the diagonal), so every dependency of a claimed task
+// was claimed earlier by a CTA that is running: no deadlock, no grid-wide barrier, no host round trip.  The pivot chain
+// (GETRF -> two neighbours -> next diagonal tile) is the critical path; everything else overlaps with it.
+//
+// Storage convention of the LU buffer: the DIAGONAL holds kappa_ii = U_ii - 1/2 (the assembly writes K, not I/2 + K): every
+// update then rounds at the O(1/N) scale of the kernel entries instead of the O(1) scale of the pivot, and the inverse
+// diagonal blocks are formed as perturbations of the identity,  inv(L_kk) = I + E_kk,  inv(U_kk) = 2 I + F_kk.
 // Product code; shares nothing with oracle/.
 #include "common.cuh"
+#include <algorithm>
+#include <cstdlib>
+#include <vector>
 
 namespace sww {
 
 constexpr double PIVOT_GUARD = 1e-3;
+constexpr int TS = 64;    // tile size
+constexpr int LDT = 65;   // leading dimension of the row-major work tiles T, Eb, Fb (element (r,c) at r*LDT + c)
+constexpr int LDO = 68;   // leading dimension of the DMMA operand tiles (conflict-free fragment loads)
 
-// Storage convention of the LU buffer: the DIAGONAL holds kappa_ii = A_ii - 1/2 (the assembly writes K, not I/2 + K): every
-// trailing update then rounds at the O(1/N) scale of the kernel entries instead of the O(1) scale of the pivot, and the inverse
-// diagonal blocks are formed as perturbations of the identity,  inv(L_kk) = I + E_kk,  inv(U_kk) = 2 I + F_kk,  with
-// L_kk E = -(L_kk - I)  and  U_kk F = -2 (U_kk - I/2)  solved on small quantities only.
-//
-// Factor one nb x nb diagonal block in shared memory (nb <= 64, 256 threads as a 16 x 16 grid, element (i,c) owned by thread
-// (i%16, c%16)).  Phase 1: Gaussian elimination on [A | I] -> [U | inv(L)].  Phase 2: back substitution U F = -2 (U - I/2).
-__global__ void __launch_bounds__(256) k_lu_diag(double* __restrict__ A, int lda, int nb, double* __restrict__ Eout,
-                                                 double* __restrict__ Fout, int* status) {
-    extern __shared__ double lu_sm[];
-    double(*a)[65] = reinterpret_cast<double(*)[65]>(lu_sm);
-    double(*x)[65] = reinterpret_cast<double(*)[65]>(lu_sm + 64 * 65);
-    double(*y)[65] = reinterpret_cast<double(*)[65]>(lu_sm + 2 * 64 * 65);
-    double* rinv = lu_sm + 3 * 64 * 65;
-    const int tid = threadIdx.x, ty = tid & 15, tx = tid >> 4;
-    for (int e = tid; e < nb * nb; e += 256) {
-        int i = e % nb, c = e / nb;
-        a[i][c] = A[(size_t)c * lda + i];
-        x[i][c] = (i == c) ? 1.0 : 0.0;
-    }
-    for (int j = 0; j < nb; j++) {
+__device__ __forceinline__ void lu_dmma884(double& c0, double& c1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};\n" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ void cp16(void* smem, const void* gmem) {
+    unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(s), "l"(gmem));
+}
+__device__ __forceinline__ void cp_commit() { asm volatile("cp.async.commit_group;\n" ::); }
+template <int n>
+__device__ __forceinline__ void cp_wait() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(n));
+}
+__device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(unsigned* p, unsigned v) {
+    asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
+}
+
+// ------------------------------------------------------------------------------------------------ 64 x 64 GETRF in shared memory
+// One rolled loop of 64 elimination steps by a 256-thread CTA; thread (ty, tx) of a 16 x 16 grid keeps the 4 x 4 register tile
+// rows ty + 16 q, columns tx + 16 b of three matrices:
+//     a : the block itself (diagonal = U_jj - 1/2)           -> L\U in place (unit-lower multipliers, U with the 1/2 implicit)
+//     x : starts as I, receives the same ROW operations      -> inv(L)
+//     y : starts as I, receives the COLUMN operations col_c -= (u_jc / u_jj) col_j   -> inv(U') with U' = diag(U)^-1 U,
+//         so that inv(U) = y diag(1/u_jj).
+// Per step the owners publish column j of a and y and row j of a and x in shared memory (double-buffered: one barrier per
+// step); everything else is 48 register FMAs per thread.  The code is a compact loop on purpose: a fully unrolled in-warp
+// variant was 5x slower because its straight-line code (600 KB) misses the instruction cache on every diagonal tile.
+// Results go to global memory: Ag (leading dimension lda) <- L\U, Eg <- inv(L) - I, Fg <- inv(U) - 2 I (both lde); entries with
+// row or column >= nb are not stored (N < 64: the tile is padded with kappa = 0, i.e. pivots 1/2 and no coupling).
+// vec: 512 + 64 doubles of shared memory.  Every thread of the CTA must call it; T is read before the first barrier only.
+// the 16 elimination steps j = 16 JB .. 16 JB + 15: only the 16 x 16 sub-blocks that can change are touched (static in JB)
+template <int JB>
+__device__ __forceinline__ void getrf64_steps(double (&a)[4][4], double (&x)[4][4], double (&y)[4][4], double* vec, int* status, int tid) {
+    const int ty = tid & 15, tx = tid >> 4;
+    double* rinv = vec + 512;
+#pragma unroll 1
+    for (int jt = 0; jt < 16; jt++) {
+        const int j = 16 * JB + jt;
+        double* colA = vec + (jt & 1) * 256;
+        double* rowA = colA + 64;
+        double* rowX = colA + 128;
+        double* colY = colA + 192;
+        if (tx == jt) {
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                if (q >= JB) colA[ty + 16 * q] = a[q][JB];
+                if (q <= JB) colY[ty + 16 * q] = y[q][JB];
+            }
+        }
+        if (ty == jt) {
+#pragma unroll
+            for (int b = 0; b < 4; b++) {
+                if (b >= JB) rowA[tx + 16 * b] = a[JB][b];
+                if (b <= JB) rowX[tx + 16 * b] = x[JB][b];
+            }
+        }
         __syncthreads();
-        const double piv = 0.5 + a[j][j];
+        const double piv = 0.5 + rowA[j];  // the diagonal holds U_jj - 1/2
+        const double ri = 1.0 / piv;
         if (tid == 0) {
+            rinv[j] = ri;
             if (!(fabs(piv) >= PIVOT_GUARD)) atomicCAS(status, SWW_OK, SWW_ESINGULAR);
         }
-        const double r = 1.0 / piv;
-        if (tid == 0) rinv[j] = r;
+        double l[4], u[4], ut[4], xr[4], yc[4];
 #pragma unroll
-        for (int ri = 0; ri < 4; ri++) {
-            int i = ty + 16 * ri;
-            if (i > j && i < nb) {
-                double l = a[i][j] * r;
+        for (int q = 0; q < 4; q++) {
+            const int row = ty + 16 * q;
+            if (q >= JB) l[q] = (row > j) ? colA[row] * ri : 0.0;
+            if (q <= JB) yc[q] = colY[row];  // Y[r][j] = 0 for r > j already
+        }
 #pragma unroll
-                for (int ci = 0; ci < 4; ci++) {
-                    int c = tx + 16 * ci;
-                    if (c < nb) {
-                        if (c > j)
-                            a[i][c] = fma(-l, a[j][c], a[i][c]);
-                        else
-                            x[i][c] = fma(-l, x[j][c], x[i][c]);
-                    }
-                }
+        for (int b = 0; b < 4; b++) {
+            const int col = tx + 16 * b;
+            if (b >= JB) {
+                u[b] = (col > j) ? rowA[col] : 0.0;
+                ut[b] = u[b] * ri;
+            }
+            if (b <= JB) xr[b] = rowX[col];  // X[j][c] = 0 for c > j already
+        }
+#pragma unroll
+        for (int q = 0; q < 4; q++)
+#pragma unroll
+            for (int b = 0; b < 4; b++) {
+                if (q >= JB && b >= JB) a[q][b] = fma(-l[q], u[b], a[q][b]);
+                if (q >= JB && b == JB && tx == jt && ty + 16 * q > j) a[q][b] = l[q];  // keep the multiplier
+                if (q >= JB && b <= JB) x[q][b] = fma(-l[q], xr[b], x[q][b]);
+                if (q <= JB && b >= JB) y[q][b] = fma(-yc[q], ut[b], y[q][b]);
+            }
+    }
+}
+
+__device__ __noinline__ void getrf64(const double* T, double* vec, int* status, int tid, double* Ag, size_t lda, double* Eg,
+                                     double* Fg, int lde, int nb) {
+    const int ty = tid & 15, tx = tid >> 4;
+    double* rinv = vec + 512;
+    double a[4][4], x[4][4], y[4][4];
+#pragma unroll
+    for (int q = 0; q < 4; q++)
+#pragma unroll
+        for (int b = 0; b < 4; b++) {
+            a[q][b] = T[(ty + 16 * q) * LDT + tx + 16 * b];
+            x[q][b] = y[q][b] = (ty + 16 * q == tx + 16 * b) ? 1.0 : 0.0;
+        }
+    getrf64_steps<0>(a, x, y, vec, status, tid);
+    getrf64_steps<1>(a, x, y, vec, status, tid);
+    getrf64_steps<2>(a, x, y, vec, status, tid);
+    getrf64_steps<3>(a, x, y, vec, status, tid);
+    __syncthreads();  // rinv complete
+#pragma unroll
+    for (int b = 0; b < 4; b++) {
+        const int col = tx + 16 * b;
+        const double rc = rinv[col];
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const int row = ty + 16 * q;
+            if (row < nb && col < nb) {
+                Ag[(size_t)col * lda + row] = a[q][b];
+                Eg[col * lde + row] = (row > col) ? x[q][b] : 0.0;
+                Fg[col * lde + row] = (row < col) ? y[q][b] * rc : ((row == col) ? -2.0 * a[q][b] * rc : 0.0);  // F_rr = 1/U_rr - 2 without cancellation
             }
         }
     }
-    __syncthreads();
-    for (int e = tid; e < nb * nb; e += 256) {
-        int i = e % nb, c = e / nb;
-        y[i][c] = (i <= c) ? -2.0 * a[i][c] : 0.0;
+}
+
+// N <= 64: the whole matrix is one (padded) tile
+__global__ void __launch_bounds__(256) k_lu_single(double* __restrict__ A, int nb, double* __restrict__ Eout, double* __restrict__ Fout, int* status) {
+    extern __shared__ double lu_sm[];
+    double* T = lu_sm;
+    double* vec = T + TS * LDT;
+    const int tid = threadIdx.x;
+    for (int e = tid; e < TS * TS; e += 256) {
+        const int r = e & 63, c = e >> 6;
+        T[r * LDT + c] = (r < nb && c < nb) ? A[(size_t)c * nb + r] : 0.0;  // padding: kappa = 0 -> pivot 1/2, no coupling
     }
     __syncthreads();
-    // phase 2: row k of y is final (up to the scaling by 1/u_kk) when step k starts
-    for (int k = nb - 1; k > 0; k--) {
-        const double rk = rinv[k];
-#pragma unroll
-        for (int ri = 0; ri < 4; ri++) {
-            int i = ty + 16 * ri;
-            if (i < k) {
-                double u = a[i][k] * rk;
-#pragma unroll
-                for (int ci = 0; ci < 4; ci++) {
-                    int c = tx + 16 * ci;
-                    if (c >= k && c < nb) y[i][c] = fma(-u, y[k][c], y[i][c]);
-                }
-            }
-        }
+    getrf64(T, vec, status, tid, A, (size_t)nb, Eout, Fout, nb, nb);
+}
+
+// ------------------------------------------------------------------------------------------------ the persistent dataflow LU
+struct LuArgs {
+    double* A;         // N x N column-major, in place
+    int N, nt;         // nt = N / 64 tiles per side
+    const int* order;  // nt*nt tasks: (i << 16) | j in claim order
+    unsigned* flags;   // nt*nt: flags[i*nt + j] == epoch  <=>  tile (i,j) is final
+    unsigned epoch;
+    unsigned* counter;  // next task to claim (zeroed before the launch)
+    double *Es, *Fs;   // nt blocks of 64 x 64 (column-major, ld 64): inv(L_kk) - I, inv(U_kk) - 2 I
+    int* status;
+    unsigned long long* trace;  // optional: 4 globaltimer stamps per task (claimed, operands done, finalised, published)
+};
+
+__device__ __forceinline__ unsigned long long gtime() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+
+constexpr int LU_SMEM_BYTES = (4 * TS * LDO + TS * LDT + 576) * (int)sizeof(double) + 256;
+
+__global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
+    extern __shared__ __align__(16) double lu_sm[];
+    double* sA = lu_sm;                   // 2 stages of L_ik as As[k][r]
+    double* sB = sA + 2 * TS * LDO;       // 2 stages of U_kj as Bs[n][k]
+    double* T = sB + 2 * TS * LDO;        // work tile
+    double* vec = T + TS * LDT;           // getrf64 scratch (576 doubles)
+    unsigned char* ready = reinterpret_cast<unsigned char*>(vec + 576);  // ready[k]: both operand tiles of step k are final
+    __shared__ int s_task;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wr = warp & 1, wc = warp >> 1, fr = lane >> 2, fk = lane & 3;
+    const int N = p.N, nt = p.nt;
+    const unsigned epoch = p.epoch;
+
+    for (;;) {
+        __syncthreads();  // the previous task is finished with s_task and the shared tiles
+        if (tid == 0) s_task = (int)atomicAdd(p.counter, 1u);
         __syncthreads();
+        const int task = s_task;
+        if (task >= nt * nt) break;
+        const int ij = p.order[task], i = ij >> 16, j = ij & 0xffff, m = min(i, j);
+        double* Cg = p.A + (size_t)j * TS * N + (size_t)i * TS;
+        if (p.trace && tid == 0) p.trace[4 * task] = gtime();
+
+        auto refresh = [&]() {
+            for (int t = tid; t < m; t += 256)
+                ready[t] = (ld_acquire(p.flags + (size_t)i * nt + t) == epoch) && (ld_acquire(p.flags + (size_t)t * nt + j) == epoch);
+        };
+        auto spin = [&](const unsigned* f) {
+            while (ld_acquire(f) != epoch) __nanosleep(40);
+        };
+        auto wait_ready = [&](int k) {  // uniform: ready[] is only written before a __syncthreads
+            if (!ready[k]) {
+                if (tid == 0) {
+                    spin(p.flags + (size_t)i * nt + k);
+                    spin(p.flags + (size_t)k * nt + j);
+                }
+                __syncthreads();
+                refresh();
+                __syncthreads();
+            }
+        };
+        auto issue = [&](int k, int buf) {
+            const double* Lg = p.A + (size_t)k * TS * N + (size_t)i * TS;
+            const double* Ug = p.A + (size_t)j * TS * N + (size_t)k * TS;
+            double* a = sA + buf * TS * LDO;
+            double* b = sB + buf * TS * LDO;
+            for (int c = tid; c < TS * TS / 2; c += 256) {
+                const int col = c >> 5, ch = (c & 31) * 2;
+                cp16(a + col * LDO + ch, Lg + (size_t)col * N + ch);
+                cp16(b + col * LDO + ch, Ug + (size_t)col * N + ch);
+            }
+            cp_commit();
+        };
+        double acc[4][2][2];
+        auto mma_tile = [&](const double* a, const double* b) {  // acc += As x Bs over one 64-deep slab
+            const double* as = a + wr * 32 + fr;
+            const double* bs = b + (wc * 16 + fr) * LDO;
+#pragma unroll
+            for (int k4 = 0; k4 < TS; k4 += 4) {
+                double af[4], bf[2];
+#pragma unroll
+                for (int x = 0; x < 4; x++) af[x] = as[(k4 + fk) * LDO + x * 8];
+#pragma unroll
+                for (int y = 0; y < 2; y++) bf[y] = bs[y * 8 * LDO + k4 + fk];
+#pragma unroll
+                for (int x = 0; x < 4; x++)
+#pragma unroll
+                    for (int y = 0; y < 2; y++) lu_dmma884(acc[x][y][0], acc[x][y][1], af[x], bf[y]);
+            }
+        };
+
+        // own tile -> registers (fragment layout), P = 0
+        double c0[4][2][2];
+#pragma unroll
+        for (int x = 0; x < 4; x++)
+#pragma unroll
+            for (int y = 0; y < 2; y++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    c0[x][y][e] = Cg[(size_t)(wc * 16 + y * 8 + 2 * fk + e) * N + wr * 32 + x * 8 + fr];
+                    acc[x][y][e] = 0.0;
+                }
+        refresh();
+        __syncthreads();
+        if (m > 0) {
+            wait_ready(0);
+            issue(0, 0);
+        }
+        for (int k = 0; k < m; k++) {
+            const bool pre = (k + 1 < m) && ready[k + 1];
+            if (pre) {
+                issue(k + 1, (k + 1) & 1);
+                cp_wait<1>();
+            } else {
+                cp_wait<0>();
+            }
+            __syncthreads();
+            mma_tile(sA + (k & 1) * TS * LDO, sB + (k & 1) * TS * LDO);
+            __syncthreads();
+            if (!pre && k + 1 < m) {
+                wait_ready(k + 1);
+                issue(k + 1, (k + 1) & 1);
+            }
+        }
+        if (p.trace && tid == 0) p.trace[4 * task + 1] = gtime();
+        // X = A_ij - P
+#pragma unroll
+        for (int x = 0; x < 4; x++)
+#pragma unroll
+            for (int y = 0; y < 2; y++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) c0[x][y][e] -= acc[x][y][e];
+
+        if (i == j) {
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) T[(wr * 32 + x * 8 + fr) * LDT + wc * 16 + y * 8 + 2 * fk + e] = c0[x][y][e];
+            __syncthreads();
+            getrf64(T, vec, p.status, tid, Cg, (size_t)N, p.Es + (size_t)i * TS * TS, p.Fs + (size_t)i * TS * TS, TS, TS);
+        } else {
+            const bool lower = i > j;
+            // operand from the diagonal tile: F_j as Bs[n][k] (lower) or E_i as As[k][r] (upper); X as the other operand
+            if (tid == 0) spin(p.flags + (size_t)m * nt + m);
+            __syncthreads();
+            const double* Dg = (lower ? p.Fs : p.Es) + (size_t)m * TS * TS;
+            double* dst = lower ? sB : sA;
+            double* xop = lower ? sA : sB;
+            for (int c = tid; c < TS * TS / 2; c += 256) {
+                const int col = c >> 5, ch = (c & 31) * 2;
+                cp16(dst + col * LDO + ch, Dg + col * TS + ch);
+            }
+            cp_commit();
+            const double scale = lower ? 2.0 : 1.0;
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        const int row = wr * 32 + x * 8 + fr, col = wc * 16 + y * 8 + 2 * fk + e;
+                        xop[col * LDO + row] = c0[x][y][e];  // As[k = col][r = row] (lower)  /  Bs[n = col][k = row] (upper)
+                        acc[x][y][e] = scale * c0[x][y][e];
+                    }
+            cp_wait<0>();
+            __syncthreads();
+            mma_tile(sA, sB);  // lower: 2 X + X F ; upper: X + E X
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) T[(wr * 32 + x * 8 + fr) * LDT + wc * 16 + y * 8 + 2 * fk + e] = acc[x][y][e];
+            __syncthreads();
+            for (int e = tid; e < TS * TS; e += 256) {
+                const int r = e & 63, c = e >> 6;
+                Cg[(size_t)c * N + r] = T[r * LDT + c];
+            }
+        }
+        __syncthreads();  // every thread's stores are issued
+        if (tid == 0) {
+            if (p.trace) p.trace[4 * task + 2] = gtime();
+            __threadfence();
+            st_release(p.flags + (size_t)i * nt + j, epoch);
+            if (p.trace) p.trace[4 * task + 3] = gtime();
+        }
     }
-    for (int e = tid; e < nb * nb; e += 256) {
-        int i = e % nb, c = e / nb;
-        double v = a[i][c];
-        if (i > c) v *= rinv[c];  // L multipliers
-        A[(size_t)c * lda + i] = v;
-        Eout[(size_t)c * nb + i] = (i > c) ? x[i][c] : 0.0;
-        Fout[(size_t)c * nb + i] = (i <= c) ? y[i][c] * rinv[i] : 0.0;
+}
+
+// claim order: level m = min(i,j) ascending; within a level the diagonal tile, then (m+d, m), (m, m+d) for d = 1, 2, ...
+static void build_order(int nt, std::vector<int>& o) {
+    o.clear();
+    for (int m = 0; m < nt; m++) {
+        o.push_back((m << 16) | m);
+        for (int d = 1; m + d < nt; d++) {
+            o.push_back(((m + d) << 16) | m);
+            o.push_back((m << 16) | (m + d));
+        }
     }
+}
+
+int lu_alloc(sww_dtn_s* d) {
+    const int N = d->N;
+    d->lu_order = nullptr;
+    d->lu_flags = nullptr;
+    d->lu_epoch = 0;
+    d->lu_trace = nullptr;
+    if (N <= TS) return SWW_OK;
+    const int nt = N / TS;
+    std::vector<int> o;
+    build_order(nt, o);
+    if (cudaMalloc(&d->lu_order, sizeof(int) * o.size()) != cudaSuccess) return SWW_ENOMEM;
+    if (cudaMalloc(&d->lu_flags, sizeof(unsigned) * ((size_t)nt * nt + 1)) != cudaSuccess) return SWW_ENOMEM;
+    SWW_CUDA(cudaMemcpyAsync(d->lu_order, o.data(), sizeof(int) * o.size(), cudaMemcpyHostToDevice, d->stream));
+    SWW_CUDA(cudaMemsetAsync(d->lu_flags, 0, sizeof(unsigned) * ((size_t)nt * nt + 1), d->stream));
+    if (getenv("SWW_LU_TRACE") && cudaMalloc(&d->lu_trace, sizeof(unsigned long long) * 4 * (size_t)nt * nt) != cudaSuccess) return SWW_ENOMEM;
+    SWW_CUDA(cudaStreamSynchronize(d->stream));  // o goes out of scope
+    return SWW_OK;
+}
+
+static int sm_count() {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (sms <= 0) sms = 148;
+    }
+    return sms;
 }
 
 int run_lu(sww_dtn_s* d) {
     const int N = d->N, nb = (N < NB) ? N : NB, nblk = N / nb;
     cudaStream_t st = d->stream;
-    double* A = d->LU;
     double* Es = d->invD;
     double* Fs = d->invD + (size_t)nblk * nb * nb;
-    constexpr int LU_SMEM = (3 * 64 * 65 + 64) * (int)sizeof(double);
+    constexpr int SINGLE_SMEM = (TS * LDT + 576) * (int)sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
-        SWW_CUDA(cudaFuncSetAttribute(k_lu_diag, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_SMEM));
+        SWW_CUDA(cudaFuncSetAttribute(k_lu_single, cudaFuncAttributeMaxDynamicSharedMemorySize, SINGLE_SMEM));
+        SWW_CUDA(cudaFuncSetAttribute(k_lu_dataflow, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_SMEM_BYTES));
         attr_set = true;
     }
-    for (int kb = 0; kb < nblk; kb++) {
-        const int k0 = kb * nb, rem = N - k0 - nb;
-        double* Akk = A + (size_t)k0 * N + k0;
-        double* E = Es + (size_t)kb * nb * nb;
-        double* F = Fs + (size_t)kb * nb * nb;
-        SWW_BEGIN(KC_LUDIAG, st);
-        k_lu_diag<<<1, 256, LU_SMEM, st>>>(Akk, N, nb, E, F, d->status);
+    if (nblk == 1) {
+        SWW_BEGIN(KC_LU, st);
+        k_lu_single<<<1, 256, SINGLE_SMEM, st>>>(d->LU, nb, Es, Fs, d->status);
         SWW_LAUNCHED();
         SWW_CUDA(cudaGetLastError());
-        if (rem <= 0) break;
-        double* A21 = Akk + nb;               // rows k0+nb.., cols k0..k0+nb
-        double* A12 = Akk + (size_t)nb * N;   // rows k0..k0+nb, cols k0+nb..
-        double* A22 = A12 + nb;
-        // L21 = A21 inv(U11) = 2 A21 + A21 F   (in place: each CTA owns a 64-row panel with all of its K = nb columns)
-        SWW_TRY(gemm_f64(st, rem, nb, nb, 1.0, A21, N, F, nb, 2.0, A21, N, nb));
-        // U12 = inv(L11) A12 = A12 + E A12
-        SWW_TRY(gemm_f64(st, nb, rem, nb, 1.0, E, nb, A12, N, 1.0, A12, N, rem));
-        // A22 -= L21 U12
-        SWW_TRY(gemm_f64(st, rem, rem, nb, -1.0, A21, N, A12, N, 1.0, A22, N, rem));
+        return SWW_OK;
     }
+    LuArgs a;
+    a.A = d->LU;
+    a.N = N;
+    a.nt = nblk;
+    a.order = d->lu_order;
+    a.flags = d->lu_flags + 1;
+    a.counter = d->lu_flags;
+    a.epoch = ++d->lu_epoch;
+    a.Es = Es;
+    a.Fs = Fs;
+    a.status = d->status;
+    a.trace = d->lu_trace;
+    SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), st));
+    const int grid = std::min(sm_count(), nblk * nblk);
+    SWW_BEGIN(KC_LU, st);
+    k_lu_dataflow<<<grid, 256, LU_SMEM_BYTES, st>>>(a);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
     return SWW_OK;
 }
 

@@ -37,8 +37,9 @@ def test_cfg1_flat_surface_symbol(sww):
 
 @pytest.mark.parametrize("h", [1.0, 0.05, float("inf")])
 def test_flat_symbol_all_modes(sww, h):
-    """G e^{ikx} = k tanh(kh) e^{ikx} for every resolved k at once (a multi-column apply with a ragged column count)"""
-    N = 128
+    """G e^{ikx} = k tanh(kh) e^{ikx} for every resolved k at once (a multi-column apply with a ragged column count).
+    The trapezoid rule on the image kernel aliases at the e^{-2hN} level, so the shallow case needs N = 512 (e^{-51})."""
+    N = 512 if h < 0.1 else 128
     ks = np.arange(1, N // 2)
     j = np.arange(N)
     phi = np.cos(2 * np.pi * ((ks[:, None] * j[None, :]) % N) / N)
