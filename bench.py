@@ -31,6 +31,8 @@ import sww_inputs as si  # noqa: E402
 METRIC = "DtN RHS-columns/sec at N=2048 (fp64)"
 UNIT = "columns/s"
 N_METRIC, NRHS_METRIC, NRHS_DD = 2048, 512, 128
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (None = not captured yet)
+TRAFFIC_NCU = {"lu": None, "gemm_dmma": None}
 NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # blackwell_cuda_programming.md: B200 FP64 tensor 45 TFLOP/s, bf16 dense 2250 TFLOP/s
 
 
@@ -250,18 +252,31 @@ def main():
     tm = sww.timing_read()
     sww.timing_enable(False)
     kernels = {k: {"ms_per_step": v[0] / kp, "launches_per_step": v[1] / kp} for k, v in tm.items() if v[1]}
-    gemm_ms, gemm_launches = tm["gemm_dmma"][0] / kp, tm["gemm_dmma"][1] / kp
-    flops_step = (2.0 / 3.0) * N ** 3 + 4.0 * N * N * (nrhs + 2)  # LU + (solve + G product) for nrhs columns and the 2 base-state solves
+    # algorithmic FLOPs per step of the two contraction kernels
+    flops = {"lu": (2.0 / 3.0) * N ** 3,                    # S2: k_lu_dataflow
+             "gemm_dmma": 4.0 * N * N * (nrhs + 2)}         # S4 + S6: triangular solves and G product, nrhs columns + 2 base-state solves
+    flops_step = flops["lu"] + flops["gemm_dmma"]
     peaks = measured_peaks()
     peak_tf = peaks["bf16_tflops"] * NOMINAL_FP64_OVER_BF16
-    achieved_tf = flops_step / (gemm_ms * 1e-3) / 1e12
     probe = {"dfma_tflops": sww.probe_fp64_peak(0) / 1e12, "dmma_tflops": sww.probe_fp64_peak(1) / 1e12}
-    roofline = {"bound": "tensor", "kernel": "k_gemm_f64 (DMMA.8x8x4), all launches of one step", "achieved": achieved_tf, "peak": peak_tf,
-                "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": None,
+    names = {"lu": "k_lu_dataflow (persistent DMMA.8x8x4 tile dataflow, one launch)",
+             "gemm_dmma": "k_gemm_f64 (DMMA.8x8x4), all launches of one step"}
+    per_kernel = {}
+    for cls in ("lu", "gemm_dmma"):
+        ms_c, n_c = tm[cls][0] / kp, tm[cls][1] / kp
+        ach = flops[cls] / (ms_c * 1e-3) / 1e12 if ms_c > 0 else 0.0
+        per_kernel[cls] = {"kernel": names[cls], "achieved": ach, "frac": ach / peak_tf, "flops_per_step": flops[cls],
+                           "kernel_ms_per_step": ms_c, "kernel_launches_per_step": n_c,
+                           "frac_of_probe_dmma": ach / probe["dmma_tflops"] if probe["dmma_tflops"] else None}
+    dom = max(per_kernel, key=lambda c: per_kernel[c]["kernel_ms_per_step"])  # the dominant kernel = the one with the most time
+    roofline = {"bound": "tensor", "kernel": per_kernel[dom]["kernel"], "achieved": per_kernel[dom]["achieved"], "peak": peak_tf,
+                "unit": "TFLOP/s", "frac": per_kernel[dom]["frac"], "traffic": TRAFFIC_NCU.get(dom),
                 "peak_source": f"bf16 {peaks['bf16_tflops']} TFLOP/s {peaks['source']} x nominal FP64/bf16 ratio 45/2250",
-                "flops_per_step": flops_step, "kernel_ms_per_step": gemm_ms, "kernel_launches_per_step": gemm_launches,
-                "probe_peaks_this_box": probe, "frac_of_probe_dmma": achieved_tf / probe["dmma_tflops"] if probe["dmma_tflops"] else None,
-                "whole_step_tflops": flops_step / (ms_per_step * 1e-3) / 1e12}
+                "flops_per_step": per_kernel[dom]["flops_per_step"], "kernel_ms_per_step": per_kernel[dom]["kernel_ms_per_step"],
+                "kernel_launches_per_step": per_kernel[dom]["kernel_launches_per_step"],
+                "probe_peaks_this_box": probe, "frac_of_probe_dmma": per_kernel[dom]["frac_of_probe_dmma"],
+                "contraction_kernels": per_kernel, "whole_step_tflops": flops_step / (ms_per_step * 1e-3) / 1e12,
+                "whole_step_frac": flops_step / (ms_per_step * 1e-3) / 1e12 / peak_tf}
 
     # ---- e2e: the HOST-buffer entry point, copies inside the timed region
     e2e = None
