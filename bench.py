@@ -32,7 +32,7 @@ METRIC = "DtN RHS-columns/sec at N=2048 (fp64)"
 UNIT = "columns/s"
 N_METRIC, NRHS_METRIC, NRHS_DD = 2048, 512, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (None = not captured yet)
-TRAFFIC_NCU = {"lu": None, "gemm_dmma": None}
+TRAFFIC_NCU = {"lu": None, "trsm": None, "gemm_dmma": None}
 NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # blackwell_cuda_programming.md: B200 FP64 tensor 45 TFLOP/s, bf16 dense 2250 TFLOP/s
 
 
@@ -254,15 +254,17 @@ def main():
     kernels = {k: {"ms_per_step": v[0] / kp, "launches_per_step": v[1] / kp} for k, v in tm.items() if v[1]}
     # algorithmic FLOPs per step of the two contraction kernels
     flops = {"lu": (2.0 / 3.0) * N ** 3,                    # S2: k_lu_dataflow
-             "gemm_dmma": 4.0 * N * N * (nrhs + 2)}         # S4 + S6: triangular solves and G product, nrhs columns + 2 base-state solves
-    flops_step = flops["lu"] + flops["gemm_dmma"]
+             "trsm": 2.0 * N * N * (nrhs + 2),              # S4: k_trsm_dataflow, nrhs columns + 2 base-state solves
+             "gemm_dmma": 2.0 * N * N * nrhs}               # S6: G product
+    flops_step = sum(flops.values())
     peaks = measured_peaks()
     peak_tf = peaks["bf16_tflops"] * NOMINAL_FP64_OVER_BF16
     probe = {"dfma_tflops": sww.probe_fp64_peak(0) / 1e12, "dmma_tflops": sww.probe_fp64_peak(1) / 1e12}
     names = {"lu": "k_lu_dataflow (persistent DMMA.8x8x4 tile dataflow, one launch)",
-             "gemm_dmma": "k_gemm_f64 (DMMA.8x8x4), all launches of one step"}
+             "trsm": "k_trsm_dataflow (persistent DMMA.8x8x4 multi-RHS triangular solves: 2 base-state launches + 1 batch launch)",
+             "gemm_dmma": "k_gemm_f64 (DMMA.8x8x4): G product"}
     per_kernel = {}
-    for cls in ("lu", "gemm_dmma"):
+    for cls in ("lu", "trsm", "gemm_dmma"):
         ms_c, n_c = tm[cls][0] / kp, tm[cls][1] / kp
         ach = flops[cls] / (ms_c * 1e-3) / 1e12 if ms_c > 0 else 0.0
         per_kernel[cls] = {"kernel": names[cls], "achieved": ach, "frac": ach / peak_tf, "flops_per_step": flops[cls],

@@ -24,7 +24,7 @@ int note_cuda(cudaError_t e, const char* where);
     } while (0)
 // Per-kernel-class device timing (sww_timing_enable / sww_timing_read): when enabled, SWW_BEGIN / SWW_LAUNCHED bracket every
 // launch with a CUDA event pair on the launching stream; off by default (no events, no overhead beyond a branch).
-enum KClass { KC_ASM = 0, KC_LU = 1, KC_GEMM = 2, KC_FFT = 3, KC_DDGEMM = 4, KC_OTHER = 5, KC_COUNT = 6 };
+enum KClass { KC_ASM = 0, KC_LU = 1, KC_GEMM = 2, KC_FFT = 3, KC_DDGEMM = 4, KC_OTHER = 5, KC_TRSM = 6, KC_COUNT = 7 };
 extern bool g_timing;
 void timing_begin(int cls, cudaStream_t st);
 void timing_end();
@@ -80,6 +80,8 @@ struct sww_dtn_s {
     int* lu_order;        // dataflow LU (lu.cu): task order, tile flags (+ the claim counter in slot 0), epoch of the last run
     unsigned* lu_flags;
     unsigned lu_epoch;
+    unsigned* tr_flags;   // dataflow TRSM: claim counter (slot 0) + flags[2][N/64][slabs]
+    unsigned tr_epoch;
     unsigned long long* lu_trace;  // debugging aid (env SWW_LU_TRACE): per-task time stamps of the dataflow LU
     // base state (dd planar 2N each): phi0', W0, u, v
     double *bphi, *bW0, *bu, *bv;

@@ -28,6 +28,7 @@
 namespace sww {
 
 constexpr double PIVOT_GUARD = 1e-3;
+constexpr int TR_MAXNS = 256;  // column slabs per TRSM launch (more columns: several launches)
 constexpr int TS = 64;    // tile size
 constexpr int LDT = 65;   // leading dimension of the row-major work tiles T, Eb, Fb (element (r,c) at r*LDT + c)
 constexpr int LDO = 68;   // leading dimension of the DMMA operand tiles (conflict-free fragment loads)
@@ -384,6 +385,8 @@ int lu_alloc(sww_dtn_s* d) {
     d->lu_flags = nullptr;
     d->lu_epoch = 0;
     d->lu_trace = nullptr;
+    d->tr_flags = nullptr;
+    d->tr_epoch = 0;
     if (N <= TS) return SWW_OK;
     const int nt = N / TS;
     std::vector<int> o;
@@ -392,6 +395,8 @@ int lu_alloc(sww_dtn_s* d) {
     if (cudaMalloc(&d->lu_flags, sizeof(unsigned) * ((size_t)nt * nt + 1)) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaMemcpyAsync(d->lu_order, o.data(), sizeof(int) * o.size(), cudaMemcpyHostToDevice, d->stream));
     SWW_CUDA(cudaMemsetAsync(d->lu_flags, 0, sizeof(unsigned) * ((size_t)nt * nt + 1), d->stream));
+    if (cudaMalloc(&d->tr_flags, sizeof(unsigned) * (2 * (size_t)nt * TR_MAXNS + 1)) != cudaSuccess) return SWW_ENOMEM;
+    SWW_CUDA(cudaMemsetAsync(d->tr_flags, 0, sizeof(unsigned) * (2 * (size_t)nt * TR_MAXNS + 1), d->stream));
     if (getenv("SWW_LU_TRACE") && cudaMalloc(&d->lu_trace, sizeof(unsigned long long) * 4 * (size_t)nt * nt) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaStreamSynchronize(d->stream));  // o goes out of scope
     return SWW_OK;
@@ -480,41 +485,255 @@ __global__ void __launch_bounds__(64) k_solve_small(int N, const double* __restr
     }
 }
 
-// Solve (LU) X = B for ncols columns, in place.  Forward then backward, right-looking by 64-row blocks:
-//   Y_kb = B_kb + E_kb B_kb ;  B_below -= L_below,kb Y_kb     then     X_kb = 2 Y_kb + F_kb Y_kb ;  Y_above -= U_above,kb X_kb.
-// The O(1) vectors are carried as hi + lo (B + Blo) through every accumulation (gemm.cu, compensated epilogue).
+// ------------------------------------------------------------------------------------------------ the persistent dataflow TRSM
+// Solve L Y = B, then U X = Y, for a batch of columns, in place, as ONE persistent kernel in the style of k_lu_dataflow.
+// A task is (phase, row block i, column slab s of WS columns).  Forward:  Y_i = (I + E_i)(B_i - sum_{k<i} L_ik Y_k);
+// backward:  X_i = (2 I + F_i)(Y_i - sum_{k>i} U_ik X_k).  The sums run left-looking in DMMA fragments over the blocks that are
+// already final (acquire-polled flags per (phase, k, s)); the chain of a slab is sequential in i, different slabs and the
+// accumulation over old blocks run in parallel.  Tasks are claimed in dependency order (forward i ascending, then backward i
+// descending), so a claimed task only waits for tasks claimed earlier.
+// Accuracy: the O(1) vectors are carried as hi + lo (B + Blo).  P = sum L_ik Y_k is accumulated from zero (its terms are
+// O(1/N)) and folded into a two-sum (hi, lo) pair every TR_FOLD blocks; B_i - P and the diagonal-block products are added by
+// error-free two-sums, so each block of the result is the correctly rounded sum plus a remainder word -- the density is
+// differentiated afterwards, which amplifies white rounding noise by ~N/3.
+struct TrsmArgs {
+    const double* A;     // LU factors, N x N column-major (L multipliers below the diagonal, U above)
+    const double *Es, *Fs;
+    double *B, *Blo;     // N x (ns*WS) column-major, ld = N; in: right-hand sides (Blo ignored), out: solution hi, lo
+    int N, nt, ns;       // nt row blocks of 64, ns column slabs
+    unsigned* flags;     // [2][nt][ns]
+    unsigned epoch;
+    unsigned* counter;
+};
+constexpr int TR_FOLD = 4;
+
+__device__ __forceinline__ void two_sum_d(double a, double b, double& s, double& e) {
+    s = __dadd_rn(a, b);
+    const double bb = __dsub_rn(s, a);
+    e = __dadd_rn(__dsub_rn(a, __dsub_rn(s, bb)), __dsub_rn(b, bb));
+}
+
+template <int WS>
+struct TrsmCfg {
+    static constexpr int WC = (WS >= 32) ? 4 : 1;   // warps across the slab's columns (8 columns per warp)
+    static constexpr int WR = 8 / WC;               // warps across the 64 rows
+    static constexpr int FM = (TS / WR) / 8;        // 8 x 8 fragments per warp along the rows
+    static constexpr int WSP = WC * 8;              // columns covered = WS
+    static constexpr int SMEM = (2 * TS * LDO + 2 * WS * LDO) * (int)sizeof(double) + 256;
+};
+
+template <int WS>
+__global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
+    using C = TrsmCfg<WS>;
+    extern __shared__ __align__(16) double tr_sm[];
+    double* sA = tr_sm;                    // 2 stages of the factor tile as As[k][r]
+    double* sB = sA + 2 * TS * LDO;        // 2 stages of the solution tile as Bs[n][k]
+    unsigned char* ready = reinterpret_cast<unsigned char*>(sB + 2 * WS * LDO);
+    __shared__ int s_task;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int wr = warp % C::WR, wc = warp / C::WR, fr = lane >> 2, fk = lane & 3;
+    const int N = p.N, nt = p.nt, ns = p.ns;
+    const unsigned epoch = p.epoch;
+    const int row0 = wr * (TS / C::WR) + fr;   // + 8 x : row of this lane's fragment element
+    const int col0 = wc * 8 + 2 * fk;          // + e   : column within the slab
+
+    for (;;) {
+        __syncthreads();
+        if (tid == 0) s_task = (int)atomicAdd(p.counter, 1u);
+        __syncthreads();
+        int task = s_task;
+        if (task >= 2 * nt * ns) break;
+        const int phase = task >= nt * ns;
+        if (phase) task -= nt * ns;
+        const int s = task % ns, i = phase ? nt - 1 - task / ns : task / ns;
+        const int m = phase ? nt - 1 - i : i;  // number of finished blocks this one depends on
+        const unsigned* fl = p.flags + (size_t)phase * nt * ns;
+        double* Bg = p.B + (size_t)s * WS * N + (size_t)i * TS;
+        double* Lg = p.Blo + (size_t)s * WS * N + (size_t)i * TS;
+        auto kblock = [&](int kk) { return phase ? nt - 1 - kk : kk; };
+
+        auto refresh = [&]() {
+            for (int t = tid; t < m; t += 256) ready[t] = ld_acquire(fl + (size_t)kblock(t) * ns + s) == epoch;
+        };
+        auto wait_ready = [&](int kk) {
+            if (!ready[kk]) {
+                if (tid == 0)
+                    while (ld_acquire(fl + (size_t)kblock(kk) * ns + s) != epoch) __nanosleep(40);
+                __syncthreads();
+                refresh();
+                __syncthreads();
+            }
+        };
+        auto issue = [&](int kk, int buf) {
+            const int k = kblock(kk);
+            const double* Ag = p.A + (size_t)k * TS * N + (size_t)i * TS;          // factor tile (i, k)
+            const double* Yg = p.B + (size_t)s * WS * N + (size_t)k * TS;          // solution block k of this slab
+            double* a = sA + buf * TS * LDO;
+            double* b = sB + buf * WS * LDO;
+            for (int c = tid; c < TS * TS / 2; c += 256) {
+                const int col = c >> 5, ch = (c & 31) * 2;
+                cp16(a + col * LDO + ch, Ag + (size_t)col * N + ch);
+            }
+            for (int c = tid; c < WS * TS / 2; c += 256) {
+                const int col = c >> 5, ch = (c & 31) * 2;
+                cp16(b + col * LDO + ch, Yg + (size_t)col * N + ch);
+            }
+            cp_commit();
+        };
+        double acc[C::FM][2];
+        auto mma_tile = [&](const double* a, const double* b) {
+            const double* as = a + row0;
+            const double* bs = b + (wc * 8 + fr) * LDO;
+#pragma unroll
+            for (int k4 = 0; k4 < TS; k4 += 4) {
+                const double bf = bs[k4 + fk];
+#pragma unroll
+                for (int x = 0; x < C::FM; x++) lu_dmma884(acc[x][0], acc[x][1], as[(k4 + fk) * LDO + x * 8], bf);
+            }
+        };
+
+        if (phase) {  // the block's own forward result must be visible before it is read
+            if (tid == 0)
+                while (ld_acquire(p.flags + (size_t)i * ns + s) != epoch) __nanosleep(40);
+            __syncthreads();
+        }
+        double bh[C::FM][2], bl[C::FM][2], ph[C::FM][2], pl[C::FM][2];
+#pragma unroll
+        for (int x = 0; x < C::FM; x++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
+                bh[x][e] = Bg[o];
+                bl[x][e] = phase ? Lg[o] : 0.0;  // the forward sweep starts from plain fp64 right-hand sides
+                acc[x][e] = ph[x][e] = pl[x][e] = 0.0;
+            }
+        auto fold = [&]() {  // (ph, pl) += acc, error-free; acc = 0
+#pragma unroll
+            for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    double s_, e_;
+                    two_sum_d(ph[x][e], acc[x][e], s_, e_);
+                    ph[x][e] = s_;
+                    pl[x][e] += e_;
+                    acc[x][e] = 0.0;
+                }
+        };
+        refresh();
+        __syncthreads();
+        if (m > 0) {
+            wait_ready(0);
+            issue(0, 0);
+        }
+        for (int kk = 0; kk < m; kk++) {
+            const bool pre = (kk + 1 < m) && ready[kk + 1];
+            if (pre) {
+                issue(kk + 1, (kk + 1) & 1);
+                cp_wait<1>();
+            } else {
+                cp_wait<0>();
+            }
+            __syncthreads();
+            mma_tile(sA + (kk & 1) * TS * LDO, sB + (kk & 1) * WS * LDO);
+            if ((kk % TR_FOLD) == TR_FOLD - 1) fold();
+            __syncthreads();
+            if (!pre && kk + 1 < m) {
+                wait_ready(kk + 1);
+                issue(kk + 1, (kk + 1) & 1);
+            }
+        }
+        fold();
+        // z = (bh + bl) - (ph + pl) as sh + sl ; then the diagonal block: forward y = z + E z, backward x = 2 z + F z
+        const double* Dg = (phase ? p.Fs : p.Es) + (size_t)i * TS * TS;
+        for (int c = tid; c < TS * TS / 2; c += 256) {
+            const int col = c >> 5, ch = (c & 31) * 2;
+            cp16(sA + col * LDO + ch, Dg + col * TS + ch);  // As[k][r] = D[r][k]
+        }
+        cp_commit();
+        double sh[C::FM][2], sl[C::FM][2];
+#pragma unroll
+        for (int x = 0; x < C::FM; x++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                double s_, e_;
+                two_sum_d(bh[x][e], -ph[x][e], s_, e_);
+                sh[x][e] = s_;
+                sl[x][e] = e_ + (bl[x][e] - pl[x][e]);
+                sB[(col0 + e) * LDO + row0 + x * 8] = s_;  // Bs[n][k] = z[k][n]
+                acc[x][e] = 0.0;
+            }
+        cp_wait<0>();
+        __syncthreads();
+        mma_tile(sA, sB);
+        const double sc = phase ? 2.0 : 1.0;
+#pragma unroll
+        for (int x = 0; x < C::FM; x++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
+                double t_, e_;
+                two_sum_d(sc * sh[x][e], acc[x][e], t_, e_);
+                const double lo = fma(sc, sl[x][e], e_);
+                const double hi = __dadd_rn(t_, lo);
+                Bg[o] = hi;
+                Lg[o] = __dsub_rn(lo, __dsub_rn(hi, t_));
+            }
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            st_release(p.flags + ((size_t)phase * nt + i) * ns + s, epoch);
+        }
+    }
+}
+
+template <int WS>
+static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
+    using C = TrsmCfg<WS>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        SWW_CUDA(cudaFuncSetAttribute(k_trsm_dataflow<WS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
+        attr_set = true;
+    }
+    const int N = d->N, nt = N / TS;
+    TrsmArgs a;
+    a.A = d->LU;
+    a.Es = d->invD;
+    a.Fs = d->invD + (size_t)nt * TS * TS;
+    a.B = B;
+    a.Blo = Blo;
+    a.N = N;
+    a.nt = nt;
+    a.ns = ns;
+    a.counter = d->tr_flags;
+    a.flags = d->tr_flags + 1;
+    a.epoch = ++d->tr_epoch;
+    SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), d->stream));
+    const int grid = std::min(sm_count(), 2 * nt * ns);
+    SWW_BEGIN(KC_TRSM, d->stream);
+    k_trsm_dataflow<WS><<<grid, 256, C::SMEM, d->stream>>>(a);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+// Solve (LU) X = B for ncols columns, in place; B and Blo are N x (ncols rounded up to the slab width) buffers (the padding
+// columns are solved too and ignored).  On return B + Blo is the solution (B = its fp64 rounding).
 int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
     const int N = d->N, nb = (N < NB) ? N : NB, nblk = N / nb;
     cudaStream_t st = d->stream;
-    const double* A = d->LU;
-    const double* Es = d->invD;
-    const double* Fs = d->invD + (size_t)nblk * nb * nb;
     if (nblk == 1) {
+        const double* Es = d->invD;
+        const double* Fs = d->invD + (size_t)nblk * nb * nb;
         SWW_BEGIN(KC_GEMM, st);
         k_solve_small<<<ncols, 64, 0, st>>>(N, Es, Fs, B, Blo);
         SWW_LAUNCHED();
         SWW_CUDA(cudaGetLastError());
         return SWW_OK;
     }
-    for (int kb = 0; kb < nblk; kb++) {
-        const int k0 = kb * nb, rem = N - k0 - nb;
-        double* Bk = B + k0;
-        Epi e1{Blo + k0, kb == 0 ? 2 : 1, 1};
-        SWW_TRY(gemm_f64(st, nb, ncols, nb, 1.0, Es + (size_t)kb * nb * nb, nb, Bk, N, 1.0, Bk, N, ncols, e1));
-        if (rem > 0) {
-            Epi e2{Blo + k0 + nb, kb == 0 ? 2 : 1, 0};
-            SWW_TRY(gemm_f64(st, rem, ncols, nb, -1.0, A + (size_t)k0 * N + k0 + nb, N, Bk, N, 1.0, Bk + nb, N, ncols, e2));
-        }
-    }
-    for (int kb = nblk - 1; kb >= 0; kb--) {
-        const int k0 = kb * nb;
-        double* Bk = B + k0;
-        Epi e1{Blo + k0, 1, 1};
-        SWW_TRY(gemm_f64(st, nb, ncols, nb, 1.0, Fs + (size_t)kb * nb * nb, nb, Bk, N, 2.0, Bk, N, ncols, e1));
-        if (k0 > 0) {
-            Epi e2{Blo, 1, 0};
-            SWW_TRY(gemm_f64(st, k0, ncols, nb, -1.0, A + (size_t)k0 * N, N, Bk, N, 1.0, B, N, ncols, e2));
-        }
+    if (ncols <= 8) return launch_trsm<8>(d, B, Blo, 1);
+    for (int c0 = 0; c0 < ncols; c0 += TR_MAXNS * 32) {
+        const int nc = std::min(ncols - c0, TR_MAXNS * 32);
+        SWW_TRY(launch_trsm<32>(d, B + (size_t)c0 * N, Blo + (size_t)c0 * N, (nc + 31) / 32));
     }
     return SWW_OK;
 }
