@@ -8,54 +8,10 @@
 // Twiddles exp(-2 pi i m/N) come from the dd-accurate table rounded to fp64 (tables.cu).
 // Product code; shares nothing with oracle/.
 #include "common.cuh"
+#include "fft.cuh"
 
 namespace sww {
 
-__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
-    return make_double2(fma(a.x, b.x, -a.y * b.y), fma(a.x, b.y, a.y * b.x));
-}
-__device__ __forceinline__ double2 cmulc(double2 a, double2 b) {  // a * conj(b)
-    return make_double2(fma(a.x, b.x, a.y * b.y), fma(a.y, b.x, -a.x * b.y));
-}
-
-// in-place forward DIF FFT of z[0..N) in shared memory; output in bit-reversed order
-__device__ void fft_dif(double2* z, int N, const double2* __restrict__ tw) {
-    for (int half = N >> 1; half >= 1; half >>= 1) {
-        int tstride = N / (2 * half);
-        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
-            int blk = t / half, o = t - blk * half;
-            int i = blk * 2 * half + o;
-            double2 a = z[i], b = z[i + half];
-            double2 w = tw[o * tstride];
-            z[i] = make_double2(a.x + b.x, a.y + b.y);
-            z[i + half] = cmul(make_double2(a.x - b.x, a.y - b.y), w);
-        }
-        __syncthreads();
-    }
-}
-// in-place inverse DIT FFT (input bit-reversed, output natural), unscaled
-__device__ void ifft_dit(double2* z, int N, const double2* __restrict__ tw) {
-    for (int half = 1; half < N; half <<= 1) {
-        int tstride = N / (2 * half);
-        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
-            int blk = t / half, o = t - blk * half;
-            int i = blk * 2 * half + o;
-            double2 a = z[i];
-            double2 b = cmulc(z[i + half], tw[o * tstride]);
-            z[i] = make_double2(a.x + b.x, a.y + b.y);
-            z[i + half] = make_double2(a.x - b.x, a.y - b.y);
-        }
-        __syncthreads();
-    }
-}
-// signed wavenumber of bit-reversed position p (Nyquist -> 0: every multiplier here vanishes there, R4)
-__device__ __forceinline__ int wavenumber(int p, int N, int logN) {
-    int k = (int)(__brev((unsigned)p) >> (32 - logN));
-    if (2 * k == N) return 0;
-    return (2 * k < N) ? k : k - N;
-}
-
-constexpr int FFT_MAX_PER_THREAD = 8;  // ceil(N / blockDim.x) <= 8
 
 // Gam_c = D M_c ;  W_c = |D| M_c / 2 - (T ? D T_c : 0)     for the column pair (2*blockIdx.x, 2*blockIdx.x + 1)
 __global__ void __launch_bounds__(1024) k_spectral_gamma_w(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ M,
@@ -143,18 +99,6 @@ __global__ void __launch_bounds__(1024) k_spectral_deriv(int N, int logN, const 
     }
 }
 
-static int ilog2(int n) {
-    int l = 0;
-    while ((1 << l) < n) l++;
-    return l;
-}
-static int fft_threads(int N) {
-    int t = N / 2;
-    if (t > 1024) t = 1024;
-    if (t < 32) t = 32;
-    return t;
-}
-
 int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols) {
     const int N = d->N;
     size_t smem = sizeof(double2) * (size_t)N;
@@ -165,7 +109,7 @@ int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam
         attr_set = true;
     }
     SWW_BEGIN(KC_FFT, d->stream);
-    k_spectral_gamma_w<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, ilog2(N), d->tab->tw, M, T, Gam, W, ncols, w_cols);
+    k_spectral_gamma_w<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, fft_ilog2(N), d->tab->tw, M, T, Gam, W, ncols, w_cols);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -180,7 +124,7 @@ int spectral_deriv(sww_dtn_s* d, const double* in, double* out, int ncols) {
         attr_set = true;
     }
     SWW_BEGIN(KC_FFT, d->stream);
-    k_spectral_deriv<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, ilog2(N), d->tab->tw, in, out, ncols);
+    k_spectral_deriv<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, fft_ilog2(N), d->tab->tw, in, out, ncols);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

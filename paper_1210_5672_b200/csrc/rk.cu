@@ -1,9 +1,384 @@
-// rk.cu -- time stepper (placeholder until the RK kernels land; returns SWW_EINVAL)
+// rk.cu -- S8/S9: right-hand sides of the free-surface Euler equations (2.1) and of the batched variational
+// equation (B.1)-(B.3), (3.32), the 36th-order filter (2.14), and the explicit
+// 11-stage order-8 Runge-Kutta stepper (reading R6 of DESIGN.md section 3: the paper cites DOP853 without printing it).
+//
+//   eta_t   = W0                         phi_t   = P[ v W0 - u^2/2 - v^2/2 - g eta ]
+//   deta_t  = w_c - D(u deta_c)          dphi_t  = P[ -D(deta_c u v) - u D(b_c) + v w_c - g deta_c ],  b_c = dphi_c - v deta_c,
+//   w_c = G[b_c],  every right-hand side multiplied by the filter, the state filtered after every step (R5).
+// One DtN setup (S0-S2), one base state and one batched linearized solve per stage, all through the entry points of api.cu.
+// State layout: y = [eta (N) | phi (N) | deta (N x nc) | dphi (N x nc)], fp64.  Product code; shares nothing with oracle/.
 #include "common.cuh"
-extern "C" {
-int sww_state_create(int, double, double, int, int, const void*, const void*, const void*, const void*, unsigned, void*, sww_state_t*) { return SWW_EINVAL; }
-int sww_rk_advance(sww_state_t, double, int) { return SWW_EINVAL; }
-int sww_state_read(sww_state_t, void*, void*, void*, void*, double*) { return SWW_EINVAL; }
-int sww_state_energy(sww_state_t, double*) { return SWW_EINVAL; }
-int sww_state_destroy(sww_state_t) { return SWW_EINVAL; }
+#include "fft.cuh"
+#include <new>
+#include <cstring>
+
+using namespace sww;
+
+constexpr int RK_S = 11;
+
+struct sww_state_s {
+    int N, nc, prec;
+    double h, g;
+    bool filter;
+    cudaStream_t stream;
+    sww_dtn_t dtn;
+    size_t L;            // 2 N (1 + nc)
+    double* y;           // state
+    double* ys;          // stage state
+    double* k;           // RK_S stage derivatives, L each
+    double* w;           // N x nc: unfiltered deta_t of the current stage
+    double* red;         // 1 double: energy reduction
+    double t;
+    double a[RK_S][RK_S], b[RK_S], c[RK_S];
+};
+
+namespace sww {
+
+// the tableau of DESIGN.md section 3 (R6): coefficients in Q(sqrt 21), evaluated in double
+static void rk_tableau(double a[RK_S][RK_S], double b[RK_S], double c[RK_S]) {
+    const double s = sqrt(21.0);
+    memset(a, 0, sizeof(double) * RK_S * RK_S);
+    memset(b, 0, sizeof(double) * RK_S);
+    const double cv[RK_S] = {0.0, 0.5, 0.5, (7 + s) / 14, (7 + s) / 14, 0.5, (7 - s) / 14, (7 - s) / 14, 0.5, (7 + s) / 14, 1.0};
+    memcpy(c, cv, sizeof(cv));
+    b[0] = 1.0 / 20; b[7] = 49.0 / 180; b[8] = 16.0 / 45; b[9] = 49.0 / 180; b[10] = 1.0 / 20;
+    a[1][0] = 0.5;
+    a[2][0] = 0.25; a[2][1] = 0.25;
+    a[3][0] = 1.0 / 7; a[3][1] = (-7 - 3 * s) / 98; a[3][2] = (21 + 5 * s) / 49;
+    a[4][0] = (11 + s) / 84; a[4][2] = (18 + 4 * s) / 63; a[4][3] = (21 - s) / 252;
+    a[5][0] = (5 + s) / 48; a[5][2] = (9 + s) / 36; a[5][3] = (-231 + 14 * s) / 360; a[5][4] = (63 - 7 * s) / 80;
+    a[6][0] = (10 - s) / 42; a[6][2] = (-432 + 92 * s) / 315; a[6][3] = (633 - 145 * s) / 90; a[6][4] = (-504 + 115 * s) / 70; a[6][5] = (63 - 13 * s) / 35;
+    a[7][0] = 1.0 / 14; a[7][4] = (14 - 3 * s) / 126; a[7][5] = (13 - 3 * s) / 63; a[7][6] = 1.0 / 9;
+    a[8][0] = 1.0 / 32; a[8][4] = (91 - 21 * s) / 576; a[8][5] = 11.0 / 72; a[8][6] = (-385 - 75 * s) / 1152; a[8][7] = (63 + 13 * s) / 128;
+    a[9][0] = 1.0 / 14; a[9][4] = 1.0 / 9; a[9][5] = (-733 - 147 * s) / 2205; a[9][6] = (515 + 111 * s) / 504; a[9][7] = (-51 - 11 * s) / 56; a[9][8] = (132 + 28 * s) / 245;
+    a[10][4] = (-42 + 7 * s) / 18; a[10][5] = (-18 + 28 * s) / 45; a[10][6] = (-273 - 53 * s) / 72; a[10][7] = (301 + 53 * s) / 72; a[10][8] = (28 - 28 * s) / 45; a[10][9] = (49 - 7 * s) / 18;
 }
+
+// S9: out = y + sum_j coef[j] k_j   (coef = dt a_ij or dt b_j; zero coefficients are skipped on the host side)
+struct Comb {
+    int n;
+    int idx[RK_S];
+    double coef[RK_S];
+};
+__global__ void k_rk_combine(size_t L, const double* __restrict__ y, const double* __restrict__ k, Comb cb, double* __restrict__ out) {
+    size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= L) return;
+    double s = y[q];
+    for (int j = 0; j < cb.n; j++) s = fma(cb.coef[j], k[(size_t)cb.idx[j] * L + q], s);
+    out[q] = s;
+}
+
+__device__ __forceinline__ int dft_index(int p, int logN) { return (int)(__brev((unsigned)p) >> (32 - logN)); }
+
+// S8, base state: eta_t = F[W0], phi_t = F P[v W0 - u^2/2 - v^2/2 - g eta]   (2.1), one CTA; F = filter (or identity), P = zero mean
+__global__ void __launch_bounds__(1024) k_rhs_base(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                   int filter_on, double g, const double* __restrict__ eta, const double* __restrict__ W0,
+                                                   const double* __restrict__ u, const double* __restrict__ v, double* __restrict__ eta_t,
+                                                   double* __restrict__ phi_t) {
+    extern __shared__ __align__(16) double2 z[];
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double w = W0[j], uu = u[j], vv = v[j];
+        z[j] = make_double2(w, fma(vv, w, -0.5 * uu * uu) - 0.5 * vv * vv - g * eta[j]);
+    }
+    __syncthreads();
+    fft_dif(z, N, tw);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double f = (filter_on ? filt[dft_index(p, logN)] : 1.0) * rN;
+        double2 t = z[p];
+        t.x *= f;
+        t.y = (p == 0) ? 0.0 : t.y * f;  // P: the mean of phi_t is removed (2.2)
+        z[p] = t;
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        eta_t[j] = z[j].x;
+        phi_t[j] = z[j].y;
+    }
+}
+
+// S8, variational columns (B.1)-(B.3): one CTA per column pair.  wout = w_c - D(u deta_c) is the linearized DtN (api.cu).
+//   deta_t = F[wout] ;  dphi_t = F P[ -D(deta u v) - u D(b) + v w - g deta ],  w = wout + D(u deta),  b = dphi - v deta
+__global__ void __launch_bounds__(1024) k_rhs_cols(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                   int filter_on, double g, int ncols, const double* __restrict__ u, const double* __restrict__ v,
+                                                   const double* __restrict__ deta, const double* __restrict__ dphi, const double* __restrict__ wout,
+                                                   double* __restrict__ deta_t, double* __restrict__ dphi_t) {
+    extern __shared__ __align__(16) double2 z[];
+    double2* z2 = z + N;
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const size_t o0 = (size_t)c0 * N, o1 = (size_t)c1 * N;
+    const double rN = 1.0 / (double)N;
+    auto deriv_inplace = [&]() {  // z <- D z (natural order in and out)
+        __syncthreads();
+        fft_dif(z, N, tw);
+        for (int p = threadIdx.x; p < N; p += blockDim.x) {
+            const double k = (double)wavenumber(p, N, logN) * rN;
+            const double2 t = z[p];
+            z[p] = make_double2(-k * t.y, k * t.x);
+        }
+        __syncthreads();
+        ifft_dit(z, N, tw);
+    };
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double uu = u[j];
+        z[j] = make_double2(uu * deta[o0 + j], has1 ? uu * deta[o1 + j] : 0.0);
+    }
+    deriv_inplace();  // z = D(u deta)
+    double2 wv[FFT_MAX_PER_THREAD];
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) wv[r] = make_double2(wout[o0 + j] + z[j].x, has1 ? wout[o1 + j] + z[j].y : 0.0);
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double vv = v[j];
+        z[j] = make_double2(fma(-vv, deta[o0 + j], dphi[o0 + j]), has1 ? fma(-vv, deta[o1 + j], dphi[o1 + j]) : 0.0);
+    }
+    deriv_inplace();  // z = D(b)
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) {
+            const double uu = u[j], vv = v[j];
+            const double2 a3 = z[j];
+            const double d0 = deta[o0 + j], d1 = has1 ? deta[o1 + j] : 0.0;
+            z[j] = make_double2(fma(vv, wv[r].x, -uu * a3.x) - g * d0, fma(vv, wv[r].y, -uu * a3.y) - g * d1);
+        }
+    }
+    __syncthreads();
+    fft_dif(z, N, tw);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) z2[p] = z[p];
+    __syncthreads();
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double uv = u[j] * v[j];
+        z[j] = make_double2(uv * deta[o0 + j], has1 ? uv * deta[o1 + j] : 0.0);
+    }
+    __syncthreads();
+    fft_dif(z, N, tw);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber(p, N, logN);
+        const double f = (filter_on ? filt[dft_index(p, logN)] : 1.0) * rN;
+        const double2 q = z2[p], t = z[p];
+        z2[p] = (p == 0) ? make_double2(0.0, 0.0) : make_double2(f * fma(k, t.y, q.x), f * fma(-k, t.x, q.y));  // F P (q^ - i k t^)
+    }
+    __syncthreads();
+    ifft_dit(z2, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        dphi_t[o0 + j] = z2[j].x;
+        if (has1) dphi_t[o1 + j] = z2[j].y;
+        z[j] = make_double2(wout[o0 + j], has1 ? wout[o1 + j] : 0.0);
+    }
+    __syncthreads();
+    fft_dif(z, N, tw);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double f = (filter_on ? filt[dft_index(p, logN)] : 1.0) * rN;
+        z[p] = make_double2(f * z[p].x, f * z[p].y);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        deta_t[o0 + j] = z[j].x;
+        if (has1) deta_t[o1 + j] = z[j].y;
+    }
+}
+
+// the filter (2.14) applied in place to ncols columns (the state after every step)
+__global__ void __launch_bounds__(1024) k_filter_cols(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                      int ncols, double* __restrict__ y) {
+    extern __shared__ __align__(16) double2 z[];
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const size_t o0 = (size_t)c0 * N, o1 = (size_t)c1 * N;
+    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(y[o0 + j], has1 ? y[o1 + j] : 0.0);
+    __syncthreads();
+    fft_dif(z, N, tw);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double f = filt[dft_index(p, logN)] * rN;
+        z[p] = make_double2(f * z[p].x, f * z[p].y);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        y[o0 + j] = z[j].x;
+        if (has1) y[o1 + j] = z[j].y;
+    }
+}
+
+// E = (pi/N) sum_j [ phi_j (G phi)_j + g eta_j^2 ], one CTA, pairwise tree in shared memory
+__global__ void __launch_bounds__(256) k_energy(int N, double g, const double* __restrict__ eta, const double* __restrict__ phi,
+                                                const double* __restrict__ W0, double* __restrict__ out) {
+    __shared__ double s[256];
+    double a = 0.0;
+    for (int j = threadIdx.x; j < N; j += 256) a += fma(phi[j], W0[j], g * eta[j] * eta[j]);
+    s[threadIdx.x] = a;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) s[threadIdx.x] += s[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[0] = s[0] * 3.14159265358979323846 / (double)N;
+}
+
+}  // namespace sww
+
+namespace sww {
+
+static int rk_set_attrs() {
+    static bool done = false;
+    if (!done) {
+        SWW_CUDA(cudaFuncSetAttribute(k_rhs_base, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        SWW_CUDA(cudaFuncSetAttribute(k_rhs_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 4096 * 32));
+        SWW_CUDA(cudaFuncSetAttribute(k_filter_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        done = true;
+    }
+    return SWW_OK;
+}
+
+// one evaluation of the right-hand sides at the stage state ys -> kout (same layout as the state)
+static int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
+    const int N = s->N, nc = s->nc, logN = fft_ilog2(N), thr = fft_threads(N);
+    sww_dtn_s* d = s->dtn;
+    cudaStream_t st = s->stream;
+    const double* eta = ys;
+    const double* phi = ys + N;
+    SWW_TRY(sww_dtn_refactor(d, eta));   // S0-S2 for this stage's surface
+    SWW_TRY(sww_dtn_set_base(d, phi));   // W0 = G phi, u, v of (2.9)
+    const Tables* t = d->tab;
+    SWW_BEGIN(KC_FFT, st);
+    k_rhs_base<<<1, thr, sizeof(double2) * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->g, eta, d->bW0, d->bu, d->bv, kout,
+                                                              kout + N);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    if (nc > 0) {
+        const double* deta = ys + 2 * (size_t)N;
+        const double* dphi = deta + (size_t)N * nc;
+        SWW_TRY(sww_dtn_linearized_apply(d, deta, dphi, nc, s->w));  // w_c - D(u deta_c)   (B.1d), (B.2)
+        SWW_BEGIN(KC_FFT, st);
+        k_rhs_cols<<<(nc + 1) / 2, thr, sizeof(double2) * 2 * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->g, nc, d->bu, d->bv,
+                                                                                deta, dphi, s->w, kout + 2 * (size_t)N,
+                                                                                kout + 2 * (size_t)N + (size_t)N * nc);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+    }
+    return SWW_OK;
+}
+
+static int rk_combine(sww_state_s* s, const double* coef, int n, double dt, double* out) {
+    Comb cb;
+    cb.n = 0;
+    for (int j = 0; j < n; j++)
+        if (coef[j] != 0.0) {
+            cb.idx[cb.n] = j;
+            cb.coef[cb.n] = dt * coef[j];
+            cb.n++;
+        }
+    SWW_BEGIN(KC_OTHER, s->stream);
+    k_rk_combine<<<(unsigned)((s->L + 255) / 256), 256, 0, s->stream>>>(s->L, s->y, s->k, cb, out);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+}  // namespace sww
+
+extern "C" {
+
+int sww_state_create(int N, double h, double g, int prec, int ncols, const void* eta, const void* phi, const void* deta,
+                     const void* dphi, unsigned flags, void* stream, sww_state_t* out) {
+    if (!out || !eta || !phi || ncols < 0 || (ncols > 0 && (!deta || !dphi))) return SWW_EINVAL;
+    if (prec != SWW_F64) return SWW_EINVAL;  // the double-double stepper is not built yet
+    if (N > 4096) return SWW_EINVAL;         // k_rhs_cols keeps two N-point complex arrays in shared memory
+    sww_state_s* s = new (std::nothrow) sww_state_s();
+    if (!s) return SWW_ENOMEM;
+    memset(s, 0, sizeof(*s));
+    s->N = N; s->nc = ncols; s->prec = prec; s->h = h; s->g = g;
+    s->filter = !(flags & 1u);
+    s->stream = (cudaStream_t)stream;
+    s->L = 2 * (size_t)N * (1 + (size_t)ncols);
+    rk_tableau(s->a, s->b, s->c);
+    int rc = sww_dtn_setup(eta, N, h, prec, stream, &s->dtn);  // validates N, h; also the first factorisation
+    if (rc) { delete s; return rc; }
+    bool ok = cudaMalloc(&s->y, sizeof(double) * s->L) == cudaSuccess && cudaMalloc(&s->ys, sizeof(double) * s->L) == cudaSuccess &&
+              cudaMalloc(&s->k, sizeof(double) * s->L * RK_S) == cudaSuccess &&
+              cudaMalloc(&s->w, sizeof(double) * (size_t)N * (ncols > 0 ? ncols : 1)) == cudaSuccess &&
+              cudaMalloc(&s->red, sizeof(double)) == cudaSuccess;
+    if (!ok) { sww_state_destroy(s); return SWW_ENOMEM; }
+    const size_t v = sizeof(double) * N, bsz = v * ncols;
+    cudaStream_t st = s->stream;
+    if (cudaMemcpyAsync(s->y, eta, v, cudaMemcpyDeviceToDevice, st) || cudaMemcpyAsync(s->y + N, phi, v, cudaMemcpyDeviceToDevice, st) ||
+        (ncols && (cudaMemcpyAsync(s->y + 2 * (size_t)N, deta, bsz, cudaMemcpyDeviceToDevice, st) ||
+                   cudaMemcpyAsync(s->y + 2 * (size_t)N + (size_t)N * ncols, dphi, bsz, cudaMemcpyDeviceToDevice, st)))) {
+        sww_state_destroy(s);
+        return SWW_ECUDA;
+    }
+    rc = rk_set_attrs();
+    if (rc) { sww_state_destroy(s); return rc; }
+    *out = s;
+    return SWW_OK;
+}
+
+int sww_rk_advance(sww_state_t s, double dt, int nsteps) {
+    if (!s || nsteps < 0) return SWW_EINVAL;
+    const int N = s->N, logN = fft_ilog2(N);
+    for (int n = 0; n < nsteps; n++) {
+        for (int i = 0; i < RK_S; i++) {
+            const double* ys = s->y;
+            if (i > 0) {
+                SWW_TRY(rk_combine(s, s->a[i], i, dt, s->ys));
+                ys = s->ys;
+            }
+            SWW_TRY(rk_rhs(s, ys, s->k + (size_t)i * s->L));
+        }
+        SWW_TRY(rk_combine(s, s->b, RK_S, dt, s->y));
+        if (s->filter) {
+            const int ncol = 2 + 2 * s->nc;
+            SWW_BEGIN(KC_FFT, s->stream);
+            k_filter_cols<<<(ncol + 1) / 2, fft_threads(N), sizeof(double2) * (size_t)N, s->stream>>>(N, logN, s->dtn->tab->tw, s->dtn->tab->filt,
+                                                                                                       ncol, s->y);
+            SWW_LAUNCHED();
+            SWW_CUDA(cudaGetLastError());
+        }
+        s->t += dt;
+    }
+    return SWW_OK;
+}
+
+int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, double* t) {
+    if (!s) return SWW_EINVAL;
+    const size_t v = sizeof(double) * s->N, bsz = v * s->nc;
+    cudaStream_t st = s->stream;
+    if (eta) SWW_CUDA(cudaMemcpyAsync(eta, s->y, v, cudaMemcpyDeviceToDevice, st));
+    if (phi) SWW_CUDA(cudaMemcpyAsync(phi, s->y + s->N, v, cudaMemcpyDeviceToDevice, st));
+    if (deta && s->nc) SWW_CUDA(cudaMemcpyAsync(deta, s->y + 2 * (size_t)s->N, bsz, cudaMemcpyDeviceToDevice, st));
+    if (dphi && s->nc) SWW_CUDA(cudaMemcpyAsync(dphi, s->y + 2 * (size_t)s->N + (size_t)s->N * s->nc, bsz, cudaMemcpyDeviceToDevice, st));
+    if (t) *t = s->t;
+    return sww_dtn_status(s->dtn);  // synchronises the stream
+}
+
+int sww_state_energy(sww_state_t s, double* energy_hl) {
+    if (!s || !energy_hl) return SWW_EINVAL;
+    sww_dtn_s* d = s->dtn;
+    SWW_TRY(sww_dtn_refactor(d, s->y));
+    SWW_TRY(sww_dtn_set_base(d, s->y + s->N));
+    SWW_BEGIN(KC_OTHER, s->stream);
+    k_energy<<<1, 256, 0, s->stream>>>(s->N, s->g, s->y, s->y + s->N, d->bW0, s->red);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    SWW_CUDA(cudaMemcpyAsync(energy_hl, s->red, sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+    energy_hl[1] = 0.0;
+    return sww_dtn_status(d);
+}
+
+int sww_state_destroy(sww_state_t s) {
+    if (!s) return SWW_EINVAL;
+    if (s->dtn) sww_dtn_destroy(s->dtn);
+    cudaFree(s->y); cudaFree(s->ys); cudaFree(s->k); cudaFree(s->w); cudaFree(s->red);
+    delete s;
+    return SWW_OK;
+}
+
+}  // extern "C"
