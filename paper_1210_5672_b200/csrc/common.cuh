@@ -81,6 +81,7 @@ struct sww_dtn_s {
     int* lu_order;        // dataflow LU (lu.cu): task order, tile flags (+ the claim counter in slot 0), epoch of the last run
     unsigned* lu_flags;
     unsigned lu_epoch;
+    int lu_ntasks;
     unsigned* tr_flags;   // dataflow TRSM: claim counter (slot 0) + flags[2][N/64][slabs]
     unsigned tr_epoch;
     unsigned long long* lu_trace;  // debugging aid (env SWW_LU_TRACE): per-task time stamps of the dataflow LU

@@ -175,17 +175,103 @@ __global__ void __launch_bounds__(256) k_lu_single(double* __restrict__ A, int n
     getrf64(T, vec, status, tid, A, (size_t)nb, Eout, Fout, nb, nb);
 }
 
+// ------------------------------------------------------------------------------------------------ 64 x 64 Gauss-Jordan inverse
+// In-place inversion of S = I/2 + kappa by 64 Gauss-Jordan steps, 256 threads, thread (ty, tx) of a 16 x 16 grid keeping the
+// 4 x 4 register tile rows ty + 16 q, columns tx + 16 b.  The diagonal is carried as a DEVIATION: kappa_jj = S_jj - 1/2 before
+// pivot j is processed, Z_jj - 2 afterwards (the update formulas never touch the nominal part), so the result is F = inv(S) - 2 I
+// with every entry accurate relative to its own size.  Per step the owners publish column j and row j in shared memory
+// (double-buffered: one barrier per step); the rest is 16 register FMAs per thread.  vec: 256 doubles.
+template <int JB>
+__device__ __forceinline__ void gj64_steps(double (&a)[4][4], double* vec, int* status, int tid) {
+    const int ty = tid & 15, tx = tid >> 4;
+#pragma unroll 1
+    for (int jt = 0; jt < 16; jt++) {
+        const int j = 16 * JB + jt;
+        double* colA = vec + (jt & 1) * 128;
+        double* rowA = colA + 64;
+        const bool pcol = (tx == jt), prow = (ty == jt);
+        if (pcol) {
+#pragma unroll
+            for (int q = 0; q < 4; q++) colA[ty + 16 * q] = a[q][JB];
+        }
+        if (prow) {
+#pragma unroll
+            for (int b = 0; b < 4; b++) rowA[tx + 16 * b] = a[JB][b];
+        }
+        __syncthreads();
+        const double dj = rowA[j];
+        const double piv = 0.5 + dj;
+        const double r = 1.0 / piv;
+        if (tid == 0 && !(fabs(piv) >= PIVOT_GUARD)) atomicCAS(status, SWW_OK, SWW_ESINGULAR);
+        double f[4], ut[4];
+#pragma unroll
+        for (int q = 0; q < 4; q++) f[q] = colA[ty + 16 * q];
+#pragma unroll
+        for (int b = 0; b < 4; b++) ut[b] = rowA[tx + 16 * b] * r;
+#pragma unroll
+        for (int q = 0; q < 4; q++)
+#pragma unroll
+            for (int b = 0; b < 4; b++) {
+                double v = fma(-f[q], ut[b], a[q][b]);
+                if (q == JB && prow) v = ut[b];                              // pivot row:    M(j,c) / p
+                if (b == JB && pcol) v = -f[q] * r;                          // pivot column: -M(i,j) / p
+                if (q == JB && b == JB && prow && pcol) v = -2.0 * dj * r;   // 1/p - 2 without cancellation
+                a[q][b] = v;
+            }
+    }
+}
+
+// T (row-major, LDT) holds kappa = S - I/2.  On return F = inv(S) - 2 I is in Fg (global, column-major, ld 64) and in Fs_sm
+// (shared, operand layout Bs[n][k] = F[k][n], ld LDO).  Every thread of the CTA must call it.
+__device__ __noinline__ void gj64(const double* T, double* vec, int* status, int tid, double* Fg, double* Fs_sm) {
+    const int ty = tid & 15, tx = tid >> 4;
+    double a[4][4];
+#pragma unroll
+    for (int q = 0; q < 4; q++)
+#pragma unroll
+        for (int b = 0; b < 4; b++) a[q][b] = T[(ty + 16 * q) * LDT + tx + 16 * b];
+    gj64_steps<0>(a, vec, status, tid);
+    gj64_steps<1>(a, vec, status, tid);
+    gj64_steps<2>(a, vec, status, tid);
+    gj64_steps<3>(a, vec, status, tid);
+#pragma unroll
+    for (int b = 0; b < 4; b++)
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const int row = ty + 16 * q, col = tx + 16 * b;
+            Fg[col * TS + row] = a[q][b];
+            Fs_sm[col * LDO + row] = a[q][b];
+        }
+}
+
 // ------------------------------------------------------------------------------------------------ the persistent dataflow LU
+// BLOCK LU without pivoting, 64 x 64 tiles:  A = L U  with identity diagonal blocks in L and the Schur complements S_m on the
+// block diagonal of U; what is stored is  L_im = X_im Z_m  (i > m),  U_mj = X_mj  (j > m)  and  F_m = Z_m - 2 I,  Z_m = inv(S_m),
+// where  X_ij = A_ij - sum_{k < min(i,j)} L_ik U_kj.  (Well posed: every S_m is I/2 plus a small block.)
+// The recurrence of the diagonal,  S_m = [A_mm - sum_{k<m-1} L_mk U_km] - (X_{m,m-1} Z_{m-1}) U_{m-1,m},  is the critical path.
+// It runs on ONE dedicated CTA (the "spine", block 0) with no flag hop inside a step: Gauss-Jordan inverse of S_{m-1}, then two
+// 64^3 DMMA products; everything it needs from outside (X_{m,m-1}, U_{m-1,m} and the partial sum P_m) depends on Z_{m-2} at the
+// latest, so it arrives while the spine inverts.  All other CTAs are workers claiming tile tasks in level order:
+//     U tile (i < j)   : X_ij, final as soon as the left-looking sum is done;
+//     L tile (i > j+1) : X_ij, then wait for Z_j and store L_ij = 2 X + X F_j;
+//     X tile (j+1, j)  : X only (the spine turns it into L_{j+1,j} on its way);
+//     P tile (m, m)    : the partial sum over k < m-1, in place.
+// A tile is published by a release store of the launch's epoch into its flag; consumers acquire-poll.  Tasks are claimed in
+// level order (level = min(i,j); P_{m+1}, whose inputs belong to levels < m, opens level m), so a claimed task waits only for tasks
+// claimed earlier or for the spine, and the spine waits only for tasks of earlier levels: no deadlock, no grid barrier.
 struct LuArgs {
     double* A;         // N x N column-major, in place
     int N, nt;         // nt = N / 64 tiles per side
-    const int* order;  // nt*nt tasks: (i << 16) | j in claim order
-    unsigned* flags;   // nt*nt: flags[i*nt + j] == epoch  <=>  tile (i,j) is final
+    int ntasks;
+    const int* order;  // worker tasks: (i << 16) | j in claim order
+    unsigned* flags;   // nt*nt: flags[i*nt + j] == epoch  <=>  tile (i,j) is final (i != j) / P_i is ready (i == j)
+    unsigned* xflags;  // nt: X_{m,m-1} is in place
+    unsigned* zflags;  // nt: F_m is in Fs
     unsigned epoch;
     unsigned* counter;  // next task to claim (zeroed before the launch)
-    double *Es, *Fs;   // nt blocks of 64 x 64 (column-major, ld 64): inv(L_kk) - I, inv(U_kk) - 2 I
+    double* Fs;        // nt blocks of 64 x 64 (column-major, ld 64): inv(S_m) - 2 I
     int* status;
-    unsigned long long* trace;  // optional: 4 globaltimer stamps per task (claimed, operands done, finalised, published)
+    unsigned long long* trace;  // optional: 4 globaltimer stamps per worker task, then 4 per spine step
 };
 
 __device__ __forceinline__ unsigned long long gtime() {
@@ -194,18 +280,142 @@ __device__ __forceinline__ unsigned long long gtime() {
     return t;
 }
 
-constexpr int LU_SMEM_BYTES = (4 * TS * LDO + TS * LDT + 576) * (int)sizeof(double) + 256;
+constexpr int LU_SMEM_BYTES = (4 * TS * LDO + TS * LDT + 256) * (int)sizeof(double) + 256;
+
+// fragment coordinates of this lane: rows wr*32 + x*8 + fr (x < 4), columns wc*16 + y*8 + 2 fk + e (y, e < 2)
+struct Frag {
+    int wr, wc, fr, fk;
+    __device__ __forceinline__ Frag(int tid) : wr((tid >> 5) & 1), wc(tid >> 6), fr((tid & 31) >> 2), fk(tid & 3) {}
+    __device__ __forceinline__ int row(int x) const { return wr * 32 + x * 8 + fr; }
+    __device__ __forceinline__ int col(int y, int e) const { return wc * 16 + y * 8 + 2 * fk + e; }
+};
+
+// acc += As x Bs over one 64-deep slab; As[k][r] (ld LDO), Bs[n][k] (ld LDO)
+__device__ __forceinline__ void mma_tile64(double (&acc)[4][2][2], const double* a, const double* b, const Frag& f) {
+    const double* as = a + f.wr * 32 + f.fr;
+    const double* bs = b + (f.wc * 16 + f.fr) * LDO;
+#pragma unroll
+    for (int k4 = 0; k4 < TS; k4 += 4) {
+        double af[4], bf[2];
+#pragma unroll
+        for (int x = 0; x < 4; x++) af[x] = as[(k4 + f.fk) * LDO + x * 8];
+#pragma unroll
+        for (int y = 0; y < 2; y++) bf[y] = bs[y * 8 * LDO + k4 + f.fk];
+#pragma unroll
+        for (int x = 0; x < 4; x++)
+#pragma unroll
+            for (int y = 0; y < 2; y++) lu_dmma884(acc[x][y][0], acc[x][y][1], af[x], bf[y]);
+    }
+}
+// 64 x 64 column-major tile (leading dimension ld) -> shared, ld LDO, same orientation; 256 threads, cp.async (not committed)
+__device__ __forceinline__ void tile_async(double* dst, const double* src, size_t ld, int tid) {
+    for (int c = tid; c < TS * TS / 2; c += 256) {
+        const int col = c >> 5, ch = (c & 31) * 2;
+        cp16(dst + col * LDO + ch, src + (size_t)col * ld + ch);
+    }
+}
+
+__device__ __forceinline__ void spin_until(const unsigned* f, unsigned epoch) {
+    while (ld_acquire(f) != epoch) __nanosleep(20);
+}
+
+// ---- the spine: block 0
+__device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, double* vec) {
+    const int tid = threadIdx.x;
+    const Frag f(tid);
+    const int N = p.N, nt = p.nt;
+    const unsigned epoch = p.epoch;
+    double* sA0 = sA;
+    double* sA1 = sA + TS * LDO;
+    double* sB0 = sB;               // F_{m-1}, written by gj64
+    double* sB1 = sB + TS * LDO;
+    for (int m = 0; m < nt; m++) {
+        unsigned long long* tr = p.trace ? p.trace + 4 * ((size_t)p.ntasks + m) : nullptr;
+        double* Cg = p.A + (size_t)m * TS * N + (size_t)m * TS;
+        if (tr && tid == 0) tr[0] = gtime();
+        if (m == 0) {
+            for (int e = tid; e < TS * TS; e += 256) {
+                const int r = e & 63, c = e >> 6;
+                T[r * LDT + c] = Cg[(size_t)c * N + r];
+            }
+        } else {
+            double* Xg = p.A + (size_t)(m - 1) * TS * N + (size_t)m * TS;        // tile (m, m-1)
+            const double* Ug = p.A + (size_t)m * TS * N + (size_t)(m - 1) * TS;  // tile (m-1, m)
+            if (tid == 0) {
+                spin_until(p.xflags + m, epoch);
+                spin_until(p.flags + (size_t)(m - 1) * nt + m, epoch);
+                if (m >= 2) spin_until(p.flags + (size_t)m * nt + m, epoch);
+            }
+            __syncthreads();
+            if (tr && tid == 0) tr[1] = gtime();
+            tile_async(sA0, Xg, N, tid);
+            tile_async(sB1, Ug, N, tid);
+            cp_commit();
+            double c0[4][2][2], acc[4][2][2];
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) c0[x][y][e] = Cg[(size_t)f.col(y, e) * N + f.row(x)];
+            cp_wait<0>();
+            __syncthreads();
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) acc[x][y][e] = 2.0 * sA0[f.col(y, e) * LDO + f.row(x)];
+            mma_tile64(acc, sA0, sB0, f);  // L_{m,m-1} = 2 X + X F_{m-1}
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        Xg[(size_t)f.col(y, e) * N + f.row(x)] = acc[x][y][e];
+                        sA1[f.col(y, e) * LDO + f.row(x)] = acc[x][y][e];
+                        acc[x][y][e] = 0.0;
+                    }
+            __syncthreads();
+            if (tid == 0) {
+                __threadfence();
+                st_release(p.flags + (size_t)m * nt + (m - 1), epoch);
+            }
+            mma_tile64(acc, sA1, sB1, f);  // L_{m,m-1} U_{m-1,m}
+#pragma unroll
+            for (int x = 0; x < 4; x++)
+#pragma unroll
+                for (int y = 0; y < 2; y++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) T[f.row(x) * LDT + f.col(y, e)] = c0[x][y][e] - acc[x][y][e];
+        }
+        __syncthreads();
+        if (tr && tid == 0) tr[2] = gtime();
+        gj64(T, vec, p.status, tid, p.Fs + (size_t)m * TS * TS, sB0);
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence();
+            st_release(p.zflags + m, epoch);
+            if (tr) tr[3] = gtime();
+        }
+    }
+}
 
 __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
     extern __shared__ __align__(16) double lu_sm[];
     double* sA = lu_sm;                   // 2 stages of L_ik as As[k][r]
     double* sB = sA + 2 * TS * LDO;       // 2 stages of U_kj as Bs[n][k]
-    double* T = sB + 2 * TS * LDO;        // work tile
-    double* vec = T + TS * LDT;           // getrf64 scratch (576 doubles)
-    unsigned char* ready = reinterpret_cast<unsigned char*>(vec + 576);  // ready[k]: both operand tiles of step k are final
+    double* T = sB + 2 * TS * LDO;        // spine: work tile (row-major)
+    double* vec = T + TS * LDT;           // spine: gj64 scratch (256 doubles)
+    unsigned char* ready = reinterpret_cast<unsigned char*>(vec + 256);  // ready[k]: both operand tiles of step k are final
     __shared__ int s_task;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int wr = warp & 1, wc = warp >> 1, fr = lane >> 2, fk = lane & 3;
+    const int tid = threadIdx.x;
+    if (blockIdx.x == 0) {
+        lu_spine(p, sA, sB, T, vec);
+        return;
+    }
+    const Frag f(tid);
     const int N = p.N, nt = p.nt;
     const unsigned epoch = p.epoch;
 
@@ -214,8 +424,9 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
         if (tid == 0) s_task = (int)atomicAdd(p.counter, 1u);
         __syncthreads();
         const int task = s_task;
-        if (task >= nt * nt) break;
-        const int ij = p.order[task], i = ij >> 16, j = ij & 0xffff, m = min(i, j);
+        if (task >= p.ntasks) break;
+        const int ij = p.order[task], i = ij >> 16, j = ij & 0xffff;
+        const int m = (i == j) ? i - 1 : min(i, j);  // number of finished block columns / rows this tile sums over
         double* Cg = p.A + (size_t)j * TS * N + (size_t)i * TS;
         if (p.trace && tid == 0) p.trace[4 * task] = gtime();
 
@@ -223,14 +434,11 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
             for (int t = tid; t < m; t += 256)
                 ready[t] = (ld_acquire(p.flags + (size_t)i * nt + t) == epoch) && (ld_acquire(p.flags + (size_t)t * nt + j) == epoch);
         };
-        auto spin = [&](const unsigned* f) {
-            while (ld_acquire(f) != epoch) __nanosleep(40);
-        };
         auto wait_ready = [&](int k) {  // uniform: ready[] is only written before a __syncthreads
             if (!ready[k]) {
                 if (tid == 0) {
-                    spin(p.flags + (size_t)i * nt + k);
-                    spin(p.flags + (size_t)k * nt + j);
+                    spin_until(p.flags + (size_t)i * nt + k, epoch);
+                    spin_until(p.flags + (size_t)k * nt + j, epoch);
                 }
                 __syncthreads();
                 refresh();
@@ -238,44 +446,19 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
             }
         };
         auto issue = [&](int k, int buf) {
-            const double* Lg = p.A + (size_t)k * TS * N + (size_t)i * TS;
-            const double* Ug = p.A + (size_t)j * TS * N + (size_t)k * TS;
-            double* a = sA + buf * TS * LDO;
-            double* b = sB + buf * TS * LDO;
-            for (int c = tid; c < TS * TS / 2; c += 256) {
-                const int col = c >> 5, ch = (c & 31) * 2;
-                cp16(a + col * LDO + ch, Lg + (size_t)col * N + ch);
-                cp16(b + col * LDO + ch, Ug + (size_t)col * N + ch);
-            }
+            tile_async(sA + buf * TS * LDO, p.A + (size_t)k * TS * N + (size_t)i * TS, N, tid);
+            tile_async(sB + buf * TS * LDO, p.A + (size_t)j * TS * N + (size_t)k * TS, N, tid);
             cp_commit();
         };
-        double acc[4][2][2];
-        auto mma_tile = [&](const double* a, const double* b) {  // acc += As x Bs over one 64-deep slab
-            const double* as = a + wr * 32 + fr;
-            const double* bs = b + (wc * 16 + fr) * LDO;
-#pragma unroll
-            for (int k4 = 0; k4 < TS; k4 += 4) {
-                double af[4], bf[2];
-#pragma unroll
-                for (int x = 0; x < 4; x++) af[x] = as[(k4 + fk) * LDO + x * 8];
-#pragma unroll
-                for (int y = 0; y < 2; y++) bf[y] = bs[y * 8 * LDO + k4 + fk];
-#pragma unroll
-                for (int x = 0; x < 4; x++)
-#pragma unroll
-                    for (int y = 0; y < 2; y++) lu_dmma884(acc[x][y][0], acc[x][y][1], af[x], bf[y]);
-            }
-        };
-
-        // own tile -> registers (fragment layout), P = 0
-        double c0[4][2][2];
+        // own tile -> registers (fragment layout), sum = 0
+        double c0[4][2][2], acc[4][2][2];
 #pragma unroll
         for (int x = 0; x < 4; x++)
 #pragma unroll
             for (int y = 0; y < 2; y++)
 #pragma unroll
                 for (int e = 0; e < 2; e++) {
-                    c0[x][y][e] = Cg[(size_t)(wc * 16 + y * 8 + 2 * fk + e) * N + wr * 32 + x * 8 + fr];
+                    c0[x][y][e] = Cg[(size_t)f.col(y, e) * N + f.row(x)];
                     acc[x][y][e] = 0.0;
                 }
         refresh();
@@ -293,7 +476,7 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
                 cp_wait<0>();
             }
             __syncthreads();
-            mma_tile(sA + (k & 1) * TS * LDO, sB + (k & 1) * TS * LDO);
+            mma_tile64(acc, sA + (k & 1) * TS * LDO, sB + (k & 1) * TS * LDO, f);
             __syncthreads();
             if (!pre && k + 1 < m) {
                 wait_ready(k + 1);
@@ -301,77 +484,57 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
             }
         }
         if (p.trace && tid == 0) p.trace[4 * task + 1] = gtime();
-        // X = A_ij - P
+        // X = A_ij - sum
 #pragma unroll
         for (int x = 0; x < 4; x++)
 #pragma unroll
             for (int y = 0; y < 2; y++)
 #pragma unroll
                 for (int e = 0; e < 2; e++) c0[x][y][e] -= acc[x][y][e];
-
-        if (i == j) {
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) T[(wr * 32 + x * 8 + fr) * LDT + wc * 16 + y * 8 + 2 * fk + e] = c0[x][y][e];
+        unsigned* flag = p.flags + (size_t)i * nt + j;
+        if (i > j + 1) {
+            // L_ij = 2 X + X F_j
+            if (tid == 0) spin_until(p.zflags + j, epoch);
             __syncthreads();
-            getrf64(T, vec, p.status, tid, Cg, (size_t)N, p.Es + (size_t)i * TS * TS, p.Fs + (size_t)i * TS * TS, TS, TS);
-        } else {
-            const bool lower = i > j;
-            // operand from the diagonal tile: F_j as Bs[n][k] (lower) or E_i as As[k][r] (upper); X as the other operand
-            if (tid == 0) spin(p.flags + (size_t)m * nt + m);
-            __syncthreads();
-            const double* Dg = (lower ? p.Fs : p.Es) + (size_t)m * TS * TS;
-            double* dst = lower ? sB : sA;
-            double* xop = lower ? sA : sB;
-            for (int c = tid; c < TS * TS / 2; c += 256) {
-                const int col = c >> 5, ch = (c & 31) * 2;
-                cp16(dst + col * LDO + ch, Dg + col * TS + ch);
-            }
+            tile_async(sB, p.Fs + (size_t)j * TS * TS, TS, tid);
             cp_commit();
-            const double scale = lower ? 2.0 : 1.0;
 #pragma unroll
             for (int x = 0; x < 4; x++)
 #pragma unroll
                 for (int y = 0; y < 2; y++)
 #pragma unroll
                     for (int e = 0; e < 2; e++) {
-                        const int row = wr * 32 + x * 8 + fr, col = wc * 16 + y * 8 + 2 * fk + e;
-                        xop[col * LDO + row] = c0[x][y][e];  // As[k = col][r = row] (lower)  /  Bs[n = col][k = row] (upper)
-                        acc[x][y][e] = scale * c0[x][y][e];
+                        sA[f.col(y, e) * LDO + f.row(x)] = c0[x][y][e];  // As[k = col][r = row]
+                        c0[x][y][e] *= 2.0;
                     }
             cp_wait<0>();
             __syncthreads();
-            mma_tile(sA, sB);  // lower: 2 X + X F ; upper: X + E X
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) T[(wr * 32 + x * 8 + fr) * LDT + wc * 16 + y * 8 + 2 * fk + e] = acc[x][y][e];
-            __syncthreads();
-            for (int e = tid; e < TS * TS; e += 256) {
-                const int r = e & 63, c = e >> 6;
-                Cg[(size_t)c * N + r] = T[r * LDT + c];
-            }
+            mma_tile64(c0, sA, sB, f);
+        } else if (i == j + 1) {
+            flag = p.xflags + i;
         }
+#pragma unroll
+        for (int x = 0; x < 4; x++)
+#pragma unroll
+            for (int y = 0; y < 2; y++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) Cg[(size_t)f.col(y, e) * N + f.row(x)] = c0[x][y][e];
         __syncthreads();  // every thread's stores are issued
         if (tid == 0) {
             if (p.trace) p.trace[4 * task + 2] = gtime();
             __threadfence();
-            st_release(p.flags + (size_t)i * nt + j, epoch);
+            st_release(flag, epoch);
             if (p.trace) p.trace[4 * task + 3] = gtime();
         }
     }
 }
 
-// claim order: level m = min(i,j) ascending; within a level the diagonal tile, then (m+d, m), (m, m+d) for d = 1, 2, ...
+// claim order: level m = 0, 1, ...: the partial sum P_{m+1} of the next diagonal tile (its inputs belong to levels < m), the two
+// tiles next to the diagonal, then the rest of block column / block row m by distance from the diagonal
 static void build_order(int nt, std::vector<int>& o) {
     o.clear();
     for (int m = 0; m < nt; m++) {
-        o.push_back((m << 16) | m);
+        if (m + 1 >= 2 && m + 1 < nt) o.push_back(((m + 1) << 16) | (m + 1));
         for (int d = 1; m + d < nt; d++) {
             o.push_back(((m + d) << 16) | m);
             o.push_back((m << 16) | (m + d));
@@ -391,13 +554,15 @@ int lu_alloc(sww_dtn_s* d) {
     const int nt = N / TS;
     std::vector<int> o;
     build_order(nt, o);
+    d->lu_ntasks = (int)o.size();
+    const size_t nflags = (size_t)nt * nt + 2 * nt + 1;
     if (cudaMalloc(&d->lu_order, sizeof(int) * o.size()) != cudaSuccess) return SWW_ENOMEM;
-    if (cudaMalloc(&d->lu_flags, sizeof(unsigned) * ((size_t)nt * nt + 1)) != cudaSuccess) return SWW_ENOMEM;
+    if (cudaMalloc(&d->lu_flags, sizeof(unsigned) * nflags) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaMemcpyAsync(d->lu_order, o.data(), sizeof(int) * o.size(), cudaMemcpyHostToDevice, d->stream));
-    SWW_CUDA(cudaMemsetAsync(d->lu_flags, 0, sizeof(unsigned) * ((size_t)nt * nt + 1), d->stream));
+    SWW_CUDA(cudaMemsetAsync(d->lu_flags, 0, sizeof(unsigned) * nflags, d->stream));
     if (cudaMalloc(&d->tr_flags, sizeof(unsigned) * (2 * (size_t)nt * TR_MAXNS + 1)) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaMemsetAsync(d->tr_flags, 0, sizeof(unsigned) * (2 * (size_t)nt * TR_MAXNS + 1), d->stream));
-    if (getenv("SWW_LU_TRACE") && cudaMalloc(&d->lu_trace, sizeof(unsigned long long) * 4 * (size_t)nt * nt) != cudaSuccess) return SWW_ENOMEM;
+    if (getenv("SWW_LU_TRACE") && cudaMalloc(&d->lu_trace, sizeof(unsigned long long) * 4 * ((size_t)nt * nt + nt)) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaStreamSynchronize(d->stream));  // o goes out of scope
     return SWW_OK;
 }
@@ -436,16 +601,18 @@ int run_lu(sww_dtn_s* d) {
     a.A = d->LU;
     a.N = N;
     a.nt = nblk;
+    a.ntasks = d->lu_ntasks;
     a.order = d->lu_order;
-    a.flags = d->lu_flags + 1;
     a.counter = d->lu_flags;
+    a.flags = d->lu_flags + 1;
+    a.xflags = a.flags + (size_t)nblk * nblk;
+    a.zflags = a.xflags + nblk;
     a.epoch = ++d->lu_epoch;
-    a.Es = Es;
     a.Fs = Fs;
     a.status = d->status;
     a.trace = d->lu_trace;
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), st));
-    const int grid = std::min(sm_count(), nblk * nblk);
+    const int grid = std::min(sm_count(), 1 + a.ntasks);
     SWW_BEGIN(KC_LU, st);
     k_lu_dataflow<<<grid, 256, LU_SMEM_BYTES, st>>>(a);
     SWW_LAUNCHED();
@@ -486,9 +653,9 @@ __global__ void __launch_bounds__(64) k_solve_small(int N, const double* __restr
 }
 
 // ------------------------------------------------------------------------------------------------ the persistent dataflow TRSM
-// Solve L Y = B, then U X = Y, for a batch of columns, in place, as ONE persistent kernel in the style of k_lu_dataflow.
-// A task is (phase, row block i, column slab s of WS columns).  Forward:  Y_i = (I + E_i)(B_i - sum_{k<i} L_ik Y_k);
-// backward:  X_i = (2 I + F_i)(Y_i - sum_{k>i} U_ik X_k).  The sums run left-looking in DMMA fragments over the blocks that are
+// Solve L Y = B, then U X = Y (block LU of k_lu_dataflow), for a batch of columns, in place, as ONE persistent kernel in the
+// same style.  A task is (phase, row block i, column slab s of WS columns).  Forward:  Y_i = B_i - sum_{k<i} L_ik Y_k;
+// backward:  X_i = (2 I + F_i)(Y_i - sum_{k>i} U_ik X_k),  2 I + F_i = inv(S_i).  The sums run left-looking in DMMA fragments over the blocks that are
 // already final (acquire-polled flags per (phase, k, s)); the chain of a slab is sequential in i, different slabs and the
 // accumulation over old blocks run in parallel.  Tasks are claimed in dependency order (forward i ascending, then backward i
 // descending), so a claimed task only waits for tasks claimed earlier.
@@ -643,13 +810,15 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             }
         }
         fold();
-        // z = (bh + bl) - (ph + pl) as sh + sl ; then the diagonal block: forward y = z + E z, backward x = 2 z + F z
-        const double* Dg = (phase ? p.Fs : p.Es) + (size_t)i * TS * TS;
-        for (int c = tid; c < TS * TS / 2; c += 256) {
-            const int col = c >> 5, ch = (c & 31) * 2;
-            cp16(sA + col * LDO + ch, Dg + col * TS + ch);  // As[k][r] = D[r][k]
+        // z = (bh + bl) - (ph + pl) as sh + sl ; then the diagonal block: forward y = z, backward x = Z_i z = 2 z + F_i z
+        if (phase) {  // block LU: L has identity diagonal blocks, only the backward sweep has a diagonal product
+            const double* Dg = p.Fs + (size_t)i * TS * TS;
+            for (int c = tid; c < TS * TS / 2; c += 256) {
+                const int col = c >> 5, ch = (c & 31) * 2;
+                cp16(sA + col * LDO + ch, Dg + col * TS + ch);  // As[k][r] = D[r][k]
+            }
+            cp_commit();
         }
-        cp_commit();
         double sh[C::FM][2], sl[C::FM][2];
 #pragma unroll
         for (int x = 0; x < C::FM; x++)
@@ -662,9 +831,11 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 sB[(col0 + e) * LDO + row0 + x * 8] = s_;  // Bs[n][k] = z[k][n]
                 acc[x][e] = 0.0;
             }
-        cp_wait<0>();
-        __syncthreads();
-        mma_tile(sA, sB);
+        if (phase) {
+            cp_wait<0>();
+            __syncthreads();
+            mma_tile(sA, sB);
+        }
         const double sc = phase ? 2.0 : 1.0;
 #pragma unroll
         for (int x = 0; x < C::FM; x++)
