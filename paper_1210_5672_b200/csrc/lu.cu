@@ -50,6 +50,11 @@ __device__ __forceinline__ unsigned ld_acquire(const unsigned* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ unsigned ld_relaxed(const unsigned* p) {
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_release(unsigned* p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
 }
@@ -181,59 +186,89 @@ __global__ void __launch_bounds__(256) k_lu_single(double* __restrict__ A, int n
 // pivot j is processed, Z_jj - 2 afterwards (the update formulas never touch the nominal part), so the result is F = inv(S) - 2 I
 // with every entry accurate relative to its own size.  Per step the owners publish column j and row j in shared memory
 // (double-buffered: one barrier per step); the rest is 16 register FMAs per thread.  vec: 256 doubles.
+// reciprocal of a pivot (|p| ~ 1/2, far from the denormal / overflow ranges the slow path of 1.0 / p guards against):
+// MUFU seed + three Newton steps (the third is a no-op correction in all but the last bit)
+__device__ __forceinline__ double pivot_rcp(double p) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(p));
+    double e = fma(-p, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-p, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-p, r, 1.0);
+    r = fma(r, e, r);
+    return r;
+}
+
+// The pivot row and the pivot column are folded into the rank-1 update itself: the column owner publishes p - 1 in place of
+// the pivot (a - (p - 1)(a / p) = a / p for the pivot row) and the pivot column uses the multiplier 1 + 1/p
+// (f - f (1 + 1/p) = -f / p); only the pivot entry itself is set separately (-2 kappa_jj / p = 1/p - 2 without cancellation).
+// explicit 32-bit shared-window accesses: with generic pointers the compiler rebuilds the window base (S2UR + ULEA) in front
+// of every predicated store, on the critical path of each elimination step
+__device__ __forceinline__ double lds64(unsigned addr) {
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts64(unsigned addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
+
 template <int JB>
-__device__ __forceinline__ void gj64_steps(double (&a)[4][4], double* vec, int* status, int tid) {
+__device__ __forceinline__ void gj64_steps(double (&a)[4][4], unsigned vec_s, int tid, double& pmin) {
     const int ty = tid & 15, tx = tid >> 4;
+    const unsigned pf = vec_s + 8 * ty;                // column j at rows ty + 16 q
+    const unsigned pu = vec_s + 8 * (64 + tx);         // row j at columns tx + 16 b
+    const unsigned pp = vec_s + 8 * (64 + 16 * JB);
 #pragma unroll 1
     for (int jt = 0; jt < 16; jt++) {
-        const int j = 16 * JB + jt;
-        double* colA = vec + (jt & 1) * 128;
-        double* rowA = colA + 64;
+        const unsigned par = (jt & 1) * 1024;
         const bool pcol = (tx == jt), prow = (ty == jt);
         if (pcol) {
 #pragma unroll
-            for (int q = 0; q < 4; q++) colA[ty + 16 * q] = a[q][JB];
+            for (int q = 0; q < 4; q++) sts64(pf + par + 128 * q, (q == JB && prow) ? a[q][JB] - 0.5 : a[q][JB]);
         }
         if (prow) {
 #pragma unroll
-            for (int b = 0; b < 4; b++) rowA[tx + 16 * b] = a[JB][b];
+            for (int b = 0; b < 4; b++) sts64(pu + par + 128 * b, a[JB][b]);
         }
         __syncthreads();
-        const double dj = rowA[j];
+        const double dj = lds64(pp + par + 8 * jt);
         const double piv = 0.5 + dj;
-        const double r = 1.0 / piv;
-        if (tid == 0 && !(fabs(piv) >= PIVOT_GUARD)) atomicCAS(status, SWW_OK, SWW_ESINGULAR);
+        const double r = pivot_rcp(piv);
+        pmin = fmin(pmin, fabs(piv));
         double f[4], ut[4];
 #pragma unroll
-        for (int q = 0; q < 4; q++) f[q] = colA[ty + 16 * q];
+        for (int q = 0; q < 4; q++) f[q] = lds64(pf + par + 128 * q);
 #pragma unroll
-        for (int b = 0; b < 4; b++) ut[b] = rowA[tx + 16 * b] * r;
+        for (int b = 0; b < 4; b++) ut[b] = lds64(pu + par + 128 * b) * r;
+        if (pcol) ut[JB] = 1.0 + r;
 #pragma unroll
         for (int q = 0; q < 4; q++)
 #pragma unroll
-            for (int b = 0; b < 4; b++) {
-                double v = fma(-f[q], ut[b], a[q][b]);
-                if (q == JB && prow) v = ut[b];                              // pivot row:    M(j,c) / p
-                if (b == JB && pcol) v = -f[q] * r;                          // pivot column: -M(i,j) / p
-                if (q == JB && b == JB && prow && pcol) v = -2.0 * dj * r;   // 1/p - 2 without cancellation
-                a[q][b] = v;
-            }
+            for (int b = 0; b < 4; b++) a[q][b] = fma(-f[q], ut[b], a[q][b]);
+        if (pcol && prow) a[JB][JB] = -2.0 * dj * r;
     }
 }
 
 // T (row-major, LDT) holds kappa = S - I/2.  On return F = inv(S) - 2 I is in Fg (global, column-major, ld 64) and in Fs_sm
-// (shared, operand layout Bs[n][k] = F[k][n], ld LDO).  Every thread of the CTA must call it.
-__device__ __noinline__ void gj64(const double* T, double* vec, int* status, int tid, double* Fg, double* Fs_sm) {
+// (shared, operand layout Bs[n][k] = F[k][n], ld LDO).  Every thread of the CTA must call it; hook() is called (by every
+// thread) after 32 steps (argument 0) and 48 steps (argument 1) -- the spine uses it to start fetching the next step's inputs.
+template <class Hook>
+__device__ __forceinline__ void gj64(const double* T, double* vec, int* status, int tid, double* Fg, double* Fs_sm, Hook&& hook) {
     const int ty = tid & 15, tx = tid >> 4;
     double a[4][4];
 #pragma unroll
     for (int q = 0; q < 4; q++)
 #pragma unroll
         for (int b = 0; b < 4; b++) a[q][b] = T[(ty + 16 * q) * LDT + tx + 16 * b];
-    gj64_steps<0>(a, vec, status, tid);
-    gj64_steps<1>(a, vec, status, tid);
-    gj64_steps<2>(a, vec, status, tid);
-    gj64_steps<3>(a, vec, status, tid);
+    double pmin = 1.0;
+    const unsigned vec_s = (unsigned)__cvta_generic_to_shared(vec);
+    gj64_steps<0>(a, vec_s, tid, pmin);
+    gj64_steps<1>(a, vec_s, tid, pmin);
+    hook(0);
+    gj64_steps<2>(a, vec_s, tid, pmin);
+    hook(1);
+    gj64_steps<3>(a, vec_s, tid, pmin);
+    if (tid == 0 && !(pmin >= PIVOT_GUARD)) atomicCAS(status, SWW_OK, SWW_ESINGULAR);  // every thread sees every pivot
 #pragma unroll
     for (int b = 0; b < 4; b++)
 #pragma unroll
@@ -325,47 +360,60 @@ __device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, dou
     const Frag f(tid);
     const int N = p.N, nt = p.nt;
     const unsigned epoch = p.epoch;
-    double* sA0 = sA;
-    double* sA1 = sA + TS * LDO;
+    double* sA0 = sA;               // X_{m,m-1}
+    double* sA1 = sA + TS * LDO;    // P_m, then L_{m,m-1}
     double* sB0 = sB;               // F_{m-1}, written by gj64
-    double* sB1 = sB + TS * LDO;
+    double* sB1 = sB + TS * LDO;    // U_{m-1,m}
+    __shared__ int s_ready;
+    // the three input flags of step m, polled by lanes 0..2 of warp 0 in parallel (an acquire load is an L2 round trip);
+    // returns (to every lane of warp 0) whether all are set; block: spin until they are
+    auto inputs_ready = [&](int m, bool block) -> bool {  // warp 1 (warp 0's lane 0 is busy publishing: fence + release)
+        const int q = tid - 32;
+        const unsigned* fl = (q == 0) ? p.xflags + m : (q == 1) ? p.flags + (size_t)(m - 1) * nt + m : p.flags + (size_t)m * nt + m;
+        const bool mine = (q < 2) || (q == 2 && m >= 2);  // P_1 is the raw diagonal tile
+        bool ok = true;
+        if (mine) {
+            if (block) spin_until(fl, epoch);
+            else ok = (ld_acquire(fl) == epoch);
+        }
+        return __all_sync(0xffffffffu, ok);
+    };
+    auto issue_inputs = [&](int m) {
+        tile_async(sA0, p.A + (size_t)(m - 1) * TS * N + (size_t)m * TS, N, tid);   // tile (m, m-1)
+        tile_async(sB1, p.A + (size_t)m * TS * N + (size_t)(m - 1) * TS, N, tid);   // tile (m-1, m)
+        tile_async(sA1, p.A + (size_t)m * TS * N + (size_t)m * TS, N, tid);         // tile (m, m)
+        cp_commit();
+    };
+    bool pre = false;  // the inputs of this step were requested before the previous inversion started
     for (int m = 0; m < nt; m++) {
         unsigned long long* tr = p.trace ? p.trace + 4 * ((size_t)p.ntasks + m) : nullptr;
-        double* Cg = p.A + (size_t)m * TS * N + (size_t)m * TS;
         if (tr && tid == 0) tr[0] = gtime();
         if (m == 0) {
+            const double* Cg = p.A;
             for (int e = tid; e < TS * TS; e += 256) {
                 const int r = e & 63, c = e >> 6;
                 T[r * LDT + c] = Cg[(size_t)c * N + r];
             }
         } else {
-            double* Xg = p.A + (size_t)(m - 1) * TS * N + (size_t)m * TS;        // tile (m, m-1)
-            const double* Ug = p.A + (size_t)m * TS * N + (size_t)(m - 1) * TS;  // tile (m-1, m)
-            if (tid == 0) {
-                spin_until(p.xflags + m, epoch);
-                spin_until(p.flags + (size_t)(m - 1) * nt + m, epoch);
-                if (m >= 2) spin_until(p.flags + (size_t)m * nt + m, epoch);
+            double* Xg = p.A + (size_t)(m - 1) * TS * N + (size_t)m * TS;
+            if (!pre) {
+                if (tid >= 32 && tid < 64) inputs_ready(m, true);
+                __syncthreads();
+                issue_inputs(m);
             }
-            __syncthreads();
             if (tr && tid == 0) tr[1] = gtime();
-            tile_async(sA0, Xg, N, tid);
-            tile_async(sB1, Ug, N, tid);
-            cp_commit();
+            cp_wait<0>();
+            __syncthreads();
             double c0[4][2][2], acc[4][2][2];
 #pragma unroll
             for (int x = 0; x < 4; x++)
 #pragma unroll
                 for (int y = 0; y < 2; y++)
 #pragma unroll
-                    for (int e = 0; e < 2; e++) c0[x][y][e] = Cg[(size_t)f.col(y, e) * N + f.row(x)];
-            cp_wait<0>();
-            __syncthreads();
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) acc[x][y][e] = 2.0 * sA0[f.col(y, e) * LDO + f.row(x)];
+                    for (int e = 0; e < 2; e++) {
+                        c0[x][y][e] = sA1[f.col(y, e) * LDO + f.row(x)];
+                        acc[x][y][e] = 2.0 * sA0[f.col(y, e) * LDO + f.row(x)];
+                    }
             mma_tile64(acc, sA0, sB0, f);  // L_{m,m-1} = 2 X + X F_{m-1}
 #pragma unroll
             for (int x = 0; x < 4; x++)
@@ -374,7 +422,7 @@ __device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, dou
 #pragma unroll
                     for (int e = 0; e < 2; e++) {
                         Xg[(size_t)f.col(y, e) * N + f.row(x)] = acc[x][y][e];
-                        sA1[f.col(y, e) * LDO + f.row(x)] = acc[x][y][e];
+                        sA1[f.col(y, e) * LDO + f.row(x)] = acc[x][y][e];  // same thread, same slot as the P entry it read
                         acc[x][y][e] = 0.0;
                     }
             __syncthreads();
@@ -390,10 +438,43 @@ __device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, dou
 #pragma unroll
                     for (int e = 0; e < 2; e++) T[f.row(x) * LDT + f.col(y, e)] = c0[x][y][e] - acc[x][y][e];
         }
-        __syncthreads();
+        __syncthreads();  // T complete; sA0, sA1, sB1 free
+        pre = false;
+        // Non-blocking look at the inputs of step m + 1 (they become final about a third of the way into this inversion): after 32
+        // elimination steps lanes 0..2 of warp 1 issue one relaxed flag load each, after 48 steps the values are looked at
+        // (the L2 round trip is hidden behind 16 steps); if all three flags are set, the tiles are fetched while the last 16
+        // steps run.  No fence here (a gpu-scope fence in the middle of the inversion costs 2 us): the tile reads are
+        // cp.async.cg, served by L2 -- the point of coherence the producer's release made the tiles visible at before the
+        // flag -- and they are issued after a CTA barrier behind the flag observation.  Otherwise step m + 1 waits (with
+        // acquire loads) for its inputs at its start.
+        unsigned pending = 0;
+        const unsigned* myflag = nullptr;
+        if (m + 1 < nt && tid >= 32 && tid < 35) {
+            const int q = tid - 32, mn = m + 1;
+            if (q == 0) myflag = p.xflags + mn;
+            if (q == 1) myflag = p.flags + (size_t)m * nt + mn;
+            if (q == 2 && mn >= 2) myflag = p.flags + (size_t)mn * nt + mn;  // P_1 is the raw diagonal tile
+        }
+        auto try_prefetch = [&](int k) {
+            if (m + 1 >= nt) return;
+            if (k == 0) {
+                if (myflag) pending = ld_relaxed(myflag);
+                return;
+            }
+            if (tid >= 32 && tid < 64) {
+                const bool ok = __all_sync(0xffffffffu, !myflag || pending == epoch);
+                if (tid == 32) s_ready = ok;
+            }
+            __syncthreads();
+            pre = s_ready;
+            __syncthreads();
+            if (pre) issue_inputs(m + 1);
+        };
         if (tr && tid == 0) tr[2] = gtime();
-        gj64(T, vec, p.status, tid, p.Fs + (size_t)m * TS * TS, sB0);
+        const long long ck0 = clock64();
+        gj64(T, vec, p.status, tid, p.Fs + (size_t)m * TS * TS, sB0, try_prefetch);
         __syncthreads();
+        if (tr && tid == 0 && m == 0) tr[1] = (unsigned long long)(clock64() - ck0);  // SM cycles of one inversion (clock check)
         if (tid == 0) {
             __threadfence();
             st_release(p.zflags + m, epoch);
