@@ -176,22 +176,27 @@ struct TabDD {  // functions of m = (i - j) mod N
 };
 
 // K_ij, G_ij of (2.13) in dd (already scaled by 1/N); dist = circular distance |i-j|
+// rc: shared table of dd reciprocals 1 / (m (m + 1)) (fill_rc below) for the in-band series
 template <bool FINITE>
-__device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, const TabDD& t, int dist, double rN, dd* kv, dd* gv) {
+__device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, const TabDD& t, int dist, double rN, const double* rc,
+                                         dd* kv, dd* gv) {
     dd k1, g1;
     if (dist != 0) {
         dd sh, ch;
-        if (dist <= DD_BAND) {
-            dd_sinhcosh(dd_sub(ni.eta, nj.eta), &sh, &ch);
+        const dd y = dd_sub(ni.eta, nj.eta);
+        if (dist <= DD_BAND && fabs(y.hi) < 0.5) {
+            dd_sinhcosh_tab(y, rc, &sh, &ch);
+        } else if (dist <= DD_BAND) {
+            dd_sinhcosh(y, &sh, &ch);
         } else {
             sh = dd_sub(dd_mul(ni.Sh, nj.Ch), dd_mul(ni.Ch, nj.Sh));
             ch = dd_sub(dd_mul(ni.Ch, nj.Ch), dd_mul(ni.Sh, nj.Sh));
         }
         dd p;
         if (t.cs.hi >= 0.0)
-            p = dd_div(dd_add(t.cs, ch), dd_add(dd_sqr(t.sn), dd_sqr(sh)));
+            p = dd_div_fast(dd_add(t.cs, ch), dd_add(dd_sqr(t.sn), dd_sqr(sh)));
         else
-            p = dd_div(dd{1.0, 0.0}, dd_sub(ch, t.cs));
+            p = dd_div_fast(dd{1.0, 0.0}, dd_sub(ch, t.cs));
         dd hp = dd_half(p);
         k1 = dd_mul(hp, dd_sub(dd_mul(nj.d1, t.sn), sh));
         g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(ni.d1, sh), t.sn)), t.c0);
@@ -205,13 +210,23 @@ __device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, con
         dd Eij = dd_mul(ni.E, nj.E);
         dd omE = dd_add(dd_mul(ni.E, nj.Dm), ni.Dm);
         dd den = dd_add(dd_sqr(omE), dd_mul_d(dd_mul(Eij, t.s2), 4.0));
-        dd cr = dd_div(dd_mul(Eij, t.sn), den);
-        dd ci = dd_neg(dd_half(dd_div(dd_mul(omE, dd_add_d(Eij, 1.0)), den)));
+        const double rb = rcp_normal(den.hi);  // both quotients share the reciprocal
+        dd cr = dd_div_rb(dd_mul(Eij, t.sn), den, rb);
+        dd ci = dd_neg(dd_half(dd_div_rb(dd_mul(omE, dd_add_d(Eij, 1.0)), den, rb)));
         k2 = dd_sub(ci, dd_mul(nj.d1, cr));
         g2 = dd_sub(cr, dd_mul(ni.d1, ci));
     }
     *kv = dd_mul_d(dd_sub(k1, k2), rN);
     *gv = dd_mul_d(dd_sub(g1, g2), rN);
+}
+// rc[m] (+ rc[32 + m]) = 1 / (m (m + 1)) in dd, m = 1..30; call with every thread of the CTA (ends with a barrier)
+__device__ __forceinline__ void fill_rc(double* rc, int tid) {
+    if (tid >= 1 && tid <= 30) {
+        const dd r = dd_div(dd{1.0, 0.0}, dd{(double)(tid * (tid + 1)), 0.0});
+        rc[tid] = r.hi;
+        rc[32 + tid] = r.lo;
+    }
+    __syncthreads();
 }
 
 __device__ __forceinline__ NodeDD load_node(int N, int j, const double* eta, const double* d1, const double* d2, const double* E,
@@ -238,6 +253,8 @@ __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* _
     const int tid = threadIdx.x, mask = N - 1;
     const int i0 = blockIdx.x * ASMDD_TI, j0 = blockIdx.y * ASMDD_TJ;
     const int i = i0 + tid;
+    __shared__ double rc[64];
+    fill_rc(rc, tid);
     if (i >= N) return;
     const size_t NN = (size_t)N * N;
     const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
@@ -248,7 +265,7 @@ __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* _
         const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
         TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
         dd kv, gv;
-        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, &kv, &gv);
+        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
         size_t o = (size_t)i + (size_t)j * N;
         dd_store(K, NN, o, kv);
         dd_store(G, NN, o, gv);
@@ -273,6 +290,8 @@ __global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const
                                                         const double* __restrict__ gam, double* __restrict__ part) {
     const int tid = threadIdx.x, mask = N - 1;
     const int i = blockIdx.x * BP_TI + tid, j0 = blockIdx.y * jchunk;
+    __shared__ double rc[64];
+    fill_rc(rc, tid);
     if (i >= N) return;
     const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
     const double rN = 1.0 / (double)N;
@@ -282,7 +301,7 @@ __global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const
         const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
         TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
         dd kv, gv;
-        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, &kv, &gv);
+        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
         aK = dd_fma(kv, dd_load(mu, N, j), aK);
         aG = dd_fma(gv, dd_load(gam, N, j), aG);
     }

@@ -98,6 +98,46 @@ __device__ __forceinline__ dd dd_div(dd a, dd b) {
     return dd_add_d(q, q3);
 }
 __device__ __forceinline__ dd dd_div_d(dd a, double b) { return dd_div(a, dd{b, 0.0}); }
+// fp64 reciprocal of a normal, well-scaled number: MUFU seed + Newton steps, no slow path (|x| far from 0, inf, denormals)
+__device__ __forceinline__ double rcp_normal(double x) {
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = SWW_FMA(-x, r, 1.0);
+    r = SWW_FMA(r, e, r);
+    e = SWW_FMA(-x, r, 1.0);
+    r = SWW_FMA(r, e, r);
+    e = SWW_FMA(-x, r, 1.0);
+    r = SWW_FMA(r, e, r);
+    return r;
+}
+// dd / dd in the hot loops (one kernel entry = two of these): two quotient digits from ONE fp64 reciprocal of b.hi.
+// q1 = a.hi rb is within a few ulp of a/b; the remainder a - b q1 is formed exactly up to O(eps^2 |a|); q2 = r rb restores the
+// low word: relative error ~ 1e-31 (the three-digit dd_div above, ~10x the instructions, is kept for the O(N) table setup).
+__device__ __forceinline__ dd dd_div_rb(dd a, dd b, double rb) {
+    const double q1 = SWW_MUL(a.hi, rb);
+    const dd p = two_prod(b.hi, q1);
+    double r = SWW_SUB(SWW_SUB(a.hi, p.hi), p.lo);  // a.hi - p.hi is exact (q1 b.hi is within a few ulp of a.hi)
+    r = SWW_ADD(r, SWW_FMA(-b.lo, q1, a.lo));
+    const double q2 = SWW_MUL(r, rb);
+    return quick_two_sum(q1, q2);
+}
+__device__ __forceinline__ dd dd_div_fast(dd a, dd b) { return dd_div_rb(a, b, rcp_normal(b.hi)); }
+// sinh, cosh of a small dd argument by the Taylor recurrences with the divisions replaced by dd reciprocals rc[m] =
+// 1 / (m (m + 1)), m = 1..30 (hi at rc[m], lo at rc[32 + m]); the number of terms follows |x| (the last term kept is < 2^-110
+// relative).  |x| < 0.5.
+__device__ __forceinline__ void dd_sinhcosh_tab(dd x, const double* rc, dd* sh, dd* ch) {
+    const dd x2 = dd_sqr(x);
+    const int nt = (x2.hi < 1e-4) ? 6 : (x2.hi < 1e-2) ? 9 : 15;
+    dd ts = x, tc = dd{1.0, 0.0}, ss = x, cc = dd{1.0, 0.0};
+    for (int n = 1; n <= nt; n++) {
+        tc = dd_mul(dd_mul(tc, x2), dd{rc[2 * n - 1], rc[32 + 2 * n - 1]});
+        ts = dd_mul(dd_mul(ts, x2), dd{rc[2 * n], rc[32 + 2 * n]});
+        cc = dd_add(cc, tc);
+        ss = dd_add(ss, ts);
+    }
+    *sh = ss;
+    *ch = cc;
+}
 __device__ __forceinline__ dd dd_from_diff(double a, double b) { return two_sum(a, -b); }  // exact a - b
 __device__ __forceinline__ dd dd_ldexp(dd a, int e) { return dd{ldexp(a.hi, e), ldexp(a.lo, e)}; }
 __device__ __forceinline__ dd dd_half(dd a) { return dd{0.5 * a.hi, 0.5 * a.lo}; }
