@@ -767,7 +767,7 @@ struct TrsmCfg {
     static constexpr int WR = 8 / WC;               // warps across the 64 rows
     static constexpr int FM = (TS / WR) / 8;        // 8 x 8 fragments per warp along the rows
     static constexpr int WSP = WC * 8;              // columns covered = WS
-    static constexpr int SMEM = (2 * TS * LDO + 2 * WS * LDO) * (int)sizeof(double) + 256;
+    static constexpr int SMEM = (3 * TS * LDO + 2 * WS * LDO) * (int)sizeof(double) + 256;
 };
 
 template <int WS>
@@ -775,7 +775,8 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
     using C = TrsmCfg<WS>;
     extern __shared__ __align__(16) double tr_sm[];
     double* sA = tr_sm;                    // 2 stages of the factor tile as As[k][r]
-    double* sB = sA + 2 * TS * LDO;        // 2 stages of the solution tile as Bs[n][k]
+    double* sD = sA + 2 * TS * LDO;        // the diagonal block F_i of the backward sweep, as As[k][r]
+    double* sB = sD + TS * LDO;            // 2 stages of the solution tile as Bs[n][k]
     unsigned char* ready = reinterpret_cast<unsigned char*>(sB + 2 * WS * LDO);
     __shared__ int s_task;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -812,16 +813,22 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 __syncthreads();
             }
         };
-        auto issue = [&](int kk, int buf) {
+        // the factors are final before this kernel starts: their tiles are requested one step ahead of the flags, so that
+        // only the (small) solution block is loaded behind the flag on the chain of a slab
+        auto issueA = [&](int kk, int buf) {
             const int k = kblock(kk);
             const double* Ag = p.A + (size_t)k * TS * N + (size_t)i * TS;          // factor tile (i, k)
-            const double* Yg = p.B + (size_t)s * WS * N + (size_t)k * TS;          // solution block k of this slab
             double* a = sA + buf * TS * LDO;
-            double* b = sB + buf * WS * LDO;
             for (int c = tid; c < TS * TS / 2; c += 256) {
                 const int col = c >> 5, ch = (c & 31) * 2;
                 cp16(a + col * LDO + ch, Ag + (size_t)col * N + ch);
             }
+            cp_commit();
+        };
+        auto issueY = [&](int kk, int buf) {
+            const int k = kblock(kk);
+            const double* Yg = p.B + (size_t)s * WS * N + (size_t)k * TS;          // solution block k of this slab
+            double* b = sB + buf * WS * LDO;
             for (int c = tid; c < WS * TS / 2; c += 256) {
                 const int col = c >> 5, ch = (c & 31) * 2;
                 cp16(b + col * LDO + ch, Yg + (size_t)col * N + ch);
@@ -867,16 +874,22 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                     acc[x][e] = 0.0;
                 }
         };
+        if (phase) {  // block LU: L has identity diagonal blocks, only the backward sweep has a diagonal product
+            const double* Dg = p.Fs + (size_t)i * TS * TS;
+            for (int c = tid; c < TS * TS / 2; c += 256) {
+                const int col = c >> 5, ch = (c & 31) * 2;
+                cp16(sD + col * LDO + ch, Dg + col * TS + ch);  // As[k][r] = D[r][k]
+            }
+            cp_commit();
+        }
+        if (m > 0) issueA(0, 0);
         refresh();
         __syncthreads();
-        if (m > 0) {
-            wait_ready(0);
-            issue(0, 0);
-        }
         for (int kk = 0; kk < m; kk++) {
-            const bool pre = (kk + 1 < m) && ready[kk + 1];
-            if (pre) {
-                issue(kk + 1, (kk + 1) & 1);
+            wait_ready(kk);
+            issueY(kk, kk & 1);
+            if (kk + 1 < m) {
+                issueA(kk + 1, (kk + 1) & 1);  // its buffer was released by the barrier that ended step kk - 1
                 cp_wait<1>();
             } else {
                 cp_wait<0>();
@@ -885,21 +898,9 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             mma_tile(sA + (kk & 1) * TS * LDO, sB + (kk & 1) * WS * LDO);
             if ((kk % TR_FOLD) == TR_FOLD - 1) fold();
             __syncthreads();
-            if (!pre && kk + 1 < m) {
-                wait_ready(kk + 1);
-                issue(kk + 1, (kk + 1) & 1);
-            }
         }
         fold();
         // z = (bh + bl) - (ph + pl) as sh + sl ; then the diagonal block: forward y = z, backward x = Z_i z = 2 z + F_i z
-        if (phase) {  // block LU: L has identity diagonal blocks, only the backward sweep has a diagonal product
-            const double* Dg = p.Fs + (size_t)i * TS * TS;
-            for (int c = tid; c < TS * TS / 2; c += 256) {
-                const int col = c >> 5, ch = (c & 31) * 2;
-                cp16(sA + col * LDO + ch, Dg + col * TS + ch);  // As[k][r] = D[r][k]
-            }
-            cp_commit();
-        }
         double sh[C::FM][2], sl[C::FM][2];
 #pragma unroll
         for (int x = 0; x < C::FM; x++)
@@ -913,9 +914,9 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 acc[x][e] = 0.0;
             }
         if (phase) {
-            cp_wait<0>();
+            cp_wait<0>();  // F_i (requested at the start of the task) when m == 0
             __syncthreads();
-            mma_tile(sA, sB);
+            mma_tile(sD, sB);
         }
         const double sc = phase ? 2.0 : 1.0;
 #pragma unroll
