@@ -801,17 +801,8 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
         double* Lg = p.Blo + (size_t)s * WS * N + (size_t)i * TS;
         auto kblock = [&](int kk) { return phase ? nt - 1 - kk : kk; };
 
-        auto refresh = [&]() {
-            for (int t = tid; t < m; t += 256) ready[t] = ld_acquire(fl + (size_t)kblock(t) * ns + s) == epoch;
-        };
-        auto wait_ready = [&](int kk) {
-            if (!ready[kk]) {
-                if (tid == 0)
-                    while (ld_acquire(fl + (size_t)kblock(kk) * ns + s) != epoch) __nanosleep(40);
-                __syncthreads();
-                refresh();
-                __syncthreads();
-            }
+        auto refresh = [&](int from) {
+            for (int t = from + tid; t < m; t += 256) ready[t] = ld_acquire(fl + (size_t)kblock(t) * ns + s) == epoch;
         };
         // the factors are final before this kernel starts: their tiles are requested one step ahead of the flags, so that
         // only the (small) solution block is loaded behind the flag on the chain of a slab
@@ -883,13 +874,19 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             cp_commit();
         }
         if (m > 0) issueA(0, 0);
-        refresh();
+        refresh(0);
         __syncthreads();
         for (int kk = 0; kk < m; kk++) {
-            wait_ready(kk);
+            const bool missed = !ready[kk];  // uniform: ready[] is only written before a barrier
+            if (missed) {
+                if (tid == 0)
+                    while (ld_acquire(fl + (size_t)kblock(kk) * ns + s) != epoch) __nanosleep(20);
+                __syncthreads();
+            }
             issueY(kk, kk & 1);
+            if (kk + 1 < m) issueA(kk + 1, (kk + 1) & 1);  // its buffer was released by the barrier that ended step kk - 1
+            if (missed) refresh(kk + 1);                   // look at the later flags while the loads are in flight
             if (kk + 1 < m) {
-                issueA(kk + 1, (kk + 1) & 1);  // its buffer was released by the barrier that ended step kk - 1
                 cp_wait<1>();
             } else {
                 cp_wait<0>();
