@@ -116,7 +116,7 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "source": "fallback (B200_PROFILING.md)"}
 
 
-def cpu_oracle_columns_per_s(nrhs_target: int, small: int = 4, large: int = 16):
+def cpu_oracle_columns_per_s(nrhs_target: int, small: int = 8, large: int = 136):
     """the long-double oracle as it stands, timed on this host: setup + `small` and setup + `large` columns of the metric-point
     workload; columns/s extrapolated to nrhs_target columns sharing one setup."""
     import oracle
@@ -127,13 +127,13 @@ def cpu_oracle_columns_per_s(nrhs_target: int, small: int = 4, large: int = 16):
         t0 = time.perf_counter()
         orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:n], c.dphi[:n])
         ts.append(time.perf_counter() - t0)
-    t_col = max((ts[1] - ts[0]) / (large - small), 1e-9)
+    t_col = max((ts[1] - ts[0]) / (large - small), 0.0)  # the setup (pivoted elimination of one 2048^2 matrix) dominates
     t_setup = max(ts[0] - small * t_col, 0.0)
     value = nrhs_target / (t_setup + nrhs_target * t_col)
     return {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
             "sample": f"long-double oracle, N={c.N}: setup+base+{small} columns ({ts[0]:.2f} s) and setup+base+{large} columns ({ts[1]:.2f} s) "
                       f"of the {nrhs_target}; columns/s extrapolated as {nrhs_target}/(t_setup + {nrhs_target} t_col), "
-                      f"t_setup={t_setup:.2f} s, t_col={t_col:.4f} s"}
+                      f"t_setup={t_setup:.2f} s, t_col={t_col:.5f} s"}
 
 
 def run_reference(args):
@@ -285,13 +285,14 @@ def main():
     if not args.no_e2e:
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
         h_eta, h_phi0, h_deta, h_dphi = pin(case.eta), pin(case.phi0), pin(case.deta), pin(case.dphi)
+        h_out = torch.empty_like(h_dphi).pin_memory()
         ke = max(3, min(K, 20))
-        for _ in range(2):
-            sww.dtn_linearized_host(h_eta, h_phi0, h_deta, h_dphi, case.h)
+        for _ in range(3):
+            sww.dtn_linearized_host(h_eta, h_phi0, h_deta, h_dphi, case.h, out=h_out)
         barrier()
         t0 = time.perf_counter()
         for _ in range(ke):
-            res = sww.dtn_linearized_host(h_eta, h_phi0, h_deta, h_dphi, case.h)
+            res = sww.dtn_linearized_host(h_eta, h_phi0, h_deta, h_dphi, case.h, out=h_out)
         barrier()
         te = torch.tensor([(time.perf_counter() - t0) / ke], dtype=torch.float64, device="cuda")
         if dist is not None:

@@ -16,7 +16,7 @@ EXPORTS = [
     "sww_dtn_setup", "sww_dtn_refactor", "sww_dtn_apply", "sww_dtn_set_base", "sww_dtn_linearized_apply", "sww_dtn_get",
     "sww_dtn_status", "sww_dtn_destroy", "sww_state_create", "sww_rk_advance", "sww_state_read", "sww_state_energy",
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
-    "sww_dtn_linearized_host", "sww_timing_enable", "sww_timing_read",
+    "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
 ]
 
 
@@ -249,17 +249,26 @@ class State:
             pass
 
 
-def dtn_linearized_host(eta, phi0, deta, dphi, h: float, prec: int = F64):
-    """HOST-buffer path (sww_dtn_linearized_host): CPU float64 tensors in, CPU tensor out; copies are inside the call."""
+def dtn_linearized_host(eta, phi0, deta, dphi, h: float, prec: int = F64, out=None):
+    """HOST-buffer path (sww_dtn_linearized_host): CPU float64 tensors in, CPU tensor out; copies are inside the call.
+    out: optional preallocated (ideally pinned) CPU tensor shaped like dphi."""
     _require_cuda()
     mul = 2 if prec == DD else 1
     N = eta.numel() // mul
     nrhs = dphi.numel() // (N * mul)
     for t in (eta, phi0, deta, dphi):
         assert (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous()
-    out = torch.empty_like(dphi)
-    if dphi.is_pinned():
-        out = out.pin_memory()
+    if out is None:
+        out = torch.empty_like(dphi)
+        if dphi.is_pinned():
+            out = out.pin_memory()
+    else:
+        assert (not out.is_cuda) and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == dphi.numel()
     _check(lib().sww_dtn_linearized_host(eta.data_ptr(), phi0.data_ptr(), deta.data_ptr(), dphi.data_ptr(), out.data_ptr(), N, float(h), prec, nrhs),
            "sww_dtn_linearized_host")
     return out
+
+
+def host_cache_clear():
+    """free the context cached by dtn_linearized_host (sww_host_cache_clear)"""
+    _check(lib().sww_host_cache_clear(), "sww_host_cache_clear")

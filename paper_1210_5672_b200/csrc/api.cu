@@ -212,27 +212,69 @@ const char* sww_strerror(int status) {
 const char* sww_last_cuda_error(void) { return g_cuda_err; }
 unsigned long long sww_launch_count(void) { return g_launches; }
 
+// One cached context (handle + device staging buffers) for the HOST-pointer entry point: a caller that steps a surface calls
+// this once per stage with the same N and precision, and creating a handle (about 150 MB of cudaMalloc at N = 2048) would cost
+// ten times the computation.  The cache is replaced when N or the precision changes; sww_host_cache_clear() frees it.
+namespace {
+struct HostCtx {
+    sww_dtn_t h = nullptr;
+    int N = 0, prec = -1;
+    size_t cap = 0;  // staging capacity in bytes of one batch buffer
+    double *de = nullptr, *dp = nullptr, *dde = nullptr, *ddp = nullptr, *dout = nullptr;
+} g_host;
+void host_ctx_free() {
+    if (g_host.h) sww_dtn_destroy(g_host.h);
+    cudaFree(g_host.de); cudaFree(g_host.dp); cudaFree(g_host.dde); cudaFree(g_host.ddp); cudaFree(g_host.dout);
+    g_host = HostCtx();
+}
+}  // namespace
+
+int sww_host_cache_clear(void) {
+    host_ctx_free();
+    return SWW_OK;
+}
+
 int sww_dtn_linearized_host(const void* eta, const void* phi0, const void* deta, const void* dphi, void* out, int N, double h,
                             int prec, int nrhs) {
-    if (!eta || !phi0 || !deta || !dphi || !out || nrhs < 1 || !valid_N(N)) return SWW_EINVAL;
+    if (!eta || !phi0 || !deta || !dphi || !out || nrhs < 1 || !valid_N(N) || (prec != SWW_F64 && prec != SWW_DD) || !(h > 0.0))
+        return SWW_EINVAL;
     const size_t mul = prec == SWW_DD ? 2 : 1, vec = sizeof(double) * N * mul, bat = vec * nrhs;
-    double *de = nullptr, *dp = nullptr, *dde = nullptr, *ddp = nullptr, *dout = nullptr;
     cudaStream_t st = nullptr;
-    int rc = SWW_OK;
-    sww_dtn_t h_ = nullptr;
-    if (cudaMalloc(&de, vec) || cudaMalloc(&dp, vec) || cudaMalloc(&dde, bat) || cudaMalloc(&ddp, bat) || cudaMalloc(&dout, bat))
-        rc = SWW_ENOMEM;
-    if (!rc && (cudaMemcpyAsync(de, eta, vec, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(dp, phi0, vec, cudaMemcpyHostToDevice, st) ||
-                cudaMemcpyAsync(dde, deta, bat, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(ddp, dphi, bat, cudaMemcpyHostToDevice, st)))
-        rc = SWW_ECUDA;
-    if (!rc) rc = sww_dtn_setup(de, N, h, prec, st, &h_);
-    if (!rc) rc = sww_dtn_set_base(h_, dp);
-    if (!rc) rc = sww_dtn_linearized_apply(h_, dde, ddp, nrhs, dout);
-    if (!rc && cudaMemcpyAsync(out, dout, bat, cudaMemcpyDeviceToHost, st)) rc = SWW_ECUDA;
-    if (!rc) rc = sww_dtn_status(h_);
-    if (h_) sww_dtn_destroy(h_);
-    cudaFree(de); cudaFree(dp); cudaFree(dde); cudaFree(ddp); cudaFree(dout);
-    return rc;
+    HostCtx& c = g_host;
+    if (c.N != N || c.prec != prec) host_ctx_free();
+    if (!c.de) {
+        if (cudaMalloc(&c.de, vec) || cudaMalloc(&c.dp, vec)) { host_ctx_free(); return SWW_ENOMEM; }
+        c.N = N;
+        c.prec = prec;
+    }
+    if (c.cap < bat) {
+        cudaFree(c.dde); cudaFree(c.ddp); cudaFree(c.dout);
+        c.dde = c.ddp = c.dout = nullptr;
+        c.cap = 0;
+        if (cudaMalloc(&c.dde, bat) || cudaMalloc(&c.ddp, bat) || cudaMalloc(&c.dout, bat)) { host_ctx_free(); return SWW_ENOMEM; }
+        c.cap = bat;
+    }
+    if (cudaMemcpyAsync(c.de, eta, vec, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(c.dp, phi0, vec, cudaMemcpyHostToDevice, st) ||
+        cudaMemcpyAsync(c.dde, deta, bat, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(c.ddp, dphi, bat, cudaMemcpyHostToDevice, st))
+        return note_cuda(cudaGetLastError(), "host staging copies");
+    int rc;
+    if (!c.h) {
+        rc = sww_dtn_setup(c.de, N, h, prec, st, &c.h);
+    } else {
+        c.h->h = h;  // a new depth is a new surface like any other
+        c.h->finite = !std::isinf(h);
+        rc = sww_dtn_refactor(c.h, c.de);
+    }
+    if (!rc) rc = sww_dtn_set_base(c.h, c.dp);
+    if (!rc) rc = sww_dtn_linearized_apply(c.h, c.dde, c.ddp, nrhs, c.dout);
+    if (!rc && cudaMemcpyAsync(out, c.dout, bat, cudaMemcpyDeviceToHost, st)) rc = SWW_ECUDA;
+    if (!rc) rc = sww_dtn_status(c.h);  // synchronises
+    if (rc) {  // a sticky device status (EBOTTOM, ESINGULAR) must not leak into the next call
+        int keep = rc;
+        host_ctx_free();
+        return keep;
+    }
+    return SWW_OK;
 }
 
 }  // extern "C"

@@ -264,3 +264,19 @@ def test_host_buffer_entry_point(sww):
     dev, _ = gpu_linearized(c)
     host = sww.dtn_linearized_host(*(torch.from_numpy(np.ascontiguousarray(a)) for a in (c.eta, c.phi0, c.deta, c.dphi)), c.h)
     assert np.array_equal(host.numpy(), dev[0])
+    # the library caches one context between host calls: a second surface, another depth, fewer / more columns, another N
+    # must each give exactly what a fresh device-side handle gives
+    for case in (si.config3(256, 8), si.config3(256, 64), si.config5(256, 16), si.config3(128, 32), c):
+        dev, _ = gpu_linearized(case)
+        args = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (case.eta, case.phi0, case.deta, case.dphi)]
+        out = torch.empty_like(args[3]).pin_memory()
+        host = sww.dtn_linearized_host(*args, case.h, out=out)
+        assert host is out and np.array_equal(host.numpy(), dev[0]), case.name
+    # a failing call (surface below the bottom) reports its status and does not poison the next one
+    with pytest.raises(sww.SwwError) as e:
+        sww.dtn_linearized_host(torch.from_numpy(c.eta - 2.0), *(torch.from_numpy(np.ascontiguousarray(a)) for a in (c.phi0, c.deta, c.dphi)), c.h)
+    assert e.value.status == -4
+    dev, _ = gpu_linearized(c)
+    host = sww.dtn_linearized_host(*(torch.from_numpy(np.ascontiguousarray(a)) for a in (c.eta, c.phi0, c.deta, c.dphi)), c.h)
+    assert np.array_equal(host.numpy(), dev[0])
+    sww.host_cache_clear()
