@@ -102,6 +102,8 @@ int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_
     d->bp_chunks = N / 32 < 1 ? 1 : (N / 32 > 64 ? 64 : N / 32);
     alloc(&d->bp_part, (size_t)d->bp_chunks * 4 * N);
     if (ok && cudaMalloc(&d->status, sizeof(int)) != cudaSuccess) ok = false;
+    if (ok && (cudaMalloc(&d->mv_count, sizeof(unsigned) * (N / 32 + 1)) != cudaSuccess ||
+               cudaMemsetAsync(d->mv_count, 0, sizeof(unsigned) * (N / 32 + 1), d->stream) != cudaSuccess)) ok = false;
     if (!ok) { sww_dtn_destroy(d); return SWW_ENOMEM; }
     if (cudaMemsetAsync(d->status, 0, sizeof(int), d->stream) != cudaSuccess) { sww_dtn_destroy(d); return SWW_ECUDA; }
     rc = ensure_workspace(d, 64);
@@ -189,6 +191,7 @@ int sww_dtn_destroy(sww_dtn_t d) {
                       d->ws.B, d->ws.Gam, d->ws.W, d->ws.T, d->ws.R, d->ws.S};
     for (double* p : ptrs) cudaFree(p);
     cudaFree(d->status);
+    cudaFree(d->mv_count);
     cudaFree(d->lu_order);
     cudaFree(d->lu_flags);
     cudaFree(d->tr_flags);

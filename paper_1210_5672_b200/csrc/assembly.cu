@@ -17,20 +17,91 @@ __global__ void __launch_bounds__(256) k_deriv_dd(int N, const double* __restric
     int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= N) return;
     int i = warp, mask = N - 1;
-    dd acc{0.0, 0.0};
-    for (int m = 1 + lane; m < N / 2; m += 32) {
-        dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
-        dd c = dd_load(dc, N, m);
-        acc = dd_fma(c, dd_sub(a, b), acc);
+    dd acc4[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};  // independent chains: a dd multiply-add is ~30 dependent instructions
+    const bool full = ((N / 2) % 128) == 0;  // dc[N/2] = 0: the last group may run over it unguarded, loads issued together
+    for (int m0 = 1 + lane; m0 < N / 2; m0 += 128) {
+        if (full) {
+            dd c[4], a[4], b[4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                const int m = m0 + 32 * u;
+                c[u] = dd_load(dc, N, m);
+                a[u] = dd_load(f, N, (i - m) & mask);
+                b[u] = dd_load(f, N, (i + m) & mask);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; u++) acc4[u] = dd_fma(c[u], dd_sub(a[u], b[u]), acc4[u]);
+        } else {
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                const int m = m0 + 32 * u;
+                if (m < N / 2) {
+                    dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
+                    dd c = dd_load(dc, N, m);
+                    acc4[u] = dd_fma(c, dd_sub(a, b), acc4[u]);
+                }
+            }
+        }
     }
+    dd acc = dd_add(dd_add(acc4[0], acc4[1]), dd_add(acc4[2], acc4[3]));
     acc = dd_warp_sum(acc);
     if (lane == 0) dd_store(out, N, i, acc);
 }
 
+// exp / expm1 / sinh / cosh for the node tables with the series divisions replaced by dd reciprocals from a shared table
+// rn[n] (+ rn[32 + n]) = 1 / n, n = 1..31 (one accurate division per lane instead of ~80 per node)
+__device__ __forceinline__ dd exp_series_tab(dd r, const double* rn, bool minus_one) {
+    dd term = minus_one ? r : dd{1.0, 0.0}, sum = term;
+    for (int n = minus_one ? 2 : 1; n <= 27; n++) {
+        term = dd_mul(dd_mul(term, r), dd{rn[n], rn[32 + n]});
+        sum = dd_add(sum, term);
+    }
+    return sum;
+}
+__device__ __forceinline__ dd dd_exp_tab(dd x, const double* rn) {
+    double kf = rint(x.hi * 1.4426950408889634074);
+    dd r = dd_sub(x, dd_mul_d(dd_ln2(), kf));
+    return dd_ldexp(exp_series_tab(r, rn, false), (int)kf);
+}
+__device__ __forceinline__ dd dd_expm1_tab(dd x, const double* rn) {
+    if (fabs(x.hi) < 0.34) return exp_series_tab(x, rn, true);
+    return dd_add_d(dd_exp_tab(x, rn), -1.0);
+}
+__device__ __forceinline__ void dd_sinhcosh_tab_n(dd x, const double* rn, dd* sh, dd* ch) {
+    if (fabs(x.hi) < 0.5) {
+        dd x2 = dd_sqr(x);
+        dd ts = x, tc = dd{1.0, 0.0}, ss = x, cc = dd{1.0, 0.0};
+        for (int n = 1; n <= 15; n++) {
+            tc = dd_mul(dd_mul(dd_mul(tc, x2), dd{rn[2 * n - 1], rn[32 + 2 * n - 1]}), dd{rn[2 * n], rn[32 + 2 * n]});
+            ts = dd_mul(dd_mul(dd_mul(ts, x2), dd{rn[2 * n], rn[32 + 2 * n]}), dd{rn[2 * n + 1], rn[32 + 2 * n + 1]});
+            cc = dd_add(cc, tc);
+            ss = dd_add(ss, ts);
+        }
+        *sh = ss;
+        *ch = cc;
+        return;
+    }
+    dd e = dd_exp_tab(x, rn);
+    dd ei = dd_div(dd{1.0, 0.0}, e);
+    *sh = dd_half(dd_sub(e, ei));
+    *ch = dd_half(dd_add(e, ei));
+}
+
 // per-node tables in dd (planar): E = exp(-(h+eta)), Dm = 1 - E (via expm1) for the image term, sinh/cosh(eta) for the dd kernels.
 // The fp64 assembly reads the hi planes of E, Dm; the dd assembly and the dd base-state pass read everything.
-__global__ void k_node_tables(int N, double h, int finite, const double* __restrict__ eta, double* __restrict__ E,
-                              double* __restrict__ Dm, double* __restrict__ Sh, double* __restrict__ Ch, int* status) {
+// Launch with 32 threads per block (one warp fills the reciprocal table).
+__global__ void __launch_bounds__(32) k_node_tables(int N, double h, int finite, const double* __restrict__ eta, double* __restrict__ E,
+                                                    double* __restrict__ Dm, double* __restrict__ Sh, double* __restrict__ Ch, int* status) {
+    __shared__ double rn[64];
+    {
+        const int n = threadIdx.x;
+        if (n >= 1) {
+            const dd r = dd_div(dd{1.0, 0.0}, dd{(double)n, 0.0});
+            rn[n] = r.hi;
+            rn[32 + n] = r.lo;
+        }
+        __syncwarp();
+    }
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     dd e = dd_load(eta, N, j);
@@ -38,11 +109,11 @@ __global__ void k_node_tables(int N, double h, int finite, const double* __restr
         dd Y = dd_add_d(e, h);
         if (!(Y.hi > 0.0)) atomicCAS(status, SWW_OK, SWW_EBOTTOM);
         dd nY = dd_neg(Y);
-        dd_store(E, N, j, dd_exp(nY));
-        dd_store(Dm, N, j, dd_neg(dd_expm1(nY)));
+        dd_store(E, N, j, dd_exp_tab(nY, rn));
+        dd_store(Dm, N, j, dd_neg(dd_expm1_tab(nY, rn)));
     }
     dd sh, ch;
-    dd_sinhcosh(e, &sh, &ch);
+    dd_sinhcosh_tab_n(e, rn, &sh, &ch);
     dd_store(Sh, N, j, sh);
     dd_store(Ch, N, j, ch);
 }
@@ -311,16 +382,28 @@ __global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const
     p[2 * N + i] = aG.hi;
     p[3 * N + i] = aG.lo;
 }
-// res = b - mu/2 - sum pK  (2.7) ;  w = sum pG ;  res_f64 = RN(res)
-__global__ void k_base_reduce(int N, int nchunk, const double* __restrict__ part, const double* __restrict__ b, const double* __restrict__ mu,
-                              double* __restrict__ res, double* __restrict__ res_f64, double* __restrict__ w) {
-    int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N) return;
+// res = b - mu/2 - sum pK  (2.7) ;  w = sum pG ;  res_f64 = RN(res).  128 threads = 32 nodes x 4 groups of chunks (the loads of a
+// node's partial sums are the whole cost: four groups keep four of them in flight and shorten the dd chains).
+__global__ void __launch_bounds__(128) k_base_reduce(int N, int nchunk, const double* __restrict__ part, const double* __restrict__ b,
+                                                     const double* __restrict__ mu, double* __restrict__ res, double* __restrict__ res_f64,
+                                                     double* __restrict__ w) {
+    __shared__ double sh[4][4][32];
+    const int l = threadIdx.x & 31, g = threadIdx.x >> 5;
+    const int i = blockIdx.x * 32 + l;
     dd sK{0, 0}, sG{0, 0};
-    for (int c = 0; c < nchunk; c++) {
-        const double* p = part + (size_t)c * 4 * N;
-        sK = dd_add(sK, dd{p[i], p[N + i]});
-        sG = dd_add(sG, dd{p[2 * N + i], p[3 * N + i]});
+    if (i < N) {
+        for (int c = g; c < nchunk; c += 4) {
+            const double* p = part + (size_t)c * 4 * N;
+            sK = dd_add(sK, dd{p[i], p[N + i]});
+            sG = dd_add(sG, dd{p[2 * N + i], p[3 * N + i]});
+        }
+    }
+    sh[g][0][l] = sK.hi; sh[g][1][l] = sK.lo; sh[g][2][l] = sG.hi; sh[g][3][l] = sG.lo;
+    __syncthreads();
+    if (g != 0 || i >= N) return;
+    for (int q = 1; q < 4; q++) {
+        sK = dd_add(sK, dd{sh[q][0][l], sh[q][1][l]});
+        sG = dd_add(sG, dd{sh[q][2][l], sh[q][3][l]});
     }
     dd r = dd_sub(dd_sub(dd_load(b, N, i), dd_half(dd_load(mu, N, i))), sK);
     dd_store(res, N, i, r);
@@ -340,7 +423,7 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
         k_base_pass_dd<false><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
     SWW_LAUNCHED();
     SWW_BEGIN(KC_OTHER, d->stream);
-    k_base_reduce<<<(N + 127) / 128, 128, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
+    k_base_reduce<<<(N + 31) / 32, 128, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

@@ -89,6 +89,7 @@ struct sww_dtn_s {
     double *bphi, *bW0, *bu, *bv;
     double *bp_part;      // partial sums of the dd base-state pass: bp_chunks x 4 x N doubles
     int bp_chunks;
+    unsigned* mv_count;   // k_matvec_dd: arrival counters per 32-row block (zero between launches)
     double *tmp;          // 14 N doubles: dd scratch vectors of the accurate base state (ddpath.cu)
     bool has_base;
     int* status;          // device sticky status

@@ -20,21 +20,41 @@ __global__ void __launch_bounds__(256) k_circ_dd(int N, int mode, const double* 
     int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= N) return;
     int i = warp, mask = N - 1;
-    dd acc{0.0, 0.0};
-    const double hs = 4.0 / (double)N;  // exact (power of two)
-    for (int m = 1 + lane; m < N / 2; m += 32) {
-        dd c;
-        if (mode == 0) {
-            c = dd_load(dc, N, m);
+    // four independent dd accumulators per lane: one dd multiply-add is a chain of ~30 dependent fp64 instructions
+    dd acc4[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+    const double hs = (mode == 0) ? 1.0 : 4.0 / (double)N;  // exact (power of two)
+    const double* coef = (mode == 0) ? dc : c0;
+    const int step = (mode == 0) ? 1 : 2;                   // H: odd m only
+    // both tables hold 0 at m = N/2, so when the stride divides N/2 the last group may run over it unguarded and the
+    // 24 loads of a group are issued together (the kernel is bound by their latency otherwise)
+    const bool full = ((N / 2) % (4 * 32 * step)) == 0;
+    for (int m0 = 1 + step * lane; m0 < N / 2; m0 += 4 * 32 * step) {
+        if (full) {
+            dd c[4], a[4], b[4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                const int m = m0 + u * 32 * step;
+                c[u] = dd_load(coef, N, m);
+                a[u] = dd_load(f, N, (i - m) & mask);
+                b[u] = dd_load(f, N, (i + m) & mask);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; u++) acc4[u] = dd_fma(dd{c[u].hi * hs, c[u].lo * hs}, dd_sub(a[u], b[u]), acc4[u]);
         } else {
-            if (!(m & 1)) continue;
-            c = dd_load(c0, N, m);
-            c.hi *= hs;
-            c.lo *= hs;
+#pragma unroll
+            for (int u = 0; u < 4; u++) {
+                const int m = m0 + u * 32 * step;
+                if (m < N / 2) {
+                    dd c = dd_load(coef, N, m);
+                    c.hi *= hs;
+                    c.lo *= hs;
+                    dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
+                    acc4[u] = dd_fma(c, dd_sub(a, b), acc4[u]);
+                }
+            }
         }
-        dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
-        acc = dd_fma(c, dd_sub(a, b), acc);
     }
+    dd acc = dd_add(dd_add(acc4[0], acc4[1]), dd_add(acc4[2], acc4[3]));
     acc = dd_warp_sum(acc);
     if (lane == 0) dd_store(out, N, i, acc);
 }
@@ -51,27 +71,66 @@ int circ_dd(sww_dtn_s* d, int mode, const double* in, double* out) {
 // ------------------------------------------------------------------------------------------------ dd mat-vec (one column)
 // y = zs * z + beta * x + alpha * (A x), accumulated in dd.  A column-major N x N, fp64 (Alo == nullptr) or dd (Alo = lo plane).
 // x, z, y dd planar (2N).  y_f64 (optional) receives y rounded to fp64.  zs, beta, alpha must be powers of two or 0 (exact).
-// Block = 8 warps x 32 rows: warp q sums the columns j = q (mod 8) for 32 consecutive rows (coalesced 256 B per load).
+// Block = 8 warps x 32 rows: warp q sums the columns j = q (mod 8) of this block's column range for 32 consecutive rows
+// (coalesced 256 B per load, eight loads in flight per thread: the kernel streams A once and is bound by memory latency).
+// gridDim.y blocks share a row block: each writes its partial dd sums to part[y][2][N]; the last one to arrive (counter per
+// row block, left at zero again) adds them up and applies the epilogue.
 __global__ void __launch_bounds__(256) k_matvec_dd(int N, const double* __restrict__ A, const double* __restrict__ Alo,
                                                    const double* __restrict__ x, double zs, const double* __restrict__ z, double beta,
-                                                   double alpha, double* __restrict__ y, double* __restrict__ y_f64) {
+                                                   double alpha, double* __restrict__ y, double* __restrict__ y_f64,
+                                                   double* __restrict__ part, unsigned* __restrict__ count) {
     __shared__ double red_hi[8][32], red_lo[8][32];
+    __shared__ unsigned s_last;
     const int lane = threadIdx.x & 31, q = threadIdx.x >> 5;
     const int i = blockIdx.x * 32 + lane;
-    dd acc{0.0, 0.0};
+    const int ny = gridDim.y, jn = N / ny, jb = blockIdx.y * jn, je = jb + jn;
+    dd acc4[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};  // independent chains (see k_circ_dd)
     if (i < N) {
-        for (int j = q; j < N; j += 8) {
-            dd xj = dd_load(x, N, j);
-            size_t o = (size_t)j * N + i;
-            dd a{A[o], Alo ? Alo[o] : 0.0};
-            acc = dd_fma(a, xj, acc);
+        if ((jn & 63) == 0) {
+            for (int j0 = jb + q; j0 < je; j0 += 64) {
+                dd a[8], xj[8];
+#pragma unroll
+                for (int u = 0; u < 8; u++) {
+                    const int j = j0 + 8 * u;
+                    const size_t o = (size_t)j * N + i;
+                    a[u] = dd{A[o], Alo ? Alo[o] : 0.0};
+                    xj[u] = dd_load(x, N, j);
+                }
+#pragma unroll
+                for (int u = 0; u < 8; u++) acc4[u & 3] = dd_fma(a[u], xj[u], acc4[u & 3]);
+            }
+        } else {
+            for (int j = jb + q; j < je; j += 8) {
+                dd xj = dd_load(x, N, j);
+                size_t o = (size_t)j * N + i;
+                acc4[0] = dd_fma(dd{A[o], Alo ? Alo[o] : 0.0}, xj, acc4[0]);
+            }
         }
     }
+    dd acc = dd_add(dd_add(acc4[0], acc4[1]), dd_add(acc4[2], acc4[3]));
     red_hi[q][lane] = acc.hi;
     red_lo[q][lane] = acc.lo;
     __syncthreads();
-    if (q == 0 && i < N) {
-        for (int w = 1; w < 8; w++) acc = dd_add(acc, dd{red_hi[w][lane], red_lo[w][lane]});
+    if (q != 0) return;
+    for (int w = 1; w < 8; w++) acc = dd_add(acc, dd{red_hi[w][lane], red_lo[w][lane]});
+    if (ny > 1) {
+        if (i < N) {
+            part[((size_t)blockIdx.y * 2) * N + i] = acc.hi;
+            part[((size_t)blockIdx.y * 2 + 1) * N + i] = acc.lo;
+        }
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) s_last = (atomicAdd(count + blockIdx.x, 1u) == (unsigned)(ny - 1));
+        __syncwarp();
+        if (!s_last) return;
+        __threadfence();
+        if (lane == 0) count[blockIdx.x] = 0;  // ready for the next launch
+        acc = dd{0.0, 0.0};
+        if (i < N)
+            for (int c = 0; c < ny; c++)
+                acc = dd_add(acc, dd{__ldcg(part + ((size_t)c * 2) * N + i), __ldcg(part + ((size_t)c * 2 + 1) * N + i)});
+    }
+    if (i < N) {
         dd r{alpha * acc.hi, alpha * acc.lo};
         if (beta != 0.0) {
             dd xi = dd_load(x, N, i);
@@ -89,8 +148,9 @@ __global__ void __launch_bounds__(256) k_matvec_dd(int N, const double* __restri
 static int matvec_dd(sww_dtn_s* d, const double* A, const double* Alo, const double* x, double zs, const double* z, double beta,
                      double alpha, double* y, double* y_f64) {
     const int N = d->N;
+    const int ny = (N >= 512 && d->bp_chunks >= 2) ? 4 : 1;  // part = d->bp_part: bp_chunks * 4 * N doubles >= ny * 2 * N
     SWW_BEGIN(KC_DDGEMM, d->stream);
-    k_matvec_dd<<<(N + 31) / 32, 256, 0, d->stream>>>(N, A, Alo, x, zs, z, beta, alpha, y, y_f64);
+    k_matvec_dd<<<dim3((N + 31) / 32, ny), 256, 0, d->stream>>>(N, A, Alo, x, zs, z, beta, alpha, y, y_f64, d->bp_part, d->mv_count);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
