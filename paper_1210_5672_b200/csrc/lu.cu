@@ -980,6 +980,7 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
         SWW_CUDA(cudaGetLastError());
         return SWW_OK;
     }
+    if (ncols == 1 && trsv_cluster_supported(N)) return run_trsv_cluster(d, B, Blo);
     if (ncols <= 8) return launch_trsm<8>(d, B, Blo, 1);
     for (int c0 = 0; c0 < ncols; c0 += TR_MAXNS * 32) {
         const int nc = std::min(ncols - c0, TR_MAXNS * 32);
