@@ -32,7 +32,7 @@ METRIC = "DtN RHS-columns/sec at N=2048 (fp64)"
 UNIT = "columns/s"
 N_METRIC, NRHS_METRIC, NRHS_DD = 2048, 512, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (None = not captured yet)
-TRAFFIC_NCU = {"lu": None, "trsm": None, "gemm_dmma": None}
+TRAFFIC_NCU = {"lu": 33.63e6, "trsm": 42.82e6, "gemm_dmma": 51.18e6}  # profiles/r1c_summary.md (trsm: the 512-column batch launch)
 NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # blackwell_cuda_programming.md: B200 FP64 tensor 45 TFLOP/s, bf16 dense 2250 TFLOP/s
 
 
@@ -260,8 +260,8 @@ def main():
     peaks = measured_peaks()
     peak_tf = peaks["bf16_tflops"] * NOMINAL_FP64_OVER_BF16
     probe = {"dfma_tflops": sww.probe_fp64_peak(0) / 1e12, "dmma_tflops": sww.probe_fp64_peak(1) / 1e12}
-    names = {"lu": "k_lu_dataflow (persistent DMMA.8x8x4 tile dataflow, one launch)",
-             "trsm": "k_trsm_dataflow (persistent DMMA.8x8x4 multi-RHS triangular solves: 2 base-state launches + 1 batch launch)",
+    names = {"lu": "k_lu_dataflow (block LU in one persistent launch: spine CTA with Gauss-Jordan inverses of the 64x64 Schur blocks, DMMA.8x8x4 tile workers)",
+             "trsm": "k_trsm_dataflow (persistent DMMA.8x8x4 multi-RHS triangular solves, 1 launch for the batch) + k_trsv_cluster (16-CTA cluster, 2 single-column base-state solves)",
              "gemm_dmma": "k_gemm_f64 (DMMA.8x8x4): G product"}
     per_kernel = {}
     for cls in ("lu", "trsm", "gemm_dmma"):
