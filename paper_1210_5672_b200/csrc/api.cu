@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/sww.h: handle management, right-hand-side formation (S3), the DtN apply (S4-S6), the base
 // state (2.9) and the linearized DtN (B.1d),(B.2).  Product code; shares nothing with oracle/.
 #include "common.cuh"
+#include <algorithm>
 #include "dd.cuh"
 #include <new>
 #include <cstring>
@@ -99,7 +100,8 @@ int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_
     alloc(&d->E, 2 * N); alloc(&d->Dm, 2 * N); alloc(&d->Sh, 2 * N); alloc(&d->Ch, 2 * N);
     alloc(&d->K, mat); alloc(&d->G, mat); alloc(&d->LU, n2); alloc(&d->invD, 2 * (size_t)N * nb);
     alloc(&d->bphi, 2 * N); alloc(&d->bW0, 2 * N); alloc(&d->bu, 2 * N); alloc(&d->bv, 2 * N); alloc(&d->tmp, 14 * (size_t)N);
-    d->bp_chunks = N / 32 < 1 ? 1 : (N / 32 > 64 ? 64 : N / 32);
+    // column chunks of the dd base-state pass: enough CTAs to fill the chip at small N (4 columns per chunk at least)
+    d->bp_chunks = std::max(1, std::min(N / 4, std::max(N / 32, 64)));
     alloc(&d->bp_part, (size_t)d->bp_chunks * 4 * N);
     if (ok && cudaMalloc(&d->status, sizeof(int)) != cudaSuccess) ok = false;
     if (ok && (cudaMalloc(&d->mv_count, sizeof(unsigned) * (N / 32 + 1)) != cudaSuccess ||
