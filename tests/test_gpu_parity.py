@@ -233,6 +233,24 @@ def test_zero_columns_and_zero_rhs(sww):
     d.check()
 
 
+@pytest.mark.parametrize("N", [128, 256, 1024, 4096])
+def test_single_column_solver_matches_batch_solver(sww, orc_ld, N):
+    """One right-hand side runs through the cluster kernel (distributed-shared-memory chain), several through the dataflow kernel:
+    the same column must come out of both to rounding, at the smallest tiled size (2 tiles), sizes whose block count is not a
+    multiple of the cluster size, and the largest size the cluster kernel takes; N <= 256 is also checked against the oracle."""
+    c = si.config3(N, 4) if N < 4096 else si.config5(N, 4)
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    cols = to_dev(c.dphi, None, "f64")
+    batch = d.apply(cols).cpu().numpy()
+    single = np.stack([d.apply(cols[i:i + 1].contiguous()).cpu().numpy()[0] for i in range(2)])
+    d.check()
+    scale = np.abs(batch[:2]).max(axis=1, keepdims=True)
+    assert np.abs(single - batch[:2]).max() <= 4.0 * N * 2.0 ** -53 * float(np.abs(c.dphi).max() / scale.min()) * scale.max()
+    if N <= 256:
+        orc = orc_ld.dtn_apply(c.eta, c.h, c.dphi[:2])
+        check_columns((single, None), orc, "f64", N, np.abs(c.dphi[:2]).max(axis=1), f"single N={N}")
+
+
 def test_minimum_size(sww, orc_ld):
     N = 16
     a = np.zeros(4); a[1] = 0.05
