@@ -54,7 +54,10 @@ static int apply_f64(sww_dtn_s* d, const double* rhs_dev /* N x nrhs, or NULL wh
     if (rhs_dev) SWW_CUDA(cudaMemcpyAsync(w.B, rhs_dev, sizeof(double) * (size_t)N * nrhs, cudaMemcpyDeviceToDevice, d->stream));
     SWW_TRY(run_solve(d, w.B, w.S, nrhs));                                       // S4: mu = A^{-1} b
     SWW_TRY(spectral_gamma_w(d, w.B, Tcols, w.Gam, out, nrhs, nrhs));           // S5: gamma = D mu ; out = |D| mu / 2 - D t
-    SWW_TRY(gemm_f64(d->stream, N, nrhs, N, 1.0, d->G, N, w.Gam, N, 1.0, out, N, nrhs));  // S6: out += G gamma   (2.8)
+    if (nrhs <= 4 && N >= 128 && (size_t)d->bp_chunks * 4 >= 16)  // S6: out += G gamma   (2.8)
+        SWW_TRY(gemv_few_f64(d->stream, N, nrhs, N, d->G, N, w.Gam, N, out, N, d->bp_part, d->mv_count));
+    else
+        SWW_TRY(gemm_f64(d->stream, N, nrhs, N, 1.0, d->G, N, w.Gam, N, 1.0, out, N, nrhs));
     return SWW_OK;
 }
 

@@ -124,6 +124,9 @@ struct Epi {
 };
 int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* A, int lda, const double* B, int ldb,
              double beta, double* C, int ldc, int n_valid, Epi epi = Epi());
+// C[M x nc] += A B for nc <= 4 columns as a streamed GEMV (gemm.cu); part / count: the handle's bp_part / mv_count
+int gemv_few_f64(cudaStream_t st, int M, int nc, int K, const double* A, int lda, const double* B, int ldb, double* C, int ldc, double* part,
+                 unsigned* count);
 // accurate base state (ddpath.cu): phi0', W0, u, v of (2.9) with mu0 refined to dd; phi0 is dd planar iff prec == SWW_DD
 int accurate_base(sww_dtn_s* d, const double* phi0);
 // fused dd pass (assembly.cu): res = b - mu/2 - K mu, w = G gam with the kernel entries evaluated in dd on the fly; all dd planar 2N

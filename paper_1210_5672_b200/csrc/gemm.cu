@@ -202,4 +202,76 @@ int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* 
     return launch_gemm<64, 64, 16, 2, 2, 3>(st, M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid, epi);
 }
 
+// ------------------------------------------------------------------------------------------------ few columns: C += A B as a GEMV
+// A stage of the time stepper without variational columns applies G to ONE vector: the tiled kernel would run 8 CTAs over a
+// 33 MB matrix.  Here the matrix is streamed once by (M / 32) x ny CTAs: block = 8 warps x 32 rows, warp q takes the columns
+// j = q (mod 8) of its block's column range, eight loads in flight per thread; the ny partial sums of a row block are combined by
+// the last CTA to arrive (counter per row block, left at zero), in a fixed order -- the result is deterministic.
+template <int NC>
+__global__ void __launch_bounds__(256) k_gemv_few(int M, int K, const double* __restrict__ A, int lda, const double* __restrict__ B, int ldb,
+                                                  double* __restrict__ C, int ldc, double* __restrict__ part, unsigned* __restrict__ count) {
+    __shared__ double red[8][NC][32];
+    __shared__ unsigned s_last;
+    const int lane = threadIdx.x & 31, q = threadIdx.x >> 5;
+    const int i = blockIdx.x * 32 + lane;
+    const int ny = gridDim.y, jn = K / ny, jb = blockIdx.y * jn, je = jb + jn;
+    double acc[NC];
+#pragma unroll
+    for (int c = 0; c < NC; c++) acc[c] = 0.0;
+    for (int j0 = jb + q; j0 < je; j0 += 64) {
+        double a[8];
+#pragma unroll
+        for (int u = 0; u < 8; u++) a[u] = (j0 + 8 * u < je) ? A[(size_t)(j0 + 8 * u) * lda + i] : 0.0;
+#pragma unroll
+        for (int u = 0; u < 8; u++) {
+            const int j = min(j0 + 8 * u, je - 1);
+#pragma unroll
+            for (int c = 0; c < NC; c++) acc[c] = fma(a[u], B[(size_t)c * ldb + j], acc[c]);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < NC; c++) red[q][c][lane] = acc[c];
+    __syncthreads();
+    if (q != 0) return;
+#pragma unroll
+    for (int c = 0; c < NC; c++)
+        for (int w = 1; w < 8; w++) acc[c] += red[w][c][lane];
+    if (ny > 1) {
+#pragma unroll
+        for (int c = 0; c < NC; c++) part[((size_t)blockIdx.y * NC + c) * M + i] = acc[c];
+        __threadfence();
+        __syncwarp();
+        if (lane == 0) s_last = (atomicAdd(count + blockIdx.x, 1u) == (unsigned)(ny - 1));
+        __syncwarp();
+        if (!s_last) return;
+        __threadfence();
+        if (lane == 0) count[blockIdx.x] = 0;
+#pragma unroll
+        for (int c = 0; c < NC; c++) {
+            acc[c] = 0.0;
+            for (int y = 0; y < ny; y++) acc[c] += __ldcg(part + ((size_t)y * NC + c) * M + i);
+        }
+    }
+#pragma unroll
+    for (int c = 0; c < NC; c++) C[(size_t)c * ldc + i] += acc[c];
+}
+
+// C[M x nc] += A[M x K] B[K x nc], nc <= 4, M a multiple of 32, K a multiple of 64 ny; part: >= 4 * 4 * M doubles, count: M / 32
+// zeroed counters (both owned by the handle)
+int gemv_few_f64(cudaStream_t st, int M, int nc, int K, const double* A, int lda, const double* B, int ldb, double* C, int ldc, double* part,
+                 unsigned* count) {
+    const int ny = (K % 256 == 0 && M >= 256) ? 4 : 1;
+    dim3 grid(M / 32, ny);
+    SWW_BEGIN(KC_GEMM, st);
+    switch (nc) {
+        case 1: k_gemv_few<1><<<grid, 256, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, part, count); break;
+        case 2: k_gemv_few<2><<<grid, 256, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, part, count); break;
+        case 3: k_gemv_few<3><<<grid, 256, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, part, count); break;
+        default: k_gemv_few<4><<<grid, 256, 0, st>>>(M, K, A, lda, B, ldb, C, ldc, part, count); break;
+    }
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
 }  // namespace sww
