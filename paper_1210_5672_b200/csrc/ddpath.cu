@@ -159,19 +159,23 @@ static int matvec_dd(sww_dtn_s* d, const double* A, const double* Alo, const dou
 // ------------------------------------------------------------------------------------------------ dd GEMM (many columns)
 // Y = zs * Z + beta * X + alpha * (A X): A dd (or fp64) N x N, X, Z, Y dd planar N x ncols (plane size L = N * ld_cols).
 // CTA tile 64 rows x 32 columns, 256 threads, thread tile 4 x 2 (rows ty + 16 r, columns tx + 16 c), k-slab 16.
-constexpr int DG_BM = 64, DG_BN = 32, DG_BK = 16;
+// CN = columns per thread: 2 (tile 64 x 32) or 1 (tile 64 x 16, used when the wider tile would leave fewer than two CTAs per SM:
+// the k-slabs are loaded synchronously, so a second resident CTA is what hides the load latency).
+constexpr int DG_BM = 64, DG_BK = 16;
+template <int CN>
 __global__ void __launch_bounds__(256) k_gemm_dd(int N, int ncols, size_t L, const double* __restrict__ A, const double* __restrict__ Alo,
                                                  const double* __restrict__ X, double zs, const double* __restrict__ Z, double beta,
                                                  double alpha, double* __restrict__ Y, double* __restrict__ Y_f64) {
     __shared__ double As_hi[DG_BK][DG_BM], As_lo[DG_BK][DG_BM];
+    constexpr int DG_BN = 16 * CN;
     __shared__ double Xs_hi[DG_BN][DG_BK + 1], Xs_lo[DG_BN][DG_BK + 1];
     const int tid = threadIdx.x, ty = tid & 15, tx = tid >> 4;
     const int i0 = blockIdx.x * DG_BM, c0 = blockIdx.y * DG_BN;
-    dd acc[4][2];
+    dd acc[4][CN];
 #pragma unroll
     for (int r = 0; r < 4; r++)
 #pragma unroll
-        for (int c = 0; c < 2; c++) acc[r][c] = dd{0.0, 0.0};
+        for (int c = 0; c < CN; c++) acc[r][c] = dd{0.0, 0.0};
     for (int k0 = 0; k0 < N; k0 += DG_BK) {
         for (int e = tid; e < DG_BK * DG_BM; e += 256) {
             int kk = e / DG_BM, ii = e % DG_BM;
@@ -190,20 +194,20 @@ __global__ void __launch_bounds__(256) k_gemm_dd(int N, int ncols, size_t L, con
         __syncthreads();
 #pragma unroll 4
         for (int kk = 0; kk < DG_BK; kk++) {
-            dd a[4], x[2];
+            dd a[4], x[CN];
 #pragma unroll
             for (int r = 0; r < 4; r++) a[r] = dd{As_hi[kk][ty + 16 * r], As_lo[kk][ty + 16 * r]};
 #pragma unroll
-            for (int c = 0; c < 2; c++) x[c] = dd{Xs_hi[tx + 16 * c][kk], Xs_lo[tx + 16 * c][kk]};
+            for (int c = 0; c < CN; c++) x[c] = dd{Xs_hi[tx + 16 * c][kk], Xs_lo[tx + 16 * c][kk]};
 #pragma unroll
             for (int r = 0; r < 4; r++)
 #pragma unroll
-                for (int c = 0; c < 2; c++) acc[r][c] = dd_fma(a[r], x[c], acc[r][c]);
+                for (int c = 0; c < CN; c++) acc[r][c] = dd_fma(a[r], x[c], acc[r][c]);
         }
         __syncthreads();
     }
 #pragma unroll
-    for (int c = 0; c < 2; c++) {
+    for (int c = 0; c < CN; c++) {
         int col = c0 + tx + 16 * c;
         if (col >= ncols) continue;
 #pragma unroll
@@ -226,9 +230,14 @@ static int gemm_dd(sww_dtn_s* d, int ncols, size_t L, const double* A, const dou
     if (N < DG_BM) {  // tiny N: column by column through the mat-vec kernel (planes are L apart, so repack is not needed when ncols == 1)
         return SWW_EINVAL;
     }
-    dim3 grid(N / DG_BM, (ncols + DG_BN - 1) / DG_BN);
+    const bool narrow = (long)(N / DG_BM) * ((ncols + 31) / 32) < 2 * 148;
+    const int bn = narrow ? 16 : 32;
+    dim3 grid(N / DG_BM, (ncols + bn - 1) / bn);
     SWW_BEGIN(KC_DDGEMM, d->stream);
-    k_gemm_dd<<<grid, 256, 0, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
+    if (narrow)
+        k_gemm_dd<1><<<grid, 256, 0, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
+    else
+        k_gemm_dd<2><<<grid, 256, 0, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
