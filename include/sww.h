@@ -114,7 +114,8 @@ int sww_probe_fp64_peak(int which, double* flops_per_s);
  * Same computation as setup + set_base + linearized_apply, but every array is a HOST pointer (pinned or pageable);
  * the call copies inputs to the device, runs the device path, copies the result back and synchronises.  The library keeps ONE
  * cached context (handle + device staging buffers) between calls, reused while N and prec stay the same (a caller stepping a
- * surface calls this once per stage); it runs on the default stream and is not thread-safe.  sww_host_cache_clear() frees the
+ * surface calls this once per stage); it runs on the default stream (the batch columns are uploaded on an internal second
+ * stream while setup and base state run, so pinned host buffers make the upload free) and is not thread-safe.  sww_host_cache_clear() frees the
  * cached context (it is also dropped after any failing call). */
 int sww_dtn_linearized_host(const void* eta, const void* phi0, const void* deta, const void* dphi, void* out,
                             int N, double h, int prec, int nrhs);

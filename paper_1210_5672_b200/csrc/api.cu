@@ -229,8 +229,13 @@ struct HostCtx {
     int N = 0, prec = -1;
     size_t cap = 0;  // staging capacity in bytes of one batch buffer
     double *de = nullptr, *dp = nullptr, *dde = nullptr, *ddp = nullptr, *dout = nullptr;
+    cudaStream_t copy_st = nullptr;  // the batch columns are uploaded here while setup + base state run on the compute stream
+    cudaEvent_t in_ev = nullptr;
 } g_host;
 void host_ctx_free() {
+    if (g_host.copy_st) cudaStreamSynchronize(g_host.copy_st);
+    if (g_host.in_ev) cudaEventDestroy(g_host.in_ev);
+    if (g_host.copy_st) cudaStreamDestroy(g_host.copy_st);
     if (g_host.h) sww_dtn_destroy(g_host.h);
     cudaFree(g_host.de); cudaFree(g_host.dp); cudaFree(g_host.dde); cudaFree(g_host.ddp); cudaFree(g_host.dout);
     g_host = HostCtx();
@@ -262,8 +267,15 @@ int sww_dtn_linearized_host(const void* eta, const void* phi0, const void* deta,
         if (cudaMalloc(&c.dde, bat) || cudaMalloc(&c.ddp, bat) || cudaMalloc(&c.dout, bat)) { host_ctx_free(); return SWW_ENOMEM; }
         c.cap = bat;
     }
+    if (!c.copy_st && (cudaStreamCreateWithFlags(&c.copy_st, cudaStreamNonBlocking) || cudaEventCreateWithFlags(&c.in_ev, cudaEventDisableTiming))) {
+        host_ctx_free();
+        return SWW_ECUDA;
+    }
+    // the surface and the base potential go first on the compute stream; the batch (the bulk of the bytes) is uploaded on a
+    // second stream behind them and is only waited for where it is first read, after setup and the base state
     if (cudaMemcpyAsync(c.de, eta, vec, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(c.dp, phi0, vec, cudaMemcpyHostToDevice, st) ||
-        cudaMemcpyAsync(c.dde, deta, bat, cudaMemcpyHostToDevice, st) || cudaMemcpyAsync(c.ddp, dphi, bat, cudaMemcpyHostToDevice, st))
+        cudaMemcpyAsync(c.dde, deta, bat, cudaMemcpyHostToDevice, c.copy_st) || cudaMemcpyAsync(c.ddp, dphi, bat, cudaMemcpyHostToDevice, c.copy_st) ||
+        cudaEventRecord(c.in_ev, c.copy_st))
         return note_cuda(cudaGetLastError(), "host staging copies");
     int rc;
     if (!c.h) {
@@ -274,9 +286,11 @@ int sww_dtn_linearized_host(const void* eta, const void* phi0, const void* deta,
         rc = sww_dtn_refactor(c.h, c.de);
     }
     if (!rc) rc = sww_dtn_set_base(c.h, c.dp);
+    if (cudaStreamWaitEvent(st, c.in_ev, 0) && !rc) rc = SWW_ECUDA;  // always waited for: the staging buffers must be idle on return
     if (!rc) rc = sww_dtn_linearized_apply(c.h, c.dde, c.ddp, nrhs, c.dout);
     if (!rc && cudaMemcpyAsync(out, c.dout, bat, cudaMemcpyDeviceToHost, st)) rc = SWW_ECUDA;
     if (!rc) rc = sww_dtn_status(c.h);  // synchronises
+    else cudaStreamSynchronize(c.copy_st);
     if (rc) {  // a sticky device status (EBOTTOM, ESINGULAR) must not leak into the next call
         int keep = rc;
         host_ctx_free();
