@@ -158,18 +158,18 @@ __device__ __forceinline__ void sinhcosh_f64(double y, double* sh, double* ch) {
 constexpr int ASM_TI = 128;  // rows (targets i) per block = threads per block
 constexpr int ASM_TJ = 32;   // columns (sources j) per block
 
-template <bool FINITE>
+template <bool FINITE, int TJ>
 __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __restrict__ eta, const double* __restrict__ d1,
                                                          const double* __restrict__ d2, const double* __restrict__ E,
                                                          const double* __restrict__ Dm, const double* __restrict__ cs,
                                                          const double* __restrict__ sn, const double* __restrict__ c0,
                                                          const double* __restrict__ s2, double* __restrict__ K,
                                                          double* __restrict__ G, double* __restrict__ LU) {
-    __shared__ double s_eta[ASM_TJ], s_d1[ASM_TJ], s_E[ASM_TJ], s_Dm[ASM_TJ];
-    __shared__ double s_cs[ASM_TI + ASM_TJ], s_sn[ASM_TI + ASM_TJ], s_c0[ASM_TI + ASM_TJ], s_s2[ASM_TI + ASM_TJ];
+    __shared__ double s_eta[TJ], s_d1[TJ], s_E[TJ], s_Dm[TJ];
+    __shared__ double s_cs[ASM_TI + TJ], s_sn[ASM_TI + TJ], s_c0[ASM_TI + TJ], s_s2[ASM_TI + TJ];
     const int tid = threadIdx.x, mask = N - 1;
-    const int i0 = blockIdx.x * ASM_TI, j0 = blockIdx.y * ASM_TJ;
-    if (tid < ASM_TJ) {
+    const int i0 = blockIdx.x * ASM_TI, j0 = blockIdx.y * TJ;
+    if (tid < TJ) {
         int j = (j0 + tid) & mask;
         s_eta[tid] = eta[j];
         s_d1[tid] = d1[j];
@@ -179,8 +179,8 @@ __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __
         }
     }
     // table slice: index s <-> m = (i0 - j0 - (TJ-1) + s) mod N, s = tid - jj + TJ - 1
-    for (int s = tid; s < ASM_TI + ASM_TJ - 1; s += ASM_TI) {
-        int m = (i0 - j0 - (ASM_TJ - 1) + s) & mask;
+    for (int s = tid; s < ASM_TI + TJ - 1; s += ASM_TI) {
+        int m = (i0 - j0 - (TJ - 1) + s) & mask;
         s_cs[s] = cs[m];
         s_sn[s] = sn[m];
         s_c0[s] = c0[m];
@@ -192,9 +192,9 @@ __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __
     const double eta_i = eta[i], d1_i = d1[i], d2_i = d2[i];
     const double E_i = FINITE ? E[i] : 0.0, Dm_i = FINITE ? Dm[i] : 0.0;
     const double rN = 1.0 / (double)N;
-    const int jmax = min(ASM_TJ, N - j0);
+    const int jmax = min(TJ, N - j0);
     for (int jj = 0; jj < jmax; jj++) {
-        const int j = j0 + jj, s = tid - jj + ASM_TJ - 1;
+        const int j = j0 + jj, s = tid - jj + TJ - 1;
         const double sx = s_sn[s], cx = s_cs[s], d1_j = s_d1[jj];
         double k1, g1;
         if (i != j) {
@@ -450,12 +450,18 @@ int run_setup_f64(sww_dtn_s* d) {
     SWW_TRY(run_node_prep(d));
     const int N = d->N;
     const Tables* t = d->tab;
-    dim3 grid((N + ASM_TI - 1) / ASM_TI, (N + ASM_TJ - 1) / ASM_TJ);
+    // sources per CTA: 32, or 4 at small N (N = 256 would otherwise run on 16 CTAs)
+    const int tj = (N <= 512) ? 4 : ASM_TJ;
+    dim3 grid((N + ASM_TI - 1) / ASM_TI, (N + tj - 1) / tj);
     SWW_BEGIN(KC_ASM, d->stream);
-    if (d->finite)
-        k_assemble_f64<true><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
-    else
-        k_assemble_f64<false><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
+#define SWW_ASM_LAUNCH(FIN, TJV) \
+    k_assemble_f64<FIN, TJV><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU)
+    if (d->finite) {
+        if (tj == 4) SWW_ASM_LAUNCH(true, 4); else SWW_ASM_LAUNCH(true, ASM_TJ);
+    } else {
+        if (tj == 4) SWW_ASM_LAUNCH(false, 4); else SWW_ASM_LAUNCH(false, ASM_TJ);
+    }
+#undef SWW_ASM_LAUNCH
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

@@ -129,6 +129,8 @@ int gemv_few_f64(cudaStream_t st, int M, int nc, int K, const double* A, int lda
                  unsigned* count);
 // accurate base state (ddpath.cu): phi0', W0, u, v of (2.9) with mu0 refined to dd; phi0 is dd planar iff prec == SWW_DD
 int accurate_base(sww_dtn_s* d, const double* phi0);
+// the plain fp64 base state (fp64 handles only; see ddpath.cu for when the stepper may use it)
+int fast_base_f64(sww_dtn_s* d, const double* phi0);
 // fused dd pass (assembly.cu): res = b - mu/2 - K mu, w = G gam with the kernel entries evaluated in dd on the fly; all dd planar 2N
 int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* gam, double* res, double* res_f64, double* w);
 // spectral (fft.cu)

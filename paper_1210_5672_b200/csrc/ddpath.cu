@@ -484,6 +484,43 @@ int accurate_base(sww_dtn_s* d, const double* phi0) {
     return SWW_OK;
 }
 
+// ------------------------------------------------------------------------------------------------ plain fp64 base state
+// (2.9) for a state that is NOT linearized about: phi0', W0 = G phi0, u, v straight from the fp64 pipeline (one solve, one
+// spectral pass, one product with G), written as dd pairs with zero low words.  The time stepper without variational columns
+// uses it for N <= 1024: there u, v enter the right-hand sides of (2.1) only, nothing differentiates them a second time, and the
+// rounding noise of the first-order operator (~2 N eps) stays three digits under the parity bar (SURVEY.md section 0, fact 4:
+// fp64 against long double over config 2's full period: 3e-14 / 2e-13).
+__global__ void k_base_uv_f64(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* __restrict__ W0,
+                              double* __restrict__ bphi, double* __restrict__ bW0, double* __restrict__ u, double* __restrict__ v) {
+    int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    const double e1 = d1[j], p = dphi[j], w = W0[j];
+    const double rden = 1.0 / fma(e1, e1, 1.0);
+    bphi[j] = p;       bphi[N + j] = 0.0;
+    bW0[j] = w;        bW0[N + j] = 0.0;
+    u[j] = (p - e1 * w) * rden;       u[N + j] = 0.0;
+    v[j] = fma(e1, p, w) * rden;      v[N + j] = 0.0;
+}
+
+int fast_base_f64(sww_dtn_s* d, const double* phi0) {
+    const int N = d->N;
+    cudaStream_t st = d->stream;
+    Workspace& w = d->ws;
+    SWW_CUDA(cudaMemcpyAsync(w.B, phi0, sizeof(double) * N, cudaMemcpyDeviceToDevice, st));
+    SWW_TRY(run_solve(d, w.B, w.S, 1));                               // mu0
+    SWW_TRY(spectral_gamma_w(d, w.B, nullptr, w.Gam, w.W, 1, 1));     // gamma = D mu0 ; W = |D| mu0 / 2
+    if (N >= 128 && (size_t)d->bp_chunks * 4 >= 16)
+        SWW_TRY(gemv_few_f64(st, N, 1, N, d->G, N, w.Gam, N, w.W, N, d->bp_part, d->mv_count));
+    else
+        SWW_TRY(gemm_f64(st, N, 1, N, 1.0, d->G, N, w.Gam, N, 1.0, w.W, N, 1));
+    SWW_TRY(spectral_deriv(d, phi0, w.T, 1));                          // phi0'
+    SWW_BEGIN(KC_OTHER, st);
+    k_base_uv_f64<<<(N + 255) / 256, 256, 0, st>>>(N, d->d1, w.T, w.W, d->bphi, d->bW0, d->bu, d->bv);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ flow (2): dd apply
 // rhs: dd planar N x nrhs with plane size Lin (ignored when rhs_in_ws: ws.B (dd) and ws.R (fp64 rounding) are already filled).
 // Tcols: dd planar in ws layout or nullptr.  out: dd planar N x nrhs, plane size Lout = N * nrhs.

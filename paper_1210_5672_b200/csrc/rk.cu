@@ -246,7 +246,13 @@ static int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
     const double* eta = ys;
     const double* phi = ys + N;
     SWW_TRY(sww_dtn_refactor(d, eta));   // S0-S2 for this stage's surface
-    SWW_TRY(sww_dtn_set_base(d, phi));   // W0 = G phi, u, v of (2.9)
+    if (nc == 0 && N <= 1024 && d->prec == SWW_F64) {  // nothing is linearized about this state: the plain fp64 base state (ddpath.cu)
+        SWW_TRY(ensure_workspace(d, 1));
+        SWW_TRY(fast_base_f64(d, phi));
+        d->has_base = true;
+    } else {
+        SWW_TRY(sww_dtn_set_base(d, phi));   // W0 = G phi, u, v of (2.9)
+    }
     const Tables* t = d->tab;
     SWW_BEGIN(KC_FFT, st);
     k_rhs_base<<<1, thr, sizeof(double2) * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->g, eta, d->bW0, d->bu, d->bv, kout,
