@@ -763,7 +763,7 @@ __device__ __forceinline__ void two_sum_d(double a, double b, double& s, double&
 
 template <int WS>
 struct TrsmCfg {
-    static constexpr int WC = (WS >= 32) ? 4 : 1;   // warps across the slab's columns (8 columns per warp)
+    static constexpr int WC = WS / 8;               // warps across the slab's columns (8 columns per warp): 1, 2 or 4
     static constexpr int WR = 8 / WC;               // warps across the 64 rows
     static constexpr int FM = (TS / WR) / 8;        // 8 x 8 fragments per warp along the rows
     static constexpr int WSP = WC * 8;              // columns covered = WS
@@ -981,10 +981,21 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
         return SWW_OK;
     }
     if (ncols == 1 && trsv_cluster_supported(N)) return run_trsv_cluster(d, B, Blo);
-    if (ncols <= 8) return launch_trsm<8>(d, B, Blo, 1);
-    for (int c0 = 0; c0 < ncols; c0 += TR_MAXNS * 32) {
-        const int nc = std::min(ncols - c0, TR_MAXNS * 32);
-        SWW_TRY(launch_trsm<32>(d, B + (size_t)c0 * N, Blo + (size_t)c0 * N, (nc + 31) / 32));
+    // slab width: the chain of a slab is 2 N/64 links of (flag hop + one or two 64 x 64 x WS products), so narrow slabs finish
+    // sooner as long as there are few of them; every slab re-reads the factors from L2, so many columns want wide slabs
+    // (measured at N = 2048: 128 columns 0.19 ms with 16-column slabs against 0.27 ms with 32; 512 columns 0.36 against 0.34)
+    static int ws_env = -1;
+    if (ws_env < 0) ws_env = getenv("SWW_TRSM_WS") ? atoi(getenv("SWW_TRSM_WS")) : 0;
+    const int ws = ws_env ? ws_env : (ncols <= 64 ? 8 : (ncols <= 256 ? 16 : 32));
+    for (int c0 = 0; c0 < ncols; c0 += TR_MAXNS * ws) {
+        const int nc = std::min(ncols - c0, TR_MAXNS * ws);
+        double *b = B + (size_t)c0 * N, *bl = Blo + (size_t)c0 * N;
+        if (ws == 8)
+            SWW_TRY(launch_trsm<8>(d, b, bl, (nc + 7) / 8));
+        else if (ws == 16)
+            SWW_TRY(launch_trsm<16>(d, b, bl, (nc + 15) / 16));
+        else
+            SWW_TRY(launch_trsm<32>(d, b, bl, (nc + 31) / 32));
     }
     return SWW_OK;
 }
