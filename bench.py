@@ -261,7 +261,7 @@ def main():
     peak_tf = peaks["bf16_tflops"] * NOMINAL_FP64_OVER_BF16
     probe = {"dfma_tflops": sww.probe_fp64_peak(0) / 1e12, "dmma_tflops": sww.probe_fp64_peak(1) / 1e12}
     names = {"lu": "k_lu_dataflow (block LU in one persistent launch: spine CTA with Gauss-Jordan inverses of the 64x64 Schur blocks, DMMA.8x8x4 tile workers)",
-             "trsm": "k_trsm_dataflow (persistent DMMA.8x8x4 multi-RHS triangular solves, 1 launch for the batch) + k_trsv_cluster (16-CTA cluster, 2 single-column base-state solves)",
+             "trsm": "k_trsm_dataflow (persistent DMMA.8x8x4 multi-RHS triangular solves, tasks handing blocks over through L2 with the data as the flag: 2 base-state launches + 1 batch launch)",
              "gemm_dmma": "k_gemm_f64 (DMMA.8x8x4): G product"}
     per_kernel = {}
     for cls in ("lu", "trsm", "gemm_dmma"):

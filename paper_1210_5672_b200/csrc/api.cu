@@ -200,6 +200,7 @@ int sww_dtn_destroy(sww_dtn_t d) {
     cudaFree(d->lu_order);
     cudaFree(d->lu_flags);
     cudaFree(d->tr_flags);
+    cudaFree(d->tr_scr);
     cudaFree(d->lu_trace);
     delete d;
     return SWW_OK;

@@ -84,6 +84,8 @@ struct sww_dtn_s {
     int lu_ntasks;
     unsigned* tr_flags;   // dataflow TRSM: claim counter (slot 0) + flags[2][N/64][slabs]
     unsigned tr_epoch;
+    double* tr_scr;       // dataflow TRSM: forward (hi, lo) and backward (hi) results, the hand-over buffers between tasks
+    size_t tr_scr_cap;    // doubles
     unsigned long long* lu_trace;  // debugging aid (env SWW_LU_TRACE): per-task time stamps of the dataflow LU
     // base state (dd planar 2N each): phi0', W0, u, v
     double *bphi, *bW0, *bu, *bv;
@@ -112,9 +114,6 @@ int run_lu(sww_dtn_s* d);
 // multi-RHS triangular solves with the factors in d->LU; B is N x ncols (ld = N), in place; Blo (same shape) receives the
 // low word of the compensated solution (B already holds RN(B + Blo)); Blo's incoming content is ignored
 int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols);
-// one column as one 8-CTA cluster passing the solution blocks through distributed shared memory (trsv.cu)
-bool trsv_cluster_supported(int N);
-int run_trsv_cluster(sww_dtn_s* d, double* B, double* Blo);
 // GEMM (gemm.cu): C[M x Nc] = alpha * A[M x K] * B[K x Nc] + beta * C, all column-major fp64; C may alias A or B only in the
 // panel patterns documented in gemm.cu.  n_valid: columns >= n_valid are not stored.
 struct Epi {

@@ -737,9 +737,14 @@ __global__ void __launch_bounds__(64) k_solve_small(int N, const double* __restr
 // Solve L Y = B, then U X = Y (block LU of k_lu_dataflow), for a batch of columns, in place, as ONE persistent kernel in the
 // same style.  A task is (phase, row block i, column slab s of WS columns).  Forward:  Y_i = B_i - sum_{k<i} L_ik Y_k;
 // backward:  X_i = (2 I + F_i)(Y_i - sum_{k>i} U_ik X_k),  2 I + F_i = inv(S_i).  The sums run left-looking in DMMA fragments over the blocks that are
-// already final (acquire-polled flags per (phase, k, s)); the chain of a slab is sequential in i, different slabs and the
-// accumulation over old blocks run in parallel.  Tasks are claimed in dependency order (forward i ascending, then backward i
-// descending), so a claimed task only waits for tasks claimed earlier.
+// already final; the chain of a slab is sequential in i, different slabs and the accumulation over old blocks run in parallel.
+// Tasks are claimed in dependency order (forward i ascending, then backward i descending), so a claimed task only waits for
+// tasks claimed earlier.
+// Hand-over between tasks: THE DATA IS THE FLAG.  The forward results go to Yh / Yl and the backward results to Xh, scratch
+// buffers filled with an all-ones bit pattern (a NaN no computation produces) before the launch; a consumer loads the block
+// it needs (cp.async.cg / ld.cg, i.e. from L2) and simply reloads while any entry still shows the pattern.  Every entry is one
+// aligned 8-byte store, so it is either absent or final: no fence, no release/acquire pair, no separate flag -- a link of the
+// chain costs one store-to-L2 plus one load-from-L2 latency instead of store + fence + flag + poll + load (~2 us).
 // Accuracy: the O(1) vectors are carried as hi + lo (B + Blo).  P = sum L_ik Y_k is accumulated from zero (its terms are
 // O(1/N)) and folded into a two-sum (hi, lo) pair every TR_FOLD blocks; B_i - P and the diagonal-block products are added by
 // error-free two-sums, so each block of the result is the correctly rounded sum plus a remainder word -- the density is
@@ -749,10 +754,12 @@ struct TrsmArgs {
     const double *Es, *Fs;
     double *B, *Blo;     // N x (ns*WS) column-major, ld = N; in: right-hand sides (Blo ignored), out: solution hi, lo
     int N, nt, ns;       // nt row blocks of 64, ns column slabs
-    unsigned* flags;     // [2][nt][ns]
-    unsigned epoch;
+    double *Yh, *Yl, *Xh;  // scratch, same shape as B: forward result (hi, lo) and backward result (hi); pre-filled with TR_ABSENT
     unsigned* counter;
+    int* status;
 };
+constexpr long long TR_ABSENT = -1LL;       // bit pattern of "not written yet" (cudaMemset 0xFF)
+constexpr int TR_SPIN_LIMIT = 1 << 22;      // reloads before a task gives up (inputs that contain the pattern itself): SWW_ECUDA
 constexpr int TR_FOLD = 4;
 
 __device__ __forceinline__ void two_sum_d(double a, double b, double& s, double& e) {
@@ -777,12 +784,10 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
     double* sA = tr_sm;                    // 2 stages of the factor tile as As[k][r]
     double* sD = sA + 2 * TS * LDO;        // the diagonal block F_i of the backward sweep, as As[k][r]
     double* sB = sD + TS * LDO;            // 2 stages of the solution tile as Bs[n][k]
-    unsigned char* ready = reinterpret_cast<unsigned char*>(sB + 2 * WS * LDO);
     __shared__ int s_task;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wr = warp % C::WR, wc = warp / C::WR, fr = lane >> 2, fk = lane & 3;
     const int N = p.N, nt = p.nt, ns = p.ns;
-    const unsigned epoch = p.epoch;
     const int row0 = wr * (TS / C::WR) + fr;   // + 8 x : row of this lane's fragment element
     const int col0 = wc * 8 + 2 * fk;          // + e   : column within the slab
 
@@ -796,14 +801,11 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
         if (phase) task -= nt * ns;
         const int s = task % ns, i = phase ? nt - 1 - task / ns : task / ns;
         const int m = phase ? nt - 1 - i : i;  // number of finished blocks this one depends on
-        const unsigned* fl = p.flags + (size_t)phase * nt * ns;
-        double* Bg = p.B + (size_t)s * WS * N + (size_t)i * TS;
-        double* Lg = p.Blo + (size_t)s * WS * N + (size_t)i * TS;
+        const size_t blk = (size_t)s * WS * N + (size_t)i * TS;
+        double* Bg = p.B + blk;
+        double* Lg = p.Blo + blk;
+        const double* Vin = phase ? p.Xh : p.Yh;  // the vector this sweep consumes block by block
         auto kblock = [&](int kk) { return phase ? nt - 1 - kk : kk; };
-
-        auto refresh = [&](int from) {
-            for (int t = from + tid; t < m; t += 256) ready[t] = ld_acquire(fl + (size_t)kblock(t) * ns + s) == epoch;
-        };
         // the factors are final before this kernel starts: their tiles are requested one step ahead of the flags, so that
         // only the (small) solution block is loaded behind the flag on the chain of a slab
         auto issueA = [&](int kk, int buf) {
@@ -814,17 +816,28 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 const int col = c >> 5, ch = (c & 31) * 2;
                 cp16(a + col * LDO + ch, Ag + (size_t)col * N + ch);
             }
-            cp_commit();
+        };
+        // true if any of the entries THIS thread requested in issueY is still absent (call after its cp.async group completed)
+        auto absentY = [&](int buf) {
+            const double* b = sB + buf * WS * LDO;
+            bool bad = false;
+            for (int c = tid; c < WS * TS / 2; c += 256) {
+                const int col = c >> 5, ch = (c & 31) * 2;
+                bad |= (__double_as_longlong(b[col * LDO + ch]) == TR_ABSENT) | (__double_as_longlong(b[col * LDO + ch + 1]) == TR_ABSENT);
+            }
+            return bad;
+        };
+        auto give_up = [&]() {
+            if (tid == 0) atomicCAS(p.status, SWW_OK, SWW_ECUDA);
         };
         auto issueY = [&](int kk, int buf) {
             const int k = kblock(kk);
-            const double* Yg = p.B + (size_t)s * WS * N + (size_t)k * TS;          // solution block k of this slab
+            const double* Yg = Vin + (size_t)s * WS * N + (size_t)k * TS;          // solution block k of this slab
             double* b = sB + buf * WS * LDO;
             for (int c = tid; c < WS * TS / 2; c += 256) {
                 const int col = c >> 5, ch = (c & 31) * 2;
                 cp16(b + col * LDO + ch, Yg + (size_t)col * N + ch);
             }
-            cp_commit();
         };
         double acc[C::FM][2];
         auto mma_tile = [&](const double* a, const double* b) {
@@ -838,21 +851,30 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             }
         };
 
-        if (phase) {  // the block's own forward result must be visible before it is read
-            if (tid == 0)
-                while (ld_acquire(p.flags + (size_t)i * ns + s) != epoch) __nanosleep(40);
-            __syncthreads();
-        }
         double bh[C::FM][2], bl[C::FM][2], ph[C::FM][2], pl[C::FM][2];
+        for (int spin = 0;; spin++) {  // backward: the block's own forward result (hi and lo), reloaded until all of it is there
+            bool bad = false;
 #pragma unroll
-        for (int x = 0; x < C::FM; x++)
+            for (int x = 0; x < C::FM; x++)
 #pragma unroll
-            for (int e = 0; e < 2; e++) {
-                const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
-                bh[x][e] = Bg[o];
-                bl[x][e] = phase ? Lg[o] : 0.0;  // the forward sweep starts from plain fp64 right-hand sides
-                acc[x][e] = ph[x][e] = pl[x][e] = 0.0;
+                for (int e = 0; e < 2; e++) {
+                    const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
+                    if (phase) {
+                        bh[x][e] = __ldcg(p.Yh + blk + o);
+                        bl[x][e] = __ldcg(p.Yl + blk + o);
+                        bad |= (__double_as_longlong(bh[x][e]) == TR_ABSENT) | (__double_as_longlong(bl[x][e]) == TR_ABSENT);
+                    } else {
+                        bh[x][e] = Bg[o];
+                        bl[x][e] = 0.0;  // the forward sweep starts from plain fp64 right-hand sides
+                    }
+                    acc[x][e] = ph[x][e] = pl[x][e] = 0.0;
+                }
+            if (!phase || !__syncthreads_or(bad)) break;
+            if (spin > TR_SPIN_LIMIT) {
+                give_up();
+                break;
             }
+        }
         auto fold = [&]() {  // (ph, pl) += acc, error-free; acc = 0
 #pragma unroll
             for (int x = 0; x < C::FM; x++)
@@ -873,25 +895,32 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             }
             cp_commit();
         }
-        if (m > 0) issueA(0, 0);
-        refresh(0);
-        __syncthreads();
+        // The factor tile of step kk + 1 is requested while step kk computes (its buffer was released by the barrier that ended
+        // step kk - 1); the solution block is asked for at its own step (asking one step early did not pay: on the chain it
+        // is never there yet, behind the front the load is hidden by the other resident work).
+        if (m > 0) {
+            issueA(0, 0);
+            cp_commit();
+        }
         for (int kk = 0; kk < m; kk++) {
-            const bool missed = !ready[kk];  // uniform: ready[] is only written before a barrier
-            if (missed) {
-                if (tid == 0)
-                    while (ld_acquire(fl + (size_t)kblock(kk) * ns + s) != epoch) __nanosleep(20);
-                __syncthreads();
-            }
             issueY(kk, kk & 1);
-            if (kk + 1 < m) issueA(kk + 1, (kk + 1) & 1);  // its buffer was released by the barrier that ended step kk - 1
-            if (missed) refresh(kk + 1);                   // look at the later flags while the loads are in flight
+            cp_commit();
             if (kk + 1 < m) {
+                issueA(kk + 1, (kk + 1) & 1);
+                cp_commit();
                 cp_wait<1>();
             } else {
                 cp_wait<0>();
             }
-            __syncthreads();
+            for (int spin = 0; __syncthreads_or(absentY(kk & 1)); spin++) {  // the barrier also makes the tiles visible to all
+                if (spin > TR_SPIN_LIMIT) {
+                    give_up();
+                    break;
+                }
+                issueY(kk, kk & 1);  // not there yet: ask L2 again
+                cp_commit();
+                cp_wait<0>();
+            }
             mma_tile(sA + (kk & 1) * TS * LDO, sB + (kk & 1) * WS * LDO);
             if ((kk % TR_FOLD) == TR_FOLD - 1) fold();
             __syncthreads();
@@ -925,14 +954,16 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 two_sum_d(sc * sh[x][e], acc[x][e], t_, e_);
                 const double lo = fma(sc, sl[x][e], e_);
                 const double hi = __dadd_rn(t_, lo);
-                Bg[o] = hi;
-                Lg[o] = __dsub_rn(lo, __dsub_rn(hi, t_));
+                const double low = __dsub_rn(lo, __dsub_rn(hi, t_));
+                if (phase) {  // x_i: to its consumers, and the result
+                    p.Xh[blk + o] = hi;
+                    Bg[o] = hi;
+                    Lg[o] = low;
+                } else {      // y_i: hi for the forward tasks below, hi and lo for this block's backward task
+                    p.Yh[blk + o] = hi;
+                    p.Yl[blk + o] = low;
+                }
             }
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            st_release(p.flags + ((size_t)phase * nt + i) * ns + s, epoch);
-        }
     }
 }
 
@@ -955,8 +986,20 @@ static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     a.nt = nt;
     a.ns = ns;
     a.counter = d->tr_flags;
-    a.flags = d->tr_flags + 1;
-    a.epoch = ++d->tr_epoch;
+    a.status = d->status;
+    const size_t span = (size_t)N * ns * WS;  // doubles per scratch vector
+    if (d->tr_scr_cap < 3 * span) {
+        SWW_CUDA(cudaStreamSynchronize(d->stream));
+        cudaFree(d->tr_scr);
+        d->tr_scr = nullptr;
+        d->tr_scr_cap = 0;
+        if (cudaMalloc(&d->tr_scr, sizeof(double) * 3 * span) != cudaSuccess) return SWW_ENOMEM;
+        d->tr_scr_cap = 3 * span;
+    }
+    a.Yh = d->tr_scr;
+    a.Yl = d->tr_scr + span;
+    a.Xh = d->tr_scr + 2 * span;
+    SWW_CUDA(cudaMemsetAsync(d->tr_scr, 0xFF, sizeof(double) * 3 * span, d->stream));  // every entry "absent"
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), d->stream));
     const int grid = std::min(sm_count(), 2 * nt * ns);
     SWW_BEGIN(KC_TRSM, d->stream);
@@ -980,7 +1023,6 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
         SWW_CUDA(cudaGetLastError());
         return SWW_OK;
     }
-    if (ncols == 1 && trsv_cluster_supported(N)) return run_trsv_cluster(d, B, Blo);
     // slab width: the chain of a slab is 2 N/64 links of (flag hop + one or two 64 x 64 x WS products), so narrow slabs finish
     // sooner as long as there are few of them; every slab re-reads the factors from L2, so many columns want wide slabs
     // (measured at N = 2048: 128 columns 0.19 ms with 16-column slabs against 0.27 ms with 32; 512 columns 0.36 against 0.34)

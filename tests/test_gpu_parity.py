@@ -235,10 +235,10 @@ def test_zero_columns_and_zero_rhs(sww):
 
 @pytest.mark.parametrize("N", [128, 256, 1024, 4096])
 def test_single_column_solver_matches_batch_solver(sww, orc_ld, N):
-    """One right-hand side runs through the cluster kernel (distributed-shared-memory chain), several through the dataflow kernel:
-    the same column must come out of both to rounding, at the smallest tiled size (2 tiles), sizes whose block count is not a
-    multiple of the cluster size, and the largest size the cluster kernel takes; N <= 256 is also checked against the oracle."""
-    c = si.config3(N, 4) if N < 4096 else si.config5(N, 4)
+    """One right-hand side runs through the 8-column slab instantiation of the dataflow solver, a wider batch through another:
+    the same column must come out of both to rounding, from the smallest tiled size (2 tiles) to N = 4096; N <= 256 is also
+    checked against the oracle."""
+    c = si.config3(N, 80) if N < 4096 else si.config5(N, 80)
     d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
     cols = to_dev(c.dphi, None, "f64")
     batch = d.apply(cols).cpu().numpy()
