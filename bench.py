@@ -32,7 +32,7 @@ METRIC = "DtN RHS-columns/sec at N=2048 (fp64)"
 UNIT = "columns/s"
 N_METRIC, NRHS_METRIC, NRHS_DD = 2048, 512, 128
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the ncu --set full capture under profiles/ (None = not captured yet)
-TRAFFIC_NCU = {"lu": 33.63e6, "trsm": 42.82e6, "gemm_dmma": 51.18e6}  # profiles/r1c_summary.md (trsm: the 512-column batch launch)
+TRAFFIC_NCU = {"lu": 33.63e6, "trsm": 58.79e6, "gemm_dmma": 51.18e6}  # profiles/r1d_summary.md (trsm: the 512-column batch launch)
 NOMINAL_FP64_OVER_BF16 = 45.0 / 2250.0  # blackwell_cuda_programming.md: B200 FP64 tensor 45 TFLOP/s, bf16 dense 2250 TFLOP/s
 
 
