@@ -58,7 +58,12 @@ int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_
 int sww_dtn_refactor(sww_dtn_t d, const void* eta);
 
 /* out_c = G(eta) phi_c, c < nrhs: solve (I/2 + K) mu_c = phi_c (2.7); gamma_c = D mu_c; out_c = H gamma_c / 2 + G gamma_c (2.8)
- * (1/|xi'| = 1 on the uniform grid, R3).  phi, out: DEVICE, N x nrhs; may alias.  Pure: no hidden state. */
+ * (1/|xi'| = 1 on the uniform grid, R3).  phi, out: DEVICE, N x nrhs; may alias.  Pure: no hidden state.
+ * A non-finite input column gives a non-finite output column, spoils the column it shares a complex FFT with (2c and 2c + 1)
+ * and leaves all others untouched.  One bit pattern is reserved:
+ * the triangular solves mark "not computed yet" by the all-ones NaN (0xFFFFFFFFFFFFFFFF), which no arithmetic produces; a
+ * right-hand side that propagates exactly that payload makes the solve give up after a bounded wait with the sticky status
+ * SWW_ECUDA instead of hanging. */
 int sww_dtn_apply(sww_dtn_t d, const void* phi, int nrhs, void* out);
 
 /* Store the state the linearization is taken about: phi0' = D phi0, W0 = G phi0, and the surface velocities of (2.9)

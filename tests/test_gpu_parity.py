@@ -251,6 +251,22 @@ def test_single_column_solver_matches_batch_solver(sww, orc_ld, N):
         check_columns((single, None), orc, "f64", N, np.abs(c.dphi[:2]).max(axis=1), f"single N={N}")
 
 
+def test_nan_column_stays_in_its_column(sww):
+    """a non-finite right-hand side must neither hang the dataflow solves (they poll the data itself) nor leak beyond the column
+    it shares a complex FFT with (columns 2c and 2c + 1 are transformed as one complex vector)"""
+    c = si.config3(256, 8)
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    good = d.apply(to_dev(c.dphi, None, "f64")).cpu().numpy()
+    bad_in = c.dphi.copy()
+    bad_in[2, 17] = np.nan
+    bad_in[4, :] = np.inf
+    out = d.apply(to_dev(bad_in, None, "f64")).cpu().numpy()
+    d.check()
+    for col in (0, 1, 6, 7):
+        assert np.array_equal(out[col], good[col])
+    assert not np.isfinite(out[2]).any() and not np.isfinite(out[4]).any()
+
+
 def test_minimum_size(sww, orc_ld):
     N = 16
     a = np.zeros(4); a[1] = 0.05
