@@ -15,8 +15,14 @@ namespace sww {
 // mode 0: out = D f,  coefficient (1/2)(-1)^m cot(pi m/N)                       (Fourier differentiation, Nyquist symbol 0, R4)
 // mode 1: out = H f,  coefficient (1/N) cot(pi m/N) (1 - (-1)^m) = 4 c0[m]/N for odd m, 0 for even m   (symbol -i sgn k)
 // Both kernels are odd in m, so out_i = sum_{m=1}^{N/2-1} coef[m] (f_{i-m} - f_{i+m}).  One warp per output node.
+// blockIdx.y = 1 (two-vector launches) applies the same circulant to a second, independent vector f2 -> out2.
 __global__ void __launch_bounds__(256) k_circ_dd(int N, int mode, const double* __restrict__ dc, const double* __restrict__ c0,
-                                                 const double* __restrict__ f, double* __restrict__ out) {
+                                                 const double* __restrict__ f, double* __restrict__ out, const double* __restrict__ f2,
+                                                 double* __restrict__ out2) {
+    if (blockIdx.y) {
+        f = f2;
+        out = out2;
+    }
     int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
     if (warp >= N) return;
     int i = warp, mask = N - 1;
@@ -62,7 +68,16 @@ __global__ void __launch_bounds__(256) k_circ_dd(int N, int mode, const double* 
 int circ_dd(sww_dtn_s* d, int mode, const double* in, double* out) {
     const int N = d->N;
     SWW_BEGIN(KC_OTHER, d->stream);
-    k_circ_dd<<<(N * 32 + 255) / 256, 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in, out);
+    k_circ_dd<<<(N * 32 + 255) / 256, 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in, out, nullptr, nullptr);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+// two independent vectors in one launch
+static int circ_dd2(sww_dtn_s* d, int mode, const double* in1, double* out1, const double* in2, double* out2) {
+    const int N = d->N;
+    SWW_BEGIN(KC_OTHER, d->stream);
+    k_circ_dd<<<dim3((N * 32 + 255) / 256, 2), 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in1, out1, in2, out2);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -457,7 +472,7 @@ int accurate_base(sww_dtn_s* d, const double* phi0) {
         SWW_BEGIN(KC_OTHER, st);
         k_dd_axpy_f64<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, 1, rcol, rlo, mu);     // mu~
         SWW_LAUNCHED();
-        SWW_TRY(circ_dd(d, 0, mu, gam));                                                   // gam~ = D mu~
+        SWW_TRY(circ_dd2(d, 0, mu, gam, b, d->bphi));                                      // gam~ = D mu~ ; phi0' = D phi0
         SWW_TRY(base_pass_dd(d, b, mu, gam, res, rcol, wt));
         SWW_TRY(run_solve(d, rcol, rlo, 1));                                               // delta
         SWW_BEGIN(KC_OTHER, st);
@@ -476,7 +491,7 @@ int accurate_base(sww_dtn_s* d, const double* phi0) {
         k_dd_add<<<blocks, 256, 0, st>>>(N, res, wt, d->bW0);                              // W0   (2.8)
         SWW_LAUNCHED();
     }
-    SWW_TRY(circ_dd(d, 0, b, d->bphi));                                                    // phi0'
+    if (isdd) SWW_TRY(circ_dd(d, 0, b, d->bphi));                                          // phi0' (fp64 handles: done with gam~ above)
     SWW_BEGIN(KC_OTHER, st);
     k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, d->bW0, d->bu, d->bv);
     SWW_LAUNCHED();
