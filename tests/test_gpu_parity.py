@@ -51,6 +51,26 @@ def test_flat_symbol_all_modes(sww, h):
     assert err.max() <= 1e-11, err.max()
 
 
+def test_maximum_size_flat_symbol(sww):
+    """N = 8192, the largest size the ABI accepts (128 x 128 tiles in the LU, 128-link solve chains): G cos(kx) = k tanh(kh) cos(kx)
+    on the flat surface for low, middle and near-Nyquist modes, and a wavy surface must still report a clean status"""
+    N, h = 8192, 1.0
+    ks = np.array([1, 2, 3, 17, 500, 2047, 4000])
+    j = np.arange(N)
+    phi = np.cos(2 * np.pi * ((ks[:, None] * j[None, :]) % N) / N)
+    d = sww.DtN(torch.zeros(N, dtype=torch.float64, device="cuda"), h)
+    out = d.apply(torch.from_numpy(phi).cuda()).cpu().numpy()
+    d.check()
+    sym = ks * np.tanh(ks * h)
+    err = np.abs(out - sym[:, None] * phi).max(axis=1) / sym
+    assert err.max() <= 1e-11, err
+    a, _ = si._family_surface(si.SEED_BASE + 3, N, 0.2, kmax=64)
+    d.refactor(torch.from_numpy(si.synth(N, a)[0]).cuda())
+    w = d.apply(torch.from_numpy(phi[:2]).cuda())
+    d.check()
+    assert torch.isfinite(w).all() and abs(float(w.mean())) < 1e-12   # mean(G phi) = 0 (PAPER.md:74-78)
+
+
 def test_cfg1_single_rhs(sww, orc_ld):
     c = si.config1()
     d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
