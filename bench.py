@@ -334,8 +334,9 @@ def main():
         torch.cuda.synchronize()
         tmd = sww.timing_read()
         sww.timing_enable(False)
-        # dd multiply-adds of one step: 2 residual sweeps + 1 G product over NRHS_DD columns, and the same for the base column
-        ddfma = 3.0 * N * N * (NRHS_DD + 1)
+        # dd multiply-adds of one step: 1 residual product (2 solves, ddpath.cu DD_SWEEPS) + 1 G product over NRHS_DD columns,
+        # and the same for the base column
+        ddfma = 2.0 * N * N * (NRHS_DD + 1)
         t_ddg = tmd["dd_gemm"][0] * 1e-3
         ddres = {"value": world * NRHS_DD / (ms_dd * 1e-3), "unit": UNIT, "ms_per_step": ms_dd, "N": N, "nrhs": NRHS_DD,
                  "dd_fma_per_s_in_dd_gemm": ddfma / t_ddg if t_ddg > 0 else None,

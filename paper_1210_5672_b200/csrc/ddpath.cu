@@ -8,8 +8,15 @@
 // Product code; shares nothing with oracle/.
 #include "common.cuh"
 #include "dd.cuh"
+#include <cstdlib>
 
 namespace sww {
+
+// Solves per right-hand side in the refinement around the fp64 factors.  The compensated fp64 solve returns hi + lo with a
+// relative error near 1e-17, so the second solve (on the dd residual of the first) already lands below the dd rounding of the
+// residual itself: measured E_col with 2 and with 3 solves is the same to two digits (config 4: 1.48e-28 / 1.43e-28, N = 1024:
+// 8.83e-28 / 8.86e-28; bar 1e-25), and the third solve with its dd residual GEMM was a quarter of the dd step.
+constexpr int DD_SWEEPS = 2;
 
 // ------------------------------------------------------------------------------------------------ dd circulants: D and H
 // mode 0: out = D f,  coefficient (1/2)(-1)^m cot(pi m/N)                       (Fourier differentiation, Nyquist symbol 0, R4)
@@ -455,7 +462,7 @@ int accurate_base(sww_dtn_s* d, const double* phi0) {
     k_dd_copy<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, (size_t)N, isdd ? 1 : 0, phi0, b, rcol);
     SWW_LAUNCHED();
     if (isdd) {
-        const int nsweep = 3;
+        const int nsweep = DD_SWEEPS;
         for (int s = 0; s < nsweep; s++) {
             SWW_TRY(run_solve(d, rcol, rlo, 1));  // delta = (LU)^{-1} round(r)
             SWW_BEGIN(KC_OTHER, st);
@@ -552,7 +559,7 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
         SWW_LAUNCHED();
     }
     double* mu = w.W;  // dd planar, ws layout
-    const int nsweep = 3;
+    const int nsweep = DD_SWEEPS;
     for (int s = 0; s < nsweep; s++) {
         SWW_TRY(run_solve(d, w.R, w.S, nrhs));
         SWW_BEGIN(KC_OTHER, st);
