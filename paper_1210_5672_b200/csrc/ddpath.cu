@@ -181,46 +181,74 @@ static int matvec_dd(sww_dtn_s* d, const double* A, const double* Alo, const dou
 // ------------------------------------------------------------------------------------------------ dd GEMM (many columns)
 // Y = zs * Z + beta * X + alpha * (A X): A dd (or fp64) N x N, X, Z, Y dd planar N x ncols (plane size L = N * ld_cols).
 // CTA tile 64 rows x 32 columns, 256 threads, thread tile 4 x 2 (rows ty + 16 r, columns tx + 16 c), k-slab 16.
-// CN = columns per thread: 2 (tile 64 x 32) or 1 (tile 64 x 16, used when the wider tile would leave fewer than two CTAs per SM:
-// the k-slabs are loaded synchronously, so a second resident CTA is what hides the load latency).
-constexpr int DG_BM = 64, DG_BK = 16;
+// CN = columns per thread: 2 (tile 64 x 32) or 1 (tile 64 x 16, used when the wider tile would leave fewer than two CTAs per SM).
+constexpr int DG_BM = 64, DG_BK = 16, DG_XLD = DG_BK + 2;  // even padding: 16-byte cp.async destinations
+// 16 bytes global -> shared, zero-filled when !valid (cp.async src-size 0)
+__device__ __forceinline__ void dg_cp16(void* smem, const void* gmem, bool valid) {
+    unsigned s_ = (unsigned)__cvta_generic_to_shared(smem);
+    int sz = valid ? 16 : 0;
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(s_), "l"(gmem), "r"(sz));
+}
+template <int CN>
+struct DgSmem {
+    static constexpr int BN = 16 * CN;
+    static constexpr int A_PLANE = DG_BK * DG_BM, X_PLANE = BN * DG_XLD;
+    static constexpr int STAGE = 2 * A_PLANE + 2 * X_PLANE;  // doubles: A hi, A lo, X hi, X lo
+    static constexpr int BYTES = 2 * STAGE * (int)sizeof(double);
+};
+// The k-slabs are double-buffered through cp.async: slab s + 1 is in flight while slab s is multiplied.
 template <int CN>
 __global__ void __launch_bounds__(256) k_gemm_dd(int N, int ncols, size_t L, const double* __restrict__ A, const double* __restrict__ Alo,
                                                  const double* __restrict__ X, double zs, const double* __restrict__ Z, double beta,
                                                  double alpha, double* __restrict__ Y, double* __restrict__ Y_f64) {
-    __shared__ double As_hi[DG_BK][DG_BM], As_lo[DG_BK][DG_BM];
-    constexpr int DG_BN = 16 * CN;
-    __shared__ double Xs_hi[DG_BN][DG_BK + 1], Xs_lo[DG_BN][DG_BK + 1];
+    using S = DgSmem<CN>;
+    constexpr int DG_BN = S::BN;
+    extern __shared__ __align__(16) double dg_sm[];
     const int tid = threadIdx.x, ty = tid & 15, tx = tid >> 4;
     const int i0 = blockIdx.x * DG_BM, c0 = blockIdx.y * DG_BN;
+    auto issue = [&](int k0, int st) {
+        double* base = dg_sm + st * S::STAGE;
+        for (int e = tid; e < S::A_PLANE / 2; e += 256) {  // A: rows contiguous
+            const int kk = e / (DG_BM / 2), ii = (e % (DG_BM / 2)) * 2;
+            const size_t o = (size_t)(k0 + kk) * N + i0 + ii;
+            dg_cp16(base + kk * DG_BM + ii, A + o, true);
+            dg_cp16(base + S::A_PLANE + kk * DG_BM + ii, Alo ? Alo + o : A + o, Alo != nullptr);
+        }
+        for (int e = tid; e < DG_BN * DG_BK / 2; e += 256) {  // X: k contiguous
+            const int cc = e / (DG_BK / 2), kk = (e % (DG_BK / 2)) * 2;
+            const int c = c0 + cc;
+            const bool ok = c < ncols;
+            const size_t o = (size_t)(ok ? c : 0) * N + k0 + kk;
+            dg_cp16(base + 2 * S::A_PLANE + cc * DG_XLD + kk, X + o, ok);
+            dg_cp16(base + 2 * S::A_PLANE + S::X_PLANE + cc * DG_XLD + kk, X + L + o, ok);
+        }
+        asm volatile("cp.async.commit_group;\n" ::);
+    };
     dd acc[4][CN];
 #pragma unroll
     for (int r = 0; r < 4; r++)
 #pragma unroll
         for (int c = 0; c < CN; c++) acc[r][c] = dd{0.0, 0.0};
-    for (int k0 = 0; k0 < N; k0 += DG_BK) {
-        for (int e = tid; e < DG_BK * DG_BM; e += 256) {
-            int kk = e / DG_BM, ii = e % DG_BM;
-            size_t o = (size_t)(k0 + kk) * N + i0 + ii;
-            As_hi[kk][ii] = A[o];
-            As_lo[kk][ii] = Alo ? Alo[o] : 0.0;
-        }
-        for (int e = tid; e < DG_BN * DG_BK; e += 256) {
-            int cc = e / DG_BK, kk = e % DG_BK;
-            int c = c0 + cc;
-            size_t o = (size_t)c * N + k0 + kk;
-            bool ok = c < ncols;
-            Xs_hi[cc][kk] = ok ? X[o] : 0.0;
-            Xs_lo[cc][kk] = ok ? X[L + o] : 0.0;
+    issue(0, 0);
+    for (int k0 = 0, st = 0; k0 < N; k0 += DG_BK, st ^= 1) {
+        if (k0 + DG_BK < N) {
+            issue(k0 + DG_BK, st ^ 1);  // its buffer was released by the barrier that ended the previous slab
+            asm volatile("cp.async.wait_group 1;\n" ::);
+        } else {
+            asm volatile("cp.async.wait_group 0;\n" ::);
         }
         __syncthreads();
+        const double* As_hi = dg_sm + st * S::STAGE;
+        const double* As_lo = As_hi + S::A_PLANE;
+        const double* Xs_hi = As_hi + 2 * S::A_PLANE;
+        const double* Xs_lo = Xs_hi + S::X_PLANE;
 #pragma unroll 4
         for (int kk = 0; kk < DG_BK; kk++) {
             dd a[4], x[CN];
 #pragma unroll
-            for (int r = 0; r < 4; r++) a[r] = dd{As_hi[kk][ty + 16 * r], As_lo[kk][ty + 16 * r]};
+            for (int r = 0; r < 4; r++) a[r] = dd{As_hi[kk * DG_BM + ty + 16 * r], As_lo[kk * DG_BM + ty + 16 * r]};
 #pragma unroll
-            for (int c = 0; c < CN; c++) x[c] = dd{Xs_hi[tx + 16 * c][kk], Xs_lo[tx + 16 * c][kk]};
+            for (int c = 0; c < CN; c++) x[c] = dd{Xs_hi[(tx + 16 * c) * DG_XLD + kk], Xs_lo[(tx + 16 * c) * DG_XLD + kk]};
 #pragma unroll
             for (int r = 0; r < 4; r++)
 #pragma unroll
@@ -256,10 +284,16 @@ static int gemm_dd(sww_dtn_s* d, int ncols, size_t L, const double* A, const dou
     const int bn = narrow ? 16 : 32;
     dim3 grid(N / DG_BM, (ncols + bn - 1) / bn);
     SWW_BEGIN(KC_DDGEMM, d->stream);
+    static bool attr_set = false;
+    if (!attr_set) {
+        SWW_CUDA(cudaFuncSetAttribute(k_gemm_dd<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DgSmem<1>::BYTES));
+        SWW_CUDA(cudaFuncSetAttribute(k_gemm_dd<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DgSmem<2>::BYTES));
+        attr_set = true;
+    }
     if (narrow)
-        k_gemm_dd<1><<<grid, 256, 0, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
+        k_gemm_dd<1><<<grid, 256, DgSmem<1>::BYTES, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
     else
-        k_gemm_dd<2><<<grid, 256, 0, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
+        k_gemm_dd<2><<<grid, 256, DgSmem<2>::BYTES, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
