@@ -181,7 +181,7 @@ static int matvec_dd(sww_dtn_s* d, const double* A, const double* Alo, const dou
 // ------------------------------------------------------------------------------------------------ dd GEMM (many columns)
 // Y = zs * Z + beta * X + alpha * (A X): A dd (or fp64) N x N, X, Z, Y dd planar N x ncols (plane size L = N * ld_cols).
 // CTA tile 64 rows x 32 columns, 256 threads, thread tile 4 x 2 (rows ty + 16 r, columns tx + 16 c), k-slab 16.
-// CN = columns per thread: 2 (tile 64 x 32) or 1 (tile 64 x 16, used when the wider tile would leave fewer than two CTAs per SM).
+// CN = columns per thread: 2 (tile 64 x 32) or 1 (tile 64 x 16, used when there would be fewer than 100 wide tiles).
 constexpr int DG_BM = 64, DG_BK = 16, DG_XLD = DG_BK + 2;  // even padding: 16-byte cp.async destinations
 // 16 bytes global -> shared, zero-filled when !valid (cp.async src-size 0)
 __device__ __forceinline__ void dg_cp16(void* smem, const void* gmem, bool valid) {
@@ -280,7 +280,7 @@ static int gemm_dd(sww_dtn_s* d, int ncols, size_t L, const double* A, const dou
     if (N < DG_BM) {  // tiny N: column by column through the mat-vec kernel (planes are L apart, so repack is not needed when ncols == 1)
         return SWW_EINVAL;
     }
-    const bool narrow = (long)(N / DG_BM) * ((ncols + 31) / 32) < 2 * 148;
+    const bool narrow = (long)(N / DG_BM) * ((ncols + 31) / 32) < 100;  // too few wide tiles to occupy the chip
     const int bn = narrow ? 16 : 32;
     dim3 grid(N / DG_BM, (ncols + bn - 1) / bn);
     SWW_BEGIN(KC_DDGEMM, d->stream);
