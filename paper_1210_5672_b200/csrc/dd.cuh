@@ -98,13 +98,12 @@ __device__ __forceinline__ dd dd_div(dd a, dd b) {
     return dd_add_d(q, q3);
 }
 __device__ __forceinline__ dd dd_div_d(dd a, double b) { return dd_div(a, dd{b, 0.0}); }
-// fp64 reciprocal of a normal, well-scaled number: MUFU seed + Newton steps, no slow path (|x| far from 0, inf, denormals)
+// fp64 reciprocal of a normal, well-scaled number: MUFU seed (2^-20) + two Newton steps (within an ulp), no slow path
+// (|x| far from 0, inf, denormals)
 __device__ __forceinline__ double rcp_normal(double x) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
     double e = SWW_FMA(-x, r, 1.0);
-    r = SWW_FMA(r, e, r);
-    e = SWW_FMA(-x, r, 1.0);
     r = SWW_FMA(r, e, r);
     e = SWW_FMA(-x, r, 1.0);
     r = SWW_FMA(r, e, r);

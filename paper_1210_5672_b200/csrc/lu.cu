@@ -187,13 +187,11 @@ __global__ void __launch_bounds__(256) k_lu_single(double* __restrict__ A, int n
 // with every entry accurate relative to its own size.  Per step the owners publish column j and row j in shared memory
 // (double-buffered: one barrier per step); the rest is 16 register FMAs per thread.  vec: 256 doubles.
 // reciprocal of a pivot (|p| ~ 1/2, far from the denormal / overflow ranges the slow path of 1.0 / p guards against):
-// MUFU seed + three Newton steps (the third is a no-op correction in all but the last bit)
+// MUFU seed (relative error <= 2^-20) + two Newton steps (2^-40, 2^-80): within an ulp of 1/p
 __device__ __forceinline__ double pivot_rcp(double p) {
     double r;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(p));
     double e = fma(-p, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-p, r, 1.0);
     r = fma(r, e, r);
     e = fma(-p, r, 1.0);
     r = fma(r, e, r);
