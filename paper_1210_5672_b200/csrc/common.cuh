@@ -82,8 +82,7 @@ struct sww_dtn_s {
     unsigned* lu_flags;
     unsigned lu_epoch;
     int lu_ntasks;
-    unsigned* tr_flags;   // dataflow TRSM: claim counter (slot 0) + flags[2][N/64][slabs]
-    unsigned tr_epoch;
+    unsigned* tr_flags;   // dataflow TRSM: the claim counter
     double* tr_scr;       // dataflow TRSM: forward (hi, lo) and backward (hi) results, the hand-over buffers between tasks
     size_t tr_scr_cap;    // doubles
     unsigned long long* lu_trace;  // debugging aid (env SWW_LU_TRACE): per-task time stamps of the dataflow LU

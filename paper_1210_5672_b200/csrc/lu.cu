@@ -628,7 +628,6 @@ int lu_alloc(sww_dtn_s* d) {
     d->lu_epoch = 0;
     d->lu_trace = nullptr;
     d->tr_flags = nullptr;
-    d->tr_epoch = 0;
     if (N <= TS) return SWW_OK;
     const int nt = N / TS;
     std::vector<int> o;
@@ -639,8 +638,8 @@ int lu_alloc(sww_dtn_s* d) {
     if (cudaMalloc(&d->lu_flags, sizeof(unsigned) * nflags) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaMemcpyAsync(d->lu_order, o.data(), sizeof(int) * o.size(), cudaMemcpyHostToDevice, d->stream));
     SWW_CUDA(cudaMemsetAsync(d->lu_flags, 0, sizeof(unsigned) * nflags, d->stream));
-    if (cudaMalloc(&d->tr_flags, sizeof(unsigned) * (2 * (size_t)nt * TR_MAXNS + 1)) != cudaSuccess) return SWW_ENOMEM;
-    SWW_CUDA(cudaMemsetAsync(d->tr_flags, 0, sizeof(unsigned) * (2 * (size_t)nt * TR_MAXNS + 1), d->stream));
+    if (cudaMalloc(&d->tr_flags, sizeof(unsigned)) != cudaSuccess) return SWW_ENOMEM;  // the claim counter of the dataflow solves
+    SWW_CUDA(cudaMemsetAsync(d->tr_flags, 0, sizeof(unsigned), d->stream));
     if (getenv("SWW_LU_TRACE") && cudaMalloc(&d->lu_trace, sizeof(unsigned long long) * 4 * ((size_t)nt * nt + nt)) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaStreamSynchronize(d->stream));  // o goes out of scope
     return SWW_OK;
@@ -749,7 +748,7 @@ __global__ void __launch_bounds__(64) k_solve_small(int N, const double* __restr
 // differentiated afterwards, which amplifies white rounding noise by ~N/3.
 struct TrsmArgs {
     const double* A;     // LU factors, N x N column-major (L multipliers below the diagonal, U above)
-    const double *Es, *Fs;
+    const double* Fs;    // nt blocks of 64 x 64 (column-major, ld 64): inv(S_i) - 2 I
     double *B, *Blo;     // N x (ns*WS) column-major, ld = N; in: right-hand sides (Blo ignored), out: solution hi, lo
     int N, nt, ns;       // nt row blocks of 64, ns column slabs
     double *Yh, *Yl, *Xh;  // scratch, same shape as B: forward result (hi, lo) and backward result (hi); pre-filled with TR_ABSENT
@@ -976,7 +975,6 @@ static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     const int N = d->N, nt = N / TS;
     TrsmArgs a;
     a.A = d->LU;
-    a.Es = d->invD;
     a.Fs = d->invD + (size_t)nt * TS * TS;
     a.B = B;
     a.Blo = Blo;
