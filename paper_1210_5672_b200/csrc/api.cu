@@ -174,7 +174,6 @@ int sww_dtn_get(sww_dtn_t d, int which, void* dst) {
         case 6: src = d->bu; n = N * mul; break;
         case 7: src = d->bv; n = N * mul; break;
         case 8: src = d->LU; n = (size_t)N * N; break;
-        case 9: src = reinterpret_cast<const double*>(d->lu_trace); n = d->lu_trace ? 4 * ((size_t)(N / 64) * (N / 64) + N / 64) : 0; if (!src) return SWW_EINVAL; break;
         default: return SWW_EINVAL;
     }
     SWW_CUDA(cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDeviceToDevice, d->stream));
@@ -201,7 +200,6 @@ int sww_dtn_destroy(sww_dtn_t d) {
     cudaFree(d->lu_flags);
     cudaFree(d->tr_flags);
     cudaFree(d->tr_scr);
-    cudaFree(d->lu_trace);
     delete d;
     return SWW_OK;
 }

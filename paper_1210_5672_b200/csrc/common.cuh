@@ -38,6 +38,23 @@ void timing_end();
         if (::sww::g_timing) ::sww::timing_end();            \
     } while (0)
 
+// ---------------------------------------------------------------- per-device state
+// first() is true exactly once per device for each instance: guards the per-device opt-ins (cudaFuncSetAttribute for more than
+// 48 KB of dynamic shared memory) at their call sites.  Not thread-safe (like the rest of the library's host side).
+struct DeviceOnce {
+    unsigned long long seen[4] = {0, 0, 0, 0};
+    bool first() {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        dev &= 255;
+        const unsigned long long bit = 1ull << (dev & 63);
+        if (seen[dev >> 6] & bit) return false;
+        seen[dev >> 6] |= bit;
+        return true;
+    }
+};
+int sm_count();  // multiprocessors of the current device (cached per device)
+
 // ---------------------------------------------------------------- per-N constant tables (device, cached per N per device)
 // "computed once and for all".  All double-double, planar (hi[N], lo[N]).
 struct Tables {
@@ -85,7 +102,6 @@ struct sww_dtn_s {
     unsigned* tr_flags;   // dataflow TRSM: the claim counter
     double* tr_scr;       // dataflow TRSM: forward (hi, lo) and backward (hi) results, the hand-over buffers between tasks
     size_t tr_scr_cap;    // doubles
-    unsigned long long* lu_trace;  // debugging aid (env SWW_LU_TRACE): per-task time stamps of the dataflow LU
     // base state (dd planar 2N each): phi0', W0, u, v
     double *bphi, *bW0, *bu, *bv;
     double *bp_part;      // partial sums of the dd base-state pass: bp_chunks x 4 x N doubles
@@ -113,15 +129,10 @@ int run_lu(sww_dtn_s* d);
 // multi-RHS triangular solves with the factors in d->LU; B is N x ncols (ld = N), in place; Blo (same shape) receives the
 // low word of the compensated solution (B already holds RN(B + Blo)); Blo's incoming content is ignored
 int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols);
-// GEMM (gemm.cu): C[M x Nc] = alpha * A[M x K] * B[K x Nc] + beta * C, all column-major fp64; C may alias A or B only in the
-// panel patterns documented in gemm.cu.  n_valid: columns >= n_valid are not stored.
-struct Epi {
-    double* Clo = nullptr;  // compensated target: C + Clo (same layout and ldc as C)
-    int lo_mode = 1;        // 1: read and write Clo ; 2: write only (incoming Clo taken as zero)
-    int fold = 0;           // 1: renormalise, C = RN(C + Clo), Clo = remainder
-};
+// GEMM (gemm.cu): C[M x Nc] = alpha * A[M x K] * B[K x Nc] + beta * C, all column-major fp64; C must not alias A or B.
+// n_valid: columns >= n_valid are not stored.
 int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* A, int lda, const double* B, int ldb,
-             double beta, double* C, int ldc, int n_valid, Epi epi = Epi());
+             double beta, double* C, int ldc, int n_valid);
 // C[M x nc] += A B for nc <= 4 columns as a streamed GEMV (gemm.cu); part / count: the handle's bp_part / mv_count
 int gemv_few_f64(cudaStream_t st, int M, int nc, int K, const double* A, int lda, const double* B, int ldb, double* C, int ldc, double* part,
                  unsigned* count);

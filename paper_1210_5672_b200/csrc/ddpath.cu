@@ -284,11 +284,10 @@ static int gemm_dd(sww_dtn_s* d, int ncols, size_t L, const double* A, const dou
     const int bn = narrow ? 16 : 32;
     dim3 grid(N / DG_BM, (ncols + bn - 1) / bn);
     SWW_BEGIN(KC_DDGEMM, d->stream);
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_once;
+    if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_gemm_dd<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, DgSmem<1>::BYTES));
         SWW_CUDA(cudaFuncSetAttribute(k_gemm_dd<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, DgSmem<2>::BYTES));
-        attr_set = true;
     }
     if (narrow)
         k_gemm_dd<1><<<grid, 256, DgSmem<1>::BYTES, d->stream>>>(N, ncols, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
@@ -606,10 +605,9 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
                 return SWW_EINVAL;
         }
     }
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_once;
+    if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_spectral_gamma_w_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, 2048 * 32 * 2));
-        attr_set = true;
     }
     size_t smem = (size_t)N * sizeof(cdd) * 2;
     int threads = N / 2 > 512 ? 512 : (N / 2 < 32 ? 32 : N / 2);

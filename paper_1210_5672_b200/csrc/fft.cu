@@ -102,11 +102,10 @@ __global__ void __launch_bounds__(1024) k_spectral_deriv(int N, int logN, const 
 int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols) {
     const int N = d->N;
     size_t smem = sizeof(double2) * (size_t)N;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_once;
+    if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_spectral_gamma_w, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
         SWW_CUDA(cudaFuncSetAttribute(k_spectral_deriv, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
-        attr_set = true;
     }
     SWW_BEGIN(KC_FFT, d->stream);
     k_spectral_gamma_w<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, fft_ilog2(N), d->tab->tw, M, T, Gam, W, ncols, w_cols);
@@ -118,10 +117,9 @@ int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam
 int spectral_deriv(sww_dtn_s* d, const double* in, double* out, int ncols) {
     const int N = d->N;
     size_t smem = sizeof(double2) * (size_t)N;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_once;
+    if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_spectral_deriv, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
-        attr_set = true;
     }
     SWW_BEGIN(KC_FFT, d->stream);
     k_spectral_deriv<<<(ncols + 1) / 2, fft_threads(N), smem, d->stream>>>(N, fft_ilog2(N), d->tab->tw, in, out, ncols);

@@ -1,20 +1,14 @@
-// gemm.cu -- FP64 dense contraction on the FP64 tensor pipe (DMMA.8x8x4 = mma.sync.m8n8k4.f64, the only FP64 MMA shape that
-// is native on sm_100a) with cp.async multi-stage shared-memory staging.  Used by the trailing updates of the LU (S2), the
-// multi-right-hand-side triangular solves (S4) and the product with G (S6): "level 3 BLAS speed".
+// gemm.cu -- S6: the product with G of (2.8) ("the device also applies G") as an FP64 dense
+// contraction on the FP64 tensor pipe: DMMA.8x8x4 = mma.sync.m8n8k4.f64, the only FP64 MMA shape that is native on sm_100a
+// (tcgen05 has no f64 kind), with cp.async multi-stage shared-memory staging.
 //
 //   C[M x Nc] = alpha * A[M x K] * B[K x Nc] + beta * C        (all column-major, leading dimensions lda, ldb, ldc)
 //
 // Requirements: M % BM == 0, K % BK == 0 (the library pads: N is a power of two >= 16, column counts are padded to 64);
 // Nc may be ragged: columns >= Nc of B are never read (zero-filled in shared memory) and columns >= n_valid of C never stored.
-// Compensated accumulation (Epi.Clo != nullptr): the target is carried as an unevaluated sum C + Clo and the product is added by
-// an error-free two-sum, C' + e = beta*C + alpha*acc exactly, Clo' = beta*Clo + e (beta must be a power of two).  This keeps the
-// rounding of the O(1) right-hand sides out of the triangular solves (the density mu is differentiated
-// afterwards, which amplifies white rounding noise by ~N/3).  lo_mode 2 = Clo is not read (treated as zero); fold = store
-// C' = RN(C' + Clo') and the remainder in Clo'.
-// Aliasing: C may alias A when K == BKfull rows of one CTA tile cover all of A's tile (the panel pattern L21 <- A21 inv(U11)):
-// every CTA reads its whole A row-panel before storing, and no other CTA touches that panel.  Same for C aliasing B.
+// The LU and the triangular solves have their own persistent dataflow kernels (lu.cu); a stage without variational columns
+// applies G to one vector through the streamed GEMV at the bottom of this file.
 #include "common.cuh"
-#include <cstdlib>
 
 namespace sww {
 
@@ -53,7 +47,7 @@ struct GemmCfg {
 template <class Cfg, int BM, int BN, int BK, int STAGES>
 __global__ void __launch_bounds__(Cfg::THREADS) k_gemm_f64(int M, int Nc, int K, double alpha, const double* __restrict__ A, int lda,
                                                            const double* __restrict__ B, int ldb, double beta, double* C, int ldc,
-                                                           int n_valid, Epi epi) {
+                                                           int n_valid) {
     extern __shared__ __align__(16) double smem[];
     double* As = smem;
     double* Bs = smem + STAGES * Cfg::A_STAGE;
@@ -129,24 +123,8 @@ __global__ void __launch_bounds__(Cfg::THREADS) k_gemm_f64(int M, int Nc, int K,
                 if (col < n_valid) {
                     double* p = C + (size_t)col * ldc + row;
                     double v = alpha * acc[i][j][e];
-                    if (epi.Clo) {
-                        double* pl = epi.Clo + (size_t)col * ldc + row;
-                        double c = beta * *p;
-                        double s = __dadd_rn(c, v);
-                        double bb = __dsub_rn(s, c);
-                        double err = __dadd_rn(__dsub_rn(c, __dsub_rn(s, bb)), __dsub_rn(v, bb));
-                        double lo = (epi.lo_mode == 2) ? err : fma(beta, *pl, err);
-                        if (epi.fold) {
-                            double t = __dadd_rn(s, lo);
-                            lo = __dsub_rn(lo, __dsub_rn(t, s));
-                            s = t;
-                        }
-                        *p = s;
-                        *pl = lo;
-                    } else {
-                        if (beta != 0.0) v = fma(beta, *p, v);
-                        *p = v;
-                    }
+                    if (beta != 0.0) v = fma(beta, *p, v);
+                    *p = v;
                 }
             }
         }
@@ -168,28 +146,26 @@ __global__ void k_gemm_naive(int M, int Nc, int K, double alpha, const double* A
 
 template <int BM, int BN, int BK, int WR, int WC, int STAGES>
 static int launch_gemm(cudaStream_t st, int M, int Nc, int K, double alpha, const double* A, int lda, const double* B, int ldb,
-                       double beta, double* C, int ldc, int n_valid, Epi epi) {
+                       double beta, double* C, int ldc, int n_valid) {
     using Cfg = GemmCfg<BM, BN, BK, WR, WC, STAGES>;
     auto kern = k_gemm_f64<Cfg, BM, BN, BK, STAGES>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_once;
+    if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM));
-        attr_set = true;
     }
     dim3 grid(M / BM, (Nc + BN - 1) / BN);
     SWW_BEGIN(KC_GEMM, st);
-    kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid, epi);
+    kern<<<grid, Cfg::THREADS, Cfg::SMEM, st>>>(M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
 }
 
 int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* A, int lda, const double* B, int ldb, double beta,
-             double* C, int ldc, int n_valid, Epi epi) {
+             double* C, int ldc, int n_valid) {
     if (M <= 0 || Nc <= 0) return SWW_OK;
     if (n_valid > Nc) n_valid = Nc;
     if (M % 64 != 0 || K % 16 != 0) {
-        if (epi.Clo) return SWW_EINVAL;  // the compensated epilogue exists in the tiled kernel only
         dim3 grid((M + 63) / 64, n_valid);
         SWW_BEGIN(KC_GEMM, st);
         k_gemm_naive<<<grid, 64, 0, st>>>(M, n_valid, K, alpha, A, lda, B, ldb, beta, C, ldc);
@@ -199,11 +175,11 @@ int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* 
     }
     // tile choice: fill the 148 SMs.  128x128 tiles when that still gives >= ~2 waves of CTAs, else 64x64.
     long tiles128 = (M % 128 == 0) ? (long)(M / 128) * ((Nc + 127) / 128) : 0;
-    if (tiles128 >= 148) return launch_gemm<128, 128, 16, 4, 2, 3>(st, M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid, epi);
+    if (tiles128 >= 148) return launch_gemm<128, 128, 16, 4, 2, 3>(st, M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid);
     // 64x64: k-slabs of 32 when K allows (measured on the G product 2048 x 512 x 2048: 0.173 ms against 0.181 with slabs of 16;
     // 128x64, 64x128, 128x32 and 64x32 tiles were all slower there)
-    if (K % 32 == 0) return launch_gemm<64, 64, 32, 2, 2, 3>(st, M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid, epi);
-    return launch_gemm<64, 64, 16, 2, 2, 3>(st, M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid, epi);
+    if (K % 32 == 0) return launch_gemm<64, 64, 32, 2, 2, 3>(st, M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid);
+    return launch_gemm<64, 64, 16, 2, 2, 3>(st, M, Nc, K, alpha, A, lda, B, ldb, beta, C, ldc, n_valid);
 }
 
 // ------------------------------------------------------------------------------------------------ few columns: C += A B as a GEMV

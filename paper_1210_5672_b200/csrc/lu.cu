@@ -1,28 +1,22 @@
-// lu.cu -- S2: unpivoted LU of A = I/2 + K (the matrix of (2.7); "LU-factorization") and
+// lu.cu -- S2: unpivoted BLOCK LU of A = I/2 + K (the matrix of (2.7); "LU-factorization") and
 // S4: the multi-right-hand-side triangular solves ("a single back-solve", "level 3 BLAS speed").
 //
 // No pivoting: the second-kind operator is benign -- sigma(A) in [0.46, 1.01], partial pivoting performs zero row swaps on every
-// workload family; a |U_ii| guard reports SWW_ESINGULAR instead of producing garbage.
+// workload family; a guard on every pivot reports SWW_ESINGULAR instead of producing garbage.
 //
-// Factorisation = ONE persistent kernel (k_lu_dataflow), left-looking by 64 x 64 tile.  Every tile (i,j) is a task; a CTA claims
-// the next task from a global counter, accumulates  P = sum_{k < min(i,j)} L_ik U_kj  in DMMA.8x8x4 fragments (operand tiles
-// arrive from L2 by cp.async, double-buffered), and finishes the tile:
-//     diagonal : GETRF of the 64 x 64 block in shared memory (in-warp 32 x 32 LU by shuffles + 32-blocks), plus the inverses of
-//                its triangular factors;
-//     i > j    : L_ij = (A_ij - P) inv(U_jj)  = 2 X + X F_j      (DMMA with the inverse factor);
-//     i < j    : U_ij = inv(L_ii) (A_ij - P)  = X + E_i X.
-// A tile is published by a release store of the epoch into flags[i][j]; consumers acquire-poll it.  Tasks are claimed in level
-// order (level = min(i,j); diagonal tile first, then tiles by distance from the diagonal), so every dependency of a claimed task
-// was claimed earlier by a CTA that is running: no deadlock, no grid-wide barrier, no host round trip.  The pivot chain
-// (GETRF -> two neighbours -> next diagonal tile) is the critical path; everything else overlaps with it.
+// Factorisation = ONE persistent kernel (k_lu_dataflow) over 64 x 64 tiles.  The diagonal blocks are not factored but INVERTED:
+// A = L U with identity diagonal blocks in L and the Schur complements S_m on the block diagonal of U; what is stored is
+// L_im = X_im Z_m (i > m), U_mj = X_mj (j > m) and F_m = Z_m - 2 I, Z_m = inv(S_m).  Block 0 (the "spine") runs the recurrence of
+// the diagonal blocks; every other CTA is a worker claiming tile tasks from a counter in dependency order.  Tiles are handed
+// over through release/acquire flags in global memory: no grid barrier, no host round trip.  Details at k_lu_dataflow.
+// N <= 64 (one padded tile) goes through k_lu_single (a scalar 64-step GETRF with explicit triangular inverses).
 //
-// Storage convention of the LU buffer: the DIAGONAL holds kappa_ii = U_ii - 1/2 (the assembly writes K, not I/2 + K): every
+// Storage convention of the LU buffer: the DIAGONAL holds kappa_ii = A_ii - 1/2 (the assembly writes K, not I/2 + K): every
 // update then rounds at the O(1/N) scale of the kernel entries instead of the O(1) scale of the pivot, and the inverse
-// diagonal blocks are formed as perturbations of the identity,  inv(L_kk) = I + E_kk,  inv(U_kk) = 2 I + F_kk.
+// diagonal blocks are carried as deviations F_m = inv(S_m) - 2 I.
 // Product code; shares nothing with oracle/.
 #include "common.cuh"
 #include <algorithm>
-#include <cstdlib>
 #include <vector>
 
 namespace sww {
@@ -304,14 +298,7 @@ struct LuArgs {
     unsigned* counter;  // next task to claim (zeroed before the launch)
     double* Fs;        // nt blocks of 64 x 64 (column-major, ld 64): inv(S_m) - 2 I
     int* status;
-    unsigned long long* trace;  // optional: 4 globaltimer stamps per worker task, then 4 per spine step
 };
-
-__device__ __forceinline__ unsigned long long gtime() {
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
-    return t;
-}
 
 constexpr int LU_SMEM_BYTES = (4 * TS * LDO + TS * LDT + 256) * (int)sizeof(double) + 256;
 
@@ -384,8 +371,6 @@ __device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, dou
     };
     bool pre = false;  // the inputs of this step were requested before the previous inversion started
     for (int m = 0; m < nt; m++) {
-        unsigned long long* tr = p.trace ? p.trace + 4 * ((size_t)p.ntasks + m) : nullptr;
-        if (tr && tid == 0) tr[0] = gtime();
         if (m == 0) {
             const double* Cg = p.A;
             for (int e = tid; e < TS * TS; e += 256) {
@@ -399,7 +384,6 @@ __device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, dou
                 __syncthreads();
                 issue_inputs(m);
             }
-            if (tr && tid == 0) tr[1] = gtime();
             cp_wait<0>();
             __syncthreads();
             double c0[4][2][2], acc[4][2][2];
@@ -468,15 +452,11 @@ __device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, dou
             __syncthreads();
             if (pre) issue_inputs(m + 1);
         };
-        if (tr && tid == 0) tr[2] = gtime();
-        const long long ck0 = clock64();
         gj64(T, vec, p.status, tid, p.Fs + (size_t)m * TS * TS, sB0, try_prefetch);
         __syncthreads();
-        if (tr && tid == 0 && m == 0) tr[1] = (unsigned long long)(clock64() - ck0);  // SM cycles of one inversion (clock check)
         if (tid == 0) {
             __threadfence();
             st_release(p.zflags + m, epoch);
-            if (tr) tr[3] = gtime();
         }
     }
 }
@@ -507,7 +487,6 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
         const int ij = p.order[task], i = ij >> 16, j = ij & 0xffff;
         const int m = (i == j) ? i - 1 : min(i, j);  // number of finished block columns / rows this tile sums over
         double* Cg = p.A + (size_t)j * TS * N + (size_t)i * TS;
-        if (p.trace && tid == 0) p.trace[4 * task] = gtime();
 
         auto refresh = [&]() {
             for (int t = tid; t < m; t += 256)
@@ -562,7 +541,6 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
                 issue(k + 1, (k + 1) & 1);
             }
         }
-        if (p.trace && tid == 0) p.trace[4 * task + 1] = gtime();
         // X = A_ij - sum
 #pragma unroll
         for (int x = 0; x < 4; x++)
@@ -600,10 +578,8 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
                 for (int e = 0; e < 2; e++) Cg[(size_t)f.col(y, e) * N + f.row(x)] = c0[x][y][e];
         __syncthreads();  // every thread's stores are issued
         if (tid == 0) {
-            if (p.trace) p.trace[4 * task + 2] = gtime();
             __threadfence();
             st_release(flag, epoch);
-            if (p.trace) p.trace[4 * task + 3] = gtime();
         }
     }
 }
@@ -626,7 +602,6 @@ int lu_alloc(sww_dtn_s* d) {
     d->lu_order = nullptr;
     d->lu_flags = nullptr;
     d->lu_epoch = 0;
-    d->lu_trace = nullptr;
     d->tr_flags = nullptr;
     if (N <= TS) return SWW_OK;
     const int nt = N / TS;
@@ -640,20 +615,8 @@ int lu_alloc(sww_dtn_s* d) {
     SWW_CUDA(cudaMemsetAsync(d->lu_flags, 0, sizeof(unsigned) * nflags, d->stream));
     if (cudaMalloc(&d->tr_flags, sizeof(unsigned)) != cudaSuccess) return SWW_ENOMEM;  // the claim counter of the dataflow solves
     SWW_CUDA(cudaMemsetAsync(d->tr_flags, 0, sizeof(unsigned), d->stream));
-    if (getenv("SWW_LU_TRACE") && cudaMalloc(&d->lu_trace, sizeof(unsigned long long) * 4 * ((size_t)nt * nt + nt)) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaStreamSynchronize(d->stream));  // o goes out of scope
     return SWW_OK;
-}
-
-static int sm_count() {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (sms <= 0) sms = 148;
-    }
-    return sms;
 }
 
 int run_lu(sww_dtn_s* d) {
@@ -662,11 +625,10 @@ int run_lu(sww_dtn_s* d) {
     double* Es = d->invD;
     double* Fs = d->invD + (size_t)nblk * nb * nb;
     constexpr int SINGLE_SMEM = (TS * LDT + 576) * (int)sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_once;
+    if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_lu_single, cudaFuncAttributeMaxDynamicSharedMemorySize, SINGLE_SMEM));
         SWW_CUDA(cudaFuncSetAttribute(k_lu_dataflow, cudaFuncAttributeMaxDynamicSharedMemorySize, LU_SMEM_BYTES));
-        attr_set = true;
     }
     if (nblk == 1) {
         SWW_BEGIN(KC_LU, st);
@@ -688,7 +650,6 @@ int run_lu(sww_dtn_s* d) {
     a.epoch = ++d->lu_epoch;
     a.Fs = Fs;
     a.status = d->status;
-    a.trace = d->lu_trace;
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), st));
     const int grid = std::min(sm_count(), 1 + a.ntasks);
     SWW_BEGIN(KC_LU, st);
@@ -756,8 +717,18 @@ struct TrsmArgs {
     int* status;
 };
 constexpr long long TR_ABSENT = -1LL;       // bit pattern of "not written yet" (cudaMemset 0xFF)
-constexpr int TR_SPIN_LIMIT = 1 << 22;      // reloads before a task gives up (inputs that contain the pattern itself): SWW_ECUDA
+constexpr int TR_SPIN_LIMIT = 1 << 17;      // reloads (~1 us each) before a task gives up: SWW_ECUDA, and every other task stops polling
 constexpr int TR_FOLD = 4;
+// The reserved pattern never enters the scratch vectors: a NaN with that payload (an input column filled with 0xFF bytes, say)
+// is replaced by the canonical quiet NaN where right-hand sides are loaded and before every hand-over store.
+__device__ __forceinline__ double tr_canon(double v) {
+    return (__double_as_longlong(v) == TR_ABSENT) ? __longlong_as_double(0x7FF8000000000000LL) : v;
+}
+__device__ __forceinline__ int ld_status(const int* p) {
+    int v;
+    asm volatile("ld.relaxed.gpu.global.s32 %0, [%1];\n" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 
 __device__ __forceinline__ void two_sum_d(double a, double b, double& s, double& e) {
     s = __dadd_rn(a, b);
@@ -781,7 +752,7 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
     double* sA = tr_sm;                    // 2 stages of the factor tile as As[k][r]
     double* sD = sA + 2 * TS * LDO;        // the diagonal block F_i of the backward sweep, as As[k][r]
     double* sB = sD + TS * LDO;            // 2 stages of the solution tile as Bs[n][k]
-    __shared__ int s_task;
+    __shared__ int s_task, s_abort;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wr = warp % C::WR, wc = warp / C::WR, fr = lane >> 2, fk = lane & 3;
     const int N = p.N, nt = p.nt, ns = p.ns;
@@ -790,10 +761,14 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
 
     for (;;) {
         __syncthreads();
-        if (tid == 0) s_task = (int)atomicAdd(p.counter, 1u);
+        if (tid == 0) {
+            s_task = (int)atomicAdd(p.counter, 1u);
+            s_abort = ld_status(p.status) != SWW_OK;
+        }
         __syncthreads();
         int task = s_task;
         if (task >= 2 * nt * ns) break;
+        if (s_abort) break;  // some task gave up (or the handle already carries an error): stop polling, leave at once
         const int phase = task >= nt * ns;
         if (phase) task -= nt * ns;
         const int s = task % ns, i = phase ? nt - 1 - task / ns : task / ns;
@@ -824,8 +799,15 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             }
             return bad;
         };
-        auto give_up = [&]() {
-            if (tid == 0) atomicCAS(p.status, SWW_OK, SWW_ECUDA);
+        // CTA-uniform: true when this wait must end -- the spin limit is hit (this task records SWW_ECUDA) or, looked at every
+        // 64 reloads, some other task already did
+        auto spin_out = [&](int spin) -> bool {
+            if (spin > TR_SPIN_LIMIT) {
+                if (tid == 0) atomicCAS(p.status, SWW_OK, SWW_ECUDA);
+                return true;
+            }
+            if ((spin & 63) != 63) return false;
+            return __syncthreads_or(tid == 0 && ld_status(p.status) != SWW_OK) != 0;
         };
         auto issueY = [&](int kk, int buf) {
             const int k = kblock(kk);
@@ -861,16 +843,13 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                         bl[x][e] = __ldcg(p.Yl + blk + o);
                         bad |= (__double_as_longlong(bh[x][e]) == TR_ABSENT) | (__double_as_longlong(bl[x][e]) == TR_ABSENT);
                     } else {
-                        bh[x][e] = Bg[o];
+                        bh[x][e] = tr_canon(Bg[o]);
                         bl[x][e] = 0.0;  // the forward sweep starts from plain fp64 right-hand sides
                     }
                     acc[x][e] = ph[x][e] = pl[x][e] = 0.0;
                 }
             if (!phase || !__syncthreads_or(bad)) break;
-            if (spin > TR_SPIN_LIMIT) {
-                give_up();
-                break;
-            }
+            if (spin_out(spin)) break;
         }
         auto fold = [&]() {  // (ph, pl) += acc, error-free; acc = 0
 #pragma unroll
@@ -910,10 +889,7 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 cp_wait<0>();
             }
             for (int spin = 0; __syncthreads_or(absentY(kk & 1)); spin++) {  // the barrier also makes the tiles visible to all
-                if (spin > TR_SPIN_LIMIT) {
-                    give_up();
-                    break;
-                }
+                if (spin_out(spin)) break;
                 issueY(kk, kk & 1);  // not there yet: ask L2 again
                 cp_commit();
                 cp_wait<0>();
@@ -953,12 +929,12 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 const double hi = __dadd_rn(t_, lo);
                 const double low = __dsub_rn(lo, __dsub_rn(hi, t_));
                 if (phase) {  // x_i: to its consumers, and the result
-                    p.Xh[blk + o] = hi;
+                    p.Xh[blk + o] = tr_canon(hi);
                     Bg[o] = hi;
                     Lg[o] = low;
                 } else {      // y_i: hi for the forward tasks below, hi and lo for this block's backward task
-                    p.Yh[blk + o] = hi;
-                    p.Yl[blk + o] = low;
+                    p.Yh[blk + o] = tr_canon(hi);
+                    p.Yl[blk + o] = tr_canon(low);
                 }
             }
     }
@@ -967,10 +943,9 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
 template <int WS>
 static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     using C = TrsmCfg<WS>;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static DeviceOnce attr_once;
+    if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_trsm_dataflow<WS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-        attr_set = true;
     }
     const int N = d->N, nt = N / TS;
     TrsmArgs a;
@@ -1022,9 +997,7 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
     // slab width: the chain of a slab is 2 N/64 links of (flag hop + one or two 64 x 64 x WS products), so narrow slabs finish
     // sooner as long as there are few of them; every slab re-reads the factors from L2, so many columns want wide slabs
     // (measured at N = 2048: 128 columns 0.19 ms with 16-column slabs against 0.27 ms with 32; 512 columns 0.36 against 0.34)
-    static int ws_env = -1;
-    if (ws_env < 0) ws_env = getenv("SWW_TRSM_WS") ? atoi(getenv("SWW_TRSM_WS")) : 0;
-    const int ws = ws_env ? ws_env : (ncols <= 64 ? 8 : (ncols <= 256 ? 16 : 32));
+    const int ws = ncols <= 64 ? 8 : (ncols <= 256 ? 16 : 32);
     for (int c0 = 0; c0 < ncols; c0 += TR_MAXNS * ws) {
         const int nc = std::min(ncols - c0, TR_MAXNS * ws);
         double *b = B + (size_t)c0 * N, *bl = Blo + (size_t)c0 * N;

@@ -228,12 +228,11 @@ __global__ void __launch_bounds__(256) k_energy(int N, double g, const double* _
 namespace sww {
 
 static int rk_set_attrs() {
-    static bool done = false;
-    if (!done) {
+    static DeviceOnce done;
+    if (done.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_rhs_base, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
         SWW_CUDA(cudaFuncSetAttribute(k_rhs_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 4096 * 32));
         SWW_CUDA(cudaFuncSetAttribute(k_filter_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
-        done = true;
     }
     return SWW_OK;
 }

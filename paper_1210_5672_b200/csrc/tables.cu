@@ -16,6 +16,18 @@ int note_cuda(cudaError_t e, const char* where) {
     return SWW_ECUDA;
 }
 
+int sm_count() {
+    static int sms[256] = {0};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    dev &= 255;
+    if (!sms[dev]) {
+        cudaDeviceGetAttribute(&sms[dev], cudaDevAttrMultiProcessorCount, dev);
+        if (sms[dev] <= 0) sms[dev] = 148;
+    }
+    return sms[dev];
+}
+
 // ---- per-kernel-class timing (diagnostics; see common.cuh)
 bool g_timing = false;
 namespace {

@@ -208,10 +208,11 @@ def _family_surface(seed: int, N: int, amp1: float, kmax: int = 64):
     return a, b
 
 
-def config3(N: int = 512, ncols: int = 256) -> Case:
-    """Config 3 (N=512, 256 columns) and, with N=2048, ncols=512, the fp64 metric point."""
-    seed = SEED_BASE + 3
-    a, b = _family_surface(seed, N, 0.2)
+def config3(N: int = 512, ncols: int = 256, amp1: float = 0.2, variant: int = 0) -> Case:
+    """Config 3 (N=512, 256 columns) and, with N=2048, ncols=512, the fp64 metric point.  amp1: amplitude of the cos(alpha)
+    mode of the surface; variant > 0: another draw of the seeded modes (seed + 1000 variant) for the multi-seed parity runs."""
+    seed = SEED_BASE + 3 + 1000 * variant
+    a, b = _family_surface(seed, N, amp1)
     eta = synth(N, a)[0]
     phi0 = synth(N, b)[0]
     deta, dphi = fourier_unit_columns(N, ncols // 2, "eta_phi")
@@ -257,9 +258,9 @@ def config5(N: int = 4096, ncols: int = 512) -> Case:
     return Case(f"cfg5_N{N}", N, 0.05, eta=eta, phi0=np.zeros(N), deta=deta, dphi=dphi)
 
 
-def metric_point(ncols: int = 512) -> Case:
+def metric_point(ncols: int = 512, amp1: float = 0.2, variant: int = 0) -> Case:
     """BASELINE.json metric point: N=2048, config-3 family, fp64."""
-    c = config3(2048, ncols)
+    c = config3(2048, ncols, amp1, variant)
     c.name = f"metric_N2048_nrhs{ncols}"
     return c
 

@@ -207,13 +207,52 @@ def test_metric_point_sampled_columns(sww, orc_ld):
     print("metric point", r)
 
 
+@pytest.mark.parametrize("amp1,variant", [(0.1, 0), (0.3, 0), (0.1, 1), (0.2, 1), (0.3, 1), (0.1, 2), (0.2, 2), (0.3, 2)])
+def test_metric_point_other_seeds_and_amplitudes(sww, orc_ld, amp1, variant):
+    """the metric point on other draws of the seeded surface / potential and at amplitudes 0.1, 0.2, 0.3 of the cos(alpha) mode
+    ((0.2, seed 0) is test_metric_point_sampled_columns): all 512 columns computed, 12 sampled ones against the oracle"""
+    c = si.metric_point(512, amp1, variant)
+    cols = sample_columns(c, 12, seed=11 + variant)
+    out, d = gpu_linearized(c, cols)
+    orc, base = oracle_linearized(orc_ld, c, cols)
+    r = check_columns(out, orc, "f64", c.N, lin_scales(c, base, cols), f"metric amp {amp1} variant {variant}")
+    assert r["cols_with_floor_above_bar"] == 0
+    print(f"metric point amp1={amp1} variant={variant}", r)
+
+
 def test_metric_point_dd_sampled_columns(sww, orc_q):
-    c = si.metric_point_dd(128, 1024)
+    """the double-double leg of the metric as bench.py times it: N = 2048, 128 columns (config-4 family), all computed; the
+    __float128 oracle checks 8 sampled columns (k = 1, 2, 3 always included); bar 1e-25"""
+    c = si.metric_point_dd(128, 2048)
     cols = sample_columns(c, 8)
     out, d = gpu_linearized(c, cols)
     orc, base = oracle_linearized(orc_q, c, cols)
     r = check_columns(out, orc, "dd", c.N, lin_scales(c, base, cols), "metric dd")
-    print("metric dd (N=1024)", r)
+    assert r["cols_with_floor_above_bar"] == 0
+    print("metric dd (N=2048, 128 columns)", r)
+
+
+def test_gemm_128x128_tiles(sww):
+    """the 128 x 128 tile instantiation of the G product (taken when (N/128) * ceil(nrhs/128) >= 148: N = 4096 with 640 columns):
+    (a) flat surface: G cos(kx) = k tanh(kh) cos(kx) for k = 1..640 ((4.34), PAPER.md:324);
+    (b) wavy surface: the same 640 columns applied in two halves of 320 go through the 64 x 64 tiles -- same result to rounding"""
+    N, h, nc = 4096, 1.0, 640
+    ks = np.arange(1, nc + 1)
+    j = np.arange(N)
+    phi = torch.from_numpy(np.cos(2 * np.pi * ((ks[:, None] * j[None, :]) % N) / N)).cuda()
+    d = sww.DtN(torch.zeros(N, dtype=torch.float64, device="cuda"), h)
+    out = d.apply(phi)
+    d.check()
+    sym = torch.from_numpy(ks * np.tanh(ks * h)).cuda()
+    err = ((out - sym[:, None] * phi).abs().max(dim=1).values / sym).max()
+    assert float(err) <= 1e-11, float(err)
+    a, _ = si._family_surface(si.SEED_BASE + 3, N, 0.2, kmax=64)
+    d.refactor(torch.from_numpy(si.synth(N, a)[0]).cuda())
+    wide = d.apply(phi)
+    halves = torch.cat([d.apply(phi[:320].contiguous()), d.apply(phi[320:].contiguous())])
+    d.check()
+    scale = wide.abs().max(dim=1).values
+    assert float(((wide - halves).abs().max(dim=1).values / scale).max()) <= 1e-12
 
 
 def test_cfg5_shallow_sampled_columns(sww, orc_ld):
@@ -224,7 +263,9 @@ def test_cfg5_shallow_sampled_columns(sww, orc_ld):
     out, d = gpu_linearized(c, cols)
     orc, base = oracle_linearized(orc_ld, c, cols)
     r = check_columns(out, orc, "f64", c.N, lin_scales(c, base, cols), "cfg5")
-    assert r["cols_with_floor_above_bar"] <= 6
+    # F_c = 4 N eps S_c / ||orc_c|| = 1.8e-12 / (k tanh(k h)) exceeds the bar for k = 1 only (3.6e-11; k = 2: 9.1e-12): the two
+    # k = 1 columns of the sample (cos and sin), as DESIGN.md section 6 states
+    assert r["cols_with_floor_above_bar"] == 2, r
     print("cfg5", r)
 
 
@@ -285,6 +326,48 @@ def test_nan_column_stays_in_its_column(sww):
     for col in (0, 1, 6, 7):
         assert np.array_equal(out[col], good[col])
     assert not np.isfinite(out[2]).any() and not np.isfinite(out[4]).any()
+
+
+def test_all_ones_payload_column(sww):
+    """a right-hand side filled with 0xFF bytes is a NaN with the payload the triangular solves reserve for "not computed yet":
+    it must behave like any other NaN column (no hang, no give-up status, its FFT partner spoiled, all other columns exact)"""
+    c = si.config3(256, 40)
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    good = d.apply(to_dev(c.dphi, None, "f64")).cpu().numpy()
+    bad_in = to_dev(c.dphi, None, "f64")
+    bad_in[6].view(torch.int64).fill_(-1)
+    out = d.apply(bad_in).cpu().numpy()
+    assert d.status() == 0
+    for col in range(40):
+        if col not in (6, 7):
+            assert np.array_equal(out[col], good[col]), col
+    assert np.isnan(out[6]).all()
+    assert np.array_equal(d.apply(to_dev(c.dphi, None, "f64")).cpu().numpy(), good)
+
+
+def test_repeated_solves_are_bit_identical_under_concurrent_copies(sww):
+    """the dataflow kernels hand tiles over through L2 without grid barriers: 500 repeated setup-free applies of the metric-point
+    batch (N = 2048, 512 columns) and 40 refactor + apply rounds while a second stream keeps copying 64 MB buffers must all
+    return the same bits, with a clean status"""
+    c = si.metric_point(512)
+    d = sww.DtN(to_dev(c.eta, None, "f64"), c.h)
+    phi = to_dev(c.dphi + c.deta, None, "f64")
+    ref = d.apply(phi).clone()
+    side = torch.cuda.Stream()
+    src = torch.empty(8 << 20, dtype=torch.float64, device="cuda").normal_()
+    dst = torch.empty_like(src)
+    out = torch.empty_like(ref)
+    bad = 0
+    for it in range(500):
+        with torch.cuda.stream(side):
+            dst.copy_(src, non_blocking=True)
+        if it % 12 == 11 and it < 480:
+            d.refactor(to_dev(c.eta, None, "f64"))
+        d.apply(phi, out=out)
+        bad += int(not torch.equal(out, ref))
+    torch.cuda.synchronize()
+    d.check()
+    assert bad == 0, f"{bad} of 500 repeated applies differed"
 
 
 def test_minimum_size(sww, orc_ld):

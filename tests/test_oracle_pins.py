@@ -528,6 +528,22 @@ def test_energy_mean_symmetry_under_time_stepping(orc_ld):
     assert np.abs(ld(bwd["phi"]) + ld(fwd["phi"])).max() < 1e-17
 
 
+def test_energy_absolute_scale(orc_ld):
+    """E = (1/2) int_0^{2 pi} [phi G phi + g eta^2] dx in closed form, so that the constant in front of the
+    oracle's sum is pinned (conservation alone passes with any factor):
+      eta = a cos x, phi = 0           ->  E = g a^2 pi / 2          (int cos^2 = pi);
+      eta = 0, phi = b cos(k x), h     ->  E = b^2 k tanh(k h) pi / 2   (flat-surface symbol (4.34))."""
+    N = 64
+    x = si.grid(N)
+    a, g = 0.05, 1.7
+    E = orc_ld.rhs(a * np.cos(x), np.zeros(N), 1.0, g)["energy"]
+    assert abs(float(ld((np.array([E[0]]), np.array([E[1]])))[0]) - 0.5 * g * a * a * math.pi) < 1e-17
+    b, k, h = 0.3, 3, 0.7
+    E = orc_ld.rhs(np.zeros(N), b * np.cos(k * x), h, g)["energy"]
+    want = 0.5 * b * b * k * math.tanh(k * h) * math.pi
+    assert abs(float(E[0] + E[1]) - want) < 1e-15 * want + 1e-17
+
+
 def test_variational_columns_track_finite_differences(orc_ld):
     """(3.32): the column batch advanced with q equals d/de of the advanced nonlinear state."""
     N, h, g = 32, 1.0, 1.0
