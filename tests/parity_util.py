@@ -76,7 +76,7 @@ def check_columns(gpu, orc, prec, N, S, what=""):
     d = np.abs(diff(gpu, orc)).max(axis=1)
     ref = np.abs(ld(orc)).max(axis=1)
     S = np.asarray(S, dtype=LD)
-    worst, nfloor = 0.0, 0
+    worst, nfloor, floor_cols = 0.0, 0, []
     for c in range(d.shape[0]):
         if ref[c] == 0:
             assert d[c] <= bar * 4 * N * S[c], f"{what} column {c}: zero oracle column, |gpu| = {float(d[c]):.3e}"
@@ -84,10 +84,12 @@ def check_columns(gpu, orc, prec, N, S, what=""):
         e = float(d[c] / ref[c])
         floor = float(4 * N * eps * S[c] / ref[c])
         nfloor += floor > bar
+        if floor > bar:
+            floor_cols.append(c)
         assert e <= max(bar, floor), f"{what} column {c}: E_col = {e:.3e} > max(bar {bar:.1e}, floor {floor:.3e})"
         worst = max(worst, e)
     e_blk = float(d.max() / ref.max()) if ref.max() > 0 else 0.0
-    return {"E_col_max": worst, "E_blk": e_blk, "cols_with_floor_above_bar": int(nfloor)}
+    return {"E_col_max": worst, "E_blk": e_blk, "cols_with_floor_above_bar": int(nfloor), "floor_cols": floor_cols}
 
 
 def lin_scales(case: si.Case, base, cols=None):
