@@ -16,12 +16,13 @@
 // diagonal blocks are carried as deviations F_m = inv(S_m) - 2 I.
 // Product code; shares nothing with oracle/.
 #include "common.cuh"
+#include "bgj.cuh"
 #include <algorithm>
 #include <vector>
 
 namespace sww {
 
-constexpr double PIVOT_GUARD = 1e-3;
+constexpr double PIVOT_GUARD = BGJ_PIVOT_GUARD;
 constexpr int TR_MAXNS = 256;  // column slabs per TRSM launch (more columns: several launches)
 constexpr int TS = 64;    // tile size
 constexpr int LDT = 65;   // leading dimension of the row-major work tiles T, Eb, Fb (element (r,c) at r*LDT + c)
@@ -174,141 +175,63 @@ __global__ void __launch_bounds__(256) k_lu_single(double* __restrict__ A, int n
     getrf64(T, vec, status, tid, A, (size_t)nb, Eout, Fout, nb, nb);
 }
 
-// ------------------------------------------------------------------------------------------------ 64 x 64 Gauss-Jordan inverse
-// In-place inversion of S = I/2 + kappa by 64 Gauss-Jordan steps, 256 threads, thread (ty, tx) of a 16 x 16 grid keeping the
-// 4 x 4 register tile rows ty + 16 q, columns tx + 16 b.  The diagonal is carried as a DEVIATION: kappa_jj = S_jj - 1/2 before
-// pivot j is processed, Z_jj - 2 afterwards (the update formulas never touch the nominal part), so the result is F = inv(S) - 2 I
-// with every entry accurate relative to its own size.  Per step the owners publish column j and row j in shared memory
-// (double-buffered: one barrier per step); the rest is 16 register FMAs per thread.  vec: 256 doubles.
-// reciprocal of a pivot (|p| ~ 1/2, far from the denormal / overflow ranges the slow path of 1.0 / p guards against):
-// MUFU seed (relative error <= 2^-20) + two Newton steps (2^-40, 2^-80): within an ulp of 1/p
-__device__ __forceinline__ double pivot_rcp(double p) {
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(p));
-    double e = fma(-p, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-p, r, 1.0);
-    r = fma(r, e, r);
-    return r;
-}
-
-// The pivot row and the pivot column are folded into the rank-1 update itself: the column owner publishes p - 1 in place of
-// the pivot (a - (p - 1)(a / p) = a / p for the pivot row) and the pivot column uses the multiplier 1 + 1/p
-// (f - f (1 + 1/p) = -f / p); only the pivot entry itself is set separately (-2 kappa_jj / p = 1/p - 2 without cancellation).
-// explicit 32-bit shared-window accesses: with generic pointers the compiler rebuilds the window base (S2UR + ULEA) in front
-// of every predicated store, on the critical path of each elimination step
-__device__ __forceinline__ double lds64(unsigned addr) {
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ void sts64(unsigned addr, double v) { asm volatile("st.shared.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory"); }
-
-template <int JB>
-__device__ __forceinline__ void gj64_steps(double (&a)[4][4], unsigned vec_s, int tid, double& pmin) {
-    const int ty = tid & 15, tx = tid >> 4;
-    const unsigned pf = vec_s + 8 * ty;                // column j at rows ty + 16 q
-    const unsigned pu = vec_s + 8 * (64 + tx);         // row j at columns tx + 16 b
-    const unsigned pp = vec_s + 8 * (64 + 16 * JB);
-#pragma unroll 1
-    for (int jt = 0; jt < 16; jt++) {
-        const unsigned par = (jt & 1) * 1024;
-        const bool pcol = (tx == jt), prow = (ty == jt);
-        if (pcol) {
-#pragma unroll
-            for (int q = 0; q < 4; q++) sts64(pf + par + 128 * q, (q == JB && prow) ? a[q][JB] - 0.5 : a[q][JB]);
-        }
-        if (prow) {
-#pragma unroll
-            for (int b = 0; b < 4; b++) sts64(pu + par + 128 * b, a[JB][b]);
-        }
-        __syncthreads();
-        const double dj = lds64(pp + par + 8 * jt);
-        const double piv = 0.5 + dj;
-        const double r = pivot_rcp(piv);
-        pmin = fmin(pmin, fabs(piv));
-        double f[4], ut[4];
-#pragma unroll
-        for (int q = 0; q < 4; q++) f[q] = lds64(pf + par + 128 * q);
-#pragma unroll
-        for (int b = 0; b < 4; b++) ut[b] = lds64(pu + par + 128 * b) * r;
-        if (pcol) ut[JB] = 1.0 + r;
-#pragma unroll
-        for (int q = 0; q < 4; q++)
-#pragma unroll
-            for (int b = 0; b < 4; b++) a[q][b] = fma(-f[q], ut[b], a[q][b]);
-        if (pcol && prow) a[JB][JB] = -2.0 * dj * r;
-    }
-}
-
-// T (row-major, LDT) holds kappa = S - I/2.  On return F = inv(S) - 2 I is in Fg (global, column-major, ld 64) and in Fs_sm
-// (shared, operand layout Bs[n][k] = F[k][n], ld LDO).  Every thread of the CTA must call it; hook() is called (by every
-// thread) after 32 steps (argument 0) and 48 steps (argument 1) -- the spine uses it to start fetching the next step's inputs.
-template <class Hook>
-__device__ __forceinline__ void gj64(const double* T, double* vec, int* status, int tid, double* Fg, double* Fs_sm, Hook&& hook) {
-    const int ty = tid & 15, tx = tid >> 4;
-    double a[4][4];
-#pragma unroll
-    for (int q = 0; q < 4; q++)
-#pragma unroll
-        for (int b = 0; b < 4; b++) a[q][b] = T[(ty + 16 * q) * LDT + tx + 16 * b];
-    double pmin = 1.0;
-    const unsigned vec_s = (unsigned)__cvta_generic_to_shared(vec);
-    gj64_steps<0>(a, vec_s, tid, pmin);
-    gj64_steps<1>(a, vec_s, tid, pmin);
-    hook(0);
-    gj64_steps<2>(a, vec_s, tid, pmin);
-    hook(1);
-    gj64_steps<3>(a, vec_s, tid, pmin);
-    if (tid == 0 && !(pmin >= PIVOT_GUARD)) atomicCAS(status, SWW_OK, SWW_ESINGULAR);  // every thread sees every pivot
-#pragma unroll
-    for (int b = 0; b < 4; b++)
-#pragma unroll
-        for (int q = 0; q < 4; q++) {
-            const int row = ty + 16 * q, col = tx + 16 * b;
-            Fg[col * TS + row] = a[q][b];
-            Fs_sm[col * LDO + row] = a[q][b];
-        }
-}
-
 // ------------------------------------------------------------------------------------------------ the persistent dataflow LU
 // BLOCK LU without pivoting, 64 x 64 tiles:  A = L U  with identity diagonal blocks in L and the Schur complements S_m on the
 // block diagonal of U; what is stored is  L_im = X_im Z_m  (i > m),  U_mj = X_mj  (j > m)  and  F_m = Z_m - 2 I,  Z_m = inv(S_m),
 // where  X_ij = A_ij - sum_{k < min(i,j)} L_ik U_kj.  (Well posed: every S_m is I/2 plus a small block.)
-// The recurrence of the diagonal,  S_m = [A_mm - sum_{k<m-1} L_mk U_km] - (X_{m,m-1} Z_{m-1}) U_{m-1,m},  is the critical path.
-// It runs on ONE dedicated CTA (the "spine", block 0) with no flag hop inside a step: Gauss-Jordan inverse of S_{m-1}, then two
-// 64^3 DMMA products; everything it needs from outside (X_{m,m-1}, U_{m-1,m} and the partial sum P_m) depends on Z_{m-2} at the
-// latest, so it arrives while the spine inverts.  All other CTAs are workers claiming tile tasks in level order:
-//     U tile (i < j)   : X_ij, final as soon as the left-looking sum is done;
-//     L tile (i > j+1) : X_ij, then wait for Z_j and store L_ij = 2 X + X F_j;
-//     X tile (j+1, j)  : X only (the spine turns it into L_{j+1,j} on its way);
-//     P tile (m, m)    : the partial sum over k < m-1, in place.
+//
+// The recurrence of the diagonal,  S_m = P_m - X_{m,m-1} Z_{m-1} U_{m-1,m}  with  P_m = A_mm - sum_{k<m-1} L_mk U_km,  is the
+// critical path.  It runs on ONE dedicated CTA (the "spine", block 0): blocked Gauss-Jordan inverse of S_{m-1} on the tensor
+// pipe (bgj.cuh), then V = Z_{m-1} U_{m-1,m} and S_m = P_m - X_{m,m-1} V (two 64^3 DMMA products), all in shared memory; its
+// three inputs are fetched while the previous inverse runs.  Everything else is done by worker CTAs claiming tile tasks from a
+// counter.  A tile of level l = min(i,j) sums its terms k < l-1 from finished tiles; its LAST term needs Z_{l-1}, which has only
+// just been published -- waiting for a neighbour task to turn X_{i,l-1} into L_{i,l-1} first would put two tasks and two trips
+// through L2 between consecutive inverses.  So every task forms the L it needs for its last term itself, L = X Z_{l-1} (a
+// chained pair of products right behind the flag of Z_{l-1}), from an X that is available long before:
+//     lower (i > j)  : sum over k < j-1; wait for Z_{j-1}; L_{i,j-1} = X_{i,j-1} Z_{j-1}; X_ij = sum - L_{i,j-1} U_{j-1,j}, stored in
+//                      place (xready) -- for j = i-1 in the staging block Xs[i] (xflags), the tile itself keeps A; then the
+//                      finished L_{i,j-1} overwrites X_{i,j-1} (final).  Every lower tile is finished by its right neighbour.
+//     upper (i < j)  : sum over k < i-1; wait for Z_{i-1}; L_{i,i-1} = Xs[i] Z_{i-1}; U_ij = sum - L_{i,i-1} U_{i-1,j} (final); the
+//                      tile next to the diagonal (j = i+1) also stores L_{i,i-1} (row nt-1 has a task that does only that).
+//     P (i, i)       : partial sum P_i over k < i-2, then the term of k = i-2 from X_{i,i-2} in the same way, in place; it
+//                      tells the task of tile (i, i-1) when it has read X_{i,i-2} (pflags), which may then overwrite it.
 // A tile is published by a release store of the launch's epoch into its flag; consumers acquire-poll.  Tasks are claimed in
-// level order (level = min(i,j); P_{m+1}, whose inputs belong to levels < m, opens level m), so a claimed task waits only for tasks
-// claimed earlier or for the spine, and the spine waits only for tasks of earlier levels: no deadlock, no grid barrier.
+// order of the generation g of the inverse Z_g they wait for (build_order); every other dependency of a task is on a task of an
+// earlier generation (pflags: earlier in the same generation), and the spine computing Z_m waits only for tasks of
+// generation m - 2: a claimed task waits only for tasks claimed earlier or for the spine -- no deadlock, no grid barrier.
+constexpr int LU_THREADS = BGJ_CTA_THREADS;  // 352: 8 MMA warps (tid < 256) + the extra warps the inversion's role map needs
+enum LuTaskType { T_U = 0, T_L = 1, T_P = 2 };
+__host__ __device__ constexpr int lu_task(int type, int i, int j) { return (type << 28) | (i << 14) | j; }
+// kl: the term a tile forms from X and Z on the fly (upper: i-1, lower: j-1, diagonal P: i-2); its plain terms are k < kl
+__host__ __device__ constexpr int lu_kl(int i, int j) { return i < j ? i - 1 : (i > j ? j - 1 : i - 2); }
+
 struct LuArgs {
     double* A;         // N x N column-major, in place
     int N, nt;         // nt = N / 64 tiles per side
     int ntasks;
-    const int* order;  // worker tasks: (i << 16) | j in claim order
+    const int* order;  // worker tasks in claim order: lu_task(type, i, j)
     unsigned* flags;   // nt*nt: flags[i*nt + j] == epoch  <=>  tile (i,j) is final (i != j) / P_i is ready (i == j)
-    unsigned* xflags;  // nt: X_{m,m-1} is in place
+    unsigned* xready;  // nt*nt: X_ij is in place (lower tiles, j < i-1)
+    unsigned* xflags;  // nt: X_{m,m-1} is in Xs[m]
+    unsigned* pflags;  // nt: the P task of row m has read X_{m,m-2}
     unsigned* zflags;  // nt: F_m is in Fs
     unsigned epoch;
     unsigned* counter;  // next task to claim (zeroed before the launch)
     double* Fs;        // nt blocks of 64 x 64 (column-major, ld 64): inv(S_m) - 2 I
+    double* Xs;        // nt blocks of 64 x 64 (column-major, ld 64): staging of X_{m,m-1}
     int* status;
 };
 
-constexpr int LU_SMEM_BYTES = (4 * TS * LDO + TS * LDT + 256) * (int)sizeof(double) + 256;
+constexpr int LU_SMEM_BYTES = (5 * TS * LDO + BGJ_SCRATCH) * (int)sizeof(double) + 256;
 
-// fragment coordinates of this lane: rows wr*32 + x*8 + fr (x < 4), columns wc*16 + y*8 + 2 fk + e (y, e < 2)
+// fragment coordinates of this lane (threads 0..255): rows wr*32 + x*8 + fr (x < 4), columns wc*16 + y*8 + 2 fk + e (y, e < 2)
 struct Frag {
     int wr, wc, fr, fk;
-    __device__ __forceinline__ Frag(int tid) : wr((tid >> 5) & 1), wc(tid >> 6), fr((tid & 31) >> 2), fk(tid & 3) {}
+    __device__ __forceinline__ Frag(int tid) : wr((tid >> 5) & 1), wc((tid >> 6) & 3), fr((tid & 31) >> 2), fk(tid & 3) {}
     __device__ __forceinline__ int row(int x) const { return wr * 32 + x * 8 + fr; }
     __device__ __forceinline__ int col(int y, int e) const { return wc * 16 + y * 8 + 2 * fk + e; }
 };
+#define SWW_FRAG_LOOP for (int x = 0; x < 4; x++) for (int y = 0; y < 2; y++) for (int e = 0; e < 2; e++)
 
 // acc += As x Bs over one 64-deep slab; As[k][r] (ld LDO), Bs[n][k] (ld LDO)
 __device__ __forceinline__ void mma_tile64(double (&acc)[4][2][2], const double* a, const double* b, const Frag& f) {
@@ -327,9 +250,9 @@ __device__ __forceinline__ void mma_tile64(double (&acc)[4][2][2], const double*
             for (int y = 0; y < 2; y++) lu_dmma884(acc[x][y][0], acc[x][y][1], af[x], bf[y]);
     }
 }
-// 64 x 64 column-major tile (leading dimension ld) -> shared, ld LDO, same orientation; 256 threads, cp.async (not committed)
-__device__ __forceinline__ void tile_async(double* dst, const double* src, size_t ld, int tid) {
-    for (int c = tid; c < TS * TS / 2; c += 256) {
+// 64 x 64 column-major tile (leading dimension ld) -> shared, ld LDO, same orientation; thread t of nthr, cp.async (not committed)
+__device__ __forceinline__ void tile_async(double* dst, const double* src, size_t ld, int t, int nthr) {
+    for (int c = t; c < TS * TS / 2; c += nthr) {
         const int col = c >> 5, ch = (c & 31) * 2;
         cp16(dst + col * LDO + ch, src + (size_t)col * ld + ch);
     }
@@ -338,158 +261,164 @@ __device__ __forceinline__ void tile_async(double* dst, const double* src, size_
 __device__ __forceinline__ void spin_until(const unsigned* f, unsigned epoch) {
     while (ld_acquire(f) != epoch) __nanosleep(20);
 }
-
-// ---- the spine: block 0
-__device__ void lu_spine(const LuArgs& p, double* sA, double* sB, double* T, double* vec) {
-    const int tid = threadIdx.x;
-    const Frag f(tid);
-    const int N = p.N, nt = p.nt;
-    const unsigned epoch = p.epoch;
-    double* sA0 = sA;               // X_{m,m-1}
-    double* sA1 = sA + TS * LDO;    // P_m, then L_{m,m-1}
-    double* sB0 = sB;               // F_{m-1}, written by gj64
-    double* sB1 = sB + TS * LDO;    // U_{m-1,m}
-    __shared__ int s_ready;
-    // the three input flags of step m, polled by lanes 0..2 of warp 0 in parallel (an acquire load is an L2 round trip);
-    // returns (to every lane of warp 0) whether all are set; block: spin until they are
-    auto inputs_ready = [&](int m, bool block) -> bool {  // warp 1 (warp 0's lane 0 is busy publishing: fence + release)
-        const int q = tid - 32;
-        const unsigned* fl = (q == 0) ? p.xflags + m : (q == 1) ? p.flags + (size_t)(m - 1) * nt + m : p.flags + (size_t)m * nt + m;
-        const bool mine = (q < 2) || (q == 2 && m >= 2);  // P_1 is the raw diagonal tile
-        bool ok = true;
-        if (mine) {
-            if (block) spin_until(fl, epoch);
-            else ok = (ld_acquire(fl) == epoch);
-        }
-        return __all_sync(0xffffffffu, ok);
-    };
-    auto issue_inputs = [&](int m) {
-        tile_async(sA0, p.A + (size_t)(m - 1) * TS * N + (size_t)m * TS, N, tid);   // tile (m, m-1)
-        tile_async(sB1, p.A + (size_t)m * TS * N + (size_t)(m - 1) * TS, N, tid);   // tile (m-1, m)
-        tile_async(sA1, p.A + (size_t)m * TS * N + (size_t)m * TS, N, tid);         // tile (m, m)
-        cp_commit();
-    };
-    bool pre = false;  // the inputs of this step were requested before the previous inversion started
-    for (int m = 0; m < nt; m++) {
-        if (m == 0) {
-            const double* Cg = p.A;
-            for (int e = tid; e < TS * TS; e += 256) {
-                const int r = e & 63, c = e >> 6;
-                T[r * LDT + c] = Cg[(size_t)c * N + r];
-            }
-        } else {
-            double* Xg = p.A + (size_t)(m - 1) * TS * N + (size_t)m * TS;
-            if (!pre) {
-                if (tid >= 32 && tid < 64) inputs_ready(m, true);
-                __syncthreads();
-                issue_inputs(m);
-            }
-            cp_wait<0>();
-            __syncthreads();
-            double c0[4][2][2], acc[4][2][2];
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) {
-                        c0[x][y][e] = sA1[f.col(y, e) * LDO + f.row(x)];
-                        acc[x][y][e] = 2.0 * sA0[f.col(y, e) * LDO + f.row(x)];
-                    }
-            mma_tile64(acc, sA0, sB0, f);  // L_{m,m-1} = 2 X + X F_{m-1}
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) {
-                        Xg[(size_t)f.col(y, e) * N + f.row(x)] = acc[x][y][e];
-                        sA1[f.col(y, e) * LDO + f.row(x)] = acc[x][y][e];  // same thread, same slot as the P entry it read
-                        acc[x][y][e] = 0.0;
-                    }
-            __syncthreads();
-            if (tid == 0) {
-                __threadfence();
-                st_release(p.flags + (size_t)m * nt + (m - 1), epoch);
-            }
-            mma_tile64(acc, sA1, sB1, f);  // L_{m,m-1} U_{m-1,m}
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) T[f.row(x) * LDT + f.col(y, e)] = c0[x][y][e] - acc[x][y][e];
-        }
-        __syncthreads();  // T complete; sA0, sA1, sB1 free
-        pre = false;
-        // Non-blocking look at the inputs of step m + 1 (they become final about a third of the way into this inversion): after 32
-        // elimination steps lanes 0..2 of warp 1 issue one relaxed flag load each, after 48 steps the values are looked at
-        // (the L2 round trip is hidden behind 16 steps); if all three flags are set, the tiles are fetched while the last 16
-        // steps run.  No fence here (a gpu-scope fence in the middle of the inversion costs 2 us): the tile reads are
-        // cp.async.cg, served by L2 -- the point of coherence the producer's release made the tiles visible at before the
-        // flag -- and they are issued after a CTA barrier behind the flag observation.  Otherwise step m + 1 waits (with
-        // acquire loads) for its inputs at its start.
-        unsigned pending = 0;
-        const unsigned* myflag = nullptr;
-        if (m + 1 < nt && tid >= 32 && tid < 35) {
-            const int q = tid - 32, mn = m + 1;
-            if (q == 0) myflag = p.xflags + mn;
-            if (q == 1) myflag = p.flags + (size_t)m * nt + mn;
-            if (q == 2 && mn >= 2) myflag = p.flags + (size_t)mn * nt + mn;  // P_1 is the raw diagonal tile
-        }
-        auto try_prefetch = [&](int k) {
-            if (m + 1 >= nt) return;
-            if (k == 0) {
-                if (myflag) pending = ld_relaxed(myflag);
-                return;
-            }
-            if (tid >= 32 && tid < 64) {
-                const bool ok = __all_sync(0xffffffffu, !myflag || pending == epoch);
-                if (tid == 32) s_ready = ok;
-            }
-            __syncthreads();
-            pre = s_ready;
-            __syncthreads();
-            if (pre) issue_inputs(m + 1);
-        };
-        gj64(T, vec, p.status, tid, p.Fs + (size_t)m * TS * TS, sB0, try_prefetch);
-        __syncthreads();
-        if (tid == 0) {
-            __threadfence();
-            st_release(p.zflags + m, epoch);
-        }
+// for the few waits that sit on the spine's critical path: no back-off
+__device__ __forceinline__ void spin_tight(const unsigned* f, unsigned epoch) {
+    while (ld_acquire(f) != epoch) {
     }
 }
 
-__global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
-    extern __shared__ __align__(16) double lu_sm[];
-    double* sA = lu_sm;                   // 2 stages of L_ik as As[k][r]
-    double* sB = sA + 2 * TS * LDO;       // 2 stages of U_kj as Bs[n][k]
-    double* T = sB + 2 * TS * LDO;        // spine: work tile (row-major)
-    double* vec = T + TS * LDT;           // spine: gj64 scratch (256 doubles)
-    unsigned char* ready = reinterpret_cast<unsigned char*>(vec + 256);  // ready[k]: both operand tiles of step k are final
-    __shared__ int s_task;
-    const int tid = threadIdx.x;
-    if (blockIdx.x == 0) {
-        lu_spine(p, sA, sB, T, vec);
-        return;
+#ifdef SWW_LU_TRACE  // development aid, compiled out of the product (build.py never defines it): per-step time stamps of the spine
+__device__ unsigned long long g_lu_trace[4 * 128 + 3 * 8 * 128];
+__device__ __forceinline__ void lu_stamp(int m, int k) {
+    if (threadIdx.x == 0) {
+        unsigned long long t;
+        asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+        g_lu_trace[4 * m + k] = t;
     }
+}
+#define SWW_STAMP(m, k) lu_stamp(m, k)
+// worker stamps of the three tasks that feed the spine: which = 0 (tile (i, i-1)), 1 (tile (i-1, i)), 2 (P_i); 8 stamps per task
+#define SWW_WSTAMP(k)                                                                                              \
+    do {                                                                                                           \
+        const int which_ = (type == T_L && j == i - 1) ? 0 : (type == T_U && j == i + 1) ? 1 : (type == T_P) ? 2 : -1; \
+        if (which_ >= 0 && threadIdx.x == 0) {                                                                     \
+            unsigned long long t_;                                                                                 \
+            asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_));                                                 \
+            g_lu_trace[4 * 128 + (which_ * 128 + (which_ == 1 ? i + 1 : i)) * 8 + (k)] = t_;                      \
+        }                                                                                                          \
+    } while (0)
+#else
+#define SWW_STAMP(m, k)
+#define SWW_WSTAMP(k)
+#endif
+
+// ---- the spine: block 0
+__device__ void lu_spine(const LuArgs& p, double* sm) {
+    double* sX = sm;                  // X_{m,m-1}                 (A operand: As[k][r])
+    double* sU = sX + TS * LDO;       // U_{m-1,m}                 (B operand: Bs[n][k])
+    double* sF = sU + TS * LDO;       // F_{m-1}, written by bgj64 (A operand)
+    double* sV = sF + TS * LDO;       // V = Z_{m-1} U_{m-1,m}     (B operand)
+    double* sT = sV + TS * LDO;       // P_m (column-major, ld LDO), then kappa_m = S_m - I/2 (row-major, ld LDT) for bgj64
+    double* scr = sT + TS * LDO;
+    const int tid = threadIdx.x;
     const Frag f(tid);
+    const bool mm = tid < 256;        // the 8 MMA warps of the two products
     const int N = p.N, nt = p.nt;
     const unsigned epoch = p.epoch;
+    const int role = bgj_role(tid >> 5);
+    const int at = role * 32 + (tid & 31);  // index among the BGJ_THREADS threads that are inside bgj64 (role >= 0)
+    __shared__ int s_ready;
+    // the three input flags of step m: Xs[m], tile (m-1, m), P_m (P_1 is the raw diagonal tile)
+    auto input_flag = [&](int m, int q) -> const unsigned* {
+        if (q == 0) return p.xflags + m;
+        if (q == 1) return p.flags + (size_t)(m - 1) * nt + m;
+        return (m >= 2) ? p.flags + (size_t)m * nt + m : nullptr;
+    };
+    auto issue_inputs = [&](int m, int t, int nthr) {
+        tile_async(sX, p.Xs + (size_t)m * TS * TS, TS, t, nthr);
+        tile_async(sU, p.A + (size_t)m * TS * N + (size_t)(m - 1) * TS, N, t, nthr);   // tile (m-1, m)
+        tile_async(sT, p.A + (size_t)m * TS * N + (size_t)m * TS, N, t, nthr);         // tile (m, m)
+        cp_commit();
+    };
+    // The two warps that have no role in the inversion (bgj_role < 0) fetch the inputs of the next step meanwhile: they wait for
+    // the three flags (acquire) and issue the tile copies, which land in sX, sU, sT while the other warps invert -- none of the
+    // three regions is touched by bgj64 once the idle warps are back from it (sT has been read by then).
+    const int it = (tid >> 5) == 4 ? (tid & 31) : 32 + (tid & 31);  // index among the 64 idle threads (warps 4 and 8)
+    auto fetch_inputs = [&](int m) {
+        if (it < 3) {
+            const unsigned* fl = input_flag(m, it);
+            if (fl) spin_tight(fl, epoch);
+        }
+        asm volatile("bar.sync 4, 64;" ::: "memory");  // the two idle warps
+        issue_inputs(m, it, 64);
+        cp_wait<0>();
+    };
+    for (int m = 0; m < nt; m++) {
+        SWW_STAMP(m, 0);
+        if (m == 0) {
+            for (int e = tid; e < TS * TS; e += LU_THREADS) {
+                const int r = e & 63, c = e >> 6;
+                sT[r * LDT + c] = p.A[(size_t)c * N + r];
+            }
+        } else {
+            SWW_STAMP(m, 1);
+            double v[4][2][2], c0[4][2][2];
+            if (mm) {  // V = Z_{m-1} U_{m-1,m} = 2 U + F U
+#pragma unroll
+                SWW_FRAG_LOOP v[x][y][e] = 2.0 * sU[f.col(y, e) * LDO + f.row(x)];
+                mma_tile64(v, sF, sU, f);
+#pragma unroll
+                SWW_FRAG_LOOP sV[f.col(y, e) * LDO + f.row(x)] = v[x][y][e];
+            }
+            __syncthreads();
+            if (mm) {  // S_m = P_m - X_{m,m-1} V
+#pragma unroll
+                SWW_FRAG_LOOP {
+                    c0[x][y][e] = sT[f.col(y, e) * LDO + f.row(x)];
+                    v[x][y][e] = 0.0;
+                }
+                mma_tile64(v, sX, sV, f);
+            }
+            __syncthreads();  // P has been read: sT becomes the row-major work tile
+            if (mm) {
+#pragma unroll
+                SWW_FRAG_LOOP sT[f.row(x) * LDT + f.col(y, e)] = c0[x][y][e] - v[x][y][e];
+            }
+        }
+        __syncthreads();  // kappa_m complete; sX, sU, sV free
+        SWW_STAMP(m, 2);
+        bgj64(sT, scr, p.status, tid, p.Fs + (size_t)m * TS * TS, sF);
+        if (role < 0 && m + 1 < nt) fetch_inputs(m + 1);  // (the idle warps are back once sT has been read)
+        __syncthreads();  // F_m in sF and in global memory; the inputs of step m + 1 in shared memory
+        SWW_STAMP(m, 3);
+        if (tid == LU_THREADS - 32) st_release(p.zflags + m, epoch);  // a lane of a warp that has no part in the two products
+    }
+}
 
+__global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
+    extern __shared__ __align__(16) double lu_sm[];
+    const int tid = threadIdx.x;
+    if (blockIdx.x == 0) {
+        lu_spine(p, lu_sm);
+        return;
+    }
+    double* sA = lu_sm;                   // 2 stages of L_ik as As[k][r]
+    double* sB = sA + 2 * TS * LDO;       // 2 stages of U_kj as Bs[n][k]
+    unsigned char* ready = reinterpret_cast<unsigned char*>(sB + 2 * TS * LDO);  // ready[k]: both operand tiles of step k are final
+    __shared__ int s_task;
+    const Frag f(tid);
+    const bool mm = tid < 256;
+    const int N = p.N, nt = p.nt;
+    const unsigned epoch = p.epoch;
+    auto tile = [&](int r, int c) { return p.A + (size_t)c * TS * N + (size_t)r * TS; };
+    // after a CTA barrier behind the stores: the barrier orders every thread's stores before thread 0's release (which is a
+    // gpu-scope fence followed by the store; a separate __threadfence in front of it would fence twice)
+    auto publish = [&](unsigned* flag) {
+        if (tid == 0) st_release(flag, epoch);
+    };
+
+    if (blockIdx.x == 1) {  // block row 0 and block column 0 are A itself: final / X-ready from the start
+        for (int t = tid; t < nt; t += LU_THREADS) {
+            st_release(p.flags + t, epoch);
+            st_release(p.xready + (size_t)t * nt, epoch);
+        }
+    }
     for (;;) {
         __syncthreads();  // the previous task is finished with s_task and the shared tiles
         if (tid == 0) s_task = (int)atomicAdd(p.counter, 1u);
         __syncthreads();
         const int task = s_task;
         if (task >= p.ntasks) break;
-        const int ij = p.order[task], i = ij >> 16, j = ij & 0xffff;
-        const int m = (i == j) ? i - 1 : min(i, j);  // number of finished block columns / rows this tile sums over
-        double* Cg = p.A + (size_t)j * TS * N + (size_t)i * TS;
+        const int code = p.order[task], type = code >> 28, i = (code >> 14) & 0x3fff, j = code & 0x3fff;
+        const bool has_tile = j < nt;  // the upper task (nt-1, nt) only finishes L_{nt-1,nt-2}
+        // kl: the term that is formed from X and Z on the fly (-1: none); the plain left-looking sum runs over k < m
+        const int kl = has_tile ? lu_kl(i, j) : i - 1;
+        const int m = (has_tile && kl > 0) ? kl : 0;
+        double* Cg = has_tile ? tile(i, j) : nullptr;
+        SWW_WSTAMP(0);
 
         auto refresh = [&]() {
-            for (int t = tid; t < m; t += 256)
+            for (int t = tid; t < m; t += LU_THREADS)
                 ready[t] = (ld_acquire(p.flags + (size_t)i * nt + t) == epoch) && (ld_acquire(p.flags + (size_t)t * nt + j) == epoch);
         };
         auto wait_ready = [&](int k) {  // uniform: ready[] is only written before a __syncthreads
@@ -504,21 +433,17 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
             }
         };
         auto issue = [&](int k, int buf) {
-            tile_async(sA + buf * TS * LDO, p.A + (size_t)k * TS * N + (size_t)i * TS, N, tid);
-            tile_async(sB + buf * TS * LDO, p.A + (size_t)j * TS * N + (size_t)k * TS, N, tid);
+            tile_async(sA + buf * TS * LDO, tile(i, k), N, tid, LU_THREADS);
+            tile_async(sB + buf * TS * LDO, tile(k, j), N, tid, LU_THREADS);
             cp_commit();
         };
         // own tile -> registers (fragment layout), sum = 0
         double c0[4][2][2], acc[4][2][2];
 #pragma unroll
-        for (int x = 0; x < 4; x++)
-#pragma unroll
-            for (int y = 0; y < 2; y++)
-#pragma unroll
-                for (int e = 0; e < 2; e++) {
-                    c0[x][y][e] = Cg[(size_t)f.col(y, e) * N + f.row(x)];
-                    acc[x][y][e] = 0.0;
-                }
+        SWW_FRAG_LOOP {
+            c0[x][y][e] = (mm && has_tile) ? Cg[(size_t)f.col(y, e) * N + f.row(x)] : 0.0;
+            acc[x][y][e] = 0.0;
+        }
         refresh();
         __syncthreads();
         if (m > 0) {
@@ -534,66 +459,96 @@ __global__ void __launch_bounds__(256, 1) k_lu_dataflow(LuArgs p) {
                 cp_wait<0>();
             }
             __syncthreads();
-            mma_tile64(acc, sA + (k & 1) * TS * LDO, sB + (k & 1) * TS * LDO, f);
+            if (mm) mma_tile64(acc, sA + (k & 1) * TS * LDO, sB + (k & 1) * TS * LDO, f);
             __syncthreads();
             if (!pre && k + 1 < m) {
                 wait_ready(k + 1);
                 issue(k + 1, (k + 1) & 1);
             }
         }
-        // X = A_ij - sum
+        auto store_tile = [&](double* dst, size_t ld, const double (&v)[4][2][2]) {
+            if (mm) {
 #pragma unroll
-        for (int x = 0; x < 4; x++)
-#pragma unroll
-            for (int y = 0; y < 2; y++)
-#pragma unroll
-                for (int e = 0; e < 2; e++) c0[x][y][e] -= acc[x][y][e];
-        unsigned* flag = p.flags + (size_t)i * nt + j;
-        if (i > j + 1) {
-            // L_ij = 2 X + X F_j
-            if (tid == 0) spin_until(p.zflags + j, epoch);
+                SWW_FRAG_LOOP dst[(size_t)f.col(y, e) * ld + f.row(x)] = v[x][y][e];
+            }
+        };
+        // ---- the last term, k = kl: L = X Z_kl = 2 X + X F_kl formed here, then sum += L U_{kl,j}
+        // X: the left neighbour X_{i,kl} in place (lower tiles, P) or the staging block Xs[i] (upper tiles)
+        double l[4][2][2];
+        const bool finish_left = kl >= 0 && (type == T_L || (type == T_U && j == i + 1));
+        SWW_WSTAMP(1);
+        if (kl >= 0) {
+            const bool upper = (type == T_U);
+            const double* Xg = upper ? p.Xs + (size_t)i * TS * TS : tile(i, kl);
+            const size_t ldx = upper ? (size_t)TS : (size_t)N;
+            if (tid < 2) {  // inputs that are final long before Z_kl
+                const unsigned* fl = (tid == 0) ? (upper ? p.xflags + i : p.xready + (size_t)i * nt + kl)
+                                                : (has_tile ? p.flags + (size_t)kl * nt + j : nullptr);
+                if (fl) spin_until(fl, epoch);
+            }
             __syncthreads();
-            tile_async(sB, p.Fs + (size_t)j * TS * TS, TS, tid);
+            tile_async(sA, Xg, ldx, tid, LU_THREADS);                                  // X_{i,kl}
+            if (has_tile) tile_async(sB + TS * LDO, tile(kl, j), N, tid, LU_THREADS);  // U_{kl,j}
             cp_commit();
-#pragma unroll
-            for (int x = 0; x < 4; x++)
-#pragma unroll
-                for (int y = 0; y < 2; y++)
-#pragma unroll
-                    for (int e = 0; e < 2; e++) {
-                        sA[f.col(y, e) * LDO + f.row(x)] = c0[x][y][e];  // As[k = col][r = row]
-                        c0[x][y][e] *= 2.0;
-                    }
+            SWW_WSTAMP(2);
+            if (tid == 0) spin_tight(p.zflags + kl, epoch);
+            __syncthreads();
+            SWW_WSTAMP(3);
+            tile_async(sB, p.Fs + (size_t)kl * TS * TS, TS, tid, LU_THREADS);          // F_kl
+            cp_commit();
             cp_wait<0>();
             __syncthreads();
-            mma_tile64(c0, sA, sB, f);
-        } else if (i == j + 1) {
-            flag = p.xflags + i;
+            SWW_WSTAMP(4);
+            if (type == T_P && tid == 0) st_release(p.pflags + i, epoch);  // X_{i,i-2} has been read (nothing was written: no fence)
+            if (mm) {
+#pragma unroll
+                SWW_FRAG_LOOP l[x][y][e] = 2.0 * sA[f.col(y, e) * LDO + f.row(x)];
+                mma_tile64(l, sA, sB, f);
+#pragma unroll
+                SWW_FRAG_LOOP sA[TS * LDO + f.col(y, e) * LDO + f.row(x)] = l[x][y][e];  // L as an A operand, second stage
+            }
+            // The finished left neighbour L_{i,kl} goes out at once: the tasks of the next generation sum it as a plain term and
+            // must be through with that before Z_{kl+1} arrives.
+            if (finish_left) {
+                if (type == T_L && j == i - 1 && i >= 2) {  // the P task of this row reads X_{i,i-2} too
+                    if (tid == 0) spin_until(p.pflags + i, epoch);
+                    __syncthreads();
+                }
+                store_tile(tile(i, kl), N, l);
+            }
+            __syncthreads();
+            if (finish_left) publish(p.flags + (size_t)i * nt + kl);
+            if (mm && has_tile) mma_tile64(acc, sA + TS * LDO, sB + TS * LDO, f);
         }
+        SWW_WSTAMP(5);
 #pragma unroll
-        for (int x = 0; x < 4; x++)
-#pragma unroll
-            for (int y = 0; y < 2; y++)
-#pragma unroll
-                for (int e = 0; e < 2; e++) Cg[(size_t)f.col(y, e) * N + f.row(x)] = c0[x][y][e];
-        __syncthreads();  // every thread's stores are issued
-        if (tid == 0) {
-            __threadfence();
-            st_release(flag, epoch);
+        SWW_FRAG_LOOP c0[x][y][e] -= acc[x][y][e];
+        // ---- publish X_ij / U_ij / P_i
+        if (has_tile) {
+            const bool staged = (type == T_L && j == i - 1);
+            store_tile(staged ? p.Xs + (size_t)i * TS * TS : Cg, staged ? (size_t)TS : (size_t)N, c0);
+            __syncthreads();
+            publish(staged ? p.xflags + i : (type == T_L ? p.xready + (size_t)i * nt + j : p.flags + (size_t)i * nt + j));
+            SWW_WSTAMP(6);
         }
     }
 }
 
-// claim order: level m = 0, 1, ...: the partial sum P_{m+1} of the next diagonal tile (its inputs belong to levels < m), the two
-// tiles next to the diagonal, then the rest of block column / block row m by distance from the diagonal
+// Claim order: generation g = -1, 0, 1, ... of the inverse Z_g a task waits for; within a generation first what the spine
+// needs for step g + 2 (P_{g+2} -- ahead of the task of tile (g+2, g+1), which waits for its pflag --, the tiles (g+2, g+1) and
+// (g+1, g+2)), then block column g+1 / block row g+1 by distance from the diagonal.  Block row 0 and block column 0 need no
+// task (A itself), except tile (1, 0), which is copied to its staging block.
 static void build_order(int nt, std::vector<int>& o) {
     o.clear();
-    for (int m = 0; m < nt; m++) {
-        if (m + 1 >= 2 && m + 1 < nt) o.push_back(((m + 1) << 16) | (m + 1));
-        for (int d = 1; m + d < nt; d++) {
-            o.push_back(((m + d) << 16) | m);
-            o.push_back((m << 16) | (m + d));
-        }
+    for (int g = -1; g <= nt - 2; g++) {
+        if (g + 2 >= 2 && g + 2 <= nt - 1) o.push_back(lu_task(T_P, g + 2, g + 2));
+        if (g + 2 <= nt - 1) o.push_back(lu_task(T_L, g + 2, g + 1));
+        if (g >= 0) o.push_back(lu_task(T_U, g + 1, g + 2));  // j = nt for the last row: only finishes L_{nt-1,nt-2}
+        if (g >= 0)
+            for (int d = 1; g + 2 + d <= nt - 1; d++) {
+                o.push_back(lu_task(T_L, g + 2 + d, g + 1));
+                o.push_back(lu_task(T_U, g + 1, g + 2 + d));
+            }
     }
 }
 
@@ -608,7 +563,7 @@ int lu_alloc(sww_dtn_s* d) {
     std::vector<int> o;
     build_order(nt, o);
     d->lu_ntasks = (int)o.size();
-    const size_t nflags = (size_t)nt * nt + 2 * nt + 1;
+    const size_t nflags = 2 * (size_t)nt * nt + 3 * nt + 1;
     if (cudaMalloc(&d->lu_order, sizeof(int) * o.size()) != cudaSuccess) return SWW_ENOMEM;
     if (cudaMalloc(&d->lu_flags, sizeof(unsigned) * nflags) != cudaSuccess) return SWW_ENOMEM;
     SWW_CUDA(cudaMemcpyAsync(d->lu_order, o.data(), sizeof(int) * o.size(), cudaMemcpyHostToDevice, d->stream));
@@ -622,7 +577,7 @@ int lu_alloc(sww_dtn_s* d) {
 int run_lu(sww_dtn_s* d) {
     const int N = d->N, nb = (N < NB) ? N : NB, nblk = N / nb;
     cudaStream_t st = d->stream;
-    double* Es = d->invD;
+    double* Es = d->invD;                           // N <= 64: inv(L) - I ; larger N: the staging blocks Xs of the dataflow LU
     double* Fs = d->invD + (size_t)nblk * nb * nb;
     constexpr int SINGLE_SMEM = (TS * LDT + 576) * (int)sizeof(double);
     static DeviceOnce attr_once;
@@ -645,19 +600,28 @@ int run_lu(sww_dtn_s* d) {
     a.order = d->lu_order;
     a.counter = d->lu_flags;
     a.flags = d->lu_flags + 1;
-    a.xflags = a.flags + (size_t)nblk * nblk;
-    a.zflags = a.xflags + nblk;
+    a.xready = a.flags + (size_t)nblk * nblk;
+    a.xflags = a.xready + (size_t)nblk * nblk;
+    a.pflags = a.xflags + nblk;
+    a.zflags = a.pflags + nblk;
     a.epoch = ++d->lu_epoch;
     a.Fs = Fs;
+    a.Xs = Es;
     a.status = d->status;
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), st));
     const int grid = std::min(sm_count(), 1 + a.ntasks);
     SWW_BEGIN(KC_LU, st);
-    k_lu_dataflow<<<grid, 256, LU_SMEM_BYTES, st>>>(a);
+    k_lu_dataflow<<<grid, LU_THREADS, LU_SMEM_BYTES, st>>>(a);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
 }
+
+#ifdef SWW_LU_TRACE
+extern "C" int sww_debug_lu_trace(unsigned long long* dst, int n) {
+    return cudaMemcpyFromSymbol(dst, g_lu_trace, sizeof(unsigned long long) * n) == cudaSuccess ? 0 : -3;
+}
+#endif
 
 // N <= 64 (a single diagonal block): one CTA per column, x = (2 I + F)(I + E) b with the same compensation as below
 __global__ void __launch_bounds__(64) k_solve_small(int N, const double* __restrict__ E, const double* __restrict__ F,
