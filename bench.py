@@ -116,56 +116,142 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "source": "fallback (B200_PROFILING.md)"}
 
 
-def cpu_oracle_columns_per_s(nrhs_target: int, small: int = 8, large: int = 136):
-    """the long-double oracle as it stands, timed on this host: setup + `small` and setup + `large` columns of the metric-point
-    workload; columns/s extrapolated to nrhs_target columns sharing one setup."""
+WORKLOAD = (f"metric point: N={N_METRIC}, h=1, config-3 surface family, nrhs={NRHS_METRIC} linearized-DtN columns per GPU, "
+            "setup (assembly+LU) + base state + batched columns inside every step")
+
+
+def oracle_step(orc, c, n=None):
+    """one pass of the hot path through the CPU oracle: setup + base state + the first n (default: all) columns"""
+    n = c.nrhs if n is None else n
+    t0 = time.perf_counter()
+    orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:n], c.dphi[:n])
+    return time.perf_counter() - t0
+
+
+def cpu_oracle_baseline(nrhs: int):
+    """the oracle source built twice, timed as it stands on this host.  REAL=double (the fairer speed baseline,
+    same precision as the timed GPU path) runs the WHOLE workload once; REAL=long double (the parity oracle, with __float128
+    multipliers: a precision the GPU path does not compute in) runs a bounded sample, labelled as such."""
     import oracle
-    orc = oracle.Oracle("ld")
-    c = si.metric_point(nrhs_target)
-    ts = []
-    for n in (small, large):
-        t0 = time.perf_counter()
-        orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:n], c.dphi[:n])
-        ts.append(time.perf_counter() - t0)
-    t_col = max((ts[1] - ts[0]) / (large - small), 0.0)  # the setup (pivoted elimination of one 2048^2 matrix) dominates
-    t_setup = max(ts[0] - small * t_col, 0.0)
-    value = nrhs_target / (t_setup + nrhs_target * t_col)
-    return {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
-            "sample": f"long-double oracle, N={c.N}: setup+base+{small} columns ({ts[0]:.2f} s) and setup+base+{large} columns ({ts[1]:.2f} s) "
-                      f"of the {nrhs_target}; columns/s extrapolated as {nrhs_target}/(t_setup + {nrhs_target} t_col), "
-                      f"t_setup={t_setup:.2f} s, t_col={t_col:.5f} s"}
+    c = si.metric_point(nrhs)
+    o64 = oracle.Oracle("f64")
+    t64 = oracle_step(o64, c)
+    old = oracle.Oracle("ld")
+    n_ld = 8
+    t_ld = oracle_step(old, c, n_ld)
+    return {"value": nrhs / t64, "unit": UNIT, "cores": o64.num_threads(), "kind": "oracle",
+            "sample": f"oracle built with REAL=double, N={c.N}: one full step = setup + base state + all {nrhs} columns in {t64:.2f} s "
+                      "(no extrapolation)",
+            "long_double": {"value": n_ld / t_ld, "unit": UNIT, "cores": old.num_threads(),
+                            "sample": f"the parity oracle (REAL=long double, __float128 multipliers): setup + base state + {n_ld} of the "
+                                      f"{nrhs} columns in {t_ld:.2f} s; columns/s of that sample (setup-dominated), not extrapolated"}}
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle (the only 'reference implementation' this paper-only tier has), rank 0 only."""
+    """--impl reference: the CPU oracle (the only 'reference implementation' this paper-only tier has), rank 0 only.
+    Every step is one full pass of the workload (setup + base state + all 512 columns) through the REAL=double build of the
+    oracle; ms_per_step is the measured time of exactly that."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     import oracle
-    orc = oracle.Oracle("ld")
+    orc = oracle.Oracle("f64")
     c = si.metric_point(NRHS_METRIC)
-    n_s, n_l = 8, 136
-    t0 = time.perf_counter()
-    orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:n_l], c.dphi[:n_l])
-    t_l = time.perf_counter() - t0
-    step = lambda: orc.dtn_linearized(c.eta, c.h, c.phi0, c.deta[:n_s], c.dphi[:n_s])
     for _ in range(args.warmup):
-        step()
+        oracle_step(orc, c)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        step()
+        oracle_step(orc, c)
     t_step = (time.perf_counter() - t0) / max(args.steps, 1)
-    t_col = max((t_l - t_step) / (n_l - n_s), 0.0)
-    t_setup = max(t_step - n_s * t_col, 0.0)
-    value = NRHS_METRIC / (t_setup + NRHS_METRIC * t_col)
-    sample = (f"each step = long-double oracle setup+base+{n_s} of the {NRHS_METRIC} columns at N={c.N} ({t_step:.2f} s); one untimed "
-              f"{n_l}-column call ({t_l:.2f} s) gives t_col={t_col:.5f} s; value = {NRHS_METRIC}/(t_setup + {NRHS_METRIC} t_col)")
+    value = NRHS_METRIC / t_step
+    sample = (f"each step = the whole workload through the oracle built with REAL=double: setup + base state + all {NRHS_METRIC} columns at "
+              f"N={c.N} ({t_step:.2f} s per step, {orc.num_threads()} threads); nothing extrapolated")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-            "warmup": args.warmup, "ms_per_step": 1e3 * (t_setup + NRHS_METRIC * t_col), "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f80 (x87 long double)", "data": "synthetic",
-            "config": {"workload": f"metric point: N={c.N}, h=1, config-3 surface family, nrhs={NRHS_METRIC} linearized-DtN columns, setup inside the step"},
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "N": N_METRIC, "nrhs_per_gpu": NRHS_METRIC},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
     print(json.dumps(line), flush=True)
+
+
+def time_events(fn, reps, flush=None):
+    """mean milliseconds of fn() over reps runs, CUDA events on the current stream, optional L2 flush between runs"""
+    import torch
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+    for e0, e1 in ev:
+        if flush is not None:
+            flush.zero_()
+        e0.record()
+        fn()
+        e1.record()
+    torch.cuda.synchronize()
+    return sum(e0.elapsed_time(e1) for e0, e1 in ev) / reps
+
+
+def other_configs(sww, flush, peak_tf):
+    """BASELINE.json configs 1-5 on the device (north_star: 'N from 64 to 4096'): one step = setup + base state + columns unless
+    stated; small configs are launch/latency-bound and are reported as time, config 5 also as a roofline fraction"""
+    import torch
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    out = {}
+
+    def lin_case(c, prec, reps):
+        if prec == sww.DD:
+            pk = lambda hi, lo: torch.from_numpy(np.stack([hi, lo])).cuda().contiguous()
+            eta, phi0, de, dp = pk(c.eta, c.eta_lo), pk(c.phi0, c.phi0_lo), pk(c.deta, c.deta_lo), pk(c.dphi, c.dphi_lo)
+        else:
+            eta, phi0, de, dp = dev(c.eta), dev(c.phi0), dev(c.deta), dev(c.dphi)
+        res = torch.empty_like(dp)
+        d = sww.DtN(eta, c.h, prec)
+
+        def step():
+            d.refactor(eta)
+            d.set_base(phi0)
+            d.linearized_apply(de, dp, res)
+        for _ in range(3):
+            step()
+        d.check()
+        ms = time_events(step, reps, flush)
+        d.close()
+        return ms
+
+    c1 = si.config1()
+    eta1, phi1 = dev(c1.eta), dev(c1.dphi)
+    d1 = sww.DtN(eta1, c1.h)
+    o1 = torch.empty_like(phi1)
+
+    def step1():
+        d1.refactor(eta1)
+        d1.apply(phi1, o1)
+    for _ in range(3):
+        step1()
+    ms = time_events(step1, 50)
+    out["config1"] = {"workload": "N=64, 1 right-hand side: setup + apply", "ms_per_step": ms, "bound": "latency (12 launches)"}
+    d1.close()
+
+    c2 = si.config2()
+    st = sww.State(dev(c2.eta), dev(c2.phi0), c2.h, c2.g)
+    st.advance(c2.meta["dt"], 2)
+    nst = 8
+    ms = time_events(lambda: st.advance(c2.meta["dt"], nst), 3) / nst
+    out["config2"] = {"workload": "N=256 standing wave, RK8 (11 stages, one setup + solve per stage)", "ms_per_rk_step": ms,
+                      "rk_steps_per_s": 1e3 / ms, "ms_per_stage": ms / 11, "bound": "latency (4-block LU chain + ~25 launches per stage)"}
+    st.close()
+
+    c3 = si.config3()
+    ms = lin_case(c3, sww.F64, 20)
+    out["config3"] = {"workload": "N=512, 256 columns, fp64", "ms_per_step": ms, "columns_per_s": c3.nrhs / (ms * 1e-3),
+                      "bound": "latency (8-block LU chain, launch sequence)"}
+    c4 = si.config4()
+    ms = lin_case(c4, sww.DD, 10)
+    out["config4"] = {"workload": "N=512, 128 columns, double-double", "ms_per_step": ms, "columns_per_s": c4.nrhs / (ms * 1e-3),
+                      "bound": "FP64 ALU (error-free-transformation kernels)"}
+    c5 = si.config5()
+    ms = lin_case(c5, sww.F64, 5)
+    fl = (2.0 / 3.0) * c5.N ** 3 + 2.0 * c5.N ** 2 * (c5.nrhs + 2) + 2.0 * c5.N ** 2 * c5.nrhs
+    out["config5"] = {"workload": "N=4096, h=0.05, 512 columns, fp64", "ms_per_step": ms, "columns_per_s": c5.nrhs / (ms * 1e-3),
+                      "tflops": fl / (ms * 1e-3) / 1e12, "frac_of_fp64_tensor_roofline": fl / (ms * 1e-3) / 1e12 / peak_tf, "bound": "FP64 tensor"}
+    return out
 
 
 def main():
@@ -177,6 +263,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-dd", action="store_true", help="skip the double-double leg")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-configs", action="store_true", help="skip the block that times BASELINE.json configs 1-5")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
@@ -345,20 +432,23 @@ def main():
             # one dd multiply-add (dd_fma, dd.cuh) is 15 dependent fp64 instructions; the bound is the fp64 pipe issue rate = DFMA probe FLOP/s / 2
             ddres["frac_of_dfma_issue_peak"] = (ddfma / t_ddg) * 15 / (probe["dfma_tflops"] * 1e12 / 2)
 
+    configs = None
+    if rank == 0 and not args.no_configs:
+        configs = other_configs(sww, flush, peak_tf)
+
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        cpu = cpu_oracle_columns_per_s(nrhs)
+        cpu = cpu_oracle_baseline(nrhs)
 
     if rank == 0:
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
                 "data": "synthetic",
-                "config": {"workload": f"metric point: N={N}, h=1, config-3 surface family, nrhs={nrhs} linearized-DtN columns per GPU, "
-                                       "setup (assembly+LU) + base state + batched columns inside every step",
+                "config": {"workload": WORKLOAD,
                            "N": N, "nrhs_per_gpu": nrhs, "parallelism": f"columns sharded over {world} GPU(s), no data-path collective",
                            "l2": "256 MB buffer written between timed iterations (L2 flush), outside the event pairs"},
                 "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "gpu_launches_per_step": launches / K,
-                "roofline": roofline, "kernels": kernels, "dd": ddres, "cpu_baseline": cpu,
+                "roofline": roofline, "kernels": kernels, "dd": ddres, "configs": configs, "cpu_baseline": cpu,
                 "wall_s_timed_region_incl_flush": t_wall}
         print(json.dumps(line), flush=True)
     if dist is not None:

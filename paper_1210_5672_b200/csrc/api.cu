@@ -61,22 +61,22 @@ static int apply_f64(sww_dtn_s* d, const double* rhs_dev /* N x nrhs, or NULL wh
     return SWW_OK;
 }
 
-int dd_apply(sww_dtn_s* d, const double* rhs_dev, bool rhs_in_ws, const double* Tcols, int nrhs, double* out);
-int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out);
 
-static int do_setup(sww_dtn_s* d, const void* eta) {
+// eta_lo: the low words (double-double handles; nullptr = the N doubles behind eta)
+int setup_surface(sww_dtn_s* d, const double* eta, const double* eta_lo) {
     const int N = d->N;
     d->has_base = false;
+    SWW_CUDA(cudaMemcpyAsync(d->eta, eta, sizeof(double) * N, cudaMemcpyDeviceToDevice, d->stream));
     if (d->prec == SWW_F64) {
-        SWW_CUDA(cudaMemcpyAsync(d->eta, eta, sizeof(double) * N, cudaMemcpyDeviceToDevice, d->stream));
         SWW_CUDA(cudaMemsetAsync(d->eta + N, 0, sizeof(double) * N, d->stream));
         SWW_TRY(run_setup_f64(d));
     } else {
-        SWW_CUDA(cudaMemcpyAsync(d->eta, eta, sizeof(double) * 2 * N, cudaMemcpyDeviceToDevice, d->stream));
+        SWW_CUDA(cudaMemcpyAsync(d->eta + N, eta_lo ? eta_lo : eta + N, sizeof(double) * N, cudaMemcpyDeviceToDevice, d->stream));
         SWW_TRY(run_setup_dd(d));
     }
     return run_lu(d);
 }
+static int do_setup(sww_dtn_s* d, const void* eta) { return setup_surface(d, (const double*)eta, nullptr); }
 
 }  // namespace sww
 

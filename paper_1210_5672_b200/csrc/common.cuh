@@ -66,6 +66,7 @@ struct Tables {
     double* dc;    // differentiation circulant: (1/2) (-1)^m cot(pi m / N), m >= 1; dc[0] = 0, dc[N/2] = 0
     double2* tw;   // fp64 FFT twiddles exp(-2 pi i m / N) = (cs, -sn) rounded, m = 0..N-1
     double* filt;  // 36th-order filter exp(-36 (|k|/(N/2))^36) of (2.14) at DFT index m (|k| = min(m, N - m))
+    double* filt_dd;  // the same in double-double (planar 2N)
 };
 int get_tables(int N, cudaStream_t st, const Tables** out);
 
@@ -137,7 +138,12 @@ int gemm_f64(cudaStream_t st, int M, int Nc, int K, double alpha, const double* 
 int gemv_few_f64(cudaStream_t st, int M, int nc, int K, const double* A, int lda, const double* B, int ldb, double* C, int ldc, double* part,
                  unsigned* count);
 // accurate base state (ddpath.cu): phi0', W0, u, v of (2.9) with mu0 refined to dd; phi0 is dd planar iff prec == SWW_DD
-int accurate_base(sww_dtn_s* d, const double* phi0);
+int accurate_base(sww_dtn_s* d, const double* phi0, size_t phi_plane = 0);
+// double-double apply / linearized apply (ddpath.cu); Lin, Lout: plane sizes of the dd planar inputs / output (0 = N * nrhs)
+int dd_apply(sww_dtn_s* d, const double* rhs_dev, bool rhs_in_ws, const double* Tcols, int nrhs, double* out, size_t Lin = 0, size_t Lout = 0);
+int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out, size_t Lin = 0, size_t Lout = 0);
+// S0-S2 for a new surface (api.cu); eta_lo: low words of a double-double surface held apart from the high words (nullptr: at eta + N)
+int setup_surface(sww_dtn_s* d, const double* eta, const double* eta_lo);
 // the plain fp64 base state (fp64 handles only; see ddpath.cu for when the stepper may use it)
 int fast_base_f64(sww_dtn_s* d, const double* phi0);
 // fused dd pass (assembly.cu): res = b - mu/2 - K mu, w = G gam with the kernel entries evaluated in dd on the fly; all dd planar 2N

@@ -8,7 +8,7 @@
 // Product code; shares nothing with oracle/.
 #include "common.cuh"
 #include "dd.cuh"
-#include <cstdlib>
+#include "ddfft.cuh"
 
 namespace sww {
 
@@ -274,11 +274,36 @@ __global__ void __launch_bounds__(256) k_gemm_dd(int N, int ncols, size_t L, con
     }
 }
 
+// N < 64 (one tile would be mostly padding): Y = zs Z + beta X + alpha A X, one thread per element
+__global__ void k_gemm_dd_small(int N, size_t L, const double* __restrict__ A, const double* __restrict__ Alo, const double* __restrict__ X,
+                                double zs, const double* __restrict__ Z, double beta, double alpha, double* __restrict__ Y,
+                                double* __restrict__ Y_f64) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x, c = blockIdx.y;
+    if (i >= N) return;
+    dd acc{0.0, 0.0};
+    for (int k = 0; k < N; k++) {
+        const size_t o = (size_t)k * N + i, ox = (size_t)c * N + k;
+        acc = dd_fma(dd{A[o], Alo ? Alo[o] : 0.0}, dd{X[ox], X[L + ox]}, acc);
+    }
+    const size_t o = (size_t)c * N + i;
+    dd v{alpha * acc.hi, alpha * acc.lo};
+    if (beta != 0.0) v = dd_add(v, dd{beta * X[o], beta * X[L + o]});
+    if (zs != 0.0) v = dd_add(v, dd{zs * Z[o], zs * Z[L + o]});
+    Y[o] = v.hi;
+    Y[L + o] = v.lo;
+    if (Y_f64) Y_f64[o] = v.hi;
+}
+
 static int gemm_dd(sww_dtn_s* d, int ncols, size_t L, const double* A, const double* Alo, const double* X, double zs, const double* Z,
                    double beta, double alpha, double* Y, double* Y_f64) {
     const int N = d->N;
-    if (N < DG_BM) {  // tiny N: column by column through the mat-vec kernel (planes are L apart, so repack is not needed when ncols == 1)
-        return SWW_EINVAL;
+    if (N < DG_BM) {  // N = 16, 32: one thread per output element
+        dim3 grid((N + 31) / 32, ncols);
+        SWW_BEGIN(KC_DDGEMM, d->stream);
+        k_gemm_dd_small<<<grid, 32, 0, d->stream>>>(N, L, A, Alo, X, zs, Z, beta, alpha, Y, Y_f64);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+        return SWW_OK;
     }
     const bool narrow = (long)(N / DG_BM) * ((ncols + 31) / 32) < 100;  // too few wide tiles to occupy the chip
     const int bn = narrow ? 16 : 32;
@@ -351,47 +376,6 @@ __global__ void k_rhs_lin_dd(int N, size_t total, size_t Lin, size_t Lws, const 
     R[e] = b.hi;
 }
 
-// ------------------------------------------------------------------------------------------------ dd FFT (column pairs)
-struct cdd {
-    dd re, im;
-};
-__device__ __forceinline__ cdd cdd_add(cdd a, cdd b) { return cdd{dd_add(a.re, b.re), dd_add(a.im, b.im)}; }
-__device__ __forceinline__ cdd cdd_sub(cdd a, cdd b) { return cdd{dd_sub(a.re, b.re), dd_sub(a.im, b.im)}; }
-// a * (wr + i wi)
-__device__ __forceinline__ cdd cdd_mul(cdd a, dd wr, dd wi) {
-    return cdd{dd_sub(dd_mul(a.re, wr), dd_mul(a.im, wi)), dd_add(dd_mul(a.re, wi), dd_mul(a.im, wr))};
-}
-__device__ void fft_dif_dd(cdd* z, int N, const double* __restrict__ cs, const double* __restrict__ sn) {
-    for (int half = N >> 1; half >= 1; half >>= 1) {
-        int tstride = N / (2 * half);
-        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
-            int blk = t / half, o = t - blk * half, i = blk * 2 * half + o, m = o * tstride;
-            cdd a = z[i], b = z[i + half];
-            dd wr = dd_load(cs, N, m), wi = dd_neg(dd_load(sn, N, m));  // exp(-2 pi i m/N)
-            z[i] = cdd_add(a, b);
-            z[i + half] = cdd_mul(cdd_sub(a, b), wr, wi);
-        }
-        __syncthreads();
-    }
-}
-__device__ void ifft_dit_dd(cdd* z, int N, const double* __restrict__ cs, const double* __restrict__ sn) {
-    for (int half = 1; half < N; half <<= 1) {
-        int tstride = N / (2 * half);
-        for (int t = threadIdx.x; t < N / 2; t += blockDim.x) {
-            int blk = t / half, o = t - blk * half, i = blk * 2 * half + o, m = o * tstride;
-            cdd a = z[i];
-            cdd b = cdd_mul(z[i + half], dd_load(cs, N, m), dd_load(sn, N, m));  // conj twiddle exp(+2 pi i m/N)
-            z[i] = cdd_add(a, b);
-            z[i + half] = cdd_sub(a, b);
-        }
-        __syncthreads();
-    }
-}
-__device__ __forceinline__ int wavenumber_dd(int p, int N, int logN) {
-    int k = (int)(__brev((unsigned)p) >> (32 - logN));
-    if (2 * k == N) return 0;
-    return (2 * k < N) ? k : k - N;
-}
 // Gam_c = D M_c ;  W_c = |D| M_c / 2 - (T ? D T_c : 0), dd planar in/out (plane sizes Lws for M, T, Gam; Lw for W)
 __global__ void __launch_bounds__(512) k_spectral_gamma_w_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
                                                              size_t Lws, size_t Lw, const double* __restrict__ M, const double* __restrict__ T,
@@ -468,14 +452,14 @@ __global__ void k_dd_add(int N, const double* a, const double* b, double* out) {
 }
 
 // ------------------------------------------------------------------------------------------------ flow (1): accurate base state
-// phi0: dd planar (2N) when d->prec == SWW_DD, N doubles otherwise.  Uses d->tmp (14N doubles) and column 0 of ws.T|R and ws.S.
+// phi0: dd planar when d->prec == SWW_DD (lo plane at phi0 + phi_plane; 0 = N), N doubles otherwise.  Uses d->tmp (14N doubles) and column 0 of ws.T|R and ws.S.
 //   dd handle : mu0 by refinement sweeps around the fp64 LU with residuals from the stored dd K; W0 from the stored dd G.
 //   f64 handle: the stored K, G are fp64-rounded, which is not enough here (their rounding alone leaves ~2e-15 of white noise in
 //               v at N = 2048, and every linearized column multiplies v into its right-hand side and differentiates: 3e-12 in
 //               the output).  One fused pass evaluates the kernels in dd on the fly (assembly.cu, base_pass_dd):
 //               mu~ = LU \ phi0 ; gam~ = D mu~ ; [res, w~] = [phi0 - mu~/2 - K mu~, G gam~] (dd) ; delta = LU \ res ;
 //               mu0 = mu~ + delta ; W0 = H D mu0 / 2 + w~ + G_f64 (D delta)   (2.7), (2.8).
-int accurate_base(sww_dtn_s* d, const double* phi0) {
+int accurate_base(sww_dtn_s* d, const double* phi0, size_t phi_plane) {
     const int N = d->N;
     cudaStream_t st = d->stream;
     const bool isdd = d->prec == SWW_DD;
@@ -492,7 +476,7 @@ int accurate_base(sww_dtn_s* d, const double* phi0) {
     double* rlo = d->ws.S;
     unsigned blocks = (unsigned)((N + 255) / 256);
     SWW_BEGIN(KC_OTHER, st);
-    k_dd_copy<<<blocks, 256, 0, st>>>((size_t)N, (size_t)N, (size_t)N, isdd ? 1 : 0, phi0, b, rcol);
+    k_dd_copy<<<blocks, 256, 0, st>>>((size_t)N, phi_plane ? phi_plane : (size_t)N, (size_t)N, isdd ? 1 : 0, phi0, b, rcol);
     SWW_LAUNCHED();
     if (isdd) {
         const int nsweep = DD_SWEEPS;
@@ -577,18 +561,18 @@ int fast_base_f64(sww_dtn_s* d, const double* phi0) {
 }
 
 // ------------------------------------------------------------------------------------------------ flow (2): dd apply
-// rhs: dd planar N x nrhs with plane size Lin (ignored when rhs_in_ws: ws.B (dd) and ws.R (fp64 rounding) are already filled).
-// Tcols: dd planar in ws layout or nullptr.  out: dd planar N x nrhs, plane size Lout = N * nrhs.
-int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcols, int nrhs, double* out) {
+// rhs: dd planar N x nrhs with plane size Lin (0 = N * nrhs; ignored when rhs_in_ws: ws.B (dd) and ws.R (fp64 rounding) are
+// already filled).  Tcols: dd planar in ws layout or nullptr.  out: dd planar N x nrhs, plane size Lout (0 = N * nrhs).
+int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcols, int nrhs, double* out, size_t Lin, size_t Lout) {
     const int N = d->N;
     if (N > 2048) return SWW_EINVAL;  // the dd FFT keeps two N-point complex dd arrays in shared memory (2 x 32 B x N <= 128 KB)
     cudaStream_t st = d->stream;
     Workspace& w = d->ws;
-    const size_t NN = (size_t)N * N, Lws = (size_t)N * w.cap_cols, Lio = (size_t)N * nrhs, n = Lio;
+    const size_t NN = (size_t)N * N, Lws = (size_t)N * w.cap_cols, n = (size_t)N * nrhs, Lio = Lout ? Lout : n;
     unsigned blocks = (unsigned)((n + 255) / 256);
     if (!rhs_in_ws) {
         SWW_BEGIN(KC_OTHER, st);
-        k_dd_copy<<<blocks, 256, 0, st>>>(n, Lio, Lws, 1, rhs, w.B, w.R);
+        k_dd_copy<<<blocks, 256, 0, st>>>(n, Lin ? Lin : n, Lws, 1, rhs, w.B, w.R);
         SWW_LAUNCHED();
     }
     double* mu = w.W;  // dd planar, ws layout
@@ -599,10 +583,7 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
         k_dd_axpy_f64<<<blocks, 256, 0, st>>>(n, Lws, s == 0, w.R, w.S, mu);
         SWW_LAUNCHED();
         if (s + 1 < nsweep) {  // R = B - mu/2 - K mu in dd, rounded to fp64 for the next LU solve
-            if (N >= DG_BM)
-                SWW_TRY(gemm_dd(d, nrhs, Lws, d->K, d->K + NN, mu, 1.0, w.B, -0.5, -1.0, w.Gam, w.R));
-            else
-                return SWW_EINVAL;
+            SWW_TRY(gemm_dd(d, nrhs, Lws, d->K, d->K + NN, mu, 1.0, w.B, -0.5, -1.0, w.Gam, w.R));
         }
     }
     static DeviceOnce attr_once;
@@ -628,15 +609,15 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
     return SWW_OK;
 }
 
-int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out) {
+int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out, size_t Lin, size_t Lout) {
     const int N = d->N;
     Workspace& w = d->ws;
-    const size_t Lws = (size_t)N * w.cap_cols, Lio = (size_t)N * nrhs;
+    const size_t Lws = (size_t)N * w.cap_cols, n = (size_t)N * nrhs;
     SWW_BEGIN(KC_OTHER, d->stream);
-    k_rhs_lin_dd<<<(unsigned)((Lio + 255) / 256), 256, 0, d->stream>>>(N, Lio, Lio, Lws, deta, dphi, d->bu, d->bv, w.B, w.T, w.R);
+    k_rhs_lin_dd<<<(unsigned)((n + 255) / 256), 256, 0, d->stream>>>(N, n, Lin ? Lin : n, Lws, deta, dphi, d->bu, d->bv, w.B, w.T, w.R);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
-    return dd_apply(d, nullptr, true, w.T, nrhs, out);
+    return dd_apply(d, nullptr, true, w.T, nrhs, out, 0, Lout);
 }
 
 }  // namespace sww

@@ -6,9 +6,11 @@
 //   deta_t  = w_c - D(u deta_c)          dphi_t  = P[ -D(deta_c u v) - u D(b_c) + v w_c - g deta_c ],  b_c = dphi_c - v deta_c,
 //   w_c = G[b_c],  every right-hand side multiplied by the filter, the state filtered after every step (R5).
 // One DtN setup (S0-S2), one base state and one batched linearized solve per stage, all through the entry points of api.cu.
-// State layout: y = [eta (N) | phi (N) | deta (N x nc) | dphi (N x nc)], fp64.  Product code; shares nothing with oracle/.
+// State layout: y = [eta (N) | phi (N) | deta (N x nc) | dphi (N x nc)] = L doubles; double-double states are planar (hi plane of
+// L doubles, then lo plane) and run through the kernels of rk_dd.cu.  Product code; shares nothing with oracle/.
 #include "common.cuh"
 #include "fft.cuh"
+#include "rk_dd.cuh"
 #include <new>
 #include <cstring>
 
@@ -27,12 +29,72 @@ struct sww_state_s {
     double* ys;          // stage state
     double* k;           // RK_S stage derivatives, L each
     double* w;           // N x nc: unfiltered deta_t of the current stage
-    double* red;         // 1 double: energy reduction
+    double* red;         // 2 doubles: energy reduction (hi, lo)
     double t;
     double a[RK_S][RK_S], b[RK_S], c[RK_S];
+    double alo[RK_S][RK_S], blo[RK_S];  // low words of the tableau (double-double states)
+    size_t mul() const { return prec == SWW_DD ? 2 : 1; }
 };
 
 namespace sww {
+
+// ---- the tableau in double-double: (p + q sqrt 21) / r with small integers p, q, r, by error-free transformations on the host
+struct hdd {
+    double hi, lo;
+};
+static hdd h_two_sum(double a, double b) {
+    const double s = a + b, bb = s - a;
+    return hdd{s, (a - (s - bb)) + (b - bb)};
+}
+static hdd h_add(hdd a, hdd b) {
+    hdd s = h_two_sum(a.hi, b.hi);
+    s.lo += a.lo + b.lo;
+    return h_two_sum(s.hi, s.lo);
+}
+static hdd h_mul_d(hdd a, double b) {
+    const double p = a.hi * b, e = fma(a.hi, b, -p) + a.lo * b;
+    return h_two_sum(p, e);
+}
+static hdd h_div_d(hdd a, double b) {  // b a small integer
+    const double q1 = a.hi / b;
+    const double r = fma(-q1, b, a.hi) + a.lo;  // exact remainder of the high word (fma) plus the low word
+    return h_two_sum(q1, r / b);
+}
+static hdd h_sqrt21() {
+    const double x = sqrt(21.0);
+    const double x2 = x * x, e = fma(x, x, -x2);            // x^2 = x2 + e exactly
+    return h_two_sum(x, ((21.0 - x2) - e) / (2.0 * x));      // one Newton step carried in the low word
+}
+static hdd h_coef(int p, int q, int r) {  // (p + q sqrt 21) / r
+    return h_div_d(h_add(hdd{(double)p, 0.0}, h_mul_d(h_sqrt21(), (double)q)), (double)r);
+}
+static void rk_tableau_dd(double a[RK_S][RK_S], double alo[RK_S][RK_S], double b[RK_S], double blo[RK_S]) {
+    memset(a, 0, sizeof(double) * RK_S * RK_S);
+    memset(alo, 0, sizeof(double) * RK_S * RK_S);
+    memset(b, 0, sizeof(double) * RK_S);
+    memset(blo, 0, sizeof(double) * RK_S);
+    auto A = [&](int i, int j, int p, int q, int r) {
+        const hdd v = h_coef(p, q, r);
+        a[i][j] = v.hi;
+        alo[i][j] = v.lo;
+    };
+    auto B = [&](int i, int p, int r) {
+        const hdd v = h_coef(p, 0, r);
+        b[i] = v.hi;
+        blo[i] = v.lo;
+    };
+    B(0, 1, 20); B(7, 49, 180); B(8, 16, 45); B(9, 49, 180); B(10, 1, 20);
+    A(1, 0, 1, 0, 2);
+    A(2, 0, 1, 0, 4); A(2, 1, 1, 0, 4);
+    A(3, 0, 1, 0, 7); A(3, 1, -7, -3, 98); A(3, 2, 21, 5, 49);
+    A(4, 0, 11, 1, 84); A(4, 2, 18, 4, 63); A(4, 3, 21, -1, 252);
+    A(5, 0, 5, 1, 48); A(5, 2, 9, 1, 36); A(5, 3, -231, 14, 360); A(5, 4, 63, -7, 80);
+    A(6, 0, 10, -1, 42); A(6, 2, -432, 92, 315); A(6, 3, 633, -145, 90); A(6, 4, -504, 115, 70); A(6, 5, 63, -13, 35);
+    A(7, 0, 1, 0, 14); A(7, 4, 14, -3, 126); A(7, 5, 13, -3, 63); A(7, 6, 1, 0, 9);
+    A(8, 0, 1, 0, 32); A(8, 4, 91, -21, 576); A(8, 5, 11, 0, 72); A(8, 6, -385, -75, 1152); A(8, 7, 63, 13, 128);
+    A(9, 0, 1, 0, 14); A(9, 4, 1, 0, 9); A(9, 5, -733, -147, 2205); A(9, 6, 515, 111, 504); A(9, 7, -51, -11, 56); A(9, 8, 132, 28, 245);
+    A(10, 4, -42, 7, 18); A(10, 5, -18, 28, 45); A(10, 6, -273, -53, 72); A(10, 7, 301, 53, 72); A(10, 8, 28, -28, 45); A(10, 9, 49, -7, 18);
+}
 
 // the tableau of DESIGN.md section 3 (R6): coefficients in Q(sqrt 21), evaluated in double
 static void rk_tableau(double a[RK_S][RK_S], double b[RK_S], double c[RK_S]) {
@@ -238,7 +300,26 @@ static int rk_set_attrs() {
 }
 
 // one evaluation of the right-hand sides at the stage state ys -> kout (same layout as the state)
+static int rk_rhs_dd(sww_state_s* s, const double* ys, double* kout) {
+    const int N = s->N, nc = s->nc;
+    const size_t L = s->L;
+    sww_dtn_s* d = s->dtn;
+    SWW_TRY(ensure_workspace(d, nc > 0 ? nc : 1));
+    SWW_TRY(setup_surface(d, ys, ys + L));          // S0-S2 for this stage's surface (eta: high and low planes)
+    SWW_TRY(accurate_base(d, ys + N, L));           // W0 = G phi, u, v of (2.9)
+    d->has_base = true;
+    SWW_TRY(rkdd_rhs_base(d, s->filter, s->g, L, ys, kout));
+    if (nc > 0) {
+        const double* deta = ys + 2 * (size_t)N;
+        const double* dphi = deta + (size_t)N * nc;
+        SWW_TRY(dd_linearized(d, deta, dphi, nc, s->w, L, 0));   // w_c - D(u deta_c)   (B.1d), (B.2)
+        SWW_TRY(rkdd_rhs_cols(d, s->filter, s->g, nc, L, ys, s->w, kout));
+    }
+    return SWW_OK;
+}
+
 static int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
+    if (s->prec == SWW_DD) return rk_rhs_dd(s, ys, kout);
     const int N = s->N, nc = s->nc, logN = fft_ilog2(N), thr = fft_threads(N);
     sww_dtn_s* d = s->dtn;
     cudaStream_t st = s->stream;
@@ -272,7 +353,20 @@ static int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
     return SWW_OK;
 }
 
-static int rk_combine(sww_state_s* s, const double* coef, int n, double dt, double* out) {
+static int rk_combine(sww_state_s* s, const double* coef, const double* coef_lo, int n, double dt, double* out) {
+    if (s->prec == SWW_DD) {
+        CombDD cd;
+        cd.n = 0;
+        for (int j = 0; j < n; j++)
+            if (coef[j] != 0.0) {
+                const hdd v = h_mul_d(hdd{coef[j], coef_lo[j]}, dt);
+                cd.idx[cd.n] = j;
+                cd.chi[cd.n] = v.hi;
+                cd.clo[cd.n] = v.lo;
+                cd.n++;
+            }
+        return rkdd_combine(s->stream, s->L, s->y, s->k, cd, out);
+    }
     Comb cb;
     cb.n = 0;
     for (int j = 0; j < n; j++)
@@ -295,8 +389,9 @@ extern "C" {
 int sww_state_create(int N, double h, double g, int prec, int ncols, const void* eta, const void* phi, const void* deta,
                      const void* dphi, unsigned flags, void* stream, sww_state_t* out) {
     if (!out || !eta || !phi || ncols < 0 || (ncols > 0 && (!deta || !dphi))) return SWW_EINVAL;
-    if (prec != SWW_F64) return SWW_EINVAL;  // the double-double stepper is not built yet
-    if (N > 4096) return SWW_EINVAL;         // k_rhs_cols keeps two N-point complex arrays in shared memory
+    if (prec != SWW_F64 && prec != SWW_DD) return SWW_EINVAL;
+    // k_rhs_cols / k_rhs_cols_dd keep two N-point complex arrays in shared memory (include/sww.h states the limits)
+    if (N > (prec == SWW_DD ? RKDD_MAX_N : 4096)) return SWW_EINVAL;
     sww_state_s* s = new (std::nothrow) sww_state_s();
     if (!s) return SWW_ENOMEM;
     memset(s, 0, sizeof(*s));
@@ -305,22 +400,31 @@ int sww_state_create(int N, double h, double g, int prec, int ncols, const void*
     s->stream = (cudaStream_t)stream;
     s->L = 2 * (size_t)N * (1 + (size_t)ncols);
     rk_tableau(s->a, s->b, s->c);
+    if (prec == SWW_DD) rk_tableau_dd(s->a, s->alo, s->b, s->blo);
     int rc = sww_dtn_setup(eta, N, h, prec, stream, &s->dtn);  // validates N, h; also the first factorisation
     if (rc) { delete s; return rc; }
-    bool ok = cudaMalloc(&s->y, sizeof(double) * s->L) == cudaSuccess && cudaMalloc(&s->ys, sizeof(double) * s->L) == cudaSuccess &&
-              cudaMalloc(&s->k, sizeof(double) * s->L * RK_S) == cudaSuccess &&
-              cudaMalloc(&s->w, sizeof(double) * (size_t)N * (ncols > 0 ? ncols : 1)) == cudaSuccess &&
-              cudaMalloc(&s->red, sizeof(double)) == cudaSuccess;
+    const size_t mul = s->mul();
+    bool ok = cudaMalloc(&s->y, sizeof(double) * s->L * mul) == cudaSuccess && cudaMalloc(&s->ys, sizeof(double) * s->L * mul) == cudaSuccess &&
+              cudaMalloc(&s->k, sizeof(double) * s->L * mul * RK_S) == cudaSuccess &&
+              cudaMalloc(&s->w, sizeof(double) * mul * (size_t)N * (ncols > 0 ? ncols : 1)) == cudaSuccess &&
+              cudaMalloc(&s->red, 2 * sizeof(double)) == cudaSuccess;
     if (!ok) { sww_state_destroy(s); return SWW_ENOMEM; }
     const size_t v = sizeof(double) * N, bsz = v * ncols;
     cudaStream_t st = s->stream;
-    if (cudaMemcpyAsync(s->y, eta, v, cudaMemcpyDeviceToDevice, st) || cudaMemcpyAsync(s->y + N, phi, v, cudaMemcpyDeviceToDevice, st) ||
-        (ncols && (cudaMemcpyAsync(s->y + 2 * (size_t)N, deta, bsz, cudaMemcpyDeviceToDevice, st) ||
-                   cudaMemcpyAsync(s->y + 2 * (size_t)N + (size_t)N * ncols, dphi, bsz, cudaMemcpyDeviceToDevice, st)))) {
-        sww_state_destroy(s);
-        return SWW_ECUDA;
+    // double-double inputs are planar per array (hi block, lo block); the state keeps one hi plane and one lo plane of L doubles
+    for (size_t pl = 0; pl < mul; pl++) {
+        double* y = s->y + pl * s->L;
+        const double *e = (const double*)eta + pl * N, *p = (const double*)phi + pl * N;
+        const double *de = ncols ? (const double*)deta + pl * (size_t)N * ncols : nullptr, *dp = ncols ? (const double*)dphi + pl * (size_t)N * ncols : nullptr;
+        if (cudaMemcpyAsync(y, e, v, cudaMemcpyDeviceToDevice, st) || cudaMemcpyAsync(y + N, p, v, cudaMemcpyDeviceToDevice, st) ||
+            (ncols && (cudaMemcpyAsync(y + 2 * (size_t)N, de, bsz, cudaMemcpyDeviceToDevice, st) ||
+                       cudaMemcpyAsync(y + 2 * (size_t)N + (size_t)N * ncols, dp, bsz, cudaMemcpyDeviceToDevice, st)))) {
+            sww_state_destroy(s);
+            return SWW_ECUDA;
+        }
     }
     rc = rk_set_attrs();
+    if (!rc && prec == SWW_DD) rc = rkdd_set_attrs();
     if (rc) { sww_state_destroy(s); return rc; }
     *out = s;
     return SWW_OK;
@@ -333,13 +437,15 @@ int sww_rk_advance(sww_state_t s, double dt, int nsteps) {
         for (int i = 0; i < RK_S; i++) {
             const double* ys = s->y;
             if (i > 0) {
-                SWW_TRY(rk_combine(s, s->a[i], i, dt, s->ys));
+                SWW_TRY(rk_combine(s, s->a[i], s->alo[i], i, dt, s->ys));
                 ys = s->ys;
             }
-            SWW_TRY(rk_rhs(s, ys, s->k + (size_t)i * s->L));
+            SWW_TRY(rk_rhs(s, ys, s->k + (size_t)i * s->L * s->mul()));
         }
-        SWW_TRY(rk_combine(s, s->b, RK_S, dt, s->y));
-        if (s->filter) {
+        SWW_TRY(rk_combine(s, s->b, s->blo, RK_S, dt, s->y));
+        if (s->filter && s->prec == SWW_DD) {
+            SWW_TRY(rkdd_filter_state(s->dtn, 2 + 2 * s->nc, s->L, s->y));
+        } else if (s->filter) {
             const int ncol = 2 + 2 * s->nc;
             SWW_BEGIN(KC_FFT, s->stream);
             k_filter_cols<<<(ncol + 1) / 2, fft_threads(N), sizeof(double2) * (size_t)N, s->stream>>>(N, logN, s->dtn->tab->tw, s->dtn->tab->filt,
@@ -356,10 +462,14 @@ int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, 
     if (!s) return SWW_EINVAL;
     const size_t v = sizeof(double) * s->N, bsz = v * s->nc;
     cudaStream_t st = s->stream;
-    if (eta) SWW_CUDA(cudaMemcpyAsync(eta, s->y, v, cudaMemcpyDeviceToDevice, st));
-    if (phi) SWW_CUDA(cudaMemcpyAsync(phi, s->y + s->N, v, cudaMemcpyDeviceToDevice, st));
-    if (deta && s->nc) SWW_CUDA(cudaMemcpyAsync(deta, s->y + 2 * (size_t)s->N, bsz, cudaMemcpyDeviceToDevice, st));
-    if (dphi && s->nc) SWW_CUDA(cudaMemcpyAsync(dphi, s->y + 2 * (size_t)s->N + (size_t)s->N * s->nc, bsz, cudaMemcpyDeviceToDevice, st));
+    for (size_t pl = 0; pl < s->mul(); pl++) {  // double-double: each output is planar (hi block, lo block)
+        const double* y = s->y + pl * s->L;
+        if (eta) SWW_CUDA(cudaMemcpyAsync((double*)eta + pl * s->N, y, v, cudaMemcpyDeviceToDevice, st));
+        if (phi) SWW_CUDA(cudaMemcpyAsync((double*)phi + pl * s->N, y + s->N, v, cudaMemcpyDeviceToDevice, st));
+        if (deta && s->nc) SWW_CUDA(cudaMemcpyAsync((double*)deta + pl * (size_t)s->N * s->nc, y + 2 * (size_t)s->N, bsz, cudaMemcpyDeviceToDevice, st));
+        if (dphi && s->nc)
+            SWW_CUDA(cudaMemcpyAsync((double*)dphi + pl * (size_t)s->N * s->nc, y + 2 * (size_t)s->N + (size_t)s->N * s->nc, bsz, cudaMemcpyDeviceToDevice, st));
+    }
     if (t) *t = s->t;
     return sww_dtn_status(s->dtn);  // synchronises the stream
 }
@@ -367,6 +477,15 @@ int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, 
 int sww_state_energy(sww_state_t s, double* energy_hl) {
     if (!s || !energy_hl) return SWW_EINVAL;
     sww_dtn_s* d = s->dtn;
+    if (s->prec == SWW_DD) {
+        SWW_TRY(ensure_workspace(d, 1));
+        SWW_TRY(setup_surface(d, s->y, s->y + s->L));
+        SWW_TRY(accurate_base(d, s->y + s->N, s->L));
+        d->has_base = true;
+        SWW_TRY(rkdd_energy(d, s->g, s->L, s->y, s->red));
+        SWW_CUDA(cudaMemcpyAsync(energy_hl, s->red, 2 * sizeof(double), cudaMemcpyDeviceToHost, s->stream));
+        return sww_dtn_status(d);
+    }
     SWW_TRY(sww_dtn_refactor(d, s->y));
     SWW_TRY(sww_dtn_set_base(d, s->y + s->N));
     SWW_BEGIN(KC_OTHER, s->stream);

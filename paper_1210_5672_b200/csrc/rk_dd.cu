@@ -1,0 +1,283 @@
+// rk_dd.cu -- the double-double instances of S8/S9: right-hand sides of (2.1) and of the variational equation
+// (B.1)-(B.3), (3.32), the filter (2.14), the stage combination and the energy
+// (PAPER.md:501), all in error-free-transformation arithmetic on the CUDA cores with double-double FFTs in shared memory --
+// the paper's quadruple-precision time stepping.  Same formulas and the same order as rk.cu.
+// State layout: planar, hi plane of L = 2 N (1 + nc) doubles then lo plane; within a plane [eta | phi | deta (N x nc) | dphi].
+// Product code; shares nothing with oracle/.
+#include "common.cuh"
+#include "dd.cuh"
+#include "ddfft.cuh"
+#include "rk_dd.cuh"
+
+namespace sww {
+
+constexpr int DDF_MAX_PER_THREAD = 4;  // ceil(N / blockDim.x): 2 up to N = 1024 (N/2 threads), 4 at N = 2048 (512 threads)
+
+__device__ __forceinline__ int dft_index_dd(int p, int logN) { return (int)(__brev((unsigned)p) >> (32 - logN)); }
+__device__ __forceinline__ dd ldp(const double* p, size_t plane, size_t o) { return dd{p[o], p[plane + o]}; }
+__device__ __forceinline__ void stp(double* p, size_t plane, size_t o, dd v) {
+    p[o] = v.hi;
+    p[plane + o] = v.lo;
+}
+
+// S9: out = y + sum_j coef_j k_j, coefficients dt a_ij (or dt b_j) as double-double pairs
+__global__ void k_rk_combine_dd(size_t L, const double* __restrict__ y, const double* __restrict__ k, CombDD cb, double* __restrict__ out) {
+    size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= L) return;
+    dd s = ldp(y, L, q);
+    for (int j = 0; j < cb.n; j++) {
+        const double* kj = k + (size_t)cb.idx[j] * 2 * L;
+        s = dd_fma(dd{cb.chi[j], cb.clo[j]}, ldp(kj, L, q), s);
+    }
+    stp(out, L, q, s);
+}
+
+// S8, base state: eta_t = F[W0], phi_t = F P[v W0 - u^2/2 - v^2/2 - g eta]   (2.1); one CTA
+__global__ void __launch_bounds__(512) k_rhs_base_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
+                                                     const double* __restrict__ filt, int filter_on, double g, size_t L,
+                                                     const double* __restrict__ eta /* planes L apart */, const double* __restrict__ W0,
+                                                     const double* __restrict__ u, const double* __restrict__ v /* planes N apart */,
+                                                     double* __restrict__ eta_t, double* __restrict__ phi_t /* planes L apart */) {
+    extern __shared__ __align__(16) unsigned char rkdd_sm[];
+    cdd* z = reinterpret_cast<cdd*>(rkdd_sm);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const dd w = ldp(W0, N, j), uu = ldp(u, N, j), vv = ldp(v, N, j), e = ldp(eta, L, j);
+        dd r = dd_sub(dd_mul(vv, w), dd_half(dd_sqr(uu)));
+        r = dd_sub(r, dd_half(dd_sqr(vv)));
+        r = dd_sub(r, dd_mul_d(e, g));
+        z[j] = cdd{w, r};
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        dd f = filter_on ? ldp(filt, N, dft_index_dd(p, logN)) : dd{1.0, 0.0};
+        f = dd_mul_d(f, rN);  // exact: a power of two
+        cdd t = z[p];
+        t.re = dd_mul(t.re, f);
+        t.im = (p == 0) ? dd{0.0, 0.0} : dd_mul(t.im, f);  // P: the mean of phi_t is removed (2.2)
+        z[p] = t;
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        stp(eta_t, L, j, z[j].re);
+        stp(phi_t, L, j, z[j].im);
+    }
+}
+
+// S8, variational columns (B.1)-(B.3): one CTA per column pair.  wout = w_c - D(u deta_c) is the linearized DtN.
+//   deta_t = F[wout] ;  dphi_t = F P[ -D(deta u v) - u D(b) + v w - g deta ],  w = wout + D(u deta),  b = dphi - v deta
+__global__ void __launch_bounds__(512) k_rhs_cols_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
+                                                     const double* __restrict__ filt, int filter_on, double g, int ncols, size_t L,
+                                                     size_t Lw, const double* __restrict__ u, const double* __restrict__ v,
+                                                     const double* __restrict__ deta, const double* __restrict__ dphi /* planes L apart */,
+                                                     const double* __restrict__ wout /* planes Lw apart */, double* __restrict__ deta_t,
+                                                     double* __restrict__ dphi_t /* planes L apart */) {
+    extern __shared__ __align__(16) unsigned char rkdd_sm[];
+    cdd* z = reinterpret_cast<cdd*>(rkdd_sm);
+    cdd* z2 = z + N;
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const size_t o0 = (size_t)c0 * N, o1 = (size_t)c1 * N;
+    const double rN = 1.0 / (double)N;
+    const dd zero{0.0, 0.0};
+    auto deriv_inplace = [&]() {  // z <- D z (natural order in and out)
+        __syncthreads();
+        fft_dif_dd(z, N, cs, sn);
+        for (int p = threadIdx.x; p < N; p += blockDim.x) {
+            const double k = (double)wavenumber_dd(p, N, logN) * rN;
+            const cdd t = z[p];
+            z[p] = cdd{dd_mul_d(t.im, -k), dd_mul_d(t.re, k)};
+        }
+        __syncthreads();
+        ifft_dit_dd(z, N, cs, sn);
+    };
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const dd uu = ldp(u, N, j);
+        z[j] = cdd{dd_mul(uu, ldp(deta, L, o0 + j)), has1 ? dd_mul(uu, ldp(deta, L, o1 + j)) : zero};
+    }
+    deriv_inplace();  // z = D(u deta)
+    cdd wv[DDF_MAX_PER_THREAD];
+#pragma unroll
+    for (int r = 0; r < DDF_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) wv[r] = cdd{dd_add(ldp(wout, Lw, o0 + j), z[j].re), has1 ? dd_add(ldp(wout, Lw, o1 + j), z[j].im) : zero};
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const dd vv = ldp(v, N, j);
+        z[j] = cdd{dd_sub(ldp(dphi, L, o0 + j), dd_mul(vv, ldp(deta, L, o0 + j))),
+                   has1 ? dd_sub(ldp(dphi, L, o1 + j), dd_mul(vv, ldp(deta, L, o1 + j))) : zero};
+    }
+    deriv_inplace();  // z = D(b)
+#pragma unroll
+    for (int r = 0; r < DDF_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) {
+            const dd uu = ldp(u, N, j), vv = ldp(v, N, j);
+            const cdd a3 = z[j];
+            const dd d0 = ldp(deta, L, o0 + j), d1 = has1 ? ldp(deta, L, o1 + j) : zero;
+            z[j] = cdd{dd_sub(dd_sub(dd_mul(vv, wv[r].re), dd_mul(uu, a3.re)), dd_mul_d(d0, g)),
+                       dd_sub(dd_sub(dd_mul(vv, wv[r].im), dd_mul(uu, a3.im)), dd_mul_d(d1, g))};
+        }
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) z2[p] = z[p];
+    __syncthreads();
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const dd uv = dd_mul(ldp(u, N, j), ldp(v, N, j));
+        z[j] = cdd{dd_mul(uv, ldp(deta, L, o0 + j)), has1 ? dd_mul(uv, ldp(deta, L, o1 + j)) : zero};
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber_dd(p, N, logN);
+        dd f = filter_on ? ldp(filt, N, dft_index_dd(p, logN)) : dd{1.0, 0.0};
+        f = dd_mul_d(f, rN);
+        const cdd q = z2[p], t = z[p];
+        // F P (q^ - i k t^)
+        z2[p] = (p == 0) ? cdd{zero, zero} : cdd{dd_mul(f, dd_add(q.re, dd_mul_d(t.im, k))), dd_mul(f, dd_sub(q.im, dd_mul_d(t.re, k)))};
+    }
+    __syncthreads();
+    ifft_dit_dd(z2, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        stp(dphi_t, L, o0 + j, z2[j].re);
+        if (has1) stp(dphi_t, L, o1 + j, z2[j].im);
+        z[j] = cdd{ldp(wout, Lw, o0 + j), has1 ? ldp(wout, Lw, o1 + j) : zero};
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        dd f = filter_on ? ldp(filt, N, dft_index_dd(p, logN)) : dd{1.0, 0.0};
+        f = dd_mul_d(f, rN);
+        z[p] = cdd{dd_mul(f, z[p].re), dd_mul(f, z[p].im)};
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        stp(deta_t, L, o0 + j, z[j].re);
+        if (has1) stp(deta_t, L, o1 + j, z[j].im);
+    }
+}
+
+// the filter (2.14) applied in place to ncols columns of the state (column c at offset c N of each plane)
+__global__ void __launch_bounds__(512) k_filter_cols_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
+                                                        const double* __restrict__ filt, int ncols, size_t L, double* __restrict__ y) {
+    extern __shared__ __align__(16) unsigned char rkdd_sm[];
+    cdd* z = reinterpret_cast<cdd*>(rkdd_sm);
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const size_t o0 = (size_t)c0 * N, o1 = (size_t)c1 * N;
+    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = cdd{ldp(y, L, o0 + j), has1 ? ldp(y, L, o1 + j) : dd{0.0, 0.0}};
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const dd f = dd_mul_d(ldp(filt, N, dft_index_dd(p, logN)), rN);
+        z[p] = cdd{dd_mul(f, z[p].re), dd_mul(f, z[p].im)};
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        stp(y, L, o0 + j, z[j].re);
+        if (has1) stp(y, L, o1 + j, z[j].im);
+    }
+}
+
+// E = (pi/N) sum_j [ phi_j (G phi)_j + g eta_j^2 ] in double-double; one CTA, out: hi, lo
+__global__ void __launch_bounds__(256) k_energy_dd(int N, double g, size_t L, const double* __restrict__ eta, const double* __restrict__ phi,
+                                                   const double* __restrict__ W0, double* __restrict__ out) {
+    __shared__ double sh[256], sl[256];
+    dd a{0.0, 0.0};
+    for (int j = threadIdx.x; j < N; j += 256) {
+        const dd e = ldp(eta, L, j);
+        a = dd_add(a, dd_add(dd_mul(ldp(phi, L, j), ldp(W0, N, j)), dd_mul_d(dd_sqr(e), g)));
+    }
+    sh[threadIdx.x] = a.hi;
+    sl[threadIdx.x] = a.lo;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            const dd s = dd_add(dd{sh[threadIdx.x], sl[threadIdx.x]}, dd{sh[threadIdx.x + o], sl[threadIdx.x + o]});
+            sh[threadIdx.x] = s.hi;
+            sl[threadIdx.x] = s.lo;
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        const dd e = dd_mul_d(dd_mul(dd{sh[0], sl[0]}, dd_pi()), 1.0 / (double)N);
+        out[0] = e.hi;
+        out[1] = e.lo;
+    }
+}
+
+static int ddf_threads(int N) { return N / 2 > 512 ? 512 : (N / 2 < 32 ? 32 : N / 2); }
+static int ddf_log2(int n) {
+    int l = 0;
+    while ((1 << l) < n) l++;
+    return l;
+}
+
+int rkdd_set_attrs() {
+    static DeviceOnce once;
+    if (once.first()) {
+        SWW_CUDA(cudaFuncSetAttribute(k_rhs_base_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 32));
+        SWW_CUDA(cudaFuncSetAttribute(k_rhs_cols_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 64));
+        SWW_CUDA(cudaFuncSetAttribute(k_filter_cols_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 32));
+    }
+    return SWW_OK;
+}
+
+int rkdd_combine(cudaStream_t st, size_t L, const double* y, const double* k, const CombDD& cb, double* out) {
+    SWW_BEGIN(KC_OTHER, st);
+    k_rk_combine_dd<<<(unsigned)((L + 255) / 256), 256, 0, st>>>(L, y, k, cb, out);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int rkdd_rhs_base(sww_dtn_s* d, bool filter, double g, size_t L, const double* ys, double* kout) {
+    const int N = d->N;
+    const Tables* t = d->tab;
+    SWW_BEGIN(KC_FFT, d->stream);
+    k_rhs_base_dd<<<1, ddf_threads(N), (size_t)N * 32, d->stream>>>(N, ddf_log2(N), t->cs, t->sn, t->filt_dd, filter ? 1 : 0, g, L, ys, d->bW0, d->bu,
+                                                                    d->bv, kout, kout + N);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int rkdd_rhs_cols(sww_dtn_s* d, bool filter, double g, int nc, size_t L, const double* ys, const double* wout, double* kout) {
+    const int N = d->N;
+    const Tables* t = d->tab;
+    const size_t od = 2 * (size_t)N, op = od + (size_t)N * nc;
+    SWW_BEGIN(KC_FFT, d->stream);
+    k_rhs_cols_dd<<<(nc + 1) / 2, ddf_threads(N), (size_t)N * 64, d->stream>>>(N, ddf_log2(N), t->cs, t->sn, t->filt_dd, filter ? 1 : 0, g, nc, L,
+                                                                               (size_t)N * nc, d->bu, d->bv, ys + od, ys + op, wout, kout + od,
+                                                                               kout + op);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int rkdd_filter_state(sww_dtn_s* d, int ncol, size_t L, double* y) {
+    const int N = d->N;
+    const Tables* t = d->tab;
+    SWW_BEGIN(KC_FFT, d->stream);
+    k_filter_cols_dd<<<(ncol + 1) / 2, ddf_threads(N), (size_t)N * 32, d->stream>>>(N, ddf_log2(N), t->cs, t->sn, t->filt_dd, ncol, L, y);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int rkdd_energy(sww_dtn_s* d, double g, size_t L, const double* y, double* out2) {
+    SWW_BEGIN(KC_OTHER, d->stream);
+    k_energy_dd<<<1, 256, 0, d->stream>>>(d->N, g, L, y, y + d->N, d->bW0, out2);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+}  // namespace sww

@@ -59,7 +59,7 @@ void timing_end() {
     g_cur_open = false;
 }
 
-__global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, double* dc, double2* tw, double* filt) {
+__global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, double* dc, double2* tw, double* filt, double* filt_dd) {
     int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= N) return;
     {
@@ -67,6 +67,9 @@ __global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, 
         const double x = (double)ak / (double)(N / 2);
         const double x2 = x * x, x4 = x2 * x2, x8 = x4 * x4, x16 = x8 * x8, x32 = x16 * x16;
         filt[m] = exp(-36.0 * (x32 * x4));                 // (2.14)
+        // the same in double-double (x is exact: a ratio of an integer and a power of two)
+        const dd y2 = dd_sqr(dd{x, 0.0}), y4 = dd_sqr(y2), y8 = dd_sqr(y4), y16 = dd_sqr(y8), y32 = dd_sqr(y16);
+        dd_store(filt_dd, N, m, dd_exp(dd_mul_d(dd_mul(y32, y4), -36.0)));
     }
     dd s, c;
     dd_sincos_2pi_frac(m, N, &s, &c);
@@ -100,8 +103,8 @@ int get_tables(int N, cudaStream_t st, const Tables** out) {
     Tables* t = new Tables();
     t->N = N;
     double* base = nullptr;
-    // 5 dd tables of 2N doubles + N double2 + N doubles
-    SWW_CUDA(cudaMalloc(&base, sizeof(double) * (size_t)N * 13));
+    // 6 dd tables of 2N doubles + N double2 + N doubles
+    SWW_CUDA(cudaMalloc(&base, sizeof(double) * (size_t)N * 15));
     t->cs = base;
     t->sn = base + 2 * (size_t)N;
     t->c0 = base + 4 * (size_t)N;
@@ -109,9 +112,10 @@ int get_tables(int N, cudaStream_t st, const Tables** out) {
     t->dc = base + 8 * (size_t)N;
     t->tw = reinterpret_cast<double2*>(base + 10 * (size_t)N);
     t->filt = base + 12 * (size_t)N;
+    t->filt_dd = base + 13 * (size_t)N;
     // the default stream orders this before any later stream work after the synchronize below
     SWW_BEGIN(KC_OTHER, st);
-    k_tables<<<(N + 127) / 128, 128, 0, st>>>(N, t->cs, t->sn, t->c0, t->s2, t->dc, t->tw, t->filt);
+    k_tables<<<(N + 127) / 128, 128, 0, st>>>(N, t->cs, t->sn, t->c0, t->s2, t->dc, t->tw, t->filt, t->filt_dd);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     SWW_CUDA(cudaStreamSynchronize(st));

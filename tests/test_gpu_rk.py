@@ -130,12 +130,86 @@ def test_small_amplitude_wave_returns_after_linear_period(sww):
     assert np.abs(r["phi"].cpu().numpy()).max() <= 50 * amp * amp
 
 
+def _dd(hi, lo=None):
+    hi = np.ascontiguousarray(hi, dtype=np.float64)
+    lo = np.zeros_like(hi) if lo is None else np.ascontiguousarray(lo, dtype=np.float64)
+    return torch.from_numpy(np.stack([hi, lo])).cuda().contiguous()
+
+
+def _dd_err(t, ref):
+    """max |gpu - oracle| / max |oracle| for a planar (2, ...) tensor against an oracle (hi, lo) pair, word by word"""
+    g = t.cpu().numpy()
+    d = (g[0].astype(LD) - ref[0].astype(LD)) + (g[1].astype(LD) - ref[1].astype(LD))
+    return np.abs(d), np.abs(ld(ref))
+
+
+@pytest.mark.parametrize("N,nc,nsteps", [(64, 4, 2), (256, 6, 1)])
+def test_double_double_stepper(sww, orc_q, N, nc, nsteps):
+    """the quadruple-precision time stepping of PAPER.md:163-165, 314: sww_state_create(prec = SWW_DD) advances (q, Qdot) with
+    every kernel in double-double; state and every variational column against the __float128 oracle, bar 1e-25 per column"""
+    c4 = si.config4(N, max(nc, 2))
+    eta = (0.25 * c4.eta, 0.25 * c4.eta_lo)           # exact scaling of a double-double pair
+    phi = (c4.phi0, c4.phi0_lo)
+    deta = (c4.deta[:nc] * 2.0 ** -4, c4.deta_lo[:nc] * 2.0 ** -4)
+    dphi = (c4.dphi[:nc] * 2.0 ** -4, c4.dphi_lo[:nc] * 2.0 ** -4)
+    h, g, dt = 1.0, 1.0, si.config2().meta["dt"]
+    st = sww.State(_dd(*eta), _dd(*phi), h, g, prec=sww.DD, deta=_dd(*deta), dphi=_dd(*dphi))
+    e0 = st.energy()
+    st.advance(dt, nsteps)
+    r = st.read()
+    e1 = st.energy()
+    o = orc_q.rk_advance(eta, phi, h, g, dt, nsteps, deta=deta, dphi=dphi, want_energy=True)
+    for name in ("eta", "phi"):
+        d, ref = _dd_err(r[name], o[name])
+        assert float(d.max() / ref.max()) <= 1e-25, (name, float(d.max() / ref.max()))
+    worst = 0.0
+    for name in ("deta", "dphi"):
+        d, ref = _dd_err(r[name], o[name])
+        e = (d.max(axis=1) / ref.max(axis=1)).astype(np.float64)
+        worst = max(worst, float(e.max()))
+        assert float(e.max()) <= 1e-25, (name, e)
+    # energy against the oracle's, and conserved to ~29 digits over the step(s) (PAPER.md:503)
+    eo = o["energies"]
+    for mine, k in ((e0, 0), (e1, nsteps)):
+        ref = LD(eo[0][k]) + LD(eo[1][k])
+        assert abs((LD(mine[0]) - LD(eo[0][k])) + (LD(mine[1]) - LD(eo[1][k]))) <= 1e-27 * abs(ref)
+    print(f"dd stepper N={N}: worst column E_col {worst:.2e}")
+
+
+def test_double_double_energy_conservation(sww):
+    """E(t) constant "to 29 digits in quadruple precision": a smooth standing wave, 4 steps of dt = 1e-3 (the
+    order-8 truncation error is far below the double-double rounding level there)"""
+    N, h, g = 32, 1.0, 1.0
+    a = si.grid(N)
+    eta0 = 0.05 * np.cos(a) + 0.01 * np.cos(2 * a)
+    st = sww.State(_dd(eta0), _dd(np.zeros(N)), h, g, prec=sww.DD)
+    e0 = st.energy()
+    st.advance(1e-3, 4)
+    e1 = st.energy()
+    drift = abs((LD(e1[0]) - LD(e0[0])) + (LD(e1[1]) - LD(e0[1]))) / abs(LD(e0[0]))
+    assert float(drift) <= 1e-28, float(drift)
+    print(f"dd energy drift over 4 steps: {float(drift):.2e}")
+
+
+def test_double_double_stepper_tracks_fp64(sww):
+    """the same initial state through the fp64 and the double-double stepper: they agree to fp64 accuracy"""
+    eta, phi, deta, dphi, h, g, dt = small_case(64, 4)
+    a = sww.State(dev(eta), dev(phi), h, g, deta=dev(deta), dphi=dev(dphi))
+    b = sww.State(_dd(eta), _dd(phi), h, g, prec=sww.DD, deta=_dd(deta), dphi=_dd(dphi))
+    a.advance(dt, 2)
+    b.advance(dt, 2)
+    ra, rb = a.read(), b.read()
+    for name in ("eta", "phi", "deta", "dphi"):
+        x, y = ra[name].cpu().numpy(), rb[name].cpu().numpy()[0]
+        assert np.abs(x - y).max() <= 1e-11 * np.abs(y).max(), name
+
+
 def test_state_errors(sww):
     N = 64
     z = torch.zeros(N, dtype=torch.float64, device="cuda")
-    with pytest.raises(sww.SwwError) as e:
-        sww.State(torch.zeros((2, N), dtype=torch.float64, device="cuda"), torch.zeros((2, N), dtype=torch.float64, device="cuda"), 1.0, prec=sww.DD)
-    assert e.value.status == -1  # the double-double stepper is not built
+    with pytest.raises(sww.SwwError) as e:   # the double-double stepper stops at N = 2048 (include/sww.h)
+        sww.State(torch.zeros((2, 4096), dtype=torch.float64, device="cuda"), torch.zeros((2, 4096), dtype=torch.float64, device="cuda"), 1.0, prec=sww.DD)
+    assert e.value.status == -1
     st = sww.State(z - 2.0, z, 1.0)  # surface below the bottom
     with pytest.raises(sww.SwwError) as e:
         st.read()
