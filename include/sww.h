@@ -20,7 +20,12 @@
  *     Data-dependent failures (SWW_EBOTTOM, SWW_ESINGULAR) are recorded in a device flag and returned by the next
  *     synchronising call (sww_dtn_status, sww_state_read).
  *   - The caller owns every in/out buffer; handles own everything else.  Functions never throw or exit; they return a status.
- *   - N must be a power of two, 16 <= N <= 8192.
+ *   - N must be a power of two.  Size limits per entry point (checked up front, before anything is allocated; SWW_EINVAL):
+ *         sww_dtn_* with SWW_F64 ............ 16 <= N <= 8192
+ *         sww_dtn_* with SWW_DD ............. 16 <= N <= 4096   (one N-point complex double-double array per CTA in shared memory)
+ *         sww_state_* with SWW_F64 .......... 16 <= N <= 4096   (two N-point complex arrays per CTA)
+ *         sww_state_* with SWW_DD ........... 16 <= N <= 2048   (two N-point complex double-double arrays per CTA)
+ *     Mesh refinement (2.10)-(2.11) and sizes that are not powers of two are not built.
  */
 #ifndef SWW_H
 #define SWW_H
@@ -60,10 +65,10 @@ int sww_dtn_refactor(sww_dtn_t d, const void* eta);
 /* out_c = G(eta) phi_c, c < nrhs: solve (I/2 + K) mu_c = phi_c (2.7); gamma_c = D mu_c; out_c = H gamma_c / 2 + G gamma_c (2.8)
  * (1/|xi'| = 1 on the uniform grid, R3).  phi, out: DEVICE, N x nrhs; may alias.  Pure: no hidden state.
  * A non-finite input column gives a non-finite output column, spoils the column it shares a complex FFT with (2c and 2c + 1)
- * and leaves all others untouched.  One bit pattern is reserved:
- * the triangular solves mark "not computed yet" by the all-ones NaN (0xFFFFFFFFFFFFFFFF), which no arithmetic produces; a
- * right-hand side that propagates exactly that payload makes the solve give up after a bounded wait with the sticky status
- * SWW_ECUDA instead of hanging. */
+ * and leaves all others untouched.  (The triangular solves mark "not computed yet" in their scratch by the all-ones NaN
+ * 0xFFFFFFFFFFFFFFFF; an input with exactly that payload is replaced by the canonical quiet NaN on the way in, so it behaves
+ * like any other NaN.  Should a task ever wait for data beyond ~0.1 s, it records the sticky status SWW_ECUDA and every other
+ * task stops polling at once.) */
 int sww_dtn_apply(sww_dtn_t d, const void* phi, int nrhs, void* out);
 
 /* Store the state the linearization is taken about: phi0' = D phi0, W0 = G phi0, and the surface velocities of (2.9)
@@ -75,7 +80,9 @@ int sww_dtn_set_base(sww_dtn_t d, const void* phi0);
 int sww_dtn_linearized_apply(sww_dtn_t d, const void* deta, const void* dphi, int nrhs, void* out);
 
 /* Read-only views for tests and diagnostics.  which: 0 = K, 1 = G (column-major N x N: entry (i,j) at i + j*N, i = target
- * alpha_i, j = source alpha_j; DD: planar hi then lo), 2 = eta' , 3 = eta'', 4 = phi0', 5 = W0, 6 = u, 7 = v (N reals each).
+ * alpha_i, j = source alpha_j; DD: planar hi then lo), 2 = eta' , 3 = eta'', 4 = phi0', 5 = W0, 6 = u, 7 = v (N reals each),
+ * 8 = the fp64 factors of I/2 + K as lu.cu stores them (N x N doubles for either precision: L_ij = X_ij inv(S_j) below the block
+ * diagonal, U_ij above it, the raw diagonal tiles of K on it).
  * dst: DEVICE buffer of the right size; the copy is enqueued on the handle's stream. */
 int sww_dtn_get(sww_dtn_t d, int which, void* dst);
 
@@ -83,7 +90,10 @@ int sww_dtn_status(sww_dtn_t d);   /* synchronises the stream; returns the stick
 int sww_dtn_destroy(sww_dtn_t d);
 
 /* ---- time stepper (2.1) + variational equation (3.32), PAPER.md:70-72, 294-305, 689-714 ------------------------
- * sww_state_create copies the initial state (DEVICE pointers; deta/dphi may be NULL when ncols = 0).
+ * sww_state_create copies the initial state (DEVICE pointers; deta/dphi may be NULL when ncols = 0).  prec = SWW_DD: every
+ * array is double-double planar (eta, phi: 2N doubles; deta, dphi: 2 N ncols doubles, hi block then lo block), and the whole
+ * step -- DtN, right-hand sides, FFTs, filter, stage combination with the tableau in double-double -- runs in double-double
+ * (the paper's quadruple-precision time stepping).
  * flags bit 0: switch the 36th-order filter (2.14) off (R5).
  * sww_rk_advance: nsteps steps of size dt of the 11-stage order-8 explicit Runge-Kutta scheme (R6), one setup S0-S2 and
  * one batched linearized solve per stage, state filtered after each step; advances (q, Qdot) together, in place.
@@ -94,7 +104,8 @@ int sww_state_create(int N, double h, double g, int prec, int ncols, const void*
 int sww_rk_advance(sww_state_t s, double dt, int nsteps);
 int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, double* t);
 /* E = (1/2) int (phi G phi + g eta^2) dx = (pi/N) sum_j [phi_j (G phi)_j + g eta_j^2] of the current state;
- * energy_hl: HOST, 2 doubles (hi, lo; lo = 0 for SWW_F64); synchronises. */
+ * energy_hl: HOST, 2 doubles (hi, lo; lo = 0 for SWW_F64); synchronises.  The handle's internal DtN is re-set-up for the current
+ * state (one setup + base state). */
 int sww_state_energy(sww_state_t s, double* energy_hl);
 int sww_state_destroy(sww_state_t s);
 

@@ -84,6 +84,7 @@ extern "C" {
 
 int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_dtn_t* out) {
     if (!eta || !out || !valid_N(N) || (prec != SWW_F64 && prec != SWW_DD) || !(h > 0.0)) return SWW_EINVAL;
+    if (prec == SWW_DD && N > 4096) return SWW_EINVAL;  // the double-double spectral passes (ddpath.cu); include/sww.h states the limits
     sww_dtn_s* d = new (std::nothrow) sww_dtn_s();
     if (!d) return SWW_ENOMEM;
     memset(d, 0, sizeof(*d));
@@ -248,7 +249,8 @@ int sww_host_cache_clear(void) {
 
 int sww_dtn_linearized_host(const void* eta, const void* phi0, const void* deta, const void* dphi, void* out, int N, double h,
                             int prec, int nrhs) {
-    if (!eta || !phi0 || !deta || !dphi || !out || nrhs < 1 || !valid_N(N) || (prec != SWW_F64 && prec != SWW_DD) || !(h > 0.0))
+    if (!eta || !phi0 || !deta || !dphi || !out || nrhs < 1 || !valid_N(N) || (prec != SWW_F64 && prec != SWW_DD) || !(h > 0.0) ||
+        (prec == SWW_DD && N > 4096))
         return SWW_EINVAL;
     const size_t mul = prec == SWW_DD ? 2 : 1, vec = sizeof(double) * N * mul, bat = vec * nrhs;
     cudaStream_t st = nullptr;

@@ -438,6 +438,50 @@ __global__ void __launch_bounds__(512) k_spectral_gamma_w_dd(int N, int logN, co
     }
 }
 
+// One multiplier per launch, one complex dd array in shared memory (N = 4096: 128 KB; the fused kernel above needs two):
+// out_c (+)= sign * m(D) in_c for the column pair (2 b, 2 b + 1);  mode 0: m = i k (D), mode 1: m = |k| / 2.
+__global__ void __launch_bounds__(512) k_spectral_pass_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
+                                                          int mode, double sign, int accumulate, size_t Lin, size_t Lout,
+                                                          const double* __restrict__ in, double* __restrict__ out, int ncols, int out_cols,
+                                                          int zero_partner) {
+    extern __shared__ __align__(16) unsigned char dd_fft_sm[];
+    cdd* z = reinterpret_cast<cdd*>(dd_fft_sm);
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const double rN = 1.0 / (double)N;
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const size_t o0 = (size_t)c0 * N + j, o1 = (size_t)c1 * N + j;
+        z[j] = cdd{dd{in[o0], in[Lin + o0]}, has1 ? dd{in[o1], in[Lin + o1]} : dd{0, 0}};
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber_dd(p, N, logN) * rN;  // exact: an integer times a power of two (1/N of the inverse folded in)
+        const double a = sign * k, h = sign * 0.5 * fabs(k);
+        const cdd v = z[p];
+        z[p] = (mode == 0) ? cdd{dd_mul_d(v.im, -a), dd_mul_d(v.re, a)} : cdd{dd_mul_d(v.re, h), dd_mul_d(v.im, h)};
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const cdd v = z[j];
+        const size_t o0 = (size_t)c0 * N + j, o1 = (size_t)c1 * N + j;
+        if (c0 < out_cols) {
+            const dd r = accumulate ? dd_add(dd{out[o0], out[Lout + o0]}, v.re) : v.re;
+            out[o0] = r.hi;
+            out[Lout + o0] = r.lo;
+        }
+        if (c1 < out_cols) {
+            const dd r = accumulate ? dd_add(dd{out[o1], out[Lout + o1]}, v.im) : v.im;
+            out[o1] = r.hi;
+            out[Lout + o1] = r.lo;
+        } else if (zero_partner && !has1) {  // padded buffer: the odd partner column is zeroed
+            out[o1] = 0.0;
+            out[Lout + o1] = 0.0;
+        }
+    }
+}
+
 static int ilog2(int n) {
     int l = 0;
     while ((1 << l) < n) l++;
@@ -565,7 +609,7 @@ int fast_base_f64(sww_dtn_s* d, const double* phi0) {
 // already filled).  Tcols: dd planar in ws layout or nullptr.  out: dd planar N x nrhs, plane size Lout (0 = N * nrhs).
 int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcols, int nrhs, double* out, size_t Lin, size_t Lout) {
     const int N = d->N;
-    if (N > 2048) return SWW_EINVAL;  // the dd FFT keeps two N-point complex dd arrays in shared memory (2 x 32 B x N <= 128 KB)
+    if (N > 4096) return SWW_EINVAL;  // one N-point complex dd array in shared memory: 32 B x N <= 128 KB (include/sww.h states it)
     cudaStream_t st = d->stream;
     Workspace& w = d->ws;
     const size_t NN = (size_t)N * N, Lws = (size_t)N * w.cap_cols, n = (size_t)N * nrhs, Lio = Lout ? Lout : n;
@@ -589,13 +633,30 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
     static DeviceOnce attr_once;
     if (attr_once.first()) {
         SWW_CUDA(cudaFuncSetAttribute(k_spectral_gamma_w_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, 2048 * 32 * 2));
+        SWW_CUDA(cudaFuncSetAttribute(k_spectral_pass_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, 4096 * 32));
     }
-    size_t smem = (size_t)N * sizeof(cdd) * 2;
     int threads = N / 2 > 512 ? 512 : (N / 2 < 32 ? 32 : N / 2);
     // Gam = D mu (ws layout) ; out = |D| mu / 2 - D T  (user layout)
-    SWW_BEGIN(KC_FFT, st);
-    k_spectral_gamma_w_dd<<<(nrhs + 1) / 2, threads, smem, st>>>(N, ilog2(N), d->tab->cs, d->tab->sn, Lws, Lio, mu, Tcols, w.Gam, out, nrhs, nrhs);
-    SWW_LAUNCHED();
+    if (N <= 2048) {
+        size_t smem = (size_t)N * sizeof(cdd) * 2;
+        SWW_BEGIN(KC_FFT, st);
+        k_spectral_gamma_w_dd<<<(nrhs + 1) / 2, threads, smem, st>>>(N, ilog2(N), d->tab->cs, d->tab->sn, Lws, Lio, mu, Tcols, w.Gam, out, nrhs, nrhs);
+        SWW_LAUNCHED();
+    } else {  // N = 4096: the two transforms of a column pair do not fit side by side; one multiplier per launch
+        const size_t smem = (size_t)N * sizeof(cdd);
+        const int nb = (nrhs + 1) / 2, lg = ilog2(N);
+        SWW_BEGIN(KC_FFT, st);
+        k_spectral_pass_dd<<<nb, threads, smem, st>>>(N, lg, d->tab->cs, d->tab->sn, 0, 1.0, 0, Lws, Lws, mu, w.Gam, nrhs, nrhs, 1);
+        SWW_LAUNCHED();
+        SWW_BEGIN(KC_FFT, st);
+        k_spectral_pass_dd<<<nb, threads, smem, st>>>(N, lg, d->tab->cs, d->tab->sn, 1, 1.0, 0, Lws, Lio, mu, out, nrhs, nrhs, 0);
+        SWW_LAUNCHED();
+        if (Tcols) {
+            SWW_BEGIN(KC_FFT, st);
+            k_spectral_pass_dd<<<nb, threads, smem, st>>>(N, lg, d->tab->cs, d->tab->sn, 0, -1.0, 1, Lws, Lio, Tcols, out, nrhs, nrhs, 0);
+            SWW_LAUNCHED();
+        }
+    }
     SWW_CUDA(cudaGetLastError());
     // out += G Gam : Y = 1*Z + 0*X + 1*(A X) with Z = out (plane Lio) -- the kernel takes one plane size, so go through w.B:
     SWW_BEGIN(KC_OTHER, st);

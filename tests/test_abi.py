@@ -61,6 +61,7 @@ def test_argument_validation_needs_no_device(sww):
     assert L.sww_dtn_setup(p, 16384, 1.0, 0, None, ctypes.byref(h)) == -1          # N too large
     assert L.sww_dtn_setup(p, 64, 1.0, 7, None, ctypes.byref(h)) == -1             # unknown precision
     assert L.sww_dtn_setup(p, 64, -1.0, 0, None, ctypes.byref(h)) == -1            # negative depth
+    assert L.sww_dtn_setup(p, 8192, 1.0, 1, None, ctypes.byref(h)) == -1           # double-double stops at N = 4096 (include/sww.h)
     assert L.sww_dtn_apply(None, p, 1, p) == -1
     assert L.sww_dtn_linearized_apply(None, p, p, 1, p) == -1
     assert L.sww_rk_advance(None, 0.1, 1) == -1

@@ -10,7 +10,7 @@ import pytest
 import torch
 
 import sww_inputs as si
-from parity_util import (BAR, check_columns, diff, from_dev, gpu_linearized, ld, lin_scales, oracle_linearized,
+from parity_util import (BAR, LD, check_columns, diff, from_dev, gpu_linearized, ld, lin_scales, oracle_linearized,
                          sample_columns, to_dev)
 
 pytestmark = pytest.mark.gpu
@@ -255,6 +255,37 @@ def test_gemm_128x128_tiles(sww):
     d.check()
     scale = wide.abs().max(dim=1).values
     assert float(((wide - halves).abs().max(dim=1).values / scale).max()) <= 1e-12
+
+
+def test_dd_maximum_size_flat_symbol_and_small_sizes(sww, orc_q):
+    """the ends of the double-double size range (include/sww.h: 16 <= N <= 4096).  N = 4096 runs the one-multiplier spectral
+    passes: flat surface, G cos(kx) = k tanh(kh) cos(kx) ((4.34)) with the symbol from mpmath and the columns
+    synthesised in double-double; N = 16 and 32 (the small-size dd products) against the __float128 oracle"""
+    import mpmath
+    N, h = 4096, 1.0
+    ks = [1, 2, 37, 1000, 2047]
+    coef = np.zeros((len(ks), max(ks) + 1))
+    for r, k in enumerate(ks):
+        coef[r, k] = 1.0
+    phi_hi, phi_lo = si.synth_dd(N, coef)
+    d = sww.DtN(torch.zeros((2, N), dtype=torch.float64, device="cuda"), h, sww.DD)
+    out = d.apply(to_dev(phi_hi, phi_lo, "dd")).cpu().numpy()
+    d.check()
+    del d
+    for r, k in enumerate(ks):
+        with mpmath.workdps(50):   # 97 sampled entries of the column, everything in 50-digit arithmetic
+            sym = mpmath.mpf(k) * mpmath.tanh(mpmath.mpf(k) * h)
+            worst = max(abs((mpmath.mpf(float(out[0][r][j])) + mpmath.mpf(float(out[1][r][j])))
+                            - sym * (mpmath.mpf(float(phi_hi[r][j])) + mpmath.mpf(float(phi_lo[r][j])))) for j in range(0, N, 43))
+            assert worst <= mpmath.mpf(1e-25) * sym, (k, float(worst / sym))
+    for Ns in (16, 32):
+        c = si.config4(Ns, 4)
+        eta = (0.1 * c.eta, np.zeros(Ns))   # a gentle surface that N = 16 resolves
+        dd_ = sww.DtN(to_dev(*eta, "dd"), c.h, sww.DD)
+        res = from_dev(dd_.apply(to_dev(c.dphi * 2.0 ** -3, c.dphi_lo * 2.0 ** -3, "dd")), "dd")
+        dd_.check()
+        orc = orc_q.dtn_apply(eta, c.h, (c.dphi * 2.0 ** -3, c.dphi_lo * 2.0 ** -3))
+        check_columns(res, orc, "dd", Ns, np.abs(c.dphi * 2.0 ** -3).max(axis=1), f"dd N={Ns}")
 
 
 def test_cfg5_shallow_sampled_columns(sww, orc_ld):
