@@ -117,9 +117,11 @@ unsigned long long sww_launch_count(void);
 /* Per-kernel-class device timing for bench.py's roofline block.  sww_timing_enable(1): from now on every kernel launch of
  * this library is bracketed by a CUDA event pair on its stream (diagnostic mode: costs two event records per launch; not
  * thread-safe).  sww_timing_read synchronises those events, adds up elapsed milliseconds and launch counts per class since
- * the previous read and clears the list.  ms, launches: HOST arrays of nclass >= 7 entries; classes: 0 = K/G assembly (S1),
+ * the previous read and clears the list.  ms, launches: HOST arrays of nclass >= 8 entries; classes: 0 = K/G assembly (S1),
  * 1 = LU factorisation (persistent DMMA dataflow kernel, S2), 2 = FP64 DMMA GEMM (G product, S6),
- * 3 = FFT / spectral (S5, S7), 4 = double-double matrix products (EFT kernels), 5 = everything else (streaming), 6 = multi-right-hand-side triangular solves (persistent DMMA dataflow kernel, S4). */
+ * 3 = FFT / spectral (S5, S7), 4 = double-double matrix products (EFT kernels), 5 = everything else (streaming),
+ * 6 = multi-right-hand-side triangular solves (persistent DMMA dataflow kernel, 16- and 32-column slabs, S4),
+ * 7 = the same kernel's 8-column instantiation (batches of <= 64 columns: the single-vector solves of the base state). */
 int sww_timing_enable(int on);
 int sww_timing_read(double* ms, unsigned long long* launches, int nclass);
 /* Microbenchmarks used to measure the roofline denominators on the box: returns achieved FLOP/s of a

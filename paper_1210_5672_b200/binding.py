@@ -99,7 +99,7 @@ def launch_count() -> int:
     return int(lib().sww_launch_count())
 
 
-KERNEL_CLASSES = ("assembly", "lu", "gemm_dmma", "fft", "dd_gemm", "other", "trsm")
+KERNEL_CLASSES = ("assembly", "lu", "gemm_dmma", "fft", "dd_gemm", "other", "trsm", "trsv")
 
 
 def timing_enable(on: bool):

@@ -24,7 +24,7 @@ int note_cuda(cudaError_t e, const char* where);
     } while (0)
 // Per-kernel-class device timing (sww_timing_enable / sww_timing_read): when enabled, SWW_BEGIN / SWW_LAUNCHED bracket every
 // launch with a CUDA event pair on the launching stream; off by default (no events, no overhead beyond a branch).
-enum KClass { KC_ASM = 0, KC_LU = 1, KC_GEMM = 2, KC_FFT = 3, KC_DDGEMM = 4, KC_OTHER = 5, KC_TRSM = 6, KC_COUNT = 7 };
+enum KClass { KC_ASM = 0, KC_LU = 1, KC_GEMM = 2, KC_FFT = 3, KC_DDGEMM = 4, KC_OTHER = 5, KC_TRSM = 6, KC_TRSV = 7, KC_COUNT = 8 };
 extern bool g_timing;
 void timing_begin(int cls, cudaStream_t st);
 void timing_end();

@@ -937,7 +937,7 @@ static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     SWW_CUDA(cudaMemsetAsync(d->tr_scr, 0xFF, sizeof(double) * 3 * span, d->stream));  // every entry "absent"
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), d->stream));
     const int grid = std::min(sm_count(), 2 * nt * ns);
-    SWW_BEGIN(KC_TRSM, d->stream);
+    SWW_BEGIN(WS == 8 ? KC_TRSV : KC_TRSM, d->stream);  // the 8-column instantiation serves the single-vector solves: chain-latency-bound
     k_trsm_dataflow<WS><<<grid, 256, C::SMEM, d->stream>>>(a);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
