@@ -201,7 +201,7 @@ __device__ __forceinline__ void bgj_panel(double (&acc)[8][2], int w, int fr, in
 }
 
 // T (shared, row-major, leading dimension 65) holds kappa = S - I/2.  On return F = inv(S) - 2 I is in Fg (global, column-major,
-// ld 64) and in sF (shared, column-major, ld 68: the DMMA operand layout of lu.cu).  Every one of the 352 threads must call it;
+// ld 64; skipped when Fg == nullptr) and in sF (shared, column-major, ld 68: the DMMA operand layout of lu.cu).  Every one of the 352 threads must call it;
 // scr: BGJ_SCRATCH doubles of shared memory.  The two idle warps return as soon as every active warp has read T (from then on
 // the caller may overwrite it); the active warps end with a barrier among themselves: the caller must follow with a CTA-wide
 // barrier before anybody reads sF.
@@ -267,7 +267,7 @@ __device__ __forceinline__ void bgj64(const double* T, double* scr, int* status,
 #pragma unroll
         for (int e = 0; e < 2; e++) {
             const int row = 8 * w + fr, col = 8 * t + 2 * fk + e;
-            Fg[col * 64 + row] = acc[t][e];
+            if (Fg) Fg[col * 64 + row] = acc[t][e];
             sF[col * 68 + row] = acc[t][e];
         }
     bgj_bar_sync(BGJ_BAR_FULL, BGJ_THREADS);  // the closing barrier

@@ -181,10 +181,10 @@ __global__ void __launch_bounds__(256) k_lu_single(double* __restrict__ A, int n
 // where  X_ij = A_ij - sum_{k < min(i,j)} L_ik U_kj.  (Well posed: every S_m is I/2 plus a small block.)
 //
 // The recurrence of the diagonal,  S_m = P_m - X_{m,m-1} Z_{m-1} U_{m-1,m}  with  P_m = A_mm - sum_{k<m-1} L_mk U_km,  is the
-// critical path.  It runs on ONE dedicated CTA (the "spine", block 0): blocked Gauss-Jordan inverse of S_{m-1} on the tensor
-// pipe (bgj.cuh), then V = Z_{m-1} U_{m-1,m} and S_m = P_m - X_{m,m-1} V (two 64^3 DMMA products), all in shared memory; its
-// three inputs are fetched while the previous inverse runs.  Everything else is done by worker CTAs claiming tile tasks from a
-// counter.  A tile of level l = min(i,j) sums its terms k < l-1 from finished tiles; its LAST term needs Z_{l-1}, which has only
+// critical path.  It runs on a dedicated cluster of two CTAs (the "spine", blocks 0 and 1): blocked Gauss-Jordan inverse of
+// S_{m-1} on the tensor pipe (bgj.cuh; both CTAs, redundantly), then V = Z_{m-1} U_{m-1,m} and S_m = P_m - X_{m,m-1} V with the
+// columns split between the two CTAs and the halves exchanged through distributed shared memory; the three inputs are fetched
+// while the previous inverse runs.  Everything else is done by worker CTAs claiming tile tasks from a counter.  A tile of level l = min(i,j) sums its terms k < l-1 from finished tiles; its LAST term needs Z_{l-1}, which has only
 // just been published -- waiting for a neighbour task to turn X_{i,l-1} into L_{i,l-1} first would put two tasks and two trips
 // through L2 between consecutive inverses.  So every task forms the L it needs for its last term itself, L = X Z_{l-1} (a
 // chained pair of products right behind the flag of Z_{l-1}), from an X that is available long before:
@@ -222,7 +222,10 @@ struct LuArgs {
     int* status;
 };
 
-constexpr int LU_SMEM_BYTES = (5 * TS * LDO + BGJ_SCRATCH) * (int)sizeof(double) + 256;
+// spine: sX, sF (64 columns), sU, sV, sP (32 columns), two work tiles, bgj64 scratch; workers: four operand tiles + ready[]
+constexpr int LU_SMEM_SPINE = (2 * TS * LDO + 3 * 32 * LDO + 2 * TS * LDT + BGJ_SCRATCH) * (int)sizeof(double);
+constexpr int LU_SMEM_WORKER = 4 * TS * LDO * (int)sizeof(double) + 256;
+constexpr int LU_SMEM_BYTES = LU_SMEM_SPINE > LU_SMEM_WORKER ? LU_SMEM_SPINE : LU_SMEM_WORKER;
 
 // fragment coordinates of this lane (threads 0..255): rows wr*32 + x*8 + fr (x < 4), columns wc*16 + y*8 + 2 fk + e (y, e < 2)
 struct Frag {
@@ -292,93 +295,155 @@ __device__ __forceinline__ void lu_stamp(int m, int k) {
 #define SWW_WSTAMP(k)
 #endif
 
-// ---- the spine: block 0
+// ---- thread-block cluster helpers (the spine is a cluster of two CTAs)
+__device__ __forceinline__ unsigned cluster_rank() {
+    unsigned r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {  // every thread of both CTAs
+    asm volatile("barrier.cluster.arrive.release.aligned;\nbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// the address of my shared-memory location p in the shared memory of CTA `rank` of the cluster
+__device__ __forceinline__ unsigned cluster_map(const void* p, unsigned rank) {
+    unsigned a = (unsigned)__cvta_generic_to_shared(p), r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    return r;
+}
+__device__ __forceinline__ void st_cluster_f64(unsigned addr, double v) {
+    asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
+
+// fragment coordinates for a 64 x 32 half tile (threads 0..255): rows wr*16 + x*8 + fr (x < 2), columns wc*16 + y*8 + 2 fk + e
+struct FragH {
+    int wr, wc, fr, fk;
+    __device__ __forceinline__ FragH(int tid) : wr((tid >> 5) & 3), wc((tid >> 7) & 1), fr((tid & 31) >> 2), fk(tid & 3) {}
+    __device__ __forceinline__ int row(int x) const { return wr * 16 + x * 8 + fr; }
+    __device__ __forceinline__ int col(int y, int e) const { return wc * 16 + y * 8 + 2 * fk + e; }
+};
+#define SWW_FRAGH_LOOP for (int x = 0; x < 2; x++) for (int y = 0; y < 2; y++) for (int e = 0; e < 2; e++)
+// acc (64 x 32) += As (64 x 64) x Bs (64 x 32); As[k][r] (ld LDO), Bs[n][k] (ld LDO, 32 columns)
+__device__ __forceinline__ void mma_half(double (&acc)[2][2][2], const double* a, const double* b, const FragH& f) {
+    const double* as = a + f.wr * 16 + f.fr;
+    const double* bs = b + (f.wc * 16 + f.fr) * LDO;
+#pragma unroll
+    for (int k4 = 0; k4 < TS; k4 += 4) {
+        double af[2], bf[2];
+#pragma unroll
+        for (int x = 0; x < 2; x++) af[x] = as[(k4 + f.fk) * LDO + x * 8];
+#pragma unroll
+        for (int y = 0; y < 2; y++) bf[y] = bs[y * 8 * LDO + k4 + f.fk];
+#pragma unroll
+        for (int x = 0; x < 2; x++)
+#pragma unroll
+            for (int y = 0; y < 2; y++) lu_dmma884(acc[x][y][0], acc[x][y][1], af[x], bf[y]);
+    }
+}
+// 32 columns of a 64-row column-major tile -> shared, ld LDO; thread t of nthr, cp.async (not committed)
+__device__ __forceinline__ void half_async(double* dst, const double* src, size_t ld, int t, int nthr) {
+    for (int c = t; c < TS * 32 / 2; c += nthr) {
+        const int col = c >> 5, ch = (c & 31) * 2;
+        cp16(dst + col * LDO + ch, src + (size_t)col * ld + ch);
+    }
+}
+
+// ---- the spine: the cluster of blocks 0 and 1.  Both CTAs invert S_{m-1} (the same instructions on the same data: the same
+// bits), then each forms one half of the columns of V = Z_{m-1} U_{m-1,m} and of S_m = P_m - X_{m,m-1} V (two 64 x 64 x 32 products
+// instead of two 64^3), and writes its half of kappa_m = S_m - I/2 into both CTAs' work tiles through distributed shared
+// memory; one cluster barrier per step.  CTA 0 publishes F_m.
 __device__ void lu_spine(const LuArgs& p, double* sm) {
-    double* sX = sm;                  // X_{m,m-1}                 (A operand: As[k][r])
-    double* sU = sX + TS * LDO;       // U_{m-1,m}                 (B operand: Bs[n][k])
-    double* sF = sU + TS * LDO;       // F_{m-1}, written by bgj64 (A operand)
-    double* sV = sF + TS * LDO;       // V = Z_{m-1} U_{m-1,m}     (B operand)
-    double* sT = sV + TS * LDO;       // P_m (column-major, ld LDO), then kappa_m = S_m - I/2 (row-major, ld LDT) for bgj64
-    double* scr = sT + TS * LDO;
+    double* sX = sm;                  // X_{m,m-1}                               (A operand: As[k][r])
+    double* sF = sX + TS * LDO;       // F_{m-1}, written by bgj64               (A operand)
+    double* sU = sF + TS * LDO;       // my 32 columns of U_{m-1,m}              (B operand: Bs[n][k])
+    double* sV = sU + 32 * LDO;       // my 32 columns of V = Z_{m-1} U_{m-1,m}  (B operand)
+    double* sP = sV + 32 * LDO;       // my 32 columns of P_m (column-major, ld LDO)
+    double* sK = sP + 32 * LDO;       // 2 work tiles kappa_m = S_m - I/2 (row-major, ld LDT) for bgj64, alternating by step
+    double* scr = sK + 2 * TS * LDT;
     const int tid = threadIdx.x;
-    const Frag f(tid);
+    const FragH f(tid);
     const bool mm = tid < 256;        // the 8 MMA warps of the two products
     const int N = p.N, nt = p.nt;
     const unsigned epoch = p.epoch;
+    const unsigned rank = cluster_rank(), peer = rank ^ 1u;
+    const int cb = 32 * (int)rank;    // my columns of the step: cb .. cb + 31
     const int role = bgj_role(tid >> 5);
-    const int at = role * 32 + (tid & 31);  // index among the BGJ_THREADS threads that are inside bgj64 (role >= 0)
-    __shared__ int s_ready;
     // the three input flags of step m: Xs[m], tile (m-1, m), P_m (P_1 is the raw diagonal tile)
     auto input_flag = [&](int m, int q) -> const unsigned* {
         if (q == 0) return p.xflags + m;
         if (q == 1) return p.flags + (size_t)(m - 1) * nt + m;
         return (m >= 2) ? p.flags + (size_t)m * nt + m : nullptr;
     };
-    auto issue_inputs = [&](int m, int t, int nthr) {
-        tile_async(sX, p.Xs + (size_t)m * TS * TS, TS, t, nthr);
-        tile_async(sU, p.A + (size_t)m * TS * N + (size_t)(m - 1) * TS, N, t, nthr);   // tile (m-1, m)
-        tile_async(sT, p.A + (size_t)m * TS * N + (size_t)m * TS, N, t, nthr);         // tile (m, m)
-        cp_commit();
-    };
     // The two warps that have no role in the inversion (bgj_role < 0) fetch the inputs of the next step meanwhile: they wait for
-    // the three flags (acquire) and issue the tile copies, which land in sX, sU, sT while the other warps invert -- none of the
-    // three regions is touched by bgj64 once the idle warps are back from it (sT has been read by then).
+    // the three flags (acquire) and issue the tile copies, which land in sX, sU, sP while the other warps invert.
     const int it = (tid >> 5) == 4 ? (tid & 31) : 32 + (tid & 31);  // index among the 64 idle threads (warps 4 and 8)
-    auto fetch_inputs = [&](int m) {
-        if (it < 3) {
-            const unsigned* fl = input_flag(m, it);
-            if (fl) spin_tight(fl, epoch);
+    auto fetch_inputs = [&](int m) {  // warp 4: P_m, then X_{m,m-1}, together with warp 8, which first fetches U_{m-1,m}
+        const int lane = tid & 31;
+        if ((tid >> 5) == 8) {
+            if (lane == 0) spin_tight(input_flag(m, 1), epoch);
+            __syncwarp();
+            half_async(sU, p.A + ((size_t)m * TS + cb) * N + (size_t)(m - 1) * TS, N, lane, 32);   // tile (m-1, m), my columns
+        } else {
+            if (lane == 0 && input_flag(m, 2)) spin_tight(input_flag(m, 2), epoch);
+            __syncwarp();
+            half_async(sP, p.A + ((size_t)m * TS + cb) * N + (size_t)m * TS, N, lane, 32);         // tile (m, m), my columns
         }
+        if (it == 0) spin_tight(input_flag(m, 0), epoch);
         asm volatile("bar.sync 4, 64;" ::: "memory");  // the two idle warps
-        issue_inputs(m, it, 64);
+        tile_async(sX, p.Xs + (size_t)m * TS * TS, TS, it, 64);
+        cp_commit();
         cp_wait<0>();
     };
     for (int m = 0; m < nt; m++) {
+        double* T = sK + (m & 1) * TS * LDT;
         SWW_STAMP(m, 0);
         if (m == 0) {
             for (int e = tid; e < TS * TS; e += LU_THREADS) {
                 const int r = e & 63, c = e >> 6;
-                sT[r * LDT + c] = p.A[(size_t)c * N + r];
+                T[r * LDT + c] = p.A[(size_t)c * N + r];
             }
         } else {
             SWW_STAMP(m, 1);
-            double v[4][2][2], c0[4][2][2];
-            if (mm) {  // V = Z_{m-1} U_{m-1,m} = 2 U + F U
+            double v[2][2][2], c0[2][2][2];
+            if (mm) {  // V = Z_{m-1} U_{m-1,m} = 2 U + F U, my columns
 #pragma unroll
-                SWW_FRAG_LOOP v[x][y][e] = 2.0 * sU[f.col(y, e) * LDO + f.row(x)];
-                mma_tile64(v, sF, sU, f);
+                SWW_FRAGH_LOOP v[x][y][e] = 2.0 * sU[f.col(y, e) * LDO + f.row(x)];
+                mma_half(v, sF, sU, f);
 #pragma unroll
-                SWW_FRAG_LOOP sV[f.col(y, e) * LDO + f.row(x)] = v[x][y][e];
+                SWW_FRAGH_LOOP sV[f.col(y, e) * LDO + f.row(x)] = v[x][y][e];
             }
             __syncthreads();
-            if (mm) {  // S_m = P_m - X_{m,m-1} V
+            if (mm) {  // S_m = P_m - X_{m,m-1} V, my columns -> both CTAs' work tiles
 #pragma unroll
-                SWW_FRAG_LOOP {
-                    c0[x][y][e] = sT[f.col(y, e) * LDO + f.row(x)];
+                SWW_FRAGH_LOOP {
+                    c0[x][y][e] = sP[f.col(y, e) * LDO + f.row(x)];
                     v[x][y][e] = 0.0;
                 }
-                mma_tile64(v, sX, sV, f);
-            }
-            __syncthreads();  // P has been read: sT becomes the row-major work tile
-            if (mm) {
+                mma_half(v, sX, sV, f);
+                const unsigned Tpeer = cluster_map(T, peer);
 #pragma unroll
-                SWW_FRAG_LOOP sT[f.row(x) * LDT + f.col(y, e)] = c0[x][y][e] - v[x][y][e];
+                SWW_FRAGH_LOOP {
+                    const int o = f.row(x) * LDT + cb + f.col(y, e);
+                    const double k = c0[x][y][e] - v[x][y][e];
+                    T[o] = k;
+                    st_cluster_f64(Tpeer + 8u * (unsigned)o, k);
+                }
             }
         }
-        __syncthreads();  // kappa_m complete; sX, sU, sV free
+        cluster_sync_all();  // kappa_m complete in both CTAs (also the CTA barrier: sX, sU, sV, sP free)
         SWW_STAMP(m, 2);
-        bgj64(sT, scr, p.status, tid, p.Fs + (size_t)m * TS * TS, sF);
-        if (role < 0 && m + 1 < nt) fetch_inputs(m + 1);  // (the idle warps are back once sT has been read)
+        bgj64(T, scr, p.status, tid, rank == 0 ? p.Fs + (size_t)m * TS * TS : nullptr, sF);
+        if (role < 0 && m + 1 < nt) fetch_inputs(m + 1);
         __syncthreads();  // F_m in sF and in global memory; the inputs of step m + 1 in shared memory
         SWW_STAMP(m, 3);
-        if (tid == LU_THREADS - 32) st_release(p.zflags + m, epoch);  // a lane of a warp that has no part in the two products
+        if (rank == 0 && tid == LU_THREADS - 32) st_release(p.zflags + m, epoch);  // a lane of a warp that has no part in the products
     }
+    cluster_sync_all();  // neither CTA leaves while the other may still write into its shared memory
 }
 
 __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
     extern __shared__ __align__(16) double lu_sm[];
     const int tid = threadIdx.x;
-    if (blockIdx.x == 0) {
+    if (blockIdx.x < 2) {  // cluster 0
         lu_spine(p, lu_sm);
         return;
     }
@@ -397,7 +462,7 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
         if (tid == 0) st_release(flag, epoch);
     };
 
-    if (blockIdx.x == 1) {  // block row 0 and block column 0 are A itself: final / X-ready from the start
+    if (blockIdx.x == 2) {  // block row 0 and block column 0 are A itself: final / X-ready from the start
         for (int t = tid; t < nt; t += LU_THREADS) {
             st_release(p.flags + t, epoch);
             st_release(p.xready + (size_t)t * nt, epoch);
@@ -507,18 +572,25 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
 #pragma unroll
                 SWW_FRAG_LOOP sA[TS * LDO + f.col(y, e) * LDO + f.row(x)] = l[x][y][e];  // L as an A operand, second stage
             }
-            // The finished left neighbour L_{i,kl} goes out at once: the tasks of the next generation sum it as a plain term and
-            // must be through with that before Z_{kl+1} arrives.
-            if (finish_left) {
-                if (type == T_L && j == i - 1 && i >= 2) {  // the P task of this row reads X_{i,i-2} too
-                    if (tid == 0) spin_until(p.pflags + i, epoch);
-                    __syncthreads();
-                }
-                store_tile(tile(i, kl), N, l);
-            }
             __syncthreads();
-            if (finish_left) publish(p.flags + (size_t)i * nt + kl);
-            if (mm && has_tile) mma_tile64(acc, sA + TS * LDO, sB + TS * LDO, f);
+            // The finished left neighbour L_{i,kl} goes out at once (the tasks of the next generation sum it as a plain term and
+            // must be through with that before Z_{kl+1} arrives) -- by the three warps that have no part in the products, from
+            // the shared-memory copy, while the MMA warps go on with the last term.
+            if (mm) {
+                if (has_tile) mma_tile64(acc, sA + TS * LDO, sB + TS * LDO, f);
+            } else if (finish_left) {
+                const int t = tid - 256;  // 0..95
+                if (type == T_L && j == i - 1 && i >= 2 && t == 0) spin_until(p.pflags + i, epoch);  // P of this row reads X_{i,i-2} too
+                asm volatile("bar.sync 5, 96;" ::: "memory");
+                double* Lg = tile(i, kl);
+                const double* Ls = sA + TS * LDO;
+                for (int c = t; c < TS * TS / 2; c += 96) {
+                    const int col = c >> 5, ch = (c & 31) * 2;
+                    *reinterpret_cast<double2*>(Lg + (size_t)col * N + ch) = *reinterpret_cast<const double2*>(Ls + col * LDO + ch);
+                }
+                asm volatile("bar.sync 5, 96;" ::: "memory");
+                if (t == 0) st_release(p.flags + (size_t)i * nt + kl, epoch);
+            }
         }
         SWW_WSTAMP(5);
 #pragma unroll
@@ -609,9 +681,22 @@ int run_lu(sww_dtn_s* d) {
     a.Xs = Es;
     a.status = d->status;
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), st));
-    const int grid = std::min(sm_count(), 1 + a.ntasks);
+    // clusters of two CTAs: cluster 0 is the spine, every other CTA works on its own (an even grid, one CTA per SM)
+    const int grid = std::min(sm_count() & ~1, (3 + a.ntasks) & ~1);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(LU_THREADS);
+    cfg.dynamicSmemBytes = LU_SMEM_BYTES;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
     SWW_BEGIN(KC_LU, st);
-    k_lu_dataflow<<<grid, LU_THREADS, LU_SMEM_BYTES, st>>>(a);
+    SWW_CUDA(cudaLaunchKernelEx(&cfg, k_lu_dataflow, a));
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
