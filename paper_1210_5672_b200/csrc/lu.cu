@@ -486,17 +486,6 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
             for (int t = tid; t < m; t += LU_THREADS)
                 ready[t] = (ld_acquire(p.flags + (size_t)i * nt + t) == epoch) && (ld_acquire(p.flags + (size_t)t * nt + j) == epoch);
         };
-        auto wait_ready = [&](int k) {  // uniform: ready[] is only written before a __syncthreads
-            if (!ready[k]) {
-                if (tid == 0) {
-                    spin_until(p.flags + (size_t)i * nt + k, epoch);
-                    spin_until(p.flags + (size_t)k * nt + j, epoch);
-                }
-                __syncthreads();
-                refresh();
-                __syncthreads();
-            }
-        };
         auto issue = [&](int k, int buf) {
             tile_async(sA + buf * TS * LDO, tile(i, k), N, tid, LU_THREADS);
             tile_async(sB + buf * TS * LDO, tile(k, j), N, tid, LU_THREADS);
@@ -509,14 +498,31 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
             c0[x][y][e] = (mm && has_tile) ? Cg[(size_t)f.col(y, e) * N + f.row(x)] : 0.0;
             acc[x][y][e] = 0.0;
         }
-        refresh();
+        // term k is not final yet: U_kj (final a generation before L_ik) is fetched first, L_ik as soon as its flag is set
+        auto wait_issue = [&](int k, int buf) {
+            if (tid == 0) spin_tight(p.flags + (size_t)k * nt + j, epoch);
+            __syncthreads();
+            tile_async(sB + buf * TS * LDO, tile(k, j), N, tid, LU_THREADS);
+            cp_commit();
+            if (tid == 0) spin_tight(p.flags + (size_t)i * nt + k, epoch);
+            __syncthreads();
+            tile_async(sA + buf * TS * LDO, tile(i, k), N, tid, LU_THREADS);
+            cp_commit();
+        };
+        refresh();  // what is final at the start of the task
         __syncthreads();
         if (m > 0) {
-            wait_ready(0);
-            issue(0, 0);
+            if (ready[0]) issue(0, 0);
+            else wait_issue(0, 0);
         }
         for (int k = 0; k < m; k++) {
-            const bool pre = (k + 1 < m) && ready[k + 1];
+            bool pre = (k + 1 < m) && ready[k + 1];
+            if (k + 1 < m && !pre) {  // a quick look: the flags may have been set since the task started
+                bool ok = true;
+                if (tid == 0) ok = ld_acquire(p.flags + (size_t)i * nt + k + 1) == epoch;
+                if (tid == 1) ok = ld_acquire(p.flags + (size_t)(k + 1) * nt + j) == epoch;
+                pre = __syncthreads_and(ok);
+            }
             if (pre) {
                 issue(k + 1, (k + 1) & 1);
                 cp_wait<1>();
@@ -526,10 +532,7 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
             __syncthreads();
             if (mm) mma_tile64(acc, sA + (k & 1) * TS * LDO, sB + (k & 1) * TS * LDO, f);
             __syncthreads();
-            if (!pre && k + 1 < m) {
-                wait_ready(k + 1);
-                issue(k + 1, (k + 1) & 1);
-            }
+            if (!pre && k + 1 < m) wait_issue(k + 1, (k + 1) & 1);
         }
         auto store_tile = [&](double* dst, size_t ld, const double (&v)[4][2][2]) {
             if (mm) {
