@@ -1,0 +1,59 @@
+"""Oracle of the shooting map of the overdetermined shooting method -- TEST INFRASTRUCTURE, NOT PRODUCT CODE (see oracle/__init__.py
+for who may import it).  Plain restatement of PAPER.md section 3.1 / 3.3 on the uniform mesh (xi(alpha) = alpha, E = 1, M = N):
+
+  (3.15) PAPER.md:197-200   eta^_k(0) = c_|k| for even k, phi^_k(0) = c_|k| for odd k, 1 <= |k| <= n, all other modes zero:
+                            eta(x, 0) = sum_{k even} 2 c_k cos kx,  phi(x, 0) = sum_{k odd} 2 c_k cos kx  (eta about the mean level)
+  (3.16) PAPER.md:204       T = c_0
+  (3.17) PAPER.md:208       r_i = phi(alpha_i, T/4) sqrt(1/N),  f = r.r / 2
+  (3.31) PAPER.md:296       J_ik = d r_i / d c_k:  k >= 1: phidot_k(alpha_i, T/4) sqrt(1/N) with qdot_k(0) = d q_0 / d c_k, advanced
+                            together with q by (3.32);  k = 0: d/dT of phi at the time T/4, i.e. phi_t(., T/4) / 4 times the
+                            weight (the paper prints the k = 0 row without the 1/4 of the chain rule: reading R13 of DESIGN.md;
+                            tests/test_oracle_pins.py checks the row against finite differences (3.33))
+The time integration is Oracle.rk_advance with nsteps steps of size T / (4 nsteps); phi_t at T/4 is Oracle.rhs of the final state.
+"""
+from __future__ import annotations
+
+import numpy as np
+
+LD = np.longdouble
+
+
+def _split(x):
+    hi = np.asarray(x, dtype=np.float64)
+    return hi, np.asarray(x - hi.astype(LD), dtype=np.float64)
+
+
+def initial_state(c, N: int):
+    """(3.15): -> eta0, phi0 (long double, N) and the columns d q0 / d c_k, k = 1..n, as (deta, dphi) of shape (n, N)"""
+    c = np.asarray(c, dtype=np.float64)
+    n = c.shape[0] - 1
+    j = np.arange(N, dtype=np.int64)
+    eta, phi = np.zeros(N, dtype=LD), np.zeros(N, dtype=LD)
+    deta, dphi = np.zeros((n, N), dtype=LD), np.zeros((n, N), dtype=LD)
+    for k in range(1, n + 1):
+        col = 2 * np.cos(2 * LD(np.pi) * ((k * j) % N).astype(LD) / N)   # 2 cos(k alpha_j), phase reduced exactly
+        if k % 2 == 0:
+            eta += LD(c[k]) * col
+            deta[k - 1] = col
+        else:
+            phi += LD(c[k]) * col
+            dphi[k - 1] = col
+    return eta, phi, deta, dphi
+
+
+def shoot(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True):
+    """-> dict r (N), J (N x (n+1)), eta, phi (the state at T/4), all long double"""
+    c = np.asarray(c, dtype=np.float64)
+    n = c.shape[0] - 1
+    T = float(c[0])
+    eta0, phi0, deta0, dphi0 = initial_state(c, N)
+    dt = T / (4 * nsteps)
+    out = orc.rk_advance(_split(eta0), _split(phi0), h, g, dt, nsteps, deta=_split(deta0), dphi=_split(dphi0), filter=filter)
+    ld = lambda p: p[0].astype(LD) + p[1].astype(LD)
+    eta, phi, dphi = ld(out["eta"]), ld(out["phi"]), ld(out["dphi"])
+    phi_t = ld(orc.rhs(out["eta"], out["phi"], h, g, filter=filter)["phi_t"])
+    w = 1 / np.sqrt(LD(N))
+    J = np.empty((N, n + 1), dtype=LD)
+    J[:, 0] = phi_t * w / 4
+    J[:, 1:] = dphi.T * w
+    return {"r": phi * w, "J": J, "eta": eta, "phi": phi}

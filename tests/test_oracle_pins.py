@@ -561,3 +561,56 @@ def test_variational_columns_track_finite_differences(orc_ld):
         fd = _richardson(F, 2e-2)
         want = np.concatenate([ld(lin["deta"])[col], ld(lin["dphi"])[col]])
         assert np.abs(fd - want).max() < 1e-11, col
+
+
+# ------------------------------------------------------------------------------------------------ shooting map (3.15)-(3.17), (3.31)
+def test_shooting_map_linear_theory(orc_ld):
+    """small amplitude: phi(x, t) = 2 eps cos x cos(omega t) + O(eps^2), omega^2 = g tanh h ((4.35)), and a unit
+    perturbation of mode k evolves as eta' = A cos(omega_k t), phi' = -(g/omega_k) A sin(omega_k t): closed forms of r and of
+    the columns 0, 1, 2 of J at leading order"""
+    from oracle import shooting
+    N, h, g, eps, nsteps = 32, 1.0, 1.0, 1e-7, 16
+    om = [0.0] + [math.sqrt(g * k * math.tanh(k * h)) for k in range(1, 4)]
+    T = 6.9   # deliberately off the linear period 7.19976
+    c = np.array([T, eps, 0.0, 0.0])
+    s = shooting.shoot(orc_ld, c, N, h, g, nsteps)
+    x = si.grid(N)
+    w = 1 / math.sqrt(N)
+    assert np.abs(s["r"] - 2 * eps * np.cos(x) * math.cos(om[1] * T / 4) * w).max() < 1e-13 * eps + 50 * eps * eps
+    assert np.abs(s["J"][:, 0] - (-(om[1] / 4) * 2 * eps * np.cos(x) * math.sin(om[1] * T / 4) * w)).max() < 1e-13 * eps + 50 * eps * eps
+    assert np.abs(s["J"][:, 1] - 2 * np.cos(x) * math.cos(om[1] * T / 4) * w).max() < 1e-6
+    assert np.abs(s["J"][:, 2] - (-(g / om[2]) * 2 * np.cos(2 * x) * math.sin(om[2] * T / 4) * w)).max() < 1e-6
+    assert np.abs(s["J"][:, 3] - 2 * np.cos(3 * x) * math.cos(om[3] * T / 4) * w).max() < 1e-6
+
+
+def test_shooting_jacobian_matches_finite_differences(orc_ld):
+    """(3.33), PAPER.md:307-312: J_ik = [r_i(c + e e_k) - r_i(c - e e_k)] / 2e, Richardson-extrapolated, at a finite amplitude;
+    this also fixes the factor 1/4 of the k = 0 (period) column (R13)"""
+    from oracle import shooting
+    N, h, g, nsteps = 32, 1.0, 1.0, 12
+    c = np.array([7.1, 0.02, 0.004, -0.001, 0.0005])
+    s = shooting.shoot(orc_ld, c, N, h, g, nsteps)
+    for k in range(c.shape[0]):
+        def F(e):
+            ck = c.copy()
+            ck[k] += e
+            return shooting.shoot(orc_ld, ck, N, h, g, nsteps)["r"]
+        e0 = 2e-3 if k else 2e-2
+        d1 = (F(e0) - F(-e0)) / (2 * e0)
+        d2 = (F(e0 / 2) - F(-e0 / 2)) / e0
+        fd = (4 * d2 - d1) / 3
+        assert np.abs(fd - s["J"][:, k]).max() < 1e-8 * max(1.0, float(np.abs(s["J"][:, k]).max())), k
+
+
+def test_shooting_recovers_the_linear_period(orc_ld):
+    """Gauss-Newton on the period alone along the small-amplitude branch converges to T = 7.19976"""
+    from oracle import shooting
+    N, h, g, eps, nsteps = 32, 1.0, 1.0, 1e-6, 16
+    T = 7.0
+    for _ in range(6):
+        s = shooting.shoot(orc_ld, np.array([T, eps]), N, h, g, nsteps)
+        J0, r = s["J"][:, 0], s["r"]
+        T = T - float((J0 @ r) / (J0 @ J0))
+    want, tol = golden()["T_linear_h1"]
+    assert abs(T - want) < tol
+    assert float(0.5 * (s["r"] @ s["r"])) < 1e-22
