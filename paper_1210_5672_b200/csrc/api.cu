@@ -102,7 +102,7 @@ int sww_dtn_setup(const void* eta, int N, double h, int prec, void* stream, sww_
     auto alloc = [&](double** p, size_t n) { if (ok && cudaMalloc(p, n * sizeof(double)) != cudaSuccess) ok = false; };
     alloc(&d->eta, 2 * N); alloc(&d->d1, 2 * N); alloc(&d->d2, 2 * N);
     alloc(&d->E, 2 * N); alloc(&d->Dm, 2 * N); alloc(&d->Sh, 2 * N); alloc(&d->Ch, 2 * N);
-    alloc(&d->K, mat); alloc(&d->G, mat); alloc(&d->LU, n2); alloc(&d->invD, 2 * (size_t)N * nb);
+    alloc(&d->K, mat); alloc(&d->G, mat); alloc(&d->LU, n2); alloc(&d->invD, 3 * (size_t)N * nb);
     alloc(&d->bphi, 2 * N); alloc(&d->bW0, 2 * N); alloc(&d->bu, 2 * N); alloc(&d->bv, 2 * N); alloc(&d->tmp, 14 * (size_t)N);
     // column chunks of the dd base-state pass: enough CTAs to fill the chip at small N (4 columns per chunk at least)
     d->bp_chunks = std::max(1, std::min(N / 4, std::max(N / 32, 64)));

@@ -219,6 +219,7 @@ struct LuArgs {
     unsigned* counter;  // next task to claim (zeroed before the launch)
     double* Fs;        // nt blocks of 64 x 64 (column-major, ld 64): inv(S_m) - 2 I
     double* Xs;        // nt blocks of 64 x 64 (column-major, ld 64): staging of X_{m,m-1}
+    double* Vs;        // nt blocks of 64 x 64 (column-major, ld 64): V_m = inv(S_m) U_{m,m+1}, the front term of the backward sweep
     int* status;
 };
 
@@ -410,6 +411,9 @@ __device__ void lu_spine(const LuArgs& p, double* sm) {
                 mma_half(v, sF, sU, f);
 #pragma unroll
                 SWW_FRAGH_LOOP sV[f.col(y, e) * LDO + f.row(x)] = v[x][y][e];
+                double* Vg = p.Vs + (size_t)(m - 1) * TS * TS + (size_t)cb * TS;  // kept for the triangular solves
+#pragma unroll
+                SWW_FRAGH_LOOP Vg[f.col(y, e) * TS + f.row(x)] = v[x][y][e];
             }
             __syncthreads();
             if (mm) {  // S_m = P_m - X_{m,m-1} V, my columns -> both CTAs' work tiles
@@ -682,10 +686,11 @@ int run_lu(sww_dtn_s* d) {
     a.epoch = ++d->lu_epoch;
     a.Fs = Fs;
     a.Xs = Es;
+    a.Vs = d->invD + 2 * (size_t)nblk * nb * nb;
     a.status = d->status;
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), st));
     // clusters of two CTAs: cluster 0 is the spine, every other CTA works on its own (an even grid, one CTA per SM)
-    const int grid = std::min(sm_count() & ~1, (3 + a.ntasks) & ~1);
+    const int grid = std::min(SWW_TUNE_INT("SWW_LU_GRID", sm_count()) & ~1, (3 + a.ntasks) & ~1);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(LU_THREADS);
@@ -762,6 +767,7 @@ __global__ void __launch_bounds__(64) k_solve_small(int N, const double* __restr
 struct TrsmArgs {
     const double* A;     // LU factors, N x N column-major (L multipliers below the diagonal, U above)
     const double* Fs;    // nt blocks of 64 x 64 (column-major, ld 64): inv(S_i) - 2 I
+    const double* Vs;    // nt blocks of 64 x 64 (column-major, ld 64): V_i = inv(S_i) U_{i,i+1}
     double *B, *Blo;     // N x (ns*WS) column-major, ld = N; in: right-hand sides (Blo ignored), out: solution hi, lo
     int N, nt, ns;       // nt row blocks of 64, ns column slabs
     double *Yh, *Yl, *Xh;  // scratch, same shape as B: forward result (hi, lo) and backward result (hi); pre-filled with TR_ABSENT
@@ -992,6 +998,316 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
     }
 }
 
+// ------------------------------------------------------------------------------------------------ the same solve, warp-specialized
+// k_trsm_ws: the tasks, the hand-over protocol and the compensated arithmetic of k_trsm_dataflow, but the operands come through
+// a ring of ST stages filled by two dedicated LOADER warps (cp.async, mbarrier full / empty pairs) while the eight MMA warps do
+// nothing but fragment loads and DMMAs: the loaders run up to ST - 1 steps ahead of the products, look for the absent pattern
+// in the solution blocks they fetched (each thread in its own chunks) and ask L2 again until a block is complete, so the MMA
+// warps never poll, never issue a copy and meet no CTA-wide barrier inside a task.
+// Backward sweep: x_i = Z_i (y_i - sum_{k>i+1} U_ik x_k) - V_i x_{i+1} with V_i = Z_i U_{i,i+1} kept by the LU spine: the product
+// with the diagonal block is done before the front block x_{i+1} arrives, a link of the chain is one product in both sweeps.
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    asm volatile(
+        "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    while (!mbar_test(bar, parity)) {
+    }
+}
+// named barrier 1 with an OR reduction among the 256 threads of the MMA warps
+__device__ __forceinline__ bool mma_bar_or(bool pred) {
+    int r;
+    asm volatile(
+        "{\n.reg .pred p, q;\nsetp.ne.b32 p, %1, 0;\nbar.red.or.pred q, 1, 256, p;\nselp.b32 %0, 1, 0, q;\n}"
+        : "=r"(r)
+        : "r"((int)pred)
+        : "memory");
+    return r != 0;
+}
+
+template <int WS>
+struct TrsmWsCfg {
+    static constexpr int WC = WS / 8;               // MMA warps across the slab's columns (8 columns per warp)
+    static constexpr int WR = 8 / WC;               // MMA warps across the 64 rows
+    static constexpr int FM = (TS / WR) / 8;        // 8 x 8 fragments per warp along the rows
+    static constexpr int ST = WS <= 32 ? 3 : 2;     // stages of the operand ring
+    static constexpr int THREADS = 320;             // 8 MMA warps + 2 loader warps
+    static constexpr int NLOAD = 64;
+    // ring (factor tile + solution tile per stage), F_i, z (the B operand of the diagonal product)
+    static constexpr int SMEM = ((ST + 1) * TS * LDO + (ST + 1) * WS * LDO) * (int)sizeof(double) + 256;
+};
+
+template <int WS>
+__global__ void __launch_bounds__(320, 1) k_trsm_ws(TrsmArgs p) {
+    using C = TrsmWsCfg<WS>;
+    constexpr int ST = C::ST, NL = C::NLOAD;
+    extern __shared__ __align__(16) double tr_sm[];
+    double* sA = tr_sm;                    // ST stages of the factor tile as As[k][r]
+    double* sD = sA + ST * TS * LDO;       // the diagonal block F_i of the backward sweep, as As[k][r]
+    double* sB = sD + TS * LDO;            // ST stages of the solution tile as Bs[n][k]
+    double* sZ = sB + ST * WS * LDO;       // z as Bs[n][k]
+    __shared__ unsigned long long full[ST], empty[ST], fullD;
+    __shared__ int s_task, s_abort;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool loader = warp >= 8;
+    const int lt = tid - 256;                  // loader thread index 0..63
+    const int wr = warp % C::WR, wc = warp / C::WR, fr = lane >> 2, fk = lane & 3;
+    const int N = p.N, nt = p.nt, ns = p.ns;
+    const int row0 = wr * (TS / C::WR) + fr;   // + 8 x : row of this lane's fragment element
+    const int col0 = wc * 8 + 2 * fk;          // + e   : column within the slab
+    if (tid == 0) {
+        for (int s = 0; s < ST; s++) {
+            mbar_init(&full[s], NL);
+            mbar_init(&empty[s], 8);
+        }
+        mbar_init(&fullD, NL);
+        s_abort = 0;
+    }
+    unsigned it = 0;   // ring position: products done so far by this CTA (the same number in every thread)
+    unsigned nd = 0;   // backward tasks done so far (phase of fullD)
+
+    for (;;) {
+        __syncthreads();  // the previous task is through with the ring, sD and sZ; the barriers are initialised
+        if (tid == 0) {
+            s_task = (int)atomicAdd(p.counter, 1u);
+            if (ld_status(p.status) != SWW_OK) s_abort = 1;
+        }
+        __syncthreads();
+        int task = s_task;
+        if (task >= 2 * nt * ns) break;
+        if (s_abort) break;  // some task gave up (or the handle already carries an error): stop polling, leave at once
+        const int phase = task >= nt * ns;
+        if (phase) task -= nt * ns;
+        const int s = task % ns, i = phase ? nt - 1 - task / ns : task / ns;
+        const int m = phase ? nt - 1 - i : i;  // number of finished blocks this one depends on
+        const size_t blk = (size_t)s * WS * N + (size_t)i * TS;
+        const double* Vin = phase ? p.Xh : p.Yh;  // the vector this sweep consumes block by block
+
+        if (loader) {
+            // ---------------------------------------------------------------------------------- the loader warps
+            auto kblock = [&](int kk) { return phase ? nt - 1 - kk : kk; };
+            auto issueA = [&](int kk, int buf) {
+                const bool front = phase && kk == m - 1;  // backward: the term of block i + 1 goes through V_i = inv(S_i) U_{i,i+1}
+                const double* Ag = front ? p.Vs + (size_t)i * TS * TS : p.A + (size_t)kblock(kk) * TS * N + (size_t)i * TS;  // factor tile (i, k)
+                const size_t lda = front ? (size_t)TS : (size_t)N;
+                double* a = sA + buf * TS * LDO;
+#pragma unroll 4
+                for (int c = lt; c < TS * TS / 2; c += NL) {
+                    const int col = c >> 5, ch = (c & 31) * 2;
+                    cp16(a + col * LDO + ch, Ag + col * lda + ch);
+                }
+            };
+            auto issueY = [&](int kk, int buf) {
+                const double* Yg = Vin + (size_t)s * WS * N + (size_t)kblock(kk) * TS;   // solution block k of this slab
+                double* b = sB + buf * WS * LDO;
+#pragma unroll 4
+                for (int c = lt; c < WS * TS / 2; c += NL) {
+                    const int col = c >> 5, ch = (c & 31) * 2;
+                    cp16(b + col * LDO + ch, Yg + (size_t)col * N + ch);
+                }
+            };
+            if (phase) {  // block LU: L has identity diagonal blocks, only the backward sweep has a diagonal product
+                const double* Dg = p.Fs + (size_t)i * TS * TS;
+                for (int c = lt; c < TS * TS / 2; c += NL) {
+                    const int col = c >> 5, ch = (c & 31) * 2;
+                    cp16(sD + col * LDO + ch, Dg + col * TS + ch);  // As[k][r] = D[r][k]
+                }
+                cp_commit();
+            }
+            int issued = 0;
+            auto issue_stage = [&]() {
+                const unsigned g = it + (unsigned)issued;
+                const int buf = (int)(g % ST);
+                mbar_wait(&empty[buf], ((g / ST) & 1u) ^ 1u);  // the products of the stage that used this buffer are done
+                issueA(issued, buf);
+                issueY(issued, buf);
+                cp_commit();
+                issued++;
+            };
+            while (issued < m && issued < ST - 1) issue_stage();
+            for (int kk = 0; kk < m; kk++) {
+                const int buf = (int)((it + (unsigned)kk) % ST);
+                if (issued - 1 - kk >= 1) cp_wait<1>();
+                else cp_wait<0>();
+                if (kk == 0 && phase) mbar_arrive(&fullD);  // the group of F_i is older than that of stage 0
+                // my part of the block is not there yet: ask L2 again for what is missing
+                const double* Yg = Vin + (size_t)s * WS * N + (size_t)kblock(kk) * TS;
+                double* b = sB + buf * WS * LDO;
+                for (int spin = 0;; spin++) {
+                    bool bad = false;
+                    for (int c = lt; c < WS * TS / 2; c += NL) {
+                        const int col = c >> 5, ch = (c & 31) * 2;
+                        const double2 v = *reinterpret_cast<const double2*>(b + col * LDO + ch);
+                        if ((__double_as_longlong(v.x) == TR_ABSENT) | (__double_as_longlong(v.y) == TR_ABSENT)) {
+                            cp16(b + col * LDO + ch, Yg + (size_t)col * N + ch);
+                            bad = true;
+                        }
+                    }
+                    if (!bad) break;
+                    cp_commit();
+                    cp_wait<0>();
+                    if (spin > TR_SPIN_LIMIT) {
+                        atomicCAS(p.status, SWW_OK, SWW_ECUDA);
+                        s_abort = 1;
+                        break;
+                    }
+                    if ((spin & 63) == 63 && (s_abort || ld_status(p.status) != SWW_OK)) {
+                        s_abort = 1;
+                        break;
+                    }
+                }
+                mbar_arrive(&full[buf]);
+                if (issued < m) issue_stage();
+            }
+            if (phase && m == 0) {
+                cp_wait<0>();
+                mbar_arrive(&fullD);
+            }
+        } else {
+            // ---------------------------------------------------------------------------------- the MMA warps
+            double* Bg = p.B + blk;
+            double* Lg = p.Blo + blk;
+            double acc[C::FM][2], ph[C::FM][2], pl[C::FM][2];
+#pragma unroll
+            for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) acc[x][e] = ph[x][e] = pl[x][e] = 0.0;
+            auto mma_tile = [&](const double* a, const double* b) {
+                const double* as = a + row0;
+                const double* bs = b + (wc * 8 + fr) * LDO;
+#pragma unroll
+                for (int k4 = 0; k4 < TS; k4 += 4) {
+                    const double bf = bs[k4 + fk];
+#pragma unroll
+                    for (int x = 0; x < C::FM; x++) lu_dmma884(acc[x][0], acc[x][1], as[(k4 + fk) * LDO + x * 8], bf);
+                }
+            };
+            auto fold = [&]() {  // (ph, pl) += acc, error-free; acc = 0
+#pragma unroll
+                for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        double s_, e_;
+                        two_sum_d(ph[x][e], acc[x][e], s_, e_);
+                        ph[x][e] = s_;
+                        pl[x][e] += e_;
+                        acc[x][e] = 0.0;
+                    }
+            };
+            // the block's own right-hand side: forward B_i (plain fp64), backward the forward result (hi, lo), reloaded until
+            // all of it is there (it is final long before, except at the turn of the sweeps); the loaders work meanwhile
+            double bh[C::FM][2], bl[C::FM][2];
+            for (int spin = 0;; spin++) {
+                bool bad = false;
+#pragma unroll
+                for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
+                        if (phase) {
+                            bh[x][e] = __ldcg(p.Yh + blk + o);
+                            bl[x][e] = __ldcg(p.Yl + blk + o);
+                            bad |= (__double_as_longlong(bh[x][e]) == TR_ABSENT) | (__double_as_longlong(bl[x][e]) == TR_ABSENT);
+                        } else {
+                            bh[x][e] = tr_canon(Bg[o]);
+                            bl[x][e] = 0.0;  // the forward sweep starts from plain fp64 right-hand sides
+                        }
+                    }
+                if (!phase || !mma_bar_or(bad)) break;
+                if (spin > TR_SPIN_LIMIT) {
+                    if (tid == 0) atomicCAS(p.status, SWW_OK, SWW_ECUDA);
+                    break;
+                }
+                if ((spin & 63) == 63 && mma_bar_or(tid == 0 && ld_status(p.status) != SWW_OK)) break;
+            }
+            auto step = [&](int kk) {
+                const unsigned g = it + (unsigned)kk;
+                const int buf = (int)(g % ST);
+                mbar_wait(&full[buf], (g / ST) & 1u);
+                mma_tile(sA + buf * TS * LDO, sB + buf * WS * LDO);
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[buf]);
+            };
+            // forward: all m terms; backward: the terms of the blocks k > i + 1 (the front term comes last, through V_i)
+            const int mb = phase ? (m > 0 ? m - 1 : 0) : m;
+            for (int kk = 0; kk < mb; kk++) {
+                step(kk);
+                if ((kk % TR_FOLD) == TR_FOLD - 1) fold();
+            }
+            fold();
+            // z = (bh + bl) - (ph + pl) as sh + sl
+            double sh[C::FM][2], sl[C::FM][2];
+#pragma unroll
+            for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    double s_, e_;
+                    two_sum_d(bh[x][e], -ph[x][e], s_, e_);
+                    sh[x][e] = s_;
+                    sl[x][e] = e_ + (bl[x][e] - pl[x][e]);
+                    if (phase) sZ[(col0 + e) * LDO + row0 + x * 8] = s_;  // Bs[n][k] = z[k][n]
+                }
+            if (phase) {
+                // backward: w = Z_i z = 2 z + F_i z (before the front block is there), then x_i = w - V_i x_{i+1}
+                asm volatile("bar.sync 1, 256;" ::: "memory");  // z complete (the MMA warps only)
+                mbar_wait(&fullD, nd & 1u);
+                mma_tile(sD, sZ);
+#pragma unroll
+                for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        double t_, e_;
+                        two_sum_d(2.0 * sh[x][e], acc[x][e], t_, e_);
+                        sh[x][e] = t_;
+                        sl[x][e] = fma(2.0, sl[x][e], e_);
+                        acc[x][e] = 0.0;
+                    }
+                if (m > 0) {
+                    step(m - 1);
+#pragma unroll
+                    for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                        for (int e = 0; e < 2; e++) {
+                            double t_, e_;
+                            two_sum_d(sh[x][e], -acc[x][e], t_, e_);
+                            sh[x][e] = t_;
+                            sl[x][e] += e_;
+                        }
+                }
+            }
+#pragma unroll
+            for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
+                    const double hi = __dadd_rn(sh[x][e], sl[x][e]);
+                    const double low = __dsub_rn(sl[x][e], __dsub_rn(hi, sh[x][e]));
+                    if (phase) {  // x_i: to its consumers, and the result
+                        p.Xh[blk + o] = tr_canon(hi);
+                        Bg[o] = hi;
+                        Lg[o] = low;
+                    } else {      // y_i: hi for the forward tasks below, hi and lo for this block's backward task
+                        p.Yh[blk + o] = tr_canon(hi);
+                        p.Yl[blk + o] = tr_canon(low);
+                    }
+                }
+        }
+        it += (unsigned)m;
+        nd += (unsigned)phase;
+    }
+}
+
 template <int WS>
 static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     using C = TrsmCfg<WS>;
@@ -1003,6 +1319,7 @@ static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     TrsmArgs a;
     a.A = d->LU;
     a.Fs = d->invD + (size_t)nt * TS * TS;
+    a.Vs = d->invD + 2 * (size_t)nt * TS * TS;
     a.B = B;
     a.Blo = Blo;
     a.N = N;
@@ -1026,7 +1343,14 @@ static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), d->stream));
     const int grid = std::min(sm_count(), 2 * nt * ns);
     SWW_BEGIN(WS == 8 ? KC_TRSV : KC_TRSM, d->stream);  // the 8-column instantiation serves the single-vector solves: chain-latency-bound
-    k_trsm_dataflow<WS><<<grid, 256, C::SMEM, d->stream>>>(a);
+    if (SWW_TUNE_INT("SWW_TR_IMPL", WS >= 16 ? 1 : 0)) {
+        using W = TrsmWsCfg<WS>;
+        static DeviceOnce attr_ws;
+        if (attr_ws.first()) SWW_CUDA(cudaFuncSetAttribute(k_trsm_ws<WS>, cudaFuncAttributeMaxDynamicSharedMemorySize, W::SMEM));
+        k_trsm_ws<WS><<<grid, W::THREADS, W::SMEM, d->stream>>>(a);
+    } else {
+        k_trsm_dataflow<WS><<<grid, 256, C::SMEM, d->stream>>>(a);
+    }
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -1049,7 +1373,7 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
     // slab width: the chain of a slab is 2 N/64 links of (flag hop + one or two 64 x 64 x WS products), so narrow slabs finish
     // sooner as long as there are few of them; every slab re-reads the factors from L2, so many columns want wide slabs
     // (measured at N = 2048: 128 columns 0.19 ms with 16-column slabs against 0.27 ms with 32; 512 columns 0.36 against 0.34)
-    const int ws = ncols <= 64 ? 8 : (ncols <= 256 ? 16 : 32);
+    const int ws = ncols <= 64 ? 8 : SWW_TUNE_INT("SWW_TR_WS", ncols <= 256 ? 16 : 32);
     for (int c0 = 0; c0 < ncols; c0 += TR_MAXNS * ws) {
         const int nc = std::min(ncols - c0, TR_MAXNS * ws);
         double *b = B + (size_t)c0 * N, *bl = Blo + (size_t)c0 * N;
@@ -1057,8 +1381,10 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
             SWW_TRY(launch_trsm<8>(d, b, bl, (nc + 7) / 8));
         else if (ws == 16)
             SWW_TRY(launch_trsm<16>(d, b, bl, (nc + 15) / 16));
-        else
+        else if (ws == 32)
             SWW_TRY(launch_trsm<32>(d, b, bl, (nc + 31) / 32));
+        else
+            SWW_TRY(launch_trsm<64>(d, b, bl, (nc + 63) / 64));
     }
     return SWW_OK;
 }
