@@ -800,7 +800,7 @@ struct TrsmCfg {
     static constexpr int WR = 8 / WC;               // warps across the 64 rows
     static constexpr int FM = (TS / WR) / 8;        // 8 x 8 fragments per warp along the rows
     static constexpr int WSP = WC * 8;              // columns covered = WS
-    static constexpr int SMEM = (3 * TS * LDO + 2 * WS * LDO) * (int)sizeof(double) + 256;
+    static constexpr int SMEM = (3 * TS * LDO + 3 * WS * LDO) * (int)sizeof(double) + 256;
 };
 
 template <int WS>
@@ -810,6 +810,7 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
     double* sA = tr_sm;                    // 2 stages of the factor tile as As[k][r]
     double* sD = sA + 2 * TS * LDO;        // the diagonal block F_i of the backward sweep, as As[k][r]
     double* sB = sD + TS * LDO;            // 2 stages of the solution tile as Bs[n][k]
+    double* sZ = sB + 2 * WS * LDO;        // z as Bs[n][k] (the B operand of the diagonal product)
     __shared__ int s_task, s_abort;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int wr = warp % C::WR, wc = warp / C::WR, fr = lane >> 2, fk = lane & 3;
@@ -840,11 +841,13 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
         // only the (small) solution block is loaded behind the flag on the chain of a slab
         auto issueA = [&](int kk, int buf) {
             const int k = kblock(kk);
-            const double* Ag = p.A + (size_t)k * TS * N + (size_t)i * TS;          // factor tile (i, k)
+            const bool front = phase && kk == m - 1;  // backward: the term of block i + 1 goes through V_i = inv(S_i) U_{i,i+1}
+            const double* Ag = front ? p.Vs + (size_t)i * TS * TS : p.A + (size_t)k * TS * N + (size_t)i * TS;  // factor tile (i, k)
+            const size_t lda = front ? (size_t)TS : (size_t)N;
             double* a = sA + buf * TS * LDO;
             for (int c = tid; c < TS * TS / 2; c += 256) {
                 const int col = c >> 5, ch = (c & 31) * 2;
-                cp16(a + col * LDO + ch, Ag + (size_t)col * N + ch);
+                cp16(a + col * LDO + ch, Ag + col * lda + ch);
             }
         };
         // true if any of the entries THIS thread requested in issueY is still absent (call after its cp.async group completed)
@@ -936,10 +939,11 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             issueA(0, 0);
             cp_commit();
         }
-        for (int kk = 0; kk < m; kk++) {
+        // one term: the solution block is asked for at its own step and reloaded until complete, then the product
+        auto term = [&](int kk, bool more) {
             issueY(kk, kk & 1);
             cp_commit();
-            if (kk + 1 < m) {
+            if (more) {
                 issueA(kk + 1, (kk + 1) & 1);
                 cp_commit();
                 cp_wait<1>();
@@ -953,11 +957,16 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 cp_wait<0>();
             }
             mma_tile(sA + (kk & 1) * TS * LDO, sB + (kk & 1) * WS * LDO);
+        };
+        // forward: all m terms; backward: the terms of the blocks k > i + 1 (the front term comes last, through V_i)
+        const int mb = phase ? (m > 0 ? m - 1 : 0) : m;
+        for (int kk = 0; kk < mb; kk++) {
+            term(kk, kk + 1 < m);
             if ((kk % TR_FOLD) == TR_FOLD - 1) fold();
             __syncthreads();
         }
         fold();
-        // z = (bh + bl) - (ph + pl) as sh + sl ; then the diagonal block: forward y = z, backward x = Z_i z = 2 z + F_i z
+        // z = (bh + bl) - (ph + pl) as sh + sl
         double sh[C::FM][2], sl[C::FM][2];
 #pragma unroll
         for (int x = 0; x < C::FM; x++)
@@ -967,25 +976,44 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
                 two_sum_d(bh[x][e], -ph[x][e], s_, e_);
                 sh[x][e] = s_;
                 sl[x][e] = e_ + (bl[x][e] - pl[x][e]);
-                sB[(col0 + e) * LDO + row0 + x * 8] = s_;  // Bs[n][k] = z[k][n]
-                acc[x][e] = 0.0;
+                if (phase) sZ[(col0 + e) * LDO + row0 + x * 8] = s_;  // Bs[n][k] = z[k][n]
             }
         if (phase) {
-            cp_wait<0>();  // F_i (requested at the start of the task) when m == 0
+            // backward: w = Z_i z = 2 z + F_i z (before the front block is there), then x_i = w - V_i x_{i+1}
+            if (m >= 1) cp_wait<1>();  // F_i (the oldest group); the front factor tile may still be in flight
+            else cp_wait<0>();
             __syncthreads();
-            mma_tile(sD, sB);
+            mma_tile(sD, sZ);
+#pragma unroll
+            for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                for (int e = 0; e < 2; e++) {
+                    double t_, e_;
+                    two_sum_d(2.0 * sh[x][e], acc[x][e], t_, e_);
+                    sh[x][e] = t_;
+                    sl[x][e] = fma(2.0, sl[x][e], e_);
+                    acc[x][e] = 0.0;
+                }
+            if (m > 0) {
+                term(m - 1, false);
+#pragma unroll
+                for (int x = 0; x < C::FM; x++)
+#pragma unroll
+                    for (int e = 0; e < 2; e++) {
+                        double t_, e_;
+                        two_sum_d(sh[x][e], -acc[x][e], t_, e_);
+                        sh[x][e] = t_;
+                        sl[x][e] += e_;
+                    }
+            }
         }
-        const double sc = phase ? 2.0 : 1.0;
 #pragma unroll
         for (int x = 0; x < C::FM; x++)
 #pragma unroll
             for (int e = 0; e < 2; e++) {
                 const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
-                double t_, e_;
-                two_sum_d(sc * sh[x][e], acc[x][e], t_, e_);
-                const double lo = fma(sc, sl[x][e], e_);
-                const double hi = __dadd_rn(t_, lo);
-                const double low = __dsub_rn(lo, __dsub_rn(hi, t_));
+                const double hi = __dadd_rn(sh[x][e], sl[x][e]);
+                const double low = __dsub_rn(sl[x][e], __dsub_rn(hi, sh[x][e]));
                 if (phase) {  // x_i: to its consumers, and the result
                     p.Xh[blk + o] = tr_canon(hi);
                     Bg[o] = hi;
@@ -1141,30 +1169,69 @@ __global__ void __launch_bounds__(320, 1) k_trsm_ws(TrsmArgs p) {
                 if (issued - 1 - kk >= 1) cp_wait<1>();
                 else cp_wait<0>();
                 if (kk == 0 && phase) mbar_arrive(&fullD);  // the group of F_i is older than that of stage 0
-                // my part of the block is not there yet: ask L2 again for what is missing
+                // My part of the block as the copy brought it: complete?  If not (the chain front: the producer has not stored it
+                // yet), poll with plain L2 loads into registers -- first one sentinel chunk (1 KB of polling traffic per CTA and
+                // round; every row below waits for the same block), then all of my chunks until none shows the absent pattern --
+                // and put the block into the stage by hand.  A round of register loads is a third of a cp.async round + rescan.
                 const double* Yg = Vin + (size_t)s * WS * N + (size_t)kblock(kk) * TS;
                 double* b = sB + buf * WS * LDO;
-                for (int spin = 0;; spin++) {
-                    bool bad = false;
-                    for (int c = lt; c < WS * TS / 2; c += NL) {
-                        const int col = c >> 5, ch = (c & 31) * 2;
-                        const double2 v = *reinterpret_cast<const double2*>(b + col * LDO + ch);
-                        if ((__double_as_longlong(v.x) == TR_ABSENT) | (__double_as_longlong(v.y) == TR_ABSENT)) {
-                            cp16(b + col * LDO + ch, Yg + (size_t)col * N + ch);
-                            bad = true;
+                constexpr int NCH = WS * TS / 2 / NL;  // 16-byte chunks per loader thread
+                bool bad = false;
+#pragma unroll
+                for (int q = 0; q < NCH; q++) {
+                    const int c = lt + q * NL, col = c >> 5, ch = (c & 31) * 2;
+                    const double2 v = *reinterpret_cast<const double2*>(b + col * LDO + ch);
+                    bad |= (__double_as_longlong(v.x) == TR_ABSENT) | (__double_as_longlong(v.y) == TR_ABSENT);
+                }
+                if (bad) {
+                    bool out = false;
+                    {
+                        const int col = lt >> 5, ch = (lt & 31) * 2;
+                        const double2* g0 = reinterpret_cast<const double2*>(Yg + (size_t)col * N + ch);
+                        for (int spin = 0;; spin++) {
+                            const double2 v = __ldcg(g0);
+                            if (!((__double_as_longlong(v.x) == TR_ABSENT) | (__double_as_longlong(v.y) == TR_ABSENT))) break;
+                            if (spin > 8 * TR_SPIN_LIMIT) {
+                                atomicCAS(p.status, SWW_OK, SWW_ECUDA);
+                                s_abort = 1;
+                                out = true;
+                                break;
+                            }
+                            if ((spin & 255) == 255 && (s_abort || ld_status(p.status) != SWW_OK)) {
+                                s_abort = 1;
+                                out = true;
+                                break;
+                            }
                         }
                     }
-                    if (!bad) break;
-                    cp_commit();
-                    cp_wait<0>();
-                    if (spin > TR_SPIN_LIMIT) {
-                        atomicCAS(p.status, SWW_OK, SWW_ECUDA);
-                        s_abort = 1;
-                        break;
+                    double2 v[NCH];
+                    for (int spin = 0; !out; spin++) {
+                        bool miss = false;
+#pragma unroll
+                        for (int q = 0; q < NCH; q++) {
+                            const int c = lt + q * NL, col = c >> 5, ch = (c & 31) * 2;
+                            v[q] = __ldcg(reinterpret_cast<const double2*>(Yg + (size_t)col * N + ch));
+                        }
+#pragma unroll
+                        for (int q = 0; q < NCH; q++)
+                            miss |= (__double_as_longlong(v[q].x) == TR_ABSENT) | (__double_as_longlong(v[q].y) == TR_ABSENT);
+                        if (!miss) break;
+                        if (spin > TR_SPIN_LIMIT) {
+                            atomicCAS(p.status, SWW_OK, SWW_ECUDA);
+                            s_abort = 1;
+                            break;
+                        }
+                        if ((spin & 63) == 63 && (s_abort || ld_status(p.status) != SWW_OK)) {
+                            s_abort = 1;
+                            break;
+                        }
                     }
-                    if ((spin & 63) == 63 && (s_abort || ld_status(p.status) != SWW_OK)) {
-                        s_abort = 1;
-                        break;
+                    if (!out) {
+#pragma unroll
+                        for (int q = 0; q < NCH; q++) {
+                            const int c = lt + q * NL, col = c >> 5, ch = (c & 31) * 2;
+                            *reinterpret_cast<double2*>(b + col * LDO + ch) = v[q];
+                        }
                     }
                 }
                 mbar_arrive(&full[buf]);
@@ -1381,10 +1448,8 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
             SWW_TRY(launch_trsm<8>(d, b, bl, (nc + 7) / 8));
         else if (ws == 16)
             SWW_TRY(launch_trsm<16>(d, b, bl, (nc + 15) / 16));
-        else if (ws == 32)
-            SWW_TRY(launch_trsm<32>(d, b, bl, (nc + 31) / 32));
         else
-            SWW_TRY(launch_trsm<64>(d, b, bl, (nc + 63) / 64));
+            SWW_TRY(launch_trsm<32>(d, b, bl, (nc + 31) / 32));
     }
     return SWW_OK;
 }
