@@ -36,6 +36,7 @@ extern "C" {
 
 typedef struct sww_dtn_s*   sww_dtn_t;   /* one surface: K, G, LU(I/2+K), node tables, base state, workspace (device)  */
 typedef struct sww_state_s* sww_state_t; /* time-stepper state: eta, phi, optional variational columns, RK stage storage */
+typedef struct sww_shooter_s* sww_shooter_t; /* the shooting map: a stepper with n variational columns + the unknowns c */
 
 enum { SWW_F64 = 0, SWW_DD = 1 };
 enum {
@@ -108,6 +109,22 @@ int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, 
  * state (one setup + base state). */
 int sww_state_energy(sww_state_t s, double* energy_hl);
 int sww_state_destroy(sww_state_t s);
+
+/* ---- shooting map of the overdetermined shooting method, uniform mesh (section 3.1 / 3.3) ------------------------
+ * Unknowns c (HOST, n + 1 doubles): c[0] = T, the period (3.16); c[k], 1 <= k <= n, the Fourier modes of the initial
+ * state (3.15): eta(x, 0) = sum_{k even} 2 c_k cos kx, phi(x, 0) = sum_{k odd} 2 c_k cos kx (eta about the mean level).
+ * sww_shoot builds that state and the columns dq0/dc_k on the device, advances (q, Qdot) together by nsteps RK8 steps of size
+ * T / (4 nsteps) (3.32; one setup + one batched linearized solve per stage) and returns
+ *     r_i  = phi(alpha_i, T/4) / sqrt(N)                                                  (3.17; f = r.r / 2)
+ *     J_ik = dr_i/dc_k: k >= 1 the variational solution phidot_k(alpha_i, T/4) / sqrt(N), k = 0 phi_t(alpha_i, T/4) / (4 sqrt(N))
+ *                                                                                         (3.31; R13)
+ * r: DEVICE, N; J: DEVICE, N x (n + 1) column-major; eta_T4, phi_T4 (optional, DEVICE, N): the state at T/4.  SWW_DD: every
+ * output is double-double planar (hi block, lo block); c stays fp64.  Limits: those of sww_state_create, and 2 n < N.
+ * The handle keeps the stepper and its DtN between calls (a Levenberg-Marquardt iteration calls sww_shoot repeatedly, App. C);
+ * flags as in sww_state_create.  sww_shoot synchronises and returns the sticky status. */
+int sww_shooter_create(int N, int n, double h, double g, int prec, unsigned flags, void* stream, sww_shooter_t* out);
+int sww_shoot(sww_shooter_t S, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4);
+int sww_shooter_destroy(sww_shooter_t S);
 
 /* ---- diagnostics ---------------------------------------------------------------------------------------------- */
 const char* sww_strerror(int status);

@@ -10,12 +10,15 @@ for who may import it).  Plain restatement of PAPER.md section 3.1 / 3.3 on the 
                             weight (the paper prints the k = 0 row without the 1/4 of the chain rule: reading R13 of DESIGN.md;
                             tests/test_oracle_pins.py checks the row against finite differences (3.33))
 The time integration is Oracle.rk_advance with nsteps steps of size T / (4 nsteps); phi_t at T/4 is Oracle.rhs of the final state.
+shoot_quad is the same map with the initial state and the final scaling carried to ~40 digits (mpmath) as (hi, lo) fp64 pairs, for the
+__float128 build of the oracle (the double-double instance of the path); pinned against shoot in tests/test_oracle_pins.py.
 """
 from __future__ import annotations
 
 import numpy as np
 
 LD = np.longdouble
+LD_PI = LD("3.14159265358979323846264338327950288")   # pi to the precision of long double (np.pi is its fp64 rounding)
 
 
 def _split(x):
@@ -31,7 +34,7 @@ def initial_state(c, N: int):
     eta, phi = np.zeros(N, dtype=LD), np.zeros(N, dtype=LD)
     deta, dphi = np.zeros((n, N), dtype=LD), np.zeros((n, N), dtype=LD)
     for k in range(1, n + 1):
-        col = 2 * np.cos(2 * LD(np.pi) * ((k * j) % N).astype(LD) / N)   # 2 cos(k alpha_j), phase reduced exactly
+        col = 2 * np.cos(2 * LD_PI * ((k * j) % N).astype(LD) / N)   # 2 cos(k alpha_j), phase reduced exactly
         if k % 2 == 0:
             eta += LD(c[k]) * col
             deta[k - 1] = col
@@ -57,3 +60,47 @@ def shoot(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True):
     J[:, 0] = phi_t * w / 4
     J[:, 1:] = dphi.T * w
     return {"r": phi * w, "J": J, "eta": eta, "phi": phi}
+
+
+def _mp_split(x):
+    hi = float(x)
+    return hi, float(x - hi)
+
+
+def initial_state_quad(c, N: int):
+    """(3.15) to ~40 digits: -> (eta, phi, deta, dphi), each a pair (hi, lo) of float64 arrays"""
+    import mpmath as mp
+    c = np.asarray(c, dtype=np.float64)
+    n = c.shape[0] - 1
+    with mp.workprec(160):
+        col = [[2 * mp.cos(2 * mp.pi * ((k * j) % N) / N) for j in range(N)] for k in range(n + 1)]
+        eta = [sum((mp.mpf(float(c[k])) * col[k][j] for k in range(2, n + 1, 2)), mp.mpf(0)) for j in range(N)]
+        phi = [sum((mp.mpf(float(c[k])) * col[k][j] for k in range(1, n + 1, 2)), mp.mpf(0)) for j in range(N)]
+        pair = lambda v: tuple(np.array(t, dtype=np.float64) for t in zip(*[_mp_split(x) for x in v]))
+        zero = [mp.mpf(0)] * N
+        deta = [pair(col[k] if k % 2 == 0 else zero) for k in range(1, n + 1)]
+        dphi = [pair(col[k] if k % 2 == 1 else zero) for k in range(1, n + 1)]
+        stack = lambda ps: (np.stack([p[0] for p in ps]), np.stack([p[1] for p in ps]))
+        return pair(eta), pair(phi), stack(deta), stack(dphi)
+
+
+def shoot_quad(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True):
+    """shoot() for the __float128 oracle: -> dict r (hi, lo), J (hi, lo) with J[.] of shape (N, n + 1)"""
+    import mpmath as mp
+    c = np.asarray(c, dtype=np.float64)
+    n = c.shape[0] - 1
+    T = float(c[0])
+    eta0, phi0, deta0, dphi0 = initial_state_quad(c, N)
+    out = orc.rk_advance(eta0, phi0, h, g, T / (4 * nsteps), nsteps, deta=deta0, dphi=dphi0, filter=filter)
+    phi_t = orc.rhs(out["eta"], out["phi"], h, g, filter=filter)["phi_t"]
+    with mp.workprec(160):
+        w = 1 / mp.sqrt(mp.mpf(N))
+        val = lambda p, i: mp.mpf(float(p[0][i])) + mp.mpf(float(p[1][i]))
+        r = [val(out["phi"], i) * w for i in range(N)]
+        Jc = [[val(phi_t, i) * w / 4 for i in range(N)]]
+        for k in range(n):
+            Jc.append([(mp.mpf(float(out["dphi"][0][k][i])) + mp.mpf(float(out["dphi"][1][k][i]))) * w for i in range(N)])
+        sp = lambda v: tuple(np.array(t, dtype=np.float64) for t in zip(*[_mp_split(x) for x in v]))
+        rr = sp(r)
+        Js = [sp(col) for col in Jc]
+        return {"r": rr, "J": (np.stack([j[0] for j in Js], axis=1), np.stack([j[1] for j in Js], axis=1))}

@@ -4,8 +4,8 @@ Thin Python binding over the C ABI of include/sww.h (libsww.so, hand-written CUD
 arguments: torch supplies device memory and streams, every step of the path runs in the library's kernels.  There is no CPU
 fallback: importing works without a GPU (so the build and symbol checks can run), any compute call without CUDA raises.
 """
-from .binding import (DtN, State, SwwError, lib, lib_path, launch_count, probe_fp64_peak, dtn_linearized_host, host_cache_clear, F64, DD,
+from .binding import (DtN, State, Shooter, SwwError, lib, lib_path, launch_count, probe_fp64_peak, dtn_linearized_host, host_cache_clear, F64, DD,
                       dd_pack, dd_unpack, EXPORTS, timing_enable, timing_read, KERNEL_CLASSES)
 
-__all__ = ["DtN", "State", "SwwError", "lib", "lib_path", "launch_count", "probe_fp64_peak", "dtn_linearized_host", "host_cache_clear", "F64", "DD",
+__all__ = ["DtN", "State", "Shooter", "SwwError", "lib", "lib_path", "launch_count", "probe_fp64_peak", "dtn_linearized_host", "host_cache_clear", "F64", "DD",
            "dd_pack", "dd_unpack", "EXPORTS", "timing_enable", "timing_read", "KERNEL_CLASSES"]

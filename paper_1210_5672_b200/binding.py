@@ -17,6 +17,7 @@ EXPORTS = [
     "sww_dtn_status", "sww_dtn_destroy", "sww_state_create", "sww_rk_advance", "sww_state_read", "sww_state_energy",
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
+    "sww_shooter_create", "sww_shoot", "sww_shooter_destroy",
 ]
 
 
@@ -61,6 +62,9 @@ def lib() -> ctypes.CDLL:
         L.sww_launch_count.restype = ctypes.c_ulonglong
         L.sww_probe_fp64_peak.argtypes = [ci, ctypes.POINTER(cd)]
         L.sww_dtn_linearized_host.argtypes = [vp, vp, vp, vp, vp, ci, cd, ci, ci]
+        L.sww_shooter_create.argtypes = [ci, ci, cd, cd, ci, ctypes.c_uint, vp, ctypes.POINTER(vp)]
+        L.sww_shoot.argtypes = [vp, ctypes.POINTER(cd), ci, vp, vp, vp, vp]
+        L.sww_shooter_destroy.argtypes = [vp]
         L.sww_timing_enable.argtypes = [ci]
         L.sww_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_ulonglong), ci]
         _LIB = L
@@ -240,6 +244,44 @@ class State:
     def close(self):
         if getattr(self, "_h", None):
             lib().sww_state_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Shooter:
+    """The shooting map (3.15)-(3.17), (3.31): sww_shooter_create / sww_shoot.  c: n + 1 unknowns (c[0] = T)."""
+
+    def __init__(self, N: int, n: int, h: float, g: float = 1.0, prec: int = F64, filter: bool = True,
+                 stream: torch.cuda.Stream | None = None):
+        _require_cuda()
+        self.N, self.n, self.prec = int(N), int(n), prec
+        self._stream = stream if stream is not None else torch.cuda.current_stream()
+        h_ = ctypes.c_void_p()
+        _check(lib().sww_shooter_create(self.N, self.n, float(h), float(g), prec, 0 if filter else 1, self._stream.cuda_stream,
+                                        ctypes.byref(h_)), "sww_shooter_create")
+        self._h = h_
+
+    def shoot(self, c, nsteps: int, want_state: bool = False):
+        """-> r (N), J (n + 1, N) [= column-major N x (n + 1)]; double-double: leading axis 2 (hi, lo)"""
+        N, n = self.N, self.n
+        cc = (ctypes.c_double * (n + 1))(*[float(x) for x in c])
+        lead = (2,) if self.prec == DD else ()
+        r = torch.empty(lead + (N,), dtype=torch.float64, device="cuda")
+        J = torch.empty(lead + (n + 1, N), dtype=torch.float64, device="cuda")
+        eta = torch.empty(lead + (N,), dtype=torch.float64, device="cuda") if want_state else None
+        phi = torch.empty_like(eta) if want_state else None
+        _check(lib().sww_shoot(self._h, cc, int(nsteps), r.data_ptr(), J.data_ptr(), eta.data_ptr() if want_state else None,
+                               phi.data_ptr() if want_state else None), "sww_shoot")
+        return (r, J, eta, phi) if want_state else (r, J)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().sww_shooter_destroy(self._h)
             self._h = None
 
     def __del__(self):

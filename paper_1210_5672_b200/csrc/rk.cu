@@ -16,25 +16,7 @@
 
 using namespace sww;
 
-constexpr int RK_S = 11;
-
-struct sww_state_s {
-    int N, nc, prec;
-    double h, g;
-    bool filter;
-    cudaStream_t stream;
-    sww_dtn_t dtn;
-    size_t L;            // 2 N (1 + nc)
-    double* y;           // state
-    double* ys;          // stage state
-    double* k;           // RK_S stage derivatives, L each
-    double* w;           // N x nc: unfiltered deta_t of the current stage
-    double* red;         // 2 doubles: energy reduction (hi, lo)
-    double t;
-    double a[RK_S][RK_S], b[RK_S], c[RK_S];
-    double alo[RK_S][RK_S], blo[RK_S];  // low words of the tableau (double-double states)
-    size_t mul() const { return prec == SWW_DD ? 2 : 1; }
-};
+#include "rk.cuh"
 
 namespace sww {
 
@@ -318,7 +300,7 @@ static int rk_rhs_dd(sww_state_s* s, const double* ys, double* kout) {
     return SWW_OK;
 }
 
-static int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
+int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
     if (s->prec == SWW_DD) return rk_rhs_dd(s, ys, kout);
     const int N = s->N, nc = s->nc, logN = fft_ilog2(N), thr = fft_threads(N);
     sww_dtn_s* d = s->dtn;

@@ -1,0 +1,28 @@
+// rk.cuh -- the time-stepper state shared by rk.cu (S8, S9) and shoot.cu (the shooting map).  Product code; shares nothing with oracle/.
+#pragma once
+#include "common.cuh"
+
+constexpr int RK_S = 11;
+
+struct sww_state_s {
+    int N, nc, prec;
+    double h, g;
+    bool filter;
+    cudaStream_t stream;
+    sww_dtn_t dtn;
+    size_t L;            // 2 N (1 + nc)
+    double* y;           // state
+    double* ys;          // stage state
+    double* k;           // RK_S stage derivatives, L each
+    double* w;           // N x nc: unfiltered deta_t of the current stage
+    double* red;         // 2 doubles: energy reduction (hi, lo)
+    double t;
+    double a[RK_S][RK_S], b[RK_S], c[RK_S];
+    double alo[RK_S][RK_S], blo[RK_S];  // low words of the tableau (double-double states)
+    size_t mul() const { return prec == SWW_DD ? 2 : 1; }
+};
+
+namespace sww {
+// one evaluation of the right-hand sides (2.1), (B.1)-(B.3) at the stage state ys -> kout (same layout as the state)   (rk.cu)
+int rk_rhs(sww_state_s* s, const double* ys, double* kout);
+}  // namespace sww

@@ -1,0 +1,109 @@
+"""GPU parity tests of the shooting map (sww_shooter_create / sww_shoot): residual (3.17) and Jacobian (3.31) of the overdetermined
+shooting method against the oracle (oracle/shooting.py), per column as in DESIGN.md section 6, and the
+small-amplitude branch the paper prints (T = 7.19976) recovered through the device path."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+from parity_util import ld
+
+pytestmark = pytest.mark.gpu
+LD = np.longdouble
+
+
+@pytest.fixture(scope="module")
+def sww():
+    import paper_1210_5672_b200 as pkg
+    assert pkg.lib_path().exists() and torch.cuda.is_available()
+    return pkg
+
+
+def unknowns(n, T=7.0, amp=-0.02, seed=3):
+    """c_0 = T off the linear period, c_1 the carrier, the other modes decaying like the paper's small-amplitude waves"""
+    rng = np.random.default_rng(seed)
+    c = np.zeros(n + 1)
+    c[0] = T
+    c[1] = amp
+    for k in range(2, n + 1):
+        c[k] = 0.2 * abs(amp) * rng.standard_normal() * np.exp(-0.7 * k)
+    return c
+
+
+def col_err(gpu, ref):
+    """per column: max |gpu - ref| / max |ref| (columns along axis 0 of both arrays)"""
+    return np.abs(gpu.astype(LD) - ref).max(axis=1) / np.abs(ref).max(axis=1)
+
+
+@pytest.mark.parametrize("N,n,nsteps", [(64, 6, 6), (128, 9, 5), (256, 12, 4)])
+def test_residual_and_jacobian_fp64(sww, orc_ld, N, n, nsteps):
+    from oracle import shooting
+    c = unknowns(n)
+    S = sww.Shooter(N, n, 1.0, 1.0)
+    r, J, eta, phi = S.shoot(c, nsteps, want_state=True)
+    o = shooting.shoot(orc_ld, c, N, 1.0, 1.0, nsteps)
+    assert float(np.abs(r.cpu().numpy().astype(LD) - o["r"]).max() / np.abs(o["r"]).max()) <= 1e-11
+    e = col_err(J.cpu().numpy(), o["J"].T)
+    assert float(e.max()) <= 1e-11, e
+    assert float(np.abs(eta.cpu().numpy().astype(LD) - o["eta"]).max() / np.abs(o["eta"]).max()) <= 1e-11
+    assert float(np.abs(phi.cpu().numpy().astype(LD) - o["phi"]).max() / np.abs(o["phi"]).max()) <= 1e-11
+    # a second shot through the same handle (what a Levenberg-Marquardt iteration does): same bits for the same c, and a
+    # changed period changes the result
+    r2, J2 = S.shoot(c, nsteps)
+    assert torch.equal(r, r2) and torch.equal(J, J2)
+    c2 = c.copy()
+    c2[0] += 0.1
+    r3, _ = S.shoot(c2, nsteps)
+    assert not torch.equal(r, r3)
+    S.close()
+
+
+def test_residual_and_jacobian_dd(sww, orc_q):
+    from oracle import shooting
+    N, n, nsteps = 64, 5, 3
+    c = unknowns(n)
+    S = sww.Shooter(N, n, 1.0, 1.0, prec=sww.DD)
+    r, J = S.shoot(c, nsteps)
+    o = shooting.shoot_quad(orc_q, c, N, 1.0, 1.0, nsteps)
+    rg = r.cpu().numpy()
+    dr = (rg[0].astype(LD) - o["r"][0].astype(LD)) + (rg[1].astype(LD) - o["r"][1].astype(LD))
+    assert float(np.abs(dr).max() / np.abs(o["r"][0]).max()) <= 1e-25
+    Jg = J.cpu().numpy()                                     # (2, n + 1, N)
+    dJ = (Jg[0].astype(LD) - o["J"][0].T.astype(LD)) + (Jg[1].astype(LD) - o["J"][1].T.astype(LD))
+    e = np.abs(dJ).max(axis=1) / np.abs(o["J"][0].T).max(axis=1)
+    assert float(e.max()) <= 1e-25, e
+    S.close()
+
+
+def test_gauss_newton_on_the_period_finds_the_linear_period(sww):
+    """the small-amplitude branch: Gauss-Newton on c_0 = T alone with the device residual and Jacobian column 0 converges to
+    T = 2 pi / sqrt(tanh 1) = 7.19976; f = r.r / 2 falls to roundoff"""
+    golden = {}
+    from pathlib import Path
+    for line in (Path(__file__).parent / "golden" / "paper_values.txt").read_text().splitlines():
+        if line.strip() and not line.startswith("#"):
+            k, v, tol = line.split()[:3]
+            golden[k] = (float(v), float(tol))
+    N, n, nsteps, eps = 64, 1, 16, 1e-6
+    S = sww.Shooter(N, n, 1.0, 1.0)
+    T = 7.0
+    for _ in range(6):
+        r, J = S.shoot([T, eps], nsteps)
+        J0 = J[0]
+        T -= float((J0 @ r) / (J0 @ J0))
+    want, tol = golden["T_linear_h1"]
+    assert abs(T - want) < tol
+    assert float(0.5 * (r @ r)) < 1e-22
+    S.close()
+
+
+def test_argument_checks(sww):
+    with pytest.raises(sww.SwwError):
+        sww.Shooter(64, 32, 1.0)          # 2 n < N
+    S = sww.Shooter(64, 2, 1.0)
+    with pytest.raises(sww.SwwError):
+        S.shoot([0.0, 0.1, 0.0], 4)       # the period must be positive
+    with pytest.raises(sww.SwwError):
+        S.shoot([7.0, 0.1, 0.0], 0)
+    S.close()

@@ -614,3 +614,26 @@ def test_shooting_recovers_the_linear_period(orc_ld):
     want, tol = golden()["T_linear_h1"]
     assert abs(T - want) < tol
     assert float(0.5 * (s["r"] @ s["r"])) < 1e-22
+
+
+def test_shooting_quad_matches_long_double(orc_ld, orc_q):
+    """shoot_quad (initial state and scaling to ~40 digits, __float128 stepping) against shoot (long double): the two builds of the
+    same map agree to long-double accuracy; the quad initial state against its defining sum (3.15) with mpmath at one node"""
+    import mpmath as mp
+    from oracle import shooting
+    c = np.array([7.0, -0.01, 0.003, 0.001, -0.0005])
+    N = 32
+    a = shooting.shoot(orc_ld, c, N, 1.0, 1.0, 4)
+    b = shooting.shoot_quad(orc_q, c, N, 1.0, 1.0, 4)
+    assert np.abs(ld(b["r"]) - a["r"]).max() < 5e-18
+    assert np.abs(ld(b["J"]) - a["J"]).max() < 5e-18
+    eq, pq, deq, dpq = shooting.initial_state_quad(c, N)
+    with mp.workprec(200):
+        j = 5
+        x = 2 * mp.pi * j / N
+        eta = sum(2 * mp.mpf(float(c[k])) * mp.cos(k * x) for k in (2, 4))
+        phi = sum(2 * mp.mpf(float(c[k])) * mp.cos(k * x) for k in (1, 3))
+        assert abs(mp.mpf(float(eq[0][j])) + mp.mpf(float(eq[1][j])) - eta) < mp.mpf(10) ** -33
+        assert abs(mp.mpf(float(pq[0][j])) + mp.mpf(float(pq[1][j])) - phi) < mp.mpf(10) ** -33
+        assert abs(mp.mpf(float(dpq[0][2][j])) + mp.mpf(float(dpq[1][2][j])) - 2 * mp.cos(3 * x)) < mp.mpf(10) ** -31
+        assert float(deq[0][2][j]) == 0.0 and float(dpq[0][1][j]) == 0.0   # column k = 3 perturbs phi only, k = 2 eta only
