@@ -36,7 +36,7 @@ def col_err(gpu, ref):
     return np.abs(gpu.astype(LD) - ref).max(axis=1) / np.abs(ref).max(axis=1)
 
 
-@pytest.mark.parametrize("N,n,nsteps", [(64, 6, 6), (128, 9, 5), (256, 12, 4)])
+@pytest.mark.parametrize("N,n,nsteps", [(64, 6, 6), (128, 9, 5), (256, 12, 8)])   # dt inside the stability interval of the RK8 scheme (|omega_max| dt < 3)
 def test_residual_and_jacobian_fp64(sww, orc_ld, N, n, nsteps):
     from oracle import shooting
     c = unknowns(n)
