@@ -125,6 +125,31 @@ int sww_state_destroy(sww_state_t s);
 int sww_shooter_create(int N, int n, double h, double g, int prec, unsigned flags, void* stream, sww_shooter_t* out);
 int sww_shoot(sww_shooter_t S, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4);
 int sww_shooter_destroy(sww_shooter_t S);
+/* The residual alone (a stepper without variational columns inside the handle: what Levenberg-Marquardt needs for a trial step). */
+int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r);
+int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd);
+
+/* ---- Levenberg-Marquardt with delayed Jacobian updates (Appendix C) ----------------------------
+ * min f(c) = r(c).r(c) / 2 over the unknowns that are not held fixed (fixed[k] != 0 keeps c[k]: "holding c_1 constant",
+ * PAPER.md:334).  Trust-region step from the thin SVD J = U S V^T (C.3) with the O(m) Newton iteration (C.5) on the Lagrange
+ * multiplier; radius update, acceptance, roundoff regime and the rules for re-using J as in rules 1-4 of the appendix
+ * (rho_0 = 1/4, rho_1 = 0.85, alpha_0 = 3/8, alpha_1 = 1.875, alpha_2 = 0.2).  HOST algebra in fp64 (long-double sums) on an
+ * M x m matrix; every r and J comes from the callback.  sww_lm_shoot runs it on the device shooting map (M = N, unknowns c of
+ * sww_shoot; residual-only trial steps through sww_shoot_residual).  c: HOST, in/out. */
+typedef int (*sww_lm_fun)(void* ctx, const double* c, int want_J, double* r, double* J);   /* J: M x ntot column-major */
+typedef struct {
+    double f_tol, g_tol, df_tol;   /* rule 1 (the paper: 1e-26, 1e-13, 1e-5) */
+    double delta0;                 /* initial trust-region radius (<= 0: 1) */
+    double lambda_tol;             /* tolerance of (C.5) (<= 0: 1e-12) */
+    int max_stepsJ, max_iter;      /* rule 1 (the paper: 10); iteration limit (<= 0: 10, 100) */
+} sww_lm_options;
+typedef struct {
+    double f, delta;
+    int iterations, residual_evals, jacobian_evals;
+    int status;                    /* 0 iteration limit, 1 f = 0, 2 c unchanged, 3 roundoff regime ended */
+} sww_lm_report;
+int sww_lm_minimize(sww_lm_fun fun, void* ctx, int M, int ntot, double* c, const int* fixed, const sww_lm_options* opt, sww_lm_report* rep);
+int sww_lm_shoot(sww_shooter_t S, double* c, const int* fixed, int nsteps, const sww_lm_options* opt, sww_lm_report* rep);
 
 /* ---- diagnostics ---------------------------------------------------------------------------------------------- */
 const char* sww_strerror(int status);

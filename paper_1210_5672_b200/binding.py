@@ -17,8 +17,30 @@ EXPORTS = [
     "sww_dtn_status", "sww_dtn_destroy", "sww_state_create", "sww_rk_advance", "sww_state_read", "sww_state_energy",
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
-    "sww_shooter_create", "sww_shoot", "sww_shooter_destroy",
+    "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
 ]
+
+
+class LmOptions(ctypes.Structure):
+    _fields_ = [("f_tol", ctypes.c_double), ("g_tol", ctypes.c_double), ("df_tol", ctypes.c_double), ("delta0", ctypes.c_double),
+                ("lambda_tol", ctypes.c_double), ("max_stepsJ", ctypes.c_int), ("max_iter", ctypes.c_int)]
+
+
+class LmReport(ctypes.Structure):
+    _fields_ = [("f", ctypes.c_double), ("delta", ctypes.c_double), ("iterations", ctypes.c_int), ("residual_evals", ctypes.c_int),
+                ("jacobian_evals", ctypes.c_int), ("status", ctypes.c_int)]
+
+
+LM_FUN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.c_int, ctypes.POINTER(ctypes.c_double),
+                          ctypes.POINTER(ctypes.c_double))
+
+
+def _lm_options(f_tol=1e-26, g_tol=1e-13, df_tol=1e-5, delta0=1.0, lambda_tol=1e-12, max_stepsJ=10, max_iter=100):
+    return LmOptions(f_tol, g_tol, df_tol, delta0, lambda_tol, max_stepsJ, max_iter)
+
+
+def _lm_report(rep: LmReport) -> dict:
+    return {k: getattr(rep, k) for k, _ in LmReport._fields_}
 
 
 class SwwError(RuntimeError):
@@ -65,6 +87,10 @@ def lib() -> ctypes.CDLL:
         L.sww_shooter_create.argtypes = [ci, ci, cd, cd, ci, ctypes.c_uint, vp, ctypes.POINTER(vp)]
         L.sww_shoot.argtypes = [vp, ctypes.POINTER(cd), ci, vp, vp, vp, vp]
         L.sww_shooter_destroy.argtypes = [vp]
+        L.sww_shoot_residual.argtypes = [vp, ctypes.POINTER(cd), ci, vp]
+        L.sww_shooter_dims.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
+        L.sww_lm_minimize.argtypes = [LM_FUN, vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(LmOptions), ctypes.POINTER(LmReport)]
+        L.sww_lm_shoot.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ci), ci, ctypes.POINTER(LmOptions), ctypes.POINTER(LmReport)]
         L.sww_timing_enable.argtypes = [ci]
         L.sww_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_ulonglong), ci]
         _LIB = L
@@ -279,6 +305,22 @@ class Shooter:
                                phi.data_ptr() if want_state else None), "sww_shoot")
         return (r, J, eta, phi) if want_state else (r, J)
 
+    def residual(self, c, nsteps: int):
+        cc = (ctypes.c_double * (self.n + 1))(*[float(x) for x in c])
+        lead = (2,) if self.prec == DD else ()
+        r = torch.empty(lead + (self.N,), dtype=torch.float64, device="cuda")
+        _check(lib().sww_shoot_residual(self._h, cc, int(nsteps), r.data_ptr()), "sww_shoot_residual")
+        return r
+
+    def solve(self, c, nsteps: int, fixed=None, **opts):
+        """Levenberg-Marquardt with delayed Jacobian updates (Appendix C) on the shooting map: -> (c, report)"""
+        n1 = self.n + 1
+        cc = (ctypes.c_double * n1)(*[float(x) for x in c])
+        fx = (ctypes.c_int * n1)(*([0] * n1 if fixed is None else [int(bool(x)) for x in fixed]))
+        opt, rep = _lm_options(**opts), LmReport()
+        _check(lib().sww_lm_shoot(self._h, cc, fx, int(nsteps), ctypes.byref(opt), ctypes.byref(rep)), "sww_lm_shoot")
+        return list(cc), _lm_report(rep)
+
     def close(self):
         if getattr(self, "_h", None):
             lib().sww_shooter_destroy(self._h)
@@ -289,6 +331,29 @@ class Shooter:
             self.close()
         except Exception:
             pass
+
+
+def lm_minimize(fun, c0, M: int, fixed=None, **opts):
+    """sww_lm_minimize on a Python callback fun(c (numpy, ntot), want_J) -> (r (M), J (M x ntot) or None).  Host-only: needs no GPU."""
+    import numpy as np
+    ntot = len(c0)
+    cc = (ctypes.c_double * ntot)(*[float(x) for x in c0])
+    fx = (ctypes.c_int * ntot)(*([0] * ntot if fixed is None else [int(bool(x)) for x in fixed]))
+
+    def cb(_ctx, cp, want_J, rp, Jp):
+        try:
+            c = np.ctypeslib.as_array(cp, shape=(ntot,)).copy()
+            r, J = fun(c, bool(want_J))
+            np.ctypeslib.as_array(rp, shape=(M,))[:] = np.asarray(r, dtype=np.float64)
+            if want_J:
+                np.ctypeslib.as_array(Jp, shape=(ntot, M))[:] = np.asarray(J, dtype=np.float64).T   # column-major M x ntot
+            return 0
+        except Exception:
+            return -1
+
+    opt, rep = _lm_options(**opts), LmReport()
+    _check(lib().sww_lm_minimize(LM_FUN(cb), None, int(M), ntot, cc, fx, ctypes.byref(opt), ctypes.byref(rep)), "sww_lm_minimize")
+    return np.array(list(cc)), _lm_report(rep)
 
 
 def dtn_linearized_host(eta, phi0, deta, dphi, h: float, prec: int = F64, out=None):

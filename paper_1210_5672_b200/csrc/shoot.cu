@@ -15,7 +15,10 @@ using namespace sww;
 
 struct sww_shooter_s {
     int N, n, prec;
-    sww_state_t st;
+    double h, g;
+    unsigned flags;
+    sww_state_t st;  // the stepper with the n variational columns
+    sww_state_t st0; // the stepper without columns (residual-only shots), created at the first such shot
     double* c_dev;   // n + 1 unknowns
     double* zero;    // 2 N zeros (the flat state the stepper handle is created on)
 };
@@ -92,7 +95,7 @@ int sww_shooter_create(int N, int n, double h, double g, int prec, unsigned flag
     sww_shooter_s* S = new (std::nothrow) sww_shooter_s();
     if (!S) return SWW_ENOMEM;
     memset(S, 0, sizeof(*S));
-    S->N = N; S->n = n; S->prec = prec;
+    S->N = N; S->n = n; S->prec = prec; S->h = h; S->g = g; S->flags = flags;
     const size_t mul = prec == SWW_DD ? 2 : 1;
     const size_t nz = mul * (size_t)N * n;  // the larger of the zero arrays the create call reads (deta, dphi)
     if (cudaMalloc(&S->c_dev, sizeof(double) * (n + 1)) != cudaSuccess || cudaMalloc(&S->zero, sizeof(double) * nz) != cudaSuccess) {
@@ -114,23 +117,21 @@ int sww_shooter_create(int N, int n, double h, double g, int prec, unsigned flag
     return SWW_OK;
 }
 
-int sww_shoot(sww_shooter_t S, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4) {
-    if (!S || !c || nsteps < 1 || !r || !J) return SWW_EINVAL;
-    if (!(c[0] > 0.0)) return SWW_EINVAL;  // the period
-    sww_state_s* s = S->st;
+// one shot through the stepper s (with_cols: s carries the n variational columns and J is wanted)
+static int shoot_impl(sww_shooter_t S, sww_state_s* s, bool with_cols, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4) {
     const int N = S->N, n = S->n, isdd = S->prec == SWW_DD;
     cudaStream_t st = s->stream;
     SWW_CUDA(cudaMemcpyAsync(S->c_dev, c, sizeof(double) * (n + 1), cudaMemcpyHostToDevice, st));
     SWW_CUDA(cudaStreamSynchronize(st));  // c may be pageable host memory that the caller changes right after the call
     const Tables* tab = s->dtn->tab;
-    const dim3 blk(128), grd((N + 127) / 128, n + 1);
+    const dim3 blk(128), grd((N + 127) / 128, with_cols ? n + 1 : 1);
     SWW_BEGIN(KC_OTHER, st);
     k_shoot_init<<<grd, blk, 0, st>>>(N, n, isdd, s->L, tab->cs, S->c_dev, s->y);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     s->t = 0.0;
     SWW_TRY(sww_rk_advance(s, c[0] / (4.0 * nsteps), nsteps));
-    SWW_TRY(rk_rhs(s, s->y, s->k));  // phi_t at T/4 (stage slot 0)
+    if (with_cols) SWW_TRY(rk_rhs(s, s->y, s->k));  // phi_t at T/4 (stage slot 0)
     // w = 1/sqrt(N), N = 2^p: a power of two, times 1/sqrt(2) (double-double) when p is odd
     int p = 0;
     while ((1 << p) < N) p++;
@@ -139,7 +140,7 @@ int sww_shoot(sww_shooter_t S, const double* c, int nsteps, void* r, void* J, vo
         whi = ldexp(0.70710678118654757, -(p / 2));
         wlo = ldexp(-4.8336466567264567e-17, -(p / 2));
     }
-    const dim3 grd2((N + 127) / 128, n + 2);
+    const dim3 grd2((N + 127) / 128, with_cols ? n + 2 : 1);
     SWW_BEGIN(KC_OTHER, st);
     k_shoot_out<<<grd2, blk, 0, st>>>(N, n, isdd, s->L, whi, wlo, s->y, s->k, (double*)r, (double*)J);
     SWW_LAUNCHED();
@@ -147,9 +148,31 @@ int sww_shoot(sww_shooter_t S, const double* c, int nsteps, void* r, void* J, vo
     return sww_state_read(s, eta_T4, phi_T4, nullptr, nullptr, nullptr);  // synchronises; the sticky status of the stepper's DtN handle
 }
 
+int sww_shoot(sww_shooter_t S, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4) {
+    if (!S || !c || nsteps < 1 || !r || !J) return SWW_EINVAL;
+    if (!(c[0] > 0.0)) return SWW_EINVAL;  // the period
+    return shoot_impl(S, S->st, true, c, nsteps, r, J, eta_T4, phi_T4);
+}
+
+int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r) {
+    if (!S || !c || nsteps < 1 || !r) return SWW_EINVAL;
+    if (!(c[0] > 0.0)) return SWW_EINVAL;
+    if (!S->st0) SWW_TRY(sww_state_create(S->N, S->h, S->g, S->prec, 0, S->zero, S->zero, nullptr, nullptr, S->flags, S->st->stream, &S->st0));
+    return shoot_impl(S, S->st0, false, c, nsteps, r, nullptr, nullptr, nullptr);
+}
+
+int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd) {
+    if (!S) return SWW_EINVAL;
+    if (N) *N = S->N;
+    if (n) *n = S->n;
+    if (is_dd) *is_dd = S->prec == SWW_DD;
+    return SWW_OK;
+}
+
 int sww_shooter_destroy(sww_shooter_t S) {
     if (!S) return SWW_EINVAL;
     if (S->st) sww_state_destroy(S->st);
+    if (S->st0) sww_state_destroy(S->st0);
     cudaFree(S->c_dev);
     cudaFree(S->zero);
     delete S;

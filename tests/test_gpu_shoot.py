@@ -107,3 +107,28 @@ def test_argument_checks(sww):
     with pytest.raises(sww.SwwError):
         S.shoot([7.0, 0.1, 0.0], 0)
     S.close()
+
+
+def test_levenberg_marquardt_finds_a_standing_wave(sww, orc_ld):
+    """Section 4.1: from the linearized solution with c_1 held fixed, Levenberg-Marquardt with delayed Jacobian
+    updates (Appendix C) on the device shooting map reaches f at the roundoff floor; the ORACLE's shooting map confirms that the
+    c found is time-periodic, the period sits O(c_1^2) from the linear one, and the Jacobian was re-used"""
+    from oracle import shooting
+    N, n, nsteps, c1 = 64, 10, 24, -0.01
+    c0 = np.zeros(n + 1)
+    c0[0] = 7.19976
+    c0[1] = c1
+    fixed = [0] * (n + 1)
+    fixed[1] = 1
+    S = sww.Shooter(N, n, 1.0, 1.0)
+    r0 = S.residual(c0, nsteps)
+    f0 = float(0.5 * (r0 @ r0))
+    c, rep = S.solve(c0, nsteps, fixed=fixed, delta0=0.1, f_tol=1e-26, max_iter=60)
+    S.close()
+    assert c[1] == c1
+    assert rep["f"] < 1e-24 and rep["f"] < 1e-12 * f0, (rep, f0)
+    assert rep["residual_evals"] >= rep["jacobian_evals"]
+    assert 1e-8 < abs(c[0] - 7.19976) < 0.01          # a nonlinear correction of order c_1^2 to the period
+    assert abs(c[2]) > 1e-6 and abs(c[3]) > 1e-9     # second and third harmonics were found
+    o = shooting.shoot(orc_ld, np.array(c), N, 1.0, 1.0, nsteps)
+    assert float(0.5 * (o["r"] @ o["r"])) < 1e-24
