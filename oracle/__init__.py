@@ -142,7 +142,7 @@ class Oracle:
             return (ohi, olo), base
         return ohi, olo
 
-    def rhs(self, eta, phi, h: float, g: float = 1.0, deta=None, dphi=None, filter: bool = True):
+    def rhs(self, eta, phi, h: float, g: float = 1.0, deta=None, dphi=None, filter: bool = True, sigma: float = 0.0):
         """-> dict eta_t, phi_t, deta_t, dphi_t (each (hi, lo)), energy (hi, lo)"""
         ehi, elo = _split(eta)
         N = ehi.shape[0]
@@ -155,7 +155,7 @@ class Oracle:
             ncols = dehi.shape[0]
         L = 2 * N * (1 + ncols)
         ohi, olo, E = np.empty(L), np.empty(L), np.empty(2)
-        _check(self._f("rhs")(ctypes.c_int(N), ctypes.c_double(h), ctypes.c_double(g), ctypes.c_int(int(filter)),
+        _check(self._f("rhs")(ctypes.c_int(N), ctypes.c_double(h), ctypes.c_double(g), ctypes.c_double(sigma), ctypes.c_int(int(filter)),
                               _p(ehi), _p(elo), _p(phi_hi), _p(phi_lo), ctypes.c_int(ncols),
                               _p(dehi), _p(delo), _p(dphi_hi), _p(dphi_lo), _p(ohi), _p(olo), _p(E)), "rhs")
         cut = lambda a, o, n, shape: a[o:o + n].reshape(shape)
@@ -188,7 +188,7 @@ class Oracle:
         return yh[0], yl[0]
 
     def rk_advance(self, eta, phi, h: float, g: float, dt: float, nsteps: int, deta=None, dphi=None,
-                   filter: bool = True, want_energy: bool = False):
+                   filter: bool = True, want_energy: bool = False, sigma: float = 0.0):
         """-> dict eta, phi, deta, dphi (each (hi, lo)), energies ((hi, lo) arrays of nsteps+1) or None"""
         ehi, elo = _split(eta)
         N = ehi.shape[0]
@@ -206,7 +206,7 @@ class Oracle:
             delo = np.zeros_like(dehi) if delo is None else delo.copy()
             dphi_lo = np.zeros_like(dphi_hi) if dphi_lo is None else dphi_lo.copy()
         en = np.empty(2 * (nsteps + 1)) if want_energy else None
-        _check(self._f("rk_advance")(ctypes.c_int(N), ctypes.c_double(h), ctypes.c_double(g), ctypes.c_int(int(filter)),
+        _check(self._f("rk_advance")(ctypes.c_int(N), ctypes.c_double(h), ctypes.c_double(g), ctypes.c_double(sigma), ctypes.c_int(int(filter)),
                                      ctypes.c_double(dt), ctypes.c_int(nsteps), _p(ehi), _p(elo), _p(phi_hi), _p(phi_lo),
                                      ctypes.c_int(ncols), _p(dehi), _p(delo), _p(dphi_hi), _p(dphi_lo), _p(en)), "rk_advance")
         return {"eta": (ehi, elo), "phi": (phi_hi, phi_lo), "deta": (dehi, delo), "dphi": (dphi_hi, dphi_lo),

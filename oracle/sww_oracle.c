@@ -460,13 +460,23 @@ int NAME(dtn_linearized)(int N, double h, const double *ehi, const double *elo,
  * eta_t = W0 ; phi_t = P[ v W0 - u^2/2 - v^2/2 - g eta ]                                  (2.1)
  * deta_t = w_c - D(u deta_c)                                                              (B.2)
  * dphi_t = P[ -D(deta_c u v) - u D(b_c) + v w_c - g deta_c ], b_c = dphi_c - v deta_c      (B.1f)+(B.3)
- * each multiplied by the filter (2.14) when filter != 0 (R5).  All arrays REAL, columns at c*N. */
-static int rhs_eval(int N, REAL h, REAL g, int filter, const REAL *eta, const REAL *phi, int ncols,
+ * each multiplied by the filter (2.14) when filter != 0 (R5).  All arrays REAL, columns at c*N.
+ * Surface tension (sigma = sigma/rho of (2.1b); zero in sections 4.1-4.5, one in section 4.6):
+ *   phi_t  += P[ sigma D( eta' / sqrt(1 + eta'^2) ) ]                                      (2.1b)
+ *   dphi_t += P[ sigma D( D(deta_c) / (1 + eta'^2)^(3/2) ) ]                                (B.4) */
+static int rhs_eval(int N, REAL h, REAL g, REAL sigma, int filter, const REAL *eta, const REAL *phi, int ncols,
                     const REAL *deta, const REAL *dphi, REAL *eta_t, REAL *phi_t, REAL *deta_t, REAL *dphi_t, REAL *energy) {
     setup_t s; int rc = setup_make(&s, N, h, eta); if (rc) return rc;
     base_t bs; base_make(&s, phi, &bs);
     REAL *tmp = ralloc(N);
     for (int i = 0; i < N; i++) tmp[i] = bs.v[i] * bs.W0[i] - bs.u[i] * bs.u[i] / 2 - bs.v[i] * bs.v[i] / 2 - g * eta[i];
+    if (sigma != 0) {
+        REAL *cv = ralloc(N), *dcv = ralloc(N);
+        for (int i = 0; i < N; i++) cv[i] = s.d1[i] / R_SQRT(1 + s.d1[i] * s.d1[i]);
+        multiplier(&s.t, MUL_D, cv, dcv);
+        for (int i = 0; i < N; i++) tmp[i] += sigma * dcv[i];
+        free(cv); free(dcv);
+    }
     if (eta_t) { if (filter) multiplier(&s.t, MUL_FILTER, bs.W0, eta_t); else memcpy(eta_t, bs.W0, sizeof(REAL) * N); }
     if (phi_t) multiplier(&s.t, filter ? MUL_PFILTER : MUL_P, tmp, phi_t);
     if (energy) {   /* E = (1/2) int (phi G phi + g eta^2) dx */
@@ -488,6 +498,12 @@ static int rhs_eval(int N, REAL h, REAL g, int filter, const REAL *eta, const RE
         multiplier(&s.t, MUL_D, t1, t2);
         multiplier(&s.t, MUL_D, b, db);
         for (int i = 0; i < N; i++) r[i] = -t2[i] - bs.u[i] * db[i] + bs.v[i] * w[i] - g * de[i];
+        if (sigma != 0) {
+            multiplier(&s.t, MUL_D, de, t1);
+            for (int i = 0; i < N; i++) { REAL den = 1 + s.d1[i] * s.d1[i]; t1[i] = t1[i] / (den * R_SQRT(den)); }
+            multiplier(&s.t, MUL_D, t1, t2);
+            for (int i = 0; i < N; i++) r[i] += sigma * t2[i];
+        }
         multiplier(&s.t, filter ? MUL_PFILTER : MUL_P, r, dphi_t + (long)c * N);
         free(b); free(w); free(t1); free(t2); free(db); free(r);
     }
@@ -495,7 +511,7 @@ static int rhs_eval(int N, REAL h, REAL g, int filter, const REAL *eta, const RE
     return ORC_OK;
 }
 
-int NAME(rhs)(int N, double h, double g, int filter, const double *ehi, const double *elo, const double *phi_hi, const double *phi_lo,
+int NAME(rhs)(int N, double h, double g, double sigma, int filter, const double *ehi, const double *elo, const double *phi_hi, const double *phi_lo,
               int ncols, const double *dehi, const double *delo, const double *dphi, const double *dplo,
               double *out_hi, double *out_lo /* 2N(1+ncols): eta_t, phi_t, deta_t[ncols], dphi_t[ncols] */, double *energy_hl /* 2 */) {
     long n1 = N, nc = (long)N * ncols;
@@ -503,7 +519,7 @@ int NAME(rhs)(int N, double h, double g, int filter, const double *ehi, const do
     REAL *o = ralloc(2 * n1 + 2 * nc), E = 0;
     load_hl(eta, ehi, elo, n1); load_hl(phi, phi_hi, phi_lo, n1);
     if (ncols) { load_hl(de, dehi, delo, nc); load_hl(dp, dphi, dplo, nc); }
-    int rc = rhs_eval(N, (REAL)h, (REAL)g, filter, eta, phi, ncols, de, dp, o, o + n1, o + 2 * n1, o + 2 * n1 + nc, &E);
+    int rc = rhs_eval(N, (REAL)h, (REAL)g, (REAL)sigma, filter, eta, phi, ncols, de, dp, o, o + n1, o + 2 * n1, o + 2 * n1 + nc, &E);
     if (!rc) {
         store_hl(o, out_hi, out_lo, 2 * n1 + 2 * nc);
         if (energy_hl) store_hl(&E, energy_hl, energy_hl + 1, 1);
@@ -574,7 +590,7 @@ int NAME(rk_riccati_test)(double dt, int nsteps, double *y_hi, double *y_lo) {
 
 /* O9: advance (eta, phi, deta[ncols], dphi[ncols]) by nsteps RK8 steps of size dt, in place; (3.32) PAPER.md:301.
  * The state is filtered after every step when filter != 0 (R5).  energies (optional, nsteps+1 hi then nsteps+1 lo). */
-int NAME(rk_advance)(int N, double h, double g, int filter, double dt, int nsteps,
+int NAME(rk_advance)(int N, double h, double g, double sigma, int filter, double dt, int nsteps,
                      double *ehi, double *elo, double *phi_hi, double *phi_lo,
                      int ncols, double *dehi, double *delo, double *dphi, double *dplo, double *energies) {
     long n1 = N, nc = (long)N * ncols, L = 2 * n1 + 2 * nc;
@@ -590,7 +606,7 @@ int NAME(rk_advance)(int N, double h, double g, int filter, double dt, int nstep
         for (int i = 0; i < RK_S && !rc; i++) {
             for (long q = 0; q < L; q++) { REAL s = y[q]; for (int j = 0; j < i; j++) if (a[i][j] != 0) s += H * a[i][j] * k[(long)j * L + q]; ys[q] = s; }
             REAL E, *ki = k + (long)i * L;
-            rc = rhs_eval(N, (REAL)h, (REAL)g, filter, ys, ys + n1, ncols, ys + 2 * n1, ys + 2 * n1 + nc,
+            rc = rhs_eval(N, (REAL)h, (REAL)g, (REAL)sigma, filter, ys, ys + n1, ncols, ys + 2 * n1, ys + 2 * n1 + nc,
                           ki, ki + n1, ki + 2 * n1, ki + 2 * n1 + nc, (i == 0 && energies) ? &E : NULL);
             if (i == 0 && energies && !rc) store_hl(&E, energies + n, energies + (nsteps + 1) + n, 1);
         }
@@ -598,7 +614,7 @@ int NAME(rk_advance)(int N, double h, double g, int filter, double dt, int nstep
         if (filter) for (long col = 0; col < 2 + 2 * (long)ncols; col++) { multiplier(&t, MUL_FILTER, y + col * N, tmp); memcpy(y + col * N, tmp, sizeof(REAL) * N); }
     }
     if (!rc && energies) {
-        REAL E; rc = rhs_eval(N, (REAL)h, (REAL)g, filter, y, y + n1, 0, NULL, NULL, NULL, NULL, NULL, NULL, &E);
+        REAL E; rc = rhs_eval(N, (REAL)h, (REAL)g, (REAL)sigma, filter, y, y + n1, 0, NULL, NULL, NULL, NULL, NULL, NULL, &E);
         if (!rc) store_hl(&E, energies + nsteps, energies + (nsteps + 1) + nsteps, 1);
     }
     if (!rc) {

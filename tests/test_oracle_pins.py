@@ -637,3 +637,63 @@ def test_shooting_quad_matches_long_double(orc_ld, orc_q):
         assert abs(mp.mpf(float(pq[0][j])) + mp.mpf(float(pq[1][j])) - phi) < mp.mpf(10) ** -33
         assert abs(mp.mpf(float(dpq[0][2][j])) + mp.mpf(float(dpq[1][2][j])) - 2 * mp.cos(3 * x)) < mp.mpf(10) ** -31
         assert float(deq[0][2][j]) == 0.0 and float(dpq[0][1][j]) == 0.0   # column k = 3 perturbs phi only, k = 2 eta only
+
+
+# ------------------------------------------------------------------------------------------------ surface tension (2.1b), (B.4), (4.42)
+def test_surface_tension_is_the_curvature(orc_ld):
+    """a surface at rest (phi = 0): phi_t = P[-g eta + sigma kappa] with kappa = eta'' / (1 + eta'^2)^(3/2) in closed form
+    ((2.1b)); the difference of the sigma = 1 and sigma = 0 right-hand sides is P[kappa]"""
+    N = 64
+    x = 2 * LD("3.14159265358979323846264338327950288") * np.arange(N) / N    # the nodes to long-double accuracy
+    a, b = LD(0.05), LD(0.01)
+    eta = a * np.cos(x) + b * np.cos(3 * x)
+    e1 = -a * np.sin(x) - 3 * b * np.sin(3 * x)
+    e2 = -a * np.cos(x) - 9 * b * np.cos(3 * x)
+    kappa = e2 / (1 + e1 * e1) ** LD(1.5)
+    r1 = ld(orc_ld.rhs(split_ld(eta), np.zeros(N), 1.0, 1.0, filter=False, sigma=0.7)["phi_t"])
+    r0 = ld(orc_ld.rhs(split_ld(eta), np.zeros(N), 1.0, 1.0, filter=False)["phi_t"])
+    assert np.abs((r1 - r0) - LD(0.7) * (kappa - kappa.mean())).max() < 2e-17
+    assert np.abs(r0 + (eta - eta.mean())).max() < 1e-18          # phi_t = P[-g eta] at rest without surface tension
+
+
+def test_capillary_gravity_periods(orc_ld):
+    """(4.42): omega^2 = (g + sigma k^2) k tanh kh.  Gauss-Newton on the period alone along the small-amplitude
+    branch, infinite depth, g = sigma = 1, k = 1, converges to the printed T = 2 pi / sqrt 2 = 4.443; finite depth h = 1 to the formula"""
+    from oracle import shooting
+    N, eps, nsteps = 32, 1e-6, 16
+    for h, want, tol in ((float("inf"), golden()["T_capillary_hinf"][0], golden()["T_capillary_hinf"][1]),
+                         (1.0, 2 * math.pi / math.sqrt(2 * math.tanh(1.0)), 1e-9)):
+        T = 0.95 * want
+        for _ in range(6):
+            s = shooting.shoot(orc_ld, np.array([T, eps]), N, h, 1.0, nsteps, sigma=1.0)
+            J0, r = s["J"][:, 0], s["r"]
+            T = T - float((J0 @ r) / (J0 @ J0))
+        assert abs(T - want) < tol, (h, T, want)
+        assert float(0.5 * (s["r"] @ s["r"])) < 1e-22
+
+
+def test_linearized_surface_tension_matches_finite_differences(orc_q):
+    """the variation of the curvature term, sigma D(D(deta) / (1 + eta'^2)^(3/2)) ((B.4)), against Richardson
+    differences of the nonlinear right-hand side with sigma = 1: the gap closes spectrally with N as in the sigma = 0 test"""
+    h = 1.0
+    ce, se = np.array([0, 0.07, -0.03, 0.015, 0.0, 0.004]), np.array([0, 0.0, 0.02, 0.0, 0.0, 0.0])
+    cp, sp = np.array([0, 0.05, 0.0, 0.02]), np.array([0, 0.1, -0.03, 0.0])
+    cde, sde = np.array([[0, 0.5, 0.2, 0.0, 0.1], [0, 0, 0, 1.0, 0]]), np.array([[0, 0.0, 0.3, 0.0, 0.0], [0, 0, 0.5, 0, 0]])
+    cdp, sdp = np.array([[0, 0.1, 0.0, 0.4, 0.0], [0, 1.0, 0, 0, 0]]), np.array([[0, 0.6, 0.0, 0.0, 0.2], [0, 0, 0, 0, 0.3]])
+    gaps = []
+    for N in (32, 64, 128):
+        eta, phi0 = si.synth(N, ce, se)[0].astype(LD), si.synth(N, cp, sp)[0].astype(LD)
+        de, dp = si.synth(N, cde, sde), si.synth(N, cdp, sdp)
+        lin = orc_q.rhs(split_ld(eta), split_ld(phi0), h, 1.0, de, dp, filter=False, sigma=1.0)
+        lin0 = orc_q.rhs(split_ld(eta), split_ld(phi0), h, 1.0, de, dp, filter=False)
+        assert np.abs(ld(lin["deta_t"]) - ld(lin0["deta_t"])).max() == 0     # surface tension enters the phi equation only
+        gap = 0.0
+        for col in range(2):
+            def F(e):
+                r = orc_q.rhs(split_ld(eta + LD(e) * de[col]), split_ld(phi0 + LD(e) * dp[col]), h, 1.0, filter=False, sigma=1.0)
+                return ld(r["phi_t"])
+            fd = _richardson(F, 1e-4)
+            want = ld(lin["dphi_t"])[col]
+            gap = max(gap, float(np.abs(fd - want).max() / np.abs(want).max()))
+        gaps.append(gap)
+    assert gaps[0] < 1e-3 and gaps[1] < 1e-4 * gaps[0] and gaps[2] < 1e-3 * gaps[1] and gaps[2] < 1e-12, gaps
