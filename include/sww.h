@@ -103,6 +103,10 @@ int sww_dtn_destroy(sww_dtn_t d);
 int sww_state_create(int N, double h, double g, int prec, int ncols, const void* eta, const void* phi,
                      const void* deta, const void* dphi, unsigned flags, void* stream, sww_state_t* out);
 int sww_rk_advance(sww_state_t s, double dt, int nsteps);
+/* Surface tension sigma / rho >= 0 of (2.1b) (0 by default, 1 in section 4.6): from the next step on
+ *   phi_t  += P[ sigma D( eta' / sqrt(1 + eta'^2) ) ],   dphi_t += P[ sigma D( D(deta_c) / (1 + eta'^2)^(3/2) ) ]   (B.4)
+ * (filtered like the other terms).  With h = infinity and g = sigma = 1 the linear period is 2 pi / sqrt 2 (4.42). */
+int sww_state_set_sigma(sww_state_t s, double sigma);
 int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, double* t);
 /* E = (1/2) int (phi G phi + g eta^2) dx = (pi/N) sum_j [phi_j (G phi)_j + g eta_j^2] of the current state;
  * energy_hl: HOST, 2 doubles (hi, lo; lo = 0 for SWW_F64); synchronises.  The handle's internal DtN is re-set-up for the current
@@ -128,6 +132,7 @@ int sww_shooter_destroy(sww_shooter_t S);
 /* The residual alone (a stepper without variational columns inside the handle: what Levenberg-Marquardt needs for a trial step). */
 int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r);
 int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd);
+int sww_shooter_set_sigma(sww_shooter_t S, double sigma);   /* surface tension of every following shot (see sww_state_set_sigma) */
 
 /* ---- Levenberg-Marquardt with delayed Jacobian updates (Appendix C) ----------------------------
  * min f(c) = r(c).r(c) / 2 over the unknowns that are not held fixed (fixed[k] != 0 keeps c[k]: "holding c_1 constant",

@@ -18,6 +18,7 @@ EXPORTS = [
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
+    "sww_state_set_sigma", "sww_shooter_set_sigma",
 ]
 
 
@@ -87,6 +88,8 @@ def lib() -> ctypes.CDLL:
         L.sww_shooter_create.argtypes = [ci, ci, cd, cd, ci, ctypes.c_uint, vp, ctypes.POINTER(vp)]
         L.sww_shoot.argtypes = [vp, ctypes.POINTER(cd), ci, vp, vp, vp, vp]
         L.sww_shooter_destroy.argtypes = [vp]
+        L.sww_state_set_sigma.argtypes = [vp, cd]
+        L.sww_shooter_set_sigma.argtypes = [vp, cd]
         L.sww_shoot_residual.argtypes = [vp, ctypes.POINTER(cd), ci, vp]
         L.sww_shooter_dims.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
         L.sww_lm_minimize.argtypes = [LM_FUN, vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(LmOptions), ctypes.POINTER(LmReport)]
@@ -246,6 +249,9 @@ class State:
                                       0 if filter else 1, self._stream.cuda_stream, ctypes.byref(h_)), "sww_state_create")
         self._h = h_
 
+    def set_sigma(self, sigma: float):
+        _check(lib().sww_state_set_sigma(self._h, float(sigma)), "sww_state_set_sigma")
+
     def advance(self, dt: float, nsteps: int):
         _check(lib().sww_rk_advance(self._h, float(dt), int(nsteps)), "sww_rk_advance")
 
@@ -291,6 +297,9 @@ class Shooter:
         _check(lib().sww_shooter_create(self.N, self.n, float(h), float(g), prec, 0 if filter else 1, self._stream.cuda_stream,
                                         ctypes.byref(h_)), "sww_shooter_create")
         self._h = h_
+
+    def set_sigma(self, sigma: float):
+        _check(lib().sww_shooter_set_sigma(self._h, float(sigma)), "sww_shooter_set_sigma")
 
     def shoot(self, c, nsteps: int, want_state: bool = False):
         """-> r (N), J (n + 1, N) [= column-major N x (n + 1)]; double-double: leading axis 2 (hi, lo)"""

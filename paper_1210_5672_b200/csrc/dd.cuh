@@ -98,6 +98,12 @@ __device__ __forceinline__ dd dd_div(dd a, dd b) {
     return dd_add_d(q, q3);
 }
 __device__ __forceinline__ dd dd_div_d(dd a, double b) { return dd_div(a, dd{b, 0.0}); }
+// sqrt(a), a > 0: the fp64 root x corrected by (a - x^2) / (2 x) (Karp-Markstein), the square taken error-free
+__device__ __forceinline__ dd dd_sqrt(dd a) {
+    const double x = sqrt(a.hi);
+    const dd r = dd_sub(a, two_prod(x, x));
+    return quick_two_sum(x, r.hi / (2.0 * x));
+}
 // fp64 reciprocal of a normal, well-scaled number: MUFU seed (2^-20) + two Newton steps (within an ulp), no slow path
 // (|x| far from 0, inf, denormals)
 __device__ __forceinline__ double rcp_normal(double x) {

@@ -229,6 +229,67 @@ __global__ void __launch_bounds__(1024) k_rhs_cols(int N, int logN, const double
     }
 }
 
+// Surface tension, base state: phi_t += F P[ sigma D( eta' / sqrt(1 + eta'^2) ) ]   (2.1b); one CTA.
+// F and P are linear, so the term is added to the phi_t that k_rhs_base has already filtered and projected.
+__global__ void __launch_bounds__(1024) k_st_base(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                  int filter_on, double sigma, const double* __restrict__ d1, double* __restrict__ phi_t) {
+    extern __shared__ __align__(16) double2 z[];
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double e1 = d1[j];
+        z[j] = make_double2(e1 / sqrt(fma(e1, e1, 1.0)), 0.0);
+    }
+    __syncthreads();
+    fft_dif(z, N, tw);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber(p, N, logN) * (filter_on ? filt[dft_index(p, logN)] : 1.0) * rN;  // k = 0 at p = 0: P
+        const double2 t = z[p];
+        z[p] = make_double2(-k * t.y, k * t.x);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) phi_t[j] = fma(sigma, z[j].x, phi_t[j]);
+}
+
+// Surface tension, variational columns: dphi_t += F P[ sigma D( D(deta_c) / (1 + eta'^2)^(3/2) ) ]   (B.4), PAPER.md:718;
+// one CTA per column pair.
+__global__ void __launch_bounds__(1024) k_st_cols(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                  int filter_on, double sigma, int ncols, const double* __restrict__ d1,
+                                                  const double* __restrict__ deta, double* __restrict__ dphi_t) {
+    extern __shared__ __align__(16) double2 z[];
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const size_t o0 = (size_t)c0 * N, o1 = (size_t)c1 * N;
+    const double rN = 1.0 / (double)N;
+    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(deta[o0 + j], has1 ? deta[o1 + j] : 0.0);
+    __syncthreads();
+    fft_dif(z, N, tw);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber(p, N, logN) * rN;
+        const double2 t = z[p];
+        z[p] = make_double2(-k * t.y, k * t.x);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);  // D(deta)
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double e1 = d1[j], den = fma(e1, e1, 1.0), q = 1.0 / (den * sqrt(den));
+        z[j] = make_double2(z[j].x * q, z[j].y * q);
+    }
+    __syncthreads();
+    fft_dif(z, N, tw);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber(p, N, logN) * (filter_on ? filt[dft_index(p, logN)] : 1.0) * rN;
+        const double2 t = z[p];
+        z[p] = make_double2(-k * t.y, k * t.x);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        dphi_t[o0 + j] = fma(sigma, z[j].x, dphi_t[o0 + j]);
+        if (has1) dphi_t[o1 + j] = fma(sigma, z[j].y, dphi_t[o1 + j]);
+    }
+}
+
 // the filter (2.14) applied in place to ncols columns (the state after every step)
 __global__ void __launch_bounds__(1024) k_filter_cols(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
                                                       int ncols, double* __restrict__ y) {
@@ -277,6 +338,8 @@ static int rk_set_attrs() {
         SWW_CUDA(cudaFuncSetAttribute(k_rhs_base, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
         SWW_CUDA(cudaFuncSetAttribute(k_rhs_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 4096 * 32));
         SWW_CUDA(cudaFuncSetAttribute(k_filter_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        SWW_CUDA(cudaFuncSetAttribute(k_st_base, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        SWW_CUDA(cudaFuncSetAttribute(k_st_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
     }
     return SWW_OK;
 }
@@ -291,11 +354,13 @@ static int rk_rhs_dd(sww_state_s* s, const double* ys, double* kout) {
     SWW_TRY(accurate_base(d, ys + N, L));           // W0 = G phi, u, v of (2.9)
     d->has_base = true;
     SWW_TRY(rkdd_rhs_base(d, s->filter, s->g, L, ys, kout));
+    if (s->sigma != 0.0) SWW_TRY(rkdd_st_base(d, s->filter, s->sigma, L, kout));
     if (nc > 0) {
         const double* deta = ys + 2 * (size_t)N;
         const double* dphi = deta + (size_t)N * nc;
         SWW_TRY(dd_linearized(d, deta, dphi, nc, s->w, L, 0));   // w_c - D(u deta_c)   (B.1d), (B.2)
         SWW_TRY(rkdd_rhs_cols(d, s->filter, s->g, nc, L, ys, s->w, kout));
+        if (s->sigma != 0.0) SWW_TRY(rkdd_st_cols(d, s->filter, s->sigma, nc, L, ys, kout));
     }
     return SWW_OK;
 }
@@ -321,6 +386,12 @@ int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
                                                               kout + N);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
+    if (s->sigma != 0.0) {
+        SWW_BEGIN(KC_FFT, st);
+        k_st_base<<<1, thr, sizeof(double2) * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->sigma, d->d1, kout + N);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+    }
     if (nc > 0) {
         const double* deta = ys + 2 * (size_t)N;
         const double* dphi = deta + (size_t)N * nc;
@@ -331,6 +402,13 @@ int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
                                                                                 kout + 2 * (size_t)N + (size_t)N * nc);
         SWW_LAUNCHED();
         SWW_CUDA(cudaGetLastError());
+        if (s->sigma != 0.0) {
+            SWW_BEGIN(KC_FFT, st);
+            k_st_cols<<<(nc + 1) / 2, thr, sizeof(double2) * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->sigma, nc, d->d1, deta,
+                                                                              kout + 2 * (size_t)N + (size_t)N * nc);
+            SWW_LAUNCHED();
+            SWW_CUDA(cudaGetLastError());
+        }
     }
     return SWW_OK;
 }
@@ -409,6 +487,12 @@ int sww_state_create(int N, double h, double g, int prec, int ncols, const void*
     if (!rc && prec == SWW_DD) rc = rkdd_set_attrs();
     if (rc) { sww_state_destroy(s); return rc; }
     *out = s;
+    return SWW_OK;
+}
+
+int sww_state_set_sigma(sww_state_t s, double sigma) {
+    if (!s || !(sigma >= 0.0)) return SWW_EINVAL;
+    s->sigma = sigma;
     return SWW_OK;
 }
 

@@ -7,6 +7,7 @@ constexpr int RK_S = 11;
 struct sww_state_s {
     int N, nc, prec;
     double h, g;
+    double sigma;        // surface tension sigma / rho of (2.1b) (0: none)
     bool filter;
     cudaStream_t stream;
     sww_dtn_t dtn;

@@ -162,6 +162,72 @@ __global__ void __launch_bounds__(512) k_rhs_cols_dd(int N, int logN, const doub
     }
 }
 
+// Surface tension in double-double.  Base state: phi_t += F P[ sigma D( eta' / sqrt(1 + eta'^2) ) ]   (2.1b); one CTA.
+__global__ void __launch_bounds__(512) k_st_base_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
+                                                    const double* __restrict__ filt, int filter_on, double sigma, size_t L,
+                                                    const double* __restrict__ d1, double* __restrict__ phi_t) {
+    extern __shared__ __align__(16) unsigned char rkdd_sm[];
+    cdd* z = reinterpret_cast<cdd*>(rkdd_sm);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const dd e1 = ldp(d1, N, j);
+        z[j] = cdd{dd_div(e1, dd_sqrt(dd_add_d(dd_sqr(e1), 1.0))), dd{0.0, 0.0}};
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber_dd(p, N, logN) * rN;   // exact; 0 at p = 0: the projection P
+        dd f = dd{k, 0.0};
+        if (filter_on) f = dd_mul_d(ldp(filt, N, dft_index_dd(p, logN)), k);
+        const cdd t = z[p];
+        z[p] = cdd{dd_neg(dd_mul(f, t.im)), dd_mul(f, t.re)};
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) stp(phi_t, L, j, dd_add(ldp(phi_t, L, j), dd_mul_d(z[j].re, sigma)));
+}
+
+// Variational columns: dphi_t += F P[ sigma D( D(deta_c) / (1 + eta'^2)^(3/2) ) ]   (B.4); one CTA per column pair.
+__global__ void __launch_bounds__(512) k_st_cols_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
+                                                    const double* __restrict__ filt, int filter_on, double sigma, int ncols, size_t L,
+                                                    const double* __restrict__ d1, const double* __restrict__ deta, double* __restrict__ dphi_t) {
+    extern __shared__ __align__(16) unsigned char rkdd_sm[];
+    cdd* z = reinterpret_cast<cdd*>(rkdd_sm);
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const size_t o0 = (size_t)c0 * N, o1 = (size_t)c1 * N;
+    const double rN = 1.0 / (double)N;
+    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = cdd{ldp(deta, L, o0 + j), has1 ? ldp(deta, L, o1 + j) : dd{0.0, 0.0}};
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber_dd(p, N, logN) * rN;
+        const cdd t = z[p];
+        z[p] = cdd{dd_mul_d(t.im, -k), dd_mul_d(t.re, k)};
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);   // D(deta)
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const dd e1 = ldp(d1, N, j), den = dd_add_d(dd_sqr(e1), 1.0), q = dd_mul(den, dd_sqrt(den));
+        z[j] = cdd{dd_div(z[j].re, q), dd_div(z[j].im, q)};
+    }
+    __syncthreads();
+    fft_dif_dd(z, N, cs, sn);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber_dd(p, N, logN) * rN;
+        dd f = dd{k, 0.0};
+        if (filter_on) f = dd_mul_d(ldp(filt, N, dft_index_dd(p, logN)), k);
+        const cdd t = z[p];
+        z[p] = cdd{dd_neg(dd_mul(f, t.im)), dd_mul(f, t.re)};
+    }
+    __syncthreads();
+    ifft_dit_dd(z, N, cs, sn);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        stp(dphi_t, L, o0 + j, dd_add(ldp(dphi_t, L, o0 + j), dd_mul_d(z[j].re, sigma)));
+        if (has1) stp(dphi_t, L, o1 + j, dd_add(ldp(dphi_t, L, o1 + j), dd_mul_d(z[j].im, sigma)));
+    }
+}
+
 // the filter (2.14) applied in place to ncols columns of the state (column c at offset c N of each plane)
 __global__ void __launch_bounds__(512) k_filter_cols_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn,
                                                         const double* __restrict__ filt, int ncols, size_t L, double* __restrict__ y) {
@@ -226,6 +292,8 @@ int rkdd_set_attrs() {
         SWW_CUDA(cudaFuncSetAttribute(k_rhs_base_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 32));
         SWW_CUDA(cudaFuncSetAttribute(k_rhs_cols_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 64));
         SWW_CUDA(cudaFuncSetAttribute(k_filter_cols_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 32));
+        SWW_CUDA(cudaFuncSetAttribute(k_st_base_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 32));
+        SWW_CUDA(cudaFuncSetAttribute(k_st_cols_dd, cudaFuncAttributeMaxDynamicSharedMemorySize, RKDD_MAX_N * 32));
     }
     return SWW_OK;
 }
@@ -257,6 +325,28 @@ int rkdd_rhs_cols(sww_dtn_s* d, bool filter, double g, int nc, size_t L, const d
     k_rhs_cols_dd<<<(nc + 1) / 2, ddf_threads(N), (size_t)N * 64, d->stream>>>(N, ddf_log2(N), t->cs, t->sn, t->filt_dd, filter ? 1 : 0, g, nc, L,
                                                                                (size_t)N * nc, d->bu, d->bv, ys + od, ys + op, wout, kout + od,
                                                                                kout + op);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int rkdd_st_base(sww_dtn_s* d, bool filter, double sigma, size_t L, double* kout) {
+    const int N = d->N;
+    const Tables* t = d->tab;
+    SWW_BEGIN(KC_FFT, d->stream);
+    k_st_base_dd<<<1, ddf_threads(N), (size_t)N * 32, d->stream>>>(N, ddf_log2(N), t->cs, t->sn, t->filt_dd, filter ? 1 : 0, sigma, L, d->d1, kout + N);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+int rkdd_st_cols(sww_dtn_s* d, bool filter, double sigma, int nc, size_t L, const double* ys, double* kout) {
+    const int N = d->N;
+    const Tables* t = d->tab;
+    const size_t od = 2 * (size_t)N, op = od + (size_t)N * nc;
+    SWW_BEGIN(KC_FFT, d->stream);
+    k_st_cols_dd<<<(nc + 1) / 2, ddf_threads(N), (size_t)N * 32, d->stream>>>(N, ddf_log2(N), t->cs, t->sn, t->filt_dd, filter ? 1 : 0, sigma, nc, L,
+                                                                              d->d1, ys + od, kout + op);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

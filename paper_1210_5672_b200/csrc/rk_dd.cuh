@@ -21,6 +21,9 @@ int rkdd_combine(cudaStream_t st, size_t L, const double* y, const double* k, co
 int rkdd_rhs_base(sww_dtn_s* d, bool filter, double g, size_t L, const double* ys, double* kout);
 // deta_t, dphi_t of (B.1)-(B.3) for nc columns; wout: the linearized DtN of the columns, dd planar with plane size N nc
 int rkdd_rhs_cols(sww_dtn_s* d, bool filter, double g, int nc, size_t L, const double* ys, const double* wout, double* kout);
+// surface tension (2.1b), (B.4): the curvature term and its variation added to phi_t / dphi_t in kout (sigma != 0 only)
+int rkdd_st_base(sww_dtn_s* d, bool filter, double sigma, size_t L, double* kout);
+int rkdd_st_cols(sww_dtn_s* d, bool filter, double sigma, int nc, size_t L, const double* ys, double* kout);
 int rkdd_filter_state(sww_dtn_s* d, int ncol, size_t L, double* y);
 // E of PAPER.md:501 for the state y -> out2 (DEVICE, hi and lo); the handle's base state must belong to y
 int rkdd_energy(sww_dtn_s* d, double g, size_t L, const double* y, double* out2);

@@ -15,7 +15,7 @@ using namespace sww;
 
 struct sww_shooter_s {
     int N, n, prec;
-    double h, g;
+    double h, g, sigma;
     unsigned flags;
     sww_state_t st;  // the stepper with the n variational columns
     sww_state_t st0; // the stepper without columns (residual-only shots), created at the first such shot
@@ -158,7 +158,16 @@ int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r) {
     if (!S || !c || nsteps < 1 || !r) return SWW_EINVAL;
     if (!(c[0] > 0.0)) return SWW_EINVAL;
     if (!S->st0) SWW_TRY(sww_state_create(S->N, S->h, S->g, S->prec, 0, S->zero, S->zero, nullptr, nullptr, S->flags, S->st->stream, &S->st0));
+    S->st0->sigma = S->sigma;
     return shoot_impl(S, S->st0, false, c, nsteps, r, nullptr, nullptr, nullptr);
+}
+
+int sww_shooter_set_sigma(sww_shooter_t S, double sigma) {
+    if (!S || !(sigma >= 0.0)) return SWW_EINVAL;
+    S->sigma = sigma;
+    S->st->sigma = sigma;
+    if (S->st0) S->st0->sigma = sigma;
+    return SWW_OK;
 }
 
 int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd) {
