@@ -182,14 +182,28 @@ class Oracle:
                                          ctypes.c_int(nsteps), _p(yh), _p(yl)), "rk_linear_test")
         return yh, yl
 
+    def sdc_tables(self, s: int = 8):
+        """Radau IIa nodes c (s) and the integration matrix S (s x s), each (hi, lo)"""
+        c = (np.empty(s), np.empty(s))
+        S = (np.empty((s, s)), np.empty((s, s)))
+        _check(self._f("sdc_tables")(ctypes.c_int(s), _p(c[0]), _p(c[1]), _p(S[0]), _p(S[1])), "sdc_tables")
+        return c, S
+
+    def sdc_linear_test(self, lam: complex, dt: float, nsteps: int):
+        yh, yl = np.empty(2), np.empty(2)
+        _check(self._f("sdc_linear_test")(ctypes.c_double(lam.real), ctypes.c_double(lam.imag), ctypes.c_double(dt),
+                                          ctypes.c_int(nsteps), _p(yh), _p(yl)), "sdc_linear_test")
+        return yh, yl
+
     def rk_riccati_test(self, dt: float, nsteps: int):
         yh, yl = np.empty(1), np.empty(1)
         _check(self._f("rk_riccati_test")(ctypes.c_double(dt), ctypes.c_int(nsteps), _p(yh), _p(yl)), "rk_riccati_test")
         return yh[0], yl[0]
 
     def rk_advance(self, eta, phi, h: float, g: float, dt: float, nsteps: int, deta=None, dphi=None,
-                   filter: bool = True, want_energy: bool = False, sigma: float = 0.0):
-        """-> dict eta, phi, deta, dphi (each (hi, lo)), energies ((hi, lo) arrays of nsteps+1) or None"""
+                   filter: bool = True, want_energy: bool = False, sigma: float = 0.0, method: str = "rk8"):
+        """-> dict eta, phi, deta, dphi (each (hi, lo)), energies ((hi, lo) arrays of nsteps+1) or None.
+        method: "rk8" (the 11-stage order-8 scheme, R6) or "sdc15" (spectral deferred correction on 8 Radau IIa nodes, R15)"""
         ehi, elo = _split(eta)
         N = ehi.shape[0]
         phi_hi, phi_lo = _split(phi, (N,))
@@ -206,7 +220,7 @@ class Oracle:
             delo = np.zeros_like(dehi) if delo is None else delo.copy()
             dphi_lo = np.zeros_like(dphi_hi) if dphi_lo is None else dphi_lo.copy()
         en = np.empty(2 * (nsteps + 1)) if want_energy else None
-        _check(self._f("rk_advance")(ctypes.c_int(N), ctypes.c_double(h), ctypes.c_double(g), ctypes.c_double(sigma), ctypes.c_int(int(filter)),
+        _check(self._f({"rk8": "rk_advance", "sdc15": "sdc_advance"}[method])(ctypes.c_int(N), ctypes.c_double(h), ctypes.c_double(g), ctypes.c_double(sigma), ctypes.c_int(int(filter)),
                                      ctypes.c_double(dt), ctypes.c_int(nsteps), _p(ehi), _p(elo), _p(phi_hi), _p(phi_lo),
                                      ctypes.c_int(ncols), _p(dehi), _p(delo), _p(dphi_hi), _p(dphi_lo), _p(en)), "rk_advance")
         return {"eta": (ehi, elo), "phi": (phi_hi, phi_lo), "deta": (dehi, delo), "dphi": (dphi_hi, dphi_lo),

@@ -625,6 +625,155 @@ int NAME(rk_advance)(int N, double h, double g, double sigma, int filter, double
     return rc;
 }
 
+/* ---------- SDC15: spectral deferred correction on 8 Radau IIa nodes (reading R15 of DESIGN.md) ----------
+ * Nodes c_1 < ... < c_s = 1: the right Radau points, ((x + 1)/2 for the roots x of P_s - P_{s-1} on (-1, 1]).
+ * Integration matrix S_mj = int_0^{c_m} l_j(tau) dtau, l_j the Lagrange basis on the nodes (the coefficient matrix of the Radau IIa
+ * collocation method), by an n-point Gauss-Legendre rule with 2 n - 1 >= s - 1 on [0, c_m] (exact);
+ * b_j = S_sj.  One step y_n -> y_{n+1} of size h:
+ *   predictor  : Y_0 = y_n, Y_m = classical RK4 step from Y_{m-1} over (c_m - c_{m-1}) h      ("initial values ... via fourth order Runge-Kutta")
+ *   10 sweeps  : Y_m <- y_n + h sum_j S_mj F(Y_j), m = 1..s, all from the previous sweep     ("pure Picard corrections")
+ *   final      : y_{n+1} = y_n + h sum_j b_j F(Y_j)                                            ("the final integration step")
+ * The Picard iteration converges to the Radau IIa collocation solution (order 2 s - 1 = 15); every sweep gains one order on the
+ * RK4 predictor.  F is rhs_eval (filtered when filter != 0); the state is filtered after every step as in rk_advance. */
+#define SDC_S 8
+#define SDC_SWEEPS 10
+static REAL legendre(int n, REAL x, REAL *dp) {   /* P_n(x) and P_n'(x) by the three-term recurrence */
+    REAL p0 = 1, p1 = x;
+    if (n == 0) { if (dp) *dp = 0; return 1; }
+    for (int k = 2; k <= n; k++) { REAL p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) / k; p0 = p1; p1 = p2; }
+    if (dp) *dp = n * (x * p1 - p0) / (x * x - 1);
+    return p1;
+}
+static void sdc_tables(int s, REAL *c, REAL *S /* s x s row-major */) {
+    /* roots of f = P_s - P_{s-1} in (-1, 1): bracket by a scan, then bisection to the last bit; the root x = 1 is known */
+    int found = 0; const int scan = 4000;
+    REAL xa = -1, fa = legendre(s, xa, NULL) - legendre(s - 1, xa, NULL);
+    for (int i = 1; i < scan && found < s - 1; i++) {
+        REAL xb = -1 + (REAL)2 * i / scan, fb = legendre(s, xb, NULL) - legendre(s - 1, xb, NULL);
+        if ((fa < 0) != (fb < 0)) {
+            REAL lo = xa, hi = xb, flo = fa;
+            for (int it = 0; it < 200; it++) {
+                REAL mid = (lo + hi) / 2, fm = legendre(s, mid, NULL) - legendre(s - 1, mid, NULL);
+                if (mid == lo || mid == hi) break;
+                if ((fm < 0) == (flo < 0)) { lo = mid; flo = fm; } else hi = mid;
+            }
+            c[found++] = ((lo + hi) / 2 + 1) / 2;
+        }
+        xa = xb; fa = fb;
+    }
+    c[s - 1] = 1;
+    /* Gauss-Legendre rule with ng points on [-1, 1] (2 ng - 1 >= s - 1): nodes by Newton from the Chebyshev guesses */
+    const int ng = (s + 1) / 2 + 1;
+    REAL gx[16], gw[16];
+    for (int i = 0; i < ng; i++) {
+        REAL x = R_COS(R_PI * (i + (REAL)0.75) / (ng + (REAL)0.5)), dp;
+        for (int it = 0; it < 100; it++) { REAL p = legendre(ng, x, &dp); REAL dx = p / dp; x -= dx; if (R_FABS(dx) < (REAL)1e-40) break; }
+        legendre(ng, x, &dp);
+        gx[i] = x; gw[i] = 2 / ((1 - x * x) * dp * dp);
+    }
+    for (int m = 0; m < s; m++)
+        for (int j = 0; j < s; j++) {
+            REAL acc = 0;
+            for (int q = 0; q < ng; q++) {
+                REAL tau = c[m] * (gx[q] + 1) / 2, l = 1;
+                for (int i = 0; i < s; i++) if (i != j) l *= (tau - c[i]) / (c[j] - c[i]);
+                acc += gw[q] * l;
+            }
+            S[m * s + j] = acc * c[m] / 2;
+        }
+}
+int NAME(sdc_tables)(int s, double *c_hi, double *c_lo, double *S_hi, double *S_lo) {
+    if (s < 1 || s > 12) return ORC_EINVAL;
+    REAL c[12], S[144];
+    sdc_tables(s, c, S);
+    store_hl(c, c_hi, c_lo, s); store_hl(S, S_hi, S_lo, (long)s * s);
+    return ORC_OK;
+}
+/* the same driver on y' = lambda y (complex), for the order test: returns y(nsteps dt) */
+int NAME(sdc_linear_test)(double lr, double li, double dt, int nsteps, double *y_hi, double *y_lo) {
+    REAL c[SDC_S], S[SDC_S * SDC_S], h = (REAL)dt, Lr = (REAL)lr, Li = (REAL)li;
+    sdc_tables(SDC_S, c, S);
+    REAL yr = 1, yi = 0;
+#define LAM(ar, ai, or_, oi) do { (or_) = Lr * (ar) - Li * (ai); (oi) = Lr * (ai) + Li * (ar); } while (0)
+    for (int n = 0; n < nsteps; n++) {
+        REAL Yr[SDC_S], Yi[SDC_S], Fr[SDC_S], Fi[SDC_S], pr = yr, pi = yi;
+        for (int m = 0; m < SDC_S; m++) {   /* RK4 predictor */
+            REAL hm = (c[m] - (m ? c[m - 1] : 0)) * h, k1r, k1i, k2r, k2i, k3r, k3i, k4r, k4i;
+            LAM(pr, pi, k1r, k1i);
+            LAM(pr + hm / 2 * k1r, pi + hm / 2 * k1i, k2r, k2i);
+            LAM(pr + hm / 2 * k2r, pi + hm / 2 * k2i, k3r, k3i);
+            LAM(pr + hm * k3r, pi + hm * k3i, k4r, k4i);
+            pr += hm / 6 * (k1r + 2 * k2r + 2 * k3r + k4r); pi += hm / 6 * (k1i + 2 * k2i + 2 * k3i + k4i);
+            Yr[m] = pr; Yi[m] = pi;
+        }
+        for (int m = 0; m < SDC_S; m++) LAM(Yr[m], Yi[m], Fr[m], Fi[m]);
+        for (int sw = 0; sw < SDC_SWEEPS; sw++) {
+            for (int m = 0; m < SDC_S; m++) {
+                REAL sr = yr, si = yi;
+                for (int j = 0; j < SDC_S; j++) { sr += h * S[m * SDC_S + j] * Fr[j]; si += h * S[m * SDC_S + j] * Fi[j]; }
+                Yr[m] = sr; Yi[m] = si;
+            }
+            for (int m = 0; m < SDC_S; m++) LAM(Yr[m], Yi[m], Fr[m], Fi[m]);
+        }
+        for (int j = 0; j < SDC_S; j++) { yr += h * S[(SDC_S - 1) * SDC_S + j] * Fr[j]; yi += h * S[(SDC_S - 1) * SDC_S + j] * Fi[j]; }
+    }
+#undef LAM
+    REAL y[2] = { yr, yi };
+    store_hl(y, y_hi, y_lo, 2);
+    return ORC_OK;
+}
+/* advance (eta, phi, deta[ncols], dphi[ncols]) by nsteps SDC15 steps of size dt, in place (same arguments as rk_advance) */
+int NAME(sdc_advance)(int N, double h, double g, double sigma, int filter, double dt, int nsteps,
+                      double *ehi, double *elo, double *phi_hi, double *phi_lo,
+                      int ncols, double *dehi, double *delo, double *dphi, double *dplo, double *energies) {
+    long n1 = N, nc = (long)N * ncols, L = 2 * n1 + 2 * nc;
+    REAL c[SDC_S], S[SDC_S * SDC_S];
+    sdc_tables(SDC_S, c, S);
+    REAL *y = ralloc(L), *Y = ralloc(L * SDC_S), *F = ralloc(L * SDC_S), *k = ralloc(L * 4), *ys = ralloc(L), *tmp = ralloc(N);
+    if (!y || !Y || !F || !k || !ys) return ORC_ENOMEM;
+    load_hl(y, ehi, elo, n1); load_hl(y + n1, phi_hi, phi_lo, n1);
+    if (ncols) { load_hl(y + 2 * n1, dehi, delo, nc); load_hl(y + 2 * n1 + nc, dphi, dplo, nc); }
+    trig_t t; trig_init(&t, N);
+    REAL H = (REAL)dt; int rc = ORC_OK;
+#define EVAL(state, out, en) rhs_eval(N, (REAL)h, (REAL)g, (REAL)sigma, filter, (state), (state) + n1, ncols, (state) + 2 * n1, (state) + 2 * n1 + nc, \
+                                      (out), (out) + n1, (out) + 2 * n1, (out) + 2 * n1 + nc, (en))
+    for (int n = 0; n < nsteps && !rc; n++) {
+        REAL E;
+        for (int m = 0; m < SDC_S && !rc; m++) {   /* predictor: RK4 from node to node */
+            const REAL *prev = m ? Y + (long)(m - 1) * L : y;
+            REAL hm = (c[m] - (m ? c[m - 1] : 0)) * H, *k1 = k, *k2 = k + L, *k3 = k + 2 * L, *k4 = k + 3 * L, *Ym = Y + (long)m * L;
+            if (m == 0) { rc = EVAL(y, k1, energies ? &E : NULL); if (energies && !rc) store_hl(&E, energies + n, energies + (nsteps + 1) + n, 1); }
+            else memcpy(k1, F + (long)(m - 1) * L, sizeof(REAL) * L);
+            for (long q = 0; q < L; q++) ys[q] = prev[q] + hm / 2 * k1[q];
+            if (!rc) rc = EVAL(ys, k2, NULL);
+            for (long q = 0; q < L; q++) ys[q] = prev[q] + hm / 2 * k2[q];
+            if (!rc) rc = EVAL(ys, k3, NULL);
+            for (long q = 0; q < L; q++) ys[q] = prev[q] + hm * k3[q];
+            if (!rc) rc = EVAL(ys, k4, NULL);
+            for (long q = 0; q < L; q++) Ym[q] = prev[q] + hm / 6 * (k1[q] + 2 * k2[q] + 2 * k3[q] + k4[q]);
+            if (!rc) rc = EVAL(Ym, F + (long)m * L, NULL);
+        }
+        for (int sw = 0; sw < SDC_SWEEPS && !rc; sw++) {
+            for (int m = 0; m < SDC_S; m++)
+                for (long q = 0; q < L; q++) { REAL s = y[q]; for (int j = 0; j < SDC_S; j++) s += H * S[m * SDC_S + j] * F[(long)j * L + q]; Y[(long)m * L + q] = s; }
+            for (int m = 0; m < SDC_S && !rc; m++) rc = EVAL(Y + (long)m * L, F + (long)m * L, NULL);
+        }
+        for (long q = 0; q < L; q++) { REAL s = y[q]; for (int j = 0; j < SDC_S; j++) s += H * S[(SDC_S - 1) * SDC_S + j] * F[(long)j * L + q]; y[q] = s; }
+        if (filter) for (long col = 0; col < 2 + 2 * (long)ncols; col++) { multiplier(&t, MUL_FILTER, y + col * N, tmp); memcpy(y + col * N, tmp, sizeof(REAL) * N); }
+    }
+    if (!rc && energies) {
+        REAL E; rc = rhs_eval(N, (REAL)h, (REAL)g, (REAL)sigma, filter, y, y + n1, 0, NULL, NULL, NULL, NULL, NULL, NULL, &E);
+        if (!rc) store_hl(&E, energies + nsteps, energies + (nsteps + 1) + nsteps, 1);
+    }
+#undef EVAL
+    if (!rc) {
+        store_hl(y, ehi, elo, n1); store_hl(y + n1, phi_hi, phi_lo, n1);
+        if (ncols) { store_hl(y + 2 * n1, dehi, delo, nc); store_hl(y + 2 * n1 + nc, dphi, dplo, nc); }
+    }
+    trig_free(&t); free(y); free(Y); free(F); free(k); free(ys); free(tmp);
+    return rc;
+}
+
 int NAME(num_threads)(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

@@ -697,3 +697,61 @@ def test_linearized_surface_tension_matches_finite_differences(orc_q):
             gap = max(gap, float(np.abs(fd - want).max() / np.abs(want).max()))
         gaps.append(gap)
     assert gaps[0] < 1e-3 and gaps[1] < 1e-4 * gaps[0] and gaps[2] < 1e-3 * gaps[1] and gaps[2] < 1e-12, gaps
+
+
+# ------------------------------------------------------------------------------------------------ SDC15 (R15)
+def test_sdc_radau_tables(orc_q):
+    """8 Radau IIa nodes and their integration matrix: closed forms for s = 2, 3 (1/3, 1; (4 -+ sqrt 6)/10, 1), c_s = 1, exactness of the
+    rows of S on polynomials of degree < s, of the weights b = S[s-1] on degree <= 2 s - 2 (Radau quadrature), positive weights"""
+    import mpmath as mp
+    mp.mp.prec = 200
+    val = lambda p, *i: mp.mpf(float(p[0][i])) + mp.mpf(float(p[1][i]))
+    c2, _ = orc_q.sdc_tables(2)
+    assert abs(val(c2, 0) - mp.mpf(1) / 3) < mp.mpf(10) ** -32 and val(c2, 1) == 1
+    c3, _ = orc_q.sdc_tables(3)
+    assert abs(val(c3, 0) - (4 - mp.sqrt(6)) / 10) < mp.mpf(10) ** -32 and abs(val(c3, 1) - (4 + mp.sqrt(6)) / 10) < mp.mpf(10) ** -32
+    s = 8
+    c, S = orc_q.sdc_tables(s)
+    cc = [val(c, i) for i in range(s)]
+    SS = [[val(S, m, j) for j in range(s)] for m in range(s)]
+    assert cc[-1] == 1 and all(0 < cc[i] < cc[i + 1] for i in range(s - 1))
+    for m in range(s):
+        for k in range(s):
+            assert abs(sum(SS[m][j] * cc[j] ** k for j in range(s)) - cc[m] ** (k + 1) / (k + 1)) < mp.mpf(10) ** -31
+    for k in range(2 * s - 1):
+        assert abs(sum(SS[s - 1][j] * cc[j] ** k for j in range(s)) - mp.mpf(1) / (k + 1)) < mp.mpf(10) ** -31
+    assert all(SS[s - 1][j] > 0 for j in range(s))
+
+
+def test_sdc_is_fifteenth_order(orc_q):
+    """y' = lambda y: halving the step divides the error by 2^15 ("the method is 15th order")"""
+    import mpmath as mp
+    mp.mp.prec = 200
+    lam = complex(-0.3, 1.0)
+    errs = []
+    for dt, n in ((1.0, 2), (0.5, 4), (0.25, 8)):
+        yh, yl = orc_q.sdc_linear_test(lam, dt, n)
+        y = mp.mpc(mp.mpf(float(yh[0])) + mp.mpf(float(yl[0])), mp.mpf(float(yh[1])) + mp.mpf(float(yl[1])))
+        errs.append(float(abs(y - mp.exp(mp.mpc(lam.real, lam.imag) * 2))))
+    slopes = [math.log2(errs[i] / errs[i + 1]) for i in range(2)]
+    assert all(14.5 < s < 16.5 for s in slopes), (errs, slopes)
+
+
+def test_sdc_advance_agrees_with_rk8_and_conserves_energy(orc_ld, orc_q):
+    """the water-wave driver: SDC15 steps against RK8 with 16x smaller steps (long double), state and variational
+    columns; in __float128 the energy of PAPER.md:501 stays constant to 27+ digits ("29 in quadruple precision")"""
+    N, h, g = 32, 1.0, 1.0
+    a = si.grid(N)
+    eta0 = 0.05 * np.cos(a) + 0.01 * np.cos(2 * a)
+    phi0 = 0.02 * np.cos(a)
+    de = np.stack([np.cos(2 * a), np.zeros(N)])
+    dp = np.stack([np.zeros(N), np.cos(a)])
+    T = 0.8
+    # filter off: applied after every step it makes the result depend on the number of steps (1e-13 on this coarse grid)
+    s = orc_ld.rk_advance(eta0, phi0, h, g, T / 4, 4, deta=de, dphi=dp, method="sdc15", filter=False)
+    r = orc_ld.rk_advance(eta0, phi0, h, g, T / 256, 256, deta=de, dphi=dp, filter=False)
+    for name in ("eta", "phi", "deta", "dphi"):
+        assert np.abs(ld(s[name]) - ld(r[name])).max() < 2e-17, name
+    q = orc_q.rk_advance(eta0, phi0, h, g, T / 8, 8, method="sdc15", want_energy=True, filter=False)
+    E = q["energies"][0].astype(LD) + q["energies"][1].astype(LD)
+    assert float(np.abs(E - E[0]).max() / abs(E[0])) < 1e-27
