@@ -103,6 +103,12 @@ int sww_dtn_destroy(sww_dtn_t d);
 int sww_state_create(int N, double h, double g, int prec, int ncols, const void* eta, const void* phi,
                      const void* deta, const void* dphi, unsigned flags, void* stream, sww_state_t* out);
 int sww_rk_advance(sww_state_t s, double dt, int nsteps);
+/* The same advance by the 15th-order spectral deferred correction scheme the paper uses in quadruple precision:
+ * 8 Radau IIa nodes per step, initial values at the nodes by classical RK4 from node to node, 10 Picard sweeps
+ * Y_m <- y_n + dt sum_j S_mj F(Y_j) with the integration matrix of the nodes, then y_{n+1} = y_n + dt sum_j b_j F(Y_j)
+ * (R15; 113 right-hand sides per step, each one setup + one batched linearized solve); filter as in sww_rk_advance.
+ * Either precision; the first call allocates 22 more state vectors in the handle. */
+int sww_sdc_advance(sww_state_t s, double dt, int nsteps);
 /* Surface tension sigma / rho >= 0 of (2.1b) (0 by default, 1 in section 4.6): from the next step on
  *   phi_t  += P[ sigma D( eta' / sqrt(1 + eta'^2) ) ],   dphi_t += P[ sigma D( D(deta_c) / (1 + eta'^2)^(3/2) ) ]   (B.4)
  * (filtered like the other terms).  With h = infinity and g = sigma = 1 the linear period is 2 pi / sqrt 2 (4.42). */

@@ -18,7 +18,7 @@ EXPORTS = [
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
-    "sww_state_set_sigma", "sww_shooter_set_sigma",
+    "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance",
 ]
 
 
@@ -76,6 +76,7 @@ def lib() -> ctypes.CDLL:
         L.sww_dtn_destroy.argtypes = [vp]
         L.sww_state_create.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, ctypes.c_uint, vp, ctypes.POINTER(vp)]
         L.sww_rk_advance.argtypes = [vp, cd, ci]
+        L.sww_sdc_advance.argtypes = [vp, cd, ci]
         L.sww_state_read.argtypes = [vp, vp, vp, vp, vp, ctypes.POINTER(cd)]
         L.sww_state_energy.argtypes = [vp, ctypes.POINTER(cd)]
         L.sww_state_destroy.argtypes = [vp]
@@ -252,8 +253,12 @@ class State:
     def set_sigma(self, sigma: float):
         _check(lib().sww_state_set_sigma(self._h, float(sigma)), "sww_state_set_sigma")
 
-    def advance(self, dt: float, nsteps: int):
-        _check(lib().sww_rk_advance(self._h, float(dt), int(nsteps)), "sww_rk_advance")
+    def advance(self, dt: float, nsteps: int, method: str = "rk8"):
+        """method: "rk8" (sww_rk_advance) or "sdc15" (sww_sdc_advance, the paper's quadruple-precision stepper)"""
+        if method == "sdc15":
+            _check(lib().sww_sdc_advance(self._h, float(dt), int(nsteps)), "sww_sdc_advance")
+        else:
+            _check(lib().sww_rk_advance(self._h, float(dt), int(nsteps)), "sww_rk_advance")
 
     def read(self):
         N, nc = self.N, self.ncols

@@ -21,7 +21,7 @@ def _newer(target: Path, deps) -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> Path:
-    srcs = sorted(CSRC.glob("*.cu"))
+    srcs = sorted(CSRC.glob("*.cu")) + sorted(CSRC.glob("*.cpp"))   # .cpp: host-only code (nvcc hands it to the host compiler)
     hdrs = sorted(CSRC.glob("*.cuh")) + [HERE.parent / "include" / "sww.h"]
     OBJ.mkdir(exist_ok=True)
     jobs = []
@@ -46,7 +46,7 @@ def build(force: bool = False, verbose: bool = False) -> Path:
         print("\n".join(logs))
     objs = [OBJ / (s.stem + ".o") for s in srcs]
     if jobs or force or not _newer(LIB, objs):
-        cmd = ["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *map(str, objs), "-o", str(LIB)]
+        cmd = ["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *map(str, objs), "-lquadmath", "-o", str(LIB)]
         r = subprocess.run(cmd, capture_output=True, text=True)
         if r.returncode != 0:
             raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")

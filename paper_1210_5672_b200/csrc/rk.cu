@@ -413,7 +413,14 @@ int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
     return SWW_OK;
 }
 
+// out = base + dt sum_j coef_j kbuf[j]   (kbuf: n state vectors, slot j at j L mul)
+static int rk_combine_ex(sww_state_s* s, const double* base, const double* kbuf, const double* coef, const double* coef_lo, int n, double dt,
+                         double* out);
 static int rk_combine(sww_state_s* s, const double* coef, const double* coef_lo, int n, double dt, double* out) {
+    return rk_combine_ex(s, s->y, s->k, coef, coef_lo, n, dt, out);
+}
+static int rk_combine_ex(sww_state_s* s, const double* base, const double* kbuf, const double* coef, const double* coef_lo, int n, double dt,
+                         double* out) {
     if (s->prec == SWW_DD) {
         CombDD cd;
         cd.n = 0;
@@ -425,7 +432,7 @@ static int rk_combine(sww_state_s* s, const double* coef, const double* coef_lo,
                 cd.clo[cd.n] = v.lo;
                 cd.n++;
             }
-        return rkdd_combine(s->stream, s->L, s->y, s->k, cd, out);
+        return rkdd_combine(s->stream, s->L, base, kbuf, cd, out);
     }
     Comb cb;
     cb.n = 0;
@@ -436,7 +443,7 @@ static int rk_combine(sww_state_s* s, const double* coef, const double* coef_lo,
             cb.n++;
         }
     SWW_BEGIN(KC_OTHER, s->stream);
-    k_rk_combine<<<(unsigned)((s->L + 255) / 256), 256, 0, s->stream>>>(s->L, s->y, s->k, cb, out);
+    k_rk_combine<<<(unsigned)((s->L + 255) / 256), 256, 0, s->stream>>>(s->L, base, kbuf, cb, out);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -524,6 +531,77 @@ int sww_rk_advance(sww_state_t s, double dt, int nsteps) {
     return SWW_OK;
 }
 
+// ---- SDC15 (R15): 8 Radau IIa nodes, RK4 predictor from node to node, 10 Picard sweeps
+// Y_m <- y_n + h sum_j S_mj F(Y_j), final quadrature y_{n+1} = y_n + h sum_j b_j F(Y_j); every F is one rk_rhs (setup + batched
+// linearized DtN), 113 per step.  The tables come from sdc_tables.cpp (host, __float128) as double-double pairs; the fp64 stepper
+// uses their high words.  Work space: slots F[8], Fnew[8], K1..K4, Ya, Yb.
+constexpr int SDC_S = 8, SDC_SWEEPS = 10, SDC_SLOTS = 2 * SDC_S + 6;
+
+int sww_sdc_advance(sww_state_t s, double dt, int nsteps) {
+    if (!s || nsteps < 0) return SWW_EINVAL;
+    static double c_hi[SDC_S], c_lo[SDC_S], dc_hi[SDC_S], dc_lo[SDC_S], S_hi[SDC_S * SDC_S], S_lo[SDC_S * SDC_S];
+    static bool have = false;
+    if (!have) {
+        if (sdc_tables_host(SDC_S, c_hi, c_lo, dc_hi, dc_lo, S_hi, S_lo)) return SWW_EINVAL;
+        have = true;
+    }
+    const size_t Lm = s->L * s->mul();
+    if (!s->sdc && cudaMalloc(&s->sdc, sizeof(double) * Lm * SDC_SLOTS) != cudaSuccess) return SWW_ENOMEM;
+    double* F = s->sdc;                       // F(Y_m) of the previous sweep, m = 1..8
+    double* Fn = F + Lm * SDC_S;              // ... of the sweep being formed
+    double* K = Fn + Lm * SDC_S;              // K1..K4 of the predictor (contiguous: slots 0..3 of one combination)
+    double* Ya = K + Lm * 4;
+    double* Yb = Ya + Lm;
+    const int N = s->N, logN = fft_ilog2(N);
+    const bool isdd = s->prec == SWW_DD;
+    for (int n = 0; n < nsteps; n++) {
+        // predictor
+        const double* prev = s->y;
+        for (int m = 0; m < SDC_S; m++) {
+            double* Ym = (m & 1) ? Yb : Ya;
+            if (m == 0) SWW_TRY(rk_rhs(s, s->y, K));
+            else SWW_CUDA(cudaMemcpyAsync(K, F + Lm * (m - 1), sizeof(double) * Lm, cudaMemcpyDeviceToDevice, s->stream));
+            const hdd d = hdd{dc_hi[m], isdd ? dc_lo[m] : 0.0}, dh = h_mul_d(d, 0.5), d6 = h_div_d(d, 6.0), d3 = h_div_d(d, 3.0);
+            double ch[4], cl[4];
+            ch[0] = dh.hi; cl[0] = dh.lo;
+            SWW_TRY(rk_combine_ex(s, prev, K, ch, cl, 1, dt, s->ys));             // prev + hm/2 K1
+            SWW_TRY(rk_rhs(s, s->ys, K + Lm));
+            ch[0] = 0.0; cl[0] = 0.0; ch[1] = dh.hi; cl[1] = dh.lo;
+            SWW_TRY(rk_combine_ex(s, prev, K, ch, cl, 2, dt, s->ys));             // prev + hm/2 K2
+            SWW_TRY(rk_rhs(s, s->ys, K + 2 * Lm));
+            ch[1] = 0.0; cl[1] = 0.0; ch[2] = d.hi; cl[2] = d.lo;
+            SWW_TRY(rk_combine_ex(s, prev, K, ch, cl, 3, dt, s->ys));             // prev + hm K3
+            SWW_TRY(rk_rhs(s, s->ys, K + 3 * Lm));
+            ch[0] = d6.hi; cl[0] = d6.lo; ch[1] = d3.hi; cl[1] = d3.lo; ch[2] = d3.hi; cl[2] = d3.lo; ch[3] = d6.hi; cl[3] = d6.lo;
+            SWW_TRY(rk_combine_ex(s, prev, K, ch, cl, 4, dt, Ym));                // Y_m
+            SWW_TRY(rk_rhs(s, Ym, F + Lm * m));
+            prev = Ym;
+        }
+        // Picard sweeps
+        for (int sw = 0; sw < SDC_SWEEPS; sw++) {
+            for (int m = 0; m < SDC_S; m++) {
+                SWW_TRY(rk_combine_ex(s, s->y, F, S_hi + m * SDC_S, S_lo + m * SDC_S, SDC_S, dt, s->ys));
+                SWW_TRY(rk_rhs(s, s->ys, Fn + Lm * m));
+            }
+            double* t = F; F = Fn; Fn = t;
+        }
+        SWW_TRY(rk_combine_ex(s, s->y, F, S_hi + (SDC_S - 1) * SDC_S, S_lo + (SDC_S - 1) * SDC_S, SDC_S, dt, s->ys));
+        SWW_CUDA(cudaMemcpyAsync(s->y, s->ys, sizeof(double) * Lm, cudaMemcpyDeviceToDevice, s->stream));
+        if (s->filter && isdd) {
+            SWW_TRY(rkdd_filter_state(s->dtn, 2 + 2 * s->nc, s->L, s->y));
+        } else if (s->filter) {
+            const int ncol = 2 + 2 * s->nc;
+            SWW_BEGIN(KC_FFT, s->stream);
+            k_filter_cols<<<(ncol + 1) / 2, fft_threads(N), sizeof(double2) * (size_t)N, s->stream>>>(N, logN, s->dtn->tab->tw, s->dtn->tab->filt,
+                                                                                                       ncol, s->y);
+            SWW_LAUNCHED();
+            SWW_CUDA(cudaGetLastError());
+        }
+        s->t += dt;
+    }
+    return SWW_OK;
+}
+
 int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, double* t) {
     if (!s) return SWW_EINVAL;
     const size_t v = sizeof(double) * s->N, bsz = v * s->nc;
@@ -566,7 +644,7 @@ int sww_state_energy(sww_state_t s, double* energy_hl) {
 int sww_state_destroy(sww_state_t s) {
     if (!s) return SWW_EINVAL;
     if (s->dtn) sww_dtn_destroy(s->dtn);
-    cudaFree(s->y); cudaFree(s->ys); cudaFree(s->k); cudaFree(s->w); cudaFree(s->red);
+    cudaFree(s->y); cudaFree(s->ys); cudaFree(s->k); cudaFree(s->w); cudaFree(s->red); cudaFree(s->sdc);
     delete s;
     return SWW_OK;
 }

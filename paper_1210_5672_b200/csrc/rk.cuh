@@ -17,6 +17,7 @@ struct sww_state_s {
     double* k;           // RK_S stage derivatives, L each
     double* w;           // N x nc: unfiltered deta_t of the current stage
     double* red;         // 2 doubles: energy reduction (hi, lo)
+    double* sdc;         // SDC15 work space (SDC_SLOTS state vectors), allocated by the first sww_sdc_advance
     double t;
     double a[RK_S][RK_S], b[RK_S], c[RK_S];
     double alo[RK_S][RK_S], blo[RK_S];  // low words of the tableau (double-double states)
@@ -26,4 +27,6 @@ struct sww_state_s {
 namespace sww {
 // one evaluation of the right-hand sides (2.1), (B.1)-(B.3) at the stage state ys -> kout (same layout as the state)   (rk.cu)
 int rk_rhs(sww_state_s* s, const double* ys, double* kout);
+// Radau IIa nodes c, their spacings dc and the integration matrix S (s x s row-major) as double-double pairs   (sdc_tables.cpp, host)
+int sdc_tables_host(int s, double* c_hi, double* c_lo, double* dc_hi, double* dc_lo, double* S_hi, double* S_lo);
 }  // namespace sww
