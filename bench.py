@@ -341,14 +341,14 @@ def main():
     kernels = {k: {"ms_per_step": v[0] / kp, "launches_per_step": v[1] / kp} for k, v in tm.items() if v[1]}
     # algorithmic FLOPs per step of the two contraction kernels
     flops = {"lu": (2.0 / 3.0) * N ** 3,                    # S2: k_lu_dataflow
-             "trsm": 2.0 * N * N * nrhs,                    # S4: k_trsm_dataflow<32>, the nrhs columns
+             "trsm": 2.0 * N * N * nrhs,                    # S4: k_trsm_ws<32>, the nrhs columns
              "gemm_dmma": 2.0 * N * N * nrhs}               # S6: G product
     flops_step = sum(flops.values()) + 2.0 * N * N * 2      # + the two single-vector solves of the base state (k_trsm_dataflow<8>)
     peaks = measured_peaks()
     peak_tf = peaks["bf16_tflops"] * NOMINAL_FP64_OVER_BF16
     probe = {"dfma_tflops": sww.probe_fp64_peak(0) / 1e12, "dmma_tflops": sww.probe_fp64_peak(1) / 1e12}
-    names = {"lu": "k_lu_dataflow (block LU in one persistent launch: spine CTA with blocked Gauss-Jordan inverses of the 64x64 Schur blocks on the tensor pipe, DMMA.8x8x4 tile workers)",
-             "trsm": "k_trsm_dataflow<32> (persistent DMMA.8x8x4 multi-RHS triangular solves of the column batch, tasks handing blocks over through L2 with the data as the flag)",
+    names = {"lu": "k_lu_dataflow (block LU in one persistent launch: a two-CTA cluster as the spine, blocked Gauss-Jordan inverses of the 64x64 Schur blocks on the tensor pipe, DMMA.8x8x4 tile workers)",
+             "trsm": "k_trsm_ws<32> (persistent warp-specialized DMMA.8x8x4 multi-RHS triangular solves of the column batch: loader warps + mbarrier ring, tasks handing blocks over through L2 with the data as the flag)",
              "gemm_dmma": "k_gemm_f64 (DMMA.8x8x4): G product"}
     per_kernel = {}
     for cls in ("lu", "trsm", "gemm_dmma"):
