@@ -436,7 +436,7 @@ def test_host_buffer_entry_point(sww):
     assert np.array_equal(host.numpy(), dev[0])
     # the library caches one context between host calls: a second surface, another depth, fewer / more columns, another N
     # must each give exactly what a fresh device-side handle gives
-    for case in (si.config3(256, 8), si.config3(256, 64), si.config5(256, 16), si.config3(128, 32), c):
+    for case in (si.config3(256, 8), si.config3(256, 64), si.config5(256, 16), si.config3(128, 32), si.config3(512, 256), si.config3(512, 300), c):
         dev, _ = gpu_linearized(case)
         args = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (case.eta, case.phi0, case.deta, case.dphi)]
         out = torch.empty_like(args[3]).pin_memory()
