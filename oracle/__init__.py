@@ -169,6 +169,22 @@ class Oracle:
         }
         return res
 
+    def adjoint_rhs(self, eta, phi, h: float, g: float, eta_t, phi_t, sigma: float = 0.0):
+        """(B.6): -> dict eta_s, phi_s (each (hi, lo), shape (ncols, N)) for the adjoint vectors (eta_t, phi_t) at the state (eta, phi)"""
+        ehi, elo = _split(eta)
+        N = ehi.shape[0]
+        phi_hi, phi_lo = _split(phi, (N,))
+        ethi, etlo = _split(eta_t)
+        pthi, ptlo = _split(phi_t)
+        ncols = ethi.shape[0]
+        nc = N * ncols
+        ohi, olo = np.empty(2 * nc), np.empty(2 * nc)
+        _check(self._f("adjoint_rhs")(ctypes.c_int(N), ctypes.c_double(h), ctypes.c_double(g), ctypes.c_double(sigma), _p(ehi), _p(elo),
+                                      _p(phi_hi), _p(phi_lo), ctypes.c_int(ncols), _p(ethi), _p(etlo), _p(pthi), _p(ptlo), _p(ohi), _p(olo)),
+               "adjoint_rhs")
+        return {"eta_s": (ohi[:nc].reshape(ncols, N), olo[:nc].reshape(ncols, N)),
+                "phi_s": (ohi[nc:].reshape(ncols, N), olo[nc:].reshape(ncols, N))}
+
     def rk_tableau(self):
         a = (np.empty((11, 11)), np.empty((11, 11)))
         b = (np.empty(11), np.empty(11))

@@ -528,6 +528,54 @@ int NAME(rhs)(int N, double h, double g, double sigma, int filter, const double 
     return rc;
 }
 
+/* The adjoint system (B.6): right-hand side of q~_s = DF(q)^* q~ at the state q = (eta, phi) for ncols adjoint
+ * vectors (eta~_c, phi~_c), with u = phi_x, v = phi_y on the surface (2.9):
+ *   chi_c     = eta~_c + v P phi~_c                                                              (B.6d)
+ *   phi~_s,c  = G chi_c + D( u P phi~_c )                                                        (B.6e), G chi = chi_y - eta' chi_x
+ *   eta~_s,c  = -v G chi_c + u D eta~_c - v D(u) P phi~_c - g P phi~_c + sigma D( D(phi~_c) / (1 + eta'^2)^(3/2) )   (B.6f)
+ * (no filter: the adjoint identity <DF(q) qdot, q~> = <qdot, DF(q)^* q~> is stated for the unfiltered operators). */
+static int adjoint_eval(int N, REAL h, REAL g, REAL sigma, const REAL *eta, const REAL *phi, int ncols,
+                        const REAL *etat, const REAL *phit, REAL *eta_s, REAL *phi_s) {
+    setup_t s; int rc = setup_make(&s, N, h, eta); if (rc) return rc;
+    base_t bs; base_make(&s, phi, &bs);
+    REAL *du = ralloc(N);
+    multiplier(&s.t, MUL_D, bs.u, du);
+#pragma omp parallel for schedule(dynamic) if (ncols > 1)
+    for (int c = 0; c < ncols; c++) {
+        const REAL *et = etat + (long)c * N, *pt = phit + (long)c * N;
+        REAL *pp = ralloc(N), *chi = ralloc(N), *w = ralloc(N), *t1 = ralloc(N), *t2 = ralloc(N), *det = ralloc(N);
+        multiplier(&s.t, MUL_P, pt, pp);
+        for (int i = 0; i < N; i++) chi[i] = et[i] + bs.v[i] * pp[i];
+        dtn_one(&s, chi, w, NULL);
+        for (int i = 0; i < N; i++) t1[i] = bs.u[i] * pp[i];
+        multiplier(&s.t, MUL_D, t1, t2);
+        for (int i = 0; i < N; i++) phi_s[(long)c * N + i] = w[i] + t2[i];
+        multiplier(&s.t, MUL_D, et, det);
+        for (int i = 0; i < N; i++) eta_s[(long)c * N + i] = -bs.v[i] * w[i] + bs.u[i] * det[i] - bs.v[i] * du[i] * pp[i] - g * pp[i];
+        if (sigma != 0) {
+            multiplier(&s.t, MUL_D, pt, t1);
+            for (int i = 0; i < N; i++) { REAL den = 1 + s.d1[i] * s.d1[i]; t1[i] = t1[i] / (den * R_SQRT(den)); }
+            multiplier(&s.t, MUL_D, t1, t2);
+            for (int i = 0; i < N; i++) eta_s[(long)c * N + i] += sigma * t2[i];
+        }
+        free(pp); free(chi); free(w); free(t1); free(t2); free(det);
+    }
+    free(du); base_free(&bs); setup_free(&s);
+    return ORC_OK;
+}
+int NAME(adjoint_rhs)(int N, double h, double g, double sigma, const double *ehi, const double *elo, const double *phi_hi, const double *phi_lo,
+                      int ncols, const double *ethi, const double *etlo, const double *pthi, const double *ptlo,
+                      double *out_hi, double *out_lo /* 2 N ncols: eta~_s[ncols], phi~_s[ncols] */) {
+    long n1 = N, nc = (long)N * ncols;
+    REAL *eta = ralloc(n1), *phi = ralloc(n1), *et = ralloc(nc), *pt = ralloc(nc), *o = ralloc(2 * nc);
+    load_hl(eta, ehi, elo, n1); load_hl(phi, phi_hi, phi_lo, n1);
+    load_hl(et, ethi, etlo, nc); load_hl(pt, pthi, ptlo, nc);
+    int rc = adjoint_eval(N, (REAL)h, (REAL)g, (REAL)sigma, eta, phi, ncols, et, pt, o, o + nc);
+    if (!rc) store_hl(o, out_hi, out_lo, 2 * nc);
+    free(eta); free(phi); free(et); free(pt); free(o);
+    return rc;
+}
+
 /* ---------- R6: 11-stage, order-8 explicit Runge-Kutta tableau, coefficients in Q(sqrt 21) ---------- */
 #define RK_S 11
 static void rk_tableau(REAL a[RK_S][RK_S], REAL b[RK_S], REAL c[RK_S]) {

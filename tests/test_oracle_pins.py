@@ -755,3 +755,36 @@ def test_sdc_advance_agrees_with_rk8_and_conserves_energy(orc_ld, orc_q):
     q = orc_q.rk_advance(eta0, phi0, h, g, T / 8, 8, method="sdc15", want_energy=True, filter=False)
     E = q["energies"][0].astype(LD) + q["energies"][1].astype(LD)
     assert float(np.abs(E - E[0]).max() / abs(E[0])) < 1e-27
+
+
+# ------------------------------------------------------------------------------------------------ adjoint system (B.6)
+@pytest.mark.parametrize("sigma,h", [(0.0, 1.0), (0.6, 1.0), (0.0, float("inf"))])
+def test_adjoint_identity(orc_q, sigma, h):
+    """(B.4)-(B.6): <DF(q) qdot, q~> = <qdot, DF(q)^* q~> with <a, b> = (1/2 pi) int (eta_a eta_b + phi_a phi_b) dx, for
+    the linearized right-hand side already pinned by finite differences and random smooth qdot, q~.  Each side is O(0.1); the
+    identity is one of the CONTINUOUS operators (G is self-adjoint by Green's identity (B.5)), so the gap closes spectrally with N"""
+    gaps = []
+    for N in (32, 64, 128):
+        rng = np.random.default_rng(7)
+        def smooth(amp):
+            c, s_ = np.zeros(9), np.zeros(9)
+            c[1:] = amp * rng.standard_normal(8) * np.exp(-0.5 * np.arange(1, 9))
+            s_[1:] = amp * rng.standard_normal(8) * np.exp(-0.5 * np.arange(1, 9))
+            c[0] = 0.3 * amp * rng.standard_normal()
+            return si.synth(N, c, s_)[0].astype(LD)
+        eta, phi = smooth(0.05), smooth(0.1)
+        eta = eta - eta.mean()
+        qd = (np.stack([smooth(1.0), smooth(1.0)]), np.stack([smooth(1.0), smooth(1.0)]))      # (deta, dphi), 2 columns
+        qt = (np.stack([smooth(1.0), smooth(1.0)]), np.stack([smooth(1.0), smooth(1.0)]))      # (eta~, phi~), 2 columns
+        sp = lambda a: split_ld(a) if a.ndim == 1 else tuple(np.stack(t) for t in zip(*[split_ld(r) for r in a]))
+        lin = orc_q.rhs(sp(eta), sp(phi), h, 1.0, sp(qd[0]), sp(qd[1]), filter=False, sigma=sigma)
+        adj = orc_q.adjoint_rhs(sp(eta), sp(phi), h, 1.0, sp(qt[0]), sp(qt[1]), sigma=sigma)
+        gap = 0.0
+        for a in range(2):
+            for b in range(2):
+                lhs = (ld(lin["deta_t"])[a] * qt[0][b] + ld(lin["dphi_t"])[a] * qt[1][b]).mean()
+                rhs = (qd[0][a] * ld(adj["eta_s"])[b] + qd[1][a] * ld(adj["phi_s"])[b]).mean()
+                assert abs(lhs) > 1e-3
+                gap = max(gap, float(abs(lhs - rhs)))
+        gaps.append(gap)
+    assert gaps[0] < 1e-4 and gaps[1] < 1e-6 * gaps[0] and gaps[2] < 1e-4 * gaps[1] and gaps[2] < 1e-18, gaps
