@@ -80,6 +80,15 @@ int sww_dtn_set_base(sww_dtn_t d, const void* phi0);
  * deta, dphi, out: DEVICE, N x nrhs.  Needs sww_dtn_set_base first (else SWW_ENOBASE). */
 int sww_dtn_linearized_apply(sww_dtn_t d, const void* deta, const void* dphi, int nrhs, void* out);
 
+/* Right-hand side of the adjoint system (B.6) (it serves the adjoint continuation method) at the
+ * state the handle holds (surface set up, sww_dtn_set_base done: u = phi_x, v = phi_y on the surface), for nrhs adjoint vectors:
+ *     chi_c    = eta~_c + v P phi~_c                                                                               (B.6d)
+ *     phi_s,c  = G chi_c + D(u P phi~_c)                                                                           (B.6e)
+ *     eta_s,c  = -v G chi_c + u D eta~_c - v D(u) P phi~_c - g P phi~_c + sigma D( D(phi~_c) / (1 + eta'^2)^(3/2) )   (B.6f)
+ * (unfiltered, like the identity <DF(q) qdot, q~> = <qdot, DF(q)^* q~> it satisfies).  eta_t, phi_t, eta_s, phi_s: DEVICE, N x nrhs,
+ * four distinct buffers.  fp64 handles only (SWW_DD: SWW_EINVAL); needs sww_dtn_set_base (else SWW_ENOBASE). */
+int sww_dtn_adjoint_rhs(sww_dtn_t d, const void* eta_t, const void* phi_t, int nrhs, double g, double sigma, void* eta_s, void* phi_s);
+
 /* Read-only views for tests and diagnostics.  which: 0 = K, 1 = G (column-major N x N: entry (i,j) at i + j*N, i = target
  * alpha_i, j = source alpha_j; DD: planar hi then lo), 2 = eta' , 3 = eta'', 4 = phi0', 5 = W0, 6 = u, 7 = v (N reals each),
  * 8 = the fp64 factors of I/2 + K as lu.cu stores them (N x N doubles for either precision: L_ij = X_ij inv(S_j) below the block

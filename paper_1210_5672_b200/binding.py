@@ -18,7 +18,7 @@ EXPORTS = [
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
-    "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance",
+    "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance", "sww_dtn_adjoint_rhs",
 ]
 
 
@@ -72,6 +72,7 @@ def lib() -> ctypes.CDLL:
         L.sww_dtn_set_base.argtypes = [vp, vp]
         L.sww_dtn_linearized_apply.argtypes = [vp, vp, vp, ci, vp]
         L.sww_dtn_get.argtypes = [vp, ci, vp]
+        L.sww_dtn_adjoint_rhs.argtypes = [vp, vp, vp, ci, cd, cd, vp, vp]
         L.sww_dtn_status.argtypes = [vp]
         L.sww_dtn_destroy.argtypes = [vp]
         L.sww_state_create.argtypes = [ci, cd, cd, ci, ci, vp, vp, vp, vp, ctypes.c_uint, vp, ctypes.POINTER(vp)]
@@ -197,6 +198,15 @@ class DtN:
         _check(lib().sww_dtn_linearized_apply(self._h, _dev(deta, n, "deta"), _dev(dphi, n, "dphi"), nrhs, _dev(out, n, "out")),
                "sww_dtn_linearized_apply")
         return out
+
+    def adjoint_rhs(self, eta_t: torch.Tensor, phi_t: torch.Tensor, g: float = 1.0, sigma: float = 0.0):
+        """(B.6): -> (eta_s, phi_s) for the adjoint vectors (eta_t, phi_t), each (nrhs, N); fp64 handles, base state set"""
+        nrhs = phi_t.numel() // self.N
+        n = nrhs * self.N
+        eta_s, phi_s = torch.empty_like(eta_t), torch.empty_like(phi_t)
+        _check(lib().sww_dtn_adjoint_rhs(self._h, _dev(eta_t, n, "eta_t"), _dev(phi_t, n, "phi_t"), nrhs, float(g), float(sigma),
+                                         _dev(eta_s, n, "eta_s"), _dev(phi_s, n, "phi_s")), "sww_dtn_adjoint_rhs")
+        return eta_s, phi_s
 
     _WHICH = {"K": 0, "G": 1, "d1": 2, "d2": 3, "dphi0": 4, "W0": 5, "u": 6, "v": 7, "LU": 8}
 
