@@ -53,9 +53,8 @@ def test_adjoint_rhs_against_the_oracle(sww, orc_ld, N, nc, h, sigma):
         assert float(err.max()) <= 1e-11, (name, err)
 
 
-def test_adjoint_identity_on_the_device(sww):
-    """both sides from the library: the linearized right-hand side through a one-stage look at the stepper is not exposed, so the
-    identity is checked on its DtN part: <G'[deta, dphi], eta~> - structure aside, G itself is self-adjoint (B.5): <phi_a, G phi_b> = <G phi_a, phi_b>"""
+def test_dtn_is_self_adjoint_on_the_device(sww):
+    """Green's identity (B.5), on which the adjoint system rests: G is self-adjoint, <phi_a, G phi_b> = <G phi_a, phi_b>"""
     N = 512
     eta, phi, a, b = case(N, 4, seed=5)
     d = sww.DtN(dev(eta), 1.0)
