@@ -85,6 +85,10 @@ class Oracle:
         self.lib = _lib(prec)
         self._f = lambda name: getattr(self.lib, f"orc_{prec}_{name}")
 
+    def set_num_threads(self, n: int) -> None:
+        """OpenMP threads of the following calls of this build (small N: 1 is fastest)"""
+        self._f("set_num_threads")(ctypes.c_int(int(n)))
+
     def num_threads(self) -> int:
         return int(self._f("num_threads")())
 

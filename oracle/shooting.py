@@ -51,7 +51,13 @@ def shoot(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True, 
     T = float(c[0])
     eta0, phi0, deta0, dphi0 = initial_state(c, N)
     dt = T / (4 * nsteps)
-    out = orc.rk_advance(_split(eta0), _split(phi0), h, g, dt, nsteps, deta=_split(deta0), dphi=_split(dphi0), filter=filter, sigma=sigma)
+    nthr = orc.num_threads()
+    if N * n <= 4096:
+        orc.set_num_threads(1)   # hundreds of tiny right-hand sides: the OpenMP barriers would dominate
+    try:
+        out = orc.rk_advance(_split(eta0), _split(phi0), h, g, dt, nsteps, deta=_split(deta0), dphi=_split(dphi0), filter=filter, sigma=sigma)
+    finally:
+        orc.set_num_threads(nthr)
     ld = lambda p: p[0].astype(LD) + p[1].astype(LD)
     eta, phi, dphi = ld(out["eta"]), ld(out["phi"]), ld(out["dphi"])
     phi_t = ld(orc.rhs(out["eta"], out["phi"], h, g, filter=filter, sigma=sigma)["phi_t"])

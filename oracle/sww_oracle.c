@@ -822,6 +822,14 @@ int NAME(sdc_advance)(int N, double h, double g, double sigma, int filter, doubl
     return rc;
 }
 
+/* thread count of the following calls (no arithmetic: small problems run faster on one thread than through the OpenMP barriers) */
+void NAME(set_num_threads)(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
 int NAME(num_threads)(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();
