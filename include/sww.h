@@ -86,7 +86,7 @@ int sww_dtn_linearized_apply(sww_dtn_t d, const void* deta, const void* dphi, in
  *     phi_s,c  = G chi_c + D(u P phi~_c)                                                                           (B.6e)
  *     eta_s,c  = -v G chi_c + u D eta~_c - v D(u) P phi~_c - g P phi~_c + sigma D( D(phi~_c) / (1 + eta'^2)^(3/2) )   (B.6f)
  * (unfiltered, like the identity <DF(q) qdot, q~> = <qdot, DF(q)^* q~> it satisfies).  eta_t, phi_t, eta_s, phi_s: DEVICE, N x nrhs,
- * four distinct buffers.  fp64 handles only (SWW_DD: SWW_EINVAL); needs sww_dtn_set_base (else SWW_ENOBASE). */
+ * four distinct buffers (SWW_DD: planar hi block then lo block each, N <= 2048).  Needs sww_dtn_set_base (else SWW_ENOBASE). */
 int sww_dtn_adjoint_rhs(sww_dtn_t d, const void* eta_t, const void* phi_t, int nrhs, double g, double sigma, void* eta_s, void* phi_s);
 
 /* Read-only views for tests and diagnostics.  which: 0 = K, 1 = G (column-major N x N: entry (i,j) at i + j*N, i = target

@@ -200,9 +200,9 @@ class DtN:
         return out
 
     def adjoint_rhs(self, eta_t: torch.Tensor, phi_t: torch.Tensor, g: float = 1.0, sigma: float = 0.0):
-        """(B.6): -> (eta_s, phi_s) for the adjoint vectors (eta_t, phi_t), each (nrhs, N); fp64 handles, base state set"""
-        nrhs = phi_t.numel() // self.N
-        n = nrhs * self.N
+        """(B.6): -> (eta_s, phi_s) for the adjoint vectors (eta_t, phi_t), each (nrhs, N) (double-double: (2, nrhs, N)); base state set"""
+        nrhs = phi_t.numel() // (self.N * self.mul)
+        n = nrhs * self.N * self.mul
         eta_s, phi_s = torch.empty_like(eta_t), torch.empty_like(phi_t)
         _check(lib().sww_dtn_adjoint_rhs(self._h, _dev(eta_t, n, "eta_t"), _dev(phi_t, n, "phi_t"), nrhs, float(g), float(sigma),
                                          _dev(eta_s, n, "eta_s"), _dev(phi_s, n, "phi_s")), "sww_dtn_adjoint_rhs")
