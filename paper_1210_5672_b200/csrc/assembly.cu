@@ -12,40 +12,53 @@ namespace sww {
 
 // ------------------------------------------------------------------------------------------------ S0: D in double-double
 // out_i = sum_{m=1}^{N/2-1} dc[m] (f_{i-m} - f_{i+m}),  dc[m] = (1/2)(-1)^m cot(pi m/N)  (dc[N-m] = -dc[m]; Nyquist symbol 0).
-// One warp per output node; N dd multiply-adds per node.  in/out: dd planar 2N.
+// Four warps per output node (a CTA of 8 warps serves two nodes): N dd multiply-adds per node, a quarter of them per warp -- the
+// kernel is a chain of dependent dd operations behind scattered loads, so its time is the length of the per-lane chain.
+// in/out: dd planar 2N.
 __global__ void __launch_bounds__(256) k_deriv_dd(int N, const double* __restrict__ dc, const double* __restrict__ f, double* __restrict__ out) {
-    int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (warp >= N) return;
-    int i = warp, mask = N - 1;
+    __shared__ double part[2][4][2];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, node = warp >> 2, q = warp & 3;
+    const int i = blockIdx.x * 2 + node, mask = N - 1;
+    const int l128 = q * 32 + lane;  // position among the 128 lanes that share the node
     dd acc4[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};  // independent chains: a dd multiply-add is ~30 dependent instructions
-    const bool full = ((N / 2) % 128) == 0;  // dc[N/2] = 0: the last group may run over it unguarded, loads issued together
-    for (int m0 = 1 + lane; m0 < N / 2; m0 += 128) {
-        if (full) {
-            dd c[4], a[4], b[4];
+    if (i < N) {
+        const bool full = ((N / 2) % 512) == 0;  // dc[N/2] = 0: the last group may run over it unguarded, loads issued together
+        for (int m0 = 1 + l128; m0 < N / 2; m0 += 512) {
+            if (full) {
+                dd c[4], a[4], b[4];
 #pragma unroll
-            for (int u = 0; u < 4; u++) {
-                const int m = m0 + 32 * u;
-                c[u] = dd_load(dc, N, m);
-                a[u] = dd_load(f, N, (i - m) & mask);
-                b[u] = dd_load(f, N, (i + m) & mask);
-            }
+                for (int u = 0; u < 4; u++) {
+                    const int m = m0 + 128 * u;
+                    c[u] = dd_load(dc, N, m);
+                    a[u] = dd_load(f, N, (i - m) & mask);
+                    b[u] = dd_load(f, N, (i + m) & mask);
+                }
 #pragma unroll
-            for (int u = 0; u < 4; u++) acc4[u] = dd_fma(c[u], dd_sub(a[u], b[u]), acc4[u]);
-        } else {
+                for (int u = 0; u < 4; u++) acc4[u] = dd_fma(c[u], dd_sub(a[u], b[u]), acc4[u]);
+            } else {
 #pragma unroll
-            for (int u = 0; u < 4; u++) {
-                const int m = m0 + 32 * u;
-                if (m < N / 2) {
-                    dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
-                    dd c = dd_load(dc, N, m);
-                    acc4[u] = dd_fma(c, dd_sub(a, b), acc4[u]);
+                for (int u = 0; u < 4; u++) {
+                    const int m = m0 + 128 * u;
+                    if (m < N / 2) {
+                        dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
+                        dd c = dd_load(dc, N, m);
+                        acc4[u] = dd_fma(c, dd_sub(a, b), acc4[u]);
+                    }
                 }
             }
         }
     }
     dd acc = dd_add(dd_add(acc4[0], acc4[1]), dd_add(acc4[2], acc4[3]));
     acc = dd_warp_sum(acc);
-    if (lane == 0) dd_store(out, N, i, acc);
+    if (lane == 0) {
+        part[node][q][0] = acc.hi;
+        part[node][q][1] = acc.lo;
+    }
+    __syncthreads();
+    if (q == 0 && lane == 0 && i < N) {
+        for (int r = 1; r < 4; r++) acc = dd_add(acc, dd{part[node][r][0], part[node][r][1]});
+        dd_store(out, N, i, acc);
+    }
 }
 
 // exp / expm1 / sinh / cosh for the node tables with the series divisions replaced by dd reciprocals from a shared table
@@ -382,17 +395,18 @@ __global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const
     p[2 * N + i] = aG.hi;
     p[3 * N + i] = aG.lo;
 }
-// res = b - mu/2 - sum pK  (2.7) ;  w = sum pG ;  res_f64 = RN(res).  128 threads = 32 nodes x 4 groups of chunks (the loads of a
-// node's partial sums are the whole cost: four groups keep four of them in flight and shorten the dd chains).
-__global__ void __launch_bounds__(128) k_base_reduce(int N, int nchunk, const double* __restrict__ part, const double* __restrict__ b,
-                                                     const double* __restrict__ mu, double* __restrict__ res, double* __restrict__ res_f64,
-                                                     double* __restrict__ w) {
-    __shared__ double sh[4][4][32];
+// res = b - mu/2 - sum pK  (2.7) ;  w = sum pG ;  res_f64 = RN(res).  512 threads = 32 nodes x 16 groups of chunks (the loads of a
+// node's partial sums are the whole cost: sixteen groups keep sixteen of them in flight and shorten the dd chains).
+constexpr int BR_G = 16;
+__global__ void __launch_bounds__(32 * BR_G) k_base_reduce(int N, int nchunk, const double* __restrict__ part, const double* __restrict__ b,
+                                                           const double* __restrict__ mu, double* __restrict__ res, double* __restrict__ res_f64,
+                                                           double* __restrict__ w) {
+    __shared__ double sh[BR_G][4][32];
     const int l = threadIdx.x & 31, g = threadIdx.x >> 5;
     const int i = blockIdx.x * 32 + l;
     dd sK{0, 0}, sG{0, 0};
     if (i < N) {
-        for (int c = g; c < nchunk; c += 4) {
+        for (int c = g; c < nchunk; c += BR_G) {
             const double* p = part + (size_t)c * 4 * N;
             sK = dd_add(sK, dd{p[i], p[N + i]});
             sG = dd_add(sG, dd{p[2 * N + i], p[3 * N + i]});
@@ -401,7 +415,7 @@ __global__ void __launch_bounds__(128) k_base_reduce(int N, int nchunk, const do
     sh[g][0][l] = sK.hi; sh[g][1][l] = sK.lo; sh[g][2][l] = sG.hi; sh[g][3][l] = sG.lo;
     __syncthreads();
     if (g != 0 || i >= N) return;
-    for (int q = 1; q < 4; q++) {
+    for (int q = 1; q < BR_G; q++) {
         sK = dd_add(sK, dd{sh[q][0][l], sh[q][1][l]});
         sG = dd_add(sG, dd{sh[q][2][l], sh[q][3][l]});
     }
@@ -423,7 +437,7 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
         k_base_pass_dd<false><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
     SWW_LAUNCHED();
     SWW_BEGIN(KC_OTHER, d->stream);
-    k_base_reduce<<<(N + 31) / 32, 128, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
+    k_base_reduce<<<(N + 31) / 32, 32 * BR_G, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -432,7 +446,7 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
 static int run_node_prep(sww_dtn_s* d) {
     const int N = d->N;
     cudaStream_t st = d->stream;
-    int blocks = (N * 32 + 255) / 256;
+    int blocks = (N + 1) / 2;  // two nodes per CTA, four warps each
     SWW_BEGIN(KC_OTHER, st);
     k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->eta, d->d1);
     SWW_LAUNCHED();

@@ -21,61 +21,73 @@ constexpr int DD_SWEEPS = 2;
 // ------------------------------------------------------------------------------------------------ dd circulants: D and H
 // mode 0: out = D f,  coefficient (1/2)(-1)^m cot(pi m/N)                       (Fourier differentiation, Nyquist symbol 0, R4)
 // mode 1: out = H f,  coefficient (1/N) cot(pi m/N) (1 - (-1)^m) = 4 c0[m]/N for odd m, 0 for even m   (symbol -i sgn k)
-// Both kernels are odd in m, so out_i = sum_{m=1}^{N/2-1} coef[m] (f_{i-m} - f_{i+m}).  One warp per output node.
+// Both kernels are odd in m, so out_i = sum_{m=1}^{N/2-1} coef[m] (f_{i-m} - f_{i+m}).  Four warps per output node (two nodes per
+// CTA): the time of the kernel is the length of the per-lane chain of dependent dd operations behind scattered loads.
 // blockIdx.y = 1 (two-vector launches) applies the same circulant to a second, independent vector f2 -> out2.
 __global__ void __launch_bounds__(256) k_circ_dd(int N, int mode, const double* __restrict__ dc, const double* __restrict__ c0,
                                                  const double* __restrict__ f, double* __restrict__ out, const double* __restrict__ f2,
                                                  double* __restrict__ out2) {
+    __shared__ double part[2][4][2];
     if (blockIdx.y) {
         f = f2;
         out = out2;
     }
-    int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-    if (warp >= N) return;
-    int i = warp, mask = N - 1;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, node = warp >> 2, q = warp & 3;
+    const int i = blockIdx.x * 2 + node, mask = N - 1;
+    const int l128 = q * 32 + lane;
     // four independent dd accumulators per lane: one dd multiply-add is a chain of ~30 dependent fp64 instructions
     dd acc4[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
     const double hs = (mode == 0) ? 1.0 : 4.0 / (double)N;  // exact (power of two)
     const double* coef = (mode == 0) ? dc : c0;
     const int step = (mode == 0) ? 1 : 2;                   // H: odd m only
-    // both tables hold 0 at m = N/2, so when the stride divides N/2 the last group may run over it unguarded and the
-    // 24 loads of a group are issued together (the kernel is bound by their latency otherwise)
-    const bool full = ((N / 2) % (4 * 32 * step)) == 0;
-    for (int m0 = 1 + step * lane; m0 < N / 2; m0 += 4 * 32 * step) {
-        if (full) {
-            dd c[4], a[4], b[4];
+    if (i < N) {
+        // both tables hold 0 at m = N/2, so when the stride divides N/2 the last group may run over it unguarded and the
+        // 24 loads of a group are issued together (the kernel is bound by their latency otherwise)
+        const bool full = ((N / 2) % (4 * 128 * step)) == 0;
+        for (int m0 = 1 + step * l128; m0 < N / 2; m0 += 4 * 128 * step) {
+            if (full) {
+                dd c[4], a[4], b[4];
 #pragma unroll
-            for (int u = 0; u < 4; u++) {
-                const int m = m0 + u * 32 * step;
-                c[u] = dd_load(coef, N, m);
-                a[u] = dd_load(f, N, (i - m) & mask);
-                b[u] = dd_load(f, N, (i + m) & mask);
-            }
+                for (int u = 0; u < 4; u++) {
+                    const int m = m0 + u * 128 * step;
+                    c[u] = dd_load(coef, N, m);
+                    a[u] = dd_load(f, N, (i - m) & mask);
+                    b[u] = dd_load(f, N, (i + m) & mask);
+                }
 #pragma unroll
-            for (int u = 0; u < 4; u++) acc4[u] = dd_fma(dd{c[u].hi * hs, c[u].lo * hs}, dd_sub(a[u], b[u]), acc4[u]);
-        } else {
+                for (int u = 0; u < 4; u++) acc4[u] = dd_fma(dd{c[u].hi * hs, c[u].lo * hs}, dd_sub(a[u], b[u]), acc4[u]);
+            } else {
 #pragma unroll
-            for (int u = 0; u < 4; u++) {
-                const int m = m0 + u * 32 * step;
-                if (m < N / 2) {
-                    dd c = dd_load(coef, N, m);
-                    c.hi *= hs;
-                    c.lo *= hs;
-                    dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
-                    acc4[u] = dd_fma(c, dd_sub(a, b), acc4[u]);
+                for (int u = 0; u < 4; u++) {
+                    const int m = m0 + u * 128 * step;
+                    if (m < N / 2) {
+                        dd c = dd_load(coef, N, m);
+                        c.hi *= hs;
+                        c.lo *= hs;
+                        dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
+                        acc4[u] = dd_fma(c, dd_sub(a, b), acc4[u]);
+                    }
                 }
             }
         }
     }
     dd acc = dd_add(dd_add(acc4[0], acc4[1]), dd_add(acc4[2], acc4[3]));
     acc = dd_warp_sum(acc);
-    if (lane == 0) dd_store(out, N, i, acc);
+    if (lane == 0) {
+        part[node][q][0] = acc.hi;
+        part[node][q][1] = acc.lo;
+    }
+    __syncthreads();
+    if (q == 0 && lane == 0 && i < N) {
+        for (int r = 1; r < 4; r++) acc = dd_add(acc, dd{part[node][r][0], part[node][r][1]});
+        dd_store(out, N, i, acc);
+    }
 }
 
 int circ_dd(sww_dtn_s* d, int mode, const double* in, double* out) {
     const int N = d->N;
     SWW_BEGIN(KC_OTHER, d->stream);
-    k_circ_dd<<<(N * 32 + 255) / 256, 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in, out, nullptr, nullptr);
+    k_circ_dd<<<(N + 1) / 2, 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in, out, nullptr, nullptr);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -84,7 +96,7 @@ int circ_dd(sww_dtn_s* d, int mode, const double* in, double* out) {
 static int circ_dd2(sww_dtn_s* d, int mode, const double* in1, double* out1, const double* in2, double* out2) {
     const int N = d->N;
     SWW_BEGIN(KC_OTHER, d->stream);
-    k_circ_dd<<<dim3((N * 32 + 255) / 256, 2), 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in1, out1, in2, out2);
+    k_circ_dd<<<dim3((N + 1) / 2, 2), 256, 0, d->stream>>>(N, mode, d->tab->dc, d->tab->c0, in1, out1, in2, out2);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
