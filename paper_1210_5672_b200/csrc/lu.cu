@@ -950,12 +950,43 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
             } else {
                 cp_wait<0>();
             }
-            for (int spin = 0; __syncthreads_or(absentY(kk & 1)); spin++) {  // the barrier also makes the tiles visible to all
-                if (spin_out(spin)) break;
-                issueY(kk, kk & 1);  // not there yet: ask L2 again
-                cp_commit();
-                cp_wait<0>();
+            // Not there yet (the chain front): every thread polls ITS chunks with plain L2 loads into registers until none shows
+            // the absent pattern and puts them into the tile by hand -- no copy, wait and CTA-wide vote per round, one barrier at
+            // the end (which also makes the tiles visible to all).  A thread that gives up records SWW_ECUDA; the others look at
+            // the status word every 256 rounds.
+            if (absentY(kk & 1)) {
+                const double* Yg = Vin + (size_t)s * WS * N + (size_t)kblock(kk) * TS;
+                double* b = sB + (kk & 1) * WS * LDO;
+                constexpr int NCH = (WS * TS / 2 + 255) / 256;
+                double2 v[NCH];
+                for (int spin = 0;; spin++) {
+                    bool miss = false;
+#pragma unroll
+                    for (int q = 0; q < NCH; q++) {
+                        const int c = tid + q * 256;
+                        if (c < WS * TS / 2) {
+                            const int col = c >> 5, ch = (c & 31) * 2;
+                            v[q] = __ldcg(reinterpret_cast<const double2*>(Yg + (size_t)col * N + ch));
+                            miss |= (__double_as_longlong(v[q].x) == TR_ABSENT) | (__double_as_longlong(v[q].y) == TR_ABSENT);
+                        }
+                    }
+                    if (!miss) break;
+                    if (spin > 8 * TR_SPIN_LIMIT) {
+                        atomicCAS(p.status, SWW_OK, SWW_ECUDA);
+                        break;
+                    }
+                    if ((spin & 255) == 255 && ld_status(p.status) != SWW_OK) break;
+                }
+#pragma unroll
+                for (int q = 0; q < NCH; q++) {
+                    const int c = tid + q * 256;
+                    if (c < WS * TS / 2) {
+                        const int col = c >> 5, ch = (c & 31) * 2;
+                        *reinterpret_cast<double2*>(b + col * LDO + ch) = v[q];
+                    }
+                }
             }
+            __syncthreads();
             mma_tile(sA + (kk & 1) * TS * LDO, sB + (kk & 1) * WS * LDO);
         };
         // forward: all m terms; backward: the terms of the blocks k > i + 1 (the front term comes last, through V_i)
