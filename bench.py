@@ -251,6 +251,18 @@ def other_configs(sww, flush, peak_tf):
     fl = (2.0 / 3.0) * c5.N ** 3 + 2.0 * c5.N ** 2 * (c5.nrhs + 2) + 2.0 * c5.N ** 2 * c5.nrhs
     out["config5"] = {"workload": "N=4096, h=0.05, 512 columns, fp64", "ms_per_step": ms, "columns_per_s": c5.nrhs / (ms * 1e-3),
                       "tflops": fl / (ms * 1e-3) / 1e12, "frac_of_fp64_tensor_roofline": fl / (ms * 1e-3) / 1e12 / peak_tf, "bound": "FP64 tensor"}
+    # the shooting map: residual + Jacobian of the overdetermined shooting method, one shot = nsteps RK8 steps of
+    # (q, Qdot) with n variational columns (one setup + one batched linearized solve per stage)
+    Ns, ns_, nst = 512, 64, 8
+    S = sww.Shooter(Ns, ns_, 1.0, 1.0)
+    cs = np.zeros(ns_ + 1)
+    cs[0], cs[1] = 7.2, -0.02
+    cs[2:] = 2e-3 * np.exp(-0.5 * np.arange(2, ns_ + 1)) * np.cos(np.arange(2, ns_ + 1))
+    S.shoot(cs, nst)
+    ms = time_events(lambda: S.shoot(cs, nst), 3)
+    out["shooting"] = {"workload": f"shooting map N={Ns}, n={ns_} unknowns, {nst} RK8 steps to T/4: r (3.17) and J (3.31)", "ms_per_shot": ms,
+                       "column_stages_per_s": ns_ * nst * 11 / (ms * 1e-3), "bound": "latency (8-block LU chain per stage)"}
+    S.close()
     return out
 
 
