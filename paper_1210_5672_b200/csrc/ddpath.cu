@@ -361,11 +361,16 @@ __global__ void k_dd_copy(size_t n, size_t Ls, size_t Ld, int has_lo, const doub
     if (dst_f64) dst_f64[e] = hi;
 }
 // (2.9), in dd
-__global__ void k_base_uv_dd(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* __restrict__ W0,
-                             double* __restrict__ u, double* __restrict__ v) {
+// W0 = Wa (+ Wb when given; stored to W0out) and the surface velocities (2.9) from it
+__global__ void k_base_uv_dd(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* Wa, const double* Wb,
+                             double* W0out, double* __restrict__ u, double* __restrict__ v) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
-    dd e1 = dd_load(d1, N, j), p = dd_load(dphi, N, j), w = dd_load(W0, N, j);
+    dd e1 = dd_load(d1, N, j), p = dd_load(dphi, N, j), w = dd_load(Wa, N, j);
+    if (Wb) {
+        w = dd_add(w, dd_load(Wb, N, j));
+        dd_store(W0out, N, j, w);
+    }
     dd den = dd_add_d(dd_sqr(e1), 1.0);
     dd_store(u, N, j, dd_div(dd_sub(p, dd_mul(e1, w)), den));
     dd_store(v, N, j, dd_div(dd_add(dd_mul(e1, p), w), den));
@@ -500,11 +505,12 @@ static int ilog2(int n) {
     return l;
 }
 
-// out = a + b, dd planar with plane size N
-__global__ void k_dd_add(int N, const double* a, const double* b, double* out) {  // out may alias a or b
+// two independent sums in one launch: o1 = a1 + b1, o2 = a2 + b2 (dd planar, plane size N; outputs may alias their inputs)
+__global__ void k_dd_add2(int N, const double* a1, const double* b1, double* o1, const double* a2, const double* b2, double* o2) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
-    dd_store(out, N, j, dd_add(dd_load(a, N, j), dd_load(b, N, j)));
+    dd_store(o1, N, j, dd_add(dd_load(a1, N, j), dd_load(b1, N, j)));
+    dd_store(o2, N, j, dd_add(dd_load(a2, N, j), dd_load(b2, N, j)));
 }
 
 // ------------------------------------------------------------------------------------------------ flow (1): accurate base state
@@ -560,20 +566,15 @@ int accurate_base(sww_dtn_s* d, const double* phi0, size_t phi_plane) {
         SWW_LAUNCHED();
         SWW_TRY(circ_dd(d, 0, res, dgam));                                                 // D delta
         SWW_BEGIN(KC_OTHER, st);
-        k_dd_add<<<blocks, 256, 0, st>>>(N, mu, res, mu);                                  // mu0 = mu~ + delta
-        SWW_LAUNCHED();
-        SWW_BEGIN(KC_OTHER, st);
-        k_dd_add<<<blocks, 256, 0, st>>>(N, gam, dgam, gam);                               // gamma = D mu0
+        k_dd_add2<<<blocks, 256, 0, st>>>(N, mu, res, mu, gam, dgam, gam);                 // mu0 = mu~ + delta ; gamma = D mu0
         SWW_LAUNCHED();
         SWW_TRY(circ_dd(d, 1, gam, hg));                                                   // H gamma
         SWW_TRY(matvec_dd(d, d->G, nullptr, dgam, 0.5, hg, 0.0, 1.0, res, nullptr));       // H gamma / 2 + G_f64 (D delta)
-        SWW_BEGIN(KC_OTHER, st);
-        k_dd_add<<<blocks, 256, 0, st>>>(N, res, wt, d->bW0);                              // W0   (2.8)
-        SWW_LAUNCHED();
     }
     if (isdd) SWW_TRY(circ_dd(d, 0, b, d->bphi));                                          // phi0' (fp64 handles: done with gam~ above)
     SWW_BEGIN(KC_OTHER, st);
-    k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, d->bW0, d->bu, d->bv);
+    if (isdd) k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, d->bW0, nullptr, nullptr, d->bu, d->bv);
+    else k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, res, wt, d->bW0, d->bu, d->bv);   // W0 = res + w~ (2.8), then u, v
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

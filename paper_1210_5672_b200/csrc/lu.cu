@@ -1041,17 +1041,23 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
 #pragma unroll
         for (int x = 0; x < C::FM; x++)
 #pragma unroll
-            for (int e = 0; e < 2; e++) {
+            for (int e = 0; e < 2; e++) {  // first what the chain waits for: the high words of the whole block
                 const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
                 const double hi = __dadd_rn(sh[x][e], sl[x][e]);
-                const double low = __dsub_rn(sl[x][e], __dsub_rn(hi, sh[x][e]));
-                if (phase) {  // x_i: to its consumers, and the result
-                    p.Xh[blk + o] = tr_canon(hi);
-                    Bg[o] = hi;
-                    Lg[o] = low;
-                } else {      // y_i: hi for the forward tasks below, hi and lo for this block's backward task
-                    p.Yh[blk + o] = tr_canon(hi);
-                    p.Yl[blk + o] = tr_canon(low);
+                sl[x][e] = __dsub_rn(sl[x][e], __dsub_rn(hi, sh[x][e]));
+                sh[x][e] = hi;
+                (phase ? p.Xh : p.Yh)[blk + o] = tr_canon(hi);
+            }
+#pragma unroll
+        for (int x = 0; x < C::FM; x++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const size_t o = (size_t)(col0 + e) * N + row0 + x * 8;
+                if (phase) {  // x_i: the result (hi, lo)
+                    Bg[o] = sh[x][e];
+                    Lg[o] = sl[x][e];
+                } else {      // y_i: the low word for this block's backward task
+                    p.Yl[blk + o] = tr_canon(sl[x][e]);
                 }
             }
     }
