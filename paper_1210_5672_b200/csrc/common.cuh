@@ -39,16 +39,6 @@ void timing_end();
         if (::sww::g_timing) ::sww::timing_end();            \
     } while (0)
 
-#ifdef SWW_TUNE  // development aid, compiled out of the product (build.py never defines it): integer knobs from the environment
-inline int tune_int(const char* name, int dflt) {
-    const char* s = getenv(name);
-    return s ? atoi(s) : dflt;
-}
-#define SWW_TUNE_INT(name, dflt) ::sww::tune_int(name, dflt)
-#else
-#define SWW_TUNE_INT(name, dflt) (dflt)
-#endif
-
 // ---------------------------------------------------------------- per-device state
 // first() is true exactly once per device for each instance: guards the per-device opt-ins (cudaFuncSetAttribute for more than
 // 48 KB of dynamic shared memory) at their call sites.  Not thread-safe (like the rest of the library's host side).

@@ -690,7 +690,7 @@ int run_lu(sww_dtn_s* d) {
     a.status = d->status;
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), st));
     // clusters of two CTAs: cluster 0 is the spine, every other CTA works on its own (an even grid, one CTA per SM)
-    const int grid = std::min(SWW_TUNE_INT("SWW_LU_GRID", sm_count()) & ~1, (3 + a.ntasks) & ~1);
+    const int grid = std::min(sm_count() & ~1, (3 + a.ntasks) & ~1);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid);
     cfg.blockDim = dim3(LU_THREADS);
@@ -1423,10 +1423,6 @@ __global__ void __launch_bounds__(320, 1) k_trsm_ws(TrsmArgs p) {
 template <int WS>
 static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     using C = TrsmCfg<WS>;
-    static DeviceOnce attr_once;
-    if (attr_once.first()) {
-        SWW_CUDA(cudaFuncSetAttribute(k_trsm_dataflow<WS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
-    }
     const int N = d->N, nt = N / TS;
     TrsmArgs a;
     a.A = d->LU;
@@ -1455,12 +1451,14 @@ static int launch_trsm(sww_dtn_s* d, double* B, double* Blo, int ns) {
     SWW_CUDA(cudaMemsetAsync(a.counter, 0, sizeof(unsigned), d->stream));
     const int grid = std::min(sm_count(), 2 * nt * ns);
     SWW_BEGIN(WS == 8 ? KC_TRSV : KC_TRSM, d->stream);  // the 8-column instantiation serves the single-vector solves: chain-latency-bound
-    if (SWW_TUNE_INT("SWW_TR_IMPL", WS >= 16 ? 1 : 0)) {
+    if constexpr (WS >= 16) {  // batches: the warp-specialized kernel
         using W = TrsmWsCfg<WS>;
         static DeviceOnce attr_ws;
         if (attr_ws.first()) SWW_CUDA(cudaFuncSetAttribute(k_trsm_ws<WS>, cudaFuncAttributeMaxDynamicSharedMemorySize, W::SMEM));
         k_trsm_ws<WS><<<grid, W::THREADS, W::SMEM, d->stream>>>(a);
-    } else {
+    } else {                   // up to 64 columns (the single-vector solves): pure chain latency, every warp polls and multiplies
+        static DeviceOnce attr_once;
+        if (attr_once.first()) SWW_CUDA(cudaFuncSetAttribute(k_trsm_dataflow<WS>, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM));
         k_trsm_dataflow<WS><<<grid, 256, C::SMEM, d->stream>>>(a);
     }
     SWW_LAUNCHED();
@@ -1485,7 +1483,7 @@ int run_solve(sww_dtn_s* d, double* B, double* Blo, int ncols) {
     // slab width: the chain of a slab is 2 N/64 links of (flag hop + one or two 64 x 64 x WS products), so narrow slabs finish
     // sooner as long as there are few of them; every slab re-reads the factors from L2, so many columns want wide slabs
     // (measured at N = 2048: 128 columns 0.19 ms with 16-column slabs against 0.27 ms with 32; 512 columns 0.36 against 0.34)
-    const int ws = ncols <= 64 ? 8 : SWW_TUNE_INT("SWW_TR_WS", ncols <= 256 ? 16 : 32);
+    const int ws = ncols <= 64 ? 8 : (ncols <= 256 ? 16 : 32);
     for (int c0 = 0; c0 < ncols; c0 += TR_MAXNS * ws) {
         const int nc = std::min(ncols - c0, TR_MAXNS * ws);
         double *b = B + (size_t)c0 * N, *bl = Blo + (size_t)c0 * N;
