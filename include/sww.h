@@ -147,6 +147,7 @@ int sww_shooter_destroy(sww_shooter_t S);
 /* The residual alone (a stepper without variational columns inside the handle: what Levenberg-Marquardt needs for a trial step). */
 int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r);
 int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd);
+int sww_shooter_set_method(sww_shooter_t S, int method);   /* 0: RK8 (default); 1: SDC15, the paper's quadruple-precision stepper */
 int sww_shooter_set_sigma(sww_shooter_t S, double sigma);   /* surface tension of every following shot (see sww_state_set_sigma) */
 
 /* ---- Levenberg-Marquardt with delayed Jacobian updates (Appendix C) ----------------------------

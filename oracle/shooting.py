@@ -44,7 +44,7 @@ def initial_state(c, N: int):
     return eta, phi, deta, dphi
 
 
-def shoot(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True, sigma: float = 0.0):
+def shoot(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True, sigma: float = 0.0, method: str = "rk8"):
     """-> dict r (N), J (N x (n+1)), eta, phi (the state at T/4), all long double"""
     c = np.asarray(c, dtype=np.float64)
     n = c.shape[0] - 1
@@ -55,7 +55,7 @@ def shoot(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True, 
     if N * n <= 4096:
         orc.set_num_threads(1)   # hundreds of tiny right-hand sides: the OpenMP barriers would dominate
     try:
-        out = orc.rk_advance(_split(eta0), _split(phi0), h, g, dt, nsteps, deta=_split(deta0), dphi=_split(dphi0), filter=filter, sigma=sigma)
+        out = orc.rk_advance(_split(eta0), _split(phi0), h, g, dt, nsteps, deta=_split(deta0), dphi=_split(dphi0), filter=filter, sigma=sigma, method=method)
     finally:
         orc.set_num_threads(nthr)
     ld = lambda p: p[0].astype(LD) + p[1].astype(LD)
@@ -90,14 +90,14 @@ def initial_state_quad(c, N: int):
         return pair(eta), pair(phi), stack(deta), stack(dphi)
 
 
-def shoot_quad(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True, sigma: float = 0.0):
+def shoot_quad(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True, sigma: float = 0.0, method: str = "rk8"):
     """shoot() for the __float128 oracle: -> dict r (hi, lo), J (hi, lo) with J[.] of shape (N, n + 1)"""
     import mpmath as mp
     c = np.asarray(c, dtype=np.float64)
     n = c.shape[0] - 1
     T = float(c[0])
     eta0, phi0, deta0, dphi0 = initial_state_quad(c, N)
-    out = orc.rk_advance(eta0, phi0, h, g, T / (4 * nsteps), nsteps, deta=deta0, dphi=dphi0, filter=filter, sigma=sigma)
+    out = orc.rk_advance(eta0, phi0, h, g, T / (4 * nsteps), nsteps, deta=deta0, dphi=dphi0, filter=filter, sigma=sigma, method=method)
     phi_t = orc.rhs(out["eta"], out["phi"], h, g, filter=filter, sigma=sigma)["phi_t"]
     with mp.workprec(160):
         w = 1 / mp.sqrt(mp.mpf(N))

@@ -18,7 +18,7 @@ EXPORTS = [
     "sww_state_destroy", "sww_strerror", "sww_last_cuda_error", "sww_launch_count", "sww_probe_fp64_peak",
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
-    "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance", "sww_dtn_adjoint_rhs",
+    "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance", "sww_dtn_adjoint_rhs", "sww_shooter_set_method",
 ]
 
 
@@ -92,6 +92,7 @@ def lib() -> ctypes.CDLL:
         L.sww_shooter_destroy.argtypes = [vp]
         L.sww_state_set_sigma.argtypes = [vp, cd]
         L.sww_shooter_set_sigma.argtypes = [vp, cd]
+        L.sww_shooter_set_method.argtypes = [vp, ci]
         L.sww_shoot_residual.argtypes = [vp, ctypes.POINTER(cd), ci, vp]
         L.sww_shooter_dims.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
         L.sww_lm_minimize.argtypes = [LM_FUN, vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(LmOptions), ctypes.POINTER(LmReport)]
@@ -315,6 +316,10 @@ class Shooter:
 
     def set_sigma(self, sigma: float):
         _check(lib().sww_shooter_set_sigma(self._h, float(sigma)), "sww_shooter_set_sigma")
+
+    def set_method(self, method: str):
+        """"rk8" (default) or "sdc15" for the time stepping of every following shot"""
+        _check(lib().sww_shooter_set_method(self._h, {"rk8": 0, "sdc15": 1}[method]), "sww_shooter_set_method")
 
     def shoot(self, c, nsteps: int, want_state: bool = False):
         """-> r (N), J (n + 1, N) [= column-major N x (n + 1)]; double-double: leading axis 2 (hi, lo)"""

@@ -17,6 +17,7 @@ struct sww_shooter_s {
     int N, n, prec;
     double h, g, sigma;
     unsigned flags;
+    int sdc;         // 1: advance by the SDC15 scheme (sww_sdc_advance) instead of RK8
     sww_state_t st;  // the stepper with the n variational columns
     sww_state_t st0; // the stepper without columns (residual-only shots), created at the first such shot
     double* c_dev;   // n + 1 unknowns
@@ -130,7 +131,8 @@ static int shoot_impl(sww_shooter_t S, sww_state_s* s, bool with_cols, const dou
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     s->t = 0.0;
-    SWW_TRY(sww_rk_advance(s, c[0] / (4.0 * nsteps), nsteps));
+    if (S->sdc) SWW_TRY(sww_sdc_advance(s, c[0] / (4.0 * nsteps), nsteps));
+    else SWW_TRY(sww_rk_advance(s, c[0] / (4.0 * nsteps), nsteps));
     if (with_cols) SWW_TRY(rk_rhs(s, s->y, s->k));  // phi_t at T/4 (stage slot 0)
     // w = 1/sqrt(N), N = 2^p: a power of two, times 1/sqrt(2) (double-double) when p is odd
     int p = 0;
@@ -167,6 +169,12 @@ int sww_shooter_set_sigma(sww_shooter_t S, double sigma) {
     S->sigma = sigma;
     S->st->sigma = sigma;
     if (S->st0) S->st0->sigma = sigma;
+    return SWW_OK;
+}
+
+int sww_shooter_set_method(sww_shooter_t S, int method) {
+    if (!S || (method != 0 && method != 1)) return SWW_EINVAL;
+    S->sdc = method;
     return SWW_OK;
 }
 

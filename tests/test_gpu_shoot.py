@@ -76,6 +76,25 @@ def test_residual_and_jacobian_dd(sww, orc_q):
     S.close()
 
 
+def test_residual_and_jacobian_dd_with_sdc15(sww, orc_q):
+    """the paper's quadruple-precision shooting: double-double state advanced by SDC15, two large steps to T/4"""
+    from oracle import shooting
+    N, n, nsteps = 64, 4, 2
+    c = unknowns(n)
+    S = sww.Shooter(N, n, 1.0, 1.0, prec=sww.DD)
+    S.set_method("sdc15")
+    r, J = S.shoot(c, nsteps)
+    o = shooting.shoot_quad(orc_q, c, N, 1.0, 1.0, nsteps, method="sdc15")
+    rg = r.cpu().numpy()
+    dr = (rg[0].astype(LD) - o["r"][0].astype(LD)) + (rg[1].astype(LD) - o["r"][1].astype(LD))
+    assert float(np.abs(dr).max() / np.abs(o["r"][0]).max()) <= 1e-25
+    Jg = J.cpu().numpy()
+    dJ = (Jg[0].astype(LD) - o["J"][0].T.astype(LD)) + (Jg[1].astype(LD) - o["J"][1].T.astype(LD))
+    e = np.abs(dJ).max(axis=1) / np.abs(o["J"][0].T).max(axis=1)
+    assert float(e.max()) <= 1e-25, e
+    S.close()
+
+
 def test_gauss_newton_on_the_period_finds_the_linear_period(sww):
     """the small-amplitude branch: Gauss-Newton on c_0 = T alone with the device residual and Jacobian column 0 converges to
     T = 2 pi / sqrt(tanh 1) = 7.19976; f = r.r / 2 falls to roundoff"""
