@@ -54,6 +54,31 @@ __device__ __forceinline__ void st_release(unsigned* p, unsigned v) {
     asm volatile("st.release.gpu.global.u32 [%0], %1;\n" ::"l"(p), "r"(v) : "memory");
 }
 
+// ---- mbarrier helpers (shared-memory barriers with phase parity: the full / empty pairs of the operand rings)
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(unsigned long long* bar, unsigned parity) {
+    unsigned ok;
+    asm volatile(
+        "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+        : "=r"(ok)
+        : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    while (!mbar_test(bar, parity)) {
+    }
+}
+// arrival on `bar` when every cp.async this thread has issued so far has landed (counted in the barrier's expected arrivals)
+__device__ __forceinline__ void cp_arrive_on(unsigned long long* bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------ 64 x 64 GETRF in shared memory
 // One rolled loop of 64 elimination steps by a 256-thread CTA; thread (ty, tx) of a 16 x 16 grid keeps the 4 x 4 register tile
 // rows ty + 16 q, columns tx + 16 b of three matrices:
@@ -223,9 +248,10 @@ struct LuArgs {
     int* status;
 };
 
-// spine: sX, sF (64 columns), sU, sV, sP (32 columns), two work tiles, bgj64 scratch; workers: four operand tiles + ready[]
+// spine: sX, sF (64 columns), sU, sV, sP (32 columns), two work tiles, bgj64 scratch; workers: a ring of three operand tile pairs
 constexpr int LU_SMEM_SPINE = (2 * TS * LDO + 3 * 32 * LDO + 2 * TS * LDT + BGJ_SCRATCH) * (int)sizeof(double);
-constexpr int LU_SMEM_WORKER = 4 * TS * LDO * (int)sizeof(double) + 256;
+constexpr int LU_RING = 3;          // stages of the workers' operand ring (one L tile + one U tile per stage)
+constexpr int LU_SMEM_WORKER = 2 * LU_RING * TS * LDO * (int)sizeof(double) + 256;
 constexpr int LU_SMEM_BYTES = LU_SMEM_SPINE > LU_SMEM_WORKER ? LU_SMEM_SPINE : LU_SMEM_WORKER;
 
 // fragment coordinates of this lane (threads 0..255): rows wr*32 + x*8 + fr (x < 4), columns wc*16 + y*8 + 2 fk + e (y, e < 2)
@@ -451,10 +477,16 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
         lu_spine(p, lu_sm);
         return;
     }
-    double* sA = lu_sm;                   // 2 stages of L_ik as As[k][r]
-    double* sB = sA + 2 * TS * LDO;       // 2 stages of U_kj as Bs[n][k]
-    unsigned char* ready = reinterpret_cast<unsigned char*>(sB + 2 * TS * LDO);  // ready[k]: both operand tiles of step k are final
+    double* sA = lu_sm;                         // LU_RING stages of L_ik as As[k][r]
+    double* sB = sA + LU_RING * TS * LDO;       // LU_RING stages of U_kj as Bs[n][k]
+    __shared__ unsigned long long full[LU_RING], empty[LU_RING];
     __shared__ int s_task;
+    if (tid == 0)
+        for (int q = 0; q < LU_RING; q++) {
+            mbar_init(&full[q], LU_THREADS - 256);   // the producer threads, each when its copies of the stage have landed
+            mbar_init(&empty[q], 8);                 // the eight MMA warps
+        }
+    unsigned it = 0;  // ring position: plain terms done so far by this CTA (the same number in every thread)
     const Frag f(tid);
     const bool mm = tid < 256;
     const int N = p.N, nt = p.nt;
@@ -486,15 +518,6 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
         double* Cg = has_tile ? tile(i, j) : nullptr;
         SWW_WSTAMP(0);
 
-        auto refresh = [&]() {
-            for (int t = tid; t < m; t += LU_THREADS)
-                ready[t] = (ld_acquire(p.flags + (size_t)i * nt + t) == epoch) && (ld_acquire(p.flags + (size_t)t * nt + j) == epoch);
-        };
-        auto issue = [&](int k, int buf) {
-            tile_async(sA + buf * TS * LDO, tile(i, k), N, tid, LU_THREADS);
-            tile_async(sB + buf * TS * LDO, tile(k, j), N, tid, LU_THREADS);
-            cp_commit();
-        };
         // own tile -> registers (fragment layout), sum = 0
         double c0[4][2][2], acc[4][2][2];
 #pragma unroll
@@ -502,42 +525,39 @@ __global__ void __launch_bounds__(LU_THREADS, 1) k_lu_dataflow(LuArgs p) {
             c0[x][y][e] = (mm && has_tile) ? Cg[(size_t)f.col(y, e) * N + f.row(x)] : 0.0;
             acc[x][y][e] = 0.0;
         }
-        // term k is not final yet: U_kj (final a generation before L_ik) is fetched first, L_ik as soon as its flag is set
-        auto wait_issue = [&](int k, int buf) {
-            if (tid == 0) spin_tight(p.flags + (size_t)k * nt + j, epoch);
-            __syncthreads();
-            tile_async(sB + buf * TS * LDO, tile(k, j), N, tid, LU_THREADS);
-            cp_commit();
-            if (tid == 0) spin_tight(p.flags + (size_t)i * nt + k, epoch);
-            __syncthreads();
-            tile_async(sA + buf * TS * LDO, tile(i, k), N, tid, LU_THREADS);
-            cp_commit();
-        };
-        refresh();  // what is final at the start of the task
-        __syncthreads();
-        if (m > 0) {
-            if (ready[0]) issue(0, 0);
-            else wait_issue(0, 0);
-        }
-        for (int k = 0; k < m; k++) {
-            bool pre = (k + 1 < m) && ready[k + 1];
-            if (k + 1 < m && !pre) {  // a quick look: the flags may have been set since the task started
-                bool ok = true;
-                if (tid == 0) ok = ld_acquire(p.flags + (size_t)i * nt + k + 1) == epoch;
-                if (tid == 1) ok = ld_acquire(p.flags + (size_t)(k + 1) * nt + j) == epoch;
-                pre = __syncthreads_and(ok);
+        // The plain terms k < m, warp-specialized: the three warps that have no part in the products are the PRODUCERS -- they wait for
+        // the flags of the two operand tiles of term k (U_kj is final a generation before L_ik), fetch them into the next stage of
+        // the ring as soon as the MMA warps have released it, and go on to term k + 1; each producer thread's arrival on the
+        // stage's full barrier fires when its copies have landed.  The eight MMA warps do nothing but wait, multiply and release.
+        if (mm) {
+            for (int k = 0; k < m; k++) {
+                const unsigned g = it + (unsigned)k;
+                const int buf = (int)(g % LU_RING);
+                mbar_wait(&full[buf], (g / LU_RING) & 1u);
+                mma_tile64(acc, sA + buf * TS * LDO, sB + buf * TS * LDO, f);
+                __syncwarp();
+                if ((tid & 31) == 0) mbar_arrive(&empty[buf]);
             }
-            if (pre) {
-                issue(k + 1, (k + 1) & 1);
-                cp_wait<1>();
-            } else {
-                cp_wait<0>();
+        } else {
+            const int t = tid - 256;  // 0..95
+            for (int k = 0; k < m; k++) {
+                const unsigned g = it + (unsigned)k;
+                const int buf = (int)(g % LU_RING);
+                if (t == 0) {
+                    spin_tight(p.flags + (size_t)k * nt + j, epoch);
+                    spin_tight(p.flags + (size_t)i * nt + k, epoch);
+                }
+                asm volatile("bar.sync 6, 96;" ::: "memory");  // the producers: the acquire of lane 0 orders everybody's copies behind the flags
+                mbar_wait(&empty[buf], ((g / LU_RING) & 1u) ^ 1u);
+                tile_async(sA + buf * TS * LDO, tile(i, k), N, t, LU_THREADS - 256);
+                tile_async(sB + buf * TS * LDO, tile(k, j), N, t, LU_THREADS - 256);
+                cp_arrive_on(&full[buf]);
             }
-            __syncthreads();
-            if (mm) mma_tile64(acc, sA + (k & 1) * TS * LDO, sB + (k & 1) * TS * LDO, f);
-            __syncthreads();
-            if (!pre && k + 1 < m) wait_issue(k + 1, (k + 1) & 1);
+            cp_commit();
+            cp_wait<0>();  // nothing of mine is in flight when the task goes on to its last term (which re-uses the stages)
         }
+        it += (unsigned)m;
+        __syncthreads();  // every plain term is in acc; the ring is free
         auto store_tile = [&](double* dst, size_t ld, const double (&v)[4][2][2]) {
             if (mm) {
 #pragma unroll
@@ -1071,25 +1091,6 @@ __global__ void __launch_bounds__(256, 1) k_trsm_dataflow(TrsmArgs p) {
 // warps never poll, never issue a copy and meet no CTA-wide barrier inside a task.
 // Backward sweep: x_i = Z_i (y_i - sum_{k>i+1} U_ik x_k) - V_i x_{i+1} with V_i = Z_i U_{i,i+1} kept by the LU spine: the product
 // with the diagonal block is done before the front block x_{i+1} arrives, a link of the chain is one product in both sweeps.
-__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long* bar) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
-}
-__device__ __forceinline__ bool mbar_test(unsigned long long* bar, unsigned parity) {
-    unsigned ok;
-    asm volatile(
-        "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
-        : "=r"(ok)
-        : "r"((unsigned)__cvta_generic_to_shared(bar)), "r"(parity)
-        : "memory");
-    return ok != 0;
-}
-__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
-    while (!mbar_test(bar, parity)) {
-    }
-}
 // named barrier 1 with an OR reduction among the 256 threads of the MMA warps
 __device__ __forceinline__ bool mma_bar_or(bool pred) {
     int r;
