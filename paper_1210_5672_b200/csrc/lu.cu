@@ -437,11 +437,15 @@ __device__ void lu_spine(const LuArgs& p, double* sm) {
                 mma_half(v, sF, sU, f);
 #pragma unroll
                 SWW_FRAGH_LOOP sV[f.col(y, e) * LDO + f.row(x)] = v[x][y][e];
-                double* Vg = p.Vs + (size_t)(m - 1) * TS * TS + (size_t)cb * TS;  // kept for the triangular solves
-#pragma unroll
-                SWW_FRAGH_LOOP Vg[f.col(y, e) * TS + f.row(x)] = v[x][y][e];
             }
             __syncthreads();
+            if (!mm) {  // V is kept for the triangular solves: the warps that have no part in the products copy it out meanwhile
+                double* Vg = p.Vs + (size_t)(m - 1) * TS * TS + (size_t)cb * TS;
+                for (int c = tid - 256; c < 32 * TS / 2; c += LU_THREADS - 256) {
+                    const int col = c >> 5, ch = (c & 31) * 2;
+                    *reinterpret_cast<double2*>(Vg + col * TS + ch) = *reinterpret_cast<const double2*>(sV + col * LDO + ch);
+                }
+            }
             if (mm) {  // S_m = P_m - X_{m,m-1} V, my columns -> both CTAs' work tiles
 #pragma unroll
                 SWW_FRAGH_LOOP {
