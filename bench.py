@@ -359,7 +359,7 @@ def main():
     peaks = measured_peaks()
     peak_tf = peaks["bf16_tflops"] * NOMINAL_FP64_OVER_BF16
     probe = {"dfma_tflops": sww.probe_fp64_peak(0) / 1e12, "dmma_tflops": sww.probe_fp64_peak(1) / 1e12}
-    names = {"lu": "k_lu_dataflow (block LU in one persistent launch: a two-CTA cluster as the spine, blocked Gauss-Jordan inverses of the 64x64 Schur blocks on the tensor pipe, DMMA.8x8x4 tile workers)",
+    names = {"lu": "k_lu_dataflow (block LU in one persistent launch: a two-CTA cluster as the spine, blocked Gauss-Jordan inverses of the 64x64 Schur blocks on the tensor pipe, warp-specialized DMMA.8x8x4 tile workers: producer warps + mbarrier operand ring)",
              "trsm": "k_trsm_ws<32> (persistent warp-specialized DMMA.8x8x4 multi-RHS triangular solves of the column batch: loader warps + mbarrier ring, tasks handing blocks over through L2 with the data as the flag)",
              "gemm_dmma": "k_gemm_f64 (DMMA.8x8x4): G product"}
     per_kernel = {}
