@@ -182,7 +182,9 @@ __global__ void __launch_bounds__(256) k_matvec_dd(int N, const double* __restri
 static int matvec_dd(sww_dtn_s* d, const double* A, const double* Alo, const double* x, double zs, const double* z, double beta,
                      double alpha, double* y, double* y_f64) {
     const int N = d->N;
-    const int ny = (N >= 512 && d->bp_chunks >= 2) ? 4 : 1;  // part = d->bp_part: bp_chunks * 4 * N doubles >= ny * 2 * N
+    // column splits: the per-thread chain of dd operations behind the loads sets the time (part = d->bp_part: bp_chunks * 4 * N
+    // doubles >= ny * 2 * N; every split keeps a multiple of 64 columns)
+    const int ny = (N >= 2048 && d->bp_chunks >= 8) ? 16 : ((N >= 512 && d->bp_chunks >= 2) ? 4 : 1);
     SWW_BEGIN(KC_DDGEMM, d->stream);
     k_matvec_dd<<<dim3((N + 31) / 32, ny), 256, 0, d->stream>>>(N, A, Alo, x, zs, z, beta, alpha, y, y_f64, d->bp_part, d->mv_count);
     SWW_LAUNCHED();
