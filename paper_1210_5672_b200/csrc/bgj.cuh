@@ -28,6 +28,7 @@ __device__ __forceinline__ int bgj_role(int warp) {  // 0..7: update warp owning
     if ((warp & 3) == 0 || warp > 10) return -1;
     return warp - 1 - (warp >> 2);
 }
+constexpr int BGJ_TLD = 66;   // leading dimension of the input tile T (row-major; even: entry pairs are 16-byte aligned)
 constexpr int BGJ_RLD = 66;   // leading dimension of the pivot-row panel (8 x 64, row-major): conflict-free B-fragment loads
 constexpr int BGJ_FLD = 10;   // leading dimension of the 8 x 8 pivot-block inverse
 constexpr int BGJ_SCRATCH = 2 * 8 * BGJ_RLD + 2 * 8 * BGJ_FLD + 64;  // doubles: Rs[2], Fs8[2], Ds
@@ -200,7 +201,7 @@ __device__ __forceinline__ void bgj_panel(double (&acc)[8][2], int w, int fr, in
     }
 }
 
-// T (shared, row-major, leading dimension 65) holds kappa = S - I/2.  On return F = inv(S) - 2 I is in Fg (global, column-major,
+// T (shared, row-major, leading dimension BGJ_TLD, 16-byte aligned) holds kappa = S - I/2.  On return F = inv(S) - 2 I is in Fg (global, column-major,
 // ld 64; skipped when Fg == nullptr) and in sF (shared, column-major, ld 68: the DMMA operand layout of lu.cu).  Every one of the 352 threads must call it;
 // scr: BGJ_SCRATCH doubles of shared memory.  The two idle warps return as soon as every active warp has read T (from then on
 // the caller may overwrite it); the active warps end with a barrier among themselves: the caller must follow with a CTA-wide
@@ -245,8 +246,9 @@ __device__ __forceinline__ void bgj64(const double* T, double* scr, int* status,
     double acc[8][2];
 #pragma unroll
     for (int t = 0; t < 8; t++) {
-        acc[t][0] = T[(8 * w + fr) * 65 + 8 * t + 2 * fk];
-        acc[t][1] = T[(8 * w + fr) * 65 + 8 * t + 2 * fk + 1];
+        const double2 tv = *reinterpret_cast<const double2*>(T + (8 * w + fr) * BGJ_TLD + 8 * t + 2 * fk);
+        acc[t][0] = tv.x;
+        acc[t][1] = tv.y;
     }
     bgj_bar_arrive(BGJ_BAR_TREAD, BGJ_CTA_THREADS);
     if (w == 0) {

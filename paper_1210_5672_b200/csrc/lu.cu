@@ -249,7 +249,7 @@ struct LuArgs {
 };
 
 // spine: sX, sF (64 columns), sU, sV, sP (32 columns), two work tiles, bgj64 scratch; workers: a ring of three operand tile pairs
-constexpr int LU_SMEM_SPINE = (2 * TS * LDO + 3 * 32 * LDO + 2 * TS * LDT + BGJ_SCRATCH) * (int)sizeof(double);
+constexpr int LU_SMEM_SPINE = (2 * TS * LDO + 3 * 32 * LDO + 2 * TS * BGJ_TLD + BGJ_SCRATCH) * (int)sizeof(double);
 constexpr int LU_RING = 3;          // stages of the workers' operand ring (one L tile + one U tile per stage)
 constexpr int LU_SMEM_WORKER = 2 * LU_RING * TS * LDO * (int)sizeof(double) + 256;
 constexpr int LU_SMEM_BYTES = LU_SMEM_SPINE > LU_SMEM_WORKER ? LU_SMEM_SPINE : LU_SMEM_WORKER;
@@ -337,9 +337,6 @@ __device__ __forceinline__ unsigned cluster_map(const void* p, unsigned rank) {
     asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
     return r;
 }
-__device__ __forceinline__ void st_cluster_f64(unsigned addr, double v) {
-    asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
-}
 
 // fragment coordinates for a 64 x 32 half tile (threads 0..255): rows wr*16 + x*8 + fr (x < 2), columns wc*16 + y*8 + 2 fk + e
 struct FragH {
@@ -384,8 +381,8 @@ __device__ void lu_spine(const LuArgs& p, double* sm) {
     double* sU = sF + TS * LDO;       // my 32 columns of U_{m-1,m}              (B operand: Bs[n][k])
     double* sV = sU + 32 * LDO;       // my 32 columns of V = Z_{m-1} U_{m-1,m}  (B operand)
     double* sP = sV + 32 * LDO;       // my 32 columns of P_m (column-major, ld LDO)
-    double* sK = sP + 32 * LDO;       // 2 work tiles kappa_m = S_m - I/2 (row-major, ld LDT) for bgj64, alternating by step
-    double* scr = sK + 2 * TS * LDT;
+    double* sK = sP + 32 * LDO;       // 2 work tiles kappa_m = S_m - I/2 (row-major, ld BGJ_TLD) for bgj64, alternating by step
+    double* scr = sK + 2 * TS * BGJ_TLD;
     const int tid = threadIdx.x;
     const FragH f(tid);
     const bool mm = tid < 256;        // the 8 MMA warps of the two products
@@ -421,12 +418,12 @@ __device__ void lu_spine(const LuArgs& p, double* sm) {
         cp_wait<0>();
     };
     for (int m = 0; m < nt; m++) {
-        double* T = sK + (m & 1) * TS * LDT;
+        double* T = sK + (m & 1) * TS * BGJ_TLD;
         SWW_STAMP(m, 0);
         if (m == 0) {
             for (int e = tid; e < TS * TS; e += LU_THREADS) {
                 const int r = e & 63, c = e >> 6;
-                T[r * LDT + c] = p.A[(size_t)c * N + r];
+                T[r * BGJ_TLD + c] = p.A[(size_t)c * N + r];
             }
         } else {
             SWW_STAMP(m, 1);
@@ -455,12 +452,14 @@ __device__ void lu_spine(const LuArgs& p, double* sm) {
                 mma_half(v, sX, sV, f);
                 const unsigned Tpeer = cluster_map(T, peer);
 #pragma unroll
-                SWW_FRAGH_LOOP {
-                    const int o = f.row(x) * LDT + cb + f.col(y, e);
-                    const double k = c0[x][y][e] - v[x][y][e];
-                    T[o] = k;
-                    st_cluster_f64(Tpeer + 8u * (unsigned)o, k);
-                }
+                for (int x = 0; x < 2; x++)
+#pragma unroll
+                    for (int y = 0; y < 2; y++) {  // the two entries of a fragment row are neighbours in the row-major tile: one 16-byte store each way
+                        const int o = f.row(x) * BGJ_TLD + cb + f.col(y, 0);
+                        const double k0 = c0[x][y][0] - v[x][y][0], k1 = c0[x][y][1] - v[x][y][1];
+                        *reinterpret_cast<double2*>(T + o) = make_double2(k0, k1);
+                        asm volatile("st.shared::cluster.v2.f64 [%0], {%1, %2};" ::"r"(Tpeer + 8u * (unsigned)o), "d"(k0), "d"(k1) : "memory");
+                    }
             }
         }
         cluster_sync_all();  // kappa_m complete in both CTAs (also the CTA barrier: sX, sU, sV, sP free)
