@@ -95,6 +95,32 @@ class Oracle:
     def sizeof_real(self) -> int:
         return int(self._f("sizeof_real")())
 
+    def set_mesh(self, rho: float = 1.0, where: int = 0) -> None:
+        """Mesh refinement (2.10) for the following calls of this build: rho in (0, 1] (1 = uniform), where = 0 refines near
+        x = pi, 1 near x = 0.  Reset with set_mesh() when done."""
+        _check(self._f("set_mesh")(ctypes.c_double(rho), ctypes.c_int(where)), "set_mesh")
+
+    def mesh_tables(self, N: int):
+        """-> xp = xi - alpha, E = xi', E1 = xi'' (each (hi, lo)) of the current mesh setting at alpha_j = 2 pi j / N"""
+        o = [(np.empty(N), np.empty(N)) for _ in range(3)]
+        _check(self._f("mesh_tables")(ctypes.c_int(N), _p(o[0][0]), _p(o[0][1]), _p(o[1][0]), _p(o[1][1]), _p(o[2][0]), _p(o[2][1])), "mesh_tables")
+        return tuple(o)
+
+    def respace(self, f, old, new):
+        """Values on the mesh `new` = (M, rho, where) of the functions stored on the mesh `old`; f: (ncols, M_old)"""
+        fhi, flo = _split(f)
+        one = fhi.ndim == 1
+        if one:
+            fhi = fhi[None, :]
+            flo = None if flo is None else flo[None, :]
+        Mo, Mn = int(old[0]), int(new[0])
+        ncols = fhi.shape[0]
+        assert fhi.shape == (ncols, Mo)
+        ohi, olo = np.empty((ncols, Mn)), np.empty((ncols, Mn))
+        _check(self._f("respace")(ctypes.c_int(Mo), ctypes.c_double(old[1]), ctypes.c_int(old[2]), ctypes.c_int(Mn), ctypes.c_double(new[1]),
+                                  ctypes.c_int(new[2]), ctypes.c_int(ncols), _p(fhi), _p(flo), _p(ohi), _p(olo)), "respace")
+        return (ohi[0], olo[0]) if one else (ohi, olo)
+
     def multiplier(self, which: int, f):
         hi, lo = _split(f)
         N = hi.shape[-1]

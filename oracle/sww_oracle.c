@@ -28,7 +28,8 @@
  *   R2  API eta is the elevation about the mean level; the bottom is y=0 and the surface is
  *       y = h + eta ("absorb the mean fluid depth into eta").  The system matrix that is
  *       factored is A = I/2 + K ("LU-factorization of K").
- *   R3  uniform grid xi(alpha)=alpha (rho_1 = 1), so 1/|xi'| = 1 in (2.8).
+ *   R3  uniform grid xi(alpha)=alpha (rho_1 = 1), so 1/|xi'| = 1 in (2.8), unless set_mesh() selects a
+ *       refined mesh (2.10): then zeta = xi + i eta o xi, d/dx = (1/xi') d/dalpha, P removes the mean over x.
  *   R4  Nyquist mode (N even): symbol 0 for D, H, |D|; eta'' = D(D eta); filter factor exp(-36) there.
  *   R5  the 36th-order filter (2.14) multiplies every evaluated right-hand side and the solution after
  *       every step; flag to switch it off.
@@ -230,6 +231,36 @@ static void multiplier(const trig_t *t, int which, const REAL *f, REAL *out) {
     free(wf); free(wo);
 }
 
+/* ---------- mesh refinement: the change of variables x = xi(alpha), (2.10)-(2.11), PAPER.md:122-136 ----------
+ *   E(alpha) = 1 - P[A sin^4(alpha/2)]  (refine near x = pi)   or   1 - P[A cos^4(alpha/2)]  (refine near x = 0),
+ *   A = 8 (1 - rho) / (5 + 3 rho),  xi(alpha) = int_0^alpha E,  P removes the mean (3/8 for both fourth powers).
+ * With sin^4(a/2) = 3/8 - cos(a)/2 + cos(2a)/8 and cos^4(a/2) = 3/8 + cos(a)/2 + cos(2a)/8 the primitive is elementary:
+ *   xi - alpha = +-A sin(alpha)/2 - A sin(2 alpha)/16   (+ near pi, - near 0).
+ * The state (eta, phi and the columns) is stored at the points x_j = xi(alpha_j); rho = 1 is the uniform mesh (E = 1).
+ * The setting is process-wide (set_mesh below) and read when a surface is set up; it is not changed while a call runs. */
+static REAL g_mesh_rho = 1;
+static int g_mesh_where = 0;   /* 0: refine near x = pi, 1: refine near x = 0 */
+static int mesh_on(void) { return g_mesh_rho != 1; }
+/* xp = xi - alpha, E = xi', E1 = xi'' at alpha_j = 2 pi j / N */
+static void mesh_tables(int N, REAL *xp, REAL *E, REAL *E1) {
+    REAL A = 8 * (1 - g_mesh_rho) / (5 + 3 * g_mesh_rho);
+    for (int j = 0; j < N; j++) {
+        REAL ch, sh, c1, s1, c2, s2;
+        trig_exact_r(j, 2L * N, &ch, &sh);          /* alpha_j / 2 */
+        trig_exact_r(j, N, &c1, &s1);               /* alpha_j     */
+        trig_exact_r(2L * j, N, &c2, &s2);          /* 2 alpha_j   */
+        if (g_mesh_where == 0) {
+            E[j] = 1 - A * (sh * sh * sh * sh - (REAL)3 / 8);
+            E1[j] = -2 * A * sh * sh * sh * ch;
+            xp[j] = A * s1 / 2 - A * s2 / 16;
+        } else {
+            E[j] = 1 - A * (ch * ch * ch * ch - (REAL)3 / 8);
+            E1[j] = 2 * A * ch * ch * ch * sh;
+            xp[j] = -A * s1 / 2 - A * s2 / 16;
+        }
+    }
+}
+
 /* O1: eta' = D eta, eta'' = D(D eta); the intermediate eta' stays in WIDE (R8). */
 static void surface_derivs(const trig_t *t, const REAL *eta, REAL *d1, REAL *d2) {
     int N = t->N;
@@ -254,7 +285,10 @@ static void half_cot(REAL sx, REAL cx, REAL y, REAL *cr, REAL *ci) {
 }
 
 /* ---------- O1-O3: K and G from (2.13), with reading R1 ---------- */
-static int assemble(const trig_t *t, REAL h, const REAL *eta, const REAL *d1, const REAL *d2, REAL *K, REAL *G) {
+/* On a refined mesh zeta(alpha) = xi(alpha) + i eta(xi(alpha)) (2.5): zeta' = E + i d1, zeta'' = E1 + i d2 (d1, d2: alpha-derivatives
+ * of the stored values) and Re(zeta_i - zeta_j) = (alpha_i - alpha_j) + (xp_i - xp_j); xp = NULL is the uniform mesh. */
+static int assemble(const trig_t *t, REAL h, const REAL *eta, const REAL *d1, const REAL *d2,
+                    const REAL *xp, const REAL *E, const REAL *E1, REAL *K, REAL *G) {
     int N = t->N;
     int finite = !R_ISINF(h);
     if (finite) for (int i = 0; i < N; i++) if (!(h + eta[i] > 0)) return ORC_EBOTTOM;
@@ -268,21 +302,29 @@ static int assemble(const trig_t *t, REAL h, const REAL *eta, const REAL *d1, co
             int m = ((i - j) % N + N) % N;
             REAL sx = t->s[m], cx = t->c[m];
             REAL k1, g1, k2 = 0, g2 = 0, cr, ci;
+            REAL Ei = xp ? E[i] : 1, Ej = xp ? E[j] : 1;
+            if (xp) {                                    /* sin, cos of (alpha_i - alpha_j) + (xp_i - xp_j) */
+                REAL dl = xp[i] - xp[j], sd = R_SIN(dl), cd = R_COS(dl);
+                REAL s0 = sx, c0m = cx;
+                sx = s0 * cd + c0m * sd;
+                cx = c0m * cd - s0 * sd;
+            }
             if (i != j) {
                 REAL y1 = eta[i] - eta[j];               /* Im(zeta_i - zeta_j), from the raw inputs */
                 half_cot(sx, cx, y1, &cr, &ci);
-                k1 = ci + d1[j] * cr;                    /* Im{ zeta'_j/2 cot } ; zeta' = 1 + i eta' */
-                g1 = cr - d1[i] * ci - c0[m];            /* Re{ zeta'_i/2 cot } - (1/2)cot(x/2)      */
+                k1 = Ej * ci + d1[j] * cr;               /* Im{ zeta'_j/2 cot } ; zeta' = E + i eta~' (E = 1: uniform) */
+                g1 = Ei * cr - d1[i] * ci - c0[m];       /* Re{ zeta'_i/2 cot } - (1/2)cot((alpha_i - alpha_j)/2)       */
             } else {                                     /* continuous limits */
-                REAL den = 2 * (1 + d1[i] * d1[i]);
-                k1 = -d2[i] / den;                       /* -Im{ zeta''/(2 zeta') }, zeta'' = i eta'' */
-                g1 = d1[i] * d2[i] / den;                /*  Re{ zeta''/(2 zeta') }                  */
+                REAL den = 2 * (Ei * Ei + d1[i] * d1[i]);
+                REAL Ep = xp ? E1[i] : 0;                /* zeta'' = E' + i eta~'' */
+                k1 = -(d2[i] * Ei - Ep * d1[i]) / den;   /* -Im{ zeta''/(2 zeta') } = -Im{ zeta'' conj(zeta') } / (2 |zeta'|^2) */
+                g1 = (Ep * Ei + d1[i] * d2[i]) / den;    /*  Re{ zeta''/(2 zeta') }                  */
             }
             if (finite) {
                 REAL y2 = (h + eta[i]) + (h + eta[j]);   /* Im(zeta_i - conj zeta_j) > 0 */
                 half_cot(sx, cx, y2, &cr, &ci);
-                k2 = ci - d1[j] * cr;                    /* Im{ conj(zeta'_j)/2 cot } */
-                g2 = cr - d1[i] * ci;                    /* Re{ zeta'_i/2 cot }       */
+                k2 = Ej * ci - d1[j] * cr;               /* Im{ conj(zeta'_j)/2 cot } */
+                g2 = Ei * cr - d1[i] * ci;               /* Re{ zeta'_i/2 cot }       */
             }
             K[(long)i * N + j] = (k1 - k2) / (REAL)N;    /* R1 */
             G[(long)i * N + j] = (g1 - g2) / (REAL)N;
@@ -326,10 +368,12 @@ typedef struct {
     int N; REAL h; trig_t t;
     REAL *eta, *d1, *d2;   /* eta, eta', eta'' */
     REAL *K, *G, *LU; int *piv;
+    REAL *xp, *E, *E1;     /* mesh (2.10): xi - alpha, xi', xi''; NULL on the uniform mesh */
 } setup_t;
 
 static void setup_free(setup_t *s) {
     trig_free(&s->t); free(s->eta); free(s->d1); free(s->d2); free(s->K); free(s->G); free(s->LU); free(s->piv);
+    free(s->xp); free(s->E); free(s->E1);
 }
 static int setup_make(setup_t *s, int N, REAL h, const REAL *eta) {
     memset(s, 0, sizeof(*s));
@@ -342,7 +386,12 @@ static int setup_make(setup_t *s, int N, REAL h, const REAL *eta) {
     if (!s->eta || !s->d1 || !s->d2 || !s->K || !s->G || !s->LU || !s->piv) { setup_free(s); return ORC_ENOMEM; }
     memcpy(s->eta, eta, sizeof(REAL) * N);
     surface_derivs(&s->t, s->eta, s->d1, s->d2);  /* O1: eta', eta'' = D(D eta)  (R8) */
-    rc = assemble(&s->t, h, s->eta, s->d1, s->d2, s->K, s->G); if (rc) { setup_free(s); return rc; }
+    if (mesh_on()) {
+        s->xp = ralloc(N); s->E = ralloc(N); s->E1 = ralloc(N);
+        if (!s->xp || !s->E || !s->E1) { setup_free(s); return ORC_ENOMEM; }
+        mesh_tables(N, s->xp, s->E, s->E1);
+    }
+    rc = assemble(&s->t, h, s->eta, s->d1, s->d2, s->xp, s->E, s->E1, s->K, s->G); if (rc) { setup_free(s); return rc; }
     for (long i = 0; i < (long)N * N; i++) s->LU[i] = s->K[i];
     for (int i = 0; i < N; i++) s->LU[(long)i * N + i] += (REAL)0.5;   /* A = I/2 + K, (2.7) PAPER.md:105 */
     rc = lu_factor(N, s->LU, s->piv); if (rc) { setup_free(s); return rc; }
@@ -359,8 +408,26 @@ static void dtn_one(const setup_t *s, const REAL *b, REAL *w, REAL *mu_out) {
     multiplier(&s->t, MUL_H, gam, hg);
     matvec(N, s->G, gam, w);
     for (int i = 0; i < N; i++) w[i] += hg[i] / 2;
+    if (s->E) for (int i = 0; i < N; i++) w[i] /= s->E[i];      /* the factor 1/|xi'(alpha)| of (2.8) */
     if (mu_out) memcpy(mu_out, mu, sizeof(REAL) * N);
     free(mu); free(gam); free(hg);
+}
+
+/* d/dx of a function stored on the mesh: (1/xi') d/dalpha  (chain rule for f(xi(alpha))) */
+static void deriv_x(const setup_t *s, const REAL *f, REAL *out) {
+    multiplier(&s->t, MUL_D, f, out);
+    if (s->E) for (int i = 0; i < s->N; i++) out[i] /= s->E[i];
+}
+/* P (2.2) and the filter (2.14) on the mesh: the filter acts on the stored samples (Fourier modes in alpha); the mean that P
+ * removes is the mean over x, (1/2pi) int f dx = (1/N) sum_j f_j E_j by the trapezoidal rule with dx = E dalpha. */
+static void project_x(const setup_t *s, int filter, const REAL *r, REAL *out) {
+    int N = s->N;
+    if (!s->E) { multiplier(&s->t, filter ? MUL_PFILTER : MUL_P, r, out); return; }
+    if (filter) multiplier(&s->t, MUL_FILTER, r, out); else memcpy(out, r, sizeof(REAL) * N);
+    REAL m = 0;
+    for (int i = 0; i < N; i++) m += out[i] * s->E[i];
+    m /= (REAL)N;
+    for (int i = 0; i < N; i++) out[i] -= m;
 }
 
 /* O6: base state about which the problem is linearised; (2.9) PAPER.md:116 */
@@ -369,10 +436,10 @@ static void base_free(base_t *b) { free(b->dphi); free(b->W0); free(b->u); free(
 static void base_make(const setup_t *s, const REAL *phi0, base_t *b) {
     int N = s->N;
     b->dphi = ralloc(N); b->W0 = ralloc(N); b->u = ralloc(N); b->v = ralloc(N);
-    multiplier(&s->t, MUL_D, phi0, b->dphi);
+    deriv_x(s, phi0, b->dphi);
     dtn_one(s, phi0, b->W0, NULL);
     for (int i = 0; i < N; i++) {
-        REAL e1 = s->d1[i], den = 1 + e1 * e1;
+        REAL e1 = s->E ? s->d1[i] / s->E[i] : s->d1[i], den = 1 + e1 * e1;   /* eta'(x) */
         b->u[i] = (b->dphi[i] - e1 * b->W0[i]) / den;     /* phi_x */
         b->v[i] = (e1 * b->dphi[i] + b->W0[i]) / den;     /* phi_y */
     }
@@ -447,7 +514,7 @@ int NAME(dtn_linearized)(int N, double h, const double *ehi, const double *elo,
         load_hl(dp, dphi + (long)c * N, dplo ? dplo + (long)c * N : NULL, N);
         for (int i = 0; i < N; i++) { b[i] = dp[i] - bs.v[i] * de[i]; ud[i] = bs.u[i] * de[i]; }
         dtn_one(&s, b, w, NULL);
-        multiplier(&s.t, MUL_D, ud, dud);
+        deriv_x(&s, ud, dud);
         for (int i = 0; i < N; i++) w[i] -= dud[i];
         store_hl(w, out_hi + (long)c * N, out_lo ? out_lo + (long)c * N : NULL, N);
         free(de); free(dp); free(b); free(w); free(ud); free(dud);
@@ -472,15 +539,15 @@ static int rhs_eval(int N, REAL h, REAL g, REAL sigma, int filter, const REAL *e
     for (int i = 0; i < N; i++) tmp[i] = bs.v[i] * bs.W0[i] - bs.u[i] * bs.u[i] / 2 - bs.v[i] * bs.v[i] / 2 - g * eta[i];
     if (sigma != 0) {
         REAL *cv = ralloc(N), *dcv = ralloc(N);
-        for (int i = 0; i < N; i++) cv[i] = s.d1[i] / R_SQRT(1 + s.d1[i] * s.d1[i]);
-        multiplier(&s.t, MUL_D, cv, dcv);
+        for (int i = 0; i < N; i++) { REAL e1 = s.E ? s.d1[i] / s.E[i] : s.d1[i]; cv[i] = e1 / R_SQRT(1 + e1 * e1); }
+        deriv_x(&s, cv, dcv);
         for (int i = 0; i < N; i++) tmp[i] += sigma * dcv[i];
         free(cv); free(dcv);
     }
     if (eta_t) { if (filter) multiplier(&s.t, MUL_FILTER, bs.W0, eta_t); else memcpy(eta_t, bs.W0, sizeof(REAL) * N); }
-    if (phi_t) multiplier(&s.t, filter ? MUL_PFILTER : MUL_P, tmp, phi_t);
-    if (energy) {   /* E = (1/2) int (phi G phi + g eta^2) dx */
-        REAL e = 0; for (int i = 0; i < N; i++) e += phi[i] * bs.W0[i] + g * eta[i] * eta[i];
+    if (phi_t) project_x(&s, filter, tmp, phi_t);
+    if (energy) {   /* E = (1/2) int (phi G phi + g eta^2) dx; dx = xi' dalpha on a refined mesh */
+        REAL e = 0; for (int i = 0; i < N; i++) e += (phi[i] * bs.W0[i] + g * eta[i] * eta[i]) * (s.E ? s.E[i] : 1);
         *energy = e * R_PI / (REAL)N;
     }
     free(tmp);
@@ -491,20 +558,20 @@ static int rhs_eval(int N, REAL h, REAL g, REAL sigma, int filter, const REAL *e
         for (int i = 0; i < N; i++) b[i] = dp[i] - bs.v[i] * de[i];
         dtn_one(&s, b, w, NULL);
         for (int i = 0; i < N; i++) t1[i] = bs.u[i] * de[i];
-        multiplier(&s.t, MUL_D, t1, t2);
+        deriv_x(&s, t1, t2);
         for (int i = 0; i < N; i++) r[i] = w[i] - t2[i];
         if (filter) multiplier(&s.t, MUL_FILTER, r, deta_t + (long)c * N); else memcpy(deta_t + (long)c * N, r, sizeof(REAL) * N);
         for (int i = 0; i < N; i++) t1[i] = de[i] * bs.u[i] * bs.v[i];
-        multiplier(&s.t, MUL_D, t1, t2);
-        multiplier(&s.t, MUL_D, b, db);
+        deriv_x(&s, t1, t2);
+        deriv_x(&s, b, db);
         for (int i = 0; i < N; i++) r[i] = -t2[i] - bs.u[i] * db[i] + bs.v[i] * w[i] - g * de[i];
         if (sigma != 0) {
-            multiplier(&s.t, MUL_D, de, t1);
-            for (int i = 0; i < N; i++) { REAL den = 1 + s.d1[i] * s.d1[i]; t1[i] = t1[i] / (den * R_SQRT(den)); }
-            multiplier(&s.t, MUL_D, t1, t2);
+            deriv_x(&s, de, t1);
+            for (int i = 0; i < N; i++) { REAL e1 = s.E ? s.d1[i] / s.E[i] : s.d1[i], den = 1 + e1 * e1; t1[i] = t1[i] / (den * R_SQRT(den)); }
+            deriv_x(&s, t1, t2);
             for (int i = 0; i < N; i++) r[i] += sigma * t2[i];
         }
-        multiplier(&s.t, filter ? MUL_PFILTER : MUL_P, r, dphi_t + (long)c * N);
+        project_x(&s, filter, r, dphi_t + (long)c * N);
         free(b); free(w); free(t1); free(t2); free(db); free(r);
     }
     base_free(&bs); setup_free(&s);
@@ -536,6 +603,7 @@ int NAME(rhs)(int N, double h, double g, double sigma, int filter, const double 
  * (no filter: the adjoint identity <DF(q) qdot, q~> = <qdot, DF(q)^* q~> is stated for the unfiltered operators). */
 static int adjoint_eval(int N, REAL h, REAL g, REAL sigma, const REAL *eta, const REAL *phi, int ncols,
                         const REAL *etat, const REAL *phit, REAL *eta_s, REAL *phi_s) {
+    if (mesh_on()) return ORC_EINVAL;   /* (B.6) is written out here for the uniform mesh only */
     setup_t s; int rc = setup_make(&s, N, h, eta); if (rc) return rc;
     base_t bs; base_make(&s, phi, &bs);
     REAL *du = ralloc(N);
@@ -823,6 +891,71 @@ int NAME(sdc_advance)(int N, double h, double g, double sigma, int filter, doubl
 }
 
 /* thread count of the following calls (no arithmetic: small problems run faster on one thread than through the OpenMP barriers) */
+/* ---------- mesh refinement: setting, tables, respacing (2.10)-(2.11), PAPER.md:122-136 ---------- */
+/* rho in (0, 1]; where = 0 refines near x = pi, 1 near x = 0.  rho = 1: the uniform mesh. */
+int NAME(set_mesh)(double rho, int where) {
+    if (!(rho > 0 && rho <= 1) || (where != 0 && where != 1)) return ORC_EINVAL;
+    g_mesh_rho = (REAL)rho; g_mesh_where = where;
+    return ORC_OK;
+}
+/* xi(alpha_j) - alpha_j, E = xi', E1 = xi'' of the current setting at alpha_j = 2 pi j / N */
+int NAME(mesh_tables)(int N, double *xp_hi, double *xp_lo, double *E_hi, double *E_lo, double *E1_hi, double *E1_lo) {
+    REAL *xp = ralloc(N), *E = ralloc(N), *E1 = ralloc(N);
+    mesh_tables(N, xp, E, E1);
+    store_hl(xp, xp_hi, xp_lo, N); store_hl(E, E_hi, E_lo, N); store_hl(E1, E1_hi, E1_lo, N);
+    free(xp); free(E); free(E1);
+    return ORC_OK;
+}
+/* xi(b) and xi'(b) at an arbitrary parameter value b */
+static void mesh_xi(REAL rho, int where, REAL b, REAL *xi, REAL *E) {
+    REAL A = 8 * (1 - rho) / (5 + 3 * rho), sg = where == 0 ? 1 : -1;
+    *xi = b + sg * A * R_SIN(b) / 2 - A * R_SIN(2 * b) / 16;
+    *E = 1 + sg * A * R_COS(b) / 2 - A * R_COS(2 * b) / 8;
+}
+/* Respacing from segment l to l+1: f o xi_new(alpha_j) = (f o xi_old)(beta_j), beta_j = xi_old^{-1}(xi_new(alpha_j))
+ * by Newton's method, alpha_j = 2 pi j / Mn; f o xi_old is evaluated at beta_j through its trigonometric interpolant on the
+ * old mesh (Mo points): a_k, b_k as in the multipliers above, the Nyquist mode as a cosine.  Columns of f at c*Mo, of out at c*Mn. */
+int NAME(respace)(int Mo, double rho_o, int where_o, int Mn, double rho_n, int where_n, int ncols,
+                  const double *fhi, const double *flo, double *ohi, double *olo) {
+    if (Mo < 4 || Mn < 4 || (Mo & 1)) return ORC_EINVAL;
+    REAL *beta = ralloc(Mn);
+    for (int j = 0; j < Mn; j++) {
+        REAL al = 2 * R_PI * (REAL)j / (REAL)Mn, x, e, b, xb, eb;
+        mesh_xi((REAL)rho_n, where_n, al, &x, &e);
+        b = x;
+        for (int it = 0; it < 60; it++) {
+            mesh_xi((REAL)rho_o, where_o, b, &xb, &eb);
+            REAL step = (xb - x) / eb;
+            b -= step;
+            if (step == 0) break;
+        }
+        beta[j] = b;
+    }
+#pragma omp parallel for schedule(dynamic) if (ncols > 1)
+    for (int c = 0; c < ncols; c++) {
+        REAL *f = ralloc(Mo), *a = ralloc(Mo / 2 + 1), *bb = ralloc(Mo / 2 + 1), *o = ralloc(Mn);
+        load_hl(f, fhi + (long)c * Mo, flo ? flo + (long)c * Mo : NULL, Mo);
+        for (int k = 0; k <= Mo / 2; k++) {
+            REAL sa = 0, sb = 0;
+            for (int j = 0; j < Mo; j++) {
+                REAL cc, ss; trig_exact_r((long)k * j, Mo, &cc, &ss);
+                sa += f[j] * cc; sb += f[j] * ss;
+            }
+            a[k] = sa / (REAL)Mo; bb[k] = sb / (REAL)Mo;
+        }
+        for (int j = 0; j < Mn; j++) {
+            REAL v = a[0];
+            for (int k = 1; k < Mo / 2; k++) v += 2 * (a[k] * R_COS(k * beta[j]) + bb[k] * R_SIN(k * beta[j]));
+            v += a[Mo / 2] * R_COS((Mo / 2) * beta[j]);
+            o[j] = v;
+        }
+        store_hl(o, ohi + (long)c * Mn, olo ? olo + (long)c * Mn : NULL, Mn);
+        free(f); free(a); free(bb); free(o);
+    }
+    free(beta);
+    return ORC_OK;
+}
+
 void NAME(set_num_threads)(int n) {
 #ifdef _OPENMP
     if (n > 0) omp_set_num_threads(n);
