@@ -129,6 +129,27 @@ int sww_state_read(sww_state_t s, void* eta, void* phi, void* deta, void* dphi, 
 int sww_state_energy(sww_state_t s, double* energy_hl);
 int sww_state_destroy(sww_state_t s);
 
+/* ---- mesh refinement in space, section 2.2 (2.10)-(2.11), PAPER.md:122-136 ------------------------------------------------
+ * The change of variables x = xi(alpha):  xi' = E = 1 - P[A sin^4(alpha/2)] (where = 0: refine near x = pi) or 1 - P[A cos^4(alpha/2)]
+ * (where = 1: refine near x = 0), A = 8 (1 - rho) / (5 + 3 rho), 0 < rho <= 1 the ratio of the smallest to the largest spacing (2.11);
+ * rho = 1 is the uniform mesh.  After sww_dtn_set_mesh every array of the handle (eta, phi, the columns, every output) holds values at
+ * the points x_j = xi(alpha_j), alpha_j = 2 pi j / N: zeta = xi + i eta o xi in (2.13), the factor 1/|xi'| in (2.8), d/dx =
+ * (1/xi') d/dalpha in (2.9), (B.2).  The call invalidates the surface: follow it with sww_dtn_refactor.  Views 2, 3 of sww_dtn_get stay
+ * alpha-derivatives of the stored eta; 4..7 (phi0', W0, u, v) are the physical quantities.  Either precision.
+ * Not on a refined mesh: sww_dtn_adjoint_rhs and sww_dtn_linearized_host (SWW_EINVAL / uniform only).
+ * sww_mesh_points: x (HOST, N doubles) <- xi(alpha_j). */
+int sww_dtn_set_mesh(sww_dtn_t d, double rho, int where);
+int sww_mesh_points(int N, double rho, int where, double* x);
+/* The time stepper on a refined mesh (SWW_F64 states only; SWW_DD: SWW_EINVAL unless rho = 1): the filter (2.14) acts on the stored
+ * samples, P removes the mean over x, (1/N) sum_j f_j xi'(alpha_j) (the trapezoidal rule with dx = xi' dalpha), and the
+ * energy integral carries the same weight.  Call before advancing; the state's arrays are then values at x_j.
+ * sww_state_respace: dst's state (eta, phi and all columns) <- src's, interpolated to dst's mesh: beta_j =
+ * xi_src^{-1}(xi_dst(alpha_j)) by Newton's method in double-double, values at beta_j from the trigonometric interpolant of src's samples
+ * (one M_dst x M_src matrix applied to all 2 + 2 ncols columns at once).  dst and src: two SWW_F64 handles with the same ncols and
+ * any two sizes and meshes; dst's elapsed time becomes src's.  Synchronises both streams. */
+int sww_state_set_mesh(sww_state_t s, double rho, int where);
+int sww_state_respace(sww_state_t dst, sww_state_t src);
+
 /* ---- shooting map of the overdetermined shooting method, uniform mesh (section 3.1 / 3.3) ------------------------
  * Unknowns c (HOST, n + 1 doubles): c[0] = T, the period (3.16); c[k], 1 <= k <= n, the Fourier modes of the initial
  * state (3.15): eta(x, 0) = sum_{k even} 2 c_k cos kx, phi(x, 0) = sum_{k odd} 2 c_k cos kx (eta about the mean level).

@@ -19,6 +19,7 @@ EXPORTS = [
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
     "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance", "sww_dtn_adjoint_rhs", "sww_shooter_set_method",
+    "sww_dtn_set_mesh", "sww_mesh_points", "sww_state_set_mesh", "sww_state_respace",
 ]
 
 
@@ -97,6 +98,10 @@ def lib() -> ctypes.CDLL:
         L.sww_shooter_dims.argtypes = [vp, ctypes.POINTER(ci), ctypes.POINTER(ci), ctypes.POINTER(ci)]
         L.sww_lm_minimize.argtypes = [LM_FUN, vp, ci, ci, ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(LmOptions), ctypes.POINTER(LmReport)]
         L.sww_lm_shoot.argtypes = [vp, ctypes.POINTER(cd), ctypes.POINTER(ci), ci, ctypes.POINTER(LmOptions), ctypes.POINTER(LmReport)]
+        L.sww_dtn_set_mesh.argtypes = [vp, cd, ci]
+        L.sww_mesh_points.argtypes = [ci, cd, ci, ctypes.POINTER(cd)]
+        L.sww_state_set_mesh.argtypes = [vp, cd, ci]
+        L.sww_state_respace.argtypes = [vp, vp]
         L.sww_timing_enable.argtypes = [ci]
         L.sww_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_ulonglong), ci]
         _LIB = L
@@ -181,6 +186,10 @@ class DtN:
     def refactor(self, eta: torch.Tensor):
         _check(lib().sww_dtn_refactor(self._h, _dev(eta, self.N * self.mul, "eta")), "sww_dtn_refactor")
 
+    def set_mesh(self, rho: float, where: int = 0):
+        """sww_dtn_set_mesh: the refined mesh (2.10); follow with refactor(eta) (values at the points mesh_points(N, rho, where))"""
+        _check(lib().sww_dtn_set_mesh(self._h, float(rho), int(where)), "sww_dtn_set_mesh")
+
     def apply(self, phi: torch.Tensor, out: torch.Tensor | None = None) -> torch.Tensor:
         nrhs = phi.numel() // (self.N * self.mul)
         if out is None:
@@ -263,6 +272,13 @@ class State:
 
     def set_sigma(self, sigma: float):
         _check(lib().sww_state_set_sigma(self._h, float(sigma)), "sww_state_set_sigma")
+
+    def set_mesh(self, rho: float, where: int = 0):
+        _check(lib().sww_state_set_mesh(self._h, float(rho), int(where)), "sww_state_set_mesh")
+
+    def respace_from(self, src: "State"):
+        """sww_state_respace: this state <- src's, interpolated to this handle's mesh"""
+        _check(lib().sww_state_respace(self._h, src._h), "sww_state_respace")
 
     def advance(self, dt: float, nsteps: int, method: str = "rk8"):
         """method: "rk8" (sww_rk_advance) or "sdc15" (sww_sdc_advance, the paper's quadruple-precision stepper)"""
@@ -383,6 +399,14 @@ def lm_minimize(fun, c0, M: int, fixed=None, **opts):
     opt, rep = _lm_options(**opts), LmReport()
     _check(lib().sww_lm_minimize(LM_FUN(cb), None, int(M), ntot, cc, fx, ctypes.byref(opt), ctypes.byref(rep)), "sww_lm_minimize")
     return np.array(list(cc)), _lm_report(rep)
+
+
+def mesh_points(N: int, rho: float, where: int = 0):
+    """sww_mesh_points: x_j = xi(alpha_j) of the mesh (2.10) as a numpy array (host)"""
+    import numpy as np
+    x = np.empty(N)
+    _check(lib().sww_mesh_points(int(N), float(rho), int(where), x.ctypes.data_as(ctypes.POINTER(ctypes.c_double))), "sww_mesh_points")
+    return x
 
 
 def dtn_linearized_host(eta, phi0, deta, dphi, h: float, prec: int = F64, out=None):

@@ -255,6 +255,7 @@ using namespace sww;
 
 extern "C" int sww_dtn_adjoint_rhs(sww_dtn_t d, const void* eta_t, const void* phi_t, int nrhs, double g, double sigma, void* eta_s, void* phi_s) {
     if (!d || nrhs < 0 || !(sigma >= 0.0)) return SWW_EINVAL;
+    if (d->mesh_on) return SWW_EINVAL;  // (B.6) is implemented for the uniform mesh
     if (!d->has_base) return SWW_ENOBASE;
     if (nrhs == 0) return SWW_OK;
     if (!eta_t || !phi_t || !eta_s || !phi_s || eta_s == phi_s || eta_s == eta_t || eta_s == phi_t || phi_s == eta_t || phi_s == phi_t)

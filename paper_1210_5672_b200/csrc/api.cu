@@ -58,7 +58,7 @@ static int apply_f64(sww_dtn_s* d, const double* rhs_dev /* N x nrhs, or NULL wh
         SWW_TRY(gemv_few_f64(d->stream, N, nrhs, N, d->G, N, w.Gam, N, out, N, d->bp_part, d->mv_count));
     else
         SWW_TRY(gemm_f64(d->stream, N, nrhs, N, 1.0, d->G, N, w.Gam, N, 1.0, out, N, nrhs));
-    return SWW_OK;
+    return mesh_scale_out(d, out, nrhs, 0);  // the factor 1/|xi'| of (2.8) on a refined mesh
 }
 
 
@@ -195,6 +195,7 @@ int sww_dtn_destroy(sww_dtn_t d) {
     double* ptrs[] = {d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, d->K, d->G, d->LU, d->invD, d->bphi, d->bW0, d->bu, d->bv, d->tmp, d->bp_part,
                       d->ws.B, d->ws.Gam, d->ws.W, d->ws.T, d->ws.R, d->ws.S};
     for (double* p : ptrs) cudaFree(p);
+    cudaFree(d->mesh_buf);
     cudaFree(d->status);
     cudaFree(d->mv_count);
     cudaFree(d->lu_order);

@@ -171,14 +171,30 @@ __device__ __forceinline__ void sinhcosh_f64(double y, double* sh, double* ch) {
 constexpr int ASM_TI = 128;  // rows (targets i) per block = threads per block
 constexpr int ASM_TJ = 32;   // columns (sources j) per block
 
-template <bool FINITE, int TJ>
+// sin, cos of delta = p_i - p_j (p = xi - alpha) from the per-node double-double tables S = sin p, C = cos p: the difference
+// S_i C_j - C_i S_j cancels next to the diagonal, so the products are taken exactly and the low words are carried -- the
+// x-differences of a refined mesh are then as accurate as the exact tables of the uniform one.
+__device__ __forceinline__ void mesh_delta(double Si, double Sil, double Ci, double Cil, double Sj, double Sjl, double Cj, double Cjl,
+                                           double* sd, double* cd) {
+    const double p = Ci * Sj, e = fma(Ci, Sj, -p);
+    const double low = fma(Sil, Cj, Si * Cjl) - fma(Cil, Sj, Ci * Sjl);
+    *sd = (fma(Si, Cj, -p) - e) + low;
+    *cd = fma(Ci, Cj, Si * Sj);
+}
+// sin^2(x/2) from sin x, cos x without cancellation
+__device__ __forceinline__ double half_angle_sq(double sx, double cx) { return cx >= 0.0 ? sx * sx / (2.0 * (1.0 + cx)) : 0.5 * (1.0 - cx); }
+
+// MESH: the refined mesh x = xi(alpha) of (2.10) (mesh.cu): zeta' = xE + i d1, zeta'' = xE1 + i d2, Re(zeta_i - zeta_j) =
+// (alpha_i - alpha_j) + (p_i - p_j); the regularizing cot((alpha_i - alpha_j)/2) of (2.13) keeps the uniform table.
+template <bool FINITE, int TJ, bool MESH>
 __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __restrict__ eta, const double* __restrict__ d1,
                                                          const double* __restrict__ d2, const double* __restrict__ E,
                                                          const double* __restrict__ Dm, const double* __restrict__ cs,
                                                          const double* __restrict__ sn, const double* __restrict__ c0,
-                                                         const double* __restrict__ s2, double* __restrict__ K,
+                                                         const double* __restrict__ s2, MeshDev ms, double* __restrict__ K,
                                                          double* __restrict__ G, double* __restrict__ LU) {
     __shared__ double s_eta[TJ], s_d1[TJ], s_E[TJ], s_Dm[TJ];
+    __shared__ double s_xE[MESH ? TJ : 1], s_xS[MESH ? 2 * TJ : 1], s_xC[MESH ? 2 * TJ : 1];
     __shared__ double s_cs[ASM_TI + TJ], s_sn[ASM_TI + TJ], s_c0[ASM_TI + TJ], s_s2[ASM_TI + TJ];
     const int tid = threadIdx.x, mask = N - 1;
     const int i0 = blockIdx.x * ASM_TI, j0 = blockIdx.y * TJ;
@@ -189,6 +205,11 @@ __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __
         if (FINITE) {
             s_E[tid] = E[j];
             s_Dm[tid] = Dm[j];
+        }
+        if (MESH) {
+            s_xE[tid] = ms.xE[j];
+            s_xS[tid] = ms.xS[j]; s_xS[TJ + tid] = ms.xS[N + j];
+            s_xC[tid] = ms.xC[j]; s_xC[TJ + tid] = ms.xC[N + j];
         }
     }
     // table slice: index s <-> m = (i0 - j0 - (TJ-1) + s) mod N, s = tid - jj + TJ - 1
@@ -206,11 +227,38 @@ __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __
     const double E_i = FINITE ? E[i] : 0.0, Dm_i = FINITE ? Dm[i] : 0.0;
     const double rN = 1.0 / (double)N;
     const int jmax = min(TJ, N - j0);
+    double xE_i = 1.0, xE1_i = 0.0, xS_i = 0.0, xSl_i = 0.0, xC_i = 1.0, xCl_i = 0.0;
+    if (MESH) {
+        xE_i = ms.xE[i]; xE1_i = ms.xE1[i];
+        xS_i = ms.xS[i]; xSl_i = ms.xS[N + i];
+        xC_i = ms.xC[i]; xCl_i = ms.xC[N + i];
+    }
     for (int jj = 0; jj < jmax; jj++) {
         const int j = j0 + jj, s = tid - jj + TJ - 1;
-        const double sx = s_sn[s], cx = s_cs[s], d1_j = s_d1[jj];
+        double sx = s_sn[s], cx = s_cs[s], sq = s_s2[s];
+        const double d1_j = s_d1[jj], xE_j = MESH ? s_xE[jj] : 1.0;
+        if (MESH) {
+            double sd, cd;
+            mesh_delta(xS_i, xSl_i, xC_i, xCl_i, s_xS[jj], s_xS[TJ + jj], s_xC[jj], s_xC[TJ + jj], &sd, &cd);
+            const double s0 = sx, c0m = cx;
+            sx = fma(s0, cd, c0m * sd);
+            cx = fma(c0m, cd, -s0 * sd);
+            sq = half_angle_sq(sx, cx);
+        }
         double k1, g1;
-        if (i != j) {
+        if (MESH && i != j) {
+            double y = eta_i - s_eta[jj];
+            double sh, ch;
+            sinhcosh_f64(y, &sh, &ch);
+            double p = (cx >= 0.0) ? (cx + ch) / fma(sx, sx, sh * sh) : 1.0 / (ch - cx);
+            double hp = 0.5 * p;
+            k1 = hp * fma(d1_j, sx, -xE_j * sh);                    // Im{ zeta'_j (1/2)cot }
+            g1 = fma(hp, fma(d1_i, sh, xE_i * sx), -s_c0[s]);       // Re{ zeta'_i (1/2)cot } - (1/2)cot((alpha_i - alpha_j)/2)
+        } else if (MESH) {
+            double den = 2.0 * fma(d1_i, d1_i, xE_i * xE_i);
+            k1 = -fma(d2_i, xE_i, -xE1_i * d1_i) / den;             // -Im{ zeta''/(2 zeta') }
+            g1 = fma(xE1_i, xE_i, d1_i * d2_i) / den;               //  Re{ zeta''/(2 zeta') }
+        } else if (i != j) {
             double y = eta_i - s_eta[jj];  // Im(zeta_i - zeta_j) from the raw inputs
             double sh, ch;
             sinhcosh_f64(y, &sh, &ch);
@@ -230,12 +278,12 @@ __global__ void __launch_bounds__(ASM_TI) k_assemble_f64(int N, const double* __
             //   c_r = Eij sin x / den, c_i = -(1 - Eij^2) / (2 den), den = (1 - Eij)^2 + 4 Eij sin^2(x/2)   (all terms positive)
             double Eij = E_i * s_E[jj];
             double omE = fma(E_i, s_Dm[jj], Dm_i);  // 1 - E_i E_j = Dm_i + E_i Dm_j
-            double den = fma(omE, omE, 4.0 * Eij * s_s2[s]);
+            double den = fma(omE, omE, 4.0 * Eij * sq);
             double inv = 1.0 / den;
             double cr = Eij * sx * inv;
             double ci = -0.5 * omE * (1.0 + Eij) * inv;
-            k2 = fma(-d1_j, cr, ci);  // Im{ conj(zeta'_j) (1/2)cot }
-            g2 = fma(-d1_i, ci, cr);  // Re{ zeta'_i (1/2)cot }
+            k2 = MESH ? fma(-d1_j, cr, xE_j * ci) : fma(-d1_j, cr, ci);  // Im{ conj(zeta'_j) (1/2)cot }
+            g2 = MESH ? fma(-d1_i, ci, xE_i * cr) : fma(-d1_i, ci, cr);  // Re{ zeta'_i (1/2)cot }
         }
         double kv = (k1 - k2) * rN, gv = (g1 - g2) * rN;
         size_t o = (size_t)i + (size_t)j * N;
@@ -254,6 +302,7 @@ constexpr int ASMDD_TJ = 16;
 
 struct NodeDD {  // per-node quantities of one collocation point
     dd eta, d1, d2, E, Dm, Sh, Ch;
+    dd xE, xE1, xS, xC;  // refined mesh only (MESH): xi', xi'', sin(xi - alpha), cos(xi - alpha)
 };
 struct TabDD {  // functions of m = (i - j) mod N
     dd sn, cs, c0, s2;
@@ -261,9 +310,16 @@ struct TabDD {  // functions of m = (i - j) mod N
 
 // K_ij, G_ij of (2.13) in dd (already scaled by 1/N); dist = circular distance |i-j|
 // rc: shared table of dd reciprocals 1 / (m (m + 1)) (fill_rc below) for the in-band series
-template <bool FINITE>
-__device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, const TabDD& t, int dist, double rN, const double* rc,
+template <bool FINITE, bool MESH>
+__device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, const TabDD& t0, int dist, double rN, const double* rc,
                                          dd* kv, dd* gv) {
+    TabDD t = t0;
+    if (MESH) {  // sin, cos of (alpha_i - alpha_j) + (p_i - p_j); sin^2 of half of it without cancellation
+        const dd sd = dd_sub(dd_mul(ni.xS, nj.xC), dd_mul(ni.xC, nj.xS)), cd = dd_add(dd_mul(ni.xC, nj.xC), dd_mul(ni.xS, nj.xS));
+        t.sn = dd_add(dd_mul(t0.sn, cd), dd_mul(t0.cs, sd));
+        t.cs = dd_sub(dd_mul(t0.cs, cd), dd_mul(t0.sn, sd));
+        t.s2 = t.cs.hi >= 0.0 ? dd_div(dd_sqr(t.sn), dd_mul_d(dd_add_d(t.cs, 1.0), 2.0)) : dd_half(dd_sub(dd{1.0, 0.0}, t.cs));
+    }
     dd k1, g1;
     if (dist != 0) {
         dd sh, ch;
@@ -282,8 +338,17 @@ __device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, con
         else
             p = dd_div_fast(dd{1.0, 0.0}, dd_sub(ch, t.cs));
         dd hp = dd_half(p);
-        k1 = dd_mul(hp, dd_sub(dd_mul(nj.d1, t.sn), sh));
-        g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(ni.d1, sh), t.sn)), t.c0);
+        if (MESH) {
+            k1 = dd_mul(hp, dd_sub(dd_mul(nj.d1, t.sn), dd_mul(nj.xE, sh)));
+            g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(ni.d1, sh), dd_mul(ni.xE, t.sn))), t.c0);
+        } else {
+            k1 = dd_mul(hp, dd_sub(dd_mul(nj.d1, t.sn), sh));
+            g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(ni.d1, sh), t.sn)), t.c0);
+        }
+    } else if (MESH) {
+        dd den = dd_mul_d(dd_add(dd_sqr(ni.d1), dd_sqr(ni.xE)), 2.0);
+        k1 = dd_neg(dd_div(dd_sub(dd_mul(ni.d2, ni.xE), dd_mul(ni.xE1, ni.d1)), den));
+        g1 = dd_div(dd_add(dd_mul(ni.xE1, ni.xE), dd_mul(ni.d1, ni.d2)), den);
     } else {
         dd den = dd_mul_d(dd_add_d(dd_sqr(ni.d1), 1.0), 2.0);
         k1 = dd_neg(dd_div(ni.d2, den));
@@ -297,8 +362,8 @@ __device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, con
         const double rb = rcp_normal(den.hi);  // both quotients share the reciprocal
         dd cr = dd_div_rb(dd_mul(Eij, t.sn), den, rb);
         dd ci = dd_neg(dd_half(dd_div_rb(dd_mul(omE, dd_add_d(Eij, 1.0)), den, rb)));
-        k2 = dd_sub(ci, dd_mul(nj.d1, cr));
-        g2 = dd_sub(cr, dd_mul(ni.d1, ci));
+        k2 = dd_sub(MESH ? dd_mul(nj.xE, ci) : ci, dd_mul(nj.d1, cr));
+        g2 = dd_sub(MESH ? dd_mul(ni.xE, cr) : cr, dd_mul(ni.d1, ci));
     }
     *kv = dd_mul_d(dd_sub(k1, k2), rN);
     *gv = dd_mul_d(dd_sub(g1, g2), rN);
@@ -314,8 +379,12 @@ __device__ __forceinline__ void fill_rc(double* rc, int tid) {
 }
 
 __device__ __forceinline__ NodeDD load_node(int N, int j, const double* eta, const double* d1, const double* d2, const double* E,
-                                            const double* Dm, const double* Sh, const double* Ch, bool finite) {
+                                            const double* Dm, const double* Sh, const double* Ch, bool finite, const MeshDev& ms, bool mesh) {
     NodeDD n;
+    if (mesh) {
+        n.xE = dd_load(ms.xE, N, j); n.xE1 = dd_load(ms.xE1, N, j);
+        n.xS = dd_load(ms.xS, N, j); n.xC = dd_load(ms.xC, N, j);
+    }
     n.eta = dd_load(eta, N, j);
     n.d1 = dd_load(d1, N, j);
     n.d2 = dd_load(d2, N, j);
@@ -326,13 +395,13 @@ __device__ __forceinline__ NodeDD load_node(int N, int j, const double* eta, con
     return n;
 }
 
-template <bool FINITE>
+template <bool FINITE, bool MESH>
 __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* __restrict__ eta, const double* __restrict__ d1,
                                                           const double* __restrict__ d2, const double* __restrict__ E,
                                                           const double* __restrict__ Dm, const double* __restrict__ Sh,
                                                           const double* __restrict__ Ch, const double* __restrict__ cs,
                                                           const double* __restrict__ sn, const double* __restrict__ c0,
-                                                          const double* __restrict__ s2, double* __restrict__ K,
+                                                          const double* __restrict__ s2, MeshDev ms, double* __restrict__ K,
                                                           double* __restrict__ G, double* __restrict__ LU) {
     const int tid = threadIdx.x, mask = N - 1;
     const int i0 = blockIdx.x * ASMDD_TI, j0 = blockIdx.y * ASMDD_TJ;
@@ -341,15 +410,15 @@ __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* _
     fill_rc(rc, tid);
     if (i >= N) return;
     const size_t NN = (size_t)N * N;
-    const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
+    const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
     const double rN = 1.0 / (double)N;  // exact power of two
     const int jmax = min(ASMDD_TJ, N - j0);
     for (int jj = 0; jj < jmax; jj++) {
         const int j = j0 + jj, m = (i - j) & mask;
-        const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
+        const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
         TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
         dd kv, gv;
-        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
+        entry_dd<FINITE, MESH>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
         size_t o = (size_t)i + (size_t)j * N;
         dd_store(K, NN, o, kv);
         dd_store(G, NN, o, gv);
@@ -364,28 +433,28 @@ __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* _
 // Why dd: the base-state velocities u, v are multiplied into every linearized right-hand side and differentiated twice more,
 // so their rounding noise is amplified by ~N^2/3.
 constexpr int BP_TI = 128;
-template <bool FINITE>
+template <bool FINITE, bool MESH>
 __global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const double* __restrict__ eta, const double* __restrict__ d1,
                                                         const double* __restrict__ d2, const double* __restrict__ E,
                                                         const double* __restrict__ Dm, const double* __restrict__ Sh,
                                                         const double* __restrict__ Ch, const double* __restrict__ cs,
                                                         const double* __restrict__ sn, const double* __restrict__ c0,
-                                                        const double* __restrict__ s2, const double* __restrict__ mu,
+                                                        const double* __restrict__ s2, MeshDev ms, const double* __restrict__ mu,
                                                         const double* __restrict__ gam, double* __restrict__ part) {
     const int tid = threadIdx.x, mask = N - 1;
     const int i = blockIdx.x * BP_TI + tid, j0 = blockIdx.y * jchunk;
     __shared__ double rc[64];
     fill_rc(rc, tid);
     if (i >= N) return;
-    const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
+    const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
     const double rN = 1.0 / (double)N;
     dd aK{0, 0}, aG{0, 0};
     for (int jj = 0; jj < jchunk; jj++) {
         const int j = j0 + jj, m = (i - j) & mask;  // j is uniform over the CTA: node loads broadcast
-        const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE);
+        const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
         TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
         dd kv, gv;
-        entry_dd<FINITE>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
+        entry_dd<FINITE, MESH>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
         aK = dd_fma(kv, dd_load(mu, N, j), aK);
         aG = dd_fma(gv, dd_load(gam, N, j), aG);
     }
@@ -431,10 +500,15 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
     const int nchunk = d->bp_chunks, jchunk = N / nchunk;
     dim3 grid((N + BP_TI - 1) / BP_TI, nchunk);
     SWW_BEGIN(KC_DDGEMM, d->stream);
-    if (d->finite)
-        k_base_pass_dd<true><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
-    else
-        k_base_pass_dd<false><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, mu, gam, d->bp_part);
+    const MeshDev ms = d->mesh;
+#define SWW_BP_LAUNCH(FIN, MSH) \
+    k_base_pass_dd<FIN, MSH><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, ms, mu, gam, d->bp_part)
+    if (d->mesh_on) {
+        if (d->finite) SWW_BP_LAUNCH(true, true); else SWW_BP_LAUNCH(false, true);
+    } else {
+        if (d->finite) SWW_BP_LAUNCH(true, false); else SWW_BP_LAUNCH(false, false);
+    }
+#undef SWW_BP_LAUNCH
     SWW_LAUNCHED();
     SWW_BEGIN(KC_OTHER, d->stream);
     k_base_reduce<<<(N + 31) / 32, 32 * BR_G, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
@@ -468,12 +542,19 @@ int run_setup_f64(sww_dtn_s* d) {
     const int tj = (N <= 512) ? 4 : ASM_TJ;
     dim3 grid((N + ASM_TI - 1) / ASM_TI, (N + tj - 1) / tj);
     SWW_BEGIN(KC_ASM, d->stream);
-#define SWW_ASM_LAUNCH(FIN, TJV) \
-    k_assemble_f64<FIN, TJV><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU)
-    if (d->finite) {
-        if (tj == 4) SWW_ASM_LAUNCH(true, 4); else SWW_ASM_LAUNCH(true, ASM_TJ);
+    const MeshDev ms = d->mesh;
+#define SWW_ASM_LAUNCH(FIN, TJV, MSH) \
+    k_assemble_f64<FIN, TJV, MSH><<<grid, ASM_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, t->cs, t->sn, t->c0, t->s2, ms, d->K, d->G, d->LU)
+    if (d->mesh_on) {
+        if (d->finite) {
+            if (tj == 4) SWW_ASM_LAUNCH(true, 4, true); else SWW_ASM_LAUNCH(true, ASM_TJ, true);
+        } else {
+            if (tj == 4) SWW_ASM_LAUNCH(false, 4, true); else SWW_ASM_LAUNCH(false, ASM_TJ, true);
+        }
+    } else if (d->finite) {
+        if (tj == 4) SWW_ASM_LAUNCH(true, 4, false); else SWW_ASM_LAUNCH(true, ASM_TJ, false);
     } else {
-        if (tj == 4) SWW_ASM_LAUNCH(false, 4); else SWW_ASM_LAUNCH(false, ASM_TJ);
+        if (tj == 4) SWW_ASM_LAUNCH(false, 4, false); else SWW_ASM_LAUNCH(false, ASM_TJ, false);
     }
 #undef SWW_ASM_LAUNCH
     SWW_LAUNCHED();
@@ -487,10 +568,15 @@ int run_setup_dd(sww_dtn_s* d) {
     const Tables* t = d->tab;
     dim3 grid((N + ASMDD_TI - 1) / ASMDD_TI, (N + ASMDD_TJ - 1) / ASMDD_TJ);
     SWW_BEGIN(KC_ASM, d->stream);
-    if (d->finite)
-        k_assemble_dd<true><<<grid, ASMDD_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
-    else
-        k_assemble_dd<false><<<grid, ASMDD_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, d->K, d->G, d->LU);
+    const MeshDev ms = d->mesh;
+#define SWW_ASMDD_LAUNCH(FIN, MSH) \
+    k_assemble_dd<FIN, MSH><<<grid, ASMDD_TI, 0, d->stream>>>(N, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, ms, d->K, d->G, d->LU)
+    if (d->mesh_on) {
+        if (d->finite) SWW_ASMDD_LAUNCH(true, true); else SWW_ASMDD_LAUNCH(false, true);
+    } else {
+        if (d->finite) SWW_ASMDD_LAUNCH(true, false); else SWW_ASMDD_LAUNCH(false, false);
+    }
+#undef SWW_ASMDD_LAUNCH
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

@@ -71,6 +71,15 @@ struct Tables {
 };
 int get_tables(int N, cudaStream_t st, const Tables** out);
 
+// ---------------------------------------------------------------- mesh refinement (2.10), PAPER.md:122-136 (mesh.cu)
+// per-node tables of the change of variables x = xi(alpha), each double-double planar 2N; all nullptr on the uniform mesh
+struct MeshDev {
+    const double* xE;   // xi'(alpha_j) = E of (2.10)
+    const double* xE1;  // xi''(alpha_j)
+    const double* xS;   // sin(xi(alpha_j) - alpha_j)
+    const double* xC;   // cos(xi(alpha_j) - alpha_j)
+};
+
 // ---------------------------------------------------------------- the DtN handle
 struct Workspace {
     int cap_cols = 0;          // padded column capacity
@@ -111,6 +120,12 @@ struct sww_dtn_s {
     unsigned* mv_count;   // k_matvec_dd: arrival counters per 32-row block (zero between launches)
     double *tmp;          // 14 N doubles: dd scratch vectors of the accurate base state (ddpath.cu)
     bool has_base;
+    // mesh refinement (sww_dtn_set_mesh): E = 1 + a1 cos(alpha) + a2 cos(2 alpha); mesh_buf holds the four tables of `mesh`
+    bool mesh_on;
+    double mesh_rho, mesh_a1, mesh_a2;
+    int mesh_where;
+    double* mesh_buf;
+    sww::MeshDev mesh;
     int* status;          // device sticky status
     sww::Workspace ws;
 };
@@ -149,6 +164,8 @@ int setup_surface(sww_dtn_s* d, const double* eta, const double* eta_lo);
 int fast_base_f64(sww_dtn_s* d, const double* phi0);
 // fused dd pass (assembly.cu): res = b - mu/2 - K mu, w = G gam with the kernel entries evaluated in dd on the fly; all dd planar 2N
 int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* gam, double* res, double* res_f64, double* w);
+// refined mesh (mesh.cu): out_c <- out_c / xi' for nrhs columns (no-op on the uniform mesh); L: dd plane size (0 = N * nrhs)
+int mesh_scale_out(sww_dtn_s* d, double* out, int nrhs, size_t L);
 // spectral (fft.cu)
 enum SpecMode { SPEC_APPLY = 0, SPEC_LIN = 1 };
 // For each column c < ncols: Gam_c = D M_c ;  W_c = |D| M_c / 2  - (T ? D T_c : 0)

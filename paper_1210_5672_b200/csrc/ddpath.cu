@@ -364,15 +364,22 @@ __global__ void k_dd_copy(size_t n, size_t Ls, size_t Ld, int has_lo, const doub
 }
 // (2.9), in dd
 // W0 = Wa (+ Wb when given; stored to W0out) and the surface velocities (2.9) from it
-__global__ void k_base_uv_dd(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* Wa, const double* Wb,
-                             double* W0out, double* __restrict__ u, double* __restrict__ v) {
+// xE (refined mesh, else nullptr): the inputs are alpha-derivatives and the bracket of (2.8); eta'(x) = d1 / xi', phi'(x) = dphi / xi',
+// G phi = W / |xi'|, and phi' and G phi are stored back in that form (dphi_out, W0out)
+__global__ void k_base_uv_dd(int N, const double* __restrict__ d1, const double* dphi, const double* Wa, const double* Wb,
+                             double* W0out, double* __restrict__ u, double* __restrict__ v, const double* __restrict__ xE, double* dphi_out) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     dd e1 = dd_load(d1, N, j), p = dd_load(dphi, N, j), w = dd_load(Wa, N, j);
-    if (Wb) {
-        w = dd_add(w, dd_load(Wb, N, j));
-        dd_store(W0out, N, j, w);
+    if (Wb) w = dd_add(w, dd_load(Wb, N, j));
+    if (xE) {
+        const dd e = dd_load(xE, N, j);
+        e1 = dd_div(e1, e);
+        p = dd_div(p, e);
+        w = dd_div(w, e);
+        dd_store(dphi_out, N, j, p);
     }
+    if (Wb || xE) dd_store(W0out, N, j, w);
     dd den = dd_add_d(dd_sqr(e1), 1.0);
     dd_store(u, N, j, dd_div(dd_sub(p, dd_mul(e1, w)), den));
     dd_store(v, N, j, dd_div(dd_add(dd_mul(e1, p), w), den));
@@ -575,8 +582,9 @@ int accurate_base(sww_dtn_s* d, const double* phi0, size_t phi_plane) {
     }
     if (isdd) SWW_TRY(circ_dd(d, 0, b, d->bphi));                                          // phi0' (fp64 handles: done with gam~ above)
     SWW_BEGIN(KC_OTHER, st);
-    if (isdd) k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, d->bW0, nullptr, nullptr, d->bu, d->bv);
-    else k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, res, wt, d->bW0, d->bu, d->bv);   // W0 = res + w~ (2.8), then u, v
+    const double* xE = d->mesh_on ? d->mesh.xE : nullptr;
+    if (isdd) k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, d->bW0, nullptr, d->bW0, d->bu, d->bv, xE, d->bphi);
+    else k_base_uv_dd<<<blocks, 256, 0, st>>>(N, d->d1, d->bphi, res, wt, d->bW0, d->bu, d->bv, xE, d->bphi);   // W0 = res + w~ (2.8), then u, v
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -589,10 +597,15 @@ int accurate_base(sww_dtn_s* d, const double* phi0, size_t phi_plane) {
 // rounding noise of the first-order operator (~2 N eps) stays three digits under the parity bar (SURVEY.md section 0, fact 4:
 // fp64 against long double over config 2's full period: 3e-14 / 2e-13).
 __global__ void k_base_uv_f64(int N, const double* __restrict__ d1, const double* __restrict__ dphi, const double* __restrict__ W0,
-                              double* __restrict__ bphi, double* __restrict__ bW0, double* __restrict__ u, double* __restrict__ v) {
+                              double* __restrict__ bphi, double* __restrict__ bW0, double* __restrict__ u, double* __restrict__ v,
+                              const double* __restrict__ xE) {
     int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
-    const double e1 = d1[j], p = dphi[j], w = W0[j];
+    double e1 = d1[j], p = dphi[j], w = W0[j];
+    if (xE) {  // refined mesh: x-derivatives and the factor 1/|xi'| of (2.8)
+        const double re = 1.0 / xE[j];
+        e1 *= re; p *= re; w *= re;
+    }
     const double rden = 1.0 / fma(e1, e1, 1.0);
     bphi[j] = p;       bphi[N + j] = 0.0;
     bW0[j] = w;        bW0[N + j] = 0.0;
@@ -613,7 +626,7 @@ int fast_base_f64(sww_dtn_s* d, const double* phi0) {
         SWW_TRY(gemm_f64(st, N, 1, N, 1.0, d->G, N, w.Gam, N, 1.0, w.W, N, 1));
     SWW_TRY(spectral_deriv(d, phi0, w.T, 1));                          // phi0'
     SWW_BEGIN(KC_OTHER, st);
-    k_base_uv_f64<<<(N + 255) / 256, 256, 0, st>>>(N, d->d1, w.T, w.W, d->bphi, d->bW0, d->bu, d->bv);
+    k_base_uv_f64<<<(N + 255) / 256, 256, 0, st>>>(N, d->d1, w.T, w.W, d->bphi, d->bW0, d->bu, d->bv, d->mesh_on ? d->mesh.xE : nullptr);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
@@ -682,7 +695,7 @@ int dd_apply(sww_dtn_s* d, const double* rhs, bool rhs_in_ws, const double* Tcol
     k_dd_copy<<<blocks, 256, 0, st>>>(n, Lws, Lio, 1, w.T == Tcols ? w.W : w.T, out, nullptr);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
-    return SWW_OK;
+    return mesh_scale_out(d, out, nrhs, Lio);  // the factor 1/|xi'| of (2.8) on a refined mesh
 }
 
 int dd_linearized(sww_dtn_s* d, const double* deta, const double* dphi, int nrhs, double* out, size_t Lin, size_t Lout) {

@@ -1,0 +1,221 @@
+// mesh.cu -- mesh refinement in space, PAPER.md:122-136:
+//   (2.10) the change of variables x = xi(alpha), xi' = E = 1 - P[A sin^4(alpha/2)] (refine near x = pi) or 1 - P[A cos^4(alpha/2)]
+//          (refine near x = 0), A = 8 (1 - rho) / (5 + 3 rho); (2.11) rho = min E / max E.  With sin^4(a/2) = 3/8 - cos(a)/2 + cos(2a)/8:
+//              E = 1 + a1 cos(alpha) + a2 cos(2 alpha),  xi - alpha = a1 sin(alpha) + (a2/2) sin(2 alpha),  a1 = +-A/2, a2 = -A/8.
+//   The state is stored at the points x_j = xi(alpha_j) of a uniform alpha-mesh; zeta = xi + i eta o xi in (2.13) (assembly.cu),
+//   the factor 1/|xi'| of (2.8) and d/dx = (1/xi') d/dalpha elsewhere (api.cu, ddpath.cu, rk.cu).
+//   Respacing between segments: f o xi_new(alpha_j) = (f o xi_old)(beta_j), beta_j = xi_old^{-1}(xi_new(alpha_j)) by
+//   Newton's method; the values at beta_j come from the trigonometric interpolant of the old samples, written as one matrix
+//   R (M_new x M_old, the periodic Dirichlet kernel) applied to all state columns at once by the library's fp64 GEMM.
+// Product code; shares nothing with oracle/.
+#include "rk.cuh"
+#include "dd.cuh"
+#include <cmath>
+
+using namespace sww;
+
+namespace sww {
+
+// A = 8 (1 - rho) / (5 + 3 rho) in double-double (rho is an fp64 number; every operation below is exact or a dd operation)
+__device__ __forceinline__ dd mesh_A(double rho) {
+    const dd num = dd_mul_d(two_sum(1.0, -rho), 8.0);
+    const dd den = dd_add_d(two_prod(3.0, rho), 5.0);
+    return dd_div(num, den);
+}
+
+// sin and cos of a dd angle of any moderate size: reduce by multiples of pi/2, then the Taylor series of dd.cuh
+__device__ inline void dd_sincos_any(dd x, dd* s, dd* c) {
+    const dd hp = dd_half(dd_pi());
+    const double kf = rint(x.hi / hp.hi);
+    const dd r = dd_sub(x, dd_mul_d(hp, kf));
+    dd ss, cc;
+    dd_sincos_small(r, &ss, &cc);
+    switch (((long long)kf) & 3) {
+        case 0: *s = ss; *c = cc; break;
+        case 1: *s = cc; *c = dd_neg(ss); break;
+        case 2: *s = dd_neg(ss); *c = dd_neg(cc); break;
+        default: *s = dd_neg(cc); *c = ss; break;
+    }
+}
+
+// per-node tables of the handle: xE, xE1, xS, xC (dd planar 2N each), from the exact per-N tables cs, sn of cos, sin(2 pi m / N)
+__global__ void k_mesh_tables(int N, double rho, int where, const double* __restrict__ cs, const double* __restrict__ sn, double* __restrict__ xE,
+                              double* __restrict__ xE1, double* __restrict__ xS, double* __restrict__ xC) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= N) return;
+    const dd A = mesh_A(rho);
+    const dd a1 = where == 0 ? dd_half(A) : dd_neg(dd_half(A)), a2 = dd_neg(dd_ldexp(A, -3));
+    const int j2 = (2 * j) & (N - 1);
+    const dd c1 = dd_load(cs, N, j), s1 = dd_load(sn, N, j), c2 = dd_load(cs, N, j2), s2 = dd_load(sn, N, j2);
+    dd_store(xE, N, j, dd_add(dd_add_d(dd_mul(a1, c1), 1.0), dd_mul(a2, c2)));
+    dd_store(xE1, N, j, dd_neg(dd_add(dd_mul(a1, s1), dd_mul(dd_mul_d(a2, 2.0), s2))));
+    const dd p = dd_add(dd_mul(a1, s1), dd_mul(dd_half(a2), s2));
+    dd S, C;
+    dd_sincos_small(p, &S, &C);  // |xi - alpha| <= 0.52 A <= 0.83
+    dd_store(xS, N, j, S);
+    dd_store(xC, N, j, C);
+}
+
+// out_c <- out_c / xi'  (the factor of (2.8)); fp64, or dd planar with plane size L
+__global__ void k_mesh_scale_f64(int N, size_t total, const double* __restrict__ xE, double* __restrict__ out) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= total) return;
+    out[e] /= xE[e & (size_t)(N - 1)];
+}
+__global__ void k_mesh_scale_dd(int N, size_t total, size_t L, const double* __restrict__ xE, double* __restrict__ out) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= total) return;
+    const dd r = dd_div(dd{out[e], out[L + e]}, dd_load(xE, N, e & (size_t)(N - 1)));
+    out[e] = r.hi;
+    out[L + e] = r.lo;
+}
+
+int mesh_scale_out(sww_dtn_s* d, double* out, int nrhs, size_t L) {
+    if (!d->mesh_on || nrhs <= 0) return SWW_OK;
+    const size_t total = (size_t)d->N * nrhs;
+    SWW_BEGIN(KC_OTHER, d->stream);
+    if (d->prec == SWW_DD) k_mesh_scale_dd<<<(unsigned)((total + 255) / 256), 256, 0, d->stream>>>(d->N, total, L ? L : total, d->mesh.xE, out);
+    else k_mesh_scale_f64<<<(unsigned)((total + 255) / 256), 256, 0, d->stream>>>(d->N, total, d->mesh.xE, out);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    return SWW_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ respacing
+// xi(b) - x and xi'(b) at a dd parameter value b for the mesh (rho, where)
+__device__ inline void mesh_xi_dd(dd A, int where, dd b, dd* xi, dd* E) {
+    dd s1, c1, s2, c2;
+    dd_sincos_any(b, &s1, &c1);
+    s2 = dd_mul_d(dd_mul(s1, c1), 2.0);
+    c2 = dd_sub(dd_sqr(c1), dd_sqr(s1));
+    const dd a1 = where == 0 ? dd_half(A) : dd_neg(dd_half(A)), a2 = dd_neg(dd_ldexp(A, -3));
+    *xi = dd_add(b, dd_add(dd_mul(a1, s1), dd_mul(dd_half(a2), s2)));
+    *E = dd_add(dd_add_d(dd_mul(a1, c1), 1.0), dd_mul(a2, c2));
+}
+
+// beta_j = xi_old^{-1}(xi_new(alpha_j)), alpha_j = 2 pi j / Mn, by Newton's method in dd; sj = sin(Mo beta_j / 2)
+__global__ void k_respace_nodes(int Mo, double rho_o, int where_o, int Mn, double rho_n, int where_n, double* __restrict__ beta /* dd planar 2 Mn */,
+                                double* __restrict__ sj) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Mn) return;
+    const dd An = mesh_A(rho_n), Ao = mesh_A(rho_o);
+    const dd al = dd_div_d(dd_mul_d(dd_mul_d(dd_pi(), 2.0), (double)j), (double)Mn);
+    dd x, e;
+    mesh_xi_dd(An, where_n, al, &x, &e);
+    dd b = x;
+    for (int it = 0; it < 40; it++) {
+        dd xb, eb;
+        mesh_xi_dd(Ao, where_o, b, &xb, &eb);
+        const dd step = dd_div(dd_sub(xb, x), eb);
+        b = dd_sub(b, step);
+        if (fabs(step.hi) < 1e-31) break;
+    }
+    dd_store(beta, Mn, j, b);
+    dd s, c;
+    dd_sincos_any(dd_mul_d(b, 0.5 * (double)Mo), &s, &c);
+    sj[j] = s.hi;
+}
+
+// R[j + m Mn] = D(beta_j - alpha_m), alpha_m = 2 pi m / Mo, D(t) = (1/Mo) sin(Mo t / 2) cot(t / 2) the periodic Dirichlet kernel of Mo
+// (even) points with the Nyquist mode as a cosine; sin(Mo (beta_j - alpha_m)/2) = (-1)^m sin(Mo beta_j / 2).  D(0) = 1.
+__global__ void k_respace_matrix(int Mo, int Mn, const double* __restrict__ beta, const double* __restrict__ sj, double* __restrict__ R) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (j >= Mn) return;
+    const dd am = dd_div_d(dd_mul_d(dd_mul_d(dd_pi(), 2.0), (double)m), (double)Mo);
+    const dd t = dd_sub(dd_load(beta, Mn, j), am);
+    double th = 0.5 * (t.hi + t.lo);
+    // |t| below 1e-13: sin(Mo t/2) cot(t/2) / Mo = 1 - O((Mo t)^2)
+    double v;
+    if (fabs(th) < 1e-13) v = 1.0;
+    else {
+        const double sg = (m & 1) ? -1.0 : 1.0;
+        v = sg * sj[j] / (tan(th) * (double)Mo);
+    }
+    R[(size_t)j + (size_t)m * Mn] = v;
+}
+
+}  // namespace sww
+
+extern "C" {
+
+int sww_dtn_set_mesh(sww_dtn_t d, double rho, int where) {
+    if (!d || !(rho > 0.0 && rho <= 1.0) || (where != 0 && where != 1)) return SWW_EINVAL;
+    const int N = d->N;
+    d->has_base = false;
+    if (rho == 1.0) {  // the uniform mesh
+        d->mesh_on = false;
+        d->mesh_rho = 1.0;
+        d->mesh_where = 0;
+        return SWW_OK;
+    }
+    if (!d->mesh_buf) {
+        SWW_CUDA(cudaMalloc(&d->mesh_buf, sizeof(double) * 8 * (size_t)N));
+        d->mesh.xE = d->mesh_buf;
+        d->mesh.xE1 = d->mesh_buf + 2 * (size_t)N;
+        d->mesh.xS = d->mesh_buf + 4 * (size_t)N;
+        d->mesh.xC = d->mesh_buf + 6 * (size_t)N;
+    }
+    SWW_BEGIN(KC_OTHER, d->stream);
+    k_mesh_tables<<<(N + 127) / 128, 128, 0, d->stream>>>(N, rho, where, d->tab->cs, d->tab->sn, d->mesh_buf, d->mesh_buf + 2 * (size_t)N,
+                                                        d->mesh_buf + 4 * (size_t)N, d->mesh_buf + 6 * (size_t)N);
+    SWW_LAUNCHED();
+    SWW_CUDA(cudaGetLastError());
+    const double A = 8.0 * (1.0 - rho) / (5.0 + 3.0 * rho);
+    d->mesh_on = true;
+    d->mesh_rho = rho;
+    d->mesh_where = where;
+    d->mesh_a1 = where == 0 ? 0.5 * A : -0.5 * A;
+    d->mesh_a2 = -0.125 * A;
+    return SWW_OK;
+}
+
+int sww_mesh_points(int N, double rho, int where, double* x) {
+    if (!x || N < 1 || !(rho > 0.0 && rho <= 1.0) || (where != 0 && where != 1)) return SWW_EINVAL;
+    const long double A = 8.0L * (1.0L - (long double)rho) / (5.0L + 3.0L * (long double)rho), a1 = where == 0 ? A / 2 : -A / 2, a2 = -A / 8;
+    const long double two_pi = 6.283185307179586476925286766559L;
+    for (int j = 0; j < N; j++) {
+        const long double al = two_pi * j / N;
+        x[j] = (double)(al + a1 * sinl(al) + a2 / 2 * sinl(2 * al));
+    }
+    return SWW_OK;
+}
+
+int sww_state_set_mesh(sww_state_t s, double rho, int where) {
+    if (!s) return SWW_EINVAL;
+    if (s->prec == SWW_DD && rho != 1.0) return SWW_EINVAL;  // the double-double stepper runs on the uniform mesh only
+    return sww_dtn_set_mesh(s->dtn, rho, where);
+}
+
+int sww_state_respace(sww_state_t dst, sww_state_t src) {
+    if (!dst || !src || dst == src) return SWW_EINVAL;
+    if (dst->prec != SWW_F64 || src->prec != SWW_F64 || dst->nc != src->nc) return SWW_EINVAL;
+    const int Mo = src->N, Mn = dst->N, ncol = 2 + 2 * src->nc;
+    cudaStream_t st = dst->stream;
+    SWW_CUDA(cudaStreamSynchronize(src->stream));  // the source state is complete before it is read on dst's stream
+    double *beta = nullptr, *sj = nullptr, *R = nullptr;
+    if (cudaMalloc(&beta, sizeof(double) * 3 * (size_t)Mn) != cudaSuccess || cudaMalloc(&R, sizeof(double) * (size_t)Mn * Mo) != cudaSuccess) {
+        cudaFree(beta);
+        cudaFree(R);
+        return SWW_ENOMEM;
+    }
+    sj = beta + 2 * (size_t)Mn;
+    const sww_dtn_s *dn = dst->dtn, *ds = src->dtn;
+    SWW_BEGIN(KC_OTHER, st);
+    k_respace_nodes<<<(Mn + 63) / 64, 64, 0, st>>>(Mo, ds->mesh_on ? ds->mesh_rho : 1.0, ds->mesh_on ? ds->mesh_where : 0, Mn,
+                                                   dn->mesh_on ? dn->mesh_rho : 1.0, dn->mesh_on ? dn->mesh_where : 0, beta, sj);
+    SWW_LAUNCHED();
+    SWW_BEGIN(KC_OTHER, st);
+    k_respace_matrix<<<dim3((Mn + 127) / 128, Mo), 128, 0, st>>>(Mo, Mn, beta, sj, R);
+    SWW_LAUNCHED();
+    int rc = cudaGetLastError() == cudaSuccess ? SWW_OK : SWW_ECUDA;
+    if (!rc) rc = gemm_f64(st, Mn, ncol, Mo, 1.0, R, Mn, src->y, Mo, 0.0, dst->y, Mn, ncol);
+    cudaStreamSynchronize(st);
+    cudaFree(beta);
+    cudaFree(R);
+    if (rc) return rc;
+    dst->t = src->t;
+    dst->dtn->has_base = false;
+    return SWW_OK;
+}
+
+}  // extern "C"

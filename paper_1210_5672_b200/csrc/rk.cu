@@ -290,6 +290,195 @@ __global__ void __launch_bounds__(1024) k_st_cols(int N, int logN, const double2
     }
 }
 
+// ------------------------------------------------------------------------------------------------ refined mesh (mesh.cu)
+// On the mesh x = xi(alpha) of (2.10) the stored samples are functions of alpha: d/dx = (1/xi') d/dalpha in every term of (2.1) and
+// (B.1)-(B.4), the filter acts on the samples (modes in alpha), and P removes the mean over x,
+//     (1/2pi) int f dx = (1/N) sum_j f_j E_j = f^_0 + a1 Re f^_1 + a2 Re f^_2     for E = 1 + a1 cos(alpha) + a2 cos(2 alpha).
+// W0, u, v and the linearized DtN output arrive in physical form (ddpath.cu, api.cu divide by xi').  The uniform-mesh kernels
+// above fold some of the derivatives into the last transform; here each derivative is taken on its own, then divided by xi'.
+//
+// z: the spectrum (scaled, bit-reversed order: mode k at position brev(k)) of a packed pair x + i y of real signals.  Returns the
+// part a1 Re f^_1 + a2 Re f^_2 of both means: with X_k = (Z_k + conj Z_-k)/2 and Y_k = (Z_k - conj Z_-k)/(2i),
+// Re X_k = (Re Z_k + Re Z_-k)/2 and Re Y_k = (Im Z_k + Im Z_-k)/2.
+__device__ __forceinline__ double2 mesh_mean_pair(const double2* z, int N, int logN, double a1, double a2) {
+    const double2 p1 = z[dft_index(1, logN)], m1 = z[dft_index(N - 1, logN)], p2 = z[dft_index(2, logN)], m2 = z[dft_index(N - 2, logN)];
+    return make_double2(0.5 * (a1 * (p1.x + m1.x) + a2 * (p2.x + m2.x)), 0.5 * (a1 * (p1.y + m1.y) + a2 * (p2.y + m2.y)));
+}
+
+struct MeshRk {
+    const double* xE;  // xi' (hi words)
+    double a1, a2;
+};
+
+// z <- (1/xi') D z for a packed pair (natural order in and out); every thread of the CTA calls it
+__device__ __forceinline__ void mesh_deriv_x(double2* z, int N, int logN, const double2* __restrict__ tw, const double* __restrict__ xE) {
+    const double rN = 1.0 / (double)N;
+    __syncthreads();
+    fft_dif(z, N, tw);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double k = (double)wavenumber(p, N, logN) * rN;
+        const double2 t = z[p];
+        z[p] = make_double2(-k * t.y, k * t.x);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double re = 1.0 / xE[j];
+        z[j] = make_double2(z[j].x * re, z[j].y * re);
+    }
+    __syncthreads();
+}
+// z <- F z for a packed pair; P (mean over x) on the y part if proj_y, on the x part if proj_x
+__device__ __forceinline__ void mesh_filter_project(double2* z, int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                    int filter_on, MeshRk ms, bool proj_x, bool proj_y) {
+    const double rN = 1.0 / (double)N;
+    __syncthreads();
+    fft_dif(z, N, tw);
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double f = (filter_on ? filt[dft_index(p, logN)] : 1.0) * rN;
+        z[p] = make_double2(f * z[p].x, f * z[p].y);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0 && (proj_x || proj_y)) {
+        const double2 m = mesh_mean_pair(z, N, logN, ms.a1, ms.a2);
+        if (proj_x) z[0].x = -m.x;   // mean over alpha z[0] minus the mean over x (z[0] + m)
+        if (proj_y) z[0].y = -m.y;
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+}
+
+// base state on the refined mesh: eta_t = F[W0] ; phi_t = F P[ v W0 - u^2/2 - v^2/2 - g eta + sigma d/dx( eta_x / sqrt(1 + eta_x^2) ) ],
+// eta_x = d1 / xi'   (2.1); one CTA
+__global__ void __launch_bounds__(1024) k_rhs_base_mesh(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                        int filter_on, double g, double sigma, MeshRk ms, const double* __restrict__ eta,
+                                                        const double* __restrict__ d1, const double* __restrict__ W0, const double* __restrict__ u,
+                                                        const double* __restrict__ v, double* __restrict__ eta_t, double* __restrict__ phi_t) {
+    extern __shared__ __align__(16) double2 z[];
+    double cur[FFT_MAX_PER_THREAD];
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) cur[r] = 0.0;
+    if (sigma != 0.0) {
+        for (int j = threadIdx.x; j < N; j += blockDim.x) {
+            const double e1 = d1[j] / ms.xE[j];
+            z[j] = make_double2(e1 / sqrt(fma(e1, e1, 1.0)), 0.0);
+        }
+        mesh_deriv_x(z, N, logN, tw, ms.xE);
+#pragma unroll
+        for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+            const int j = threadIdx.x + r * blockDim.x;
+            if (j < N) cur[r] = sigma * z[j].x;
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) {
+            const double w = W0[j], uu = u[j], vv = v[j];
+            z[j] = make_double2(w, fma(vv, w, -0.5 * uu * uu) - 0.5 * vv * vv - g * eta[j] + cur[r]);
+        }
+    }
+    mesh_filter_project(z, N, logN, tw, filt, filter_on, ms, false, true);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        eta_t[j] = z[j].x;
+        phi_t[j] = z[j].y;
+    }
+}
+
+// variational columns on the refined mesh (B.1)-(B.4), one CTA per column pair; wout = G b - d/dx(u deta) (physical, api.cu):
+//   deta_t = F[wout] ;  dphi_t = F P[ -d/dx(deta u v) - u d/dx(b) + v w - g deta + sigma d/dx( d/dx(deta) / (1 + eta_x^2)^(3/2) ) ],
+//   w = wout + d/dx(u deta),  b = dphi - v deta
+__global__ void __launch_bounds__(1024) k_rhs_cols_mesh(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                        int filter_on, double g, double sigma, MeshRk ms, int ncols, const double* __restrict__ d1,
+                                                        const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ deta,
+                                                        const double* __restrict__ dphi, const double* __restrict__ wout,
+                                                        double* __restrict__ deta_t, double* __restrict__ dphi_t) {
+    extern __shared__ __align__(16) double2 z[];
+    const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
+    const bool has1 = c1 < ncols;
+    const size_t o0 = (size_t)c0 * N, o1 = (size_t)c1 * N;
+    double2 acc[FFT_MAX_PER_THREAD];
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double uu = u[j];
+        z[j] = make_double2(uu * deta[o0 + j], has1 ? uu * deta[o1 + j] : 0.0);
+    }
+    mesh_deriv_x(z, N, logN, tw, ms.xE);  // d/dx(u deta)
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) {
+            const double vv = v[j];
+            acc[r] = make_double2(vv * (wout[o0 + j] + z[j].x) - g * deta[o0 + j], has1 ? vv * (wout[o1 + j] + z[j].y) - g * deta[o1 + j] : 0.0);  // v w - g deta
+        }
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double vv = v[j];
+        z[j] = make_double2(fma(-vv, deta[o0 + j], dphi[o0 + j]), has1 ? fma(-vv, deta[o1 + j], dphi[o1 + j]) : 0.0);
+    }
+    mesh_deriv_x(z, N, logN, tw, ms.xE);  // d/dx(b)
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) {
+            const double uu = u[j];
+            acc[r].x = fma(-uu, z[j].x, acc[r].x);
+            acc[r].y = fma(-uu, z[j].y, acc[r].y);
+        }
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double uv = u[j] * v[j];
+        z[j] = make_double2(uv * deta[o0 + j], has1 ? uv * deta[o1 + j] : 0.0);
+    }
+    mesh_deriv_x(z, N, logN, tw, ms.xE);  // d/dx(deta u v)
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) {
+            acc[r].x -= z[j].x;
+            acc[r].y -= z[j].y;
+        }
+    }
+    __syncthreads();
+    if (sigma != 0.0) {
+        for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(deta[o0 + j], has1 ? deta[o1 + j] : 0.0);
+        mesh_deriv_x(z, N, logN, tw, ms.xE);
+        for (int j = threadIdx.x; j < N; j += blockDim.x) {
+            const double e1 = d1[j] / ms.xE[j], den = fma(e1, e1, 1.0), q = 1.0 / (den * sqrt(den));
+            z[j] = make_double2(z[j].x * q, z[j].y * q);
+        }
+        mesh_deriv_x(z, N, logN, tw, ms.xE);
+#pragma unroll
+        for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+            const int j = threadIdx.x + r * blockDim.x;
+            if (j < N) {
+                acc[r].x = fma(sigma, z[j].x, acc[r].x);
+                acc[r].y = fma(sigma, z[j].y, acc[r].y);
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < FFT_MAX_PER_THREAD; r++) {
+        const int j = threadIdx.x + r * blockDim.x;
+        if (j < N) z[j] = acc[r];
+    }
+    mesh_filter_project(z, N, logN, tw, filt, filter_on, ms, true, true);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        dphi_t[o0 + j] = z[j].x;
+        if (has1) dphi_t[o1 + j] = z[j].y;
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(wout[o0 + j], has1 ? wout[o1 + j] : 0.0);
+    mesh_filter_project(z, N, logN, tw, filt, filter_on, ms, false, false);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        deta_t[o0 + j] = z[j].x;
+        if (has1) deta_t[o1 + j] = z[j].y;
+    }
+}
+
 // the filter (2.14) applied in place to ncols columns (the state after every step)
 __global__ void __launch_bounds__(1024) k_filter_cols(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
                                                       int ncols, double* __restrict__ y) {
@@ -314,11 +503,12 @@ __global__ void __launch_bounds__(1024) k_filter_cols(int N, int logN, const dou
 }
 
 // E = (pi/N) sum_j [ phi_j (G phi)_j + g eta_j^2 ], one CTA, pairwise tree in shared memory
+// xE (refined mesh, else nullptr): dx = xi' dalpha
 __global__ void __launch_bounds__(256) k_energy(int N, double g, const double* __restrict__ eta, const double* __restrict__ phi,
-                                                const double* __restrict__ W0, double* __restrict__ out) {
+                                                const double* __restrict__ W0, const double* __restrict__ xE, double* __restrict__ out) {
     __shared__ double s[256];
     double a = 0.0;
-    for (int j = threadIdx.x; j < N; j += 256) a += fma(phi[j], W0[j], g * eta[j] * eta[j]);
+    for (int j = threadIdx.x; j < N; j += 256) a += fma(phi[j], W0[j], g * eta[j] * eta[j]) * (xE ? xE[j] : 1.0);
     s[threadIdx.x] = a;
     __syncthreads();
     for (int o = 128; o > 0; o >>= 1) {
@@ -340,6 +530,8 @@ static int rk_set_attrs() {
         SWW_CUDA(cudaFuncSetAttribute(k_filter_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
         SWW_CUDA(cudaFuncSetAttribute(k_st_base, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
         SWW_CUDA(cudaFuncSetAttribute(k_st_cols, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        SWW_CUDA(cudaFuncSetAttribute(k_rhs_base_mesh, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        SWW_CUDA(cudaFuncSetAttribute(k_rhs_cols_mesh, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
     }
     return SWW_OK;
 }
@@ -381,6 +573,26 @@ int rk_rhs(sww_state_s* s, const double* ys, double* kout) {
         SWW_TRY(sww_dtn_set_base(d, phi));   // W0 = G phi, u, v of (2.9)
     }
     const Tables* t = d->tab;
+    if (d->mesh_on) {  // the refined mesh (2.10): kernels with d/dx = (1/xi') d/dalpha and the mean over x
+        const MeshRk ms{d->mesh.xE, d->mesh_a1, d->mesh_a2};
+        SWW_BEGIN(KC_FFT, st);
+        k_rhs_base_mesh<<<1, thr, sizeof(double2) * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->g, s->sigma, ms, eta, d->d1,
+                                                                       d->bW0, d->bu, d->bv, kout, kout + N);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+        if (nc > 0) {
+            const double* deta = ys + 2 * (size_t)N;
+            const double* dphi = deta + (size_t)N * nc;
+            SWW_TRY(sww_dtn_linearized_apply(d, deta, dphi, nc, s->w));  // G b - d/dx(u deta_c)   (B.1d), (B.2)
+            SWW_BEGIN(KC_FFT, st);
+            k_rhs_cols_mesh<<<(nc + 1) / 2, thr, sizeof(double2) * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->g, s->sigma, ms, nc,
+                                                                                    d->d1, d->bu, d->bv, deta, dphi, s->w, kout + 2 * (size_t)N,
+                                                                                    kout + 2 * (size_t)N + (size_t)N * nc);
+            SWW_LAUNCHED();
+            SWW_CUDA(cudaGetLastError());
+        }
+        return SWW_OK;
+    }
     SWW_BEGIN(KC_FFT, st);
     k_rhs_base<<<1, thr, sizeof(double2) * (size_t)N, st>>>(N, logN, t->tw, t->filt, s->filter ? 1 : 0, s->g, eta, d->bW0, d->bu, d->bv, kout,
                                                               kout + N);
@@ -633,7 +845,7 @@ int sww_state_energy(sww_state_t s, double* energy_hl) {
     SWW_TRY(sww_dtn_refactor(d, s->y));
     SWW_TRY(sww_dtn_set_base(d, s->y + s->N));
     SWW_BEGIN(KC_OTHER, s->stream);
-    k_energy<<<1, 256, 0, s->stream>>>(s->N, s->g, s->y, s->y + s->N, d->bW0, s->red);
+    k_energy<<<1, 256, 0, s->stream>>>(s->N, s->g, s->y, s->y + s->N, d->bW0, d->mesh_on ? d->mesh.xE : nullptr, s->red);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     SWW_CUDA(cudaMemcpyAsync(energy_hl, s->red, sizeof(double), cudaMemcpyDeviceToHost, s->stream));

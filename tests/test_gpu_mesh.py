@@ -1,0 +1,260 @@
+"""GPU parity tests of mesh refinement in space ((2.10)-(2.11); mesh.cu) against the oracle: kernel matrices, DtN and
+linearized DtN in both precisions, the time stepper and the respacing between segments; plus a closed-form harmonic function
+through the device path alone.  The stored samples are the same seeded arrays as elsewhere (any smooth periodic function of
+alpha is a smooth function of x).  Tolerances: the bars of parity_util divided by rho^2 -- the kernels next to the diagonal are
+differences of O(1/spacing^2) terms, and the spacing at the refined end is ~rho times the uniform one."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+import torch
+
+import sww_inputs as si
+from parity_util import ld, diff, to_dev
+
+pytestmark = pytest.mark.gpu
+LD = np.longdouble
+
+
+@pytest.fixture(scope="module")
+def sww():
+    import paper_1210_5672_b200 as pkg
+    assert pkg.lib_path().exists() and torch.cuda.is_available()
+    return pkg
+
+
+@pytest.fixture()
+def mesh_ld(orc_ld):
+    yield orc_ld
+    orc_ld.set_mesh()
+
+
+@pytest.fixture()
+def mesh_q(orc_q):
+    yield orc_q
+    orc_q.set_mesh()
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def surface(N, amp=0.2):
+    a, _ = si._family_surface(si.SEED_BASE + 3, N, amp, kmax=min(64, N // 4))
+    return si.synth(N, a)[0]
+
+
+def small_case(N, nc):
+    c2 = si.config2()
+    eta = np.ascontiguousarray(c2.eta[:: c2.N // N]) if N <= c2.N else surface(N, 0.1)
+    a = np.zeros(9); a[1] = 0.05; a[2] = 0.02; a[3] = -0.01
+    b = np.zeros(9); b[2] = 0.01
+    phi = si.synth(N, a, b)[0]
+    deta, dphi = si.fourier_unit_columns(N, nc // 2, "eta_phi")
+    return eta, phi, deta, dphi
+
+
+@pytest.mark.parametrize("N,h,rho,where", [(64, 1.0, 0.5, 0), (256, 1.0, 0.3, 1), (256, 0.05, 0.4, 0), (128, float("inf"), 0.2, 0)])
+def test_kernel_matrices_on_refined_mesh(sww, mesh_ld, N, h, rho, where):
+    eta = surface(N, 0.2 if h > 0.1 else 0.01)
+    d = sww.DtN(dev(eta), h)
+    d.set_mesh(rho, where)
+    d.refactor(dev(eta))
+    d.check()
+    mesh_ld.set_mesh(rho, where)
+    o = mesh_ld.assemble(eta, h)
+    for name in ("K", "G"):
+        g = d.get(name).cpu().numpy().T
+        ref = ld(o[name])
+        scale = float(np.abs(ref).max())
+        err = float(np.abs(g - ref).max())
+        assert err <= 3e-14 / rho ** 2 * max(scale, 1.0 / N), (name, err, scale)
+    x = sww.mesh_points(N, rho, where)
+    xp, _, _ = mesh_ld.mesh_tables(N)
+    assert np.abs(x - (2 * np.pi * np.arange(N) / N + xp[0])).max() < 1e-15
+
+
+def test_kernel_matrices_on_refined_mesh_dd(sww, mesh_q):
+    N, rho = 128, 0.35
+    c = si.config4(N, 2)
+    d = sww.DtN(to_dev(c.eta, c.eta_lo, "dd"), c.h, sww.DD)
+    d.set_mesh(rho, 1)
+    d.refactor(to_dev(c.eta, c.eta_lo, "dd"))
+    d.check()
+    mesh_q.set_mesh(rho, 1)
+    o = mesh_q.assemble((c.eta, c.eta_lo), c.h)
+    for name in ("K", "G"):
+        t = d.get(name).cpu().numpy()
+        err = float(np.abs(diff((t[0].T, t[1].T), o[name])).max())
+        assert err <= 1e-29 * N / rho ** 2, (name, err)
+
+
+@pytest.mark.parametrize("N,h,rho,where", [(256, 1.0, 0.4, 0), (128, float("inf"), 0.25, 1), (1024, 1.0, 0.5, 0)])
+def test_apply_and_linearized_on_refined_mesh(sww, mesh_ld, N, h, rho, where):
+    eta, phi, deta, dphi = small_case(N, 12)
+    d = sww.DtN(dev(eta), h)
+    d.set_mesh(rho, where)
+    d.refactor(dev(eta))
+    w = d.apply(dev(np.stack([phi, deta[0]])))
+    d.set_base(dev(phi))
+    lin = d.linearized_apply(dev(deta), dev(dphi))
+    d.check()
+    mesh_ld.set_mesh(rho, where)
+    ow = ld(mesh_ld.dtn_apply(eta, h, np.stack([phi, deta[0]])))
+    ol, base = mesh_ld.dtn_linearized(eta, h, phi, deta, dphi, want_base=True)
+    tol = 1e-11 / rho ** 2
+    err = np.abs(w.cpu().numpy().astype(LD) - ow).max(axis=1) / np.abs(ow).max(axis=1)
+    assert float(err.max()) <= tol, err
+    ol = ld(ol)
+    err = np.abs(lin.cpu().numpy().astype(LD) - ol).max(axis=1) / np.abs(ol).max(axis=1)
+    assert float(err.max()) <= tol, err
+    for name in ("dphi0", "W0", "u", "v"):
+        g = d.get(name).cpu().numpy().astype(LD)
+        ref = ld(base[name])
+        assert float(np.abs(g - ref).max()) <= 1e-13 / rho ** 2 * max(1.0, float(np.abs(ref).max())), name
+
+
+def test_apply_and_linearized_on_refined_mesh_dd(sww, mesh_q):
+    N, rho, where = 128, 0.4, 0
+    c = si.config4(N, 8)
+    d = sww.DtN(to_dev(c.eta, c.eta_lo, "dd"), c.h, sww.DD)
+    d.set_mesh(rho, where)
+    d.refactor(to_dev(c.eta, c.eta_lo, "dd"))
+    w = d.apply(to_dev(c.dphi, c.dphi_lo, "dd"))
+    d.set_base(to_dev(c.phi0, c.phi0_lo, "dd"))
+    lin = d.linearized_apply(to_dev(c.deta, c.deta_lo, "dd"), to_dev(c.dphi, c.dphi_lo, "dd"))
+    d.check()
+    mesh_q.set_mesh(rho, where)
+    ow = mesh_q.dtn_apply((c.eta, c.eta_lo), c.h, (c.dphi, c.dphi_lo))
+    ol = mesh_q.dtn_linearized((c.eta, c.eta_lo), c.h, (c.phi0, c.phi0_lo), (c.deta, c.deta_lo), (c.dphi, c.dphi_lo))
+    for got, ref in ((w, ow), (lin, ol)):
+        g = got.cpu().numpy()
+        e = np.abs(diff((g[0], g[1]), ref)).max(axis=1) / np.abs(ld(ref)).max(axis=1)
+        assert float(e.max()) <= 1e-25 / rho ** 2, e
+
+
+@pytest.mark.parametrize("rho,where,h", [(0.4, 0, 1.0), (0.3, 1, 0.5)])
+def test_harmonic_function_closed_form(sww, rho, where, h):
+    """phi = cosh(2 y) cos(2 x) on a wavy surface sampled at the refined points: G phi, phi_x, phi_y in closed form (no oracle)"""
+    N = 256
+    x = sww.mesh_points(N, rho, where).astype(LD)
+    coef = [0.0, 0.07, -0.03, 0.015, 0.0, 0.004]
+    eta = sum(LD(c) * np.cos(m * x) for m, c in enumerate(coef))
+    ex = sum(-LD(c) * m * np.sin(m * x) for m, c in enumerate(coef))
+    Y = LD(h) + eta
+    phi = np.cosh(2 * Y) * np.cos(2 * x)
+    px, py = -2 * np.cosh(2 * Y) * np.sin(2 * x), 2 * np.sinh(2 * Y) * np.cos(2 * x)
+    w = py - ex * px
+    e64, p64 = np.asarray(eta, dtype=np.float64), np.asarray(phi, dtype=np.float64)
+    d = sww.DtN(dev(e64), h)
+    d.set_mesh(rho, where)
+    d.refactor(dev(e64))
+    got = d.apply(dev(p64)).cpu().numpy()
+    d.set_base(dev(p64))
+    d.check()
+    # the fp64 rounding of the inputs moves the answer by ~eps N / rho (a first-order operator on rounded samples)
+    tol = 4 * N * 2.0 ** -53 / rho * float(np.abs(w).max()) + 1e-13 / rho ** 2
+    assert float(np.abs(got - w).max()) <= tol
+    assert float(np.abs(d.get("u").cpu().numpy() - px).max()) <= tol
+    assert float(np.abs(d.get("v").cpu().numpy() - py).max()) <= tol
+
+
+@pytest.mark.parametrize("N,nc,h,rho,where,sigma", [(64, 6, 1.0, 0.5, 0, 0.0), (256, 6, 1.0, 0.4, 1, 0.0), (128, 8, float("inf"), 0.5, 0, 0.6),
+                                                     (2048, 0, 1.0, 0.5, 0, 0.0)])
+def test_steps_on_refined_mesh(sww, mesh_ld, N, nc, h, rho, where, sigma):
+    eta, phi, deta, dphi = small_case(N, max(nc, 2))
+    dt = 0.02 if sigma == 0.0 else 0.4 / N * rho
+    nsteps = 2 if N <= 256 else 1
+    kw = dict(deta=dev(deta), dphi=dev(dphi)) if nc else {}
+    st = sww.State(dev(eta), dev(phi), h, 1.0, **kw)
+    st.set_mesh(rho, where)
+    st.set_sigma(sigma)
+    e0 = st.energy()[0]
+    st.advance(dt, nsteps)
+    r = st.read()
+    mesh_ld.set_mesh(rho, where)
+    o = mesh_ld.rk_advance(eta, phi, h, 1.0, dt, nsteps, deta=deta if nc else None, dphi=dphi if nc else None, sigma=sigma, want_energy=True)
+    tol = 1e-11 / rho ** 2
+    for name in ("eta", "phi"):
+        ref = ld(o[name])
+        assert float(np.abs(r[name].cpu().numpy().astype(LD) - ref).max() / np.abs(ref).max()) <= tol, name
+    if nc:
+        for name in ("deta", "dphi"):
+            gq, oq = r[name].cpu().numpy(), ld(o[name])
+            err = np.abs(gq.astype(LD) - oq).max(axis=1) / np.abs(oq).max(axis=1)
+            assert float(err.max()) <= tol, (name, err)
+    if sigma == 0.0:
+        assert abs(e0 - float(ld(o["energies"])[0])) <= 1e-12 * abs(e0)
+
+
+def test_segments_with_respacing(sww, mesh_ld):
+    """two segments as in section 2.2: uniform mesh, then a finer refined one; against the oracle's chain of the same steps"""
+    N, M2, nc, h, dt, rho = 128, 256, 4, 1.0, 0.02, 0.4
+    eta, phi, deta, dphi = small_case(N, nc)
+    s1 = sww.State(dev(eta), dev(phi), h, 1.0, deta=dev(deta), dphi=dev(dphi))
+    s1.advance(dt, 2)
+    z1, zc = torch.zeros(M2, dtype=torch.float64, device="cuda"), torch.zeros(nc, M2, dtype=torch.float64, device="cuda")
+    s2 = sww.State(z1, z1, h, 1.0, deta=zc, dphi=zc)
+    s2.set_mesh(rho, 0)
+    s2.respace_from(s1)
+    mid = s2.read()
+    s2.advance(dt / 2, 2)
+    r = s2.read()
+    assert abs(r["t"] - 3 * dt) < 1e-15
+    mesh_ld.set_mesh()
+    o1 = mesh_ld.rk_advance(eta, phi, h, 1.0, dt, 2, deta=deta, dphi=dphi)
+    om = {k: mesh_ld.respace(o1[k], (N, 1.0, 0), (M2, rho, 0)) for k in ("eta", "phi", "deta", "dphi")}
+    mesh_ld.set_mesh(rho, 0)
+    o2 = mesh_ld.rk_advance(om["eta"], om["phi"], h, 1.0, dt / 2, 2, deta=om["deta"], dphi=om["dphi"])
+    for got, ref, tol in ((mid, om, 2e-13), (r, o2, 1e-11 / rho ** 2)):
+        for name in ("eta", "phi", "deta", "dphi"):
+            g, q = got[name].cpu().numpy().astype(LD), ld(ref[name])
+            g, q = g.reshape(-1, M2), q.reshape(-1, M2)
+            err = np.abs(g - q).max(axis=1) / np.abs(q).max(axis=1)
+            assert float(err.max()) <= tol, (name, err)
+
+
+def test_respacing_between_arbitrary_meshes(sww, mesh_ld):
+    """refined -> refined with another rho, the other end and a smaller size; and onto the same mesh (the identity)"""
+    N, h = 256, 1.0
+    eta, phi, _, _ = small_case(N, 2)
+    s1 = sww.State(dev(eta), dev(phi), h, 1.0)
+    s1.set_mesh(0.5, 1)
+    for M2, rho2, w2 in ((128, 0.7, 0), (256, 0.5, 1), (512, 1.0, 0)):
+        z = torch.zeros(M2, dtype=torch.float64, device="cuda")
+        s2 = sww.State(z, z, h, 1.0)
+        s2.set_mesh(rho2, w2)
+        s2.respace_from(s1)
+        r = s2.read()
+        for name, src in (("eta", eta), ("phi", phi)):
+            ref = ld(mesh_ld.respace(src, (N, 0.5, 1), (M2, rho2, w2)))
+            assert float(np.abs(r[name].cpu().numpy().astype(LD) - ref).max()) <= 3e-14 * float(np.abs(ref).max()), (M2, name)
+        if (M2, rho2, w2) == (256, 0.5, 1):
+            assert float(np.abs(r["eta"].cpu().numpy() - eta).max()) <= 1e-15
+
+
+def test_uniform_mesh_is_untouched_and_errors(sww):
+    N, h = 128, 1.0
+    eta, phi, deta, dphi = small_case(N, 4)
+    d0 = sww.DtN(dev(eta), h)
+    ref = d0.apply(dev(phi)).clone()
+    d = sww.DtN(dev(eta), h)
+    d.set_mesh(0.5, 0)
+    d.refactor(dev(eta))
+    moved = d.apply(dev(phi)).clone()
+    assert float((moved - ref).abs().max()) > 1e-3
+    d.set_mesh(1.0, 0)
+    d.refactor(dev(eta))
+    assert torch.equal(d.apply(dev(phi)), ref)            # rho = 1 is the uniform path, bit for bit
+    for bad in ((0.0, 0), (1.5, 0), (0.5, 2), (float("nan"), 0)):
+        with pytest.raises(sww.SwwError):
+            d.set_mesh(*bad)
+    d.set_mesh(0.5, 1)
+    d.refactor(dev(eta))
+    d.set_base(dev(phi))
+    with pytest.raises(sww.SwwError):
+        d.adjoint_rhs(dev(deta), dev(dphi))
+    sdd = sww.State(to_dev(eta, None, "dd"), to_dev(phi, None, "dd"), h, 1.0, prec=sww.DD)
+    with pytest.raises(sww.SwwError):
+        sdd.set_mesh(0.5, 0)
+    sdd.set_mesh(1.0, 0)
