@@ -1,5 +1,6 @@
 """Oracle of the shooting map of the overdetermined shooting method -- TEST INFRASTRUCTURE, NOT PRODUCT CODE (see oracle/__init__.py
-for who may import it).  Plain restatement of PAPER.md section 3.1 / 3.3 on the uniform mesh (xi(alpha) = alpha, E = 1, M = N):
+for who may import it).  Plain restatement of PAPER.md section 3.1 / 3.3 on the uniform mesh (xi(alpha) = alpha, E = 1, M = N);
+shoot_segments below is the same map with the mesh-refinement strategy of section 2.2:
 
   (3.15) PAPER.md:197-200   eta^_k(0) = c_|k| for even k, phi^_k(0) = c_|k| for odd k, 1 <= |k| <= n, all other modes zero:
                             eta(x, 0) = sum_{k even} 2 c_k cos kx,  phi(x, 0) = sum_{k odd} 2 c_k cos kx  (eta about the mean level)
@@ -65,6 +66,43 @@ def shoot(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = True, 
     J = np.empty((N, n + 1), dtype=LD)
     J[:, 0] = phi_t * w / 4
     J[:, 1:] = dphi.T * w
+    return {"r": phi * w, "J": J, "eta": eta, "phi": phi}
+
+
+def shoot_segments(orc, c, segments, h: float, g: float, filter: bool = True, sigma: float = 0.0, method: str = "rk8"):
+    """The shooting map with the mesh-refinement strategy of section 2.2: segments = [(M_l, theta_l, rho_l, where_l,
+    N_l), ...], theta_1 + ... + theta_nu = 1, rho_1 = 1 (the initial state (3.15) lives on the uniform mesh).  Segment l advances N_l
+    steps of size theta_l (T/4) / N_l on M_l points x = xi_l(alpha); the state and the columns are respaced from l to l + 1 (Oracle.respace).
+      (3.17) PAPER.md:208-212   r_i = phi(xi_nu(alpha_i), T/4) sqrt(E_nu(alpha_i) / M_nu)   (trapezoidal weight of dx = E_nu dalpha)
+      (3.31)                    J_ik likewise from the columns on the last mesh; k = 0: phi_t(., T/4) / 4 times the weight (R13)
+    -> dict r (M_nu), J (M_nu x (n+1)), eta, phi (the state at T/4 on the last mesh), long double.  Leaves the oracle on the uniform mesh."""
+    c = np.asarray(c, dtype=np.float64)
+    n = c.shape[0] - 1
+    T = float(c[0])
+    ld = lambda p: p[0].astype(LD) + p[1].astype(LD)
+    M1, th1, rho1, where1, _ = segments[0]
+    assert rho1 == 1.0 and abs(sum(sg[1] for sg in segments) - 1.0) < 1e-12
+    eta0, phi0, deta0, dphi0 = initial_state(c, M1)
+    st = {"eta": _split(eta0), "phi": _split(phi0), "deta": _split(deta0), "dphi": _split(dphi0)}
+    prev = None
+    try:
+        for (M, theta, rho, where, nst) in segments:
+            if prev is not None:
+                st = {k: orc.respace(st[k], prev, (M, rho, where)) for k in ("eta", "phi", "deta", "dphi")}
+            orc.set_mesh(rho, where)
+            st = orc.rk_advance(st["eta"], st["phi"], h, g, theta * T / (4 * nst), nst, deta=st["deta"], dphi=st["dphi"], filter=filter,
+                                sigma=sigma, method=method)
+            prev = (M, rho, where)
+        phi_t = ld(orc.rhs(st["eta"], st["phi"], h, g, filter=filter, sigma=sigma)["phi_t"])
+        E = ld(orc.mesh_tables(prev[0])[1])
+    finally:
+        orc.set_mesh()
+    M = prev[0]
+    w = np.sqrt(E / LD(M))
+    eta, phi, dphi = ld(st["eta"]), ld(st["phi"]), ld(st["dphi"])
+    J = np.empty((M, n + 1), dtype=LD)
+    J[:, 0] = phi_t * w / 4
+    J[:, 1:] = dphi.T * w[:, None]
     return {"r": phi * w, "J": J, "eta": eta, "phi": phi}
 
 

@@ -153,3 +153,31 @@ def test_time_stepping_across_a_respacing(orc):
         want = ld(orc.respace(ref[k], old, new))
         assert np.abs(ld(fin[k]) - want).max() < 1e-13 * max(1.0, float(np.abs(want).max())), k
     assert abs(ld(fin["energies"])[-1] - ld(ref["energies"])[-1]) < 1e-15
+
+
+def test_shooting_with_segments_is_mesh_independent(orc):
+    """(3.17): f = r.r / 2 approximates (1/4pi) int phi(x, T/4)^2 dx and (J^T r)_k = (1/2pi) int phidot_k phi dx by the
+    trapezoidal rule with dx = E dalpha -- numbers that cannot depend on the mesh strategy.  A one-segment uniform shot and a three-
+    segment refined shot (both ends, growing M) of the same c agree in f, in the gradient J^T r and in the Gauss-Newton matrix J^T J;
+    the residual itself is the uniform one interpolated to the last mesh times sqrt(E/M).  A missing or misplaced weight fails this."""
+    from oracle import shooting
+    h, g = 1.0, 1.0
+    c = np.array([7.1, 0.02, 0.004, -0.001, 0.0005])
+    one = shooting.shoot(orc, c, 64, h, g, 24, filter=False)
+    segs = [(64, 0.4, 1.0, 0, 10), (80, 0.3, 0.6, 0, 8), (96, 0.3, 0.45, 1, 8)]
+    seg = shooting.shoot_segments(orc, c, segs, h, g, filter=False)
+    assert seg["r"].shape == (96,) and seg["J"].shape == (96, 5)
+    f1, f2 = 0.5 * one["r"] @ one["r"], 0.5 * seg["r"] @ seg["r"]
+    assert abs(f1 - f2) < 1e-12 * f1
+    g1, g2 = one["J"].T @ one["r"], seg["J"].T @ seg["r"]
+    assert np.abs(g1 - g2).max() < 1e-11 * np.abs(g1).max()
+    H1, H2 = one["J"].T @ one["J"], seg["J"].T @ seg["J"]
+    assert np.abs(H1 - H2).max() < 1e-11 * np.abs(H1).max()
+    orc.set_mesh(0.45, 1)
+    _, E, _ = xi_points(orc, 96)
+    orc.set_mesh()
+    want = ld(orc.respace(split_ld(one["phi"]), (64, 1.0, 0), (96, 0.45, 1))) * np.sqrt(E / 96)
+    assert np.abs(seg["r"] - want).max() < 1e-11 * np.abs(want).max()
+    # one segment on the uniform mesh through shoot_segments is shoot itself
+    same = shooting.shoot_segments(orc, c, [(64, 1.0, 1.0, 0, 24)], h, g, filter=False)
+    assert np.abs(same["r"] - one["r"]).max() == 0 and np.abs(same["J"] - one["J"]).max() == 0
