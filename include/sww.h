@@ -168,6 +168,14 @@ int sww_shooter_destroy(sww_shooter_t S);
 /* The residual alone (a stepper without variational columns inside the handle: what Levenberg-Marquardt needs for a trial step). */
 int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r);
 int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd);
+/* The mesh-refinement strategy of section 2.2 for every following shot: nu segments (1 <= nu <= 8; 0 returns to one
+ * uniform segment); segment l takes nsteps[l] steps of size theta[l] (T/4) / nsteps[l] on M[l] points of the mesh (rho[l], where[l]) of
+ * sww_dtn_set_mesh, and the state with all columns is respaced from l to l + 1 (sww_state_respace).  M[0] = N and rho[0] = 1 (the
+ * initial state (3.15) lives on the uniform mesh), sum(theta) = 1.  The residual then has m = M[nu-1] entries,
+ *     r_i = phi(xi_nu(alpha_i), T/4) sqrt(E_nu(alpha_i) / M_nu)      (3.17)
+ * and J is m x (n + 1); sww_shooter_dims reports m as N; the nsteps argument of sww_shoot, sww_shoot_residual and sww_lm_shoot is
+ * ignored.  SWW_F64 shooters only.  All arrays HOST.  Creates the steppers of segments 2..nu (memory: like nu shooters). */
+int sww_shooter_set_segments(sww_shooter_t S, int nu, const int* M, const double* theta, const double* rho, const int* where, const int* nsteps);
 int sww_shooter_set_method(sww_shooter_t S, int method);   /* 0: RK8 (default); 1: SDC15, the paper's quadruple-precision stepper */
 int sww_shooter_set_sigma(sww_shooter_t S, double sigma);   /* surface tension of every following shot (see sww_state_set_sigma) */
 

@@ -19,7 +19,7 @@ EXPORTS = [
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
     "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance", "sww_dtn_adjoint_rhs", "sww_shooter_set_method",
-    "sww_dtn_set_mesh", "sww_mesh_points", "sww_state_set_mesh", "sww_state_respace",
+    "sww_dtn_set_mesh", "sww_mesh_points", "sww_state_set_mesh", "sww_state_respace", "sww_shooter_set_segments",
 ]
 
 
@@ -102,6 +102,7 @@ def lib() -> ctypes.CDLL:
         L.sww_mesh_points.argtypes = [ci, cd, ci, ctypes.POINTER(cd)]
         L.sww_state_set_mesh.argtypes = [vp, cd, ci]
         L.sww_state_respace.argtypes = [vp, vp]
+        L.sww_shooter_set_segments.argtypes = [vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd), ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(ci)]
         L.sww_timing_enable.argtypes = [ci]
         L.sww_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_ulonglong), ci]
         _LIB = L
@@ -329,17 +330,27 @@ class Shooter:
         _check(lib().sww_shooter_create(self.N, self.n, float(h), float(g), prec, 0 if filter else 1, self._stream.cuda_stream,
                                         ctypes.byref(h_)), "sww_shooter_create")
         self._h = h_
+        self.m = self.N   # number of residuals (M of the last segment)
 
     def set_sigma(self, sigma: float):
         _check(lib().sww_shooter_set_sigma(self._h, float(sigma)), "sww_shooter_set_sigma")
+
+    def set_segments(self, segments):
+        """Mesh-refinement strategy of section 2.2: segments = [(M, theta, rho, where, nsteps), ...] with M_1 = N, rho_1 = 1 and
+        sum(theta) = 1; [] returns to one uniform segment.  With segments the nsteps argument of shoot/residual/solve is ignored."""
+        nu = len(segments)
+        arr = lambda t, col: (t * max(nu, 1))(*[t(sg[col]) for sg in segments])
+        _check(lib().sww_shooter_set_segments(self._h, nu, arr(ctypes.c_int, 0), arr(ctypes.c_double, 1), arr(ctypes.c_double, 2),
+                                              arr(ctypes.c_int, 3), arr(ctypes.c_int, 4)), "sww_shooter_set_segments")
+        self.m = int(segments[-1][0]) if nu else self.N
 
     def set_method(self, method: str):
         """"rk8" (default) or "sdc15" for the time stepping of every following shot"""
         _check(lib().sww_shooter_set_method(self._h, {"rk8": 0, "sdc15": 1}[method]), "sww_shooter_set_method")
 
     def shoot(self, c, nsteps: int, want_state: bool = False):
-        """-> r (N), J (n + 1, N) [= column-major N x (n + 1)]; double-double: leading axis 2 (hi, lo)"""
-        N, n = self.N, self.n
+        """-> r (m), J (n + 1, m) [= column-major m x (n + 1)], m = N or the last segment's M; double-double: leading axis 2 (hi, lo)"""
+        N, n = self.m, self.n
         cc = (ctypes.c_double * (n + 1))(*[float(x) for x in c])
         lead = (2,) if self.prec == DD else ()
         r = torch.empty(lead + (N,), dtype=torch.float64, device="cuda")
@@ -353,7 +364,7 @@ class Shooter:
     def residual(self, c, nsteps: int):
         cc = (ctypes.c_double * (self.n + 1))(*[float(x) for x in c])
         lead = (2,) if self.prec == DD else ()
-        r = torch.empty(lead + (self.N,), dtype=torch.float64, device="cuda")
+        r = torch.empty(lead + (self.m,), dtype=torch.float64, device="cuda")
         _check(lib().sww_shoot_residual(self._h, cc, int(nsteps), r.data_ptr()), "sww_shoot_residual")
         return r
 

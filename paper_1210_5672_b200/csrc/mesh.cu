@@ -192,27 +192,34 @@ int sww_state_respace(sww_state_t dst, sww_state_t src) {
     const int Mo = src->N, Mn = dst->N, ncol = 2 + 2 * src->nc;
     cudaStream_t st = dst->stream;
     SWW_CUDA(cudaStreamSynchronize(src->stream));  // the source state is complete before it is read on dst's stream
-    double *beta = nullptr, *sj = nullptr, *R = nullptr;
-    if (cudaMalloc(&beta, sizeof(double) * 3 * (size_t)Mn) != cudaSuccess || cudaMalloc(&R, sizeof(double) * (size_t)Mn * Mo) != cudaSuccess) {
-        cudaFree(beta);
-        cudaFree(R);
-        return SWW_ENOMEM;
-    }
-    sj = beta + 2 * (size_t)Mn;
     const sww_dtn_s *dn = dst->dtn, *ds = src->dtn;
-    SWW_BEGIN(KC_OTHER, st);
-    k_respace_nodes<<<(Mn + 63) / 64, 64, 0, st>>>(Mo, ds->mesh_on ? ds->mesh_rho : 1.0, ds->mesh_on ? ds->mesh_where : 0, Mn,
-                                                   dn->mesh_on ? dn->mesh_rho : 1.0, dn->mesh_on ? dn->mesh_where : 0, beta, sj);
-    SWW_LAUNCHED();
-    SWW_BEGIN(KC_OTHER, st);
-    k_respace_matrix<<<dim3((Mn + 127) / 128, Mo), 128, 0, st>>>(Mo, Mn, beta, sj, R);
-    SWW_LAUNCHED();
-    int rc = cudaGetLastError() == cudaSuccess ? SWW_OK : SWW_ECUDA;
-    if (!rc) rc = gemm_f64(st, Mn, ncol, Mo, 1.0, R, Mn, src->y, Mo, 0.0, dst->y, Mn, ncol);
-    cudaStreamSynchronize(st);
-    cudaFree(beta);
-    cudaFree(R);
-    if (rc) return rc;
+    const double rho_o = ds->mesh_on ? ds->mesh_rho : 1.0, rho_n = dn->mesh_on ? dn->mesh_rho : 1.0;
+    const int where_o = ds->mesh_on ? ds->mesh_where : 0, where_n = dn->mesh_on ? dn->mesh_where : 0;
+    const bool cached = dst->rsp_R && dst->rsp_Mo == Mo && dst->rsp_rho_o == rho_o && dst->rsp_where_o == where_o && dst->rsp_rho_n == rho_n &&
+                        dst->rsp_where_n == where_n;
+    if (!cached) {  // the matrix depends on the two meshes only: a shooting iteration builds it once per pair of segments
+        if (dst->rsp_R && dst->rsp_Mo != Mo) {
+            SWW_CUDA(cudaStreamSynchronize(st));
+            cudaFree(dst->rsp_R);
+            dst->rsp_R = nullptr;
+        }
+        if (!dst->rsp_R && cudaMalloc(&dst->rsp_R, sizeof(double) * (size_t)Mn * Mo) != cudaSuccess) return SWW_ENOMEM;
+        dst->rsp_Mo = 0;
+        double* beta = nullptr;
+        if (cudaMalloc(&beta, sizeof(double) * 3 * (size_t)Mn) != cudaSuccess) return SWW_ENOMEM;
+        SWW_BEGIN(KC_OTHER, st);
+        k_respace_nodes<<<(Mn + 63) / 64, 64, 0, st>>>(Mo, rho_o, where_o, Mn, rho_n, where_n, beta, beta + 2 * (size_t)Mn);
+        SWW_LAUNCHED();
+        SWW_BEGIN(KC_OTHER, st);
+        k_respace_matrix<<<dim3((Mn + 127) / 128, Mo), 128, 0, st>>>(Mo, Mn, beta, beta + 2 * (size_t)Mn, dst->rsp_R);
+        SWW_LAUNCHED();
+        const bool ok = cudaGetLastError() == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess;
+        cudaFree(beta);
+        if (!ok) return SWW_ECUDA;
+        dst->rsp_Mo = Mo; dst->rsp_rho_o = rho_o; dst->rsp_where_o = where_o; dst->rsp_rho_n = rho_n; dst->rsp_where_n = where_n;
+    }
+    SWW_TRY(gemm_f64(st, Mn, ncol, Mo, 1.0, dst->rsp_R, Mn, src->y, Mo, 0.0, dst->y, Mn, ncol));
+    SWW_CUDA(cudaStreamSynchronize(st));
     dst->t = src->t;
     dst->dtn->has_base = false;
     return SWW_OK;

@@ -856,7 +856,7 @@ int sww_state_energy(sww_state_t s, double* energy_hl) {
 int sww_state_destroy(sww_state_t s) {
     if (!s) return SWW_EINVAL;
     if (s->dtn) sww_dtn_destroy(s->dtn);
-    cudaFree(s->y); cudaFree(s->ys); cudaFree(s->k); cudaFree(s->w); cudaFree(s->red); cudaFree(s->sdc);
+    cudaFree(s->y); cudaFree(s->ys); cudaFree(s->k); cudaFree(s->w); cudaFree(s->red); cudaFree(s->sdc); cudaFree(s->rsp_R);
     delete s;
     return SWW_OK;
 }

@@ -19,6 +19,10 @@ struct sww_state_s {
     double* red;         // 2 doubles: energy reduction (hi, lo)
     double* sdc;         // SDC15 work space (SDC_SLOTS state vectors), allocated by the first sww_sdc_advance
     double t;
+    // sww_state_respace into this state (mesh.cu): the interpolation matrix of the last pair of meshes, kept for the next call
+    double* rsp_R;
+    int rsp_Mo, rsp_where_o, rsp_where_n;
+    double rsp_rho_o, rsp_rho_n;
     double a[RK_S][RK_S], b[RK_S], c[RK_S];
     double alo[RK_S][RK_S], blo[RK_S];  // low words of the tableau (double-double states)
     size_t mul() const { return prec == SWW_DD ? 2 : 1; }

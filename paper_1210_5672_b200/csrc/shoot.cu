@@ -10,10 +10,22 @@
 #include "dd.cuh"
 #include <new>
 #include <cstring>
+#include <cmath>
 
 using namespace sww;
 
+constexpr int SHOOT_MAX_SEG = 8;
+// one sub-interval of the mesh-refinement strategy of section 2.2; segment 0 runs on the shooter's own steppers
+struct ShootSeg {
+    int M, nsteps, where;
+    double theta, rho;
+    sww_state_t st, st0;  // the steppers of segments 1.. (with and without the columns; st0 created at the first residual-only shot)
+};
+
 struct sww_shooter_s {
+    int nseg;             // 0: one uniform segment, the step count is the argument of sww_shoot
+    ShootSeg seg[SHOOT_MAX_SEG];
+    size_t zero_len;      // doubles behind `zero`
     int N, n, prec;
     double h, g, sigma;
     unsigned flags;
@@ -66,12 +78,14 @@ __global__ void k_shoot_init(int N, int n, int isdd, size_t L, const double* __r
 
 // r = phi w ; J[:, 0] = phi_t w / 4 ; J[:, k] = dphi_k w  (w = 1/sqrt(N) as a double-double).  Outputs: fp64, or double-double planar
 // (r: hi block N, lo block N; J: hi block N (n+1), lo block N (n+1)).
-__global__ void k_shoot_out(int N, int n, int isdd, size_t L, double whi, double wlo, const double* __restrict__ y, const double* __restrict__ k0,
-                            double* __restrict__ r, double* __restrict__ J) {
+// xE (refined last segment, fp64 only; else nullptr): the weight is sqrt(E(alpha_j) / N) of (3.17)
+__global__ void k_shoot_out(int N, int n, int isdd, size_t L, double whi, double wlo, const double* __restrict__ xE, const double* __restrict__ y,
+                            const double* __restrict__ k0, double* __restrict__ r, double* __restrict__ J) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     const int col = blockIdx.y;  // 0: r ; 1: J column 0 ; 2..n+1: J columns 1..n
-    const dd w{whi, wlo};
+    dd w{whi, wlo};
+    if (xE) w = dd{sqrt(xE[j] / (double)N), 0.0};
     size_t src;
     const double* base = y;
     double scale = 1.0;
@@ -99,6 +113,7 @@ int sww_shooter_create(int N, int n, double h, double g, int prec, unsigned flag
     S->N = N; S->n = n; S->prec = prec; S->h = h; S->g = g; S->flags = flags;
     const size_t mul = prec == SWW_DD ? 2 : 1;
     const size_t nz = mul * (size_t)N * n;  // the larger of the zero arrays the create call reads (deta, dphi)
+    S->zero_len = nz;
     if (cudaMalloc(&S->c_dev, sizeof(double) * (n + 1)) != cudaSuccess || cudaMalloc(&S->zero, sizeof(double) * nz) != cudaSuccess) {
         sww_shooter_destroy(S);
         return SWW_ENOMEM;
@@ -118,21 +133,55 @@ int sww_shooter_create(int N, int n, double h, double g, int prec, unsigned flag
     return SWW_OK;
 }
 
-// one shot through the stepper s (with_cols: s carries the n variational columns and J is wanted)
-static int shoot_impl(sww_shooter_t S, sww_state_s* s, bool with_cols, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4) {
-    const int N = S->N, n = S->n, isdd = S->prec == SWW_DD;
+// the stepper of segment l, with or without the columns (those without are created at the first residual-only shot)
+static int seg_state(sww_shooter_t S, int l, bool with_cols, sww_state_s** out) {
+    sww_state_t* slot = l == 0 ? (with_cols ? &S->st : &S->st0) : (with_cols ? &S->seg[l].st : &S->seg[l].st0);
+    if (!*slot) {
+        const int M = l == 0 ? S->N : S->seg[l].M;
+        SWW_TRY(sww_state_create(M, S->h, S->g, S->prec, with_cols ? S->n : 0, S->zero, S->zero, with_cols ? S->zero : nullptr,
+                                 with_cols ? S->zero : nullptr, S->flags, S->st->stream, slot));
+        if (l > 0) SWW_TRY(sww_state_set_mesh(*slot, S->seg[l].rho, S->seg[l].where));
+    }
+    (*slot)->sigma = S->sigma;
+    *out = *slot;
+    return SWW_OK;
+}
+
+static int advance(sww_shooter_t S, sww_state_s* s, double dt, int nsteps) {
+    return S->sdc ? sww_sdc_advance(s, dt, nsteps) : sww_rk_advance(s, dt, nsteps);
+}
+
+// one shot (with_cols: the steppers carry the n variational columns and J is wanted)
+static int shoot_impl(sww_shooter_t S, bool with_cols, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4) {
+    const int n = S->n, isdd = S->prec == SWW_DD;
+    sww_state_s* s = nullptr;
+    SWW_TRY(seg_state(S, 0, with_cols, &s));
     cudaStream_t st = s->stream;
     SWW_CUDA(cudaMemcpyAsync(S->c_dev, c, sizeof(double) * (n + 1), cudaMemcpyHostToDevice, st));
     SWW_CUDA(cudaStreamSynchronize(st));  // c may be pageable host memory that the caller changes right after the call
-    const Tables* tab = s->dtn->tab;
-    const dim3 blk(128), grd((N + 127) / 128, with_cols ? n + 1 : 1);
-    SWW_BEGIN(KC_OTHER, st);
-    k_shoot_init<<<grd, blk, 0, st>>>(N, n, isdd, s->L, tab->cs, S->c_dev, s->y);
-    SWW_LAUNCHED();
-    SWW_CUDA(cudaGetLastError());
+    {
+        const int N = S->N;
+        const dim3 blk(128), grd((N + 127) / 128, with_cols ? n + 1 : 1);
+        SWW_BEGIN(KC_OTHER, st);
+        k_shoot_init<<<grd, blk, 0, st>>>(N, n, isdd, s->L, s->dtn->tab->cs, S->c_dev, s->y);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+    }
     s->t = 0.0;
-    if (S->sdc) SWW_TRY(sww_sdc_advance(s, c[0] / (4.0 * nsteps), nsteps));
-    else SWW_TRY(sww_rk_advance(s, c[0] / (4.0 * nsteps), nsteps));
+    if (S->nseg == 0) {
+        SWW_TRY(advance(S, s, c[0] / (4.0 * nsteps), nsteps));
+    } else {  // section 2.2: segment l takes nsteps_l steps over theta_l T/4 on its own mesh; respacing in between
+        for (int l = 0; l < S->nseg; l++) {
+            if (l > 0) {
+                sww_state_s* nx = nullptr;
+                SWW_TRY(seg_state(S, l, with_cols, &nx));
+                SWW_TRY(sww_state_respace(nx, s));
+                s = nx;
+            }
+            SWW_TRY(advance(S, s, S->seg[l].theta * c[0] / (4.0 * S->seg[l].nsteps), S->seg[l].nsteps));
+        }
+    }
+    const int N = s->N;  // the residual count m = M_nu
     if (with_cols) SWW_TRY(rk_rhs(s, s->y, s->k));  // phi_t at T/4 (stage slot 0)
     // w = 1/sqrt(N), N = 2^p: a power of two, times 1/sqrt(2) (double-double) when p is odd
     int p = 0;
@@ -142,33 +191,80 @@ static int shoot_impl(sww_shooter_t S, sww_state_s* s, bool with_cols, const dou
         whi = ldexp(0.70710678118654757, -(p / 2));
         wlo = ldexp(-4.8336466567264567e-17, -(p / 2));
     }
-    const dim3 grd2((N + 127) / 128, with_cols ? n + 2 : 1);
+    const dim3 blk(128), grd2((N + 127) / 128, with_cols ? n + 2 : 1);
     SWW_BEGIN(KC_OTHER, st);
-    k_shoot_out<<<grd2, blk, 0, st>>>(N, n, isdd, s->L, whi, wlo, s->y, s->k, (double*)r, (double*)J);
+    k_shoot_out<<<grd2, blk, 0, st>>>(N, n, isdd, s->L, whi, wlo, s->dtn->mesh_on ? s->dtn->mesh.xE : nullptr, s->y, s->k, (double*)r, (double*)J);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return sww_state_read(s, eta_T4, phi_T4, nullptr, nullptr, nullptr);  // synchronises; the sticky status of the stepper's DtN handle
 }
 
 int sww_shoot(sww_shooter_t S, const double* c, int nsteps, void* r, void* J, void* eta_T4, void* phi_T4) {
-    if (!S || !c || nsteps < 1 || !r || !J) return SWW_EINVAL;
+    if (!S || !c || (S->nseg == 0 && nsteps < 1) || !r || !J) return SWW_EINVAL;
     if (!(c[0] > 0.0)) return SWW_EINVAL;  // the period
-    return shoot_impl(S, S->st, true, c, nsteps, r, J, eta_T4, phi_T4);
+    return shoot_impl(S, true, c, nsteps, r, J, eta_T4, phi_T4);
 }
 
 int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r) {
-    if (!S || !c || nsteps < 1 || !r) return SWW_EINVAL;
+    if (!S || !c || (S->nseg == 0 && nsteps < 1) || !r) return SWW_EINVAL;
     if (!(c[0] > 0.0)) return SWW_EINVAL;
-    if (!S->st0) SWW_TRY(sww_state_create(S->N, S->h, S->g, S->prec, 0, S->zero, S->zero, nullptr, nullptr, S->flags, S->st->stream, &S->st0));
-    S->st0->sigma = S->sigma;
-    return shoot_impl(S, S->st0, false, c, nsteps, r, nullptr, nullptr, nullptr);
+    return shoot_impl(S, false, c, nsteps, r, nullptr, nullptr, nullptr);
+}
+
+static void free_segments(sww_shooter_t S) {
+    for (int l = 1; l < S->nseg; l++) {
+        if (S->seg[l].st) sww_state_destroy(S->seg[l].st);
+        if (S->seg[l].st0) sww_state_destroy(S->seg[l].st0);
+        S->seg[l].st = S->seg[l].st0 = nullptr;
+    }
+    S->nseg = 0;
+}
+
+int sww_shooter_set_segments(sww_shooter_t S, int nu, const int* M, const double* theta, const double* rho, const int* where, const int* nsteps) {
+    if (!S || nu < 0 || nu > SHOOT_MAX_SEG) return SWW_EINVAL;
+    if (nu == 0) {
+        free_segments(S);
+        return SWW_OK;
+    }
+    if (S->prec != SWW_F64 || !M || !theta || !rho || !where || !nsteps) return SWW_EINVAL;  // refined meshes: fp64 steppers (sww_state_set_mesh)
+    if (M[0] != S->N || rho[0] != 1.0) return SWW_EINVAL;  // the initial state (3.15) lives on the uniform mesh (rho_1 = 1)
+    double sum = 0.0;
+    size_t need = S->zero_len;
+    for (int l = 0; l < nu; l++) {
+        if (!(theta[l] > 0.0) || !(rho[l] > 0.0 && rho[l] <= 1.0) || (where[l] != 0 && where[l] != 1) || nsteps[l] < 1 || M[l] < 16) return SWW_EINVAL;
+        sum += theta[l];
+        need = need > (size_t)M[l] * S->n ? need : (size_t)M[l] * S->n;
+    }
+    if (fabs(sum - 1.0) > 1e-12) return SWW_EINVAL;
+    free_segments(S);
+    if (need > S->zero_len) {
+        SWW_CUDA(cudaStreamSynchronize(S->st->stream));
+        cudaFree(S->zero);
+        S->zero = nullptr;
+        S->zero_len = 0;
+        SWW_CUDA(cudaMalloc(&S->zero, sizeof(double) * need));
+        SWW_CUDA(cudaMemsetAsync(S->zero, 0, sizeof(double) * need, S->st->stream));
+        S->zero_len = need;
+    }
+    for (int l = 0; l < nu; l++) {
+        S->seg[l].M = M[l]; S->seg[l].theta = theta[l]; S->seg[l].rho = rho[l]; S->seg[l].where = where[l]; S->seg[l].nsteps = nsteps[l];
+        S->seg[l].st = S->seg[l].st0 = nullptr;
+    }
+    S->nseg = nu;
+    for (int l = 1; l < nu; l++) {  // the steppers with the columns now (validates the sizes); those without at the first residual-only shot
+        sww_state_s* s = nullptr;
+        const int rc = seg_state(S, l, true, &s);
+        if (rc) {
+            free_segments(S);
+            return rc;
+        }
+    }
+    return SWW_OK;
 }
 
 int sww_shooter_set_sigma(sww_shooter_t S, double sigma) {
     if (!S || !(sigma >= 0.0)) return SWW_EINVAL;
-    S->sigma = sigma;
-    S->st->sigma = sigma;
-    if (S->st0) S->st0->sigma = sigma;
+    S->sigma = sigma;  // handed to every stepper at its next shot (seg_state)
     return SWW_OK;
 }
 
@@ -180,7 +276,7 @@ int sww_shooter_set_method(sww_shooter_t S, int method) {
 
 int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd) {
     if (!S) return SWW_EINVAL;
-    if (N) *N = S->N;
+    if (N) *N = S->nseg > 0 ? S->seg[S->nseg - 1].M : S->N;  // the number of residuals m = M_nu (3.17)
     if (n) *n = S->n;
     if (is_dd) *is_dd = S->prec == SWW_DD;
     return SWW_OK;
@@ -188,6 +284,7 @@ int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd) {
 
 int sww_shooter_destroy(sww_shooter_t S) {
     if (!S) return SWW_EINVAL;
+    free_segments(S);
     if (S->st) sww_state_destroy(S->st);
     if (S->st0) sww_state_destroy(S->st0);
     cudaFree(S->c_dev);

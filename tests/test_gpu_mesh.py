@@ -258,3 +258,68 @@ def test_uniform_mesh_is_untouched_and_errors(sww):
     with pytest.raises(sww.SwwError):
         sdd.set_mesh(0.5, 0)
     sdd.set_mesh(1.0, 0)
+
+
+def shoot_unknowns(n, T=7.0, amp=-0.02, seed=3):
+    rng = np.random.default_rng(seed)
+    c = np.zeros(n + 1)
+    c[0], c[1] = T, amp
+    for k in range(2, n + 1):
+        c[k] = 0.2 * abs(amp) * rng.standard_normal() * np.exp(-0.7 * k)
+    return c
+
+
+@pytest.mark.parametrize("segs", [[(64, 0.5, 1.0, 0, 4), (128, 0.5, 0.5, 0, 6)],
+                                  [(128, 0.3, 1.0, 0, 3), (128, 0.3, 0.6, 1, 3), (256, 0.4, 0.4, 0, 6)]])
+def test_shooting_map_with_segments(sww, mesh_ld, segs):
+    """sww_shooter_set_segments: r (3.17) with the weight sqrt(E/M) and J (3.31) on the last mesh against oracle/shooting.shoot_segments"""
+    from oracle import shooting
+    n = 6
+    c = shoot_unknowns(n)
+    S = sww.Shooter(segs[0][0], n, 1.0, 1.0)
+    S.set_segments(segs)
+    r, J, eta, phi = S.shoot(c, 1, want_state=True)
+    o = shooting.shoot_segments(mesh_ld, c, segs, 1.0, 1.0)
+    m, rho = segs[-1][0], min(sg[2] for sg in segs)
+    assert r.shape == (m,) and J.shape == (n + 1, m)
+    tol = 1e-11 / rho ** 2
+    assert float(np.abs(r.cpu().numpy().astype(LD) - o["r"]).max() / np.abs(o["r"]).max()) <= tol
+    e = np.abs(J.cpu().numpy().astype(LD) - o["J"].T).max(axis=1) / np.abs(o["J"].T).max(axis=1)
+    assert float(e.max()) <= tol, e
+    assert float(np.abs(eta.cpu().numpy().astype(LD) - o["eta"]).max() / np.abs(o["eta"]).max()) <= tol
+    r0 = S.residual(c, 1)                                   # the steppers without columns: the same residual
+    assert float((r0 - r).abs().max()) <= 1e-13 * float(r.abs().max())
+    r2, J2 = S.shoot(c, 1)                                  # repeatable through the cached interpolation matrices
+    assert torch.equal(r, r2) and torch.equal(J, J2)
+    S.set_segments([])                                      # back to one uniform segment
+    r1, _ = S.shoot(c, 8)
+    assert r1.shape == (segs[0][0],)
+    S.close()
+
+
+def test_levenberg_marquardt_on_a_refined_mesh(sww):
+    """the small-amplitude branch through the segmented device path: the period converges to the printed T = 7.19976"""
+    n, eps = 4, 1e-6
+    S = sww.Shooter(32, n, 1.0, 1.0)
+    S.set_segments([(32, 0.5, 1.0, 0, 8), (64, 0.5, 0.5, 0, 8)])
+    c0 = [7.0, eps, 0.0, 0.0, 0.0]
+    c, rep = S.solve(c0, 1, fixed=[0, 1, 0, 0, 0])
+    assert abs(c[0] - 7.19976) < 1e-5, (c, rep)
+    assert rep["f"] < 1e-24
+    S.close()
+
+
+def test_segment_errors(sww):
+    S = sww.Shooter(64, 4, 1.0, 1.0)
+    for bad in ([(32, 1.0, 1.0, 0, 4)],                              # M_1 must be the shooter's N
+                [(64, 1.0, 0.5, 0, 4)],                              # rho_1 = 1
+                [(64, 0.5, 1.0, 0, 4), (128, 0.4, 0.5, 0, 4)],       # theta must sum to one
+                [(64, 0.5, 1.0, 0, 4), (128, 0.5, 0.5, 0, 0)],       # at least one step
+                [(64, 0.5, 1.0, 0, 4), (100, 0.5, 0.5, 0, 4)]):      # sizes the stepper supports
+        with pytest.raises(sww.SwwError):
+            S.set_segments(bad)
+    S.close()
+    Sd = sww.Shooter(64, 4, 1.0, 1.0, prec=sww.DD)
+    with pytest.raises(sww.SwwError):
+        Sd.set_segments([(64, 0.5, 1.0, 0, 4), (128, 0.5, 0.5, 0, 4)])
+    Sd.close()
