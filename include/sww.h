@@ -140,13 +140,14 @@ int sww_state_destroy(sww_state_t s);
  * sww_mesh_points: x (HOST, N doubles) <- xi(alpha_j). */
 int sww_dtn_set_mesh(sww_dtn_t d, double rho, int where);
 int sww_mesh_points(int N, double rho, int where, double* x);
-/* The time stepper on a refined mesh (SWW_F64 states only; SWW_DD: SWW_EINVAL unless rho = 1): the filter (2.14) acts on the stored
+/* The time stepper on a refined mesh (either precision, RK8 or SDC15): the filter (2.14) acts on the stored
  * samples, P removes the mean over x, (1/N) sum_j f_j xi'(alpha_j) (the trapezoidal rule with dx = xi' dalpha), and the
  * energy integral carries the same weight.  Call before advancing; the state's arrays are then values at x_j.
  * sww_state_respace: dst's state (eta, phi and all columns) <- src's, interpolated to dst's mesh: beta_j =
  * xi_src^{-1}(xi_dst(alpha_j)) by Newton's method in double-double, values at beta_j from the trigonometric interpolant of src's samples
- * (one M_dst x M_src matrix applied to all 2 + 2 ncols columns at once).  dst and src: two SWW_F64 handles with the same ncols and
- * any two sizes and meshes; dst's elapsed time becomes src's.  Synchronises both streams. */
+ * (one M_dst x M_src matrix applied to all 2 + 2 ncols columns at once; kept in dst for the next call with the same pair of meshes).
+ * dst and src: two handles of the same precision with the same ncols and any two sizes and meshes (SWW_DD: the matrix and the
+ * product in double-double); dst's elapsed time becomes src's.  Synchronises both streams. */
 int sww_state_set_mesh(sww_state_t s, double rho, int where);
 int sww_state_respace(sww_state_t dst, sww_state_t src);
 
@@ -174,7 +175,8 @@ int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd);
  * initial state (3.15) lives on the uniform mesh), sum(theta) = 1.  The residual then has m = M[nu-1] entries,
  *     r_i = phi(xi_nu(alpha_i), T/4) sqrt(E_nu(alpha_i) / M_nu)      (3.17)
  * and J is m x (n + 1); sww_shooter_dims reports m as N; the nsteps argument of sww_shoot, sww_shoot_residual and sww_lm_shoot is
- * ignored.  SWW_F64 shooters only.  All arrays HOST.  Creates the steppers of segments 2..nu (memory: like nu shooters). */
+ * ignored.  Either precision (SWW_DD with sww_shooter_set_method(S, 1) is the paper's quadruple-precision configuration of Table 3).
+ * All arrays HOST.  Creates the steppers of segments 2..nu (memory: like nu shooters). */
 int sww_shooter_set_segments(sww_shooter_t S, int nu, const int* M, const double* theta, const double* rho, const int* where, const int* nsteps);
 int sww_shooter_set_method(sww_shooter_t S, int method);   /* 0: RK8 (default); 1: SDC15, the paper's quadruple-precision stepper */
 int sww_shooter_set_sigma(sww_shooter_t S, double sigma);   /* surface tension of every following shot (see sww_state_set_sigma) */

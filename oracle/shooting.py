@@ -148,3 +148,40 @@ def shoot_quad(orc, c, N: int, h: float, g: float, nsteps: int, filter: bool = T
         rr = sp(r)
         Js = [sp(col) for col in Jc]
         return {"r": rr, "J": (np.stack([j[0] for j in Js], axis=1), np.stack([j[1] for j in Js], axis=1))}
+
+
+def shoot_segments_quad(orc, c, segments, h: float, g: float, filter: bool = True, sigma: float = 0.0, method: str = "rk8"):
+    """shoot_segments for the __float128 oracle (initial state and the weights sqrt(E/M) to ~40 digits): -> dict r (hi, lo),
+    J (hi, lo) with J[.] of shape (M_nu, n + 1)"""
+    import mpmath as mp
+    c = np.asarray(c, dtype=np.float64)
+    n = c.shape[0] - 1
+    T = float(c[0])
+    M1, _, rho1, _, _ = segments[0]
+    assert rho1 == 1.0 and abs(sum(sg[1] for sg in segments) - 1.0) < 1e-12
+    eta0, phi0, deta0, dphi0 = initial_state_quad(c, M1)
+    st = {"eta": eta0, "phi": phi0, "deta": deta0, "dphi": dphi0}
+    prev = None
+    try:
+        for (M, theta, rho, where, nst) in segments:
+            if prev is not None:
+                st = {k: orc.respace(st[k], prev, (M, rho, where)) for k in ("eta", "phi", "deta", "dphi")}
+            orc.set_mesh(rho, where)
+            st = orc.rk_advance(st["eta"], st["phi"], h, g, theta * T / (4 * nst), nst, deta=st["deta"], dphi=st["dphi"], filter=filter,
+                                sigma=sigma, method=method)
+            prev = (M, rho, where)
+        phi_t = orc.rhs(st["eta"], st["phi"], h, g, filter=filter, sigma=sigma)["phi_t"]
+        E = orc.mesh_tables(prev[0])[1]
+    finally:
+        orc.set_mesh()
+    M = prev[0]
+    with mp.workprec(160):
+        val = lambda p, i: mp.mpf(float(p[0][i])) + mp.mpf(float(p[1][i]))
+        w = [mp.sqrt(val(E, i) / M) for i in range(M)]
+        r = [val(st["phi"], i) * w[i] for i in range(M)]
+        Jc = [[val(phi_t, i) * w[i] / 4 for i in range(M)]]
+        for k in range(n):
+            Jc.append([(mp.mpf(float(st["dphi"][0][k][i])) + mp.mpf(float(st["dphi"][1][k][i]))) * w[i] for i in range(M)])
+        sp = lambda v: tuple(np.array(t, dtype=np.float64) for t in zip(*[_mp_split(x) for x in v]))
+        Js = [sp(col) for col in Jc]
+        return {"r": sp(r), "J": (np.stack([j[0] for j in Js], axis=1), np.stack([j[1] for j in Js], axis=1))}

@@ -78,6 +78,7 @@ struct MeshDev {
     const double* xE1;  // xi''(alpha_j)
     const double* xS;   // sin(xi(alpha_j) - alpha_j)
     const double* xC;   // cos(xi(alpha_j) - alpha_j)
+    const double* coef; // 4 doubles: a1 (hi, lo), a2 (hi, lo) of E = 1 + a1 cos(alpha) + a2 cos(2 alpha)
 };
 
 // ---------------------------------------------------------------- the DtN handle

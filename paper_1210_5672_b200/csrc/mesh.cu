@@ -6,7 +6,8 @@
 //   the factor 1/|xi'| of (2.8) and d/dx = (1/xi') d/dalpha elsewhere (api.cu, ddpath.cu, rk.cu).
 //   Respacing between segments: f o xi_new(alpha_j) = (f o xi_old)(beta_j), beta_j = xi_old^{-1}(xi_new(alpha_j)) by
 //   Newton's method; the values at beta_j come from the trigonometric interpolant of the old samples, written as one matrix
-//   R (M_new x M_old, the periodic Dirichlet kernel) applied to all state columns at once by the library's fp64 GEMM.
+//   R (M_new x M_old, the periodic Dirichlet kernel) applied to all state columns at once by the library's fp64 GEMM (double-double
+//   states: the matrix and the product in double-double).
 // Product code; shares nothing with oracle/.
 #include "rk.cuh"
 #include "dd.cuh"
@@ -40,11 +41,14 @@ __device__ inline void dd_sincos_any(dd x, dd* s, dd* c) {
 
 // per-node tables of the handle: xE, xE1, xS, xC (dd planar 2N each), from the exact per-N tables cs, sn of cos, sin(2 pi m / N)
 __global__ void k_mesh_tables(int N, double rho, int where, const double* __restrict__ cs, const double* __restrict__ sn, double* __restrict__ xE,
-                              double* __restrict__ xE1, double* __restrict__ xS, double* __restrict__ xC) {
+                              double* __restrict__ xE1, double* __restrict__ xS, double* __restrict__ xC, double* __restrict__ coef) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     const dd A = mesh_A(rho);
     const dd a1 = where == 0 ? dd_half(A) : dd_neg(dd_half(A)), a2 = dd_neg(dd_ldexp(A, -3));
+    if (j == 0) {
+        coef[0] = a1.hi; coef[1] = a1.lo; coef[2] = a2.hi; coef[3] = a2.lo;
+    }
     const int j2 = (2 * j) & (N - 1);
     const dd c1 = dd_load(cs, N, j), s1 = dd_load(sn, N, j), c2 = dd_load(cs, N, j2), s2 = dd_load(sn, N, j2);
     dd_store(xE, N, j, dd_add(dd_add_d(dd_mul(a1, c1), 1.0), dd_mul(a2, c2)));
@@ -95,7 +99,7 @@ __device__ inline void mesh_xi_dd(dd A, int where, dd b, dd* xi, dd* E) {
 
 // beta_j = xi_old^{-1}(xi_new(alpha_j)), alpha_j = 2 pi j / Mn, by Newton's method in dd; sj = sin(Mo beta_j / 2)
 __global__ void k_respace_nodes(int Mo, double rho_o, int where_o, int Mn, double rho_n, int where_n, double* __restrict__ beta /* dd planar 2 Mn */,
-                                double* __restrict__ sj) {
+                                double* __restrict__ sj /* dd planar 2 Mn */) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= Mn) return;
     const dd An = mesh_A(rho_n), Ao = mesh_A(rho_o);
@@ -114,6 +118,7 @@ __global__ void k_respace_nodes(int Mo, double rho_o, int where_o, int Mn, doubl
     dd s, c;
     dd_sincos_any(dd_mul_d(b, 0.5 * (double)Mo), &s, &c);
     sj[j] = s.hi;
+    sj[Mn + j] = s.lo;
 }
 
 // R[j + m Mn] = D(beta_j - alpha_m), alpha_m = 2 pi m / Mo, D(t) = (1/Mo) sin(Mo t / 2) cot(t / 2) the periodic Dirichlet kernel of Mo
@@ -134,6 +139,43 @@ __global__ void k_respace_matrix(int Mo, int Mn, const double* __restrict__ beta
     R[(size_t)j + (size_t)m * Mn] = v;
 }
 
+// the same matrix in double-double (planar, plane size Mn Mo): cot(t/2) from the dd sine and cosine
+__global__ void k_respace_matrix_dd(int Mo, int Mn, const double* __restrict__ beta, const double* __restrict__ sj, double* __restrict__ R) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, m = blockIdx.y;
+    if (j >= Mn) return;
+    const dd am = dd_div_d(dd_mul_d(dd_mul_d(dd_pi(), 2.0), (double)m), (double)Mo);
+    const dd th = dd_half(dd_sub(dd_load(beta, Mn, j), am));
+    dd v{1.0, 0.0};
+    if (fabs(th.hi) >= 1e-20) {   // below: 1 - O((Mo t)^2) = 1 in dd
+        dd sn, cn;
+        dd_sincos_any(th, &sn, &cn);
+        v = dd_div_d(dd_div(dd_mul(dd_load(sj, Mn, j), cn), sn), (double)Mo);
+        if (m & 1) v = dd_neg(v);
+    }
+    const size_t o = (size_t)j + (size_t)m * Mn;
+    R[o] = v.hi;
+    R[(size_t)Mn * Mo + o] = v.lo;
+}
+// out (Mn x ncol, planes Lout apart) = R (Mn x Mo, dd planar) y (Mo x ncol, planes Lin apart), one thread per output entry
+__global__ void k_respace_apply_dd(int Mo, int Mn, int ncol, const double* __restrict__ R, const double* __restrict__ y, size_t Lin,
+                                   double* __restrict__ out, size_t Lout) {
+    const int j = blockIdx.x * blockDim.x + threadIdx.x, c = blockIdx.y;
+    if (j >= Mn) return;
+    const size_t plane = (size_t)Mn * Mo;
+    const double* yc = y + (size_t)c * Mo;
+    dd acc[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};  // independent chains
+    for (int m = 0; m < Mo; m += 4) {
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const size_t o = (size_t)j + (size_t)(m + q) * Mn;
+            acc[q] = dd_fma(dd{R[o], R[plane + o]}, dd{yc[m + q], yc[Lin + m + q]}, acc[q]);
+        }
+    }
+    const dd r = dd_add(dd_add(acc[0], acc[1]), dd_add(acc[2], acc[3]));
+    out[(size_t)c * Mn + j] = r.hi;
+    out[Lout + (size_t)c * Mn + j] = r.lo;
+}
+
 }  // namespace sww
 
 extern "C" {
@@ -149,7 +191,8 @@ int sww_dtn_set_mesh(sww_dtn_t d, double rho, int where) {
         return SWW_OK;
     }
     if (!d->mesh_buf) {
-        SWW_CUDA(cudaMalloc(&d->mesh_buf, sizeof(double) * 8 * (size_t)N));
+        SWW_CUDA(cudaMalloc(&d->mesh_buf, sizeof(double) * (8 * (size_t)N + 4)));
+        d->mesh.coef = d->mesh_buf + 8 * (size_t)N;
         d->mesh.xE = d->mesh_buf;
         d->mesh.xE1 = d->mesh_buf + 2 * (size_t)N;
         d->mesh.xS = d->mesh_buf + 4 * (size_t)N;
@@ -157,7 +200,7 @@ int sww_dtn_set_mesh(sww_dtn_t d, double rho, int where) {
     }
     SWW_BEGIN(KC_OTHER, d->stream);
     k_mesh_tables<<<(N + 127) / 128, 128, 0, d->stream>>>(N, rho, where, d->tab->cs, d->tab->sn, d->mesh_buf, d->mesh_buf + 2 * (size_t)N,
-                                                        d->mesh_buf + 4 * (size_t)N, d->mesh_buf + 6 * (size_t)N);
+                                                        d->mesh_buf + 4 * (size_t)N, d->mesh_buf + 6 * (size_t)N, d->mesh_buf + 8 * (size_t)N);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     const double A = 8.0 * (1.0 - rho) / (5.0 + 3.0 * rho);
@@ -182,14 +225,15 @@ int sww_mesh_points(int N, double rho, int where, double* x) {
 
 int sww_state_set_mesh(sww_state_t s, double rho, int where) {
     if (!s) return SWW_EINVAL;
-    if (s->prec == SWW_DD && rho != 1.0) return SWW_EINVAL;  // the double-double stepper runs on the uniform mesh only
     return sww_dtn_set_mesh(s->dtn, rho, where);
 }
 
 int sww_state_respace(sww_state_t dst, sww_state_t src) {
     if (!dst || !src || dst == src) return SWW_EINVAL;
-    if (dst->prec != SWW_F64 || src->prec != SWW_F64 || dst->nc != src->nc) return SWW_EINVAL;
+    if (dst->prec != src->prec || dst->nc != src->nc) return SWW_EINVAL;
     const int Mo = src->N, Mn = dst->N, ncol = 2 + 2 * src->nc;
+    const bool isdd = dst->prec == SWW_DD;
+    const size_t rmul = isdd ? 2 : 1;
     cudaStream_t st = dst->stream;
     SWW_CUDA(cudaStreamSynchronize(src->stream));  // the source state is complete before it is read on dst's stream
     const sww_dtn_s *dn = dst->dtn, *ds = src->dtn;
@@ -203,22 +247,31 @@ int sww_state_respace(sww_state_t dst, sww_state_t src) {
             cudaFree(dst->rsp_R);
             dst->rsp_R = nullptr;
         }
-        if (!dst->rsp_R && cudaMalloc(&dst->rsp_R, sizeof(double) * (size_t)Mn * Mo) != cudaSuccess) return SWW_ENOMEM;
+        if (!dst->rsp_R && cudaMalloc(&dst->rsp_R, sizeof(double) * rmul * (size_t)Mn * Mo) != cudaSuccess) return SWW_ENOMEM;
         dst->rsp_Mo = 0;
         double* beta = nullptr;
-        if (cudaMalloc(&beta, sizeof(double) * 3 * (size_t)Mn) != cudaSuccess) return SWW_ENOMEM;
+        if (cudaMalloc(&beta, sizeof(double) * 4 * (size_t)Mn) != cudaSuccess) return SWW_ENOMEM;
         SWW_BEGIN(KC_OTHER, st);
         k_respace_nodes<<<(Mn + 63) / 64, 64, 0, st>>>(Mo, rho_o, where_o, Mn, rho_n, where_n, beta, beta + 2 * (size_t)Mn);
         SWW_LAUNCHED();
         SWW_BEGIN(KC_OTHER, st);
-        k_respace_matrix<<<dim3((Mn + 127) / 128, Mo), 128, 0, st>>>(Mo, Mn, beta, beta + 2 * (size_t)Mn, dst->rsp_R);
+        if (isdd) k_respace_matrix_dd<<<dim3((Mn + 127) / 128, Mo), 128, 0, st>>>(Mo, Mn, beta, beta + 2 * (size_t)Mn, dst->rsp_R);
+        else k_respace_matrix<<<dim3((Mn + 127) / 128, Mo), 128, 0, st>>>(Mo, Mn, beta, beta + 2 * (size_t)Mn, dst->rsp_R);
         SWW_LAUNCHED();
         const bool ok = cudaGetLastError() == cudaSuccess && cudaStreamSynchronize(st) == cudaSuccess;
         cudaFree(beta);
         if (!ok) return SWW_ECUDA;
         dst->rsp_Mo = Mo; dst->rsp_rho_o = rho_o; dst->rsp_where_o = where_o; dst->rsp_rho_n = rho_n; dst->rsp_where_n = where_n;
     }
-    SWW_TRY(gemm_f64(st, Mn, ncol, Mo, 1.0, dst->rsp_R, Mn, src->y, Mo, 0.0, dst->y, Mn, ncol));
+    if (isdd) {
+        if (Mo % 4 != 0) return SWW_EINVAL;
+        SWW_BEGIN(KC_DDGEMM, st);
+        k_respace_apply_dd<<<dim3((Mn + 127) / 128, ncol), 128, 0, st>>>(Mo, Mn, ncol, dst->rsp_R, src->y, src->L, dst->y, dst->L);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+    } else {
+        SWW_TRY(gemm_f64(st, Mn, ncol, Mo, 1.0, dst->rsp_R, Mn, src->y, Mo, 0.0, dst->y, Mn, ncol));
+    }
     SWW_CUDA(cudaStreamSynchronize(st));
     dst->t = src->t;
     dst->dtn->has_base = false;

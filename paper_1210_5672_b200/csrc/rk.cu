@@ -545,14 +545,15 @@ static int rk_rhs_dd(sww_state_s* s, const double* ys, double* kout) {
     SWW_TRY(setup_surface(d, ys, ys + L));          // S0-S2 for this stage's surface (eta: high and low planes)
     SWW_TRY(accurate_base(d, ys + N, L));           // W0 = G phi, u, v of (2.9)
     d->has_base = true;
-    SWW_TRY(rkdd_rhs_base(d, s->filter, s->g, L, ys, kout));
-    if (s->sigma != 0.0) SWW_TRY(rkdd_st_base(d, s->filter, s->sigma, L, kout));
+    const bool st_apart = s->sigma != 0.0 && !d->mesh_on;  // on a refined mesh the surface-tension terms are inside the mesh kernels
+    SWW_TRY(rkdd_rhs_base(d, s->filter, s->g, s->sigma, L, ys, kout));
+    if (st_apart) SWW_TRY(rkdd_st_base(d, s->filter, s->sigma, L, kout));
     if (nc > 0) {
         const double* deta = ys + 2 * (size_t)N;
         const double* dphi = deta + (size_t)N * nc;
         SWW_TRY(dd_linearized(d, deta, dphi, nc, s->w, L, 0));   // w_c - D(u deta_c)   (B.1d), (B.2)
-        SWW_TRY(rkdd_rhs_cols(d, s->filter, s->g, nc, L, ys, s->w, kout));
-        if (s->sigma != 0.0) SWW_TRY(rkdd_st_cols(d, s->filter, s->sigma, nc, L, ys, kout));
+        SWW_TRY(rkdd_rhs_cols(d, s->filter, s->g, s->sigma, nc, L, ys, s->w, kout));
+        if (st_apart) SWW_TRY(rkdd_st_cols(d, s->filter, s->sigma, nc, L, ys, kout));
     }
     return SWW_OK;
 }

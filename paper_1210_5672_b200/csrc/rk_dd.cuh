@@ -18,9 +18,9 @@ struct CombDD {
 int rkdd_set_attrs();
 int rkdd_combine(cudaStream_t st, size_t L, const double* y, const double* k, const CombDD& cb, double* out);
 // eta_t, phi_t of (2.1) at the stage state ys from the base state held by d (set_base done) -> kout
-int rkdd_rhs_base(sww_dtn_s* d, bool filter, double g, size_t L, const double* ys, double* kout);
+int rkdd_rhs_base(sww_dtn_s* d, bool filter, double g, double sigma, size_t L, const double* ys, double* kout);  // sigma: used on a refined mesh only
 // deta_t, dphi_t of (B.1)-(B.3) for nc columns; wout: the linearized DtN of the columns, dd planar with plane size N nc
-int rkdd_rhs_cols(sww_dtn_s* d, bool filter, double g, int nc, size_t L, const double* ys, const double* wout, double* kout);
+int rkdd_rhs_cols(sww_dtn_s* d, bool filter, double g, double sigma, int nc, size_t L, const double* ys, const double* wout, double* kout);
 // surface tension (2.1b), (B.4): the curvature term and its variation added to phi_t / dphi_t in kout (sigma != 0 only)
 int rkdd_st_base(sww_dtn_s* d, bool filter, double sigma, size_t L, double* kout);
 int rkdd_st_cols(sww_dtn_s* d, bool filter, double sigma, int nc, size_t L, const double* ys, double* kout);

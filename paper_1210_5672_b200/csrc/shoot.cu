@@ -78,14 +78,14 @@ __global__ void k_shoot_init(int N, int n, int isdd, size_t L, const double* __r
 
 // r = phi w ; J[:, 0] = phi_t w / 4 ; J[:, k] = dphi_k w  (w = 1/sqrt(N) as a double-double).  Outputs: fp64, or double-double planar
 // (r: hi block N, lo block N; J: hi block N (n+1), lo block N (n+1)).
-// xE (refined last segment, fp64 only; else nullptr): the weight is sqrt(E(alpha_j) / N) of (3.17)
+// xE (refined last segment, dd planar; else nullptr): the weight is sqrt(E(alpha_j) / N) of (3.17)
 __global__ void k_shoot_out(int N, int n, int isdd, size_t L, double whi, double wlo, const double* __restrict__ xE, const double* __restrict__ y,
                             const double* __restrict__ k0, double* __restrict__ r, double* __restrict__ J) {
     const int j = blockIdx.x * blockDim.x + threadIdx.x;
     if (j >= N) return;
     const int col = blockIdx.y;  // 0: r ; 1: J column 0 ; 2..n+1: J columns 1..n
     dd w{whi, wlo};
-    if (xE) w = dd{sqrt(xE[j] / (double)N), 0.0};
+    if (xE) w = isdd ? dd_sqrt(dd_div_d(dd{xE[j], xE[N + j]}, (double)N)) : dd{sqrt(xE[j] / (double)N), 0.0};
     size_t src;
     const double* base = y;
     double scale = 1.0;
@@ -226,14 +226,15 @@ int sww_shooter_set_segments(sww_shooter_t S, int nu, const int* M, const double
         free_segments(S);
         return SWW_OK;
     }
-    if (S->prec != SWW_F64 || !M || !theta || !rho || !where || !nsteps) return SWW_EINVAL;  // refined meshes: fp64 steppers (sww_state_set_mesh)
+    if (!M || !theta || !rho || !where || !nsteps) return SWW_EINVAL;
     if (M[0] != S->N || rho[0] != 1.0) return SWW_EINVAL;  // the initial state (3.15) lives on the uniform mesh (rho_1 = 1)
     double sum = 0.0;
     size_t need = S->zero_len;
     for (int l = 0; l < nu; l++) {
         if (!(theta[l] > 0.0) || !(rho[l] > 0.0 && rho[l] <= 1.0) || (where[l] != 0 && where[l] != 1) || nsteps[l] < 1 || M[l] < 16) return SWW_EINVAL;
         sum += theta[l];
-        need = need > (size_t)M[l] * S->n ? need : (size_t)M[l] * S->n;
+        const size_t nl = (S->prec == SWW_DD ? 2 : 1) * (size_t)M[l] * S->n;
+        need = need > nl ? need : nl;
     }
     if (fabs(sum - 1.0) > 1e-12) return SWW_EINVAL;
     free_segments(S);

@@ -255,9 +255,73 @@ def test_uniform_mesh_is_untouched_and_errors(sww):
     with pytest.raises(sww.SwwError):
         d.adjoint_rhs(dev(deta), dev(dphi))
     sdd = sww.State(to_dev(eta, None, "dd"), to_dev(phi, None, "dd"), h, 1.0, prec=sww.DD)
+    s64 = sww.State(dev(eta), dev(phi), h, 1.0)
     with pytest.raises(sww.SwwError):
-        sdd.set_mesh(0.5, 0)
-    sdd.set_mesh(1.0, 0)
+        s64.respace_from(sdd)                              # the two states must have the same precision and column count
+
+
+def dd_err(got, ref):
+    """per row: max |got - ref| / max |ref| for a (2, ..., N) double-double tensor against an oracle (hi, lo) pair"""
+    g = got.cpu().numpy()
+    d = np.abs(diff((g[0], g[1]), ref))
+    r = np.abs(ld(ref))
+    if d.ndim == 1:
+        return float(d.max() / r.max())
+    return float((d.max(axis=1) / r.max(axis=1)).max())
+
+
+@pytest.mark.parametrize("N,nc,h,rho,where,sigma,method", [(64, 4, 1.0, 0.5, 0, 0.0, "rk8"), (128, 2, float("inf"), 0.4, 1, 0.5, "rk8"),
+                                                            (64, 2, 1.0, 0.5, 1, 0.0, "sdc15")])
+def test_steps_on_refined_mesh_dd(sww, mesh_q, N, nc, h, rho, where, sigma, method):
+    """the paper's quadruple-precision configuration: a refined mesh under the double-double stepper (Table 3)"""
+    eta, phi, deta, dphi = small_case(N, nc)
+    dt = (0.02 if sigma == 0.0 else 0.4 / N * rho) * (4 if method == "sdc15" else 1)
+    st = sww.State(to_dev(eta, None, "dd"), to_dev(phi, None, "dd"), h, 1.0, prec=sww.DD, deta=to_dev(deta, None, "dd"), dphi=to_dev(dphi, None, "dd"))
+    st.set_mesh(rho, where)
+    st.set_sigma(sigma)
+    e0 = st.energy()
+    st.advance(dt, 1, method=method)
+    r = st.read()
+    mesh_q.set_mesh(rho, where)
+    o = mesh_q.rk_advance(eta, phi, h, 1.0, dt, 1, deta=deta, dphi=dphi, sigma=sigma, want_energy=True, method=method)
+    tol = 1e-25 / rho ** 2
+    for name in ("eta", "phi", "deta", "dphi"):
+        assert dd_err(r[name], o[name]) <= tol, name
+    if sigma == 0.0:
+        eh, el = o["energies"][0][0], o["energies"][1][0]      # word by word: a long double cannot hold a double-double
+        assert abs((LD(e0[0]) - LD(eh)) + (LD(e0[1]) - LD(el))) <= 1e-27 * abs(eh)
+
+
+def test_respacing_dd(sww, mesh_q):
+    N, M2, nc, h = 64, 128, 2, 1.0
+    eta, phi, deta, dphi = small_case(N, nc)
+    s1 = sww.State(to_dev(eta, None, "dd"), to_dev(phi, None, "dd"), h, 1.0, prec=sww.DD, deta=to_dev(deta, None, "dd"), dphi=to_dev(dphi, None, "dd"))
+    s1.advance(0.02, 1)
+    a = s1.read()
+    z1 = torch.zeros(2, M2, dtype=torch.float64, device="cuda")
+    zc = torch.zeros(2, nc, M2, dtype=torch.float64, device="cuda")
+    s2 = sww.State(z1, z1, h, 1.0, prec=sww.DD, deta=zc, dphi=zc)
+    s2.set_mesh(0.4, 0)
+    s2.respace_from(s1)
+    b = s2.read()
+    for name in ("eta", "phi", "deta", "dphi"):
+        src = a[name].cpu().numpy()
+        ref = mesh_q.respace((src[0], src[1]), (N, 1.0, 0), (M2, 0.4, 0))
+        assert dd_err(b[name], ref) <= 1e-28, name
+
+
+def test_shooting_map_with_segments_dd(sww, mesh_q):
+    from oracle import shooting
+    n, segs = 4, [(32, 0.5, 1.0, 0, 2), (64, 0.5, 0.5, 0, 3)]
+    c = shoot_unknowns(n)
+    S = sww.Shooter(32, n, 1.0, 1.0, prec=sww.DD)
+    S.set_segments(segs)
+    r, J = S.shoot(c, 1)
+    o = shooting.shoot_segments_quad(mesh_q, c, segs, 1.0, 1.0)
+    assert r.shape == (2, 64) and J.shape == (2, n + 1, 64)
+    assert dd_err(r, o["r"]) <= 1e-25 / 0.25
+    assert dd_err(J, (o["J"][0].T, o["J"][1].T)) <= 1e-25 / 0.25
+    S.close()
 
 
 def shoot_unknowns(n, T=7.0, amp=-0.02, seed=3):
@@ -319,7 +383,3 @@ def test_segment_errors(sww):
         with pytest.raises(sww.SwwError):
             S.set_segments(bad)
     S.close()
-    Sd = sww.Shooter(64, 4, 1.0, 1.0, prec=sww.DD)
-    with pytest.raises(sww.SwwError):
-        Sd.set_segments([(64, 0.5, 1.0, 0, 4), (128, 0.5, 0.5, 0, 4)])
-    Sd.close()

@@ -181,3 +181,17 @@ def test_shooting_with_segments_is_mesh_independent(orc):
     # one segment on the uniform mesh through shoot_segments is shoot itself
     same = shooting.shoot_segments(orc, c, [(64, 1.0, 1.0, 0, 24)], h, g, filter=False)
     assert np.abs(same["r"] - one["r"]).max() == 0 and np.abs(same["J"] - one["J"]).max() == 0
+
+
+def test_shooting_segments_quad_matches_long_double(orc, orc_q):
+    """the __float128 build of the segmented map against the long-double one (same c, same segments)"""
+    from oracle import shooting
+    c = np.array([7.0, -0.01, 0.003, 0.001])
+    segs = [(32, 0.5, 1.0, 0, 3), (64, 0.5, 0.5, 1, 3)]
+    try:
+        a = shooting.shoot_segments(orc, c, segs, 1.0, 1.0)
+        b = shooting.shoot_segments_quad(orc_q, c, segs, 1.0, 1.0)
+    finally:
+        orc_q.set_mesh()
+    assert np.abs(ld(b["r"]) - a["r"]).max() < 5e-18
+    assert np.abs(ld(b["J"]) - a["J"]).max() < 5e-17
