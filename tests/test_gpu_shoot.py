@@ -151,3 +151,47 @@ def test_levenberg_marquardt_finds_a_standing_wave(sww, orc_ld):
     assert abs(c[2]) > 1e-6 and abs(c[3]) > 1e-9     # second and third harmonics were found
     o = shooting.shoot(orc_ld, np.array(c), N, 1.0, 1.0, nsteps)
     assert float(0.5 * (o["r"] @ o["r"])) < 1e-24
+
+
+def test_period_correction_changes_sign_with_depth(sww):
+    """(4.36): the period of small standing waves first decreases with amplitude for h < 1.0581 and increases
+    from the start for h > 1.0581.  Standing waves are computed by Levenberg-Marquardt on the device shooting map at two small
+    amplitudes per depth; omega_2 = lim 2 (omega - omega_0) / eps^2 with eps = A = 2 |c_1| omega_0 ((4.35): phi(x, 0) = 2 c_1 cos x,
+    A/B = sqrt(tanh h)) is extrapolated to zero amplitude, compared with the printed formula, and its root in h with the printed 1.0581."""
+    import math
+    golden = {}
+    from pathlib import Path
+    for line in (Path(__file__).parent / "golden" / "paper_values.txt").read_text().splitlines():
+        if line.strip() and not line.startswith("#"):
+            k, v, tol = line.split()[:3]
+            golden[k] = (float(v), float(tol))
+    N, n, nsteps = 64, 8, 24
+
+    def omega2_measured(h):
+        w0 = math.sqrt(math.tanh(h))
+        S = sww.Shooter(N, n, h, 1.0)
+        vals = []
+        for c1 in (-0.004, -0.008):
+            c0 = np.zeros(n + 1)
+            c0[0], c0[1] = 2 * math.pi / w0, c1
+            fixed = [0] * (n + 1)
+            fixed[1] = 1
+            c, rep = S.solve(c0, nsteps, fixed=fixed, delta0=0.1, f_tol=1e-28, max_iter=60)
+            assert rep["f"] < 1e-24, rep
+            eps = 2 * abs(c1) * w0
+            vals.append(2 * (2 * math.pi / c[0] - w0) / eps ** 2)
+        S.close()
+        return (4 * vals[0] - vals[1]) / 3          # the O(eps^2) term of the measured ratio removed
+
+    def omega2_formula(h):
+        w = math.sqrt(math.tanh(h))
+        return (9 * w ** -7 - 12 * w ** -3 - 3 * w - 2 * w ** 5) / 32
+
+    hs = [1.0, 1.05, 1.066]
+    m = [omega2_measured(h) for h in hs]
+    for h, v in zip(hs, m):
+        assert abs(v - omega2_formula(h)) < 2e-3 * max(abs(omega2_formula(1.0)), abs(v)), (h, v, omega2_formula(h))
+    assert m[0] > 0 and m[1] > 0 and m[2] < 0         # positive below 1.0581, negative above
+    h_root = hs[1] + (hs[2] - hs[1]) * m[1] / (m[1] - m[2])      # secant between the bracketing depths (omega_2 is nearly linear in h there)
+    want, tol = golden["h_omega2_sign"]
+    assert abs(h_root - want) < 3e-4, (h_root, want)

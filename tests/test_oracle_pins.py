@@ -788,3 +788,16 @@ def test_adjoint_identity(orc_q, sigma, h):
                 gap = max(gap, float(abs(lhs - rhs)))
         gaps.append(gap)
     assert gaps[0] < 1e-4 and gaps[1] < 1e-6 * gaps[0] and gaps[2] < 1e-4 * gaps[1] and gaps[2] < 1e-18, gaps
+
+
+def test_paper_omega2_sign_change_depth():
+    """(4.36): the root in h of the printed omega_2 is the printed 1.0581 (the golden value used by the GPU test of
+    the period correction is consistent with the formula printed next to it)"""
+    w2 = lambda h: (lambda w: 9 * w ** -7 - 12 * w ** -3 - 3 * w - 2 * w ** 5)(math.sqrt(math.tanh(h)))
+    lo, hi = 1.0, 1.1
+    assert w2(lo) > 0 > w2(hi)
+    for _ in range(60):
+        mid = 0.5 * (lo + hi)
+        lo, hi = (mid, hi) if w2(mid) > 0 else (lo, mid)
+    want, tol = golden()["h_omega2_sign"]
+    assert abs(lo - want) < tol
