@@ -136,7 +136,7 @@ int sww_state_destroy(sww_state_t s);
  * the points x_j = xi(alpha_j), alpha_j = 2 pi j / N: zeta = xi + i eta o xi in (2.13), the factor 1/|xi'| in (2.8), d/dx =
  * (1/xi') d/dalpha in (2.9), (B.2).  The call invalidates the surface: follow it with sww_dtn_refactor.  Views 2, 3 of sww_dtn_get stay
  * alpha-derivatives of the stored eta; 4..7 (phi0', W0, u, v) are the physical quantities.  Either precision.
- * Not on a refined mesh: sww_dtn_adjoint_rhs and sww_dtn_linearized_host (SWW_EINVAL / uniform only).
+ * sww_dtn_adjoint_rhs follows the mesh as well ((B.6) with d/dx and the mean over x); sww_dtn_linearized_host is uniform only.
  * sww_mesh_points: x (HOST, N doubles) <- xi(alpha_j). */
 int sww_dtn_set_mesh(sww_dtn_t d, double rho, int where);
 int sww_mesh_points(int N, double rho, int where, double* x);

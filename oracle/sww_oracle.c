@@ -603,27 +603,26 @@ int NAME(rhs)(int N, double h, double g, double sigma, int filter, const double 
  * (no filter: the adjoint identity <DF(q) qdot, q~> = <qdot, DF(q)^* q~> is stated for the unfiltered operators). */
 static int adjoint_eval(int N, REAL h, REAL g, REAL sigma, const REAL *eta, const REAL *phi, int ncols,
                         const REAL *etat, const REAL *phit, REAL *eta_s, REAL *phi_s) {
-    if (mesh_on()) return ORC_EINVAL;   /* (B.6) is written out here for the uniform mesh only */
-    setup_t s; int rc = setup_make(&s, N, h, eta); if (rc) return rc;
+    setup_t s; int rc = setup_make(&s, N, h, eta); if (rc) return rc;   /* refined mesh: D = d/dx, P = mean over x (deriv_x, project_x) */
     base_t bs; base_make(&s, phi, &bs);
     REAL *du = ralloc(N);
-    multiplier(&s.t, MUL_D, bs.u, du);
+    deriv_x(&s, bs.u, du);
 #pragma omp parallel for schedule(dynamic) if (ncols > 1)
     for (int c = 0; c < ncols; c++) {
         const REAL *et = etat + (long)c * N, *pt = phit + (long)c * N;
         REAL *pp = ralloc(N), *chi = ralloc(N), *w = ralloc(N), *t1 = ralloc(N), *t2 = ralloc(N), *det = ralloc(N);
-        multiplier(&s.t, MUL_P, pt, pp);
+        project_x(&s, 0, pt, pp);
         for (int i = 0; i < N; i++) chi[i] = et[i] + bs.v[i] * pp[i];
         dtn_one(&s, chi, w, NULL);
         for (int i = 0; i < N; i++) t1[i] = bs.u[i] * pp[i];
-        multiplier(&s.t, MUL_D, t1, t2);
+        deriv_x(&s, t1, t2);
         for (int i = 0; i < N; i++) phi_s[(long)c * N + i] = w[i] + t2[i];
-        multiplier(&s.t, MUL_D, et, det);
+        deriv_x(&s, et, det);
         for (int i = 0; i < N; i++) eta_s[(long)c * N + i] = -bs.v[i] * w[i] + bs.u[i] * det[i] - bs.v[i] * du[i] * pp[i] - g * pp[i];
         if (sigma != 0) {
-            multiplier(&s.t, MUL_D, pt, t1);
-            for (int i = 0; i < N; i++) { REAL den = 1 + s.d1[i] * s.d1[i]; t1[i] = t1[i] / (den * R_SQRT(den)); }
-            multiplier(&s.t, MUL_D, t1, t2);
+            deriv_x(&s, pt, t1);
+            for (int i = 0; i < N; i++) { REAL e1 = s.E ? s.d1[i] / s.E[i] : s.d1[i], den = 1 + e1 * e1; t1[i] = t1[i] / (den * R_SQRT(den)); }
+            deriv_x(&s, t1, t2);
             for (int i = 0; i < N; i++) eta_s[(long)c * N + i] += sigma * t2[i];
         }
         free(pp); free(chi); free(w); free(t1); free(t2); free(det);

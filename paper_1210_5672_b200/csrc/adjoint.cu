@@ -5,7 +5,8 @@
 //     phi~_s,c  = G chi_c + D( u P phi~_c )                                                                        (B.6e)
 //     eta~_s,c  = -v G chi_c + u D eta~_c - v D(u) P phi~_c - g P phi~_c + sigma D( D(phi~_c) / (1 + eta'^2)^(3/2) )  (B.6f)
 // One batched DtN apply (S3-S6 of the hot path) between two small kernels, in fp64 and in double-double (planar hi / lo blocks,
-// N <= 2048 like the double-double stepper).  Product code; shares nothing with oracle/.
+// N <= 2048 like the double-double stepper).  On the refined mesh (2.10) (mesh.cu) D is d/dx = (1/xi') d/dalpha and P removes the mean
+// over x; G chi, u, v arrive in physical form.  Product code; shares nothing with oracle/.
 #include "common.cuh"
 #include "fft.cuh"
 #include "ddfft.cuh"
@@ -13,12 +14,13 @@
 namespace sww {
 
 // per column: pp = P phi~ (mean removed) -> PP ; chi = eta~ + v pp -> X.  One CTA per column.
-__global__ void __launch_bounds__(256) k_adj_prep(int N, const double* __restrict__ v, const double* __restrict__ eta_t,
+// xE (refined mesh (2.10), else nullptr): P removes the mean over x, (1/N) sum_j f_j xi'(alpha_j)
+__global__ void __launch_bounds__(256) k_adj_prep(int N, const double* __restrict__ v, const double* __restrict__ xE, const double* __restrict__ eta_t,
                                                   const double* __restrict__ phi_t, double* __restrict__ PP, double* __restrict__ X) {
     __shared__ double s[256];
     const size_t o = (size_t)blockIdx.x * N;
     double a = 0.0;
-    for (int j = threadIdx.x; j < N; j += 256) a += phi_t[o + j];
+    for (int j = threadIdx.x; j < N; j += 256) a += xE ? phi_t[o + j] * xE[j] : phi_t[o + j];
     s[threadIdx.x] = a;
     __syncthreads();
     for (int w = 128; w > 0; w >>= 1) {
@@ -36,7 +38,7 @@ __global__ void __launch_bounds__(256) k_adj_prep(int N, const double* __restric
 // one CTA per column pair; PPg (= eta_s on entry) holds P phi~, W (= phi_s on entry) holds G chi; both are overwritten by the result
 __global__ void __launch_bounds__(1024) k_adj_rhs(int N, int logN, const double2* __restrict__ tw, double g, double sigma, int ncols,
                                                   const double* __restrict__ u, const double* __restrict__ v, const double* __restrict__ du,
-                                                  const double* __restrict__ d1, const double* __restrict__ eta_t,
+                                                  const double* __restrict__ d1, const double* __restrict__ xE, const double* __restrict__ eta_t,
                                                   const double* __restrict__ phi_t, double* __restrict__ eta_s, double* __restrict__ phi_s) {
     extern __shared__ __align__(16) double2 z[];
     const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
@@ -53,6 +55,13 @@ __global__ void __launch_bounds__(1024) k_adj_rhs(int N, int logN, const double2
         }
         __syncthreads();
         ifft_dit(z, N, tw);
+        if (xE) {  // refined mesh: d/dx = (1/xi') d/dalpha
+            for (int j = threadIdx.x; j < N; j += blockDim.x) {
+                const double re = 1.0 / xE[j];
+                z[j] = make_double2(z[j].x * re, z[j].y * re);
+            }
+            __syncthreads();
+        }
     };
     double2 pp[FFT_MAX_PER_THREAD], w[FFT_MAX_PER_THREAD], es[FFT_MAX_PER_THREAD];
 #pragma unroll
@@ -89,7 +98,7 @@ __global__ void __launch_bounds__(1024) k_adj_rhs(int N, int logN, const double2
         for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(phi_t[o0 + j], has1 ? phi_t[o1 + j] : 0.0);
         deriv_inplace();  // D phi~
         for (int j = threadIdx.x; j < N; j += blockDim.x) {
-            const double e1 = d1[j], den = fma(e1, e1, 1.0), q = 1.0 / (den * sqrt(den));
+            const double e1 = xE ? d1[j] / xE[j] : d1[j], den = fma(e1, e1, 1.0), q = 1.0 / (den * sqrt(den));
             z[j] = make_double2(z[j].x * q, z[j].y * q);
         }
         deriv_inplace();
@@ -117,12 +126,13 @@ __device__ __forceinline__ void adj_st(double* p, size_t plane, size_t o, dd v) 
 }
 
 // per column (user arrays: planes of L = N nrhs): pp = P phi~ -> PP ; chi = eta~ + v pp -> X
-__global__ void __launch_bounds__(256) k_adj_prep_dd(int N, size_t L, const double* __restrict__ v, const double* __restrict__ eta_t,
-                                                     const double* __restrict__ phi_t, double* __restrict__ PP, double* __restrict__ X) {
+__global__ void __launch_bounds__(256) k_adj_prep_dd(int N, size_t L, const double* __restrict__ v, const double* __restrict__ xE,
+                                                     const double* __restrict__ eta_t, const double* __restrict__ phi_t, double* __restrict__ PP,
+                                                     double* __restrict__ X) {
     __shared__ double sh[256], sl[256];
     const size_t o = (size_t)blockIdx.x * N;
     dd a{0.0, 0.0};
-    for (int j = threadIdx.x; j < N; j += 256) a = dd_add(a, adj_ld(phi_t, L, o + j));
+    for (int j = threadIdx.x; j < N; j += 256) a = dd_add(a, xE ? dd_mul(adj_ld(phi_t, L, o + j), adj_ld(xE, N, j)) : adj_ld(phi_t, L, o + j));
     sh[threadIdx.x] = a.hi;
     sl[threadIdx.x] = a.lo;
     __syncthreads();
@@ -146,7 +156,7 @@ __global__ void __launch_bounds__(256) k_adj_prep_dd(int N, size_t L, const doub
 __global__ void __launch_bounds__(512) k_adj_rhs_dd(int N, int logN, const double* __restrict__ cs, const double* __restrict__ sn, double g,
                                                     double sigma, int ncols, size_t L, size_t Lws, const double* __restrict__ u,
                                                     const double* __restrict__ v, const double* __restrict__ du, const double* __restrict__ d1,
-                                                    const double* __restrict__ eta_t, const double* __restrict__ phi_t,
+                                                    const double* __restrict__ xE, const double* __restrict__ eta_t, const double* __restrict__ phi_t,
                                                     const double* __restrict__ PP, const double* __restrict__ W, double* __restrict__ OE,
                                                     double* __restrict__ OP) {
     extern __shared__ __align__(16) unsigned char adj_sm[];
@@ -166,6 +176,13 @@ __global__ void __launch_bounds__(512) k_adj_rhs_dd(int N, int logN, const doubl
         }
         __syncthreads();
         ifft_dit_dd(z, N, cs, sn);
+        if (xE) {
+            for (int j = threadIdx.x; j < N; j += blockDim.x) {
+                const dd e = adj_ld(xE, N, j);
+                z[j] = cdd{dd_div(z[j].re, e), dd_div(z[j].im, e)};
+            }
+            __syncthreads();
+        }
     };
     for (int j = threadIdx.x; j < N; j += blockDim.x) {
         const dd uu = adj_ld(u, N, j);
@@ -193,7 +210,7 @@ __global__ void __launch_bounds__(512) k_adj_rhs_dd(int N, int logN, const doubl
         for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = cdd{adj_ld(phi_t, L, o0 + j), has1 ? adj_ld(phi_t, L, o1 + j) : zero};
         deriv_inplace();  // D phi~
         for (int j = threadIdx.x; j < N; j += blockDim.x) {
-            const dd e1 = adj_ld(d1, N, j), den = dd_add_d(dd_sqr(e1), 1.0), q = dd_mul(den, dd_sqrt(den));
+            const dd e1 = xE ? dd_div(adj_ld(d1, N, j), adj_ld(xE, N, j)) : adj_ld(d1, N, j), den = dd_add_d(dd_sqr(e1), 1.0), q = dd_mul(den, dd_sqrt(den));
             z[j] = cdd{dd_div(z[j].re, q), dd_div(z[j].im, q)};
         }
         deriv_inplace();
@@ -220,9 +237,11 @@ static int adjoint_dd(sww_dtn_s* d, const double* eta_t, const double* phi_t, in
     cudaStream_t st = d->stream;
     const size_t L = (size_t)N * nrhs;
     double* du = d->tmp;  // 2 N of the base-state scratch
+    const double* xE = d->mesh_on ? d->mesh.xE : nullptr;
     SWW_TRY(circ_dd(d, 0, d->bu, du));
+    SWW_TRY(mesh_scale_out(d, du, 1, N));  // refined mesh: d/dx(u) = D(u) / xi'
     SWW_BEGIN(KC_OTHER, st);
-    k_adj_prep_dd<<<nrhs, 256, 0, st>>>(N, L, d->bv, eta_t, phi_t, eta_s, phi_s);
+    k_adj_prep_dd<<<nrhs, 256, 0, st>>>(N, L, d->bv, xE, eta_t, phi_t, eta_s, phi_s);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     SWW_TRY(sww_dtn_apply(d, phi_s, nrhs, phi_s));  // G chi in double-double, in place
@@ -234,7 +253,7 @@ static int adjoint_dd(sww_dtn_s* d, const double* eta_t, const double* phi_t, in
     while ((1 << lg) < N) lg++;
     const int thr = N / 2 > 512 ? 512 : (N / 2 < 32 ? 32 : N / 2);
     SWW_BEGIN(KC_FFT, st);
-    k_adj_rhs_dd<<<(nrhs + 1) / 2, thr, (size_t)N * sizeof(cdd), st>>>(N, lg, d->tab->cs, d->tab->sn, g, sigma, nrhs, L, Lws, d->bu, d->bv, du, d->d1, eta_t,
+    k_adj_rhs_dd<<<(nrhs + 1) / 2, thr, (size_t)N * sizeof(cdd), st>>>(N, lg, d->tab->cs, d->tab->sn, g, sigma, nrhs, L, Lws, d->bu, d->bv, du, d->d1, xE, eta_t,
                                                                       phi_t, eta_s, phi_s, w.T, w.Gam);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
@@ -255,7 +274,6 @@ using namespace sww;
 
 extern "C" int sww_dtn_adjoint_rhs(sww_dtn_t d, const void* eta_t, const void* phi_t, int nrhs, double g, double sigma, void* eta_s, void* phi_s) {
     if (!d || nrhs < 0 || !(sigma >= 0.0)) return SWW_EINVAL;
-    if (d->mesh_on) return SWW_EINVAL;  // (B.6) is implemented for the uniform mesh
     if (!d->has_base) return SWW_ENOBASE;
     if (nrhs == 0) return SWW_OK;
     if (!eta_t || !phi_t || !eta_s || !phi_s || eta_s == phi_s || eta_s == eta_t || eta_s == phi_t || phi_s == eta_t || phi_s == phi_t)
@@ -265,16 +283,18 @@ extern "C" int sww_dtn_adjoint_rhs(sww_dtn_t d, const void* eta_t, const void* p
     const int N = d->N;
     cudaStream_t st = d->stream;
     double* du = d->tmp;  // scratch of the base-state flow (14 N doubles), idle once the base state is set
+    const double* xE = d->mesh_on ? d->mesh.xE : nullptr;
     SWW_TRY(spectral_deriv(d, d->bu, du, 1));  // D(u) = "phi_x'" of (B.6f)
+    SWW_TRY(mesh_scale_out(d, du, 1, 0));      // refined mesh: d/dx(u) = D(u) / xi'
     SWW_BEGIN(KC_OTHER, st);
-    k_adj_prep<<<nrhs, 256, 0, st>>>(N, d->bv, (const double*)eta_t, (const double*)phi_t, (double*)eta_s, (double*)phi_s);
+    k_adj_prep<<<nrhs, 256, 0, st>>>(N, d->bv, xE, (const double*)eta_t, (const double*)phi_t, (double*)eta_s, (double*)phi_s);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     SWW_TRY(sww_dtn_apply(d, phi_s, nrhs, phi_s));  // G chi, in place (S3-S6)
     static DeviceOnce attr_once;
     if (attr_once.first()) SWW_CUDA(cudaFuncSetAttribute(k_adj_rhs, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
     SWW_BEGIN(KC_FFT, st);
-    k_adj_rhs<<<(nrhs + 1) / 2, fft_threads(N), sizeof(double2) * (size_t)N, st>>>(N, fft_ilog2(N), d->tab->tw, g, sigma, nrhs, d->bu, d->bv, du, d->d1,
+    k_adj_rhs<<<(nrhs + 1) / 2, fft_threads(N), sizeof(double2) * (size_t)N, st>>>(N, fft_ilog2(N), d->tab->tw, g, sigma, nrhs, d->bu, d->bv, du, d->d1, xE,
                                                                                   (const double*)eta_t, (const double*)phi_t, (double*)eta_s,
                                                                                   (double*)phi_s);
     SWW_LAUNCHED();

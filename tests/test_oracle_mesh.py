@@ -195,3 +195,39 @@ def test_shooting_segments_quad_matches_long_double(orc, orc_q):
         orc_q.set_mesh()
     assert np.abs(ld(b["r"]) - a["r"]).max() < 5e-18
     assert np.abs(ld(b["J"]) - a["J"]).max() < 5e-17
+
+
+@pytest.mark.parametrize("rho,where,sigma", [(0.5, 0, 0.0), (0.4, 1, 0.5)])
+def test_adjoint_identity_on_refined_mesh(orc_q, rho, where, sigma):
+    """(B.4)-(B.6), PAPER.md:716-747 on the mesh (2.10): <DF(q) qdot, q~> = <qdot, DF(q)^* q~> with the inner product
+    (1/2pi) int (.) dx = (1/M) sum_j (.)_j E_j.  The stored samples are smooth functions of alpha (hence of x); the gap between the
+    two sides closes spectrally with M, as on the uniform mesh."""
+    import sww_inputs as si
+    h, gaps = 1.0, []
+    try:
+        for N in (32, 64, 128):
+            rng = np.random.default_rng(11)
+            def smooth(amp):
+                c, s_ = np.zeros(7), np.zeros(7)
+                c[1:] = amp * rng.standard_normal(6) * np.exp(-0.6 * np.arange(1, 7))
+                s_[1:] = amp * rng.standard_normal(6) * np.exp(-0.6 * np.arange(1, 7))
+                return si.synth(N, c, s_)[0].astype(LD)
+            eta, phi = smooth(0.05), smooth(0.1)
+            qd = (np.stack([smooth(1.0), smooth(1.0)]), np.stack([smooth(1.0), smooth(1.0)]))
+            qt = (np.stack([smooth(1.0), smooth(1.0)]), np.stack([smooth(1.0), smooth(1.0)]))
+            sp = lambda a: split_ld(a) if a.ndim == 1 else tuple(np.stack(t) for t in zip(*[split_ld(r) for r in a]))
+            orc_q.set_mesh(rho, where)
+            E = ld(orc_q.mesh_tables(N)[1])
+            lin = orc_q.rhs(sp(eta), sp(phi), h, 1.0, sp(qd[0]), sp(qd[1]), filter=False, sigma=sigma)
+            adj = orc_q.adjoint_rhs(sp(eta), sp(phi), h, 1.0, sp(qt[0]), sp(qt[1]), sigma=sigma)
+            gap = 0.0
+            for a in range(2):
+                for b in range(2):
+                    lhs = ((ld(lin["deta_t"])[a] * qt[0][b] + ld(lin["dphi_t"])[a] * qt[1][b]) * E).mean()
+                    rhs = ((qd[0][a] * ld(adj["eta_s"])[b] + qd[1][a] * ld(adj["phi_s"])[b]) * E).mean()
+                    assert abs(lhs) > 1e-3
+                    gap = max(gap, float(abs(lhs - rhs)))
+            gaps.append(gap)
+    finally:
+        orc_q.set_mesh()
+    assert gaps[0] < 1e-3 and gaps[1] < 1e-4 * gaps[0] and gaps[2] < 1e-15, gaps
