@@ -84,3 +84,31 @@ def test_product_never_imports_the_oracle():
     for p in (ROOT / "oracle").rglob("*"):
         if p.suffix in (".py", ".c", ".h"):
             assert "paper_1210_5672_b200" not in re.sub(r"(#|//|\*).*", "", p.read_text()), p
+
+
+def test_mesh_points_host_function(sww):
+    """sww_mesh_points is host code: xi(alpha_j) of (2.10) against the oracle's tables, the printed end-point spacings (2.11) by
+    differences, monotonicity; argument checks of the mesh entry points that return before any CUDA call"""
+    import oracle
+    o = oracle.Oracle("ld")
+    N = 96   # the host function takes any N
+    for rho, where in ((1.0, 0), (0.6, 0), (0.25, 1), (0.05, 0)):
+        x = sww.mesh_points(N, rho, where)
+        try:
+            o.set_mesh(rho, where)
+            xp, E, _ = o.mesh_tables(N)
+        finally:
+            o.set_mesh()
+        assert np.abs(x - (2 * np.pi * np.arange(N) / N + xp[0])).max() < 2e-15
+        assert np.all(np.diff(x) > 0) and x[0] == 0.0
+        ratio = (x[1] - x[0]) / (x[N // 2 + 1] - x[N // 2])          # spacing at x = 0 over spacing at x = pi
+        want = (1 / rho) if where == 0 else rho
+        assert abs(ratio / want - 1) < 0.02 / rho
+    L = sww.lib()
+    buf = np.zeros(8)
+    px = buf.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+    assert L.sww_mesh_points(8, 0.0, 0, px) == -1 and L.sww_mesh_points(8, 1.5, 0, px) == -1 and L.sww_mesh_points(8, 0.5, 2, px) == -1
+    assert L.sww_mesh_points(8, 0.5, 0, None) == -1
+    assert L.sww_dtn_set_mesh(None, 0.5, 0) == -1 and L.sww_state_set_mesh(None, 0.5, 0) == -1
+    assert L.sww_state_respace(None, None) == -1
+    assert L.sww_shooter_set_segments(None, 1, None, None, None, None, None) == -1

@@ -414,3 +414,31 @@ def test_adjoint_rhs_on_refined_mesh_dd(sww, mesh_q):
     o = mesh_q.adjoint_rhs(eta, phi, h, 1.0, et, pt, sigma=sigma)
     assert dd_err(es, o["eta_s"]) <= 1e-25 / rho ** 2
     assert dd_err(ps, o["phi_s"]) <= 1e-25 / rho ** 2
+
+
+def test_maximum_and_minimum_size_on_refined_mesh(sww, mesh_ld):
+    """N = 8192 (the largest DtN): flat surface, phi = cos(k x) sampled at the refined points, G phi = k tanh(kh) cos(k x) in closed
+    form; N = 16 (the smallest) against the oracle"""
+    N, h, rho = 8192, 1.0, 0.3
+    x = sww.mesh_points(N, rho, 0)
+    ks = [1, 5, 40]
+    phi = np.stack([np.cos(k * x) for k in ks])
+    d = sww.DtN(torch.zeros(N, dtype=torch.float64, device="cuda"), h)
+    d.set_mesh(rho, 0)
+    d.refactor(torch.zeros(N, dtype=torch.float64, device="cuda"))
+    w = d.apply(dev(phi)).cpu().numpy()
+    d.check()
+    d.close()
+    for i, k in enumerate(ks):
+        want = k * np.tanh(k * h) * phi[i]
+        # rounded samples under a first-order operator: ~ N eps / rho relative to the largest mode resolved, plus the parity bar
+        assert float(np.abs(w[i] - want).max()) <= (1e-11 / rho ** 2) * k * np.tanh(k * h), k
+    N = 16
+    eta, phi1 = 0.05 * np.cos(2 * np.pi * np.arange(N) / N), np.sin(2 * np.pi * np.arange(N) / N)
+    d = sww.DtN(dev(eta), h)
+    d.set_mesh(0.5, 1)
+    d.refactor(dev(eta))
+    got = d.apply(dev(phi1[None, :])).cpu().numpy()[0]
+    mesh_ld.set_mesh(0.5, 1)
+    ref = ld(mesh_ld.dtn_apply(eta, h, phi1[None, :]))[0]
+    assert float(np.abs(got - ref).max()) <= 1e-13
