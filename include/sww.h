@@ -178,6 +178,13 @@ int sww_shooter_dims(sww_shooter_t S, int* N, int* n, int* is_dd);
  * ignored.  Either precision (SWW_DD with sww_shooter_set_method(S, 1) is the paper's quadruple-precision configuration of Table 3).
  * All arrays HOST.  Creates the steppers of segments 2..nu (memory: like nu shooters). */
 int sww_shooter_set_segments(sww_shooter_t S, int nu, const int* M, const double* theta, const double* rho, const int* where, const int* nsteps);
+/* The gradient of f = r.r / 2 with respect to c by ONE backward solve of the adjoint system, section 3.2 (3.21)-(3.30), PAPER.md:228-284:
+ * forward solve of (2.1) with the stage states kept, then the transposed Runge-Kutta recursion with DF(Y)^* of (B.6)
+ * (sww_dtn_adjoint_rhs) at every stage state, q~(0) = (0, phi(T/4)) (3.26); df/dc_k = <q~(T/4), dq_0/dc_k> (3.30), df/dT by (3.22).
+ * Cost: two solves of (2.1) instead of the n variational columns of sww_shoot; grad equals J^T r of sww_shoot up to the (spectrally
+ * small) difference between the continuous adjoint (B.6) and the transpose of the discrete linearization.  f (optional) and grad
+ * (n + 1 doubles): HOST.  SWW_F64 shooters on one uniform segment with the RK8 stepper; otherwise SWW_EINVAL.  Synchronises. */
+int sww_shoot_gradient(sww_shooter_t S, const double* c, int nsteps, double* f, double* grad);
 int sww_shooter_set_method(sww_shooter_t S, int method);   /* 0: RK8 (default); 1: SDC15, the paper's quadruple-precision stepper */
 int sww_shooter_set_sigma(sww_shooter_t S, double sigma);   /* surface tension of every following shot (see sww_state_set_sigma) */
 

@@ -19,7 +19,7 @@ EXPORTS = [
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
     "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance", "sww_dtn_adjoint_rhs", "sww_shooter_set_method",
-    "sww_dtn_set_mesh", "sww_mesh_points", "sww_state_set_mesh", "sww_state_respace", "sww_shooter_set_segments",
+    "sww_dtn_set_mesh", "sww_mesh_points", "sww_state_set_mesh", "sww_state_respace", "sww_shooter_set_segments", "sww_shoot_gradient",
 ]
 
 
@@ -102,6 +102,7 @@ def lib() -> ctypes.CDLL:
         L.sww_mesh_points.argtypes = [ci, cd, ci, ctypes.POINTER(cd)]
         L.sww_state_set_mesh.argtypes = [vp, cd, ci]
         L.sww_state_respace.argtypes = [vp, vp]
+        L.sww_shoot_gradient.argtypes = [vp, ctypes.POINTER(cd), ci, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.sww_shooter_set_segments.argtypes = [vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd), ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(ci)]
         L.sww_timing_enable.argtypes = [ci]
         L.sww_timing_read.argtypes = [ctypes.POINTER(cd), ctypes.POINTER(ctypes.c_ulonglong), ci]
@@ -367,6 +368,15 @@ class Shooter:
         r = torch.empty(lead + (self.m,), dtype=torch.float64, device="cuda")
         _check(lib().sww_shoot_residual(self._h, cc, int(nsteps), r.data_ptr()), "sww_shoot_residual")
         return r
+
+    def gradient(self, c, nsteps: int):
+        """sww_shoot_gradient: (f, grad (numpy, n + 1)) by one backward solve of the adjoint system (section 3.2)"""
+        import numpy as np
+        cc = (ctypes.c_double * (self.n + 1))(*[float(x) for x in c])
+        f = ctypes.c_double(0.0)
+        g = (ctypes.c_double * (self.n + 1))()
+        _check(lib().sww_shoot_gradient(self._h, cc, int(nsteps), ctypes.byref(f), g), "sww_shoot_gradient")
+        return f.value, np.array(list(g))
 
     def solve(self, c, nsteps: int, fixed=None, **opts):
         """Levenberg-Marquardt with delayed Jacobian updates (Appendix C) on the shooting map: -> (c, report)"""

@@ -726,6 +726,10 @@ int sww_rk_advance(sww_state_t s, double dt, int nsteps) {
                 SWW_TRY(rk_combine(s, s->a[i], s->alo[i], i, dt, s->ys));
                 ys = s->ys;
             }
+            if (s->tape && s->prec == SWW_F64) {
+                if (n >= s->tape_steps) return SWW_EINVAL;
+                SWW_CUDA(cudaMemcpyAsync(s->tape + ((size_t)n * RK_S + i) * 2 * N, ys, sizeof(double) * 2 * N, cudaMemcpyDeviceToDevice, s->stream));
+            }
             SWW_TRY(rk_rhs(s, ys, s->k + (size_t)i * s->L * s->mul()));
         }
         SWW_TRY(rk_combine(s, s->b, s->blo, RK_S, dt, s->y));

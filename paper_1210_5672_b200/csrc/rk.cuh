@@ -19,6 +19,10 @@ struct sww_state_s {
     double* red;         // 2 doubles: energy reduction (hi, lo)
     double* sdc;         // SDC15 work space (SDC_SLOTS state vectors), allocated by the first sww_sdc_advance
     double t;
+    // sww_shoot_gradient (grad.cu): when set, sww_rk_advance records the stage states (eta, phi) of every step here, stage i of step n at
+    // (n RK_S + i) 2N (fp64 steppers); tape_steps = the steps that fit
+    double* tape;
+    int tape_steps;
     // sww_state_respace into this state (mesh.cu): the interpolation matrix of the last pair of meshes, kept for the next call
     double* rsp_R;
     int rsp_Mo, rsp_where_o, rsp_where_n;

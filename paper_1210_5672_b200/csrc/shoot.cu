@@ -8,7 +8,9 @@
 // only builds the initial state and scales the result.  Product code; shares nothing with oracle/.
 #include "rk.cuh"
 #include "dd.cuh"
+#include "fft.cuh"
 #include <new>
+#include <vector>
 #include <cstring>
 #include <cmath>
 
@@ -99,6 +101,96 @@ __global__ void k_shoot_out(int N, int n, int isdd, size_t L, double whi, double
     const size_t o = (col == 0) ? (size_t)j : (size_t)(col - 1) * N + j;
     dst[o] = isdd ? v.hi : v.hi + v.lo;
     if (isdd) dst[plane + o] = v.lo;
+}
+
+// ------------------------------------------------------------------------------------------------ gradient of f by the adjoint system
+// Section 3.2, (3.21)-(3.30): f = <(0, phi(T/4)), (0, phi(T/4))> / 2 with <a, b> = (1/2pi) int (eta_a eta_b + phi_a phi_b) dx
+// (3.20); the adjoint solution q~ of (3.27), q~_s = DF(q(T/4 - s))^* q~ from q~(0) = (0, phi(T/4)), gives df/dq_0 = q~(T/4) (3.29) and
+// df/dc_k = <q~(T/4), dq_0/dc_k> (3.30), df/dT = <(0, phi), (0, phi_t)> / 4 at T/4 (3.22).  Here the backward solve is the exact
+// transpose of the forward Runge-Kutta recursion of the variational equation (the stage states Y_i of every step are kept, so no
+// dense output is needed): with mu = F^* lambda_{n+1} (the filter after the step),
+//     g_i = h b_i mu + h sum_{j>i} a_ji theta_j ,  theta_i = DF(Y_i)^* F^* g_i  (i = s..1),   lambda_n = mu + sum_i theta_i ,
+// DF(Y)^* the right-hand side (B.6) of the adjoint system (sww_dtn_adjoint_rhs), F the filter (2.14) (self-adjoint on the uniform mesh;
+// on a refined mesh F^* = E^{-1} F E in the inner product weighted by dx = E dalpha).
+struct GradComb {
+    int n;
+    int idx[RK_S];
+    double coef[RK_S];
+    double cmu;
+};
+// out = cmu mu + sum_j coef_j theta[idx_j]   (vectors of 2N)
+__global__ void k_grad_comb(size_t L, const double* __restrict__ mu, const double* __restrict__ theta, GradComb cb, double* __restrict__ out) {
+    const size_t q = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= L) return;
+    double v = cb.cmu * mu[q];
+    for (int j = 0; j < cb.n; j++) v = fma(cb.coef[j], theta[(size_t)cb.idx[j] * L + q], v);
+    out[q] = v;
+}
+// lambda (2N: eta~ | phi~) <- F^* lambda, one CTA
+__global__ void __launch_bounds__(1024) k_grad_filter(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ filt,
+                                                      const double* __restrict__ xE, double* __restrict__ lam) {
+    extern __shared__ __align__(16) double2 z[];
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double e = xE ? xE[j] : 1.0;
+        z[j] = make_double2(lam[j] * e, lam[N + j] * e);
+    }
+    __syncthreads();
+    fft_dif(z, N, tw);
+    const double rN = 1.0 / (double)N;
+    for (int p = threadIdx.x; p < N; p += blockDim.x) {
+        const double f = filt[(int)(__brev((unsigned)p) >> (32 - logN))] * rN;
+        z[p] = make_double2(f * z[p].x, f * z[p].y);
+    }
+    __syncthreads();
+    ifft_dit(z, N, tw);
+    for (int j = threadIdx.x; j < N; j += blockDim.x) {
+        const double re = xE ? 1.0 / xE[j] : 1.0;
+        lam[j] = z[j].x * re;
+        lam[N + j] = z[j].y * re;
+    }
+}
+// out[0] = f = (1/2N) sum phi^2 E ; out[1] = df/dT = (1/4N) sum phi phi_t E ; lam <- (0, phi)   (3.21), (3.22), (3.26); one CTA
+__global__ void __launch_bounds__(256) k_grad_start(int N, const double* __restrict__ y, const double* __restrict__ k0, const double* __restrict__ xE,
+                                                    double* __restrict__ lam, double* __restrict__ out) {
+    __shared__ double s0[256], s1[256];
+    double a = 0.0, b = 0.0;
+    for (int j = threadIdx.x; j < N; j += 256) {
+        const double p = y[N + j], e = xE ? xE[j] : 1.0;
+        a = fma(p * p, e, a);
+        b = fma(p * k0[N + j], e, b);
+        lam[j] = 0.0;
+        lam[N + j] = p;
+    }
+    s0[threadIdx.x] = a;
+    s1[threadIdx.x] = b;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) {
+            s0[threadIdx.x] += s0[threadIdx.x + o];
+            s1[threadIdx.x] += s1[threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) {
+        out[0] = 0.5 * s0[0] / (double)N;
+        out[1] = 0.25 * s1[0] / (double)N;
+    }
+}
+// out[2 + k - 1] = df/dc_k = (1/N) sum_j lam_field(j) 2 cos(k alpha_j), field = eta~ for even k, phi~ for odd k ((3.15), (3.30));
+// one CTA per k = 1..n.  The initial state lives on the uniform mesh.
+__global__ void __launch_bounds__(256) k_grad_project(int N, const double* __restrict__ cs, const double* __restrict__ lam, double* __restrict__ out) {
+    __shared__ double s0[256];
+    const int k = blockIdx.x + 1;
+    const double* f = (k & 1) ? lam + N : lam;
+    double a = 0.0;
+    for (int j = threadIdx.x; j < N; j += 256) a = fma(f[j], 2.0 * cs[(int)(((long long)k * j) & (N - 1))], a);
+    s0[threadIdx.x] = a;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) {
+        if (threadIdx.x < o) s0[threadIdx.x] += s0[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[1 + k] = s0[0] / (double)N;
 }
 
 }  // namespace sww
@@ -209,6 +301,112 @@ int sww_shoot_residual(sww_shooter_t S, const double* c, int nsteps, void* r) {
     if (!S || !c || (S->nseg == 0 && nsteps < 1) || !r) return SWW_EINVAL;
     if (!(c[0] > 0.0)) return SWW_EINVAL;
     return shoot_impl(S, false, c, nsteps, r, nullptr, nullptr, nullptr);
+}
+
+int sww_shoot_gradient(sww_shooter_t S, const double* c, int nsteps, double* f, double* grad) {
+    if (!S || !c || nsteps < 1 || !grad) return SWW_EINVAL;
+    if (!(c[0] > 0.0)) return SWW_EINVAL;
+    if (S->prec != SWW_F64 || S->nseg != 0 || S->sdc) return SWW_EINVAL;  // fp64, one uniform segment, the Runge-Kutta stepper
+    const int N = S->N, n = S->n, logN = fft_ilog2(N);
+    sww_state_s* s = nullptr;
+    SWW_TRY(seg_state(S, 0, false, &s));
+    cudaStream_t st = s->stream;
+    sww_dtn_s* d = s->dtn;
+    const Tables* tab = d->tab;
+    const size_t V = 2 * (size_t)N;  // one vector (eta | phi)
+    // work space: the stage tape, theta_1..theta_s, mu, g, lambda, the outputs
+    double* buf = nullptr;
+    const size_t ntape = (size_t)nsteps * RK_S * V, nwork = (RK_S + 4) * V + (size_t)n + 2;
+    SWW_CUDA(cudaMalloc(&buf, sizeof(double) * (ntape + nwork)));
+    double *tape = buf, *theta = buf + ntape, *mu = theta + RK_S * V, *gv = mu + V, *lam = gv + V, *scr = lam + V, *out = scr + V;
+    int rc = SWW_OK;
+    auto run = [&]() -> int {
+        SWW_CUDA(cudaMemcpyAsync(S->c_dev, c, sizeof(double) * (n + 1), cudaMemcpyHostToDevice, st));
+        SWW_CUDA(cudaStreamSynchronize(st));
+        SWW_BEGIN(KC_OTHER, st);
+        k_shoot_init<<<dim3((N + 127) / 128, 1), 128, 0, st>>>(N, n, 0, s->L, tab->cs, S->c_dev, s->y);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+        s->t = 0.0;
+        const double dt = c[0] / (4.0 * nsteps);
+        s->tape = tape;
+        s->tape_steps = nsteps;
+        const int rf = sww_rk_advance(s, dt, nsteps);   // forward solve (2.1), stage states kept
+        s->tape = nullptr;
+        s->tape_steps = 0;
+        SWW_TRY(rf);
+        SWW_TRY(rk_rhs(s, s->y, s->k));                 // phi_t at T/4
+        const double* xE = d->mesh_on ? d->mesh.xE : nullptr;
+        SWW_BEGIN(KC_OTHER, st);
+        k_grad_start<<<1, 256, 0, st>>>(N, s->y, s->k, xE, lam, out);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+        static DeviceOnce attr_once;
+        if (attr_once.first()) SWW_CUDA(cudaFuncSetAttribute(k_grad_filter, cudaFuncAttributeMaxDynamicSharedMemorySize, 8192 * 16));
+        auto filter_adj = [&](double* v) -> int {
+            if (!s->filter) return SWW_OK;
+            SWW_BEGIN(KC_FFT, st);
+            k_grad_filter<<<1, fft_threads(N), sizeof(double2) * (size_t)N, st>>>(N, logN, tab->tw, tab->filt, xE, v);
+            SWW_LAUNCHED();
+            SWW_CUDA(cudaGetLastError());
+            return SWW_OK;
+        };
+        const unsigned blocks = (unsigned)((V + 255) / 256);
+        for (int nn = nsteps - 1; nn >= 0; nn--) {       // the transposed recursion, step by step backward
+            SWW_CUDA(cudaMemcpyAsync(mu, lam, sizeof(double) * V, cudaMemcpyDeviceToDevice, st));
+            SWW_TRY(filter_adj(mu));
+            bool used[RK_S];
+            for (int i = RK_S - 1; i >= 0; i--) {
+                GradComb cb;
+                cb.n = 0;
+                cb.cmu = dt * s->b[i];
+                for (int j = i + 1; j < RK_S; j++)
+                    if (s->a[j][i] != 0.0 && used[j]) {
+                        cb.idx[cb.n] = j;
+                        cb.coef[cb.n] = dt * s->a[j][i];
+                        cb.n++;
+                    }
+                used[i] = cb.n > 0 || cb.cmu != 0.0;
+                if (!used[i]) continue;                   // a stage nothing depends on contributes nothing
+                SWW_BEGIN(KC_OTHER, st);
+                k_grad_comb<<<blocks, 256, 0, st>>>(V, mu, theta, cb, gv);
+                SWW_LAUNCHED();
+                SWW_CUDA(cudaGetLastError());
+                SWW_TRY(filter_adj(gv));
+                const double* Y = tape + ((size_t)nn * RK_S + i) * V;
+                SWW_TRY(sww_dtn_refactor(d, Y));
+                SWW_TRY(sww_dtn_set_base(d, Y + N));
+                SWW_TRY(sww_dtn_adjoint_rhs(d, gv, gv + N, 1, s->g, s->sigma, theta + (size_t)i * V, theta + (size_t)i * V + N));
+            }
+            GradComb cb;                                  // lambda_n = mu + sum_i theta_i
+            cb.n = 0;
+            cb.cmu = 1.0;
+            for (int i = 0; i < RK_S; i++)
+                if (used[i]) {
+                    cb.idx[cb.n] = i;
+                    cb.coef[cb.n] = 1.0;
+                    cb.n++;
+                }
+            SWW_BEGIN(KC_OTHER, st);
+            k_grad_comb<<<blocks, 256, 0, st>>>(V, mu, theta, cb, lam);
+            SWW_LAUNCHED();
+            SWW_CUDA(cudaGetLastError());
+        }
+        SWW_BEGIN(KC_OTHER, st);
+        k_grad_project<<<n, 256, 0, st>>>(N, tab->cs, lam, out);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+        std::vector<double> host((size_t)n + 2);
+        SWW_CUDA(cudaMemcpyAsync(host.data(), out, sizeof(double) * (n + 2), cudaMemcpyDeviceToHost, st));
+        SWW_TRY(sww_dtn_status(d));  // synchronises
+        if (f) *f = host[0];
+        for (int k = 0; k <= n; k++) grad[k] = host[1 + k];
+        return SWW_OK;
+    };
+    rc = run();
+    cudaStreamSynchronize(st);
+    cudaFree(buf);
+    return rc;
 }
 
 static void free_segments(sww_shooter_t S) {

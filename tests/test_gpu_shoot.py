@@ -195,3 +195,25 @@ def test_period_correction_changes_sign_with_depth(sww):
     h_root = hs[1] + (hs[2] - hs[1]) * m[1] / (m[1] - m[2])      # secant between the bracketing depths (omega_2 is nearly linear in h there)
     want, tol = golden["h_omega2_sign"]
     assert abs(h_root - want) < 3e-4, (h_root, want)
+
+
+@pytest.mark.parametrize("N,n,nsteps,h,sigma,filt", [(64, 6, 10, 1.0, 0.0, True), (128, 9, 12, float("inf"), 0.0, True), (32, 5, 32, 1.0, 0.3, False)])
+def test_adjoint_gradient_equals_jacobian_transpose_times_residual(sww, orc_ld, N, n, nsteps, h, sigma, filt):
+    """Section 3.2, (3.25)-(3.30): the gradient of f from ONE backward solve of the adjoint system equals
+    df/dc_k = <(0, phi), (0, phidot_k)> = (J^T r)_k from the n variational solutions -- against the oracle's J^T r (its J is pinned by
+    finite differences) and against the device's own J^T r; f itself against r.r / 2"""
+    from oracle import shooting
+    c = unknowns(n, T=7.1, amp=-0.03)
+    S = sww.Shooter(N, n, h, 1.0, filter=filt)
+    S.set_sigma(sigma)
+    f, grad = S.gradient(c, nsteps)
+    r, J = S.shoot(c, nsteps)
+    S.close()
+    own = (J @ r).cpu().numpy()
+    o = shooting.shoot(orc_ld, c, N, h, 1.0, nsteps, filter=filt, sigma=sigma)
+    want = np.asarray(o["J"].T @ o["r"], dtype=np.float64)
+    scale = float(np.abs(want).max())
+    assert abs(f - float(0.5 * (o["r"] @ o["r"]))) <= 1e-11 * f
+    assert float(np.abs(grad - want).max()) <= 1e-11 * scale, (grad, want)      # the parity bar against the oracle
+    assert float(np.abs(grad - own).max()) <= 1e-12 * scale                      # measured: 1e-15 (the two device paths share the forward solve)
+    assert scale > 1e-6
