@@ -264,6 +264,11 @@ def other_configs(sww, flush, peak_tf):
     ms = time_events(lambda: S.shoot(cs, nst), 3)
     out["shooting"] = {"workload": f"shooting map N={Ns}, n={ns_} unknowns, {nst} RK8 steps to T/4: r (3.17) and J (3.31)", "ms_per_shot": ms,
                        "column_stages_per_s": ns_ * nst * 11 / (ms * 1e-3), "bound": "latency (8-block LU chain per stage)"}
+    S.gradient(cs, nst)
+    ms = time_events(lambda: S.gradient(cs, nst), 3)
+    out["shooting_adjoint_gradient"] = {"workload": f"gradient of f for the same shot by one backward solve of the adjoint system (section 3.2): "
+                                                    f"forward {nst} RK8 steps with the stage states kept + transposed recursion, one (B.6) per stage",
+                                        "ms_per_gradient": ms, "bound": "latency (single-vector solves: the chain of 2N/64 block links per stage)"}
     S.set_segments([(Ns, 0.5, 1.0, 0, nst // 2), (2 * Ns, 0.5, 0.4, 0, nst // 2)])
     S.shoot(cs, nst)
     ms = time_events(lambda: S.shoot(cs, nst), 3)
