@@ -95,23 +95,27 @@ def test_residual_and_jacobian_dd_with_sdc15(sww, orc_q):
     S.close()
 
 
-def test_gauss_newton_on_the_period_finds_the_linear_period(sww):
-    """the small-amplitude branch: Gauss-Newton on c_0 = T alone with the device residual and Jacobian column 0 converges to
-    T = 2 pi / sqrt(tanh 1) = 7.19976; f = r.r / 2 falls to roundoff"""
+@pytest.mark.parametrize("h,key,T0,nsteps", [(1.0, "T_linear_h1", 7.0, 16), (0.05, "T_linear_h0.05", 27.0, 64), (float("inf"), "T_linear_hinf", 6.0, 16)])
+def test_gauss_newton_on_the_period_finds_the_linear_period(sww, h, key, T0, nsteps):
+    """the small-amplitude branch: Gauss-Newton on c_0 = T alone with the device residual and Jacobian column 0 converges to the
+    printed linear periods: T = 2 pi / sqrt(tanh 1) = 7.19976 (PAPER.md:332), 28.1110 at h = 0.05 (PAPER.md:521), 2 pi in deep water;
+    f = r.r / 2 falls to roundoff"""
     golden = {}
     from pathlib import Path
     for line in (Path(__file__).parent / "golden" / "paper_values.txt").read_text().splitlines():
         if line.strip() and not line.startswith("#"):
             k, v, tol = line.split()[:3]
             golden[k] = (float(v), float(tol))
-    N, n, nsteps, eps = 64, 1, 16, 1e-6
-    S = sww.Shooter(N, n, 1.0, 1.0)
-    T = 7.0
+    n = 1
+    N = 64 if h > 0.5 else 512           # shallow water: the image surface is 2h = 0.1 away, the mesh must resolve that distance
+    eps = 1e-6 if h > 0.5 else 1e-9      # and the Ursell number A lambda^2 / h^3 must be small too
+    S = sww.Shooter(N, n, h, 1.0)
+    T = T0
     for _ in range(6):
         r, J = S.shoot([T, eps], nsteps)
         J0 = J[0]
         T -= float((J0 @ r) / (J0 @ J0))
-    want, tol = golden["T_linear_h1"]
+    want, tol = golden[key]
     assert abs(T - want) < tol
     assert float(0.5 * (r @ r)) < 1e-22
     S.close()
