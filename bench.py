@@ -228,7 +228,7 @@ def other_configs(sww, flush, peak_tf):
     for _ in range(3):
         step1()
     ms = time_events(step1, 50)
-    out["config1"] = {"workload": "N=64, 1 right-hand side: setup + apply", "ms_per_step": ms, "bound": "latency (12 launches)"}
+    out["config1"] = {"workload": "N=64, 1 right-hand side: setup + apply", "ms_per_step": ms, "bound": "latency (10 launches)"}
     d1.close()
 
     c2 = si.config2()

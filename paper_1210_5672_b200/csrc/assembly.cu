@@ -10,57 +10,7 @@
 
 namespace sww {
 
-// ------------------------------------------------------------------------------------------------ S0: D in double-double
-// out_i = sum_{m=1}^{N/2-1} dc[m] (f_{i-m} - f_{i+m}),  dc[m] = (1/2)(-1)^m cot(pi m/N)  (dc[N-m] = -dc[m]; Nyquist symbol 0).
-// Four warps per output node (a CTA of 8 warps serves two nodes): N dd multiply-adds per node, a quarter of them per warp -- the
-// kernel is a chain of dependent dd operations behind scattered loads, so its time is the length of the per-lane chain.
-// in/out: dd planar 2N.
-__global__ void __launch_bounds__(256) k_deriv_dd(int N, const double* __restrict__ dc, const double* __restrict__ f, double* __restrict__ out) {
-    __shared__ double part[2][4][2];
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, node = warp >> 2, q = warp & 3;
-    const int i = blockIdx.x * 2 + node, mask = N - 1;
-    const int l128 = q * 32 + lane;  // position among the 128 lanes that share the node
-    dd acc4[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};  // independent chains: a dd multiply-add is ~30 dependent instructions
-    if (i < N) {
-        const bool full = ((N / 2) % 512) == 0;  // dc[N/2] = 0: the last group may run over it unguarded, loads issued together
-        for (int m0 = 1 + l128; m0 < N / 2; m0 += 512) {
-            if (full) {
-                dd c[4], a[4], b[4];
-#pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    const int m = m0 + 128 * u;
-                    c[u] = dd_load(dc, N, m);
-                    a[u] = dd_load(f, N, (i - m) & mask);
-                    b[u] = dd_load(f, N, (i + m) & mask);
-                }
-#pragma unroll
-                for (int u = 0; u < 4; u++) acc4[u] = dd_fma(c[u], dd_sub(a[u], b[u]), acc4[u]);
-            } else {
-#pragma unroll
-                for (int u = 0; u < 4; u++) {
-                    const int m = m0 + 128 * u;
-                    if (m < N / 2) {
-                        dd a = dd_load(f, N, (i - m) & mask), b = dd_load(f, N, (i + m) & mask);
-                        dd c = dd_load(dc, N, m);
-                        acc4[u] = dd_fma(c, dd_sub(a, b), acc4[u]);
-                    }
-                }
-            }
-        }
-    }
-    dd acc = dd_add(dd_add(acc4[0], acc4[1]), dd_add(acc4[2], acc4[3]));
-    acc = dd_warp_sum(acc);
-    if (lane == 0) {
-        part[node][q][0] = acc.hi;
-        part[node][q][1] = acc.lo;
-    }
-    __syncthreads();
-    if (q == 0 && lane == 0 && i < N) {
-        for (int r = 1; r < 4; r++) acc = dd_add(acc, dd{part[node][r][0], part[node][r][1]});
-        dd_store(out, N, i, acc);
-    }
-}
-
+// ------------------------------------------------------------------------------------------------ S0: node preparation
 // exp / expm1 / sinh / cosh for the node tables with the series divisions replaced by dd reciprocals from a shared table
 // rn[n] (+ rn[32 + n]) = 1 / n, n = 1..31 (one accurate division per lane instead of ~80 per node)
 __device__ __forceinline__ dd exp_series_tab(dd r, const double* rn, bool minus_one) {
@@ -100,35 +50,86 @@ __device__ __forceinline__ void dd_sinhcosh_tab_n(dd x, const double* rn, dd* sh
     *ch = dd_half(dd_add(e, ei));
 }
 
-// per-node tables in dd (planar): E = exp(-(h+eta)), Dm = 1 - E (via expm1) for the image term, sinh/cosh(eta) for the dd kernels.
-// The fp64 assembly reads the hi planes of E, Dm; the dd assembly and the dd base-state pass read everything.
-// Launch with 32 threads per block (one warp fills the reciprocal table).
-__global__ void __launch_bounds__(32) k_node_tables(int N, double h, int finite, const double* __restrict__ eta, double* __restrict__ E,
-                                                    double* __restrict__ Dm, double* __restrict__ Sh, double* __restrict__ Ch, int* status) {
+// S0 in ONE launch.  Per node i (four warps per node, two nodes per CTA of 8 warps):
+//   d1_i = sum_{m=1}^{N/2-1} dc[m] (f_{i-m} - f_{i+m}),  dc[m] = (1/2)(-1)^m cot(pi m/N)   (eta' = D eta; Nyquist symbol 0, R4)
+//   d2_i = c2[0] f_i + sum_{m=1}^{N/2} c2[m] (f_{i-m} + f_{i+m})                             (eta'' = D(D eta) as one circulant:
+//          symbol -k^2, 0 at the Nyquist mode; c2[N/2] is stored halved because the sum meets that node twice; tables.cu)
+//   and the per-node tables in dd (planar): E = exp(-(h+eta)), Dm = 1 - E (via expm1) for the image term, sinh/cosh(eta) for the dd
+//   kernels (the fp64 assembly reads the hi planes of E, Dm; the dd assembly and the dd base-state pass read everything).
+// The sums are chains of dependent dd operations behind scattered loads (their time is the length of the per-lane chain: four
+// independent chains per sum and lane); the three series of the tables run on lane 0 of the warps 1..3 of the node meanwhile.
+// Until round 2 these were three launches (D, D again on its own output, the tables): at N = 256 a third of a stage's launches.
+__global__ void __launch_bounds__(256) k_node_prep(int N, double h, int finite, const double* __restrict__ dc, const double* __restrict__ dc2,
+                                                   const double* __restrict__ f, double* __restrict__ d1, double* __restrict__ d2,
+                                                   double* __restrict__ E, double* __restrict__ Dm, double* __restrict__ Sh, double* __restrict__ Ch,
+                                                   int* status) {
+    __shared__ double part[2][4][4];
     __shared__ double rn[64];
-    {
-        const int n = threadIdx.x;
-        if (n >= 1) {
-            const dd r = dd_div(dd{1.0, 0.0}, dd{(double)n, 0.0});
-            rn[n] = r.hi;
-            rn[32 + n] = r.lo;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, node = warp >> 2, q = warp & 3;
+    const int i = blockIdx.x * 2 + node, mask = N - 1;
+    const int l128 = q * 32 + lane;  // position among the 128 lanes that share the node
+    if (threadIdx.x >= 1 && threadIdx.x < 32) {  // rn[n] (+ rn[32 + n]) = 1 / n for the series of the tables
+        const dd r = dd_div(dd{1.0, 0.0}, dd{(double)threadIdx.x, 0.0});
+        rn[threadIdx.x] = r.hi;
+        rn[32 + threadIdx.x] = r.lo;
+    }
+    dd a1[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};  // independent chains: a dd multiply-add is ~30 dependent instructions
+    dd a2[4] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+    if (i < N) {
+        if (l128 == 0) a2[0] = dd_mul(dd_load(dc2, N, 0), dd_load(f, N, i));
+        for (int m0 = 1 + l128; m0 <= N / 2; m0 += 512) {
+            dd c[4], e[4], a[4], b[4];
+            bool on[4];
+#pragma unroll
+            for (int u = 0; u < 4; u++) {  // the loads of a group are issued together
+                const int m = m0 + 128 * u;
+                on[u] = m <= N / 2;        // dc[N/2] = 0, dc2[N/2] halved: the Nyquist node is met once, with both neighbours equal
+                const int mm = on[u] ? m : 0;
+                c[u] = dd_load(dc, N, mm);
+                e[u] = dd_load(dc2, N, mm);
+                a[u] = dd_load(f, N, (i - mm) & mask);
+                b[u] = dd_load(f, N, (i + mm) & mask);
+            }
+#pragma unroll
+            for (int u = 0; u < 4; u++)
+                if (on[u]) {
+                    a1[u] = dd_fma(c[u], dd_sub(a[u], b[u]), a1[u]);
+                    a2[u] = dd_fma(e[u], dd_add(a[u], b[u]), a2[u]);
+                }
         }
-        __syncwarp();
     }
-    int j = blockIdx.x * blockDim.x + threadIdx.x;
-    if (j >= N) return;
-    dd e = dd_load(eta, N, j);
-    if (finite) {
-        dd Y = dd_add_d(e, h);
-        if (!(Y.hi > 0.0)) atomicCAS(status, SWW_OK, SWW_EBOTTOM);
-        dd nY = dd_neg(Y);
-        dd_store(E, N, j, dd_exp_tab(nY, rn));
-        dd_store(Dm, N, j, dd_neg(dd_expm1_tab(nY, rn)));
+    dd s1 = dd_warp_sum(dd_add(dd_add(a1[0], a1[1]), dd_add(a1[2], a1[3])));
+    dd s2 = dd_warp_sum(dd_add(dd_add(a2[0], a2[1]), dd_add(a2[2], a2[3])));
+    if (lane == 0) {
+        part[node][q][0] = s1.hi; part[node][q][1] = s1.lo;
+        part[node][q][2] = s2.hi; part[node][q][3] = s2.lo;
     }
-    dd sh, ch;
-    dd_sinhcosh_tab_n(e, rn, &sh, &ch);
-    dd_store(Sh, N, j, sh);
-    dd_store(Ch, N, j, ch);
+    __syncthreads();  // the partial sums and rn
+    if (lane != 0 || i >= N) return;
+    if (q == 0) {
+        for (int r = 1; r < 4; r++) {
+            s1 = dd_add(s1, dd{part[node][r][0], part[node][r][1]});
+            s2 = dd_add(s2, dd{part[node][r][2], part[node][r][3]});
+        }
+        dd_store(d1, N, i, s1);
+        dd_store(d2, N, i, s2);
+        return;
+    }
+    const dd e = dd_load(f, N, i);
+    if (q == 3) {
+        dd sh, ch;
+        dd_sinhcosh_tab_n(e, rn, &sh, &ch);
+        dd_store(Sh, N, i, sh);
+        dd_store(Ch, N, i, ch);
+    } else if (finite) {
+        const dd Y = dd_add_d(e, h);
+        if (q == 1) {
+            if (!(Y.hi > 0.0)) atomicCAS(status, SWW_OK, SWW_EBOTTOM);
+            dd_store(E, N, i, dd_exp_tab(dd_neg(Y), rn));
+        } else {
+            dd_store(Dm, N, i, dd_neg(dd_expm1_tab(dd_neg(Y), rn)));
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------ S1: fp64 assembly
@@ -520,15 +521,9 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
 static int run_node_prep(sww_dtn_s* d) {
     const int N = d->N;
     cudaStream_t st = d->stream;
-    int blocks = (N + 1) / 2;  // two nodes per CTA, four warps each
     SWW_BEGIN(KC_OTHER, st);
-    k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->eta, d->d1);
-    SWW_LAUNCHED();
-    SWW_BEGIN(KC_OTHER, st);
-    k_deriv_dd<<<blocks, 256, 0, st>>>(N, d->tab->dc, d->d1, d->d2);
-    SWW_LAUNCHED();
-    SWW_BEGIN(KC_OTHER, st);
-    k_node_tables<<<(N + 31) / 32, 32, 0, st>>>(N, d->h, d->finite ? 1 : 0, d->eta, d->E, d->Dm, d->Sh, d->Ch, d->status);
+    k_node_prep<<<(N + 1) / 2, 256, 0, st>>>(N, d->h, d->finite ? 1 : 0, d->tab->dc, d->tab->dc2, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch,
+                                              d->status);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

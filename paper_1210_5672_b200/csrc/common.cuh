@@ -65,6 +65,7 @@ struct Tables {
     double* c0;    // (1/2) cot(pi m / N), m >= 1; c0[0] = 0
     double* s2;    // sin^2(pi m / N)
     double* dc;    // differentiation circulant: (1/2) (-1)^m cot(pi m / N), m >= 1; dc[0] = 0, dc[N/2] = 0
+    double* dc2;   // the circulant of D(D .): symbol -k^2, Nyquist 0; the entry of m = N/2 stored halved (tables.cu)
     double2* tw;   // fp64 FFT twiddles exp(-2 pi i m / N) = (cs, -sn) rounded, m = 0..N-1
     double* filt;  // 36th-order filter exp(-36 (|k|/(N/2))^36) of (2.14) at DFT index m (|k| = min(m, N - m))
     double* filt_dd;  // the same in double-double (planar 2N)

@@ -59,7 +59,7 @@ void timing_end() {
     g_cur_open = false;
 }
 
-__global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, double* dc, double2* tw, double* filt, double* filt_dd) {
+__global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, double* dc, double* dc2, double2* tw, double* filt, double* filt_dd) {
     int m = blockIdx.x * blockDim.x + threadIdx.x;
     if (m >= N) return;
     {
@@ -85,6 +85,18 @@ __global__ void k_tables(int N, double* cs, double* sn, double* c0, double* s2, 
     dd_store(s2, N, m, dd_sqr(sh));
     dd d = (m & 1) ? dd_neg(cot) : cot;  // (1/2)(-1)^m cot(pi m/N): Fourier differentiation matrix for even N (Nyquist -> 0, R4)
     dd_store(dc, N, m, d);
+    // D(D .) as one circulant: symbol -k^2 for |k| < N/2 and 0 at the Nyquist mode (R4) = the textbook second-derivative matrix
+    // (-(-1)^m / (2 sin^2(pi m/N)), -N^2/12 - 1/6 on the diagonal) minus its Nyquist term (1/N)(-(N/2)^2)(-1)^m.  The entry of
+    // m = N/2 is stored halved: the node-prep kernel sums c2[m] (f_{i-m} + f_{i+m}) over m = 1 .. N/2 and meets that node twice.
+    dd c2;
+    if (m == 0) {
+        c2 = dd_add_d(dd_neg(dd_add(dd_div_d(dd{(double)N * (double)N, 0.0}, 12.0), dd_div_d(dd{1.0, 0.0}, 6.0))), 0.25 * (double)N);
+    } else {
+        c2 = dd_sub(dd{0.25 * (double)N, 0.0}, dd_div(dd{0.5, 0.0}, dd_sqr(sh)));
+        if (m & 1) c2 = dd_neg(c2);
+        if (2 * m == N) c2 = dd_half(c2);
+    }
+    dd_store(dc2, N, m, c2);
 }
 
 static std::mutex g_tab_mu;
@@ -103,8 +115,8 @@ int get_tables(int N, cudaStream_t st, const Tables** out) {
     Tables* t = new Tables();
     t->N = N;
     double* base = nullptr;
-    // 6 dd tables of 2N doubles + N double2 + N doubles
-    SWW_CUDA(cudaMalloc(&base, sizeof(double) * (size_t)N * 15));
+    // 7 dd tables of 2N doubles + N double2 + N doubles
+    SWW_CUDA(cudaMalloc(&base, sizeof(double) * (size_t)N * 17));
     t->cs = base;
     t->sn = base + 2 * (size_t)N;
     t->c0 = base + 4 * (size_t)N;
@@ -113,9 +125,10 @@ int get_tables(int N, cudaStream_t st, const Tables** out) {
     t->tw = reinterpret_cast<double2*>(base + 10 * (size_t)N);
     t->filt = base + 12 * (size_t)N;
     t->filt_dd = base + 13 * (size_t)N;
+    t->dc2 = base + 15 * (size_t)N;
     // the default stream orders this before any later stream work after the synchronize below
     SWW_BEGIN(KC_OTHER, st);
-    k_tables<<<(N + 127) / 128, 128, 0, st>>>(N, t->cs, t->sn, t->c0, t->s2, t->dc, t->tw, t->filt, t->filt_dd);
+    k_tables<<<(N + 127) / 128, 128, 0, st>>>(N, t->cs, t->sn, t->c0, t->s2, t->dc, t->dc2, t->tw, t->filt, t->filt_dd);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     SWW_CUDA(cudaStreamSynchronize(st));
