@@ -46,7 +46,8 @@ enum {
     SWW_ECUDA = -3,     /* a CUDA runtime call failed; sww_last_cuda_error() has the text                             */
     SWW_EBOTTOM = -4,   /* some h + eta_j <= 0: the surface touches the bottom                                         */
     SWW_ESINGULAR = -5, /* a pivot of the unpivoted LU fell below the guard (|U_ii| < 1e-3): I/2+K is not benign here  */
-    SWW_ENOBASE = -6    /* sww_dtn_linearized_apply before sww_dtn_set_base                                            */
+    SWW_ENOBASE = -6,   /* sww_dtn_linearized_apply before sww_dtn_set_base                                            */
+    SWW_ETOOBIG = -7    /* a size beyond the fixed scratch of a no-allocation entry point; sww_last_cuda_error() has the text */
 };
 
 /* ---- DtN operator of one surface -------------------------------------------------------------------------------
@@ -150,6 +151,19 @@ int sww_mesh_points(int N, double rho, int where, double* x);
  * product in double-double); dst's elapsed time becomes src's.  Synchronises both streams. */
 int sww_state_set_mesh(sww_state_t s, double rho, int where);
 int sww_state_respace(sww_state_t dst, sww_state_t src);
+/* The same respacing for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * cudaMalloc): out (M_new x ncol) <- the ncol columns f (M_old x ncol, fp64, column c at c * M) given on the mesh (rho_old, where_old)
+ * with M_old points, interpolated to the mesh (rho_new, where_new) with M_new points (the arithmetic of sww_state_respace for SWW_F64
+ * states; the interpolation matrix is not stored, its entries are formed where they are used).  f, out: DEVICE, distinct.  No handle.
+ * The call makes no cudaMalloc / cudaFree and calls no allocating routine: its scratch (4 M_new doubles) is a fixed device array inside
+ * the library, 128 KB held by every GPU that loads it until exit.  Limits: M_new <= SWW_RESPACE_NOALLOC_MAX (beyond: SWW_ETOOBIG, text
+ * in sww_last_cuda_error()), M_old even, 4 <= M_old <= 8192; neither size needs to be a power of two.  Two kernels are enqueued on
+ * `stream`; nothing synchronises.  The first call on each device looks the array's address up (cudaGetSymbolAddress): make it before a
+ * graph capture starts.  ALL calls share the one array, which keeps the last call's contents (every entry a call reads it has written
+ * first, nothing needs clearing): calls that overlap on the GPU (different streams, no ordering between them) race on it -- order them. */
+#define SWW_RESPACE_NOALLOC_MAX 4096
+int sww_respace_noalloc(int M_old, double rho_old, int where_old, int M_new, double rho_new, int where_new, int ncol, const double* f,
+                        double* out, void* stream);
 
 /* ---- shooting map of the overdetermined shooting method, uniform mesh (section 3.1 / 3.3) ------------------------
  * Unknowns c (HOST, n + 1 doubles): c[0] = T, the period (3.16); c[k], 1 <= k <= n, the Fourier modes of the initial

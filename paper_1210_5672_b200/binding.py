@@ -19,7 +19,7 @@ EXPORTS = [
     "sww_dtn_linearized_host", "sww_host_cache_clear", "sww_timing_enable", "sww_timing_read",
     "sww_shooter_create", "sww_shoot", "sww_shooter_destroy", "sww_shoot_residual", "sww_shooter_dims", "sww_lm_minimize", "sww_lm_shoot",
     "sww_state_set_sigma", "sww_shooter_set_sigma", "sww_sdc_advance", "sww_dtn_adjoint_rhs", "sww_shooter_set_method",
-    "sww_dtn_set_mesh", "sww_mesh_points", "sww_state_set_mesh", "sww_state_respace", "sww_shooter_set_segments", "sww_shoot_gradient",
+    "sww_dtn_set_mesh", "sww_mesh_points", "sww_state_set_mesh", "sww_state_respace", "sww_shooter_set_segments", "sww_shoot_gradient", "sww_respace_noalloc",
 ]
 
 
@@ -49,7 +49,7 @@ class SwwError(RuntimeError):
     def __init__(self, status: int, what: str):
         self.status = status
         msg = lib().sww_strerror(status).decode()
-        if status == -3:
+        if status in (-3, -7):
             msg += ": " + lib().sww_last_cuda_error().decode()
         super().__init__(f"{what}: {msg} (status {status})")
 
@@ -102,6 +102,7 @@ def lib() -> ctypes.CDLL:
         L.sww_mesh_points.argtypes = [ci, cd, ci, ctypes.POINTER(cd)]
         L.sww_state_set_mesh.argtypes = [vp, cd, ci]
         L.sww_state_respace.argtypes = [vp, vp]
+        L.sww_respace_noalloc.argtypes = [ci, cd, ci, ci, cd, ci, ci, vp, vp, vp]
         L.sww_shoot_gradient.argtypes = [vp, ctypes.POINTER(cd), ci, ctypes.POINTER(cd), ctypes.POINTER(cd)]
         L.sww_shooter_set_segments.argtypes = [vp, ci, ctypes.POINTER(ci), ctypes.POINTER(cd), ctypes.POINTER(cd), ctypes.POINTER(ci), ctypes.POINTER(ci)]
         L.sww_timing_enable.argtypes = [ci]
@@ -428,6 +429,23 @@ def mesh_points(N: int, rho: float, where: int = 0):
     x = np.empty(N)
     _check(lib().sww_mesh_points(int(N), float(rho), int(where), x.ctypes.data_as(ctypes.POINTER(ctypes.c_double))), "sww_mesh_points")
     return x
+
+
+RESPACE_NOALLOC_MAX = 4096
+
+
+def respace_noalloc(f: torch.Tensor, old, new, out: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None) -> torch.Tensor:
+    """sww_respace_noalloc: f (ncol, M_old) on the mesh old = (M_old, rho, where) -> (ncol, M_new) on new = (M_new, rho, where); the library
+    allocates nothing (pass `out` to keep torch from allocating as well).  M_new <= RESPACE_NOALLOC_MAX."""
+    _require_cuda()
+    Mo, Mn = int(old[0]), int(new[0])
+    ncol = f.numel() // Mo
+    if out is None:
+        out = torch.empty((ncol, Mn), dtype=torch.float64, device="cuda")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    _check(lib().sww_respace_noalloc(Mo, float(old[1]), int(old[2]), Mn, float(new[1]), int(new[2]), ncol, _dev(f, ncol * Mo, "f"),
+                                     _dev(out, ncol * Mn, "out"), st.cuda_stream), "sww_respace_noalloc")
+    return out
 
 
 def dtn_linearized_host(eta, phi0, deta, dphi, h: float, prec: int = F64, out=None):

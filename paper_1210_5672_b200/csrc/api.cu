@@ -215,6 +215,7 @@ const char* sww_strerror(int status) {
         case SWW_EBOTTOM: return "surface touches the bottom (h + eta <= 0)";
         case SWW_ESINGULAR: return "pivot below guard in the unpivoted LU of I/2 + K";
         case SWW_ENOBASE: return "linearized apply before set_base";
+        case SWW_ETOOBIG: return "size beyond the fixed scratch of a no-allocation entry point";
         default: return "unknown status";
     }
 }

@@ -176,6 +176,66 @@ __global__ void k_respace_apply_dd(int Mo, int Mn, int ncol, const double* __res
     out[Lout + (size_t)c * Mn + j] = r.lo;
 }
 
+// ------------------------------------------------------------------------------------------------ respacing without any allocation
+// sww_respace_noalloc: the respacing of sww_state_respace for callers that cannot call cudaMalloc (CUDA graph capture, serving loops).
+// The scratch of k_respace_nodes (beta_j and sin(Mo beta_j / 2), double-double planar: 4 Mn doubles) lives in a file-scope device
+// array of fixed size; the interpolation matrix is never stored (its entries are formed where they are used).  Every GPU that loads
+// the library holds the 128 KB until exit.  In host code `g_respace_scratch` is only a stand-in for the symbol: kernels get the
+// device address that cudaGetSymbolAddress returned for the current device (respace_scratch_ptr below).
+constexpr int RESPACE_NOALLOC_MAX = 4096;  // largest new mesh (SWW_RESPACE_NOALLOC_MAX of include/sww.h)
+static __device__ __align__(256) double g_respace_scratch[4 * RESPACE_NOALLOC_MAX];
+
+constexpr int RESPACE_MAX_DEVICES = 64;
+static double* g_respace_scratch_ptr[RESPACE_MAX_DEVICES];  // per device: the array's device address, looked up once
+static int respace_scratch_ptr(double** out) {
+    int dev = 0;
+    SWW_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= RESPACE_MAX_DEVICES) return SWW_EINVAL;
+    if (!g_respace_scratch_ptr[dev]) {
+        double* ptr = nullptr;
+        SWW_CUDA(cudaGetSymbolAddress((void**)&ptr, g_respace_scratch));
+        if (!ptr) return SWW_ECUDA;
+        g_respace_scratch_ptr[dev] = ptr;
+    }
+    *out = g_respace_scratch_ptr[dev];
+    return SWW_OK;
+}
+
+// out[j + c Mn] = sum_m D(beta_j - alpha_m) f[m + c Mo], the entries of k_respace_matrix formed on the fly (same arithmetic); a thread
+// serves one new node j and up to four columns (the entries do not depend on the column); alpha_m goes through shared memory in
+// chunks of 128 (double-double: a quotient per m, not per (j, m)).  grid: (ceil(Mn / 128), ceil(ncol / 4)), 128 threads.
+__global__ void __launch_bounds__(128) k_respace_direct(int Mo, int Mn, int ncol, const double* __restrict__ beta, const double* __restrict__ sj,
+                                                        const double* __restrict__ f, double* __restrict__ out) {
+    __shared__ double a_hi[128], a_lo[128];
+    const int j = blockIdx.x * 128 + threadIdx.x, c0 = blockIdx.y * 4;
+    const int nc = min(4, ncol - c0);
+    const bool on = j < Mn;
+    const dd bj = on ? dd_load(beta, Mn, j) : dd{0.0, 0.0};
+    const double sjj = on ? sj[j] : 0.0, rMo = (double)Mo;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (int m0 = 0; m0 < Mo; m0 += 128) {
+        __syncthreads();
+        if (m0 + threadIdx.x < Mo) {
+            const dd am = dd_div_d(dd_mul_d(dd_mul_d(dd_pi(), 2.0), (double)(m0 + threadIdx.x)), rMo);
+            a_hi[threadIdx.x] = am.hi;
+            a_lo[threadIdx.x] = am.lo;
+        }
+        __syncthreads();
+        if (!on) continue;
+        const int mn = min(128, Mo - m0);
+        for (int q = 0; q < mn; q++) {
+            const int m = m0 + q;
+            const dd t = dd_sub(bj, dd{a_hi[q], a_lo[q]});
+            const double th = 0.5 * (t.hi + t.lo);
+            double v = 1.0;
+            if (fabs(th) >= 1e-13) v = ((m & 1) ? -sjj : sjj) / (tan(th) * rMo);
+            for (int c = 0; c < nc; c++) acc[c] = fma(v, f[(size_t)(c0 + c) * Mo + m], acc[c]);
+        }
+    }
+    if (on)
+        for (int c = 0; c < nc; c++) out[(size_t)(c0 + c) * Mn + j] = acc[c];
+}
+
 }  // namespace sww
 
 extern "C" {
@@ -275,6 +335,28 @@ int sww_state_respace(sww_state_t dst, sww_state_t src) {
     SWW_CUDA(cudaStreamSynchronize(st));
     dst->t = src->t;
     dst->dtn->has_base = false;
+    return SWW_OK;
+}
+
+int sww_respace_noalloc(int Mo, double rho_o, int where_o, int Mn, double rho_n, int where_n, int ncol, const double* f, double* out, void* stream) {
+    if (!f || !out || f == out || ncol < 1) return SWW_EINVAL;
+    if (Mo < 4 || (Mo & 1) || Mo > 8192 || Mn < 1) return SWW_EINVAL;
+    if (!(rho_o > 0.0 && rho_o <= 1.0) || !(rho_n > 0.0 && rho_n <= 1.0) || (where_o != 0 && where_o != 1) || (where_n != 0 && where_n != 1))
+        return SWW_EINVAL;
+    if (Mn > RESPACE_NOALLOC_MAX) {  // the fixed scratch holds 4 doubles per new node
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "sww_respace_noalloc: M_new = %d exceeds SWW_RESPACE_NOALLOC_MAX = %d (fixed device scratch)", Mn,
+                 RESPACE_NOALLOC_MAX);
+        return SWW_ETOOBIG;
+    }
+    double* scr = nullptr;
+    SWW_TRY(respace_scratch_ptr(&scr));  // the first call on a device looks the address up; no allocation here or below
+    cudaStream_t st = (cudaStream_t)stream;
+    // beta (2 Mn) and sin(Mo beta / 2) (2 Mn) are written in full for j < Mn before they are read: nothing of an earlier call survives
+    k_respace_nodes<<<(Mn + 63) / 64, 64, 0, st>>>(Mo, rho_o, where_o, Mn, rho_n, where_n, scr, scr + 2 * (size_t)Mn);
+    ++g_launches;
+    k_respace_direct<<<dim3((Mn + 127) / 128, (ncol + 3) / 4), 128, 0, st>>>(Mo, Mn, ncol, scr, scr + 2 * (size_t)Mn, f, out);
+    ++g_launches;
+    SWW_CUDA(cudaGetLastError());
     return SWW_OK;
 }
 
