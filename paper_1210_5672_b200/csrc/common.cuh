@@ -171,7 +171,8 @@ int mesh_scale_out(sww_dtn_s* d, double* out, int nrhs, size_t L);
 // spectral (fft.cu)
 enum SpecMode { SPEC_APPLY = 0, SPEC_LIN = 1 };
 // For each column c < ncols: Gam_c = D M_c ;  W_c = |D| M_c / 2  - (T ? D T_c : 0)
-int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols);
+// Mp (optional, ncols = 2): the source of column 1 (see fft.cu)
+int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols, const double* Mp = nullptr);
 // out_c = D in_c
 int spectral_deriv(sww_dtn_s* d, const double* in, double* out, int ncols);
 

@@ -619,14 +619,14 @@ int fast_base_f64(sww_dtn_s* d, const double* phi0) {
     Workspace& w = d->ws;
     SWW_CUDA(cudaMemcpyAsync(w.B, phi0, sizeof(double) * N, cudaMemcpyDeviceToDevice, st));
     SWW_TRY(run_solve(d, w.B, w.S, 1));                               // mu0
-    SWW_TRY(spectral_gamma_w(d, w.B, nullptr, w.Gam, w.W, 1, 1));     // gamma = D mu0 ; W = |D| mu0 / 2
+    // gamma = D mu0 ; W = |D| mu0 / 2 ; phi0 rides along as the partner column of the transform pair: Gam column 1 = D phi0
+    SWW_TRY(spectral_gamma_w(d, w.B, nullptr, w.Gam, w.W, 2, 1, phi0));
     if (N >= 128 && (size_t)d->bp_chunks * 4 >= 16)
         SWW_TRY(gemv_few_f64(st, N, 1, N, d->G, N, w.Gam, N, w.W, N, d->bp_part, d->mv_count));
     else
         SWW_TRY(gemm_f64(st, N, 1, N, 1.0, d->G, N, w.Gam, N, 1.0, w.W, N, 1));
-    SWW_TRY(spectral_deriv(d, phi0, w.T, 1));                          // phi0'
     SWW_BEGIN(KC_OTHER, st);
-    k_base_uv_f64<<<(N + 255) / 256, 256, 0, st>>>(N, d->d1, w.T, w.W, d->bphi, d->bW0, d->bu, d->bv, d->mesh_on ? d->mesh.xE : nullptr);
+    k_base_uv_f64<<<(N + 255) / 256, 256, 0, st>>>(N, d->d1, w.Gam + N, w.W, d->bphi, d->bW0, d->bu, d->bv, d->mesh_on ? d->mesh.xE : nullptr);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;

@@ -14,9 +14,11 @@ namespace sww {
 
 
 // Gam_c = D M_c ;  W_c = |D| M_c / 2 - (T ? D T_c : 0)     for the column pair (2*blockIdx.x, 2*blockIdx.x + 1)
+// Mp (optional, ncols = 2): column 1 is read from Mp instead of M + N -- the single-vector base state rides phi0 along with mu0 so that
+// Gam_1 = D phi0 comes out of the same transform pair (one launch less per stage of the stepper)
 __global__ void __launch_bounds__(1024) k_spectral_gamma_w(int N, int logN, const double2* __restrict__ tw, const double* __restrict__ M,
                                    const double* __restrict__ T, double* __restrict__ Gam, double* __restrict__ W, int ncols,
-                                   int w_cols) {
+                                   int w_cols, const double* __restrict__ Mp) {
     extern __shared__ __align__(16) double2 z[];
     const int c0 = 2 * blockIdx.x, c1 = c0 + 1;
     const bool has1 = c1 < ncols;
@@ -32,7 +34,8 @@ __global__ void __launch_bounds__(1024) k_spectral_gamma_w(int N, int logN, cons
             if (r < per && threadIdx.x + r * blockDim.x < N) zt[r] = z[threadIdx.x + r * blockDim.x];
         __syncthreads();
     }
-    for (int j = threadIdx.x; j < N; j += blockDim.x) z[j] = make_double2(M[(size_t)c0 * N + j], has1 ? M[(size_t)c1 * N + j] : 0.0);
+    for (int j = threadIdx.x; j < N; j += blockDim.x)
+        z[j] = make_double2(M[(size_t)c0 * N + j], has1 ? (Mp ? Mp[j] : M[(size_t)c1 * N + j]) : 0.0);
     __syncthreads();
     fft_dif(z, N, tw);
     double2 zm[FFT_MAX_PER_THREAD];
@@ -99,7 +102,7 @@ __global__ void __launch_bounds__(1024) k_spectral_deriv(int N, int logN, const 
     }
 }
 
-int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols) {
+int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam, double* W, int ncols, int w_cols, const double* Mp) {
     const int N = d->N;
     size_t smem = sizeof(double2) * (size_t)N;
     static DeviceOnce attr_once;
@@ -111,7 +114,7 @@ int spectral_gamma_w(sww_dtn_s* d, const double* M, const double* T, double* Gam
     // 512 threads at N = 2048, 4096: two CTAs per SM hide each other's barriers (0.072 -> 0.062 ms at the metric point); the per-thread
     // register arrays hold N / threads <= 8 entries
     const int thr = (N == 2048 || N == 4096) ? 512 : fft_threads(N);
-    k_spectral_gamma_w<<<(ncols + 1) / 2, thr, smem, d->stream>>>(N, fft_ilog2(N), d->tab->tw, M, T, Gam, W, ncols, w_cols);
+    k_spectral_gamma_w<<<(ncols + 1) / 2, thr, smem, d->stream>>>(N, fft_ilog2(N), d->tab->tw, M, T, Gam, W, ncols, w_cols, Mp);
     SWW_LAUNCHED();
     SWW_CUDA(cudaGetLastError());
     return SWW_OK;
