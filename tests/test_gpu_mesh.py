@@ -442,3 +442,33 @@ def test_maximum_and_minimum_size_on_refined_mesh(sww, mesh_ld):
     mesh_ld.set_mesh(0.5, 1)
     ref = ld(mesh_ld.dtn_apply(eta, h, phi1[None, :]))[0]
     assert float(np.abs(got - ref).max()) <= 1e-13
+
+
+def test_metric_point_on_refined_mesh_sampled_columns(sww, mesh_ld):
+    """the metric workload (N = 2048, 512 columns, all computed) on the mesh (2.10) with rho = 0.3, as bench.py's configs.metric_refined_mesh
+    times it; the oracle checks 12 sampled columns (k = 1, 2, 3, N/8, N/4 always included) with the rule of parity_util, bar and floor
+    divided by rho^2"""
+    from parity_util import sample_columns, lin_scales, EPS
+    rho, where = 0.3, 0
+    c = si.metric_point(512)
+    cols = sample_columns(c, 12)
+    d = sww.DtN(dev(c.eta), c.h)
+    d.set_mesh(rho, where)
+    d.refactor(dev(c.eta))
+    d.set_base(dev(c.phi0))
+    out = d.linearized_apply(dev(c.deta), dev(c.dphi))
+    d.check()
+    got = out.cpu().numpy()[cols]
+    mesh_ld.set_mesh(rho, where)
+    orc, base = mesh_ld.dtn_linearized(c.eta, c.h, c.phi0, c.deta[cols], c.dphi[cols], want_base=True)
+    ref = ld(orc)
+    S = lin_scales(c, base, cols)
+    err = np.abs(got.astype(LD) - ref).max(axis=1)
+    nrm = np.abs(ref).max(axis=1)
+    worst = 0.0
+    for i in range(len(cols)):
+        floor = float(4 * c.N * EPS["f64"] * S[i] / nrm[i])
+        e = float(err[i] / nrm[i])
+        assert e <= max(1e-11, floor) / rho ** 2, (int(cols[i]), e, floor)
+        worst = max(worst, e)
+    print("metric point on the refined mesh: E_col_max", worst)
