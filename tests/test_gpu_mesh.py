@@ -472,3 +472,43 @@ def test_metric_point_on_refined_mesh_sampled_columns(sww, mesh_ld):
         assert e <= max(1e-11, floor) / rho ** 2, (int(cols[i]), e, floor)
         worst = max(worst, e)
     print("metric point on the refined mesh: E_col_max", worst)
+
+
+def test_sdc15_step_on_refined_mesh_fp64(sww, mesh_ld):
+    """the SDC15 stepper through the refined-mesh right-hand sides in fp64: one large step against the oracle"""
+    N, nc, h, rho, where = 64, 2, 1.0, 0.5, 0
+    eta, phi, deta, dphi = small_case(N, nc)
+    dt = 0.08
+    st = sww.State(dev(eta), dev(phi), h, 1.0, deta=dev(deta), dphi=dev(dphi))
+    st.set_mesh(rho, where)
+    st.advance(dt, 1, method="sdc15")
+    r = st.read()
+    mesh_ld.set_mesh(rho, where)
+    o = mesh_ld.rk_advance(eta, phi, h, 1.0, dt, 1, deta=deta, dphi=dphi, method="sdc15")
+    for name in ("eta", "phi", "deta", "dphi"):
+        g, q = r[name].cpu().numpy().astype(LD).reshape(-1, N), ld(o[name]).reshape(-1, N)
+        err = np.abs(g - q).max(axis=1) / np.abs(q).max(axis=1)
+        assert float(err.max()) <= 1e-11 / rho ** 2, (name, err)
+
+
+def test_capillary_shooting_with_segments_in_deep_water(sww, mesh_ld):
+    """section 4.6 meets section 2.2: infinite depth, surface tension, two segments with a refined second mesh -- every stepper of the
+    shooter gets sigma; r and J against oracle/shooting.shoot_segments"""
+    from oracle import shooting
+    n, sigma, h = 5, 0.1, float("inf")
+    # capillary waves are stiff: omega_max ~ sqrt(sigma k^3), k = (M/2) / min xi' -- 96 at the refined end here, omega dt = 1.25
+    segs = [(32, 0.5, 1.0, 0, 16), (64, 0.5, 0.6, 1, 48)]
+    c = shoot_unknowns(n, T=5.0, amp=-0.01)
+    S = sww.Shooter(32, n, h, 1.0)
+    S.set_sigma(sigma)
+    S.set_segments(segs)
+    r, J = S.shoot(c, 1)
+    S.close()
+    o = shooting.shoot_segments(mesh_ld, c, segs, h, 1.0, sigma=sigma)
+    assert np.isfinite(o["r"]).all()
+    tol = 1e-11 / 0.36
+    assert float(np.abs(r.cpu().numpy().astype(LD) - o["r"]).max() / np.abs(o["r"]).max()) <= tol
+    e = np.abs(J.cpu().numpy().astype(LD) - o["J"].T).max(axis=1) / np.abs(o["J"].T).max(axis=1)
+    assert float(e.max()) <= tol, e
+    o0 = shooting.shoot_segments(mesh_ld, c, segs, h, 1.0, sigma=0.0)
+    assert np.abs(o0["r"] - o["r"]).max() > 1e-4 * np.abs(o["r"]).max()      # the term matters
