@@ -244,6 +244,10 @@ def other_configs(sww, flush, peak_tf):
     ms = lin_case(c3, sww.F64, 20)
     out["config3"] = {"workload": "N=512, 256 columns, fp64", "ms_per_step": ms, "columns_per_s": c3.nrhs / (ms * 1e-3),
                       "bound": "latency (8-block LU chain, launch sequence)"}
+    c3b = si.config3(N=1024, ncols=256)
+    ms = lin_case(c3b, sww.F64, 20)
+    out["n1024"] = {"workload": "N=1024, 256 columns, fp64 (config-3 family; fills the N sweep between configs 3 and the metric point)", "ms_per_step": ms,
+                    "columns_per_s": c3b.nrhs / (ms * 1e-3), "bound": "latency (16-block LU chain) + FP64 tensor"}
     c4 = si.config4()
     ms = lin_case(c4, sww.DD, 10)
     out["config4"] = {"workload": "N=512, 128 columns, double-double", "ms_per_step": ms, "columns_per_s": c4.nrhs / (ms * 1e-3),

@@ -311,15 +311,25 @@ struct TabDD {  // functions of m = (i - j) mod N
 
 // K_ij, G_ij of (2.13) in dd (already scaled by 1/N); dist = circular distance |i-j|
 // rc: shared table of dd reciprocals 1 / (m (m + 1)) (fill_rc below) for the in-band series
-template <bool FINITE, bool MESH>
+// SLOPPY (the fp64 handle's base-state pass only, which needs the entries to ~1e-20, not 1e-31): sums by the 11-flop addition (error
+// ~2^-104 relative to the LARGER operand, so a cancelling difference is less accurate than with the 20-flop dd_add -- harmless at that
+// target); the argument y = eta_i - eta_j and the in-band series keep the accurate addition.
+__device__ __forceinline__ dd dd_add_sloppy(dd a, dd b) {
+    dd s = two_sum(a.hi, b.hi);
+    s.lo = SWW_ADD(s.lo, SWW_ADD(a.lo, b.lo));
+    return quick_two_sum(s.hi, s.lo);
+}
+template <bool FINITE, bool MESH, bool SLOPPY = false>
 __device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, const TabDD& t0, int dist, double rN, const double* rc,
                                          dd* kv, dd* gv) {
+    auto add_ = [](dd a, dd b) { return SLOPPY ? dd_add_sloppy(a, b) : dd_add(a, b); };
+    auto sub_ = [](dd a, dd b) { return SLOPPY ? dd_add_sloppy(a, dd_neg(b)) : dd_sub(a, b); };
     TabDD t = t0;
     if (MESH) {  // sin, cos of (alpha_i - alpha_j) + (p_i - p_j); sin^2 of half of it without cancellation
-        const dd sd = dd_sub(dd_mul(ni.xS, nj.xC), dd_mul(ni.xC, nj.xS)), cd = dd_add(dd_mul(ni.xC, nj.xC), dd_mul(ni.xS, nj.xS));
-        t.sn = dd_add(dd_mul(t0.sn, cd), dd_mul(t0.cs, sd));
-        t.cs = dd_sub(dd_mul(t0.cs, cd), dd_mul(t0.sn, sd));
-        t.s2 = t.cs.hi >= 0.0 ? dd_div(dd_sqr(t.sn), dd_mul_d(dd_add_d(t.cs, 1.0), 2.0)) : dd_half(dd_sub(dd{1.0, 0.0}, t.cs));
+        const dd sd = sub_(dd_mul(ni.xS, nj.xC), dd_mul(ni.xC, nj.xS)), cd = add_(dd_mul(ni.xC, nj.xC), dd_mul(ni.xS, nj.xS));
+        t.sn = add_(dd_mul(t0.sn, cd), dd_mul(t0.cs, sd));
+        t.cs = sub_(dd_mul(t0.cs, cd), dd_mul(t0.sn, sd));
+        t.s2 = t.cs.hi >= 0.0 ? dd_div(dd_sqr(t.sn), dd_mul_d(dd_add_d(t.cs, 1.0), 2.0)) : dd_half(sub_(dd{1.0, 0.0}, t.cs));
     }
     dd k1, g1;
     if (dist != 0) {
@@ -330,26 +340,26 @@ __device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, con
         } else if (dist <= DD_BAND) {
             dd_sinhcosh(y, &sh, &ch);
         } else {
-            sh = dd_sub(dd_mul(ni.Sh, nj.Ch), dd_mul(ni.Ch, nj.Sh));
-            ch = dd_sub(dd_mul(ni.Ch, nj.Ch), dd_mul(ni.Sh, nj.Sh));
+            sh = sub_(dd_mul(ni.Sh, nj.Ch), dd_mul(ni.Ch, nj.Sh));
+            ch = sub_(dd_mul(ni.Ch, nj.Ch), dd_mul(ni.Sh, nj.Sh));
         }
         dd p;
         if (t.cs.hi >= 0.0)
-            p = dd_div_fast(dd_add(t.cs, ch), dd_add(dd_sqr(t.sn), dd_sqr(sh)));
+            p = dd_div_fast(add_(t.cs, ch), add_(dd_sqr(t.sn), dd_sqr(sh)));
         else
-            p = dd_div_fast(dd{1.0, 0.0}, dd_sub(ch, t.cs));
+            p = dd_div_fast(dd{1.0, 0.0}, sub_(ch, t.cs));
         dd hp = dd_half(p);
         if (MESH) {
-            k1 = dd_mul(hp, dd_sub(dd_mul(nj.d1, t.sn), dd_mul(nj.xE, sh)));
-            g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(ni.d1, sh), dd_mul(ni.xE, t.sn))), t.c0);
+            k1 = dd_mul(hp, sub_(dd_mul(nj.d1, t.sn), dd_mul(nj.xE, sh)));
+            g1 = sub_(dd_mul(hp, add_(dd_mul(ni.d1, sh), dd_mul(ni.xE, t.sn))), t.c0);
         } else {
-            k1 = dd_mul(hp, dd_sub(dd_mul(nj.d1, t.sn), sh));
-            g1 = dd_sub(dd_mul(hp, dd_add(dd_mul(ni.d1, sh), t.sn)), t.c0);
+            k1 = dd_mul(hp, sub_(dd_mul(nj.d1, t.sn), sh));
+            g1 = sub_(dd_mul(hp, add_(dd_mul(ni.d1, sh), t.sn)), t.c0);
         }
     } else if (MESH) {
-        dd den = dd_mul_d(dd_add(dd_sqr(ni.d1), dd_sqr(ni.xE)), 2.0);
-        k1 = dd_neg(dd_div(dd_sub(dd_mul(ni.d2, ni.xE), dd_mul(ni.xE1, ni.d1)), den));
-        g1 = dd_div(dd_add(dd_mul(ni.xE1, ni.xE), dd_mul(ni.d1, ni.d2)), den);
+        dd den = dd_mul_d(add_(dd_sqr(ni.d1), dd_sqr(ni.xE)), 2.0);
+        k1 = dd_neg(dd_div(sub_(dd_mul(ni.d2, ni.xE), dd_mul(ni.xE1, ni.d1)), den));
+        g1 = dd_div(add_(dd_mul(ni.xE1, ni.xE), dd_mul(ni.d1, ni.d2)), den);
     } else {
         dd den = dd_mul_d(dd_add_d(dd_sqr(ni.d1), 1.0), 2.0);
         k1 = dd_neg(dd_div(ni.d2, den));
@@ -358,16 +368,16 @@ __device__ __forceinline__ void entry_dd(const NodeDD& ni, const NodeDD& nj, con
     dd k2{0, 0}, g2{0, 0};
     if (FINITE) {
         dd Eij = dd_mul(ni.E, nj.E);
-        dd omE = dd_add(dd_mul(ni.E, nj.Dm), ni.Dm);
-        dd den = dd_add(dd_sqr(omE), dd_mul_d(dd_mul(Eij, t.s2), 4.0));
+        dd omE = add_(dd_mul(ni.E, nj.Dm), ni.Dm);
+        dd den = add_(dd_sqr(omE), dd_mul_d(dd_mul(Eij, t.s2), 4.0));
         const double rb = rcp_normal(den.hi);  // both quotients share the reciprocal
         dd cr = dd_div_rb(dd_mul(Eij, t.sn), den, rb);
         dd ci = dd_neg(dd_half(dd_div_rb(dd_mul(omE, dd_add_d(Eij, 1.0)), den, rb)));
-        k2 = dd_sub(MESH ? dd_mul(nj.xE, ci) : ci, dd_mul(nj.d1, cr));
-        g2 = dd_sub(MESH ? dd_mul(ni.xE, cr) : cr, dd_mul(ni.d1, ci));
+        k2 = sub_(MESH ? dd_mul(nj.xE, ci) : ci, dd_mul(nj.d1, cr));
+        g2 = sub_(MESH ? dd_mul(ni.xE, cr) : cr, dd_mul(ni.d1, ci));
     }
-    *kv = dd_mul_d(dd_sub(k1, k2), rN);
-    *gv = dd_mul_d(dd_sub(g1, g2), rN);
+    *kv = dd_mul_d(sub_(k1, k2), rN);
+    *gv = dd_mul_d(sub_(g1, g2), rN);
 }
 // rc[m] (+ rc[32 + m]) = 1 / (m (m + 1)) in dd, m = 1..30; call with every thread of the CTA (ends with a barrier)
 __device__ __forceinline__ void fill_rc(double* rc, int tid) {
@@ -455,7 +465,7 @@ __global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const
         const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
         TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
         dd kv, gv;
-        entry_dd<FINITE, MESH>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
+        entry_dd<FINITE, MESH, true>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
         aK = dd_fma(kv, dd_load(mu, N, j), aK);
         aG = dd_fma(gv, dd_load(gam, N, j), aG);
     }
