@@ -464,8 +464,9 @@ def main():
                  "dd_fma_per_s_in_dd_gemm": ddfma / t_ddg if t_ddg > 0 else None,
                  "kernels_ms": {k: v[0] for k, v in tmd.items() if v[1]}}
         if t_ddg > 0 and probe["dfma_tflops"]:
-            # one dd multiply-add (dd_fma, dd.cuh) is 15 dependent fp64 instructions; the bound is the fp64 pipe issue rate = DFMA probe FLOP/s / 2
-            ddres["frac_of_dfma_issue_peak"] = (ddfma / t_ddg) * 15 / (probe["dfma_tflops"] * 1e12 / 2)
+            # one dd multiply-add of the dd GEMM (dd_fma_lazy, dd.cuh: renormalised once per 16 terms) is 12 fp64 instructions (+ 6 / 16 for the
+            # renormalisation); the bound is the fp64 pipe issue rate = DFMA probe FLOP/s / 2
+            ddres["frac_of_dfma_issue_peak"] = (ddfma / t_ddg) * 12.375 / (probe["dfma_tflops"] * 1e12 / 2)
 
     configs = None
     if rank == 0 and not args.no_configs:

@@ -87,6 +87,21 @@ __device__ __forceinline__ dd dd_fma(dd a, dd b, dd c) {
     s.lo = SWW_ADD(s.lo, SWW_ADD(c.lo, p.lo));
     return quick_two_sum(s.hi, s.lo);
 }
+// The same accumulation without the renormalisation: c.hi + c.lo += a * b with c.hi the running two-sum of the high products and
+// c.lo the plain fp64 sum of every error term (12 flops instead of 15).  c is NOT a normalised dd afterwards: |c.lo| grows by up to an
+// ulp of c.hi per call, so the caller renormalises with dd_renorm every few dozen calls (and before c is used as a dd number).
+__device__ __forceinline__ void dd_fma_lazy(dd a, dd b, dd& c) {
+    const double p = SWW_MUL(a.hi, b.hi);
+    double pe = SWW_FMA(a.hi, b.hi, -p);
+    pe = SWW_FMA(a.hi, b.lo, pe);
+    pe = SWW_FMA(a.lo, b.hi, pe);
+    const double t = SWW_ADD(c.hi, p);
+    const double bb = SWW_SUB(t, c.hi);
+    const double e = SWW_ADD(SWW_SUB(c.hi, SWW_SUB(t, bb)), SWW_SUB(p, bb));
+    c.lo = SWW_ADD(c.lo, SWW_ADD(e, pe));
+    c.hi = t;
+}
+__device__ __forceinline__ dd dd_renorm(dd c) { return two_sum(c.hi, c.lo); }  // no assumption on |c.lo| against |c.hi|
 // dd / dd by three quotient digits
 __device__ __forceinline__ dd dd_div(dd a, dd b) {
     double q1 = a.hi / b.hi;

@@ -266,8 +266,13 @@ __global__ void __launch_bounds__(256) k_gemm_dd(int N, int ncols, size_t L, con
 #pragma unroll
             for (int r = 0; r < 4; r++)
 #pragma unroll
-                for (int c = 0; c < CN; c++) acc[r][c] = dd_fma(a[r], x[c], acc[r][c]);
+                for (int c = 0; c < CN; c++) dd_fma_lazy(a[r], x[c], acc[r][c]);
         }
+        // the accumulators are renormalised once per k-slab (16 terms), not per term: 12 instead of 15 flops per multiply-add
+#pragma unroll
+        for (int r = 0; r < 4; r++)
+#pragma unroll
+            for (int c = 0; c < CN; c++) acc[r][c] = dd_renorm(acc[r][c]);
         __syncthreads();
     }
 #pragma unroll
