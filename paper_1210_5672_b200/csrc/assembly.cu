@@ -311,9 +311,10 @@ struct TabDD {  // functions of m = (i - j) mod N
 
 // K_ij, G_ij of (2.13) in dd (already scaled by 1/N); dist = circular distance |i-j|
 // rc: shared table of dd reciprocals 1 / (m (m + 1)) (fill_rc below) for the in-band series
-// SLOPPY (the fp64 handle's base-state pass only, which needs the entries to ~1e-20, not 1e-31): sums by the 11-flop addition (error
-// ~2^-104 relative to the LARGER operand, so a cancelling difference is less accurate than with the 20-flop dd_add -- harmless at that
-// target); the argument y = eta_i - eta_j and the in-band series keep the accurate addition.
+// SLOPPY (both callers set it): sums by the 11-flop addition (error ~2^-104 relative to the LARGER operand, so a cancelling
+// difference is less accurate than with the 20-flop dd_add: a cancellation by 1e3 leaves 5e-29 relative, against a bar of 1e-25 for the
+// dd handles and a need of ~1e-20 in the fp64 handle's base-state pass); the argument y = eta_i - eta_j and the in-band series keep
+// the accurate addition.  Entry by entry against the __float128 oracle: tests/test_gpu_parity.py, tests/test_gpu_mesh.py (1e-29 N).
 __device__ __forceinline__ dd dd_add_sloppy(dd a, dd b) {
     dd s = two_sum(a.hi, b.hi);
     s.lo = SWW_ADD(s.lo, SWW_ADD(a.lo, b.lo));
@@ -429,7 +430,7 @@ __global__ void __launch_bounds__(ASMDD_TI) k_assemble_dd(int N, const double* _
         const NodeDD nj = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
         TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
         dd kv, gv;
-        entry_dd<FINITE, MESH>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
+        entry_dd<FINITE, MESH, true>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
         size_t o = (size_t)i + (size_t)j * N;
         dd_store(K, NN, o, kv);
         dd_store(G, NN, o, gv);
