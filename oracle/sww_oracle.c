@@ -37,6 +37,10 @@
  *       the 11-stage order-8 Cooper-Verner tableau with coefficients in Q(sqrt 21) is used
  *       (SURVEY.md §8(c)-A12); pinned by the rooted-tree order conditions in tests/.
  *   R7  g eta vs g (h + eta) in (2.1b) differ by a constant that P removes; sigma = 0.
+ *   PARITY UNPINNED (conventions that no printed value or identity fixes; the CUDA path takes the same ones):
+ *       the filter being on by default and applied to every right-hand side and after every step (R5); the symbol 0 of D, H, |D| at the
+ *       Nyquist mode (R4); on a refined mesh, the filter acting on the Fourier modes in alpha of the stored samples (R16).
+ *       Everything else below is pinned in tests/test_oracle_pins.py and tests/test_oracle_mesh.py.
  *   R8  every Fourier multiplier (D, H, |D|, P, filter) is summed in __float128 in the ld and q builds
  *       (see multiplier_w below); the dense O(N^2)/O(N^3) steps run in REAL.
  */
