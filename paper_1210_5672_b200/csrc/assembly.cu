@@ -476,6 +476,158 @@ __global__ void __launch_bounds__(BP_TI) k_base_pass_dd(int N, int jchunk, const
     p[2 * N + i] = aG.hi;
     p[3 * N + i] = aG.lo;
 }
+// ------------------------------------------------------------------------------------------------ the same pass, entries in pairs
+// K_ij, G_ij and K_ji, G_ji share everything that costs: sinh/cosh(eta_i - eta_j) (odd / even under the swap), the quotient
+// p = (cos x + cosh y) / (sin^2 x + sinh^2 y) (even), the image term's denominator and its two quotients c_r (odd), c_i (even).
+// entry_pair_dd evaluates both entries of an off-diagonal pair for ~0.7 of the work of two entry_dd calls (11-flop additions as in
+// the SLOPPY instances above).  t0: the tables of m = (i - j) mod N; dist >= 1.
+template <bool FINITE, bool MESH>
+__device__ __forceinline__ void entry_pair_dd(const NodeDD& ni, const NodeDD& nj, const TabDD& t0, int dist, double rN, const double* rc,
+                                              dd* kij, dd* gij, dd* kji, dd* gji) {
+    auto add_ = [](dd a, dd b) { return dd_add_sloppy(a, b); };
+    auto sub_ = [](dd a, dd b) { return dd_add_sloppy(a, dd_neg(b)); };
+    TabDD t = t0;
+    if (MESH) {
+        const dd sd = sub_(dd_mul(ni.xS, nj.xC), dd_mul(ni.xC, nj.xS)), cd = add_(dd_mul(ni.xC, nj.xC), dd_mul(ni.xS, nj.xS));
+        t.sn = add_(dd_mul(t0.sn, cd), dd_mul(t0.cs, sd));
+        t.cs = sub_(dd_mul(t0.cs, cd), dd_mul(t0.sn, sd));
+        t.s2 = t.cs.hi >= 0.0 ? dd_div(dd_sqr(t.sn), dd_mul_d(dd_add_d(t.cs, 1.0), 2.0)) : dd_half(sub_(dd{1.0, 0.0}, t.cs));
+    }
+    dd sh, ch;
+    const dd y = dd_sub(ni.eta, nj.eta);
+    if (dist <= DD_BAND && fabs(y.hi) < 0.5) {
+        dd_sinhcosh_tab(y, rc, &sh, &ch);
+    } else if (dist <= DD_BAND) {
+        dd_sinhcosh(y, &sh, &ch);
+    } else {
+        sh = sub_(dd_mul(ni.Sh, nj.Ch), dd_mul(ni.Ch, nj.Sh));
+        ch = sub_(dd_mul(ni.Ch, nj.Ch), dd_mul(ni.Sh, nj.Sh));
+    }
+    dd p;
+    if (t.cs.hi >= 0.0)
+        p = dd_div_fast(add_(t.cs, ch), add_(dd_sqr(t.sn), dd_sqr(sh)));
+    else
+        p = dd_div_fast(dd{1.0, 0.0}, sub_(ch, t.cs));
+    const dd hp = dd_half(p);
+    // (i, j): k1 = hp (d1_j sn - xE_j sh), g1 = hp (d1_i sh + xE_i sn) - c0 ;  (j, i): sn, sh, c0 change sign, i and j change roles
+    dd k1, g1, k1t, g1t;
+    if (MESH) {
+        k1 = dd_mul(hp, sub_(dd_mul(nj.d1, t.sn), dd_mul(nj.xE, sh)));
+        g1 = sub_(dd_mul(hp, add_(dd_mul(ni.d1, sh), dd_mul(ni.xE, t.sn))), t.c0);
+        k1t = dd_mul(hp, sub_(dd_mul(ni.xE, sh), dd_mul(ni.d1, t.sn)));
+        g1t = sub_(t.c0, dd_mul(hp, add_(dd_mul(nj.d1, sh), dd_mul(nj.xE, t.sn))));
+    } else {
+        k1 = dd_mul(hp, sub_(dd_mul(nj.d1, t.sn), sh));
+        g1 = sub_(dd_mul(hp, add_(dd_mul(ni.d1, sh), t.sn)), t.c0);
+        k1t = dd_mul(hp, sub_(sh, dd_mul(ni.d1, t.sn)));
+        g1t = sub_(t.c0, dd_mul(hp, add_(dd_mul(nj.d1, sh), t.sn)));
+    }
+    dd k2{0, 0}, g2{0, 0}, k2t{0, 0}, g2t{0, 0};
+    if (FINITE) {
+        const dd Eij = dd_mul(ni.E, nj.E);
+        const dd omE = add_(dd_mul(ni.E, nj.Dm), ni.Dm);
+        const dd den = add_(dd_sqr(omE), dd_mul_d(dd_mul(Eij, t.s2), 4.0));
+        const double rb = rcp_normal(den.hi);
+        const dd cr = dd_div_rb(dd_mul(Eij, t.sn), den, rb);
+        const dd ci = dd_neg(dd_half(dd_div_rb(dd_mul(omE, dd_add_d(Eij, 1.0)), den, rb)));
+        // (i, j): k2 = xE_j ci - d1_j cr, g2 = xE_i cr - d1_i ci ;  (j, i): cr changes sign
+        k2 = sub_(MESH ? dd_mul(nj.xE, ci) : ci, dd_mul(nj.d1, cr));
+        g2 = sub_(MESH ? dd_mul(ni.xE, cr) : cr, dd_mul(ni.d1, ci));
+        k2t = add_(MESH ? dd_mul(ni.xE, ci) : ci, dd_mul(ni.d1, cr));
+        g2t = dd_neg(add_(MESH ? dd_mul(nj.xE, cr) : cr, dd_mul(nj.d1, ci)));
+    }
+    *kij = dd_mul_d(sub_(k1, k2), rN);
+    *gij = dd_mul_d(sub_(g1, g2), rN);
+    *kji = dd_mul_d(sub_(k1t, k2t), rN);
+    *gji = dd_mul_d(sub_(g1t, g2t), rN);
+}
+
+// One warp per pair of 32 x 32 tiles (Ib <= Jb) of the matrix: lane l owns row i = 32 Ib + l and meets the columns j = 32 Jb + ((l + s)
+// mod 32), s = 0..31 (each step the 32 lanes hold 32 different columns).  The row sums stay with the lane; the sums for the rows j (from
+// the transposed entries K_ji, G_ji) travel with their column from lane to lane by shuffles and end where they started.  Output in the
+// layout of k_base_pass_dd with column chunks of 32: part[Jb][.][rows of Ib] and part[Ib][.][rows of Jb], every slot written once.
+// Diagonal tiles (Ib == Jb) take the plain entries (they hold i == j).  N a multiple of 32; nT = N / 32.
+constexpr int BPS_WARPS = 4;
+template <bool FINITE, bool MESH>
+__global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT, const double* __restrict__ eta, const double* __restrict__ d1,
+                                                                  const double* __restrict__ d2, const double* __restrict__ E,
+                                                                  const double* __restrict__ Dm, const double* __restrict__ Sh,
+                                                                  const double* __restrict__ Ch, const double* __restrict__ cs,
+                                                                  const double* __restrict__ sn, const double* __restrict__ c0,
+                                                                  const double* __restrict__ s2, MeshDev ms, const double* __restrict__ mu,
+                                                                  const double* __restrict__ gam, double* __restrict__ part) {
+    constexpr int NF = MESH ? 26 : 18;  // doubles per staged node: 7 dd fields, mu, gam (+ 4 dd mesh fields)
+    __shared__ double rc[64];
+    __shared__ double sJ[BPS_WARPS][NF][32];
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, mask = N - 1;
+    fill_rc(rc, tid);
+    int u = blockIdx.x * BPS_WARPS + warp, Ib = 0;
+    const int nunits = nT * (nT + 1) / 2;
+    if (u >= nunits) return;
+    while (u >= nT - Ib) {
+        u -= nT - Ib;
+        Ib++;
+    }
+    const int Jb = Ib + u, i = 32 * Ib + lane;
+    const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
+    const dd mu_i = dd_load(mu, N, i), gam_i = dd_load(gam, N, i);
+    {   // stage the nodes of the column tile
+        const int j = 32 * Jb + lane;
+        const NodeDD n = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
+        double(*f)[32] = sJ[warp];
+        f[0][lane] = n.eta.hi; f[1][lane] = n.eta.lo; f[2][lane] = n.d1.hi; f[3][lane] = n.d1.lo; f[4][lane] = n.d2.hi; f[5][lane] = n.d2.lo;
+        f[6][lane] = n.E.hi; f[7][lane] = n.E.lo; f[8][lane] = n.Dm.hi; f[9][lane] = n.Dm.lo; f[10][lane] = n.Sh.hi; f[11][lane] = n.Sh.lo;
+        f[12][lane] = n.Ch.hi; f[13][lane] = n.Ch.lo;
+        const dd m_ = dd_load(mu, N, j), g_ = dd_load(gam, N, j);
+        f[14][lane] = m_.hi; f[15][lane] = m_.lo; f[16][lane] = g_.hi; f[17][lane] = g_.lo;
+        if (MESH) {
+            f[18][lane] = n.xE.hi; f[19][lane] = n.xE.lo; f[20][lane] = n.xE1.hi; f[21][lane] = n.xE1.lo;
+            f[22][lane] = n.xS.hi; f[23][lane] = n.xS.lo; f[24][lane] = n.xC.hi; f[25][lane] = n.xC.lo;
+        }
+    }
+    __syncwarp();
+    const double rN = 1.0 / (double)N;
+    const bool diag = Ib == Jb;
+    dd aK{0, 0}, aG{0, 0}, tK{0, 0}, tG{0, 0};
+    for (int s = 0; s < 32; s++) {
+        const int jl = (lane + s) & 31, j = 32 * Jb + jl, m = (i - j) & mask;
+        const double(*f)[32] = sJ[warp];
+        NodeDD nj;
+        nj.eta = dd{f[0][jl], f[1][jl]}; nj.d1 = dd{f[2][jl], f[3][jl]}; nj.d2 = dd{f[4][jl], f[5][jl]};
+        nj.E = dd{f[6][jl], f[7][jl]}; nj.Dm = dd{f[8][jl], f[9][jl]}; nj.Sh = dd{f[10][jl], f[11][jl]}; nj.Ch = dd{f[12][jl], f[13][jl]};
+        if (MESH) {
+            nj.xE = dd{f[18][jl], f[19][jl]}; nj.xE1 = dd{f[20][jl], f[21][jl]};
+            nj.xS = dd{f[22][jl], f[23][jl]}; nj.xC = dd{f[24][jl], f[25][jl]};
+        }
+        const dd mu_j{f[14][jl], f[15][jl]}, gam_j{f[16][jl], f[17][jl]};
+        const TabDD t{dd_load(sn, N, m), dd_load(cs, N, m), dd_load(c0, N, m), dd_load(s2, N, m)};
+        if (diag) {
+            dd kv, gv;
+            entry_dd<FINITE, MESH, true>(ni, nj, t, min(m, N - m), rN, rc, &kv, &gv);
+            aK = dd_fma(kv, mu_j, aK);
+            aG = dd_fma(gv, gam_j, aG);
+        } else {
+            dd kij, gij, kji, gji;
+            entry_pair_dd<FINITE, MESH>(ni, nj, t, min(m, N - m), rN, rc, &kij, &gij, &kji, &gji);
+            aK = dd_fma(kij, mu_j, aK);
+            aG = dd_fma(gij, gam_j, aG);
+            tK = dd_fma(kji, mu_i, tK);
+            tG = dd_fma(gji, gam_i, tG);
+            // the sums of column j move on with it: the lane below meets this column next
+            const int src = (lane + 1) & 31;
+            tK = dd{__shfl_sync(0xffffffffu, tK.hi, src), __shfl_sync(0xffffffffu, tK.lo, src)};
+            tG = dd{__shfl_sync(0xffffffffu, tG.hi, src), __shfl_sync(0xffffffffu, tG.lo, src)};
+        }
+    }
+    double* pr = part + (size_t)Jb * 4 * N;   // rows of Ib, columns of chunk Jb
+    pr[i] = aK.hi; pr[N + i] = aK.lo; pr[2 * N + i] = aG.hi; pr[3 * N + i] = aG.lo;
+    if (!diag) {                              // rows of Jb, columns of chunk Ib: after 32 moves the sums of column 32 Jb + lane are here
+        double* pc = part + (size_t)Ib * 4 * N;
+        const int j = 32 * Jb + lane;
+        pc[j] = tK.hi; pc[N + j] = tK.lo; pc[2 * N + j] = tG.hi; pc[3 * N + j] = tG.lo;
+    }
+}
+
 // res = b - mu/2 - sum pK  (2.7) ;  w = sum pG ;  res_f64 = RN(res).  512 threads = 32 nodes x 16 groups of chunks (the loads of a
 // node's partial sums are the whole cost: sixteen groups keep sixteen of them in flight and shorten the dd chains).
 constexpr int BR_G = 16;
@@ -509,10 +661,30 @@ __global__ void __launch_bounds__(32 * BR_G) k_base_reduce(int N, int nchunk, co
 int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* gam, double* res, double* res_f64, double* w) {
     const int N = d->N;
     const Tables* t = d->tab;
-    const int nchunk = d->bp_chunks, jchunk = N / nchunk;
+    int nchunk = d->bp_chunks;
+    const int jchunk = N / nchunk;
     dim3 grid((N + BP_TI - 1) / BP_TI, nchunk);
     SWW_BEGIN(KC_DDGEMM, d->stream);
     const MeshDev ms = d->mesh;
+    if (N >= 2048 && N / 32 <= d->bp_chunks) {  // enough tile pairs to fill the chip: the entries in pairs (k_base_pass_sym)
+        const int nT = N / 32, nunits = nT * (nT + 1) / 2;
+        const dim3 gs((nunits + BPS_WARPS - 1) / BPS_WARPS);
+#define SWW_BPS_LAUNCH(FIN, MSH) \
+    k_base_pass_sym<FIN, MSH><<<gs, 32 * BPS_WARPS, 0, d->stream>>>(N, nT, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, ms, mu, gam, d->bp_part)
+        if (d->mesh_on) {
+            if (d->finite) SWW_BPS_LAUNCH(true, true); else SWW_BPS_LAUNCH(false, true);
+        } else {
+            if (d->finite) SWW_BPS_LAUNCH(true, false); else SWW_BPS_LAUNCH(false, false);
+        }
+#undef SWW_BPS_LAUNCH
+        nchunk = nT;
+        SWW_LAUNCHED();
+        SWW_BEGIN(KC_OTHER, d->stream);
+        k_base_reduce<<<(N + 31) / 32, 32 * BR_G, 0, d->stream>>>(N, nchunk, d->bp_part, b, mu, res, res_f64, w);
+        SWW_LAUNCHED();
+        SWW_CUDA(cudaGetLastError());
+        return SWW_OK;
+    }
 #define SWW_BP_LAUNCH(FIN, MSH) \
     k_base_pass_dd<FIN, MSH><<<grid, BP_TI, 0, d->stream>>>(N, jchunk, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, ms, mu, gam, d->bp_part)
     if (d->mesh_on) {
