@@ -542,8 +542,10 @@ __device__ __forceinline__ void entry_pair_dd(const NodeDD& ni, const NodeDD& nj
     *gji = dd_mul_d(sub_(g1t, g2t), rN);
 }
 
-// One warp per pair of 32 x 32 tiles (Ib <= Jb) of the matrix: lane l owns row i = 32 Ib + l and meets the columns j = 32 Jb + ((l + s)
-// mod 32), s = 0..31 (each step the 32 lanes hold 32 different columns).  The row sums stay with the lane; the sums for the rows j (from
+// Two warps per pair of 32 x 32 tiles (Ib <= Jb) of the matrix (one takes the steps s = 0..15, the other s = 16..31; their sums meet
+// in shared memory -- 4160 half-size units at N = 2048 fill the 1776 resident warps of the chip more evenly than 2080 full ones:
+// 0.131 -> see DESIGN.md): lane l owns row i = 32 Ib + l and meets the columns j = 32 Jb + ((l + s) mod 32) (each step the 32 lanes hold
+// 32 different columns).  The row sums stay with the lane; the sums for the rows j (from
 // the transposed entries K_ji, G_ji) travel with their column from lane to lane by shuffles and end where they started.  Output in the
 // layout of k_base_pass_dd with column chunks of 32: part[Jb][.][rows of Ib] and part[Ib][.][rows of Jb], every slot written once.
 // Diagonal tiles (Ib == Jb) take the plain entries (they hold i == j).  N a multiple of 32; nT = N / 32.
@@ -557,13 +559,16 @@ __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT,
                                                                   const double* __restrict__ s2, MeshDev ms, const double* __restrict__ mu,
                                                                   const double* __restrict__ gam, double* __restrict__ part) {
     constexpr int NF = MESH ? 26 : 18;  // doubles per staged node: 7 dd fields, mu, gam (+ 4 dd mesh fields)
+    constexpr int NP = BPS_WARPS / 2;   // tile pairs per CTA
     __shared__ double rc[64];
-    __shared__ double sJ[BPS_WARPS][NF][32];
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, mask = N - 1;
+    __shared__ double sJ[NP][NF][32];
+    __shared__ double sX[NP][8][32];    // the second warp's sums on their way to the first: rows (4), columns (4)
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, mask = N - 1, pr_ = warp >> 1, half = warp & 1;
     fill_rc(rc, tid);
-    int u = blockIdx.x * BPS_WARPS + warp, Ib = 0;
+    int u = blockIdx.x * NP + pr_, Ib = 0;
     const int nunits = nT * (nT + 1) / 2;
-    if (u >= nunits) return;
+    const bool live = u < nunits;       // (a CTA's warps all reach the barriers below)
+    if (!live) u = 0;
     while (u >= nT - Ib) {
         u -= nT - Ib;
         Ib++;
@@ -571,10 +576,10 @@ __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT,
     const int Jb = Ib + u, i = 32 * Ib + lane;
     const NodeDD ni = load_node(N, i, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
     const dd mu_i = dd_load(mu, N, i), gam_i = dd_load(gam, N, i);
-    {   // stage the nodes of the column tile
+    if (half == 0) {   // stage the nodes of the column tile
         const int j = 32 * Jb + lane;
         const NodeDD n = load_node(N, j, eta, d1, d2, E, Dm, Sh, Ch, FINITE, ms, MESH);
-        double(*f)[32] = sJ[warp];
+        double(*f)[32] = sJ[pr_];
         f[0][lane] = n.eta.hi; f[1][lane] = n.eta.lo; f[2][lane] = n.d1.hi; f[3][lane] = n.d1.lo; f[4][lane] = n.d2.hi; f[5][lane] = n.d2.lo;
         f[6][lane] = n.E.hi; f[7][lane] = n.E.lo; f[8][lane] = n.Dm.hi; f[9][lane] = n.Dm.lo; f[10][lane] = n.Sh.hi; f[11][lane] = n.Sh.lo;
         f[12][lane] = n.Ch.hi; f[13][lane] = n.Ch.lo;
@@ -585,13 +590,13 @@ __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT,
             f[22][lane] = n.xS.hi; f[23][lane] = n.xS.lo; f[24][lane] = n.xC.hi; f[25][lane] = n.xC.lo;
         }
     }
-    __syncwarp();
+    __syncthreads();
     const double rN = 1.0 / (double)N;
     const bool diag = Ib == Jb;
     dd aK{0, 0}, aG{0, 0}, tK{0, 0}, tG{0, 0};
-    for (int s = 0; s < 32; s++) {
+    for (int s = 16 * half; s < 16 * half + 16; s++) {
         const int jl = (lane + s) & 31, j = 32 * Jb + jl, m = (i - j) & mask;
-        const double(*f)[32] = sJ[warp];
+        const double(*f)[32] = sJ[pr_];
         NodeDD nj;
         nj.eta = dd{f[0][jl], f[1][jl]}; nj.d1 = dd{f[2][jl], f[3][jl]}; nj.d2 = dd{f[4][jl], f[5][jl]};
         nj.E = dd{f[6][jl], f[7][jl]}; nj.Dm = dd{f[8][jl], f[9][jl]}; nj.Sh = dd{f[10][jl], f[11][jl]}; nj.Ch = dd{f[12][jl], f[13][jl]};
@@ -619,11 +624,24 @@ __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT,
             tG = dd{__shfl_sync(0xffffffffu, tG.hi, src), __shfl_sync(0xffffffffu, tG.lo, src)};
         }
     }
+    // after its 16 moves a lane holds the sums of column (lane + 16 (half + 1)) mod 32: the second warp's are those of column `lane`
+    if (half == 1) {
+        double(*x)[32] = sX[pr_];
+        x[0][lane] = aK.hi; x[1][lane] = aK.lo; x[2][lane] = aG.hi; x[3][lane] = aG.lo;
+        x[4][lane] = tK.hi; x[5][lane] = tK.lo; x[6][lane] = tG.hi; x[7][lane] = tG.lo;
+    }
+    __syncthreads();
+    if (half == 1 || !live) return;
+    const double(*x)[32] = sX[pr_];
+    aK = dd_add(aK, dd{x[0][lane], x[1][lane]});
+    aG = dd_add(aG, dd{x[2][lane], x[3][lane]});
     double* pr = part + (size_t)Jb * 4 * N;   // rows of Ib, columns of chunk Jb
     pr[i] = aK.hi; pr[N + i] = aK.lo; pr[2 * N + i] = aG.hi; pr[3 * N + i] = aG.lo;
-    if (!diag) {                              // rows of Jb, columns of chunk Ib: after 32 moves the sums of column 32 Jb + lane are here
+    if (!diag) {                              // rows of Jb, columns of chunk Ib
+        const int c = (lane + 16) & 31, j = 32 * Jb + c;
+        tK = dd_add(tK, dd{x[4][c], x[5][c]});
+        tG = dd_add(tG, dd{x[6][c], x[7][c]});
         double* pc = part + (size_t)Ib * 4 * N;
-        const int j = 32 * Jb + lane;
         pc[j] = tK.hi; pc[N + j] = tK.lo; pc[2 * N + j] = tG.hi; pc[3 * N + j] = tG.lo;
     }
 }
@@ -668,7 +686,7 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
     const MeshDev ms = d->mesh;
     if (N >= 2048 && N / 32 <= d->bp_chunks) {  // enough tile pairs to fill the chip: the entries in pairs (k_base_pass_sym)
         const int nT = N / 32, nunits = nT * (nT + 1) / 2;
-        const dim3 gs((nunits + BPS_WARPS - 1) / BPS_WARPS);
+        const dim3 gs((nunits + BPS_WARPS / 2 - 1) / (BPS_WARPS / 2));
 #define SWW_BPS_LAUNCH(FIN, MSH) \
     k_base_pass_sym<FIN, MSH><<<gs, 32 * BPS_WARPS, 0, d->stream>>>(N, nT, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, ms, mu, gam, d->bp_part)
         if (d->mesh_on) {
