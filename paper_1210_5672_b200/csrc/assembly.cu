@@ -542,14 +542,14 @@ __device__ __forceinline__ void entry_pair_dd(const NodeDD& ni, const NodeDD& nj
     *gji = dd_mul_d(sub_(g1t, g2t), rN);
 }
 
-// Two warps per pair of 32 x 32 tiles (Ib <= Jb) of the matrix (one takes the steps s = 0..15, the other s = 16..31; their sums meet
-// in shared memory -- 4160 half-size units at N = 2048 fill the 1776 resident warps of the chip more evenly than 2080 full ones:
-// 0.131 -> see DESIGN.md): lane l owns row i = 32 Ib + l and meets the columns j = 32 Jb + ((l + s) mod 32) (each step the 32 lanes hold
+// BPS_NWP warps per pair of 32 x 32 tiles (Ib <= Jb) of the matrix (warp q takes the steps s = 8 q .. 8 q + 7; their sums meet in shared
+// memory -- the 8320 quarter-size units at N = 2048 fill the resident warps of the chip more evenly than 2080 full ones): lane l owns row i = 32 Ib + l and meets the columns j = 32 Jb + ((l + s) mod 32) (each step the 32 lanes hold
 // 32 different columns).  The row sums stay with the lane; the sums for the rows j (from
 // the transposed entries K_ji, G_ji) travel with their column from lane to lane by shuffles and end where they started.  Output in the
 // layout of k_base_pass_dd with column chunks of 32: part[Jb][.][rows of Ib] and part[Ib][.][rows of Jb], every slot written once.
 // Diagonal tiles (Ib == Jb) take the plain entries (they hold i == j).  N a multiple of 32; nT = N / 32.
-constexpr int BPS_WARPS = 4;
+constexpr int BPS_WARPS = 4;   // warps per CTA
+constexpr int BPS_NWP = 4;     // warps per tile pair: each takes 32 / BPS_NWP of the 32 steps
 template <bool FINITE, bool MESH>
 __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT, const double* __restrict__ eta, const double* __restrict__ d1,
                                                                   const double* __restrict__ d2, const double* __restrict__ E,
@@ -559,11 +559,11 @@ __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT,
                                                                   const double* __restrict__ s2, MeshDev ms, const double* __restrict__ mu,
                                                                   const double* __restrict__ gam, double* __restrict__ part) {
     constexpr int NF = MESH ? 26 : 18;  // doubles per staged node: 7 dd fields, mu, gam (+ 4 dd mesh fields)
-    constexpr int NP = BPS_WARPS / 2;   // tile pairs per CTA
+    constexpr int NP = BPS_WARPS / BPS_NWP, NS = 32 / BPS_NWP;  // tile pairs per CTA, steps per warp
     __shared__ double rc[64];
     __shared__ double sJ[NP][NF][32];
-    __shared__ double sX[NP][8][32];    // the second warp's sums on their way to the first: rows (4), columns (4)
-    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, mask = N - 1, pr_ = warp >> 1, half = warp & 1;
+    __shared__ double sX[NP][BPS_NWP][8][32];  // the other warps' sums on their way to the first: rows (4), columns (4, by column)
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, mask = N - 1, pr_ = warp / BPS_NWP, half = warp % BPS_NWP;
     fill_rc(rc, tid);
     int u = blockIdx.x * NP + pr_, Ib = 0;
     const int nunits = nT * (nT + 1) / 2;
@@ -594,7 +594,7 @@ __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT,
     const double rN = 1.0 / (double)N;
     const bool diag = Ib == Jb;
     dd aK{0, 0}, aG{0, 0}, tK{0, 0}, tG{0, 0};
-    for (int s = 16 * half; s < 16 * half + 16; s++) {
+    for (int s = NS * half; s < NS * half + NS; s++) {
         const int jl = (lane + s) & 31, j = 32 * Jb + jl, m = (i - j) & mask;
         const double(*f)[32] = sJ[pr_];
         NodeDD nj;
@@ -624,23 +624,28 @@ __global__ void __launch_bounds__(32 * BPS_WARPS) k_base_pass_sym(int N, int nT,
             tG = dd{__shfl_sync(0xffffffffu, tG.hi, src), __shfl_sync(0xffffffffu, tG.lo, src)};
         }
     }
-    // after its 16 moves a lane holds the sums of column (lane + 16 (half + 1)) mod 32: the second warp's are those of column `lane`
-    if (half == 1) {
-        double(*x)[32] = sX[pr_];
+    // after its NS moves a lane holds the sums of column (lane + NS (half + 1)) mod 32
+    const int c = (lane + NS * (half + 1)) & 31;
+    if (half != 0) {
+        double(*x)[32] = sX[pr_][half];
         x[0][lane] = aK.hi; x[1][lane] = aK.lo; x[2][lane] = aG.hi; x[3][lane] = aG.lo;
-        x[4][lane] = tK.hi; x[5][lane] = tK.lo; x[6][lane] = tG.hi; x[7][lane] = tG.lo;
+        x[4][c] = tK.hi; x[5][c] = tK.lo; x[6][c] = tG.hi; x[7][c] = tG.lo;
     }
     __syncthreads();
-    if (half == 1 || !live) return;
-    const double(*x)[32] = sX[pr_];
-    aK = dd_add(aK, dd{x[0][lane], x[1][lane]});
-    aG = dd_add(aG, dd{x[2][lane], x[3][lane]});
+    if (half != 0 || !live) return;
+    for (int q = 1; q < BPS_NWP; q++) {
+        const double(*x)[32] = sX[pr_][q];
+        aK = dd_add(aK, dd{x[0][lane], x[1][lane]});
+        aG = dd_add(aG, dd{x[2][lane], x[3][lane]});
+        if (!diag) {
+            tK = dd_add(tK, dd{x[4][c], x[5][c]});
+            tG = dd_add(tG, dd{x[6][c], x[7][c]});
+        }
+    }
     double* pr = part + (size_t)Jb * 4 * N;   // rows of Ib, columns of chunk Jb
     pr[i] = aK.hi; pr[N + i] = aK.lo; pr[2 * N + i] = aG.hi; pr[3 * N + i] = aG.lo;
     if (!diag) {                              // rows of Jb, columns of chunk Ib
-        const int c = (lane + 16) & 31, j = 32 * Jb + c;
-        tK = dd_add(tK, dd{x[4][c], x[5][c]});
-        tG = dd_add(tG, dd{x[6][c], x[7][c]});
+        const int j = 32 * Jb + c;
         double* pc = part + (size_t)Ib * 4 * N;
         pc[j] = tK.hi; pc[N + j] = tK.lo; pc[2 * N + j] = tG.hi; pc[3 * N + j] = tG.lo;
     }
@@ -686,7 +691,7 @@ int base_pass_dd(sww_dtn_s* d, const double* b, const double* mu, const double* 
     const MeshDev ms = d->mesh;
     if (N >= 2048 && N / 32 <= d->bp_chunks) {  // enough tile pairs to fill the chip: the entries in pairs (k_base_pass_sym)
         const int nT = N / 32, nunits = nT * (nT + 1) / 2;
-        const dim3 gs((nunits + BPS_WARPS / 2 - 1) / (BPS_WARPS / 2));
+        const dim3 gs((nunits + BPS_WARPS / BPS_NWP - 1) / (BPS_WARPS / BPS_NWP));
 #define SWW_BPS_LAUNCH(FIN, MSH) \
     k_base_pass_sym<FIN, MSH><<<gs, 32 * BPS_WARPS, 0, d->stream>>>(N, nT, d->eta, d->d1, d->d2, d->E, d->Dm, d->Sh, d->Ch, t->cs, t->sn, t->c0, t->s2, ms, mu, gam, d->bp_part)
         if (d->mesh_on) {
